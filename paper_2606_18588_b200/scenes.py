@@ -1,0 +1,244 @@
+"""Seeded synthetic scenes, cameras, targets and partitions.
+
+This module holds none of the method's arithmetic (no projection, sorting,
+blending, composition, gradients or optimiser): it only draws inputs with the
+shapes, sizes and value distributions of BASELINE.json's configs (recipe in
+DESIGN.md "Input recipe", after SURVEY.md s8(d)) and orders the Gaussians so
+that each partition (one "simulated rank") is a contiguous
+slice.  It serves both the CUDA path and the oracle; it imports neither.
+
+MatrixCity and trained Gaussians are not available here; these
+scenes stand in for them.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SH0 = 0.28209479177387814  # value of the constant basis function; used only to
+                           # turn a target colour into a degree-0 coefficient
+PARAM_KEYS = ("mean", "log_scale", "quat", "opacity_logit", "sh")
+PARAM_WIDTH = {"mean": 3, "log_scale": 3, "quat": 4, "opacity_logit": 1, "sh": 48}
+
+
+@dataclass
+class Camera:
+    R: np.ndarray          # [3,3] row-major, p_cam = R @ mean + t
+    t: np.ndarray          # [3]
+    fx: float
+    fy: float
+    cx: float
+    cy: float
+    width: int
+    height: int
+    near_z: float = 0.2
+
+    def as_array(self) -> np.ndarray:
+        """The 19-double packing both sides unpack: R, t, fx, fy, cx, cy, W, H, near."""
+        a = np.zeros(19, dtype=np.float64)
+        a[0:9] = np.asarray(self.R, np.float32).astype(np.float64).reshape(9)
+        a[9:12] = np.asarray(self.t, np.float32).astype(np.float64).reshape(3)
+        a[12:16] = np.asarray([self.fx, self.fy, self.cx, self.cy], np.float32).astype(np.float64)
+        a[16:19] = (self.width, self.height, np.float64(np.float32(self.near_z)))
+        return a
+
+
+@dataclass
+class Scene:
+    name: str
+    params: dict            # PARAM_KEYS -> float32 arrays, ordered by partition
+    part_offsets: np.ndarray  # int64 [K+1]
+    cameras: list           # B cameras
+    targets: list           # B float32 [H,W,3]
+    sh_degree: int
+    bg: tuple = (0.0, 0.0, 0.0)
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def K(self) -> int:
+        return len(self.part_offsets) - 1
+
+    @property
+    def N(self) -> int:
+        return int(self.part_offsets[-1])
+
+    def partition(self, k: int) -> dict:
+        a, b = int(self.part_offsets[k]), int(self.part_offsets[k + 1])
+        return {key: self.params[key][a:b] for key in PARAM_KEYS}
+
+    def partitions(self) -> list:
+        return [self.partition(k) for k in range(self.K)]
+
+
+def look_at(position, target, up=(0.0, 0.0, 1.0)):
+    """World->camera rotation (rows right, down, forward) and translation."""
+    position = np.asarray(position, np.float64)
+    fwd = np.asarray(target, np.float64) - position
+    fwd /= np.linalg.norm(fwd)
+    right = np.cross(fwd, np.asarray(up, np.float64))
+    if np.linalg.norm(right) < 1e-9:
+        right = np.array([1.0, 0.0, 0.0])
+    right /= np.linalg.norm(right)
+    down = np.cross(fwd, right)
+    R = np.stack([right, down, fwd])
+    t = -R @ position
+    return R.astype(np.float32), t.astype(np.float32)
+
+
+def aerial_camera(width, height, fov_deg, altitude, pitch_deg, yaw_deg, target=(0.0, 0.0, 0.0)):
+    """Camera at `altitude` above `target`, looking down at `pitch` below horizontal."""
+    th, ps = np.deg2rad(pitch_deg), np.deg2rad(yaw_deg)
+    dist = altitude / np.sin(th)
+    pos = np.asarray(target, np.float64) + dist * np.array(
+        [-np.cos(th) * np.cos(ps), -np.cos(th) * np.sin(ps), np.sin(th)])
+    R, t = look_at(pos, target)
+    f = 0.5 * width / np.tan(0.5 * np.deg2rad(fov_deg))
+    return Camera(R, t, f, f, width / 2.0, height / 2.0, width, height)
+
+
+def _rand_quat(rng, n):
+    q = rng.standard_normal((n, 4)).astype(np.float32)
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    return q
+
+
+def _order_by_partition(params, part_id, K):
+    order = np.argsort(part_id, kind="stable")
+    counts = np.bincount(part_id, minlength=K)
+    offs = np.zeros(K + 1, np.int64)
+    offs[1:] = np.cumsum(counts)
+    return {k: np.ascontiguousarray(v[order]) for k, v in params.items()}, offs
+
+
+def grid_partition(mean, lo, hi, gx, gy):
+    """Half-open xy grid cells; outermost cells extend to +-inf (reading s22)."""
+    ix = np.clip(np.floor((mean[:, 0] - lo[0]) / (hi[0] - lo[0]) * gx).astype(np.int64), 0, gx - 1)
+    iy = np.clip(np.floor((mean[:, 1] - lo[1]) / (hi[1] - lo[1]) * gy).astype(np.int64), 0, gy - 1)
+    return iy * gx + ix
+
+
+def tiny(seed=0, n=4096, size=128, f=150.0, K=2, sh_degree=0):
+    """BASELINE.json configs[0]: world frame = camera frame, K contiguous depth chunks."""
+    rng = np.random.default_rng(seed)
+    mean = np.empty((n, 3), np.float32)
+    mean[:, 0:2] = rng.uniform(-1, 1, (n, 2))
+    mean[:, 2] = rng.uniform(2, 6, n)
+    params = dict(
+        mean=mean,
+        log_scale=rng.normal(-3.0, 0.3, (n, 3)).astype(np.float32),
+        quat=_rand_quat(rng, n),
+        opacity_logit=rng.normal(0.0, 1.0, n).astype(np.float32),
+        sh=np.zeros((n, 16, 3), np.float32),
+    )
+    colour = rng.uniform(0, 1, (n, 3))
+    params["sh"][:, 0, :] = ((colour - 0.5) / SH0).astype(np.float32)
+    if sh_degree > 0:
+        nsh = (sh_degree + 1) ** 2
+        params["sh"][:, 1:nsh, :] = rng.normal(0, 0.2, (n, nsh - 1, 3)).astype(np.float32)
+    # K contiguous chunks of the depth-sorted list (depth = camera z = mean z here)
+    rank = np.argsort(np.argsort(mean[:, 2], kind="stable"), kind="stable")
+    part_id = np.minimum(rank * K // n, K - 1)
+    order = np.argsort(mean[:, 2], kind="stable")
+    params = {k: np.ascontiguousarray(v[order]) for k, v in params.items()}
+    part_id = part_id[order]
+    offs = np.zeros(K + 1, np.int64)
+    offs[1:] = np.cumsum(np.bincount(part_id, minlength=K))
+    cam = Camera(np.eye(3, dtype=np.float32), np.zeros(3, np.float32), f, f, size / 2.0, size / 2.0,
+                 size, size)
+    target = np.random.default_rng(seed + 1).uniform(0, 1, (size, size, 3)).astype(np.float32)
+    return Scene("tiny", params, offs, [cam], [target], sh_degree,
+                 meta=dict(seed=seed, config="configs[0]"))
+
+
+def aerial(seed=0, n=1_000_000, width=1920, height=1080, extent=(100.0, 100.0, 20.0), grid=(2, 2),
+           altitude=80.0, pitch_deg=45.0, fov_deg=60.0, log_scale_mu=-2.5, log_scale_sigma=0.5,
+           sh_degree=3, n_views=1, name="aerial_1M"):
+    """BASELINE.json configs[1]: uniform box, K = grid xy partitions, aerial camera."""
+    rng = np.random.default_rng(seed)
+    ex, ey, ez = extent
+    mean = np.empty((n, 3), np.float32)
+    mean[:, 0] = rng.uniform(-ex / 2, ex / 2, n)
+    mean[:, 1] = rng.uniform(-ey / 2, ey / 2, n)
+    mean[:, 2] = rng.uniform(0, ez, n)
+    params = dict(
+        mean=mean,
+        log_scale=rng.normal(log_scale_mu, log_scale_sigma, (n, 3)).astype(np.float32),
+        quat=_rand_quat(rng, n),
+        opacity_logit=rng.normal(0.0, 1.0, n).astype(np.float32),
+        sh=rng.normal(0.0, 0.2, (n, 16, 3)).astype(np.float32),
+    )
+    K = grid[0] * grid[1]
+    part_id = grid_partition(mean, (-ex / 2, -ey / 2), (ex / 2, ey / 2), grid[0], grid[1])
+    params, offs = _order_by_partition(params, part_id, K)
+    crng = np.random.default_rng(seed + 2)
+    cams, targets = [], []
+    for b in range(n_views):
+        yaw = crng.uniform(0, 360)
+        cams.append(aerial_camera(width, height, fov_deg, altitude, pitch_deg, yaw))
+        targets.append(np.random.default_rng(seed + 1 + 1000 * b)
+                       .uniform(0, 1, (height, width, 3)).astype(np.float32))
+    return Scene(name, params, offs, cams, targets, sh_degree,
+                 meta=dict(seed=seed, config="configs[1]", grid=grid, extent=extent))
+
+
+def city(seed=0, n=10_000_000, width=1920, height=1080, extent=500.0, n_buildings=200, grid=(4, 2),
+         altitude=120.0, pitch_deg=45.0, fov_deg=60.0, height_range=(5.0, 50.0), sh_degree=3,
+         n_views=4, name="city_10M"):
+    """BASELINE.json configs[2]: 70 % of the means on building surfaces (roof + 4 walls,
+    area-weighted, N(0, 0.1 m) jitter), 30 % on the ground plane; K = grid partitions."""
+    rng = np.random.default_rng(seed)
+    half = extent / 2
+    nb = n_buildings
+    bc = rng.uniform(-half, half, (nb, 2))
+    bs = rng.uniform(10.0, 40.0, (nb, 2))
+    bh = rng.uniform(height_range[0], height_range[1], nb)
+    n_b = int(0.7 * n)
+    n_g = n - n_b
+    # faces per building: roof, +x wall, -x wall, +y wall, -y wall
+    area = np.stack([bs[:, 0] * bs[:, 1], bs[:, 1] * bh, bs[:, 1] * bh, bs[:, 0] * bh, bs[:, 0] * bh], 1)
+    prob = (area / area.sum()).reshape(-1)
+    face = rng.choice(nb * 5, size=n_b, p=prob)
+    b, f = face // 5, face % 5
+    a = rng.uniform(-0.5, 0.5, n_b)
+    c = rng.uniform(0.0, 1.0, n_b)
+    x = np.where(f == 0, a * bs[b, 0], np.where(f == 1, 0.5 * bs[b, 0], np.where(f == 2, -0.5 * bs[b, 0], a * bs[b, 0])))
+    y = np.where(f == 0, (c - 0.5) * bs[b, 1], np.where(f <= 2, a * bs[b, 1], np.where(f == 3, 0.5 * bs[b, 1], -0.5 * bs[b, 1])))
+    z = np.where(f == 0, bh[b], c * bh[b])
+    mean = np.empty((n, 3), np.float32)
+    mean[:n_b, 0] = bc[b, 0] + x
+    mean[:n_b, 1] = bc[b, 1] + y
+    mean[:n_b, 2] = z
+    mean[:n_b] += rng.normal(0, 0.1, (n_b, 3)).astype(np.float32)
+    mean[n_b:, 0:2] = rng.uniform(-half, half, (n_g, 2))
+    mean[n_b:, 2] = rng.normal(0, 0.05, n_g)
+    sp_b = 1.0 / np.sqrt(n_b / area.sum())
+    sp_g = 1.0 / np.sqrt(n_g / (extent * extent))
+    log_scale = np.empty((n, 3), np.float32)
+    log_scale[:n_b] = rng.normal(np.log(1.5 * sp_b), 0.5, (n_b, 3))
+    log_scale[n_b:] = rng.normal(np.log(1.0 * sp_g), 0.5, (n_g, 3))
+    logit = np.empty(n, np.float32)
+    logit[:n_b] = rng.normal(2.0, 1.0, n_b)
+    logit[n_b:] = rng.normal(0.0, 1.0, n_g)
+    params = dict(mean=mean, log_scale=log_scale, quat=_rand_quat(rng, n), opacity_logit=logit,
+                  sh=rng.normal(0.0, 0.2, (n, 16, 3)).astype(np.float32))
+    K = grid[0] * grid[1]
+    part_id = grid_partition(mean, (-half, -half), (half, half), grid[0], grid[1])
+    params, offs = _order_by_partition(params, part_id, K)
+    crng = np.random.default_rng(seed + 2)
+    cams, targets = [], []
+    for v in range(n_views):
+        tgt = np.append(crng.uniform(-0.4 * extent, 0.4 * extent, 2), 0.0)
+        cams.append(aerial_camera(width, height, fov_deg, altitude, pitch_deg, crng.uniform(0, 360), tgt))
+        targets.append(np.random.default_rng(seed + 1 + 1000 * v)
+                       .uniform(0, 1, (height, width, 3)).astype(np.float32))
+    return Scene(name, params, offs, cams, targets, sh_degree,
+                 meta=dict(seed=seed, config="configs[2]", grid=grid, extent=extent))
+
+
+def small_aerial(seed=0, n=20_000, width=320, height=176, K=(2, 2), sh_degree=3):
+    """configs[1] shrunk for CPU tests and element-by-element parity: same recipe,
+    fewer Gaussians, a smaller image (not a multiple of 16 high -> ragged tile row)
+    and scales enlarged so the per-pixel list lengths stay comparable."""
+    return aerial(seed=seed, n=n, width=width, height=height, grid=K, sh_degree=sh_degree,
+                  log_scale_mu=-0.9, fov_deg=60.0, name=f"aerial_{n}")
