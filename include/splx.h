@@ -1,0 +1,197 @@
+/* splx.h -- C ABI of libsplx.so: the single-GPU (B200, sm_100a) hot path of Splaxel's
+ * pixel-level scheme (arxiv/paper_2606_18588).  Citations are PAPER.md line numbers.
+ *
+ * K Gaussian partitions ("simulated ranks") live as K contiguous
+ * slices of one SoA parameter set.  Every call below processes ALL K partitions in one
+ * launch per stage: the partition index is folded into the high bits of the tile key, so
+ * one sort, one render grid (K x tiles) and one backward grid cover the K ranks.
+ *
+ * Conventions
+ *  - extern "C", plain pointers and sizes.  Structs are read on the HOST at call time;
+ *    every pointer INSIDE them that names data is a CUDA DEVICE pointer to caller-owned
+ *    memory (16-byte aligned), unless the field comment says "host".  The library never
+ *    frees, reallocates or keeps those pointers after the call returns.
+ *  - All calls are asynchronous on the CUDA stream given to splx_create and never
+ *    synchronise the device.  Scratch memory is a caller-owned workspace; the *_ws_bytes
+ *    queries give its size.
+ *  - Return value: SPLX_OK (0) or a negative error; splx_last_error gives text.  No
+ *    exceptions cross the boundary.  There is no CPU fallback: without a CUDA device
+ *    splx_create fails with SPLX_ERR_CUDA.
+ *  - Gradient outputs are ACCUMULATED (+=); the caller zeroes them (lets B views sum).
+ *  - fp32 everywhere; indices and keys are integers.  Tile = 16 x 16 pixels; pixel (i,j)
+ *    samples the point (i+0.5, j+0.5).
+ */
+#ifndef SPLX_H_
+#define SPLX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPLX_OK 0
+#define SPLX_ERR_INVALID_ARG (-1) /* null / misaligned pointer, bad size, sh_degree not in [0,3], K not in [1,64] */
+#define SPLX_ERR_WORKSPACE (-2)   /* workspace too small */
+#define SPLX_ERR_CAPACITY (-3)    /* reported by splx_check_capacity: more intersections than binning.capacity */
+#define SPLX_ERR_CUDA (-4)        /* a CUDA runtime call failed (text in splx_last_error) */
+
+#define SPLX_MAX_K 64
+#define SPLX_TILE 16
+#define SPLX_G2D_STRIDE 12 /* floats per Gaussian in the 2-D gradient buffer, see splx_raster_backward */
+
+typedef struct splx_ctx splx_ctx;
+
+/* Blending / projection constants.  The paper is silent on all of them except the
+ * saturation threshold (1e-4); defaults follow BASELINE.json north_star. */
+typedef struct {
+  float alpha_min;    /* skip a Gaussian at a pixel when alpha < alpha_min        (1/255) */
+  float alpha_max;    /* alpha = min(alpha_max, o * exp(power))                   (0.99)  */
+  float T_eps;        /* stop before a Gaussian that would take T below T_eps     (1e-4)  */
+  float dilation;     /* added to the diagonal of Sigma2D                         (0.3)   */
+  float lim_factor;   /* x/z, y/z clamped to +-lim_factor*tan(fov/2) inside J     (1.3)   */
+  float radius_floor; /* radius = ceil(3 sqrt(mid + sqrt(max(radius_floor, mid^2-det)))) (0.1) */
+} splx_config;
+
+/* Pinhole camera: p_cam = R * mean + t (R row-major), u = fx x/z + cx, v = fy y/z + cy. */
+typedef struct {
+  float R[9];
+  float t[3];
+  float fx, fy, cx, cy;
+  int32_t width, height;
+  float near_z; /* a Gaussian whose camera-space z <= near_z is culled */
+} splx_camera;
+
+/* Gaussian parameters Theta_i: SoA over all n Gaussians of all partitions.
+ * mean[n,3], log_scale[n,3] (S = exp), quat[n,4] = (w,x,y,z) un-normalised (R),
+ * opacity_logit[n] (o = sigmoid), sh[n,16,3] (colour c as SH degree <= 3). 59 floats. */
+typedef struct {
+  const float *mean, *log_scale, *quat, *opacity_logit, *sh;
+  int64_t n;
+} splx_gaussians;
+
+/* Same layout; every array is accumulated into (+=). */
+typedef struct {
+  float *mean, *log_scale, *quat, *opacity_logit, *sh;
+  int64_t n;
+} splx_gaussian_grads;
+
+/* 2-D attributes of PAPER.md L80 (depth d, 2-D mean, Sigma2D as its inverse "conic").
+ * means2d[n,2], depth[n], conic_opacity[n,4] = (A, B, C, o) with power = -0.5(A dx^2 +
+ * C dy^2) - B dx dy, rgb[n,3], radius[n] (0 = culled), tiles_touched[n], clamp[n]
+ * (bit c set: colour channel c was clamped at 0).  A culled Gaussian gets zeros. */
+typedef struct {
+  float *means2d, *depth, *conic_opacity, *rgb;
+  int32_t *radius;
+  uint32_t *tiles_touched;
+  uint8_t *clamp;
+} splx_projected;
+
+/* Tile binning of all K partitions.  slot = k * (TX*TY) + tile; key = (slot << 32) |
+ * float_bits(depth); val = Gaussian index (global, into the SoA).  keys/vals[capacity];
+ * tile_ranges[K*TX*TY][2] = [first, last+1) into keys/vals, (0,0) for an empty tile;
+ * num_intersections: one device uint64 = M, the number of valid entries (clamped to
+ * nothing: if M > capacity the overflowing entries are dropped and splx_check_capacity
+ * reports it). */
+typedef struct {
+  uint64_t *keys;
+  uint32_t *vals;
+  uint32_t *tile_ranges;
+  uint64_t capacity;
+  uint64_t *num_intersections;
+} splx_binning;
+
+/* Partial pixels of all K partitions (Eq.3-4): ct[K,H,W,4] =
+ * (premultiplied C^k rgb, T^k), d[K,H,W] = D^k = sum d_i alpha_i T_i, n_contrib[K,H,W] =
+ * 1 + list position of the pixel's last contributor (0 if none). */
+typedef struct {
+  float *ct;
+  float *d;
+  uint32_t *n_contrib;
+} splx_partial;
+
+/* ---- context -------------------------------------------------------------------- */
+/* cfg NULL = defaults.  cuda_stream is a cudaStream_t (NULL = default stream). */
+int splx_create(splx_ctx **out, int device, void *cuda_stream, const splx_config *cfg);
+int splx_destroy(splx_ctx *ctx);
+const char *splx_last_error(const splx_ctx *ctx); /* ctx may be NULL: last creation error */
+int splx_set_stream(splx_ctx *ctx, void *cuda_stream);
+/* Number of kernels this context has launched so far (host counter). */
+int64_t splx_launch_count(const splx_ctx *ctx);
+
+/* ---- a1 projection: PAPER.md L76 (Sigma = R S S^T R^T), L80 (cull by the mean,
+ * Sigma2D = J W Sigma W^T J^T, depth d, 2-D mean).  One thread per Gaussian. */
+int splx_project(splx_ctx *ctx, const splx_gaussians *g, const splx_camera *cam, int sh_degree,
+                 const splx_projected *out);
+
+/* ---- a2-a4 binning: PAPER.md L81 ("sorted based on ... depth d"), L165 ("in depth
+ * order").  part_offsets: HOST array of K+1 Gaussian offsets (partition k owns
+ * [part_offsets[k], part_offsets[k+1])).  Result: the STABLE ascending sort of all
+ * (key,val) pairs in Gaussian-index emission order, i.e. within a (partition, tile) by
+ * depth bits, ties by ascending Gaussian index. */
+size_t splx_bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, const splx_camera *cam);
+int splx_bin_sort(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
+                  const int64_t *part_offsets, const splx_camera *cam, const splx_binning *out,
+                  void *ws, size_t ws_bytes);
+/* Synchronises the stream and returns SPLX_ERR_CAPACITY if the last splx_bin_sort on
+ * `bins` dropped entries; writes M to *m_host (may be NULL).  The only blocking call. */
+int splx_check_capacity(splx_ctx *ctx, const splx_binning *bins, uint64_t *m_host);
+
+/* ---- a5 local render: PAPER.md Eq.1 (L84), Eq.3 (L167), Eq.4 (L172).  Grid = K x tiles,
+ * one thread per pixel, the tile's list staged 256 Gaussians at a time in shared memory.
+ * pairs (device uint64, may be NULL): += number of list entries walked, summed over pixels
+ * (the oracle's unit of work). */
+int splx_render_partial(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins, int K,
+                        const splx_camera *cam, const splx_partial *out, uint64_t *pairs);
+
+/* ---- a6 global composition: Eq.5.  Per pixel the K partials are
+ * ordered by D^k/(1-T^k) (an empty partial, T == 1, sorts last; ties by smaller k) and
+ * accumulated front to back; bg (HOST float[3]) is blended behind everything.
+ * image[H,W,3]; T_total[H,W] may be NULL. */
+int splx_compose(splx_ctx *ctx, int K, const splx_partial *partials, const splx_camera *cam,
+                 const float bg[3], float *image, float *T_total);
+
+/* ---- a7 loss (harness step): mean L1, PAPER.md L95 (L_RGB term).  dL_dimage[count] =
+ * sign(image-target) * scale / count; loss_sum (device double, may be NULL) += sum|.|. */
+int splx_l1_loss_grad(splx_ctx *ctx, const float *image, const float *target, int64_t count,
+                      float scale, float *dL_dimage, double *loss_sum);
+
+/* ---- a8 composition backward: Eq.6-7.  g_ct[K,H,W,4] =
+ * (dL/dC^k rgb, dL/dT^k).  dL_dT_total[H,W] may be NULL.  Overwrites g_ct. */
+int splx_compose_backward(splx_ctx *ctx, int K, const splx_partial *partials,
+                          const splx_camera *cam, const float bg[3], const float *dL_dimage,
+                          const float *dL_dT_total, float *g_ct);
+
+/* ---- a9 rasteriser backward: PAPER.md L184.  Walks each pixel's list in reverse from
+ * n_contrib.  g2d[n,SPLX_G2D_STRIDE] += (dL/du, dL/dv, dL/dA, dL/dB, dL/dC, dL/do,
+ * dL/dr, dL/dg, dL/db, 0, 0, 0) per Gaussian (warp-reduced, then vector atomics). */
+int splx_raster_backward(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins,
+                         int K, const splx_camera *cam, const splx_partial *partials,
+                         const float *g_ct, float *g2d);
+
+/* ---- a10 projection backward: exact derivative of splx_project.  Reads
+ * g2d, accumulates into grads (+=).  If clear_g2d != 0 the consumed g2d rows are zeroed. */
+int splx_project_backward(splx_ctx *ctx, const splx_gaussians *g, const splx_camera *cam,
+                          int sh_degree, const splx_projected *proj, float *g2d, int clear_g2d,
+                          const splx_gaussian_grads *grads);
+
+/* ---- a8+a9+a10 in one call (BASELINE.json north_star "splx_backward").  ws holds g_ct
+ * and g2d; splx_backward_ws_bytes gives its size. */
+size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera *cam);
+int splx_backward(splx_ctx *ctx, int K, const splx_partial *partials, const splx_camera *cam,
+                  const float bg[3], const float *dL_dimage, const float *dL_dT_total,
+                  const splx_gaussians *g, const splx_projected *proj, const splx_binning *bins,
+                  int sh_degree, const splx_gaussian_grads *grads, void *ws, size_t ws_bytes);
+
+/* ---- a11 Adam (paper silent on the optimiser; north_star names Adam).  Dense,
+ * bias-corrected, step is 1-based.  grad_scale multiplies grad first (1/B for B views);
+ * if zero_grad != 0 the gradient is zeroed after use.  param/grad/m/v[count]. */
+int splx_adam(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int64_t count,
+              float lr, float beta1, float beta2, float eps, int step, float grad_scale,
+              int zero_grad);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPLX_H_ */

@@ -1,0 +1,297 @@
+"""Thin ctypes binding of ``libsplx.so`` (C ABI: ``include/splx.h``) -- argument marshalling only.
+
+Every function has the name of the C entry point without the ``splx_`` prefix and takes torch
+CUDA tensors (PyTorch is used for device memory and streams only); every step of the path
+runs in the CUDA kernels behind the ABI.  There is no CPU fallback: if ``libsplx.so`` is
+missing or no CUDA device is present, the first call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsplx.so")
+_lib = None
+
+G2D_STRIDE = 12
+TILE = 16
+MAX_K = 64
+OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA = 0, -1, -2, -3, -4
+
+EXPORTS = [
+    "splx_create", "splx_destroy", "splx_last_error", "splx_set_stream", "splx_launch_count",
+    "splx_project", "splx_bin_sort_ws_bytes", "splx_bin_sort", "splx_check_capacity",
+    "splx_render_partial", "splx_compose", "splx_l1_loss_grad", "splx_compose_backward",
+    "splx_raster_backward", "splx_project_backward", "splx_backward_ws_bytes", "splx_backward",
+    "splx_adam",
+]
+
+
+class SplxError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libsplx error {code}: {msg}")
+        self.code = code
+
+
+class Config(C.Structure):
+    _fields_ = [("alpha_min", C.c_float), ("alpha_max", C.c_float), ("T_eps", C.c_float),
+                ("dilation", C.c_float), ("lim_factor", C.c_float), ("radius_floor", C.c_float)]
+
+
+class CameraS(C.Structure):
+    _fields_ = [("R", C.c_float * 9), ("t", C.c_float * 3), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("width", C.c_int32), ("height", C.c_int32),
+                ("near_z", C.c_float)]
+
+
+class GaussiansS(C.Structure):
+    _fields_ = [("mean", C.c_void_p), ("log_scale", C.c_void_p), ("quat", C.c_void_p),
+                ("opacity_logit", C.c_void_p), ("sh", C.c_void_p), ("n", C.c_int64)]
+
+
+class ProjectedS(C.Structure):
+    _fields_ = [("means2d", C.c_void_p), ("depth", C.c_void_p), ("conic_opacity", C.c_void_p),
+                ("rgb", C.c_void_p), ("radius", C.c_void_p), ("tiles_touched", C.c_void_p),
+                ("clamp", C.c_void_p)]
+
+
+class BinningS(C.Structure):
+    _fields_ = [("keys", C.c_void_p), ("vals", C.c_void_p), ("tile_ranges", C.c_void_p),
+                ("capacity", C.c_uint64), ("num_intersections", C.c_void_p)]
+
+
+class PartialS(C.Structure):
+    _fields_ = [("ct", C.c_void_p), ("d", C.c_void_p), ("n_contrib", C.c_void_p)]
+
+
+def lib():
+    """Load libsplx.so; raise loudly if it is missing (the product path has no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: build it with "
+                              "`python -m paper_2606_18588_b200.build` (nvcc, sm_100a). No CPU fallback exists.")
+        L = C.CDLL(LIB_PATH)
+        L.splx_last_error.restype = C.c_char_p
+        L.splx_last_error.argtypes = [C.c_void_p]
+        L.splx_launch_count.restype = C.c_int64
+        L.splx_launch_count.argtypes = [C.c_void_p]
+        L.splx_bin_sort_ws_bytes.restype = C.c_size_t
+        L.splx_bin_sort_ws_bytes.argtypes = [C.c_int64, C.c_uint64, C.c_int, C.c_void_p]
+        L.splx_backward_ws_bytes.restype = C.c_size_t
+        L.splx_backward_ws_bytes.argtypes = [C.c_int64, C.c_int, C.c_void_p]
+        L.splx_create.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.splx_destroy.argtypes = [C.c_void_p]
+        L.splx_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+        L.splx_project.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        L.splx_bin_sort.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p,
+                                    C.c_void_p, C.c_void_p, C.c_size_t]
+        L.splx_check_capacity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.splx_render_partial.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
+                                          C.c_void_p, C.c_void_p]
+        L.splx_compose.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                   C.c_void_p]
+        L.splx_l1_loss_grad.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_float,
+                                        C.c_void_p, C.c_void_p]
+        L.splx_compose_backward.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_void_p, C.c_void_p, C.c_void_p]
+        L.splx_raster_backward.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
+                                           C.c_void_p, C.c_void_p, C.c_void_p]
+        L.splx_project_backward.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
+                                            C.c_void_p, C.c_int, C.c_void_p]
+        L.splx_backward.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
+                                    C.c_void_p, C.c_size_t]
+        L.splx_adam.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64,
+                                C.c_float, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float, C.c_int]
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    return t.data_ptr()
+
+
+def camera_struct(cam) -> CameraS:
+    """cam: any object with R, t, fx, fy, cx, cy, width, height, near_z (scenes.Camera)."""
+    s = CameraS()
+    R = [float(x) for x in list(cam.R.reshape(-1))]
+    t = [float(x) for x in list(cam.t.reshape(-1))]
+    s.R[:] = R
+    s.t[:] = t
+    s.fx, s.fy, s.cx, s.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    s.width, s.height, s.near_z = int(cam.width), int(cam.height), float(cam.near_z)
+    return s
+
+
+def gaussians_struct(p: dict, cls=GaussiansS):
+    n = p["mean"].shape[0]
+    for k, w in (("mean", 3), ("log_scale", 3), ("quat", 4), ("opacity_logit", 1), ("sh", 48)):
+        assert p[k].dtype == torch.float32 and p[k].numel() == n * w, k
+    return cls(_ptr(p["mean"]), _ptr(p["log_scale"]), _ptr(p["quat"]), _ptr(p["opacity_logit"]),
+               _ptr(p["sh"]), n)
+
+
+class Projected:
+    def __init__(self, n, device):
+        f = dict(dtype=torch.float32, device=device)
+        self.means2d = torch.empty((n, 2), **f)
+        self.depth = torch.empty(n, **f)
+        self.conic_opacity = torch.empty((n, 4), **f)
+        self.rgb = torch.empty((n, 3), **f)
+        self.radius = torch.empty(n, dtype=torch.int32, device=device)
+        self.tiles_touched = torch.empty(n, dtype=torch.int32, device=device)  # uint32 bits
+        self.clamp = torch.empty(n, dtype=torch.uint8, device=device)
+        self.n = n
+
+    def struct(self):
+        return ProjectedS(_ptr(self.means2d), _ptr(self.depth), _ptr(self.conic_opacity), _ptr(self.rgb),
+                          _ptr(self.radius), _ptr(self.tiles_touched), _ptr(self.clamp))
+
+
+class Binning:
+    def __init__(self, capacity, K, width, height, device):
+        self.TX, self.TY = (width + TILE - 1) // TILE, (height + TILE - 1) // TILE
+        self.capacity = int(capacity)
+        self.keys = torch.empty(max(self.capacity, 2), dtype=torch.int64, device=device)     # uint64 bits
+        self.vals = torch.empty(max(self.capacity, 4), dtype=torch.int32, device=device)     # uint32 bits
+        self.tile_ranges = torch.zeros((K * self.TX * self.TY, 2), dtype=torch.int32, device=device)
+        self.num_intersections = torch.zeros(2, dtype=torch.int64, device=device)
+
+    def struct(self):
+        return BinningS(_ptr(self.keys), _ptr(self.vals), _ptr(self.tile_ranges), self.capacity,
+                        _ptr(self.num_intersections))
+
+
+class Partial:
+    def __init__(self, K, width, height, device):
+        self.ct = torch.empty((K, height, width, 4), dtype=torch.float32, device=device)
+        self.d = torch.empty((K, height, width), dtype=torch.float32, device=device)
+        self.n_contrib = torch.empty((K, height, width), dtype=torch.int32, device=device)
+
+    def struct(self):
+        return PartialS(_ptr(self.ct), _ptr(self.d), _ptr(self.n_contrib))
+
+
+class Context:
+    """One splx_ctx bound to a device and a CUDA stream (default: torch's current stream)."""
+
+    def __init__(self, device=0, stream=None, cfg=None):
+        L = lib()
+        if not torch.cuda.is_available():
+            raise SplxError(ERR_CUDA, "no CUDA device; libsplx has no CPU fallback")
+        self.device = torch.device("cuda", device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        self._h = C.c_void_p()
+        c = Config(*cfg) if cfg is not None else None
+        rc = L.splx_create(C.byref(self._h), device, C.c_void_p(stream), C.byref(c) if c is not None else None)
+        if rc != OK:
+            raise SplxError(rc, L.splx_last_error(None).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().splx_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != OK:
+            raise SplxError(rc, lib().splx_last_error(self._h).decode())
+
+    def set_stream(self, stream):
+        self._check(lib().splx_set_stream(self._h, C.c_void_p(stream)))
+
+    def launch_count(self) -> int:
+        return int(lib().splx_launch_count(self._h))
+
+    # ---- the calls of SURVEY.md s8(b) ---------------------------------------------------
+    def project(self, params: dict, cam, sh_degree: int, out: Projected):
+        g = gaussians_struct(params)
+        cs = camera_struct(cam)
+        ps = out.struct()
+        self._check(lib().splx_project(self._h, C.byref(g), C.byref(cs), sh_degree, C.byref(ps)))
+
+    def bin_sort_ws_bytes(self, n, capacity, K, cam) -> int:
+        cs = camera_struct(cam)
+        return int(lib().splx_bin_sort_ws_bytes(n, capacity, K, C.byref(cs)))
+
+    def bin_sort(self, proj: Projected, K: int, part_offsets, cam, out: Binning, ws: torch.Tensor):
+        offs = (C.c_int64 * (K + 1))(*[int(x) for x in part_offsets])
+        cs = camera_struct(cam)
+        ps, bs = proj.struct(), out.struct()
+        self._check(lib().splx_bin_sort(self._h, C.byref(ps), proj.n, K, offs, C.byref(cs), C.byref(bs),
+                                        _ptr(ws), ws.numel() * ws.element_size()))
+
+    def check_capacity(self, bins: Binning) -> int:
+        m = C.c_uint64(0)
+        bs = bins.struct()
+        self._check(lib().splx_check_capacity(self._h, C.byref(bs), C.byref(m)))
+        return int(m.value)
+
+    def render_partial(self, proj: Projected, bins: Binning, K: int, cam, out: Partial, pairs=None):
+        cs = camera_struct(cam)
+        ps, bs, os_ = proj.struct(), bins.struct(), out.struct()
+        self._check(lib().splx_render_partial(self._h, C.byref(ps), C.byref(bs), K, C.byref(cs), C.byref(os_),
+                                              _ptr(pairs)))
+
+    def compose(self, K: int, partials: Partial, cam, bg, image: torch.Tensor, T_total=None):
+        cs = camera_struct(cam)
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        ps = partials.struct()
+        self._check(lib().splx_compose(self._h, K, C.byref(ps), C.byref(cs), b, _ptr(image), _ptr(T_total)))
+
+    def l1_loss_grad(self, image, target, g_image, loss_sum=None, scale=1.0):
+        self._check(lib().splx_l1_loss_grad(self._h, _ptr(image), _ptr(target), image.numel(), scale,
+                                            _ptr(g_image), _ptr(loss_sum)))
+
+    def compose_backward(self, K, partials: Partial, cam, bg, g_image, g_T_total, g_ct):
+        cs = camera_struct(cam)
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        ps = partials.struct()
+        self._check(lib().splx_compose_backward(self._h, K, C.byref(ps), C.byref(cs), b, _ptr(g_image),
+                                                _ptr(g_T_total), _ptr(g_ct)))
+
+    def raster_backward(self, proj: Projected, bins: Binning, K, cam, partials: Partial, g_ct, g2d):
+        cs = camera_struct(cam)
+        ps, bs, pa = proj.struct(), bins.struct(), partials.struct()
+        self._check(lib().splx_raster_backward(self._h, C.byref(ps), C.byref(bs), K, C.byref(cs), C.byref(pa),
+                                               _ptr(g_ct), _ptr(g2d)))
+
+    def project_backward(self, params: dict, cam, sh_degree, proj: Projected, g2d, grads: dict, clear_g2d=False):
+        g = gaussians_struct(params)
+        gg = gaussians_struct(grads)
+        cs = camera_struct(cam)
+        ps = proj.struct()
+        self._check(lib().splx_project_backward(self._h, C.byref(g), C.byref(cs), sh_degree, C.byref(ps),
+                                                _ptr(g2d), int(clear_g2d), C.byref(gg)))
+
+    def backward_ws_bytes(self, n, K, cam) -> int:
+        cs = camera_struct(cam)
+        return int(lib().splx_backward_ws_bytes(n, K, C.byref(cs)))
+
+    def backward(self, K, partials: Partial, cam, bg, g_image, g_T_total, params: dict, proj: Projected,
+                 bins: Binning, sh_degree, grads: dict, ws: torch.Tensor):
+        cs = camera_struct(cam)
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        pa, ps, bs = partials.struct(), proj.struct(), bins.struct()
+        g, gg = gaussians_struct(params), gaussians_struct(grads)
+        self._check(lib().splx_backward(self._h, K, C.byref(pa), C.byref(cs), b, _ptr(g_image), _ptr(g_T_total),
+                                        C.byref(g), C.byref(ps), C.byref(bs), sh_degree, C.byref(gg),
+                                        _ptr(ws), ws.numel() * ws.element_size()))
+
+    def adam(self, param, grad, m, v, lr, beta1=0.9, beta2=0.999, eps=1e-15, step=1, grad_scale=1.0,
+             zero_grad=False):
+        self._check(lib().splx_adam(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), param.numel(), lr,
+                                    beta1, beta2, eps, step, grad_scale, int(zero_grad)))

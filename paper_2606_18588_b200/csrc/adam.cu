@@ -1,0 +1,65 @@
+// adam.cu -- step a11, the optimiser update.  PAPER.md L184 / L190 only say that "the parameters
+// can be optimized"; the optimiser is unnamed: dense bias-corrected Adam,
+//   m = b1 m + (1-b1) g;  v = b2 v + (1-b2) g^2;  p -= lr (m/(1-b1^t)) / (sqrt(v/(1-b2^t)) + eps).
+// HBM-bound: 16 B read + 12 B written per parameter (+4 B when the gradient is zeroed in place).
+// 128-bit loads/stores, grid = a multiple of the SM count, grid-stride.
+#include "common.cuh"
+
+namespace {
+
+constexpr int AB = 256;
+
+struct AdamK { float lr, b1, b2, omb1, omb2, eps, ibc1, ibc2; };
+
+__device__ __forceinline__ void adam1(float& p, float g, float& m, float& v, const AdamK& k) {
+  const float lr = k.lr, eps = k.eps, ibc1 = k.ibc1, ibc2 = k.ibc2;
+  m = fmaf(k.b1, m, k.omb1 * g);
+  v = fmaf(k.b2, v, k.omb2 * g * g);
+  p -= lr * (m * ibc1) / (sqrtf(v * ibc2) + eps);
+}
+
+__global__ void __launch_bounds__(AB)
+k_adam(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ m, float* __restrict__ v,
+       int64_t count, AdamK k, float gscale, int zero_grad) {
+  const int64_t nvec = count >> 2;
+  for (int64_t i = (int64_t)blockIdx.x * AB + threadIdx.x; i < nvec; i += (int64_t)gridDim.x * AB) {
+    float4 p = reinterpret_cast<float4*>(param)[i];
+    float4 g = reinterpret_cast<const float4*>(grad)[i];
+    float4 mm = reinterpret_cast<float4*>(m)[i];
+    float4 vv = reinterpret_cast<float4*>(v)[i];
+    adam1(p.x, g.x * gscale, mm.x, vv.x, k);
+    adam1(p.y, g.y * gscale, mm.y, vv.y, k);
+    adam1(p.z, g.z * gscale, mm.z, vv.z, k);
+    adam1(p.w, g.w * gscale, mm.w, vv.w, k);
+    reinterpret_cast<float4*>(param)[i] = p;
+    reinterpret_cast<float4*>(m)[i] = mm;
+    reinterpret_cast<float4*>(v)[i] = vv;
+    if (zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  if (blockIdx.x == 0 && threadIdx.x < (count & 3)) {
+    const int64_t i = (nvec << 2) + threadIdx.x;
+    float p = param[i], mm = m[i], vv = v[i];
+    adam1(p, grad[i] * gscale, mm, vv, k);
+    param[i] = p; m[i] = mm; v[i] = vv;
+    if (zero_grad) grad[i] = 0.f;
+  }
+}
+
+}  // namespace
+
+int launch_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr,
+                float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad) {
+  if (count <= 0) return SPLX_OK;
+  const double bc1 = 1.0 - pow((double)beta1, step), bc2 = 1.0 - pow((double)beta2, step);
+  const int64_t nvec = count >> 2;
+  int64_t blocks = (nvec + AB - 1) / AB;
+  const int64_t cap = (int64_t)SPLX_SM_COUNT * 8;   // 8 resident CTAs of 256 threads per SM
+  if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
+  // 1-beta and the bias corrections are formed in double on the host (0.999f is not 0.999)
+  const AdamK k{lr, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps,
+                (float)(1.0 / bc1), (float)(1.0 / bc2)};
+  k_adam<<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, count, k, grad_scale, zero_grad);
+  SPLX_LAUNCH_CHECK(ctx, "k_adam");
+  return SPLX_OK;
+}

@@ -1,0 +1,211 @@
+// api.cu -- the C ABI of include/splx.h: argument validation and stage sequencing only; every
+// step of the path runs in the kernels of project.cu / sort.cu / render.cu / compose.cu / adam.cu.
+#include "common.cuh"
+
+static char g_create_err[512] = "";
+
+static bool cam_ok(const splx_camera* c) {
+  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f;
+}
+static bool proj_ok(const splx_projected* p) {
+  return p && p->means2d && p->depth && p->conic_opacity && p->rgb && p->radius && p->tiles_touched &&
+         p->clamp && aligned16(p->means2d) && aligned16(p->conic_opacity);
+}
+static bool gauss_ok(const splx_gaussians* g) {
+  return g && g->n >= 0 && (g->n == 0 || (g->mean && g->log_scale && g->quat && g->opacity_logit && g->sh &&
+                                          aligned16(g->quat) && aligned16(g->sh)));
+}
+static bool partial_ok(const splx_partial* p) {
+  return p && p->ct && p->d && p->n_contrib && aligned16(p->ct);
+}
+static bool bins_ok(const splx_binning* b) {
+  return b && b->keys && b->vals && b->tile_ranges && b->num_intersections && aligned16(b->keys);
+}
+
+extern "C" {
+
+int splx_create(splx_ctx** out, int device, void* cuda_stream, const splx_config* cfg) {
+  if (!out) { snprintf(g_create_err, sizeof g_create_err, "splx_create: out is NULL"); return SPLX_ERR_INVALID_ARG; }
+  *out = nullptr;
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev <= 0) {
+    snprintf(g_create_err, sizeof g_create_err, "splx_create: no CUDA device (%s); there is no CPU fallback",
+             e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+    return SPLX_ERR_CUDA;
+  }
+  if (device < 0 || device >= ndev) {
+    snprintf(g_create_err, sizeof g_create_err, "splx_create: device %d out of range [0,%d)", device, ndev);
+    return SPLX_ERR_INVALID_ARG;
+  }
+  if ((e = cudaSetDevice(device)) != cudaSuccess) {
+    snprintf(g_create_err, sizeof g_create_err, "cudaSetDevice: %s", cudaGetErrorString(e));
+    return SPLX_ERR_CUDA;
+  }
+  splx_ctx* c = new splx_ctx();
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->launches = 0;
+  c->err[0] = 0;
+  if (cfg) c->cfg = *cfg;
+  else c->cfg = splx_config{1.0f / 255.0f, 0.99f, 1e-4f, 0.3f, 1.3f, 0.1f};
+  if (!(c->cfg.alpha_max > 0.f) || c->cfg.alpha_min < 0.f || c->cfg.T_eps < 0.f) {
+    delete c;
+    snprintf(g_create_err, sizeof g_create_err, "splx_create: bad config");
+    return SPLX_ERR_INVALID_ARG;
+  }
+  *out = c;
+  return SPLX_OK;
+}
+
+int splx_destroy(splx_ctx* ctx) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  delete ctx;
+  return SPLX_OK;
+}
+
+const char* splx_last_error(const splx_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+int splx_set_stream(splx_ctx* ctx, void* cuda_stream) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  ctx->stream = (cudaStream_t)cuda_stream;
+  return SPLX_OK;
+}
+
+int64_t splx_launch_count(const splx_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+int splx_project(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
+                 const splx_projected* out) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: null/misaligned argument");
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: sh_degree %d not in [0,3]", sh_degree);
+  return launch_project_fwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, out);
+}
+
+size_t splx_bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, const splx_camera* cam) {
+  if (n < 0 || !cam_ok(cam) || K < 1) return 0;
+  const int TX = (cam->width + SPLX_TILE - 1) / SPLX_TILE, TY = (cam->height + SPLX_TILE - 1) / SPLX_TILE;
+  return bin_sort_ws_bytes(n, capacity, K, TX, TY);
+}
+
+int splx_bin_sort(splx_ctx* ctx, const splx_projected* proj, int64_t n, int K, const int64_t* part_offsets,
+                  const splx_camera* cam, const splx_binning* out, void* ws, size_t ws_bytes) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !cam_ok(cam) || !bins_ok(out) || !part_offsets || n < 0 || (!ws && ws_bytes))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: null/misaligned argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  if (part_offsets[0] != 0 || part_offsets[K] != n) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: part_offsets must run from 0 to n");
+  for (int k = 0; k < K; ++k)
+    if (part_offsets[k + 1] < part_offsets[k]) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: part_offsets not monotone");
+  if (n >= ((int64_t)1 << 32) || out->capacity >= ((uint64_t)1 << 32))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: n and capacity must be < 2^32");
+  const CamDev cd = make_camdev(cam, ctx->cfg);
+  if ((uint64_t)K * cd.TX * cd.TY >= ((uint64_t)1 << 31)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles too large");
+  if (!aligned16(ws)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: workspace not 16-byte aligned");
+  return launch_bin_sort(ctx, proj, n, K, part_offsets, cd, out, ws, ws_bytes);
+}
+
+int splx_check_capacity(splx_ctx* ctx, const splx_binning* bins, uint64_t* m_host) {
+  if (!ctx || !bins || !bins->num_intersections) return SPLX_ERR_INVALID_ARG;
+  uint64_t m = 0;
+  SPLX_CUDA_OK(ctx, cudaMemcpyAsync(&m, bins->num_intersections, sizeof m, cudaMemcpyDeviceToHost, ctx->stream));
+  SPLX_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  if (m_host) *m_host = m;
+  if (m > bins->capacity)
+    SPLX_FAIL(ctx, SPLX_ERR_CAPACITY, "splx_bin_sort: %llu intersections exceed capacity %llu",
+              (unsigned long long)m, (unsigned long long)bins->capacity);
+  return SPLX_OK;
+}
+
+int splx_render_partial(splx_ctx* ctx, const splx_projected* proj, const splx_binning* bins, int K,
+                        const splx_camera* cam, const splx_partial* out, uint64_t* pairs) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !bins_ok(bins) || !cam_ok(cam) || !partial_ok(out))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: null/misaligned argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  return launch_render_fwd(ctx, proj, bins, K, make_camdev(cam, ctx->cfg), out, pairs);
+}
+
+int splx_compose(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
+                 float* image, float* T_total) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!partial_ok(partials) || !cam_ok(cam) || !bg || !image) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: null/misaligned argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  return launch_compose_fwd(ctx, K, partials, make_camdev(cam, ctx->cfg), bg, image, T_total);
+}
+
+int splx_l1_loss_grad(splx_ctx* ctx, const float* image, const float* target, int64_t count, float scale,
+                      float* dL_dimage, double* loss_sum) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!image || !target || !dL_dimage || count < 0 || !aligned16(image) || !aligned16(target) || !aligned16(dL_dimage))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_l1_loss_grad: null/misaligned argument");
+  return launch_l1(ctx, image, target, count, scale, dL_dimage, loss_sum);
+}
+
+int splx_compose_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam,
+                          const float bg[3], const float* dL_dimage, const float* dL_dT_total, float* g_ct) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!partial_ok(partials) || !cam_ok(cam) || !bg || !dL_dimage || !g_ct || !aligned16(g_ct))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: null/misaligned argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  return launch_compose_bwd(ctx, K, partials, make_camdev(cam, ctx->cfg), bg, dL_dimage, dL_dT_total, g_ct);
+}
+
+int splx_raster_backward(splx_ctx* ctx, const splx_projected* proj, const splx_binning* bins, int K,
+                         const splx_camera* cam, const splx_partial* partials, const float* g_ct, float* g2d) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !bins_ok(bins) || !cam_ok(cam) || !partial_ok(partials) || !g_ct || !g2d ||
+      !aligned16(g_ct) || !aligned16(g2d))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: null/misaligned argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  return launch_raster_bwd(ctx, proj, bins, K, make_camdev(cam, ctx->cfg), partials, g_ct, g2d);
+}
+
+int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
+                          const splx_projected* proj, float* g2d, int clear_g2d, const splx_gaussian_grads* grads) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(proj) || !g2d || !aligned16(g2d) || !grads || !grads->mean ||
+      !grads->log_scale || !grads->quat || !grads->opacity_logit || !grads->sh || !aligned16(grads->quat) || grads->n != g->n)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: null/misaligned argument");
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: sh_degree %d not in [0,3]", sh_degree);
+  return launch_project_bwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, proj, g2d, clear_g2d, grads);
+}
+
+size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera* cam) {
+  if (n < 0 || K < 1 || !cam_ok(cam)) return 0;
+  const size_t g_ct = align_up((size_t)K * cam->width * cam->height * 4 * sizeof(float), 256);
+  const size_t g2d = align_up((size_t)n * SPLX_G2D_STRIDE * sizeof(float), 256);
+  return g_ct + g2d;
+}
+
+int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
+                  const float* dL_dimage, const float* dL_dT_total, const splx_gaussians* g,
+                  const splx_projected* proj, const splx_binning* bins, int sh_degree,
+                  const splx_gaussian_grads* grads, void* ws, size_t ws_bytes) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!gauss_ok(g) || !cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: null/misaligned argument");
+  const size_t need = splx_backward_ws_bytes(g->n, K, cam);
+  if (!ws || !aligned16(ws) || ws_bytes < need)
+    SPLX_FAIL(ctx, SPLX_ERR_WORKSPACE, "splx_backward: workspace %zu B < required %zu B", ws_bytes, need);
+  float* g_ct = (float*)ws;
+  float* g2d = (float*)((char*)ws + align_up((size_t)K * cam->width * cam->height * 4 * sizeof(float), 256));
+  int rc;
+  // a8: Eq.6-7 hand dL/dC^k, dL/dT^k to every partition's rasteriser backward
+  if ((rc = splx_compose_backward(ctx, K, partials, cam, bg, dL_dimage, dL_dT_total, g_ct))) return rc;
+  SPLX_CUDA_OK(ctx, cudaMemsetAsync(g2d, 0, (size_t)g->n * SPLX_G2D_STRIDE * sizeof(float), ctx->stream));
+  // a9: reverse-order blend gradients into means2D, conic, opacity, colour
+  if ((rc = splx_raster_backward(ctx, proj, bins, K, cam, partials, g_ct, g2d))) return rc;
+  // a10: projection backward to the 3-D parameters
+  return splx_project_backward(ctx, g, cam, sh_degree, proj, g2d, 0, grads);
+}
+
+int splx_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr, float beta1,
+              float beta2, float eps, int step, float grad_scale, int zero_grad) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!param || !grad || !m || !v || count < 0 || step < 1 || !aligned16(param) || !aligned16(grad) ||
+      !aligned16(m) || !aligned16(v))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam: null/misaligned argument or step < 1");
+  return launch_adam(ctx, param, grad, m, v, count, lr, beta1, beta2, eps, step, grad_scale, zero_grad);
+}
+
+}  // extern "C"

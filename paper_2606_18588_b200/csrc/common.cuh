@@ -1,0 +1,107 @@
+// common.cuh -- shared declarations of the CUDA path (sm_100a).  Nothing here is shared
+// with oracle/: the oracle restates every formula on its own.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/splx.h"
+
+#define SPLX_SM_COUNT 148  // B200: 2 dies x 74 SMs; grids of persistent kernels are multiples of it
+
+struct splx_ctx {
+  int device;
+  cudaStream_t stream;
+  splx_config cfg;
+  int64_t launches;
+  char err[512];
+};
+
+// Device-side copy of the camera plus derived quantities, passed by value to kernels.
+struct CamDev {
+  float R[9], t[3];
+  float fx, fy, cx, cy;
+  int W, H, TX, TY;
+  float near_z;
+  float o[3];  // camera centre -R^T t
+  float limx, limy;
+};
+
+static inline CamDev make_camdev(const splx_camera* c, const splx_config& cfg) {
+  CamDev d;
+  for (int i = 0; i < 9; ++i) d.R[i] = c->R[i];
+  for (int i = 0; i < 3; ++i) d.t[i] = c->t[i];
+  d.fx = c->fx; d.fy = c->fy; d.cx = c->cx; d.cy = c->cy;
+  d.W = c->width; d.H = c->height;
+  d.TX = (c->width + SPLX_TILE - 1) / SPLX_TILE;
+  d.TY = (c->height + SPLX_TILE - 1) / SPLX_TILE;
+  d.near_z = c->near_z;
+  for (int j = 0; j < 3; ++j)
+    d.o[j] = -(c->R[0 * 3 + j] * c->t[0] + c->R[1 * 3 + j] * c->t[1] + c->R[2 * 3 + j] * c->t[2]);
+  d.limx = cfg.lim_factor * (float)c->width / (2.0f * c->fx);
+  d.limy = cfg.lim_factor * (float)c->height / (2.0f * c->fy);
+  return d;
+}
+
+#define SPLX_FAIL(ctx, code, ...)                                  \
+  do {                                                             \
+    snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__);         \
+    return (code);                                                 \
+  } while (0)
+
+#define SPLX_CUDA_OK(ctx, expr)                                                          \
+  do {                                                                                   \
+    cudaError_t e_ = (expr);                                                             \
+    if (e_ != cudaSuccess)                                                               \
+      SPLX_FAIL(ctx, SPLX_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e_));     \
+  } while (0)
+
+#define SPLX_LAUNCH_CHECK(ctx, name)                                                     \
+  do {                                                                                   \
+    cudaError_t e_ = cudaGetLastError();                                                 \
+    if (e_ != cudaSuccess)                                                               \
+      SPLX_FAIL(ctx, SPLX_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(e_)); \
+    (ctx)->launches++;                                                                   \
+  } while (0)
+
+static inline bool aligned16(const void* p) { return (((uintptr_t)p) & 15u) == 0; }
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Tile rectangle of a projected footprint (reading s11): pixel i samples i+0.5,
+// so [u-r, u+r] covers pixel columns i with u-0.5-r <= i <= u-0.5+r.  Written with explicit
+// round-to-nearest intrinsics so that no fused multiply-add can change the integer result.
+__device__ __forceinline__ void tile_rect(float u, float v, int radius, int TX, int TY, int& x0,
+                                          int& y0, int& x1, int& y1) {
+  const float rf = (float)radius;
+  const float ux = __fsub_rn(u, 0.5f), vy = __fsub_rn(v, 0.5f);
+  const float x0f = floorf(__fmul_rn(__fsub_rn(ux, rf), 0.0625f));
+  const float x1f = floorf(__fmul_rn(__fadd_rn(__fadd_rn(ux, rf), 15.0f), 0.0625f));
+  const float y0f = floorf(__fmul_rn(__fsub_rn(vy, rf), 0.0625f));
+  const float y1f = floorf(__fmul_rn(__fadd_rn(__fadd_rn(vy, rf), 15.0f), 0.0625f));
+  x0 = !(x0f > 0.0f) ? 0 : (x0f >= (float)TX ? TX : (int)x0f);
+  x1 = !(x1f > 0.0f) ? 0 : (x1f >= (float)TX ? TX : (int)x1f);
+  y0 = !(y0f > 0.0f) ? 0 : (y0f >= (float)TY ? TY : (int)y0f);
+  y1 = !(y1f > 0.0f) ? 0 : (y1f >= (float)TY ? TY : (int)y1f);
+}
+
+// ---- stage launchers (defined one per .cu file, called from api.cu) ----------------------
+int launch_project_fwd(splx_ctx*, const splx_gaussians*, const CamDev&, int sh_degree,
+                       const splx_projected*);
+int launch_project_bwd(splx_ctx*, const splx_gaussians*, const CamDev&, int sh_degree,
+                       const splx_projected*, float* g2d, int clear_g2d, const splx_gaussian_grads*);
+size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
+int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, int K, const int64_t* part_offsets,
+                    const CamDev&, const splx_binning*, void* ws, size_t ws_bytes);
+int launch_render_fwd(splx_ctx*, const splx_projected*, const splx_binning*, int K, const CamDev&,
+                      const splx_partial*, uint64_t* pairs);
+int launch_raster_bwd(splx_ctx*, const splx_projected*, const splx_binning*, int K, const CamDev&,
+                      const splx_partial*, const float* g_ct, float* g2d);
+int launch_compose_fwd(splx_ctx*, int K, const splx_partial*, const CamDev&, const float* bg,
+                       float* image, float* T_total);
+int launch_compose_bwd(splx_ctx*, int K, const splx_partial*, const CamDev&, const float* bg,
+                       const float* g_image, const float* g_T_total, float* g_ct);
+int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count, float scale,
+              float* g_image, double* loss_sum);
+int launch_adam(splx_ctx*, float* param, float* grad, float* m, float* v, int64_t count, float lr,
+                float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad);

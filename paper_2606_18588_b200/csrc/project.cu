@@ -1,0 +1,352 @@
+// project.cu -- step a1 (projection) and step a10 (its exact derivative).
+// Sigma = R S S^T R^T.  L80: frustum cull by the mean; Sigma2D = J W Sigma W^T J^T;
+// 2-D attributes depth d, 2-D mean, Sigma2D.  Readings: s5 depth = camera z,
+// s8 cull rule, s9 dilation / radius / J clamp, s10 pixel centres, s11 tile rect, s13 SH colour,
+// s14 parameterisation, s15 true derivative at clamps.
+//
+// Both kernels are HBM-bound streaming kernels: one thread per Gaussian, 236 B of parameters in
+// for a visible Gaussian (44 B for a culled one: the 192 B of SH are only read when visible).
+#include "common.cuh"
+
+namespace {
+
+constexpr int PROJ_THREADS = 256;
+
+// Real SH constants (orthonormal basis, Condon-Shortley phase; index l(l+1)+m).
+constexpr float kY0 = 0.28209479177387814f;
+constexpr float kK1 = 0.4886025119029199f;
+constexpr float kK2a = 1.0925484305920792f;
+constexpr float kK2b = 0.31539156525252005f;
+constexpr float kK2c = 0.5462742152960396f;
+constexpr float kK3a = 0.5900435899266435f;
+constexpr float kK3b = 2.890611442640554f;
+constexpr float kK3c = 0.4570457994644658f;
+constexpr float kK3d = 0.3731763325901154f;
+constexpr float kK3e = 1.445305721320277f;
+
+struct Geo {  // forward intermediates shared by both directions
+  float p[3];
+  float s[3], qh[4], qn, Rot[9], Mm[9];
+  float Tm[6];    // J * W
+  float N[6];     // Tm * Mm  (2x3):  Sigma2D = N N^T + dilation I
+  float a, b, c, det;
+  float Lx, Ly;   // clamped x/z, y/z used inside J
+  bool clx, cly;
+};
+
+__device__ __forceinline__ float det2_accurate(float a, float c, float b) {
+  // a*c - b*b with one rounding error instead of a cancellation (Kahan's fma scheme)
+  const float w = b * b;
+  const float e = fmaf(-b, b, w);
+  const float f = fmaf(a, c, -w);
+  return f + e;
+}
+
+__device__ __forceinline__ bool geometry(const splx_gaussians& g, int64_t i, const CamDev& cam,
+                                         float dilation, Geo& G) {
+  const float mx = g.mean[3 * i], my = g.mean[3 * i + 1], mz = g.mean[3 * i + 2];
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+    G.p[r] = cam.R[3 * r] * mx + cam.R[3 * r + 1] * my + cam.R[3 * r + 2] * mz + cam.t[r];
+  if (!(G.p[2] > cam.near_z)) return false;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) G.s[k] = expf(g.log_scale[3 * i + k]);
+  const float4 q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
+  G.qn = sqrtf(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
+  const float inv = 1.0f / G.qn;
+  const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
+  G.qh[0] = w; G.qh[1] = x; G.qh[2] = y; G.qh[3] = z;
+  G.Rot[0] = 1.f - 2.f * (y * y + z * z); G.Rot[1] = 2.f * (x * y - w * z); G.Rot[2] = 2.f * (x * z + w * y);
+  G.Rot[3] = 2.f * (x * y + w * z); G.Rot[4] = 1.f - 2.f * (x * x + z * z); G.Rot[5] = 2.f * (y * z - w * x);
+  G.Rot[6] = 2.f * (x * z - w * y); G.Rot[7] = 2.f * (y * z + w * x); G.Rot[8] = 1.f - 2.f * (x * x + y * y);
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) G.Mm[3 * r + c] = G.Rot[3 * r + c] * G.s[c];
+  const float pz = G.p[2], iz = 1.0f / pz;
+  const float xz = G.p[0] * iz, yz = G.p[1] * iz;
+  G.clx = (xz < -cam.limx) || (xz > cam.limx);
+  G.cly = (yz < -cam.limy) || (yz > cam.limy);
+  G.Lx = fminf(cam.limx, fmaxf(-cam.limx, xz));
+  G.Ly = fminf(cam.limy, fmaxf(-cam.limy, yz));
+  const float j00 = cam.fx * iz, j02 = -cam.fx * G.Lx * iz;  // -fx * (Lx z) / z^2
+  const float j11 = cam.fy * iz, j12 = -cam.fy * G.Ly * iz;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    G.Tm[c] = j00 * cam.R[c] + j02 * cam.R[6 + c];
+    G.Tm[3 + c] = j11 * cam.R[3 + c] + j12 * cam.R[6 + c];
+  }
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+      G.N[3 * r + c] = G.Tm[3 * r] * G.Mm[c] + G.Tm[3 * r + 1] * G.Mm[3 + c] + G.Tm[3 * r + 2] * G.Mm[6 + c];
+  G.a = G.N[0] * G.N[0] + G.N[1] * G.N[1] + G.N[2] * G.N[2] + dilation;
+  G.b = G.N[0] * G.N[3] + G.N[1] * G.N[4] + G.N[2] * G.N[5];
+  G.c = G.N[3] * G.N[3] + G.N[4] * G.N[4] + G.N[5] * G.N[5] + dilation;
+  G.det = det2_accurate(G.a, G.c, G.b);
+  return G.det > 0.0f;
+}
+
+// Y_l(dir), l < (deg+1)^2
+__device__ __forceinline__ void sh_eval(int deg, float x, float y, float z, float* Y) {
+  Y[0] = kY0;
+  if (deg < 1) return;
+  Y[1] = -kK1 * y; Y[2] = kK1 * z; Y[3] = -kK1 * x;
+  if (deg < 2) return;
+  const float xx = x * x, yy = y * y, zz = z * z;
+  Y[4] = kK2a * x * y; Y[5] = -kK2a * y * z; Y[6] = kK2b * (2.f * zz - xx - yy);
+  Y[7] = -kK2a * x * z; Y[8] = kK2c * (xx - yy);
+  if (deg < 3) return;
+  Y[9] = -kK3a * y * (3.f * xx - yy);
+  Y[10] = kK3b * x * y * z;
+  Y[11] = -kK3c * y * (4.f * zz - xx - yy);
+  Y[12] = kK3d * z * (2.f * zz - 3.f * xx - 3.f * yy);
+  Y[13] = -kK3c * x * (4.f * zz - xx - yy);
+  Y[14] = kK3e * z * (xx - yy);
+  Y[15] = -kK3a * x * (xx - 3.f * yy);
+}
+
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS)
+k_project_fwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected out) {
+  const int64_t i = (int64_t)blockIdx.x * PROJ_THREADS + threadIdx.x;
+  if (i >= g.n) return;
+  Geo G;
+  bool vis = geometry(g, i, cam, cfg.dilation, G);
+  float u = 0.f, v = 0.f;
+  int rad = 0, tt = 0;
+  if (vis) {
+    const float mid = 0.5f * (G.a + G.c);
+    const float hd = 0.5f * (G.a - G.c);
+    const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
+    rad = (int)ceilf(3.0f * sqrtf(lam));
+    const float iz = 1.0f / G.p[2];
+    u = cam.fx * G.p[0] * iz + cam.cx;
+    v = cam.fy * G.p[1] * iz + cam.cy;
+    int x0, y0, x1, y1;
+    tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
+    tt = (x1 - x0) * (y1 - y0);
+    vis = tt > 0;
+  }
+  if (!vis) {
+    *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(0.f, 0.f);
+    out.depth[i] = 0.f;
+    *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
+    out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
+    out.radius[i] = 0; out.tiles_touched[i] = 0; out.clamp[i] = 0;
+    return;
+  }
+  const float idet = 1.0f / G.det;
+  const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
+  *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
+  out.depth[i] = G.p[2];
+  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(G.c * idet, -G.b * idet, G.a * idet, op);
+  out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
+
+  // colour: SH along the direction from the camera centre to the mean (s13)
+  float dx = g.mean[3 * i] - cam.o[0], dy = g.mean[3 * i + 1] - cam.o[1], dz = g.mean[3 * i + 2] - cam.o[2];
+  const float dinv = rsqrtf(dx * dx + dy * dy + dz * dz);
+  dx *= dinv; dy *= dinv; dz *= dinv;
+  constexpr int NSH = (DEG + 1) * (DEG + 1);
+  float Y[NSH];
+  sh_eval(DEG, dx, dy, dz, Y);
+  const float4* sh4 = reinterpret_cast<const float4*>(g.sh + 48 * i);
+  float c[3] = {0.5f, 0.5f, 0.5f};
+  constexpr int NV = (NSH * 3 + 3) / 4;
+#pragma unroll
+  for (int q = 0; q < NV; ++q) {
+    const float4 f = __ldg(sh4 + q);
+    const float e[4] = {f.x, f.y, f.z, f.w};
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const int idx = 4 * q + t;
+      if (idx < NSH * 3) c[idx % 3] = fmaf(Y[idx / 3], e[t], c[idx % 3]);
+    }
+  }
+  uint8_t cl = 0;
+#pragma unroll
+  for (int ch = 0; ch < 3; ++ch) {
+    if (c[ch] < 0.f) { cl |= (uint8_t)(1u << ch); c[ch] = 0.f; }
+    out.rgb[3 * i + ch] = c[ch];
+  }
+  out.clamp[i] = cl;
+}
+
+// Gradients of Y_l with respect to the (unconstrained) direction components.
+__device__ __forceinline__ void sh_grad(int deg, float x, float y, float z, float (*dY)[3]) {
+  for (int l = 0; l < (deg + 1) * (deg + 1); ++l) dY[l][0] = dY[l][1] = dY[l][2] = 0.f;
+  if (deg < 1) return;
+  dY[1][1] = -kK1; dY[2][2] = kK1; dY[3][0] = -kK1;
+  if (deg < 2) return;
+  dY[4][0] = kK2a * y; dY[4][1] = kK2a * x;
+  dY[5][1] = -kK2a * z; dY[5][2] = -kK2a * y;
+  dY[6][0] = -2.f * kK2b * x; dY[6][1] = -2.f * kK2b * y; dY[6][2] = 4.f * kK2b * z;
+  dY[7][0] = -kK2a * z; dY[7][2] = -kK2a * x;
+  dY[8][0] = 2.f * kK2c * x; dY[8][1] = -2.f * kK2c * y;
+  if (deg < 3) return;
+  const float xx = x * x, yy = y * y, zz = z * z;
+  dY[9][0] = -6.f * kK3a * x * y; dY[9][1] = -3.f * kK3a * (xx - yy);
+  dY[10][0] = kK3b * y * z; dY[10][1] = kK3b * x * z; dY[10][2] = kK3b * x * y;
+  dY[11][0] = 2.f * kK3c * x * y; dY[11][1] = -kK3c * (4.f * zz - xx - 3.f * yy); dY[11][2] = -8.f * kK3c * y * z;
+  dY[12][0] = -6.f * kK3d * x * z; dY[12][1] = -6.f * kK3d * y * z; dY[12][2] = 3.f * kK3d * (2.f * zz - xx - yy);
+  dY[13][0] = -kK3c * (4.f * zz - 3.f * xx - yy); dY[13][1] = 2.f * kK3c * x * y; dY[13][2] = -8.f * kK3c * x * z;
+  dY[14][0] = 2.f * kK3e * x * z; dY[14][1] = -2.f * kK3e * y * z; dY[14][2] = kK3e * (xx - yy);
+  dY[15][0] = -3.f * kK3a * (xx - yy); dY[15][1] = 6.f * kK3a * x * y;
+}
+
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS)
+k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, float* __restrict__ g2d,
+              int clear_g2d, splx_gaussian_grads out) {
+  const int64_t i = (int64_t)blockIdx.x * PROJ_THREADS + threadIdx.x;
+  if (i >= g.n) return;
+  if (pr.radius[i] <= 0) return;
+  Geo G;
+  if (!geometry(g, i, cam, cfg.dilation, G)) return;
+  float4* gp = reinterpret_cast<float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
+  const float4 g0 = gp[0], g1 = gp[1], g2 = gp[2];
+  if (clear_g2d) { const float4 zz = make_float4(0.f, 0.f, 0.f, 0.f); gp[0] = zz; gp[1] = zz; gp[2] = zz; }
+  const float gu = g0.x, gv = g0.y, gA = g0.z, gB = g0.w, gC = g1.x, gop = g1.y;
+  float grgb[3] = {g1.z, g1.w, g2.x};
+
+  // opacity: o = sigmoid(logit)
+  const float op = pr.conic_opacity[4 * i + 3];
+  out.opacity_logit[i] += op * (1.f - op) * gop;
+
+  float dmu[3] = {0.f, 0.f, 0.f};
+  // colour: rgb = max(0, 0.5 + sum_l Y_l(dir) sh_l), dir = (mu - o)/|mu - o|
+  {
+    const uint8_t cl = pr.clamp[i];
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) if ((cl >> ch) & 1) grgb[ch] = 0.f;
+    float dv[3] = {g.mean[3 * i] - cam.o[0], g.mean[3 * i + 1] - cam.o[1], g.mean[3 * i + 2] - cam.o[2]};
+    const float dinv = rsqrtf(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]);
+    const float dir[3] = {dv[0] * dinv, dv[1] * dinv, dv[2] * dinv};
+    constexpr int NSH = (DEG + 1) * (DEG + 1);
+    float Y[NSH];
+    sh_eval(DEG, dir[0], dir[1], dir[2], Y);
+    float dY[NSH][3];
+    sh_grad(DEG, dir[0], dir[1], dir[2], dY);
+    float gdir[3] = {0.f, 0.f, 0.f};
+    const float* shp = g.sh + 48 * i;
+    float* gsh = out.sh + 48 * i;
+#pragma unroll
+    for (int l = 0; l < NSH; ++l) {
+      float dot = 0.f;
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        gsh[3 * l + ch] += Y[l] * grgb[ch];
+        dot = fmaf(__ldg(shp + 3 * l + ch), grgb[ch], dot);
+      }
+#pragma unroll
+      for (int k = 0; k < 3; ++k) gdir[k] = fmaf(dY[l][k], dot, gdir[k]);
+    }
+    const float dd = dir[0] * gdir[0] + dir[1] * gdir[1] + dir[2] * gdir[2];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dmu[k] += (gdir[k] - dir[k] * dd) * dinv;
+  }
+
+  // conic Q = P^-1 (P = Sigma2D):  dL/dP = -Q Gm Q,  Gm = [[gA, gB/2],[gB/2, gC]]
+  const float idet = 1.0f / G.det;
+  const float A = G.c * idet, B = -G.b * idet, C = G.a * idet;
+  const float hB = 0.5f * gB;
+  const float qg00 = A * gA + B * hB, qg01 = A * hB + B * gC;
+  const float qg10 = B * gA + C * hB, qg11 = B * hB + C * gC;
+  const float p00 = -(qg00 * A + qg01 * B), p01 = -(qg00 * B + qg01 * C);
+  const float p11 = -(qg10 * B + qg11 * C);   // symmetric: p10 == p01
+  // P = N N^T + dI, N = Tm Mm:  dL/dN = 2 Gc N;   dL/dTm = dL/dN Mm^T;  dL/dMm = Tm^T dL/dN
+  float dN[6];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    dN[c] = 2.f * (p00 * G.N[c] + p01 * G.N[3 + c]);
+    dN[3 + c] = 2.f * (p01 * G.N[c] + p11 * G.N[3 + c]);
+  }
+  float dTm[6], dMm[9];
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+      dTm[3 * r + k] = dN[3 * r] * G.Mm[3 * k] + dN[3 * r + 1] * G.Mm[3 * k + 1] + dN[3 * r + 2] * G.Mm[3 * k + 2];
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dMm[3 * k + c] = G.Tm[k] * dN[c] + G.Tm[3 + k] * dN[3 + c];
+  // Tm = J W:  dL/dJ = dL/dTm W^T.  J = [[fx/z, 0, -fx Lx/z],[0, fy/z, -fy Ly/z]]
+  const float dJ00 = dTm[0] * cam.R[0] + dTm[1] * cam.R[1] + dTm[2] * cam.R[2];
+  const float dJ02 = dTm[0] * cam.R[6] + dTm[1] * cam.R[7] + dTm[2] * cam.R[8];
+  const float dJ11 = dTm[3] * cam.R[3] + dTm[4] * cam.R[4] + dTm[5] * cam.R[5];
+  const float dJ12 = dTm[3] * cam.R[6] + dTm[4] * cam.R[7] + dTm[5] * cam.R[8];
+  const float z = G.p[2], iz = 1.f / z, iz2 = iz * iz;
+  float dp[3] = {0.f, 0.f, 0.f};
+  dp[2] += -cam.fx * iz2 * dJ00 - cam.fy * iz2 * dJ11;
+  // J02 = -fx Lx / z with Lx = clamp(x/z): inside the clamp Lx = x/z -> J02 = -fx x / z^2
+  if (!G.clx) { dp[0] += -cam.fx * iz2 * dJ02; dp[2] += 2.f * cam.fx * G.p[0] * iz2 * iz * dJ02; }
+  else        { dp[2] += cam.fx * G.Lx * iz2 * dJ02; }
+  if (!G.cly) { dp[1] += -cam.fy * iz2 * dJ12; dp[2] += 2.f * cam.fy * G.p[1] * iz2 * iz * dJ12; }
+  else        { dp[2] += cam.fy * G.Ly * iz2 * dJ12; }
+  // 2-D mean
+  dp[0] += cam.fx * iz * gu;
+  dp[1] += cam.fy * iz * gv;
+  dp[2] += -(cam.fx * G.p[0] * gu + cam.fy * G.p[1] * gv) * iz2;
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    dmu[k] += cam.R[k] * dp[0] + cam.R[3 + k] * dp[1] + cam.R[6 + k] * dp[2];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) out.mean[3 * i + k] += dmu[k];
+
+  // Mm = Rot diag(s)
+  float dRot[9];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    float ds = 0.f;
+#pragma unroll
+    for (int r = 0; r < 3; ++r) { ds = fmaf(G.Rot[3 * r + c], dMm[3 * r + c], ds); dRot[3 * r + c] = G.s[c] * dMm[3 * r + c]; }
+    out.log_scale[3 * i + c] += G.s[c] * ds;
+  }
+  // Rot(q_hat) then the normalisation q_hat = q/|q|
+  const float w = G.qh[0], x = G.qh[1], y = G.qh[2], zq = G.qh[3];
+  float gq[4];
+  gq[0] = 2.f * (-zq * dRot[1] + y * dRot[2] + zq * dRot[3] - x * dRot[5] - y * dRot[6] + x * dRot[7]);
+  gq[1] = 2.f * (y * dRot[1] + zq * dRot[2] + y * dRot[3] - 2.f * x * dRot[4] - w * dRot[5] + zq * dRot[6] + w * dRot[7] - 2.f * x * dRot[8]);
+  gq[2] = 2.f * (-2.f * y * dRot[0] + x * dRot[1] + w * dRot[2] + x * dRot[3] + zq * dRot[5] - w * dRot[6] + zq * dRot[7] - 2.f * y * dRot[8]);
+  gq[3] = 2.f * (-2.f * zq * dRot[0] - w * dRot[1] + x * dRot[2] + w * dRot[3] - 2.f * zq * dRot[4] + y * dRot[5] + x * dRot[6] + y * dRot[7]);
+  const float qd = w * gq[0] + x * gq[1] + y * gq[2] + zq * gq[3];
+  const float iqn = 1.f / G.qn;
+  float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
+  float4 cur = *oq;
+  cur.x += (gq[0] - w * qd) * iqn; cur.y += (gq[1] - x * qd) * iqn;
+  cur.z += (gq[2] - y * qd) * iqn; cur.w += (gq[3] - zq * qd) * iqn;
+  *oq = cur;
+}
+
+}  // namespace
+
+int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, int deg,
+                       const splx_projected* out) {
+  if (g->n == 0) return SPLX_OK;
+  const unsigned grid = (unsigned)((g->n + PROJ_THREADS - 1) / PROJ_THREADS);
+  switch (deg) {
+    case 0: k_project_fwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
+    case 1: k_project_fwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
+    case 2: k_project_fwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
+    default: k_project_fwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
+  }
+  SPLX_LAUNCH_CHECK(ctx, "k_project_fwd");
+  return SPLX_OK;
+}
+
+int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, int deg,
+                       const splx_projected* pr, float* g2d, int clear_g2d,
+                       const splx_gaussian_grads* grads) {
+  if (g->n == 0) return SPLX_OK;
+  const unsigned grid = (unsigned)((g->n + PROJ_THREADS - 1) / PROJ_THREADS);
+  switch (deg) {
+    case 0: k_project_bwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
+    case 1: k_project_bwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
+    case 2: k_project_bwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
+    default: k_project_bwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
+  }
+  SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
+  return SPLX_OK;
+}

@@ -1,0 +1,412 @@
+// sort.cu -- steps a2-a4: tile-intersection keys, stable radix sort, per-tile ranges.
+// PAPER.md L81 ("3D Gaussians are sorted based on their distance from the camera, i.e., depth
+// d"), L165 (each rank blends "in depth order").  Mechanism: 64-bit key =
+// (slot << 32) | float_bits(depth), slot = partition * tiles + tile; result = the STABLE sort
+// of the (key, Gaussian index) pairs emitted in Gaussian-index order.
+//
+// B200 design: the full sort is split so that the wide keys are moved as little as possible.
+//   1. compact the visible Gaussians in index order            (4 B read, 8 B written / visible)
+//   2. stable LSD radix sort of (depth bits, index), 4 x 8 bits (over N_visible, not over M)
+//   3. exclusive scan of tiles_touched in that depth order, emit the 64-bit keys in that order
+//   4. stable LSD radix sort on the SLOT bits only (ceil(log2(K*tiles)) bits, 2-3 passes)
+//   5. tile ranges from the sorted keys
+// Step 2 + step 4 give exactly the stable sort on the whole key: within a slot the entries
+// keep the order of step 2 = (depth bits, index).  No host synchronisation: the counts
+// (N_visible, M) stay on the device and every grid is sized from the caller's capacities.
+#include "common.cuh"
+
+namespace {
+
+constexpr int SCAN_THREADS = 512, SCAN_IPT = 8, SCAN_TILE = SCAN_THREADS * SCAN_IPT;    // 4096
+constexpr int RS_THREADS = 256, RS_IPT = 16, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 4096
+
+struct Counters {   // device-resident counts, written by kernels, read by later kernels
+  uint64_t n_visible;
+  uint64_t m_total;     // true number of intersections
+  uint64_t m_sorted;    // min(m_total, capacity)
+  uint64_t scratch;
+};
+
+struct PartOffs { int64_t off[SPLX_MAX_K + 1]; int K; };
+
+// ---------------------------------------------------------------- generic exclusive scan --
+// Three phases over tiles of 4096 values: per-tile sums, scan of the sums (one block), apply.
+// Op supplies load(i) and store(i, value, exclusive_prefix); n is read from device memory.
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* smem /*>=32*/, uint32_t& total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) smem[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    uint32_t w = lane < nw ? smem[lane] : 0, wi = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, wi, o); if (lane >= o) wi += t; }
+    smem[lane] = wi - w;           // exclusive warp offsets
+    if (lane == 31) smem[32] = wi;  // block total
+  }
+  __syncthreads();
+  const uint32_t res = inc - v + smem[warp];
+  total = smem[32];
+  __syncthreads();
+  return res;
+}
+
+template <class Op>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(Op op, const uint64_t* n_ptr, uint32_t* sums) {
+  __shared__ uint32_t sm[33];
+  const uint64_t n = op.count(n_ptr);
+  const uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
+  uint32_t s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_IPT; ++k) if (base + k < n) s += op.load(base + k);
+  uint32_t total;
+  block_exclusive_scan(s, sm, total);
+  if (threadIdx.x == 0) sums[blockIdx.x] = total;
+}
+
+// one block: exclusive scan of sums[0..nb) in place; *total_out = grand total
+__global__ void __launch_bounds__(1024) k_scan_sums(uint32_t* sums, uint32_t nb, uint64_t* total_out,
+                                                    uint64_t* clamp_out, uint64_t clamp_to) {
+  __shared__ uint32_t sm[33];
+  uint32_t carry = 0;
+  for (uint32_t start = 0; start < nb; start += 1024) {
+    const uint32_t i = start + threadIdx.x;
+    const uint32_t v = i < nb ? sums[i] : 0;
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(v, sm, total);
+    if (i < nb) sums[i] = carry + ex;
+    carry += total;
+  }
+  if (threadIdx.x == 0) {
+    if (total_out) *total_out = carry;
+    if (clamp_out) *clamp_out = carry < clamp_to ? carry : clamp_to;
+  }
+}
+
+template <class Op>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(Op op, const uint64_t* n_ptr, const uint32_t* sums) {
+  __shared__ uint32_t sm[33];
+  const uint64_t n = op.count(n_ptr);
+  if ((uint64_t)blockIdx.x * SCAN_TILE >= n) return;
+  const uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
+  uint32_t v[SCAN_IPT], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(base + k) : 0; s += v[k]; }
+  uint32_t total;
+  uint32_t ex = block_exclusive_scan(s, sm, total) + sums[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex); ex += v[k]; }
+}
+
+struct PlainOp {   // in-place exclusive scan of a u32 array of fixed length
+  uint32_t* data; uint64_t n;
+  __device__ uint64_t count(const uint64_t*) const { return n; }
+  __device__ uint32_t load(uint64_t i) const { return data[i]; }
+  __device__ void store(uint64_t i, uint32_t, uint32_t ex) const { data[i] = ex; }
+};
+struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order preserved
+  const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n;
+  __device__ uint64_t count(const uint64_t*) const { return n; }
+  __device__ uint32_t load(uint64_t i) const { return tiles_touched[i] > 0 ? 1u : 0u; }
+  __device__ void store(uint64_t i, uint32_t v, uint32_t ex) const {
+    if (v) { ckeys[ex] = __float_as_uint(depth[i]); cvals[ex] = (uint32_t)i; }
+  }
+};
+struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, depth order
+  const uint32_t* tiles_touched; const uint32_t* cvals; uint32_t* offs;
+  __device__ uint64_t count(const uint64_t* n_ptr) const { return *n_ptr; }
+  __device__ uint32_t load(uint64_t j) const { return tiles_touched[cvals[j]]; }
+  __device__ void store(uint64_t j, uint32_t, uint32_t ex) const { offs[j] = ex; }
+};
+
+template <class Op>
+int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_ptr, uint32_t* sums,
+                   uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to) {
+  const uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
+  if (nb == 0) return SPLX_OK;
+  k_scan_reduce<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, sums);
+  SPLX_LAUNCH_CHECK(ctx, "k_scan_reduce");
+  k_scan_sums<<<1, 1024, 0, ctx->stream>>>(sums, nb, total_out, clamp_out, clamp_to);
+  SPLX_LAUNCH_CHECK(ctx, "k_scan_sums");
+  k_scan_apply<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, sums);
+  SPLX_LAUNCH_CHECK(ctx, "k_scan_apply");
+  return SPLX_OK;
+}
+
+// ---------------------------------------------------------------------- LSD radix sort --
+// One pass = per-block digit histogram -> exclusive scan over [digit][block] -> stable scatter.
+// Block b always owns positions [b*4096, (b+1)*4096) of the current input buffer.
+
+template <typename KeyT>
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_hist(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t* __restrict__ ghist,
+             int shift, int bits, uint32_t nblocks) {
+  __shared__ uint32_t hist[256];
+  const uint64_t n = *n_ptr;
+  const uint32_t radix = 1u << bits, mask = radix - 1;
+  hist[threadIdx.x] = 0;
+  __syncthreads();
+  const uint64_t start = (uint64_t)blockIdx.x * RS_TILE;
+  if (start < n) {
+    const int lane = threadIdx.x & 31;
+#pragma unroll 4
+    for (int it = 0; it < RS_IPT; ++it) {
+      const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
+      const bool valid = idx < n;
+      const unsigned vm = __ballot_sync(0xffffffffu, valid);
+      if (valid) {
+        const uint32_t d = (uint32_t)(keys[idx] >> shift) & mask;
+        const unsigned peers = __match_any_sync(vm, d);   // aggregate equal digits in the warp
+        if (lane == __ffs(peers) - 1) atomicAdd(&hist[d], __popc(peers));
+      }
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < radix) ghist[(uint64_t)threadIdx.x * nblocks + blockIdx.x] = hist[threadIdx.x];
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_scatter(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
+                uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ gbase,
+                int shift, int bits, uint32_t nblocks) {
+  __shared__ uint32_t whist[RS_WARPS][256];
+  __shared__ uint32_t dbase[256];
+  const uint64_t n = *n_ptr;
+  const uint64_t start = (uint64_t)blockIdx.x * RS_TILE;
+  if (start >= n) return;
+  const uint32_t radix = 1u << bits, mask = radix - 1;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int w = 0; w < RS_WARPS; ++w) whist[w][threadIdx.x] = 0;
+  if (threadIdx.x < radix) dbase[threadIdx.x] = gbase[(uint64_t)threadIdx.x * nblocks + blockIdx.x];
+  __syncthreads();
+  // warp w owns the contiguous segment [start + w*512, +512); iteration `it` covers 32 consecutive
+  // positions, so (it, lane) is the input order and the ranks below are stable.
+  const uint64_t seg = start + (uint64_t)warp * (32 * RS_IPT);
+  KeyT key[RS_IPT];
+  uint32_t rank[RS_IPT];
+  const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    const uint64_t idx = seg + (uint64_t)it * 32 + lane;
+    const bool valid = idx < n;
+    const unsigned vm = __ballot_sync(0xffffffffu, valid);
+    key[it] = 0; rank[it] = 0;
+    if (valid) {
+      key[it] = kin[idx];
+      const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
+      const unsigned peers = __match_any_sync(vm, d);
+      const int leader = __ffs(peers) - 1;
+      uint32_t old = 0;
+      if (lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
+      old = __shfl_sync(peers, old, leader);
+      rank[it] = old + __popc(peers & lt);
+    }
+    __syncwarp();
+  }
+  __syncthreads();
+  {  // exclusive prefix over the warps, per digit
+    const int d = threadIdx.x;
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    const uint64_t idx = seg + (uint64_t)it * 32 + lane;
+    if (idx < n) {
+      const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
+      const uint32_t pos = dbase[d] + whist[warp][d] + rank[it];
+      kout[pos] = key[it];
+      vout[pos] = vin[idx];
+    }
+  }
+}
+
+// Sorts bits [begin_bit, end_bit) in passes of <= 8 bits.  Input in (ka, va); buffers alternate;
+// returns the number of passes (result is in (ka, va) if even, (kb, vb) if odd).
+static int radix_passes(int begin_bit, int end_bit) { return (end_bit - begin_bit + 7) / 8; }
+
+template <typename KeyT>
+int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
+               const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* hist, uint32_t* sums) {
+  const uint32_t nblocks = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
+  if (nblocks == 0) return SPLX_OK;
+  const int passes = radix_passes(begin_bit, end_bit);
+  const int total = end_bit - begin_bit;
+  int shift = begin_bit;
+  for (int p = 0; p < passes; ++p) {
+    const int bits = (total + passes - 1 - p) / passes;  // spread the bits evenly over the passes
+    k_radix_hist<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, hist, shift, bits, nblocks);
+    SPLX_LAUNCH_CHECK(ctx, "k_radix_hist");
+    PlainOp op{hist, (uint64_t)nblocks << bits};
+    int rc = scan_exclusive(ctx, op, op.n, nullptr, sums, nullptr, nullptr, 0);
+    if (rc) return rc;
+    k_radix_scatter<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, hist, shift, bits, nblocks);
+    SPLX_LAUNCH_CHECK(ctx, "k_radix_scatter");
+    shift += bits;
+    KeyT* tk = ka; ka = kb; kb = tk;
+    uint32_t* tv = va; va = vb; vb = tv;
+  }
+  return SPLX_OK;
+}
+
+// ------------------------------------------------------------------------- key emission --
+__global__ void __launch_bounds__(256)
+k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
+            const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
+            const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
+            uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  const uint64_t nvis = cnt->n_visible;
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  int x0 = 0, y0 = 0, w = 0, tt = 0;
+  uint32_t i = 0, o = 0, dbits = 0, slot0 = 0;
+  if (j < nvis) {
+    i = cvals[j]; dbits = ckeys[j]; o = offs[j];
+    const float2 m = *reinterpret_cast<const float2*>(means2d + 2 * (uint64_t)i);
+    int x1, y1;
+    tile_rect(m.x, m.y, radius[i], TX, TY, x0, y0, x1, y1);
+    w = x1 - x0; tt = w * (y1 - y0);
+    int lo = 0, hi = parts.K - 1;  // partition of Gaussian i: last k with off[k] <= i
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (parts.off[mid] <= (int64_t)i) lo = mid; else hi = mid - 1;
+    }
+    slot0 = (uint32_t)lo * (uint32_t)(TX * TY);
+  }
+  const bool big = tt > 32;
+  if (!big) {
+    for (int t = 0; t < tt; ++t) {
+      const uint64_t pos = (uint64_t)o + t;
+      if (pos < capacity) {
+        const uint32_t slot = slot0 + (uint32_t)((y0 + t / w) * TX + x0 + t % w);
+        keys[pos] = ((uint64_t)slot << 32) | dbits;
+        vals[pos] = i;
+      }
+    }
+  }
+  // footprints covering many tiles are emitted by the whole warp (coalesced, no long serial tail)
+  unsigned bm = __ballot_sync(0xffffffffu, big);
+  while (bm) {
+    const int src = __ffs(bm) - 1;
+    bm &= bm - 1;
+    const int sx0 = __shfl_sync(0xffffffffu, x0, src), sy0 = __shfl_sync(0xffffffffu, y0, src);
+    const int sw = __shfl_sync(0xffffffffu, w, src), stt = __shfl_sync(0xffffffffu, tt, src);
+    const uint32_t so = __shfl_sync(0xffffffffu, o, src), si = __shfl_sync(0xffffffffu, i, src);
+    const uint32_t sd = __shfl_sync(0xffffffffu, dbits, src), ss = __shfl_sync(0xffffffffu, slot0, src);
+    for (int t = lane; t < stt; t += 32) {
+      const uint64_t pos = (uint64_t)so + t;
+      if (pos < capacity) {
+        const uint32_t slot = ss + (uint32_t)((sy0 + t / sw) * TX + sx0 + t % sw);
+        keys[pos] = ((uint64_t)slot << 32) | sd;
+        vals[pos] = si;
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, uint32_t* __restrict__ ranges) {
+  const uint64_t m = cnt->m_sorted;
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= m) return;
+  const uint32_t s = (uint32_t)(keys[j] >> 32);
+  if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
+  if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
+}
+
+__global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_total; }
+
+struct Layout {
+  size_t counters, ckeys_a, cvals_a, ckeys_b, cvals_b, offs, keys_tmp, vals_tmp, hist, sums, total;
+};
+
+static int slot_bits(int K, int TX, int TY) {
+  const uint64_t slots = (uint64_t)K * TX * TY;
+  int b = 1;
+  while (((uint64_t)1 << b) < slots) ++b;
+  return b;
+}
+
+static Layout make_layout(int64_t n, uint64_t capacity) {
+  Layout L;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  L.counters = take(sizeof(Counters));
+  L.ckeys_a = take((size_t)n * 4); L.cvals_a = take((size_t)n * 4);
+  L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
+  L.offs = take((size_t)n * 4);
+  L.keys_tmp = take((size_t)capacity * 8); L.vals_tmp = take((size_t)capacity * 4);
+  const uint64_t big = (uint64_t)n > capacity ? (uint64_t)n : capacity;
+  const uint64_t nblocks = (big + RS_TILE - 1) / RS_TILE;
+  L.hist = take((size_t)nblocks * 256 * 4);
+  const uint64_t scan_len = nblocks * 256 > big ? nblocks * 256 : big;
+  L.sums = take(((size_t)(scan_len + SCAN_TILE - 1) / SCAN_TILE + 1) * 4);
+  L.total = off;
+  return L;
+}
+
+}  // namespace
+
+size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY) {
+  (void)K; (void)TX; (void)TY;
+  return make_layout(n, capacity).total;
+}
+
+int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, const int64_t* part_offsets,
+                    const CamDev& cam, const splx_binning* out, void* ws, size_t ws_bytes) {
+  const Layout L = make_layout(n, out->capacity);
+  if (ws_bytes < L.total)
+    SPLX_FAIL(ctx, SPLX_ERR_WORKSPACE, "splx_bin_sort: workspace %zu B < required %zu B", ws_bytes, L.total);
+  char* base = (char*)ws;
+  Counters* cnt = (Counters*)(base + L.counters);
+  uint32_t* ckeys_a = (uint32_t*)(base + L.ckeys_a); uint32_t* cvals_a = (uint32_t*)(base + L.cvals_a);
+  uint32_t* ckeys_b = (uint32_t*)(base + L.ckeys_b); uint32_t* cvals_b = (uint32_t*)(base + L.cvals_b);
+  uint32_t* offs = (uint32_t*)(base + L.offs);
+  uint64_t* keys_tmp = (uint64_t*)(base + L.keys_tmp); uint32_t* vals_tmp = (uint32_t*)(base + L.vals_tmp);
+  uint32_t* hist = (uint32_t*)(base + L.hist); uint32_t* sums = (uint32_t*)(base + L.sums);
+  const int ntiles = cam.TX * cam.TY;
+
+  SPLX_CUDA_OK(ctx, cudaMemsetAsync(cnt, 0, sizeof(Counters), ctx->stream));
+  SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->tile_ranges, 0, (size_t)K * ntiles * 2 * sizeof(uint32_t), ctx->stream));
+  if (n == 0 || out->capacity == 0) {
+    k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
+    SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
+    return SPLX_OK;
+  }
+  int rc;
+  // 1. visible Gaussians, index order
+  VisibleOp vop{pr->tiles_touched, pr->depth, ckeys_a, cvals_a, (uint64_t)n};
+  if ((rc = scan_exclusive(ctx, vop, (uint64_t)n, nullptr, sums, &cnt->n_visible, nullptr, 0))) return rc;
+  // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers)
+  if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n, &cnt->n_visible, 0, 32, hist, sums))) return rc;
+  // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
+  TouchedOp top{pr->tiles_touched, cvals_a, offs};
+  if ((rc = scan_exclusive(ctx, top, (uint64_t)n, &cnt->n_visible, sums, &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
+  const int sbits = slot_bits(K, cam.TX, cam.TY);
+  const int passes = radix_passes(32, 32 + sbits);
+  uint64_t* k0 = (passes & 1) ? keys_tmp : out->keys;   // so that the last pass lands in out->keys
+  uint32_t* v0 = (passes & 1) ? vals_tmp : out->vals;
+  uint64_t* k1 = (passes & 1) ? out->keys : keys_tmp;
+  uint32_t* v1 = (passes & 1) ? out->vals : vals_tmp;
+  PartOffs parts;
+  parts.K = K;
+  for (int k = 0; k <= K; ++k) parts.off[k] = part_offsets[k];
+  k_emit_keys<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(
+      pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0);
+  SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
+  // 4. stable sort on the slot bits
+  if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits, hist, sums))) return rc;
+  // 5. ranges
+  k_tile_ranges<<<(unsigned)((out->capacity + 255) / 256), 256, 0, ctx->stream>>>(out->keys, cnt, out->tile_ranges);
+  SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
+  k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
+  SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
+  return SPLX_OK;
+}

@@ -1,0 +1,80 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol
+include/splx.h declares; the product path fails loudly without a CUDA device; the product
+package never imports the oracle."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2606_18588_b200 import build
+    return build.build()
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "splx.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(splx_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    names = _declared()
+    assert len(names) >= 18 and "splx_project" in names and "splx_adam" in names
+    L = ctypes.CDLL(libpath)
+    for n in names:
+        assert hasattr(L, n), n
+    from paper_2606_18588_b200 import binding
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_binding_mirrors_the_abi_names():
+    from paper_2606_18588_b200 import binding
+    for n in _declared():
+        short = n[len("splx_"):]
+        if short in ("create", "destroy", "last_error"):
+            continue
+        assert hasattr(binding.Context, short), short
+
+
+def test_struct_sizes_match_the_header(libpath):
+    from paper_2606_18588_b200 import binding as b
+    assert ctypes.sizeof(b.Config) == 24
+    assert ctypes.sizeof(b.CameraS) == 4 * (9 + 3 + 4) + 8 + 4
+    assert ctypes.sizeof(b.GaussiansS) == 48 and ctypes.sizeof(b.ProjectedS) == 56
+    assert ctypes.sizeof(b.BinningS) == 40 and ctypes.sizeof(b.PartialS) == 24
+
+
+def test_no_cpu_fallback_without_a_device(libpath):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    from paper_2606_18588_b200 import binding
+    with pytest.raises(binding.SplxError) as e:
+        binding.Context(0)
+    assert "no CPU fallback" in str(e.value) or "no CUDA device" in str(e.value)
+    # and straight through the C ABI
+    L = binding.lib()
+    h = ctypes.c_void_p()
+    rc = L.splx_create(ctypes.byref(h), 0, None, None)
+    assert rc == binding.ERR_CUDA and not h.value
+    assert b"no CUDA device" in L.splx_last_error(None)
+
+
+def test_product_package_never_touches_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_18588_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "liboracle" not in txt and "splx_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_2606_18588_b200\b", txt, flags=re.M), f
+            assert "libsplx" not in txt
