@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the hot path of BASELINE.json on N B200s (replicas only).
+
+A "step" is one pass of the whole hot path over one view of the
+workload: project -> bin/sort -> render K partials -> compose -> L1 grad -> compose bwd ->
+raster bwd -> project bwd -> Adam.  Workload at N=1: BASELINE.json configs[1] (1M Gaussians, SH3,
+1920x1080, K=4 partitions, 2x2 xy grid), synthetic and seeded.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fwd+compose+bwd+adam Mpixels/s (train iteration)"
+UNIT = "Mpixels/s"
+
+# Algorithmic FP32 work of the blend loops, flops per pair (FMA = 2)
+FLOPS_EVAL = 16      # alpha evaluation of one (pixel, Gaussian) pair: Eq.1 + the skip tests
+FLOPS_BLEND_FWD = 12  # one contributing pair in the forward: Eq.3-4 accumulation
+FLOPS_BLEND_BWD = 55  # one contributing pair in the backward incl. its 9 reduction adds
+FP32_LANES_PER_SM = 128
+SM_COUNT = 148
+
+
+def workload(name):
+    from paper_2606_18588_b200 import scenes
+    if name == "aerial_1M":
+        return scenes.aerial()                       # BASELINE configs[1]
+    if name == "tiny":
+        return scenes.tiny()                         # configs[0]
+    if name == "aerial_small":
+        return scenes.small_aerial()
+    raise SystemExit(f"unknown workload {name}")
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (profiling recipe)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-i", str(index), "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+        self.marks = []
+
+    def mark(self):
+        self.marks.append(time.time())
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.p is None:
+            return out
+        time.sleep(0.12)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = []
+        for line in open(self.f.name):
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 8:
+                continue
+            try:
+                ts = time.mktime(time.strptime(parts[0].split(".")[0], "%Y/%m/%d %H:%M:%S")) + float("0." + parts[0].split(".")[1])
+                rows.append((ts, float(parts[1]), float(parts[2]), parts[4:8]))
+            except Exception:
+                continue
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        lo, hi = (self.marks + [0, 1e18])[:2] if len(self.marks) >= 2 else (0, 1e18)
+        sel = [r for r in rows if lo - 0.05 <= r[0] <= hi + 0.05] or rows
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in sel for i in range(4) if r[3][i].lower().startswith("active")})
+        out.update(sm_mhz=statistics.median(r[1] for r in sel), sm_max_mhz=max(r[2] for r in sel), reasons=reasons,
+                   samples=len(sel))
+        return out
+
+
+# ------------------------------------------------------------------------------- CPU oracle --
+def oracle_sample(sc, n_tiles=96, seed=5):
+    """Time the oracle, as it stands, on a bounded sample of the workload: whole-frame stages
+    (projection, binning, projection backward) on all N Gaussians, per-pixel stages (render, compose,
+    their backwards) on `n_tiles` random tiles, Adam on a 1M-parameter slice; extrapolated to one frame."""
+    import oracle
+    oracle.build()
+    cam = sc.cameras[0]
+    camv = cam.as_array()
+    W, H = cam.width, cam.height
+    TX, TY = (W + 15) // 16, (H + 15) // 16
+    rng = np.random.default_rng(seed)
+    tiles = np.sort(rng.choice(TX * TY, size=min(n_tiles, TX * TY), replace=False)).astype(np.int32)
+    parts = sc.partitions()
+    t = {}
+    t0 = time.perf_counter()
+    proj = [oracle.project(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sc.sh_degree, camv)
+            for p in parts]
+    t["project"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    bins = [oracle.bin_sort(pr.means2d, pr.radius, pr.depth, W, H) for pr in proj]
+    t["bin_sort"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    pas = [oracle.render_partial(pr.means2d, pr.conic_opacity, pr.rgb, pr.depth, b.vals, b.ranges, W, H,
+                                 tile_list=tiles) for pr, b in zip(proj, bins)]
+    ct = np.stack([pa.ct for pa in pas]); d = np.stack([pa.d for pa in pas])
+    img, Tt, _, _ = oracle.compose(ct, d, sc.bg, tiles)
+    _, g_img = oracle.l1(img, sc.targets[0])
+    g_ct = oracle.compose_bwd(ct, d, g_img, sc.bg, None, tiles)
+    g2 = [oracle.raster_bwd(pr.means2d, pr.conic_opacity, pr.rgb, b.vals, b.ranges, W, H, g_ct[k], tile_list=tiles)
+          for k, (pr, b) in enumerate(zip(proj, bins))]
+    t["tiles"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    for p, pr, g in zip(parts, proj, g2):
+        oracle.project_bwd(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sc.sh_degree, camv,
+                           pr.radius, pr.clamp, *g)
+    t["project_bwd"] = time.perf_counter() - t0
+    na = 1_000_000
+    pp = np.zeros(na); mm = np.zeros(na); vv = np.zeros(na); gg = rng.standard_normal(na)
+    t0 = time.perf_counter()
+    oracle.adam(pp, gg, mm, vv, 1e-3, step=1)
+    t["adam_1M"] = time.perf_counter() - t0
+    frac = len(tiles) / (TX * TY)
+    frame_s = t["project"] + t["bin_sort"] + t["project_bwd"] + t["tiles"] / frac + t["adam_1M"] * (59 * sc.N / na)
+    walked = sum(pa.walked for pa in pas)
+    return dict(frame_s=frame_s, spent_s=sum(t.values()), stages=t, tiles=len(tiles), total_tiles=TX * TY,
+                walked_sample=int(walked))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sc = workload(args.workload)
+    cam = sc.cameras[0]
+    n_tiles = 600
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        oracle_sample(sc, n_tiles=8)
+    times = []
+    for s in range(args.steps):
+        times.append(oracle_sample(sc, n_tiles=n_tiles, seed=5 + s))
+    frame_s = statistics.mean(x["frame_s"] for x in times)
+    mpix = cam.width * cam.height / frame_s / 1e6
+    sample = (f"per step: projection/binning/projection-backward on all {sc.N} Gaussians, render+compose+backward on "
+              f"{n_tiles} random tiles of {times[0]['total_tiles']} (extrapolated by tile count), Adam on a 1M-parameter "
+              f"slice (extrapolated to 59N)")
+    line = dict(metric=METRIC, value=mpix, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=frame_s * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference",
+                config=dict(workload=args.workload, gaussians=sc.N, K=sc.K, width=cam.width, height=cam.height,
+                            sh_degree=sc.sh_degree, views_per_step=1),
+                cpu_baseline=dict(value=mpix, unit=UNIT, cores=1, kind="oracle", sample=sample),
+                e2e=dict(value=mpix, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------- CUDA path --
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_18588_b200.engine import Trainer
+    from paper_2606_18588_b200.scenes import PARAM_KEYS
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    sc = workload(args.workload)
+    cam = sc.cameras[0]
+    W, H = cam.width, cam.height
+    cap = {"aerial_1M": 6_000_000}.get(args.workload)
+    tr = Trainer(sc.params, sc.part_offsets, W, H, sc.sh_degree, sc.bg, capacity=cap, device=local)
+    c = tr.ctx
+    target = torch.from_numpy(sc.targets[0]).cuda()
+    tr._workspaces(cam); tr._cam = cam
+    K = tr.K
+    g_ct = torch.empty((K, H, W, 4), dtype=torch.float32, device="cuda")
+    g2d = torch.zeros((tr.n, 12), dtype=torch.float32, device="cuda")
+    STAGES = ["project", "bin_sort", "render_partial", "compose", "l1_loss_grad", "compose_backward",
+              "raster_backward", "project_backward", "adam"]
+
+    def step(ev=None):
+        def rec(i):
+            if ev is not None:
+                ev[i].record()
+        rec(0); c.project(tr.params, cam, tr.sh_degree, tr.proj)
+        rec(1); c.bin_sort(tr.proj, K, tr.part_offsets, cam, tr.bins, tr._ws_sort)
+        rec(2); c.render_partial(tr.proj, tr.bins, K, cam, tr.partials)
+        rec(3); c.compose(K, tr.partials, cam, tr.bg, tr.image, tr.T_total)
+        rec(4); c.l1_loss_grad(tr.image, target, tr.g_image, tr.loss_sum)
+        rec(5); c.compose_backward(K, tr.partials, cam, tr.bg, tr.g_image, None, g_ct)
+        rec(6); c.raster_backward(tr.proj, tr.bins, K, cam, tr.partials, g_ct, g2d)
+        rec(7); c.project_backward(tr.params, cam, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True)
+        rec(8); tr.adam_step(1, zero_grad=True)
+        rec(9)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # unit counts of this view (outside the timed region): pair evaluations and intersections
+    tr.pairs.zero_()
+    c.project(tr.params, cam, tr.sh_degree, tr.proj)
+    c.bin_sort(tr.proj, K, tr.part_offsets, cam, tr.bins, tr._ws_sort)
+    c.render_partial(tr.proj, tr.bins, K, cam, tr.partials, tr.pairs)
+    M = tr.num_intersections()
+    pairs_fwd = int(tr.pairs[0].item())
+    pairs_blend = int(tr.pairs[1].item())                          # (pixel, Gaussian) pairs that are blended
+    n_contrib = tr.partials.n_contrib
+    pairs_bwd = int(n_contrib.to(torch.int64).sum().item())       # list entries the backward re-evaluates
+    n_visible = int((tr.proj.radius > 0).sum().item())
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    for _ in range(max(args.warmup, 3)):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(10)] for _ in range(args.steps)]
+    l0 = c.launch_count()
+    barrier()
+    if sampler: sampler.mark()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for s in range(args.steps):
+        step(evs[s])
+    e1.record()
+    barrier()
+    if sampler: sampler.mark()
+    launches = c.launch_count() - l0
+    ms_total = e0.elapsed_time(e1)
+    tmax = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_step = float(tmax.item()) / args.steps
+    stage_ms = {n: statistics.mean(evs[s][i].elapsed_time(evs[s][i + 1]) for s in range(args.steps))
+                for i, n in enumerate(STAGES)}
+    clocks = sampler.stop() if sampler else None
+
+    # end to end through the public API with HOST buffers: the step's input (target image) comes from
+    # pinned host memory, the result (rendered image + loss) goes back to pinned host memory, every step
+    tgt_host = torch.from_numpy(sc.targets[0]).pin_memory()
+    img_host = torch.empty((H, W, 3), dtype=torch.float32).pin_memory()
+    loss_host = torch.empty(1, dtype=torch.float64).pin_memory()
+
+    def step_e2e():
+        target.copy_(tgt_host, non_blocking=True)
+        tr.loss_sum.zero_()
+        step()
+        img_host.copy_(tr.image, non_blocking=True)
+        loss_host.copy_(tr.loss_sum, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    for _ in range(3):
+        step_e2e()
+    barrier()
+    n_e2e = max(3, args.steps // 2)
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        step_e2e()
+    barrier()
+    e2e_ms = torch.tensor([(time.perf_counter() - t0) * 1e3 / n_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
+    e2e_ms = float(e2e_ms.item())
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    mpix = world * W * H / (ms_step * 1e-3) / 1e6
+    # dominant kernel: the rasteriser backward (FP32 issue + shuffles + atomics): algorithmic flops
+    dom = max(stage_ms, key=stage_ms.get)
+    fp32_peak = SM_COUNT * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12   # TFLOP/s
+    flops_bwd = pairs_bwd * FLOPS_EVAL + pairs_blend * FLOPS_BLEND_BWD
+    flops_fwd = pairs_fwd * FLOPS_EVAL + pairs_blend * FLOPS_BLEND_FWD
+    hbm_bytes = dict(project=n_visible * 285 + (tr.n - n_visible) * 93, adam=28 * 59 * tr.n,
+                     compose=(20 * K + 16) * W * H, compose_backward=(12 + 36 * K) * W * H,
+                     project_backward=n_visible * 740, l1_loss_grad=36 * W * H)
+    if dom == "raster_backward":
+        ach = flops_bwd / (stage_ms[dom] * 1e-3) / 1e12
+        roof = dict(kernel="k_raster_bwd", bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak,
+                    traffic=None, peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} clock)")
+    elif dom == "render_partial":
+        ach = flops_fwd / (stage_ms[dom] * 1e-3) / 1e12
+        roof = dict(kernel="k_render_fwd", bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak,
+                    traffic=None, peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} clock)")
+    else:
+        b = hbm_bytes.get(dom, 0)
+        ach = b / (stage_ms[dom] * 1e-3) / 1e9
+        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
+                    traffic=None, peak_source=pk["source"])
+    per_kernel = {}
+    for n, b in hbm_bytes.items():
+        gbs = b / (stage_ms[n] * 1e-3) / 1e9
+        per_kernel[n] = dict(ms=stage_ms[n], algorithmic_GBps=gbs, frac_of_hbm=gbs / pk["hbm_gbs"])
+    per_kernel["render_partial"] = dict(ms=stage_ms["render_partial"], Gpairs_per_s=pairs_fwd / stage_ms["render_partial"] / 1e6,
+                                        algorithmic_TFLOPs=flops_fwd / stage_ms["render_partial"] / 1e9,
+                                        frac_of_fp32=flops_fwd / stage_ms["render_partial"] / 1e9 / fp32_peak)
+    per_kernel["raster_backward"] = dict(ms=stage_ms["raster_backward"], Gpairs_per_s=pairs_bwd / stage_ms["raster_backward"] / 1e6,
+                                         algorithmic_TFLOPs=flops_bwd / stage_ms["raster_backward"] / 1e9,
+                                         frac_of_fp32=flops_bwd / stage_ms["raster_backward"] / 1e9 / fp32_peak)
+    per_kernel["bin_sort"] = dict(ms=stage_ms["bin_sort"], intersections=M)
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        o = oracle_sample(sc, n_tiles=1500)
+        cpu = dict(value=W * H / o["frame_s"] / 1e6, unit=UNIT, cores=1, kind="oracle",
+                   sample=(f"projection/binning/projection-backward on all {sc.N} Gaussians + render/compose/backward on "
+                           f"{o['tiles']} random tiles of {o['total_tiles']} (extrapolated by tile count) + Adam on 1M "
+                           f"parameters (extrapolated to 59N); {o['spent_s']:.1f} s of CPU work"),
+                   ms_per_frame_extrapolated=o["frame_s"] * 1e3)
+
+    line = dict(metric=METRIC, value=mpix, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                data="synthetic",
+                config=dict(workload=args.workload, gaussians=tr.n, K=K, width=W, height=H, sh_degree=sc.sh_degree,
+                            views_per_step=1, parallelism=f"replicas x{world} (one GPU per replica, no collective)",
+                            l2="working set (params+grads+moments 944 MB at 1M) is larger than the 126 MB L2",
+                            intersections=M, visible=n_visible, pairs_fwd=pairs_fwd, pairs_bwd=pairs_bwd,
+                            pairs_blended=pairs_blend),
+                iters_per_s=world * 1e3 / ms_step, stages_ms=stage_ms, per_kernel=per_kernel, roofline=roof,
+                cpu_baseline=cpu, clocks=clocks, gpu_launches=int(launches),
+                e2e=dict(value=world * W * H / (e2e_ms * 1e-3) / 1e6, unit=UNIT, ms_per_step=e2e_ms,
+                         h2d_bytes_per_step=int(tgt_host.numel() * 4),
+                         d2h_bytes_per_step=int(img_host.numel() * 4 + 8)))
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="aerial_1M")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 2 if args.steps is None else min(args.steps, 4)
+        args.warmup = 1 if args.warmup is None else min(args.warmup, 1)
+        run_reference(args)
+    else:
+        args.steps = 50 if args.steps is None else args.steps
+        args.warmup = 5 if args.warmup is None else args.warmup
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

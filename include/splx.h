@@ -140,8 +140,8 @@ int splx_check_capacity(splx_ctx *ctx, const splx_binning *bins, uint64_t *m_hos
 
 /* ---- a5 local render: PAPER.md Eq.1 (L84), Eq.3 (L167), Eq.4 (L172).  Grid = K x tiles,
  * one thread per pixel, the tile's list staged 256 Gaussians at a time in shared memory.
- * pairs (device uint64, may be NULL): += number of list entries walked, summed over pixels
- * (the oracle's unit of work). */
+ * pairs (device uint64[2], may be NULL): pairs[0] += number of list entries walked, summed over
+ * pixels (the oracle's unit of work); pairs[1] += number of (pixel, Gaussian) pairs blended. */
 int splx_render_partial(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins, int K,
                         const splx_camera *cam, const splx_partial *out, uint64_t *pairs);
 

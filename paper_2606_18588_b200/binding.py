@@ -131,7 +131,7 @@ def camera_struct(cam) -> CameraS:
 
 
 def gaussians_struct(p: dict, cls=GaussiansS):
-    n = p["mean"].shape[0]
+    n = p["opacity_logit"].numel()
     for k, w in (("mean", 3), ("log_scale", 3), ("quat", 4), ("opacity_logit", 1), ("sh", 48)):
         assert p[k].dtype == torch.float32 and p[k].numel() == n * w, k
     return cls(_ptr(p["mean"]), _ptr(p["log_scale"]), _ptr(p["quat"]), _ptr(p["opacity_logit"]),

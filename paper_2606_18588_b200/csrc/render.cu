@@ -75,7 +75,7 @@ k_render_fwd(const float* __restrict__ means2d, const float* __restrict__ conic_
   const float px = (float)pxi + 0.5f, py = (float)pyi + 0.5f;
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
   float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
-  uint32_t walked = 0, last = 0;
+  uint32_t walked = 0, last = 0, blended = 0;
   bool done = !inside;
   for (uint32_t start = r0; start < r1; start += BLOCK) {
     if (__syncthreads_count(done) == BLOCK) break;
@@ -98,6 +98,7 @@ k_render_fwd(const float* __restrict__ means2d, const float* __restrict__ conic_
       C0 = fmaf(w, cd.x, C0); C1 = fmaf(w, cd.y, C1); C2 = fmaf(w, cd.z, C2); D = fmaf(w, cd.w, D);
       T = Tn;
       last = walked;
+      ++blended;
     }
   }
   if (inside) {
@@ -107,9 +108,12 @@ k_render_fwd(const float* __restrict__ means2d, const float* __restrict__ conic_
     out_n[pix] = last;
   }
   if (pairs) {
-    uint32_t wsum = inside ? walked : 0;
-    wsum = __reduce_add_sync(0xffffffffu, wsum);
-    if ((threadIdx.x & 31) == 0 && wsum) atomicAdd(pairs, (unsigned long long)wsum);
+    const uint32_t wsum = __reduce_add_sync(0xffffffffu, inside ? walked : 0u);
+    const uint32_t bsum = __reduce_add_sync(0xffffffffu, blended);
+    if ((threadIdx.x & 31) == 0 && wsum) {
+      atomicAdd(pairs, (unsigned long long)wsum);
+      atomicAdd(pairs + 1, (unsigned long long)bsum);
+    }
   }
 }
 
