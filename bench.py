@@ -224,8 +224,8 @@ def run_ours(args):
         rec(4); c.l1_loss_grad(tr.image, target, tr.g_image, tr.loss_sum)
         rec(5); c.compose_backward(K, tr.partials, cam, tr.bg, tr.g_image, None, g_ct)
         rec(6); c.raster_backward(tr.proj, tr.bins, K, cam, tr.partials, g_ct, g2d)
-        rec(7); c.project_backward(tr.params, cam, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True)
-        rec(8); tr.adam_step(1, zero_grad=True)
+        rec(7); c.project_backward(tr.params, cam, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True, overwrite=True)
+        rec(8); tr.adam_step(1)
         rec(9)
 
     def barrier():

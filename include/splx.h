@@ -39,6 +39,7 @@ extern "C" {
 
 #define SPLX_MAX_K 64
 #define SPLX_TILE 16
+#define SPLX_ADAM_MAX_GROUPS 8
 #define SPLX_G2D_STRIDE 12 /* floats per Gaussian in the 2-D gradient buffer, see splx_raster_backward */
 
 typedef struct splx_ctx splx_ctx;
@@ -171,18 +172,25 @@ int splx_raster_backward(splx_ctx *ctx, const splx_projected *proj, const splx_b
                          const float *g_ct, float *g2d);
 
 /* ---- a10 projection backward: exact derivative of splx_project.  Reads
- * g2d, accumulates into grads (+=).  If clear_g2d != 0 the consumed g2d rows are zeroed. */
+ * g2d and accumulates into grads (+=).  flags: SPLX_PB_CLEAR_G2D zeroes the consumed g2d rows
+ * (so the next view can accumulate into g2d again); SPLX_PB_OVERWRITE stores (=) instead of
+ * accumulating: EVERY row of every grads array is written (zeros for culled Gaussians and for
+ * SH coefficients above sh_degree), so the first view of an iteration needs no zeroed
+ * gradient buffer and reads none.  All five grads arrays must be 16-byte aligned. */
+#define SPLX_PB_CLEAR_G2D 1
+#define SPLX_PB_OVERWRITE 2
 int splx_project_backward(splx_ctx *ctx, const splx_gaussians *g, const splx_camera *cam,
-                          int sh_degree, const splx_projected *proj, float *g2d, int clear_g2d,
+                          int sh_degree, const splx_projected *proj, float *g2d, int flags,
                           const splx_gaussian_grads *grads);
 
 /* ---- a8+a9+a10 in one call (BASELINE.json north_star "splx_backward").  ws holds g_ct
- * and g2d; splx_backward_ws_bytes gives its size. */
+ * and g2d; splx_backward_ws_bytes gives its size.  flags: SPLX_PB_OVERWRITE as above (0 = +=). */
 size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera *cam);
 int splx_backward(splx_ctx *ctx, int K, const splx_partial *partials, const splx_camera *cam,
                   const float bg[3], const float *dL_dimage, const float *dL_dT_total,
                   const splx_gaussians *g, const splx_projected *proj, const splx_binning *bins,
-                  int sh_degree, const splx_gaussian_grads *grads, void *ws, size_t ws_bytes);
+                  int sh_degree, const splx_gaussian_grads *grads, void *ws, size_t ws_bytes,
+                  int flags);
 
 /* ---- a11 Adam (paper silent on the optimiser; north_star names Adam).  Dense,
  * bias-corrected, step is 1-based.  grad_scale multiplies grad first (1/B for B views);
@@ -190,6 +198,15 @@ int splx_backward(splx_ctx *ctx, int K, const splx_partial *partials, const splx
 int splx_adam(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int64_t count,
               float lr, float beta1, float beta2, float eps, int step, float grad_scale,
               int zero_grad);
+
+/* The same update for several parameter groups that live back to back in ONE flat buffer
+ * (param/grad/m/v[group_offsets[n_groups]]), in a single launch.  group_offsets: HOST array of
+ * n_groups+1 float offsets, group_offsets[0] == 0, every offset a multiple of 4 (16-byte
+ * vectors never straddle groups); lr: HOST array of n_groups learning rates; 1 <= n_groups <=
+ * SPLX_ADAM_MAX_GROUPS.  Elementwise identical to n_groups calls of splx_adam. */
+int splx_adam_groups(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int n_groups,
+                     const int64_t *group_offsets, const float *lr, float beta1, float beta2,
+                     float eps, int step, float grad_scale, int zero_grad);
 
 #ifdef __cplusplus
 }

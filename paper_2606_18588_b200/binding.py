@@ -19,6 +19,7 @@ _lib = None
 G2D_STRIDE = 12
 TILE = 16
 MAX_K = 64
+PB_CLEAR_G2D, PB_OVERWRITE = 1, 2
 OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA = 0, -1, -2, -3, -4
 
 EXPORTS = [
@@ -26,7 +27,7 @@ EXPORTS = [
     "splx_project", "splx_bin_sort_ws_bytes", "splx_bin_sort", "splx_check_capacity",
     "splx_render_partial", "splx_compose", "splx_l1_loss_grad", "splx_compose_backward",
     "splx_raster_backward", "splx_project_backward", "splx_backward_ws_bytes", "splx_backward",
-    "splx_adam",
+    "splx_adam", "splx_adam_groups",
 ]
 
 
@@ -104,9 +105,12 @@ def lib():
                                             C.c_void_p, C.c_int, C.c_void_p]
         L.splx_backward.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
-                                    C.c_void_p, C.c_size_t]
+                                    C.c_void_p, C.c_size_t, C.c_int]
         L.splx_adam.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64,
                                 C.c_float, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float, C.c_int]
+        L.splx_adam_groups.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                       C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int,
+                                       C.c_float, C.c_int]
         _lib = L
     return _lib
 
@@ -269,29 +273,39 @@ class Context:
         self._check(lib().splx_raster_backward(self._h, C.byref(ps), C.byref(bs), K, C.byref(cs), C.byref(pa),
                                                _ptr(g_ct), _ptr(g2d)))
 
-    def project_backward(self, params: dict, cam, sh_degree, proj: Projected, g2d, grads: dict, clear_g2d=False):
+    def project_backward(self, params: dict, cam, sh_degree, proj: Projected, g2d, grads: dict, clear_g2d=False,
+                         overwrite=False):
         g = gaussians_struct(params)
         gg = gaussians_struct(grads)
         cs = camera_struct(cam)
         ps = proj.struct()
         self._check(lib().splx_project_backward(self._h, C.byref(g), C.byref(cs), sh_degree, C.byref(ps),
-                                                _ptr(g2d), int(clear_g2d), C.byref(gg)))
+                                                _ptr(g2d), (PB_CLEAR_G2D if clear_g2d else 0) | (PB_OVERWRITE if overwrite else 0),
+                                                C.byref(gg)))
 
     def backward_ws_bytes(self, n, K, cam) -> int:
         cs = camera_struct(cam)
         return int(lib().splx_backward_ws_bytes(n, K, C.byref(cs)))
 
     def backward(self, K, partials: Partial, cam, bg, g_image, g_T_total, params: dict, proj: Projected,
-                 bins: Binning, sh_degree, grads: dict, ws: torch.Tensor):
+                 bins: Binning, sh_degree, grads: dict, ws: torch.Tensor, overwrite=False):
         cs = camera_struct(cam)
         b = (C.c_float * 3)(*[float(x) for x in bg])
         pa, ps, bs = partials.struct(), proj.struct(), bins.struct()
         g, gg = gaussians_struct(params), gaussians_struct(grads)
         self._check(lib().splx_backward(self._h, K, C.byref(pa), C.byref(cs), b, _ptr(g_image), _ptr(g_T_total),
                                         C.byref(g), C.byref(ps), C.byref(bs), sh_degree, C.byref(gg),
-                                        _ptr(ws), ws.numel() * ws.element_size()))
+                                        _ptr(ws), ws.numel() * ws.element_size(), PB_OVERWRITE if overwrite else 0))
 
     def adam(self, param, grad, m, v, lr, beta1=0.9, beta2=0.999, eps=1e-15, step=1, grad_scale=1.0,
              zero_grad=False):
         self._check(lib().splx_adam(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), param.numel(), lr,
                                     beta1, beta2, eps, step, grad_scale, int(zero_grad)))
+
+    def adam_groups(self, param, grad, m, v, group_offsets, lrs, beta1=0.9, beta2=0.999, eps=1e-15, step=1,
+                    grad_scale=1.0, zero_grad=False):
+        n = len(lrs)
+        offs = (C.c_int64 * (n + 1))(*[int(x) for x in group_offsets])
+        lr = (C.c_float * n)(*[float(x) for x in lrs])
+        self._check(lib().splx_adam_groups(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, lr,
+                                           beta1, beta2, eps, step, grad_scale, int(zero_grad)))

@@ -45,7 +45,58 @@ k_adam(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ 
   }
 }
 
+// All parameter groups of one flat buffer in ONE launch: the groups differ only in their learning
+// rate; group boundaries are multiples of 4 floats, so a 128-bit vector never straddles two groups.
+struct AdamGroups { long long end4[SPLX_ADAM_MAX_GROUPS]; float lr[SPLX_ADAM_MAX_GROUPS]; int n; };
+
+__global__ void __launch_bounds__(AB)
+k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ m, float* __restrict__ v,
+              int64_t nvec, AdamK k, AdamGroups gr, float gscale, int zero_grad) {
+  for (int64_t i = (int64_t)blockIdx.x * AB + threadIdx.x; i < nvec; i += (int64_t)gridDim.x * AB) {
+    float lr = gr.lr[0];
+#pragma unroll
+    for (int j = 1; j < SPLX_ADAM_MAX_GROUPS; ++j)
+      if (j < gr.n && i >= gr.end4[j - 1]) lr = gr.lr[j];
+    AdamK kk = k; kk.lr = lr;
+    float4 p = reinterpret_cast<float4*>(param)[i];
+    float4 g = reinterpret_cast<const float4*>(grad)[i];
+    float4 mm = reinterpret_cast<float4*>(m)[i];
+    float4 vv = reinterpret_cast<float4*>(v)[i];
+    adam1(p.x, g.x * gscale, mm.x, vv.x, kk);
+    adam1(p.y, g.y * gscale, mm.y, vv.y, kk);
+    adam1(p.z, g.z * gscale, mm.z, vv.z, kk);
+    adam1(p.w, g.w * gscale, mm.w, vv.w, kk);
+    reinterpret_cast<float4*>(param)[i] = p;
+    reinterpret_cast<float4*>(m)[i] = mm;
+    reinterpret_cast<float4*>(v)[i] = vv;
+    if (zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+}
+
 }  // namespace
+
+int launch_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int n_groups,
+                       const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
+                       float grad_scale, int zero_grad) {
+  const int64_t count = group_offsets[n_groups];
+  if (count <= 0) return SPLX_OK;
+  const double bc1 = 1.0 - pow((double)beta1, step), bc2 = 1.0 - pow((double)beta2, step);
+  const int64_t nvec = count >> 2;
+  int64_t blocks = (nvec + AB - 1) / AB;
+  const int64_t cap = (int64_t)SPLX_SM_COUNT * 8;
+  if (blocks > cap) blocks = cap;
+  const AdamK k{0.f, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps,
+                (float)(1.0 / bc1), (float)(1.0 / bc2)};
+  AdamGroups gr;
+  gr.n = n_groups;
+  for (int j = 0; j < SPLX_ADAM_MAX_GROUPS; ++j) {
+    gr.end4[j] = j < n_groups ? group_offsets[j + 1] >> 2 : nvec;
+    gr.lr[j] = j < n_groups ? lr[j] : 0.f;
+  }
+  k_adam_groups<<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, zero_grad);
+  SPLX_LAUNCH_CHECK(ctx, "k_adam_groups");
+  return SPLX_OK;
+}
 
 int launch_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr,
                 float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad) {

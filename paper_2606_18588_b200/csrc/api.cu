@@ -162,13 +162,16 @@ int splx_raster_backward(splx_ctx* ctx, const splx_projected* proj, const splx_b
 }
 
 int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
-                          const splx_projected* proj, float* g2d, int clear_g2d, const splx_gaussian_grads* grads) {
+                          const splx_projected* proj, float* g2d, int flags, const splx_gaussian_grads* grads) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(proj) || !g2d || !aligned16(g2d) || !grads || !grads->mean ||
-      !grads->log_scale || !grads->quat || !grads->opacity_logit || !grads->sh || !aligned16(grads->quat) || grads->n != g->n)
+      !grads->log_scale || !grads->quat || !grads->opacity_logit || !grads->sh || !aligned16(grads->quat) ||
+      !aligned16(grads->mean) || !aligned16(grads->log_scale) || !aligned16(grads->sh) || !aligned16(grads->opacity_logit) ||
+      grads->n != g->n)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: null/misaligned argument");
   if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: sh_degree %d not in [0,3]", sh_degree);
-  return launch_project_bwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, proj, g2d, clear_g2d, grads);
+  if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: unknown flags %d", flags);
+  return launch_project_bwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, proj, g2d, flags, grads);
 }
 
 size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera* cam) {
@@ -181,8 +184,9 @@ size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera* cam) {
 int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
                   const float* dL_dimage, const float* dL_dT_total, const splx_gaussians* g,
                   const splx_projected* proj, const splx_binning* bins, int sh_degree,
-                  const splx_gaussian_grads* grads, void* ws, size_t ws_bytes) {
+                  const splx_gaussian_grads* grads, void* ws, size_t ws_bytes, int flags) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (flags & ~SPLX_PB_OVERWRITE) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: unknown flags %d", flags);
   if (!gauss_ok(g) || !cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: null/misaligned argument");
   const size_t need = splx_backward_ws_bytes(g->n, K, cam);
   if (!ws || !aligned16(ws) || ws_bytes < need)
@@ -196,7 +200,7 @@ int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx
   // a9: reverse-order blend gradients into means2D, conic, opacity, colour
   if ((rc = splx_raster_backward(ctx, proj, bins, K, cam, partials, g_ct, g2d))) return rc;
   // a10: projection backward to the 3-D parameters
-  return splx_project_backward(ctx, g, cam, sh_degree, proj, g2d, 0, grads);
+  return splx_project_backward(ctx, g, cam, sh_degree, proj, g2d, flags, grads);
 }
 
 int splx_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr, float beta1,
@@ -206,6 +210,23 @@ int splx_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int6
       !aligned16(m) || !aligned16(v))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam: null/misaligned argument or step < 1");
   return launch_adam(ctx, param, grad, m, v, count, lr, beta1, beta2, eps, step, grad_scale, zero_grad);
+}
+
+int splx_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int n_groups,
+                     const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
+                     float grad_scale, int zero_grad) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!param || !grad || !m || !v || !group_offsets || !lr || step < 1 || !aligned16(param) || !aligned16(grad) ||
+      !aligned16(m) || !aligned16(v))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups: null/misaligned argument or step < 1");
+  if (n_groups < 1 || n_groups > SPLX_ADAM_MAX_GROUPS)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups: n_groups=%d not in [1,%d]", n_groups, SPLX_ADAM_MAX_GROUPS);
+  if (group_offsets[0] != 0) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups: group_offsets[0] must be 0");
+  for (int j = 0; j < n_groups; ++j)
+    if (group_offsets[j + 1] < group_offsets[j] || (group_offsets[j + 1] & 3))
+      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups: offsets must be monotone multiples of 4");
+  return launch_adam_groups(ctx, param, grad, m, v, n_groups, group_offsets, lr, beta1, beta2, eps, step, grad_scale,
+                            zero_grad);
 }
 
 }  // extern "C"

@@ -89,7 +89,7 @@ __device__ __forceinline__ void tile_rect(float u, float v, int radius, int TX, 
 int launch_project_fwd(splx_ctx*, const splx_gaussians*, const CamDev&, int sh_degree,
                        const splx_projected*);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const CamDev&, int sh_degree,
-                       const splx_projected*, float* g2d, int clear_g2d, const splx_gaussian_grads*);
+                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
 int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, int K, const int64_t* part_offsets,
                     const CamDev&, const splx_binning*, void* ws, size_t ws_bytes);
@@ -103,5 +103,8 @@ int launch_compose_bwd(splx_ctx*, int K, const splx_partial*, const CamDev&, con
                        const float* g_image, const float* g_T_total, float* g_ct);
 int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count, float scale,
               float* g_image, double* loss_sum);
+int launch_adam_groups(splx_ctx*, float* param, float* grad, float* m, float* v, int n_groups,
+                       const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
+                       float grad_scale, int zero_grad);
 int launch_adam(splx_ctx*, float* param, float* grad, float* m, float* v, int64_t count, float lr,
                 float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad);

@@ -195,129 +195,244 @@ __device__ __forceinline__ void sh_grad(int deg, float x, float y, float z, floa
   dY[15][0] = -3.f * kK3a * (xx - yy); dY[15][1] = 6.f * kK3a * x * y;
 }
 
-template <int DEG>
-__global__ void __launch_bounds__(PROJ_THREADS)
+// Backward block = 128 Gaussians.  The 48 SH coefficients of a Gaussian are 192 contiguous bytes, so a
+// thread-per-Gaussian access has a 192-byte stride: scattered 4-byte read-modify-writes of the SH
+// gradient ran at 9 % of the HBM roof (profiles/r01a).  Here the block's SH tile [128][48] and, when
+// accumulating, the tile of the SH gradient travel global -> shared with 16-byte cp.async (LDGSTS)
+// issued before the geometry chain, so ~50 KB per block are in flight while the ALU work runs; the
+// result leaves with coalesced 128-bit stores.  Row stride 52 floats keeps 16-byte alignment and makes
+// both the row-wise LDS.128 of a thread and the cooperative pass conflict-free.  mean / log_scale
+// gradients (12-byte stride) are staged the same way.  Culled rows are never read.
+constexpr int PB_THREADS = 128;
+constexpr int PB_STRIDE = 52;
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+  asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+template <int DEG, bool ACC>
+__global__ void __launch_bounds__(PB_THREADS)
 k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, float* __restrict__ g2d,
               int clear_g2d, splx_gaussian_grads out) {
-  const int64_t i = (int64_t)blockIdx.x * PROJ_THREADS + threadIdx.x;
-  if (i >= g.n) return;
-  if (pr.radius[i] <= 0) return;
+  extern __shared__ __align__(16) float s_dyn[];
+  float* s_sh = s_dyn;                                   // [128][52] sh in, SH gradient out
+  float* s_old = s_dyn + PB_THREADS * PB_STRIDE;         // [128][52] previous SH gradient (ACC only)
+  __shared__ __align__(16) float s_m[PB_THREADS * 3];    // mean gradient tile
+  __shared__ __align__(16) float s_s[PB_THREADS * 3];    // log_scale gradient tile
+  __shared__ uint8_t s_vis[PB_THREADS];
+  const int64_t base = (int64_t)blockIdx.x * PB_THREADS;
+  const int64_t i = base + threadIdx.x;
+  const int nrows = (int)min((int64_t)PB_THREADS, g.n - base);
+  constexpr int NSH = (DEG + 1) * (DEG + 1);
+  constexpr int NV = (NSH * 3 + 3) / 4;        // float4 chunks of a row that hold used coefficients
+  const bool vis = (i < g.n) && (pr.radius[i] > 0);
+  s_vis[threadIdx.x] = vis ? 1 : 0;
+  __syncthreads();
+#pragma unroll
+  for (int c = 0; c < NV; ++c) {
+    const int q = c * PB_THREADS + threadIdx.x;
+    const int row = q / NV, c4 = q - row * NV;
+    if (row < nrows && s_vis[row]) {
+      cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * (base + row) + 4 * c4);
+      if (ACC) cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * (base + row) + 4 * c4);
+    }
+  }
+  float dmu[3] = {0.f, 0.f, 0.f}, dls[3] = {0.f, 0.f, 0.f};
+  float4 dq = make_float4(0.f, 0.f, 0.f, 0.f);
+  float dlogit = 0.f;
+  float grgb[3] = {0.f, 0.f, 0.f};
   Geo G;
-  if (!geometry(g, i, cam, cfg.dilation, G)) return;
-  float4* gp = reinterpret_cast<float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
-  const float4 g0 = gp[0], g1 = gp[1], g2 = gp[2];
-  if (clear_g2d) { const float4 zz = make_float4(0.f, 0.f, 0.f, 0.f); gp[0] = zz; gp[1] = zz; gp[2] = zz; }
-  const float gu = g0.x, gv = g0.y, gA = g0.z, gB = g0.w, gC = g1.x, gop = g1.y;
-  float grgb[3] = {g1.z, g1.w, g2.x};
-
-  // opacity: o = sigmoid(logit)
-  const float op = pr.conic_opacity[4 * i + 3];
-  out.opacity_logit[i] += op * (1.f - op) * gop;
-
-  float dmu[3] = {0.f, 0.f, 0.f};
-  // colour: rgb = max(0, 0.5 + sum_l Y_l(dir) sh_l), dir = (mu - o)/|mu - o|
-  {
+  if (vis && geometry(g, i, cam, cfg.dilation, G)) {
+    float4* gp = reinterpret_cast<float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
+    const float4 g0 = gp[0], g1 = gp[1], g2 = gp[2];
+    if (clear_g2d) { const float4 zz = make_float4(0.f, 0.f, 0.f, 0.f); gp[0] = zz; gp[1] = zz; gp[2] = zz; }
+    const float gu = g0.x, gv = g0.y, gA = g0.z, gB = g0.w, gC = g1.x, gop = g1.y;
+    grgb[0] = g1.z; grgb[1] = g1.w; grgb[2] = g2.x;
     const uint8_t cl = pr.clamp[i];
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) if ((cl >> ch) & 1) grgb[ch] = 0.f;
+
+    // opacity: o = sigmoid(logit)
+    const float op = pr.conic_opacity[4 * i + 3];
+    dlogit = op * (1.f - op) * gop;
+
+    // conic Q = P^-1 (P = Sigma2D):  dL/dP = -Q Gm Q,  Gm = [[gA, gB/2],[gB/2, gC]]
+    const float idet = 1.0f / G.det;
+    const float A = G.c * idet, B = -G.b * idet, C = G.a * idet;
+    const float hB = 0.5f * gB;
+    const float qg00 = A * gA + B * hB, qg01 = A * hB + B * gC;
+    const float qg10 = B * gA + C * hB, qg11 = B * hB + C * gC;
+    const float p00 = -(qg00 * A + qg01 * B), p01 = -(qg00 * B + qg01 * C);
+    const float p11 = -(qg10 * B + qg11 * C);   // symmetric: p10 == p01
+    // P = N N^T + dI, N = Tm Mm:  dL/dN = 2 Gc N;   dL/dTm = dL/dN Mm^T;  dL/dMm = Tm^T dL/dN
+    float dN[6];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      dN[c] = 2.f * (p00 * G.N[c] + p01 * G.N[3 + c]);
+      dN[3 + c] = 2.f * (p01 * G.N[c] + p11 * G.N[3 + c]);
+    }
+    float dTm[6], dMm[9];
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int k = 0; k < 3; ++k)
+        dTm[3 * r + k] = dN[3 * r] * G.Mm[3 * k] + dN[3 * r + 1] * G.Mm[3 * k + 1] + dN[3 * r + 2] * G.Mm[3 * k + 2];
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) dMm[3 * k + c] = G.Tm[k] * dN[c] + G.Tm[3 + k] * dN[3 + c];
+    // Tm = J W:  dL/dJ = dL/dTm W^T.  J = [[fx/z, 0, -fx Lx/z],[0, fy/z, -fy Ly/z]]
+    const float dJ00 = dTm[0] * cam.R[0] + dTm[1] * cam.R[1] + dTm[2] * cam.R[2];
+    const float dJ02 = dTm[0] * cam.R[6] + dTm[1] * cam.R[7] + dTm[2] * cam.R[8];
+    const float dJ11 = dTm[3] * cam.R[3] + dTm[4] * cam.R[4] + dTm[5] * cam.R[5];
+    const float dJ12 = dTm[3] * cam.R[6] + dTm[4] * cam.R[7] + dTm[5] * cam.R[8];
+    const float z = G.p[2], iz = 1.f / z, iz2 = iz * iz;
+    float dp[3] = {0.f, 0.f, 0.f};
+    dp[2] += -cam.fx * iz2 * dJ00 - cam.fy * iz2 * dJ11;
+    // J02 = -fx Lx / z with Lx = clamp(x/z): inside the clamp Lx = x/z -> J02 = -fx x / z^2
+    if (!G.clx) { dp[0] += -cam.fx * iz2 * dJ02; dp[2] += 2.f * cam.fx * G.p[0] * iz2 * iz * dJ02; }
+    else        { dp[2] += cam.fx * G.Lx * iz2 * dJ02; }
+    if (!G.cly) { dp[1] += -cam.fy * iz2 * dJ12; dp[2] += 2.f * cam.fy * G.p[1] * iz2 * iz * dJ12; }
+    else        { dp[2] += cam.fy * G.Ly * iz2 * dJ12; }
+    // 2-D mean
+    dp[0] += cam.fx * iz * gu;
+    dp[1] += cam.fy * iz * gv;
+    dp[2] += -(cam.fx * G.p[0] * gu + cam.fy * G.p[1] * gv) * iz2;
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+      dmu[k] = cam.R[k] * dp[0] + cam.R[3 + k] * dp[1] + cam.R[6 + k] * dp[2];
+
+    // Mm = Rot diag(s)
+    float dRot[9];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      float ds = 0.f;
+#pragma unroll
+      for (int r = 0; r < 3; ++r) { ds = fmaf(G.Rot[3 * r + c], dMm[3 * r + c], ds); dRot[3 * r + c] = G.s[c] * dMm[3 * r + c]; }
+      dls[c] = G.s[c] * ds;
+    }
+    // Rot(q_hat) then the normalisation q_hat = q/|q|
+    const float w = G.qh[0], x = G.qh[1], y = G.qh[2], zq = G.qh[3];
+    float gq[4];
+    gq[0] = 2.f * (-zq * dRot[1] + y * dRot[2] + zq * dRot[3] - x * dRot[5] - y * dRot[6] + x * dRot[7]);
+    gq[1] = 2.f * (y * dRot[1] + zq * dRot[2] + y * dRot[3] - 2.f * x * dRot[4] - w * dRot[5] + zq * dRot[6] + w * dRot[7] - 2.f * x * dRot[8]);
+    gq[2] = 2.f * (-2.f * y * dRot[0] + x * dRot[1] + w * dRot[2] + x * dRot[3] + zq * dRot[5] - w * dRot[6] + zq * dRot[7] - 2.f * y * dRot[8]);
+    gq[3] = 2.f * (-2.f * zq * dRot[0] - w * dRot[1] + x * dRot[2] + w * dRot[3] - 2.f * zq * dRot[4] + y * dRot[5] + x * dRot[6] + y * dRot[7]);
+    const float qd = w * gq[0] + x * gq[1] + y * gq[2] + zq * gq[3];
+    const float iqn = 1.f / G.qn;
+    dq = make_float4((gq[0] - w * qd) * iqn, (gq[1] - x * qd) * iqn, (gq[2] - y * qd) * iqn, (gq[3] - zq * qd) * iqn);
+  }
+  cp_async_wait_all();
+  __syncthreads();
+  if (vis) {
+    // colour: rgb = max(0, 0.5 + sum_l Y_l(dir) sh_l), dir = (mu - o)/|mu - o|
     float dv[3] = {g.mean[3 * i] - cam.o[0], g.mean[3 * i + 1] - cam.o[1], g.mean[3 * i + 2] - cam.o[2]};
     const float dinv = rsqrtf(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]);
     const float dir[3] = {dv[0] * dinv, dv[1] * dinv, dv[2] * dinv};
-    constexpr int NSH = (DEG + 1) * (DEG + 1);
     float Y[NSH];
     sh_eval(DEG, dir[0], dir[1], dir[2], Y);
+    float dot[NSH];
+#pragma unroll
+    for (int l = 0; l < NSH; ++l) dot[l] = 0.f;
+    float4* row = reinterpret_cast<float4*>(s_sh + threadIdx.x * PB_STRIDE);
+    // the row is read (sh) and overwritten in place with this view's SH gradient Y_l * dL/drgb
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+      const float4 f = row[q];
+      const float e[4] = {f.x, f.y, f.z, f.w};
+      float o4[4];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const int idx = 4 * q + t;
+        if (idx < NSH * 3) {
+          dot[idx / 3] = fmaf(e[t], grgb[idx % 3], dot[idx / 3]);
+          o4[t] = Y[idx / 3] * grgb[idx % 3];
+        } else {
+          o4[t] = 0.f;
+        }
+      }
+      row[q] = make_float4(o4[0], o4[1], o4[2], o4[3]);
+    }
     float dY[NSH][3];
     sh_grad(DEG, dir[0], dir[1], dir[2], dY);
     float gdir[3] = {0.f, 0.f, 0.f};
-    const float* shp = g.sh + 48 * i;
-    float* gsh = out.sh + 48 * i;
 #pragma unroll
-    for (int l = 0; l < NSH; ++l) {
-      float dot = 0.f;
+    for (int l = 0; l < NSH; ++l)
 #pragma unroll
-      for (int ch = 0; ch < 3; ++ch) {
-        gsh[3 * l + ch] += Y[l] * grgb[ch];
-        dot = fmaf(__ldg(shp + 3 * l + ch), grgb[ch], dot);
-      }
-#pragma unroll
-      for (int k = 0; k < 3; ++k) gdir[k] = fmaf(dY[l][k], dot, gdir[k]);
-    }
+      for (int k = 0; k < 3; ++k) gdir[k] = fmaf(dY[l][k], dot[l], gdir[k]);
     const float dd = dir[0] * gdir[0] + dir[1] * gdir[1] + dir[2] * gdir[2];
 #pragma unroll
     for (int k = 0; k < 3; ++k) dmu[k] += (gdir[k] - dir[k] * dd) * dinv;
   }
-
-  // conic Q = P^-1 (P = Sigma2D):  dL/dP = -Q Gm Q,  Gm = [[gA, gB/2],[gB/2, gC]]
-  const float idet = 1.0f / G.det;
-  const float A = G.c * idet, B = -G.b * idet, C = G.a * idet;
-  const float hB = 0.5f * gB;
-  const float qg00 = A * gA + B * hB, qg01 = A * hB + B * gC;
-  const float qg10 = B * gA + C * hB, qg11 = B * hB + C * gC;
-  const float p00 = -(qg00 * A + qg01 * B), p01 = -(qg00 * B + qg01 * C);
-  const float p11 = -(qg10 * B + qg11 * C);   // symmetric: p10 == p01
-  // P = N N^T + dI, N = Tm Mm:  dL/dN = 2 Gc N;   dL/dTm = dL/dN Mm^T;  dL/dMm = Tm^T dL/dN
-  float dN[6];
 #pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    dN[c] = 2.f * (p00 * G.N[c] + p01 * G.N[3 + c]);
-    dN[3 + c] = 2.f * (p01 * G.N[c] + p11 * G.N[3 + c]);
+  for (int k = 0; k < 3; ++k) { s_m[3 * threadIdx.x + k] = dmu[k]; s_s[3 * threadIdx.x + k] = dls[k]; }
+  if (i < g.n) {
+    float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
+    if (ACC) {
+      if (vis) {
+        float4 cur = *oq;
+        cur.x += dq.x; cur.y += dq.y; cur.z += dq.z; cur.w += dq.w;
+        *oq = cur;
+        out.opacity_logit[i] += dlogit;
+      }
+    } else {
+      *oq = dq;
+      out.opacity_logit[i] = dlogit;
+    }
   }
-  float dTm[6], dMm[9];
+  __syncthreads();
+  // coalesced write-back of the SH-gradient tile (+= needs visible rows only; = writes every row)
 #pragma unroll
-  for (int r = 0; r < 2; ++r)
-#pragma unroll
-    for (int k = 0; k < 3; ++k)
-      dTm[3 * r + k] = dN[3 * r] * G.Mm[3 * k] + dN[3 * r + 1] * G.Mm[3 * k + 1] + dN[3 * r + 2] * G.Mm[3 * k + 2];
-#pragma unroll
-  for (int k = 0; k < 3; ++k)
-#pragma unroll
-    for (int c = 0; c < 3; ++c) dMm[3 * k + c] = G.Tm[k] * dN[c] + G.Tm[3 + k] * dN[3 + c];
-  // Tm = J W:  dL/dJ = dL/dTm W^T.  J = [[fx/z, 0, -fx Lx/z],[0, fy/z, -fy Ly/z]]
-  const float dJ00 = dTm[0] * cam.R[0] + dTm[1] * cam.R[1] + dTm[2] * cam.R[2];
-  const float dJ02 = dTm[0] * cam.R[6] + dTm[1] * cam.R[7] + dTm[2] * cam.R[8];
-  const float dJ11 = dTm[3] * cam.R[3] + dTm[4] * cam.R[4] + dTm[5] * cam.R[5];
-  const float dJ12 = dTm[3] * cam.R[6] + dTm[4] * cam.R[7] + dTm[5] * cam.R[8];
-  const float z = G.p[2], iz = 1.f / z, iz2 = iz * iz;
-  float dp[3] = {0.f, 0.f, 0.f};
-  dp[2] += -cam.fx * iz2 * dJ00 - cam.fy * iz2 * dJ11;
-  // J02 = -fx Lx / z with Lx = clamp(x/z): inside the clamp Lx = x/z -> J02 = -fx x / z^2
-  if (!G.clx) { dp[0] += -cam.fx * iz2 * dJ02; dp[2] += 2.f * cam.fx * G.p[0] * iz2 * iz * dJ02; }
-  else        { dp[2] += cam.fx * G.Lx * iz2 * dJ02; }
-  if (!G.cly) { dp[1] += -cam.fy * iz2 * dJ12; dp[2] += 2.f * cam.fy * G.p[1] * iz2 * iz * dJ12; }
-  else        { dp[2] += cam.fy * G.Ly * iz2 * dJ12; }
-  // 2-D mean
-  dp[0] += cam.fx * iz * gu;
-  dp[1] += cam.fy * iz * gv;
-  dp[2] += -(cam.fx * G.p[0] * gu + cam.fy * G.p[1] * gv) * iz2;
-#pragma unroll
-  for (int k = 0; k < 3; ++k)
-    dmu[k] += cam.R[k] * dp[0] + cam.R[3 + k] * dp[1] + cam.R[6 + k] * dp[2];
-#pragma unroll
-  for (int k = 0; k < 3; ++k) out.mean[3 * i + k] += dmu[k];
-
-  // Mm = Rot diag(s)
-  float dRot[9];
-#pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    float ds = 0.f;
-#pragma unroll
-    for (int r = 0; r < 3; ++r) { ds = fmaf(G.Rot[3 * r + c], dMm[3 * r + c], ds); dRot[3 * r + c] = G.s[c] * dMm[3 * r + c]; }
-    out.log_scale[3 * i + c] += G.s[c] * ds;
+  for (int c = 0; c < 12; ++c) {
+    const int q = c * PB_THREADS + threadIdx.x;
+    const int row = q / 12, c4 = q - row * 12;
+    if (row < nrows) {
+      float4* dst = reinterpret_cast<float4*>(out.sh + 48 * (base + row)) + c4;
+      const bool live = s_vis[row] && c4 < NV;
+      if (ACC) {
+        if (live) {
+          const float4 a = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
+          const float4 o = *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
+          *dst = make_float4(o.x + a.x, o.y + a.y, o.z + a.z, o.w + a.w);
+        }
+      } else {
+        *dst = live ? *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    }
   }
-  // Rot(q_hat) then the normalisation q_hat = q/|q|
-  const float w = G.qh[0], x = G.qh[1], y = G.qh[2], zq = G.qh[3];
-  float gq[4];
-  gq[0] = 2.f * (-zq * dRot[1] + y * dRot[2] + zq * dRot[3] - x * dRot[5] - y * dRot[6] + x * dRot[7]);
-  gq[1] = 2.f * (y * dRot[1] + zq * dRot[2] + y * dRot[3] - 2.f * x * dRot[4] - w * dRot[5] + zq * dRot[6] + w * dRot[7] - 2.f * x * dRot[8]);
-  gq[2] = 2.f * (-2.f * y * dRot[0] + x * dRot[1] + w * dRot[2] + x * dRot[3] + zq * dRot[5] - w * dRot[6] + zq * dRot[7] - 2.f * y * dRot[8]);
-  gq[3] = 2.f * (-2.f * zq * dRot[0] - w * dRot[1] + x * dRot[2] + w * dRot[3] - 2.f * zq * dRot[4] + y * dRot[5] + x * dRot[6] + y * dRot[7]);
-  const float qd = w * gq[0] + x * gq[1] + y * gq[2] + zq * gq[3];
-  const float iqn = 1.f / G.qn;
-  float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
-  float4 cur = *oq;
-  cur.x += (gq[0] - w * qd) * iqn; cur.y += (gq[1] - x * qd) * iqn;
-  cur.z += (gq[2] - y * qd) * iqn; cur.w += (gq[3] - zq * qd) * iqn;
-  *oq = cur;
+  // mean / log_scale gradient tiles: 96 float4 each; a partial last block falls back to scalars
+  if (nrows == PB_THREADS) {
+    if (threadIdx.x < 96) {
+      float4* dm = reinterpret_cast<float4*>(out.mean + 3 * base) + threadIdx.x;
+      float4* ds = reinterpret_cast<float4*>(out.log_scale + 3 * base) + threadIdx.x;
+      float4 a = reinterpret_cast<const float4*>(s_m)[threadIdx.x], b = reinterpret_cast<const float4*>(s_s)[threadIdx.x];
+      if (ACC) {
+        const float4 om = *dm, os = *ds;
+        a.x += om.x; a.y += om.y; a.z += om.z; a.w += om.w;
+        b.x += os.x; b.y += os.y; b.z += os.z; b.w += os.w;
+      }
+      *dm = a; *ds = b;
+    }
+  } else if (i < g.n) {
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      if (ACC) { out.mean[3 * i + k] += dmu[k]; out.log_scale[3 * i + k] += dls[k]; }
+      else     { out.mean[3 * i + k] = dmu[k]; out.log_scale[3 * i + k] = dls[k]; }
+    }
+  }
+}
+
+template <int DEG, bool ACC>
+static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, const splx_projected* pr, float* g2d,
+                      int clear_g2d, const splx_gaussian_grads* grads) {
+  const unsigned grid = (unsigned)((g->n + PB_THREADS - 1) / PB_THREADS);
+  const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  k_project_bwd<DEG, ACC><<<grid, PB_THREADS, smem, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads);
 }
 
 }  // namespace
@@ -337,15 +452,23 @@ int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam
 }
 
 int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, int deg,
-                       const splx_projected* pr, float* g2d, int clear_g2d,
-                       const splx_gaussian_grads* grads) {
+                       const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads) {
   if (g->n == 0) return SPLX_OK;
-  const unsigned grid = (unsigned)((g->n + PROJ_THREADS - 1) / PROJ_THREADS);
-  switch (deg) {
-    case 0: k_project_bwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
-    case 1: k_project_bwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
-    case 2: k_project_bwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
-    default: k_project_bwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads); break;
+  const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
+  if (flags & SPLX_PB_OVERWRITE) {
+    switch (deg) {
+      case 0: launch_pb<0, false>(ctx, g, cam, pr, g2d, clr, grads); break;
+      case 1: launch_pb<1, false>(ctx, g, cam, pr, g2d, clr, grads); break;
+      case 2: launch_pb<2, false>(ctx, g, cam, pr, g2d, clr, grads); break;
+      default: launch_pb<3, false>(ctx, g, cam, pr, g2d, clr, grads); break;
+    }
+  } else {
+    switch (deg) {
+      case 0: launch_pb<0, true>(ctx, g, cam, pr, g2d, clr, grads); break;
+      case 1: launch_pb<1, true>(ctx, g, cam, pr, g2d, clr, grads); break;
+      case 2: launch_pb<2, true>(ctx, g, cam, pr, g2d, clr, grads); break;
+      default: launch_pb<3, true>(ctx, g, cam, pr, g2d, clr, grads); break;
+    }
   }
   SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
   return SPLX_OK;

@@ -83,25 +83,28 @@ class Trainer:
         """a7: mean-L1 gradient (harness step)."""
         self.ctx.l1_loss_grad(self.image, target, self.g_image, self.loss_sum, scale)
 
-    def backward(self, g_image=None, g_T_total=None):
-        """a8-a10: composition backward, rasteriser backward, projection backward (grads +=)."""
+    def backward(self, g_image=None, g_T_total=None, overwrite=False):
+        """a8-a10: composition backward, rasteriser backward, projection backward (grads +=, or = for the
+        first view of an iteration when overwrite is set)."""
         self.ctx.backward(self.K, self.partials, self._cam, self.bg, self.g_image if g_image is None else g_image,
-                          g_T_total, self.params, self.proj, self.bins, self.sh_degree, self.grads, self._ws_bwd)
+                          g_T_total, self.params, self.proj, self.bins, self.sh_degree, self.grads, self._ws_bwd,
+                          overwrite=overwrite)
 
-    def adam_step(self, n_views=1, zero_grad=True):
-        """a11: one Adam step per parameter group."""
+    def adam_step(self, n_views=1, zero_grad=False):
+        """a11: one Adam step over the flat parameter buffer (five groups = five learning rates, one launch)."""
         self.step_count += 1
-        for k in PARAM_KEYS:
-            self.ctx.adam(self.params[k], self.grads[k], self.m[k], self.v[k], self.lr[k], step=self.step_count,
-                          grad_scale=1.0 / n_views, zero_grad=zero_grad)
+        offs = [self._offs[k] for k in PARAM_KEYS] + [self._total]
+        self.ctx.adam_groups(self.flat["param"], self.flat["grad"], self.flat["m"], self.flat["v"], offs,
+                             [self.lr[k] for k in PARAM_KEYS], step=self.step_count, grad_scale=1.0 / n_views,
+                             zero_grad=zero_grad)
 
     def iteration(self, cams, targets):
         """One training iteration over B views (gradients of the B mean losses are averaged)."""
-        for cam, tgt in zip(cams, targets):
+        for b, (cam, tgt) in enumerate(zip(cams, targets)):
             self.forward(cam)
             self.loss_grad(tgt)
-            self.backward()
-        self.adam_step(len(cams))
+            self.backward(overwrite=(b == 0))     # the first view stores, the others accumulate
+        self.adam_step(len(cams))                 # no gradient zeroing needed: next iteration overwrites
 
     def num_intersections(self) -> int:
         return self.ctx.check_capacity(self.bins)

@@ -246,6 +246,15 @@ def test_a10_projection_backward(run):
     before = grads["mean"].clone()
     tr.ctx.project_backward(tr.params, run.cam, tr.sh_degree, tr.proj, g2d_dev, grads)
     assert torch.allclose(grads["mean"], 2 * before, rtol=1e-6, atol=0)
+    # overwrite mode (=): every row written, whatever the buffers held before; equals the += result from zero
+    dirty = {k: torch.full_like(v, 123.0) for k, v in tr.params.items()}
+    g2d_dev = torch.from_numpy(g2d).cuda()
+    tr.ctx.project_backward(tr.params, run.cam, tr.sh_degree, tr.proj, g2d_dev, dirty, overwrite=True)
+    clean = {k: torch.zeros_like(v) for k, v in tr.params.items()}
+    g2d_dev = torch.from_numpy(g2d).cuda()
+    tr.ctx.project_backward(tr.params, run.cam, tr.sh_degree, tr.proj, g2d_dev, clean)
+    for key in scenes.PARAM_KEYS:
+        assert torch.equal(dirty[key], clean[key]), key
 
 
 def test_free_running_iteration_end_to_end(run):
@@ -288,3 +297,34 @@ def test_a11_adam(run):
         assert not gd.any()
     assert np.abs(G.np32(p) - P).max() <= 1e-5
     assert G.rel_l2(G.np32(m), Mo) <= 1e-5 and G.rel_l2(G.np32(v), Vo) <= 1e-5
+
+
+def test_a11_adam_groups_equals_per_group_calls(run):
+    """splx_adam_groups (one launch over the flat buffer) == one splx_adam call per group, bit for bit."""
+    tr = run.tr
+    rng = np.random.default_rng(12)
+    offs = [0, 1000, 1000, 5004, 9008]      # an empty group included; multiples of 4
+    lrs = [1e-3, 7e-2, 3e-4, 5e-3]
+    n = offs[-1]
+    p0 = rng.standard_normal(n).astype(np.float32)
+    g0 = rng.standard_normal(n).astype(np.float32)
+    a = [torch.from_numpy(x.copy()).cuda() for x in (p0, g0, np.zeros(n, np.float32), np.zeros(n, np.float32))]
+    b = [t.clone() for t in a]
+    for step in (1, 2, 3):
+        tr.ctx.adam_groups(a[0], a[1], a[2], a[3], offs, lrs, step=step, grad_scale=0.25)
+        for j, lr in enumerate(lrs):
+            s = slice(offs[j], offs[j + 1])
+            if offs[j + 1] > offs[j]:
+                tr.ctx.adam(b[0][s], b[1][s], b[2][s], b[3][s], lr=lr, step=step, grad_scale=0.25)
+    for x, y in zip(a, b):
+        assert torch.equal(x, y)
+    # and against the oracle
+    P = p0.astype(np.float64); Mo = np.zeros(n); Vo = np.zeros(n)
+    for step in (1, 2, 3):
+        for j, lr in enumerate(lrs):
+            s = slice(offs[j], offs[j + 1])
+            Ps, Ms, Vs = P[s].copy(), Mo[s].copy(), Vo[s].copy()
+            oracle.adam(Ps, g0[s].astype(np.float64) * 0.25, Ms, Vs, lr=float(np.float32(lr)), beta1=float(np.float32(0.9)),
+                        beta2=float(np.float32(0.999)), eps=float(np.float32(1e-15)), step=step)
+            P[s], Mo[s], Vo[s] = Ps, Ms, Vs
+    assert np.abs(G.np32(a[0]) - P).max() <= 1e-5
