@@ -40,6 +40,7 @@ extern "C" {
 #define SPLX_MAX_K 64
 #define SPLX_TILE 16
 #define SPLX_ADAM_MAX_GROUPS 8
+#define SPLX_BLEND_STRIDE 12 /* floats per Gaussian in splx_projected.blend */
 #define SPLX_G2D_STRIDE 12 /* floats per Gaussian in the 2-D gradient buffer, see splx_raster_backward */
 
 typedef struct splx_ctx splx_ctx;
@@ -87,6 +88,11 @@ typedef struct {
   int32_t *radius;
   uint32_t *tiles_touched;
   uint8_t *clamp;
+  /* blend[n,12]: the 48-byte record the blend kernels stage per list entry, written by
+   * splx_project from the values above (no new arithmetic beyond the log2(e) pre-scaling of the
+   * conic): (u, v, o, depth | -0.5 log2e A, -log2e B, -0.5 log2e C, bits(Gaussian index) |
+   * r, g, b, 0).  Zeros for a culled Gaussian. */
+  float *blend;
 } splx_projected;
 
 /* Tile binning of all K partitions.  slot = k * (TX*TY) + tile; key = (slot << 32) |
@@ -139,10 +145,14 @@ int splx_bin_sort(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
  * `bins` dropped entries; writes M to *m_host (may be NULL).  The only blocking call. */
 int splx_check_capacity(splx_ctx *ctx, const splx_binning *bins, uint64_t *m_host);
 
-/* ---- a5 local render: PAPER.md Eq.1 (L84), Eq.3 (L167), Eq.4 (L172).  Grid = K x tiles,
- * one thread per pixel, the tile's list staged 256 Gaussians at a time in shared memory.
- * pairs (device uint64[2], may be NULL): pairs[0] += number of list entries walked, summed over
- * pixels (the oracle's unit of work); pairs[1] += number of (pixel, Gaussian) pairs blended. */
+/* ---- a5 local render: PAPER.md Eq.1 (L84), Eq.3 (L167), Eq.4 (L172).  Grid = K x tiles;
+ * one warp per half tile (16 x 8 pixels, 4 pixels per lane), the tile's list staged 32 records
+ * at a time in shared memory with cp.async and culled per 8 x 4 pixel block (exact: only
+ * entries whose alpha stays below alpha_min on the whole block are dropped).
+ * pairs (device uint64[4], may be NULL): pairs[0] += number of list entries walked, summed over
+ * pixels (the oracle's unit of work, independent of the culling); pairs[1] += number of
+ * (pixel, Gaussian) pairs blended; pairs[2] += alpha evaluations actually executed;
+ * pairs[3] += (Gaussian, half tile) items that survived the culling. */
 int splx_render_partial(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins, int K,
                         const splx_camera *cam, const splx_partial *out, uint64_t *pairs);
 

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libsplx.so")
 _lib = None
 
 G2D_STRIDE = 12
+BLEND_STRIDE = 12
 TILE = 16
 MAX_K = 64
 PB_CLEAR_G2D, PB_OVERWRITE = 1, 2
@@ -56,7 +57,7 @@ class GaussiansS(C.Structure):
 class ProjectedS(C.Structure):
     _fields_ = [("means2d", C.c_void_p), ("depth", C.c_void_p), ("conic_opacity", C.c_void_p),
                 ("rgb", C.c_void_p), ("radius", C.c_void_p), ("tiles_touched", C.c_void_p),
-                ("clamp", C.c_void_p)]
+                ("clamp", C.c_void_p), ("blend", C.c_void_p)]
 
 
 class BinningS(C.Structure):
@@ -152,11 +153,12 @@ class Projected:
         self.radius = torch.empty(n, dtype=torch.int32, device=device)
         self.tiles_touched = torch.empty(n, dtype=torch.int32, device=device)  # uint32 bits
         self.clamp = torch.empty(n, dtype=torch.uint8, device=device)
+        self.blend = torch.empty((n, BLEND_STRIDE), **f)
         self.n = n
 
     def struct(self):
         return ProjectedS(_ptr(self.means2d), _ptr(self.depth), _ptr(self.conic_opacity), _ptr(self.rgb),
-                          _ptr(self.radius), _ptr(self.tiles_touched), _ptr(self.clamp))
+                          _ptr(self.radius), _ptr(self.tiles_touched), _ptr(self.clamp), _ptr(self.blend))
 
 
 class Binning:

@@ -9,7 +9,7 @@ static bool cam_ok(const splx_camera* c) {
 }
 static bool proj_ok(const splx_projected* p) {
   return p && p->means2d && p->depth && p->conic_opacity && p->rgb && p->radius && p->tiles_touched &&
-         p->clamp && aligned16(p->means2d) && aligned16(p->conic_opacity);
+         p->clamp && p->blend && aligned16(p->means2d) && aligned16(p->conic_opacity) && aligned16(p->blend);
 }
 static bool gauss_ok(const splx_gaussians* g) {
   return g && g->n >= 0 && (g->n == 0 || (g->mean && g->log_scale && g->quat && g->opacity_logit && g->sh &&

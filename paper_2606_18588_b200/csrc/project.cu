@@ -135,14 +135,21 @@ k_project_fwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected out)
     *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
     out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
     out.radius[i] = 0; out.tiles_touched[i] = 0; out.clamp[i] = 0;
+    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+    bl[0] = bl[1] = bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
     return;
   }
   const float idet = 1.0f / G.det;
   const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
   *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
   out.depth[i] = G.p[2];
-  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(G.c * idet, -G.b * idet, G.a * idet, op);
+  const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
+  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
   out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
+  float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+  constexpr float kLog2e = 1.4426950408889634f;
+  bl[0] = make_float4(u, v, op, G.p[2]);
+  bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
 
   // colour: SH along the direction from the camera centre to the mean (s13)
   float dx = g.mean[3 * i] - cam.o[0], dy = g.mean[3 * i + 1] - cam.o[1], dz = g.mean[3 * i + 2] - cam.o[2];
@@ -170,6 +177,7 @@ k_project_fwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected out)
     if (c[ch] < 0.f) { cl |= (uint8_t)(1u << ch); c[ch] = 0.f; }
     out.rgb[3 * i + ch] = c[ch];
   }
+  bl[2] = make_float4(c[0], c[1], c[2], 0.f);
   out.clamp[i] = cl;
 }
 

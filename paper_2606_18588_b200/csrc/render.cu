@@ -6,113 +6,209 @@
 // below T_eps.  Backward: PAPER.md L184 ("the per-Gaussian gradient backpropagates through the
 // intermediate partial pixel"), with dL/dC^m and dL/dT^m coming from Eq.6-7 (compose.cu).
 //
-// Grid = (tiles, K): one CTA per (partition, tile), 256 threads = 16x16 pixels, the tile's sorted
-// list staged 256 Gaussians at a time in shared memory.  A warp owns an 8x4 pixel block (not a
-// 32x1 row) so that small footprints leave whole warps idle in the backward, where a warp that
-// has no contributor for a Gaussian skips its reduction.  Neither kernel is HBM-bound: the
-// forward is FP32/MUFU issue bound, the backward FP32 + shuffle + atomics.
+// Both kernels are instruction-issue bound (profiles/r01a: 90 % issue-slot utilisation, DRAM 2 %),
+// so the design minimises instructions per useful (pixel, Gaussian) pair:
+//   * grid = (tiles, K), CTA = 2 autonomous warps, one per HALF tile (16 x 8 pixels).  A lane owns 4
+//     pixels, one in each 8 x 4 block ("slot") of the half tile, so the record of a Gaussian is read
+//     from shared memory once per 4 pixel evaluations and the x / y terms of the quadratic form are
+//     shared between the slots.  No __syncthreads anywhere: a warp stages its own copy of the list.
+//   * the tile's sorted list is staged 32 records (48 B each, splx_projected.blend) at a time with
+//     16-byte cp.async into a two-deep ring, one record per lane, prefetched a batch ahead.
+//   * exact culling: the lane that staged a record computes, per slot, the maximum of the Gaussian's
+//     exponent over the slot's pixel rectangle (closed form for a concave quadratic on a box); a slot
+//     whose best pixel stays below alpha_min is skipped for that Gaussian.  Only pairs that the
+//     alpha_min rule would skip anyway are dropped, so results are bit-identical to walking the list.
+//   * backward: a lane accumulates the six moments of dL/dG over its 4 pixels and the colour sums in
+//     registers; ONE warp reduction (14 shuffles for 9 values) and one set of atomics per
+//     (Gaussian, half tile) that has a contributor.
 #include "common.cuh"
 
 namespace {
 
-constexpr int BLOCK = 256;
-constexpr float LOG2E = 1.4426950408889634f;
+constexpr int WARPS = 2;                 // warps per CTA = half tiles per tile
+constexpr int BLOCK = 32 * WARPS;
+constexpr int NBUF = 2;                  // staging ring depth
 constexpr float LN2 = 0.6931471805599453f;
-
-struct Splat {          // one staged list entry; conic pre-scaled so that alpha = o * 2^p2
-  float2 xy;
-  float4 con;           // (-0.5 log2e A, -log2e B, -0.5 log2e C, o)
-};
+constexpr float CULL_MARGIN = 0.02f;     // in log2(alpha): 1.4 % slack, far above fp32 rounding of the exponent
+constexpr unsigned FULL = 0xffffffffu;
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float lg2_approx(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// The same instruction sequence in the forward and the backward, so that both take identical
-// skip / clamp decisions for every (pixel, Gaussian) pair.
-__device__ __forceinline__ bool eval_alpha(float px, float py, const float2 xy, const float4 con,
-                                           float amin, float amax, float& dx, float& dy, float& G,
-                                           float& alpha, bool& clamped) {
-  dx = __fsub_rn(xy.x, px);
-  dy = __fsub_rn(xy.y, py);
-  const float p2 = fmaf(__fmul_rn(con.x, dx), dx, fmaf(__fmul_rn(con.z, dy), dy, __fmul_rn(__fmul_rn(con.y, dx), dy)));
+// Staging ring of one warp: [buffer][quarter of the record][entry].  Quarter 0 = (u, v, o, depth),
+// 1 = (A', B', C', bits(index)), 2 = (r, g, b, 0).
+struct Ring { float4 q[NBUF][3][32]; };
+
+// Issue the copies of list entry `idx` (if inside [.., end)) into slot `lane` of ring buffer `buf`.
+__device__ __forceinline__ void stage_issue(Ring& ring, int buf, int lane, const float* __restrict__ blend,
+                                            const uint32_t* __restrict__ vals, uint32_t idx, uint32_t end) {
+  if (idx < end) {
+    const float* src = blend + (size_t)SPLX_BLEND_STRIDE * __ldg(vals + idx);
+    cp_async16(&ring.q[buf][0][lane], src);
+    cp_async16(&ring.q[buf][1][lane], src + 4);
+    cp_async16(&ring.q[buf][2][lane], src + 8);
+  }
+  cp_async_commit();
+}
+
+// Maximum over the rectangle [x0,x1] x [y0,y1] of q(dx,dy) = A dx^2 + B dx dy + C dy^2 with
+// (dx,dy) = (gx - x, gy - y), for a negative definite form (A, C < 0).  The maximiser lies on one
+// of the (at most two) box edges that face the centre; on the line through the clamped centre
+// coordinate the 1-D optimum is the unconstrained one clamped to the edge's extent.
+__device__ __forceinline__ float quad_max_rect(float gx, float gy, float A, float B, float C, float hBC, float hBA,
+                                               float x0, float x1, float y0, float y1) {
+  const float dxc = gx - fminf(fmaxf(gx, x0), x1);
+  const float dyc = gy - fminf(fmaxf(gy, y0), y1);
+  const float dy1 = fminf(fmaxf(hBC * dxc, gy - y1), gy - y0);     // hBC = -B / (2C)
+  const float q1 = A * dxc * dxc + (B * dxc + C * dy1) * dy1;
+  const float dx2 = fminf(fmaxf(hBA * dyc, gx - x1), gx - x0);     // hBA = -B / (2A)
+  const float q2 = C * dyc * dyc + (B * dyc + A * dx2) * dx2;
+  return fmaxf(q1, q2);
+}
+
+// 4-bit mask of the slots of this warp's half tile on which the Gaussian can reach alpha_min.
+// (X0, Y0) = pixel coordinates of the half tile's first pixel; slot s covers columns 8(s&1)..+7 and
+// rows 4(s>>1)..+3; pixel i samples i + 0.5.
+__device__ __forceinline__ unsigned cull_mask(const float4 a, const float4 b, float X0, float Y0, float log2_amin) {
+  const float A = b.x, B = b.y, C = b.z, o = a.z;
+  if (!(A < 0.f) || !(C < 0.f) || !(log2_amin > -1e30f)) return 0xFu;   // degenerate conic or alpha_min == 0: keep all
+  const float tau = log2_amin - lg2_approx(o) - CULL_MARGIN;           // keep the slot if max exponent >= tau
+  const float hBC = -0.5f * __fdividef(B, C), hBA = -0.5f * __fdividef(B, A);
+  unsigned m = 0;
+#pragma unroll
+  for (int s = 0; s < 4; ++s) {
+    const float x0 = X0 + (float)(8 * (s & 1)) + 0.5f, y0 = Y0 + (float)(4 * (s >> 1)) + 0.5f;
+    const float qm = quad_max_rect(a.x, a.y, A, B, C, hBC, hBA, x0, x0 + 7.0f, y0, y0 + 3.0f);
+    if (!(qm < tau)) m |= 1u << s;
+  }
+  return m;
+}
+
+// The alpha of one (pixel, Gaussian) pair: the same instruction sequence in the forward and the
+// backward, so that both take identical skip / clamp decisions.  adx = A' dx, bdx = B' dx, cdy = C' dy.
+__device__ __forceinline__ bool eval_alpha(float dx, float dy, float adx, float bdx, float cdy, float o, float amin,
+                                           float amax, float& G, float& alpha, bool& clamped) {
+  const float p2 = fmaf(adx, dx, fmaf(cdy, dy, __fmul_rn(bdx, dy)));
   G = ex2_approx(p2);
-  const float a = __fmul_rn(con.w, G);
+  const float a = __fmul_rn(o, G);
   clamped = a >= amax;
   alpha = fminf(amax, a);
   return (p2 <= 0.0f) && (alpha >= amin);
 }
 
-__device__ __forceinline__ void pixel_of_thread(int tile, int TX, int& px, int& py) {
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tx = tile % TX, ty = tile / TX;
-  px = tx * SPLX_TILE + (warp & 1) * 8 + (lane & 7);
-  py = ty * SPLX_TILE + (warp >> 1) * 4 + (lane >> 3);
-}
-
-__device__ __forceinline__ Splat stage(const float* means2d, const float* conic_opacity, uint32_t g) {
-  Splat s;
-  s.xy = *reinterpret_cast<const float2*>(means2d + 2 * (size_t)g);
-  const float4 co = *reinterpret_cast<const float4*>(conic_opacity + 4 * (size_t)g);
-  s.con = make_float4(co.x * (-0.5f * LOG2E), co.y * (-LOG2E), co.z * (-0.5f * LOG2E), co.w);
-  return s;
-}
-
+template <bool COUNT>
 __global__ void __launch_bounds__(BLOCK)
-k_render_fwd(const float* __restrict__ means2d, const float* __restrict__ conic_opacity,
-             const float* __restrict__ rgb, const float* __restrict__ depth,
-             const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges, int W, int H, int TX,
-             int ntiles, splx_config cfg, float* __restrict__ out_ct, float* __restrict__ out_d,
-             uint32_t* __restrict__ out_n, unsigned long long* pairs) {
-  __shared__ Splat s_sp[BLOCK];
-  __shared__ float4 s_cd[BLOCK];   // rgb, depth
+k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
+             int W, int H, int TX, int ntiles, splx_config cfg, float* __restrict__ out_ct,
+             float* __restrict__ out_d, uint32_t* __restrict__ out_n, unsigned long long* pairs) {
+  __shared__ Ring rings[WARPS];
   const int tile = blockIdx.x, k = blockIdx.y;
-  int pxi, pyi;
-  pixel_of_thread(tile, TX, pxi, pyi);
-  const bool inside = pxi < W && pyi < H;
-  const float px = (float)pxi + 0.5f, py = (float)pyi + 0.5f;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  Ring& ring = rings[warp];
+  const int X0 = (tile % TX) * SPLX_TILE, Y0 = (tile / TX) * SPLX_TILE + 8 * warp;
+  const int pxi = X0 + (lane & 7), pyi = Y0 + (lane >> 3);          // slot 0 pixel; slot s adds (8(s&1), 4(s>>1))
+  const float px0 = (float)pxi + 0.5f, px1 = px0 + 8.0f, py0 = (float)pyi + 0.5f, py1 = py0 + 4.0f;
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
-  float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
-  uint32_t walked = 0, last = 0, blended = 0;
-  bool done = !inside;
-  for (uint32_t start = r0; start < r1; start += BLOCK) {
-    if (__syncthreads_count(done) == BLOCK) break;
-    const uint32_t idx = start + threadIdx.x;
-    if (idx < r1) {
-      const uint32_t g = vals[idx];
-      s_sp[threadIdx.x] = stage(means2d, conic_opacity, g);
-      s_cd[threadIdx.x] = make_float4(rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1], rgb[3 * (size_t)g + 2], depth[g]);
-    }
-    __syncthreads();
-    const int nb = min((uint32_t)BLOCK, r1 - start);
-    for (int j = 0; !done && j < nb; ++j) {
-      ++walked;
-      float dx, dy, G, alpha; bool clamped;
-      if (!eval_alpha(px, py, s_sp[j].xy, s_sp[j].con, cfg.alpha_min, cfg.alpha_max, dx, dy, G, alpha, clamped)) continue;
-      const float Tn = T * (1.0f - alpha);
-      if (Tn < cfg.T_eps) { done = true; continue; }
-      const float w = alpha * T;
-      const float4 cd = s_cd[j];
-      C0 = fmaf(w, cd.x, C0); C1 = fmaf(w, cd.y, C1); C2 = fmaf(w, cd.z, C2); D = fmaf(w, cd.w, D);
-      T = Tn;
-      last = walked;
-      ++blended;
-    }
+  const float log2_amin = cfg.alpha_min > 0.f ? log2f(cfg.alpha_min) : -INFINITY;
+
+  float T[4], C0[4], C1[4], C2[4], D[4];
+  uint32_t last[4], wdone[4];
+  unsigned done = 0;                       // bit s: slot s finished (exit rule fired, or outside the image)
+  uint32_t blended = 0, evaluated = 0, items = 0;
+#pragma unroll
+  for (int s = 0; s < 4; ++s) {
+    T[s] = 1.f; C0[s] = C1[s] = C2[s] = D[s] = 0.f; last[s] = 0; wdone[s] = 0;
+    if (pxi + 8 * (s & 1) >= W || pyi + 4 * (s >> 1) >= H) done |= 1u << s;
   }
-  if (inside) {
-    const size_t pix = ((size_t)k * H + pyi) * W + pxi;
-    *reinterpret_cast<float4*>(out_ct + 4 * pix) = make_float4(C0, C1, C2, T);
-    out_d[pix] = D;
-    out_n[pix] = last;
+  const unsigned outside = done;
+
+  if (r0 < r1 && !__all_sync(FULL, done == 0xFu)) {
+    stage_issue(ring, 0, lane, blend, vals, r0 + lane, r1);
+    int buf = 0;
+    for (uint32_t start = r0; start < r1; start += 32, buf ^= 1) {
+      stage_issue(ring, buf ^ 1, lane, blend, vals, start + 32 + lane, r1);
+      cp_async_wait<1>();
+      __syncwarp();
+      unsigned m = 0;
+      if (start + lane < r1) m = cull_mask(ring.q[buf][0][lane], ring.q[buf][1][lane], (float)X0, (float)Y0, log2_amin);
+      const unsigned open_slots = ~__reduce_and_sync(FULL, done) & 0xFu;   // slots not yet finished in every lane
+      m &= open_slots;
+      unsigned live = __ballot_sync(FULL, m != 0);
+      while (live) {
+        const int j = __ffs(live) - 1;
+        live &= live - 1;
+        const unsigned mj = __shfl_sync(FULL, m, j);
+        const float4 a = ring.q[buf][0][j], b = ring.q[buf][1][j], c = ring.q[buf][2][j];
+        const uint32_t pos = start - r0 + (uint32_t)j + 1;     // 1-based list position, as in n_contrib
+        const float dxs[2] = {__fsub_rn(a.x, px0), __fsub_rn(a.x, px1)};
+        const float dys[2] = {__fsub_rn(a.y, py0), __fsub_rn(a.y, py1)};
+        const float adx[2] = {__fmul_rn(b.x, dxs[0]), __fmul_rn(b.x, dxs[1])};
+        const float bdx[2] = {__fmul_rn(b.y, dxs[0]), __fmul_rn(b.y, dxs[1])};
+        const float cdy[2] = {__fmul_rn(b.z, dys[0]), __fmul_rn(b.z, dys[1])};
+        if (COUNT) ++items;
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+          if (!((mj >> s) & 1)) continue;     // warp-uniform
+          if (COUNT) ++evaluated;
+          float G, alpha; bool clamped;
+          const bool ok = eval_alpha(dxs[s & 1], dys[s >> 1], adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min,
+                                     cfg.alpha_max, G, alpha, clamped);
+          if (ok && !((done >> s) & 1)) {
+            const float Tn = T[s] * (1.0f - alpha);
+            if (Tn < cfg.T_eps) {
+              done |= 1u << s;
+              wdone[s] = pos;
+            } else {
+              const float w = alpha * T[s];
+              C0[s] = fmaf(w, c.x, C0[s]); C1[s] = fmaf(w, c.y, C1[s]); C2[s] = fmaf(w, c.z, C2[s]);
+              D[s] = fmaf(w, a.w, D[s]);
+              T[s] = Tn;
+              last[s] = pos;
+              if (COUNT) ++blended;
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if (__all_sync(FULL, done == 0xFu)) break;
+    }
+    cp_async_wait<0>();
   }
-  if (pairs) {
-    const uint32_t wsum = __reduce_add_sync(0xffffffffu, inside ? walked : 0u);
-    const uint32_t bsum = __reduce_add_sync(0xffffffffu, blended);
-    if ((threadIdx.x & 31) == 0 && wsum) {
+
+  uint32_t walked = 0;
+#pragma unroll
+  for (int s = 0; s < 4; ++s) {
+    if ((outside >> s) & 1) continue;
+    const int x = pxi + 8 * (s & 1), y = pyi + 4 * (s >> 1);
+    const size_t pix = ((size_t)k * H + y) * W + x;
+    *reinterpret_cast<float4*>(out_ct + 4 * pix) = make_float4(C0[s], C1[s], C2[s], T[s]);
+    out_d[pix] = D[s];
+    out_n[pix] = last[s];
+    if (COUNT) walked += ((done >> s) & 1) ? wdone[s] : (r1 - r0);
+  }
+  if (COUNT && pairs) {
+    const uint32_t wsum = __reduce_add_sync(FULL, walked);
+    const uint32_t bsum = __reduce_add_sync(FULL, blended);
+    if (lane == 0 && wsum) {
       atomicAdd(pairs, (unsigned long long)wsum);
       atomicAdd(pairs + 1, (unsigned long long)bsum);
+      atomicAdd(pairs + 2, 32ull * evaluated);
+      atomicAdd(pairs + 3, (unsigned long long)items);
     }
   }
 }
@@ -126,101 +222,128 @@ __device__ __forceinline__ float warp_reduce9(float (&v)[8], float& v8, int lane
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const float send = h16 ? v[i] : v[i + 4], keep = h16 ? v[i + 4] : v[i];
-    a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    a[i] = keep + __shfl_xor_sync(FULL, send, 16);
   }
 #pragma unroll
   for (int i = 0; i < 2; ++i) {
     const float send = h8 ? a[i] : a[i + 2], keep = h8 ? a[i + 2] : a[i];
-    b[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    b[i] = keep + __shfl_xor_sync(FULL, send, 8);
   }
   {
     const float send = h4 ? b[0] : b[1], keep = h4 ? b[1] : b[0];
-    c = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    c = keep + __shfl_xor_sync(FULL, send, 4);
   }
-  c += __shfl_xor_sync(0xffffffffu, c, 2);
-  c += __shfl_xor_sync(0xffffffffu, c, 1);
+  c += __shfl_xor_sync(FULL, c, 2);
+  c += __shfl_xor_sync(FULL, c, 1);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v8 += __shfl_xor_sync(0xffffffffu, v8, o);
+  for (int o = 16; o > 0; o >>= 1) v8 += __shfl_xor_sync(FULL, v8, o);
   return c;   // lane L: total of v[((L>>4)&1)*4 + ((L>>3)&1)*2 + ((L>>2)&1)]
 }
 
 __global__ void __launch_bounds__(BLOCK)
-k_raster_bwd(const float* __restrict__ means2d, const float* __restrict__ conic_opacity,
-             const float* __restrict__ rgb, const uint32_t* __restrict__ vals,
-             const uint32_t* __restrict__ ranges, int W, int H, int TX, int ntiles, splx_config cfg,
-             const float* __restrict__ ct, const uint32_t* __restrict__ n_contrib,
-             const float* __restrict__ g_ct, float* __restrict__ g2d) {
-  __shared__ Splat s_sp[BLOCK];
-  __shared__ float4 s_ci[BLOCK];   // rgb, Gaussian index (as bits)
-  __shared__ uint32_t s_max[BLOCK / 32];
+k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
+             int W, int H, int TX, int ntiles, splx_config cfg, const float* __restrict__ ct,
+             const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d) {
+  __shared__ Ring rings[WARPS];
   const int tile = blockIdx.x, k = blockIdx.y;
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
   if (r0 == r1) return;
-  int pxi, pyi;
-  pixel_of_thread(tile, TX, pxi, pyi);
-  const bool inside = pxi < W && pyi < H;
-  const float px = (float)pxi + 0.5f, py = (float)pyi + 0.5f;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  uint32_t last = 0;
-  float T = 1.f, Tfin = 1.f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gT = 0.f;
-  if (inside) {
-    const size_t pix = ((size_t)k * H + pyi) * W + pxi;
-    last = n_contrib[pix];
-    Tfin = ct[4 * pix + 3];
-    const float4 g = *reinterpret_cast<const float4*>(g_ct + 4 * pix);
-    gC0 = g.x; gC1 = g.y; gC2 = g.z; gT = g.w;
-  }
-  T = Tfin;
-  const uint32_t wmax = __reduce_max_sync(0xffffffffu, last);
-  if (lane == 0) s_max[warp] = wmax;
-  __syncthreads();
-  uint32_t bmax = 0;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  Ring& ring = rings[warp];
+  const int X0 = (tile % TX) * SPLX_TILE, Y0 = (tile / TX) * SPLX_TILE + 8 * warp;
+  const int pxi = X0 + (lane & 7), pyi = Y0 + (lane >> 3);
+  const float px0 = (float)pxi + 0.5f, px1 = px0 + 8.0f, py0 = (float)pyi + 0.5f, py1 = py0 + 4.0f;
+  const float log2_amin = cfg.alpha_min > 0.f ? log2f(cfg.alpha_min) : -INFINITY;
+
+  uint32_t last[4];
+  float T[4], S0[4], S1[4], S2[4], gC0[4], gC1[4], gC2[4], gTfin[4];
+  uint32_t lmax = 0;
 #pragma unroll
-  for (int w = 0; w < BLOCK / 32; ++w) bmax = max(bmax, s_max[w]);
-  if (bmax == 0) return;
-  float S0 = 0.f, S1 = 0.f, S2 = 0.f;   // colour behind the current Gaussian (relative to its T)
-  const float gTfin = gT * Tfin;
-  for (int b = (int)((bmax - 1) / BLOCK); b >= 0; --b) {
-    __syncthreads();
-    const uint32_t pos = (uint32_t)b * BLOCK + threadIdx.x;
-    if (pos < bmax) {
-      const uint32_t g = vals[r0 + pos];
-      s_sp[threadIdx.x] = stage(means2d, conic_opacity, g);
-      s_ci[threadIdx.x] = make_float4(rgb[3 * (size_t)g], rgb[3 * (size_t)g + 1], rgb[3 * (size_t)g + 2], __uint_as_float(g));
+  for (int s = 0; s < 4; ++s) {
+    const int x = pxi + 8 * (s & 1), y = pyi + 4 * (s >> 1);
+    last[s] = 0; T[s] = 1.f; S0[s] = S1[s] = S2[s] = 0.f; gC0[s] = gC1[s] = gC2[s] = gTfin[s] = 0.f;
+    if (x < W && y < H) {
+      const size_t pix = ((size_t)k * H + y) * W + x;
+      last[s] = n_contrib[pix];
+      T[s] = ct[4 * pix + 3];                // the walk starts from the final transmittance
+      const float4 g = *reinterpret_cast<const float4*>(g_ct + 4 * pix);
+      gC0[s] = g.x; gC1[s] = g.y; gC2[s] = g.z; gTfin[s] = g.w * T[s];
     }
-    __syncthreads();
-    const int jtop = (int)min((uint32_t)BLOCK, bmax - (uint32_t)b * BLOCK) - 1;
-    for (int j = jtop; j >= 0; --j) {
-      const uint32_t c = (uint32_t)b * BLOCK + j + 1;   // 1-based list position, as in n_contrib
-      float dx, dy, G, alpha; bool clamped;
-      const Splat sp = s_sp[j];
-      bool on = (c <= last) && eval_alpha(px, py, sp.xy, sp.con, cfg.alpha_min, cfg.alpha_max, dx, dy, G, alpha, clamped);
-      if (!__any_sync(0xffffffffu, on)) continue;
-      float v[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, v8 = 0.f;
-      const float4 ci = s_ci[j];
-      if (on) {
-        const float om = 1.0f - alpha;
-        const float rom = __fdividef(1.0f, om);
-        T *= rom;                              // T_i = T_{i+1} / (1 - alpha_i)
-        const float w = alpha * T;
-        v[6] = w * gC0; v[7] = w * gC1; v8 = w * gC2;                       // dL/dc_i
-        float dLda = T * (gC0 * (ci.x - S0) + gC1 * (ci.y - S1) + gC2 * (ci.z - S2)) - gTfin * rom;
-        S0 = fmaf(alpha, ci.x - S0, S0); S1 = fmaf(alpha, ci.y - S1, S1); S2 = fmaf(alpha, ci.z - S2, S2);
-        if (!clamped) {
-          const float gG = dLda * G;           // dL/do
-          const float gp = sp.con.w * gG;      // dL/dpower
-          const float gl = gp * LN2;
-          v[0] = gl * fmaf(2.0f * sp.con.x, dx, sp.con.y * dy);   // dL/du
-          v[1] = gl * fmaf(2.0f * sp.con.z, dy, sp.con.y * dx);   // dL/dv
-          v[2] = -0.5f * dx * dx * gp;                             // dL/dA
-          v[3] = -dx * dy * gp;                                    // dL/dB
-          v[4] = -0.5f * dy * dy * gp;                             // dL/dC
-          v[5] = gG;
+    lmax = max(lmax, last[s]);
+  }
+  const uint32_t bmax = __reduce_max_sync(FULL, lmax);
+  if (bmax == 0) return;
+  // per-slot maximum of `last` over the warp: a slot is skipped for list positions beyond it
+  uint32_t smax[4];
+#pragma unroll
+  for (int s = 0; s < 4; ++s) smax[s] = __reduce_max_sync(FULL, last[s]);
+
+  const int nb = (int)((bmax + 31) / 32);
+  int buf = 0;
+  stage_issue(ring, 0, lane, blend, vals, r0 + 32u * (uint32_t)(nb - 1) + lane, r0 + bmax);
+  for (int bi = nb - 1; bi >= 0; --bi, buf ^= 1) {
+    const uint32_t start = 32u * (uint32_t)bi;      // list position (0-based) of entry 0 of this batch
+    if (bi > 0) stage_issue(ring, buf ^ 1, lane, blend, vals, r0 + start - 32 + lane, r0 + bmax);
+    else cp_async_commit();
+    cp_async_wait<1>();
+    __syncwarp();
+    unsigned m = 0;
+    if (start + lane < bmax) m = cull_mask(ring.q[buf][0][lane], ring.q[buf][1][lane], (float)X0, (float)Y0, log2_amin);
+    unsigned reach = 0;                              // slots in which some pixel's walk reaches this batch
+#pragma unroll
+    for (int s = 0; s < 4; ++s) if (smax[s] > start) reach |= 1u << s;
+    m &= reach;
+    unsigned live = __ballot_sync(FULL, m != 0);
+    while (live) {
+      const int j = 31 - __clz(live);
+      live &= ~(1u << j);
+      const uint32_t c1 = start + (uint32_t)j + 1;    // 1-based list position
+      const unsigned mj = __shfl_sync(FULL, m, j);
+      const float4 a = ring.q[buf][0][j], b = ring.q[buf][1][j], c = ring.q[buf][2][j];
+      const float dxs[2] = {__fsub_rn(a.x, px0), __fsub_rn(a.x, px1)};
+      const float dys[2] = {__fsub_rn(a.y, py0), __fsub_rn(a.y, py1)};
+      const float adx[2] = {__fmul_rn(b.x, dxs[0]), __fmul_rn(b.x, dxs[1])};
+      const float bdx[2] = {__fmul_rn(b.y, dxs[0]), __fmul_rn(b.y, dxs[1])};
+      const float cdy[2] = {__fmul_rn(b.z, dys[0]), __fmul_rn(b.z, dys[1])};
+      // moments of dL/dG over this lane's pixels, and the colour sums
+      float n0 = 0.f, nx = 0.f, ny = 0.f, nxx = 0.f, nxy = 0.f, nyy = 0.f, q0 = 0.f, q1 = 0.f, q2 = 0.f;
+      bool any = false;
+#pragma unroll
+      for (int s = 0; s < 4; ++s) {
+        if (!((mj >> s) & 1)) continue;     // warp-uniform
+        const float dx = dxs[s & 1], dy = dys[s >> 1];
+        float G, alpha; bool clamped;
+        const bool on = (c1 <= last[s]) &&
+                        eval_alpha(dx, dy, adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min, cfg.alpha_max, G, alpha, clamped);
+        if (on) {
+          any = true;
+          const float rom = __fdividef(1.0f, 1.0f - alpha);
+          T[s] *= rom;                              // T_i = T_{i+1} / (1 - alpha_i)
+          const float w = alpha * T[s];
+          q0 = fmaf(w, gC0[s], q0); q1 = fmaf(w, gC1[s], q1); q2 = fmaf(w, gC2[s], q2);     // dL/dc_i
+          const float dLda = T[s] * (gC0[s] * (c.x - S0[s]) + gC1[s] * (c.y - S1[s]) + gC2[s] * (c.z - S2[s])) - gTfin[s] * rom;
+          S0[s] = fmaf(alpha, c.x - S0[s], S0[s]); S1[s] = fmaf(alpha, c.y - S1[s], S1[s]); S2[s] = fmaf(alpha, c.z - S2[s], S2[s]);
+          if (!clamped) {
+            const float gG = dLda * G;              // dL/dG-weight of this pixel (dL/do contribution)
+            const float t1 = gG * dx, t2 = gG * dy;
+            n0 += gG; nx += t1; ny += t2;
+            nxx = fmaf(t1, dx, nxx); nxy = fmaf(t1, dy, nxy); nyy = fmaf(t2, dy, nyy);
+          }
         }
       }
+      if (!__any_sync(FULL, any)) continue;
+      // linear map from the moments to the gradients of (u, v, A, B, C, o); alpha = o 2^(A' dx^2 + B' dx dy + C' dy^2)
+      const float go = a.z * LN2;
+      float v[8], v8 = q2;
+      v[0] = go * fmaf(2.0f * b.x, nx, b.y * ny);    // dL/du
+      v[1] = go * fmaf(2.0f * b.z, ny, b.y * nx);    // dL/dv
+      v[2] = -0.5f * a.z * nxx;                      // dL/dA
+      v[3] = -a.z * nxy;                             // dL/dB
+      v[4] = -0.5f * a.z * nyy;                      // dL/dC
+      v[5] = n0;                                     // dL/do
+      v[6] = q0; v[7] = q1;
       const float tot = warp_reduce9(v, v8, lane);
-      const uint32_t g = __float_as_uint(ci.w);
-      float* dst = g2d + (size_t)SPLX_G2D_STRIDE * g;
+      float* dst = g2d + (size_t)SPLX_G2D_STRIDE * __float_as_uint(b.w);
       if ((lane & 3) == 0) {
         const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
         atomicAdd(dst + idx, tot);
@@ -228,7 +351,9 @@ k_raster_bwd(const float* __restrict__ means2d, const float* __restrict__ conic_
         atomicAdd(dst + 8, v8);
       }
     }
+    __syncwarp();
   }
+  cp_async_wait<0>();
 }
 
 }  // namespace
@@ -237,9 +362,12 @@ int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binnin
                       const CamDev& cam, const splx_partial* out, uint64_t* pairs) {
   const int ntiles = cam.TX * cam.TY;
   dim3 grid(ntiles, K);
-  k_render_fwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->means2d, pr->conic_opacity, pr->rgb, pr->depth, bins->vals,
-                                                bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles, ctx->cfg,
-                                                out->ct, out->d, out->n_contrib, (unsigned long long*)pairs);
+  if (pairs)
+    k_render_fwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles,
+                                                        ctx->cfg, out->ct, out->d, out->n_contrib, (unsigned long long*)pairs);
+  else
+    k_render_fwd<false><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles,
+                                                         ctx->cfg, out->ct, out->d, out->n_contrib, nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_render_fwd");
   return SPLX_OK;
 }
@@ -248,9 +376,8 @@ int launch_raster_bwd(splx_ctx* ctx, const splx_projected* pr, const splx_binnin
                       const CamDev& cam, const splx_partial* part, const float* g_ct, float* g2d) {
   const int ntiles = cam.TX * cam.TY;
   dim3 grid(ntiles, K);
-  k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->means2d, pr->conic_opacity, pr->rgb, bins->vals,
-                                                bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles, ctx->cfg,
-                                                part->ct, part->n_contrib, g_ct, g2d);
+  k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles,
+                                                ctx->cfg, part->ct, part->n_contrib, g_ct, g2d);
   SPLX_LAUNCH_CHECK(ctx, "k_raster_bwd");
   return SPLX_OK;
 }

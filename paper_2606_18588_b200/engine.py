@@ -54,7 +54,7 @@ class Trainer:
         self.T_total = torch.empty((self.H, self.W), dtype=torch.float32, device=dev)
         self.g_image = torch.empty((self.H, self.W, 3), dtype=torch.float32, device=dev)
         self.loss_sum = torch.zeros(1, dtype=torch.float64, device=dev)
-        self.pairs = torch.zeros(2, dtype=torch.int64, device=dev)
+        self.pairs = torch.zeros(4, dtype=torch.int64, device=dev)
         self.step_count = 0
         self._cam = None
         self._ws_sort = None
