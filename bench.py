@@ -242,6 +242,8 @@ def run_ours(args):
     M = tr.num_intersections()
     pairs_fwd = int(tr.pairs[0].item())
     pairs_blend = int(tr.pairs[1].item())                          # (pixel, Gaussian) pairs that are blended
+    pairs_eval = int(tr.pairs[2].item())                           # alpha evaluations executed after the exact culling
+    items_fwd = int(tr.pairs[3].item())                            # (Gaussian, half tile) items that survive the culling
     n_contrib = tr.partials.n_contrib
     pairs_bwd = int(n_contrib.to(torch.int64).sum().item())       # list entries the backward re-evaluates
     n_visible = int((tr.proj.radius > 0).sum().item())
@@ -352,7 +354,7 @@ def run_ours(args):
                             views_per_step=1, parallelism=f"replicas x{world} (one GPU per replica, no collective)",
                             l2="working set (params+grads+moments 944 MB at 1M) is larger than the 126 MB L2",
                             intersections=M, visible=n_visible, pairs_fwd=pairs_fwd, pairs_bwd=pairs_bwd,
-                            pairs_blended=pairs_blend),
+                            pairs_blended=pairs_blend, pairs_evaluated_fwd=pairs_eval, half_tile_items_fwd=items_fwd),
                 iters_per_s=world * 1e3 / ms_step, stages_ms=stage_ms, per_kernel=per_kernel, roofline=roof,
                 cpu_baseline=cpu, clocks=clocks, gpu_launches=int(launches),
                 e2e=dict(value=world * W * H / (e2e_ms * 1e-3) / 1e6, unit=UNIT, ms_per_step=e2e_ms,

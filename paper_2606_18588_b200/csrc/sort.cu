@@ -19,21 +19,51 @@ namespace {
 
 constexpr int SCAN_THREADS = 512, SCAN_IPT = 8, SCAN_TILE = SCAN_THREADS * SCAN_IPT;    // 4096
 constexpr int RS_THREADS = 256, RS_IPT = 16, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 4096
+constexpr int MAX_PASSES = 4;
 
 struct Counters {   // device-resident counts, written by kernels, read by later kernels
   uint64_t n_visible;
   uint64_t m_total;     // true number of intersections
   uint64_t m_sorted;    // min(m_total, capacity)
-  uint64_t scratch;
+  uint32_t ticket[16];  // dynamic tile counters, one per single-pass kernel of the pipeline
 };
 
 struct PartOffs { int64_t off[SPLX_MAX_K + 1]; int K; };
 
-// ---------------------------------------------------------------- generic exclusive scan --
-// Three phases over tiles of 4096 values: per-tile sums, scan of the sums (one block), apply.
-// Op supplies load(i) and store(i, value, exclusive_prefix); n is read from device memory.
+// Tile status word of the single-pass ("decoupled look-back") scans: flag in the top two bits,
+// running count below.  A tile publishes its own total (AGG) as soon as it knows it and its
+// inclusive prefix (PREFIX) once it has walked back to a predecessor that published one.
+// Tiles take their index from an atomic ticket, so every predecessor of a running tile has
+// started: the spin below cannot wait on a CTA that was never scheduled.
+constexpr uint64_t ST_AGG = 1ull << 62, ST_PREFIX = 2ull << 62, ST_MASK = 3ull << 62;
 
-__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* smem /*>=32*/, uint32_t& total) {
+__device__ __forceinline__ uint64_t ld_status(const uint64_t* p) {
+  uint64_t v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_status(uint64_t* p, uint64_t v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// exclusive prefix of tile t (t > 0) given its own total: publish, look back, publish again
+__device__ __forceinline__ uint64_t lookback(uint64_t* status, uint32_t t, uint32_t stride, uint64_t total) {
+  st_status(status + (uint64_t)t * stride, ST_AGG | total);
+  uint64_t excl = 0;
+  for (int64_t p = (int64_t)t - 1; p >= 0; --p) {
+    uint64_t v;
+    do { v = ld_status(status + (uint64_t)p * stride); } while ((v & ST_MASK) == 0);
+    excl += v & ~ST_MASK;
+    if ((v & ST_MASK) == ST_PREFIX) break;
+  }
+  st_status(status + (uint64_t)t * stride, ST_PREFIX | (excl + total));
+  return excl;
+}
+
+// ---------------------------------------------------------------- generic exclusive scan --
+// One launch: tiles of 4096 values, chained by look-back.  Op supplies count(), load(i) and
+// store(i, value, exclusive_prefix).  The grand total goes to *total_out (and, clamped, to *clamp_out).
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* smem /*>=33*/, uint32_t& total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   uint32_t inc = v;
 #pragma unroll
@@ -55,58 +85,47 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
 }
 
 template <class Op>
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(Op op, const uint64_t* n_ptr, uint32_t* sums) {
+__global__ void __launch_bounds__(SCAN_THREADS)
+k_scan(Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
+       uint64_t clamp_to) {
   __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_tile;
+  __shared__ uint64_t s_excl;
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+  __syncthreads();
+  const uint32_t t = s_tile;
   const uint64_t n = op.count(n_ptr);
-  const uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
-  uint32_t s = 0;
-#pragma unroll
-  for (int k = 0; k < SCAN_IPT; ++k) if (base + k < n) s += op.load(base + k);
-  uint32_t total;
-  block_exclusive_scan(s, sm, total);
-  if (threadIdx.x == 0) sums[blockIdx.x] = total;
-}
-
-// one block: exclusive scan of sums[0..nb) in place; *total_out = grand total
-__global__ void __launch_bounds__(1024) k_scan_sums(uint32_t* sums, uint32_t nb, uint64_t* total_out,
-                                                    uint64_t* clamp_out, uint64_t clamp_to) {
-  __shared__ uint32_t sm[33];
-  uint32_t carry = 0;
-  for (uint32_t start = 0; start < nb; start += 1024) {
-    const uint32_t i = start + threadIdx.x;
-    const uint32_t v = i < nb ? sums[i] : 0;
-    uint32_t total;
-    const uint32_t ex = block_exclusive_scan(v, sm, total);
-    if (i < nb) sums[i] = carry + ex;
-    carry += total;
+  const uint64_t ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+  if (t >= ntiles) {
+    if (n == 0 && t == 0 && threadIdx.x == 0) {
+      if (total_out) *total_out = 0;
+      if (clamp_out) *clamp_out = 0;
+    }
+    return;
   }
-  if (threadIdx.x == 0) {
-    if (total_out) *total_out = carry;
-    if (clamp_out) *clamp_out = carry < clamp_to ? carry : clamp_to;
-  }
-}
-
-template <class Op>
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(Op op, const uint64_t* n_ptr, const uint32_t* sums) {
-  __shared__ uint32_t sm[33];
-  const uint64_t n = op.count(n_ptr);
-  if ((uint64_t)blockIdx.x * SCAN_TILE >= n) return;
-  const uint64_t base = (uint64_t)blockIdx.x * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
+  const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
   uint32_t v[SCAN_IPT], s = 0;
 #pragma unroll
   for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(base + k) : 0; s += v[k]; }
   uint32_t total;
-  uint32_t ex = block_exclusive_scan(s, sm, total) + sums[blockIdx.x];
+  uint32_t ex = block_exclusive_scan(s, sm, total);
+  if (threadIdx.x == 0) {
+    uint64_t excl = 0;
+    if (t == 0) st_status(status, ST_PREFIX | (uint64_t)total);
+    else excl = lookback(status, t, 1, total);
+    s_excl = excl;
+    if (t + 1 == ntiles) {
+      const uint64_t grand = excl + total;
+      if (total_out) *total_out = grand;
+      if (clamp_out) *clamp_out = grand < clamp_to ? grand : clamp_to;
+    }
+  }
+  __syncthreads();
+  ex += (uint32_t)s_excl;
 #pragma unroll
   for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex); ex += v[k]; }
 }
 
-struct PlainOp {   // in-place exclusive scan of a u32 array of fixed length
-  uint32_t* data; uint64_t n;
-  __device__ uint64_t count(const uint64_t*) const { return n; }
-  __device__ uint32_t load(uint64_t i) const { return data[i]; }
-  __device__ void store(uint64_t i, uint32_t, uint32_t ex) const { data[i] = ex; }
-};
 struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order preserved
   const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n;
   __device__ uint64_t count(const uint64_t*) const { return n; }
@@ -123,67 +142,89 @@ struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, d
 };
 
 template <class Op>
-int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_ptr, uint32_t* sums,
+int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket,
                    uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to) {
   const uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
   if (nb == 0) return SPLX_OK;
-  k_scan_reduce<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, sums);
-  SPLX_LAUNCH_CHECK(ctx, "k_scan_reduce");
-  k_scan_sums<<<1, 1024, 0, ctx->stream>>>(sums, nb, total_out, clamp_out, clamp_to);
-  SPLX_LAUNCH_CHECK(ctx, "k_scan_sums");
-  k_scan_apply<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, sums);
-  SPLX_LAUNCH_CHECK(ctx, "k_scan_apply");
+  k_scan<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to);
+  SPLX_LAUNCH_CHECK(ctx, "k_scan");
   return SPLX_OK;
 }
 
 // ---------------------------------------------------------------------- LSD radix sort --
-// One pass = per-block digit histogram -> exclusive scan over [digit][block] -> stable scatter.
-// Block b always owns positions [b*4096, (b+1)*4096) of the current input buffer.
+// "Onesweep" organisation: the digit histograms of ALL passes are counted in one read of the
+// input (a histogram does not depend on the order), then each pass is ONE kernel: a tile ranks
+// its 4096 keys (stable, warp multisplit with __match_any_sync), chains its per-digit counts to
+// its predecessors by look-back (256 independent chains, one per thread) and scatters.
+// Per item and pass: key+value read once and written once (24 B for 64-bit keys, 16 B for 32-bit).
 
-template <typename KeyT>
-__global__ void __launch_bounds__(RS_THREADS)
-k_radix_hist(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t* __restrict__ ghist,
-             int shift, int bits, uint32_t nblocks) {
-  __shared__ uint32_t hist[256];
-  const uint64_t n = *n_ptr;
-  const uint32_t radix = 1u << bits, mask = radix - 1;
-  hist[threadIdx.x] = 0;
-  __syncthreads();
-  const uint64_t start = (uint64_t)blockIdx.x * RS_TILE;
-  if (start < n) {
-    const int lane = threadIdx.x & 31;
-#pragma unroll 4
-    for (int it = 0; it < RS_IPT; ++it) {
-      const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
-      const bool valid = idx < n;
-      const unsigned vm = __ballot_sync(0xffffffffu, valid);
-      if (valid) {
-        const uint32_t d = (uint32_t)(keys[idx] >> shift) & mask;
-        const unsigned peers = __match_any_sync(vm, d);   // aggregate equal digits in the warp
-        if (lane == __ffs(peers) - 1) atomicAdd(&hist[d], __popc(peers));
-      }
-    }
+struct PassPlan { int npass; int shift[MAX_PASSES]; int bits[MAX_PASSES]; };
+
+static PassPlan plan_passes(int begin_bit, int end_bit) {
+  PassPlan p;
+  const int total = end_bit - begin_bit;
+  p.npass = (total + 7) / 8;
+  int shift = begin_bit;
+  for (int i = 0; i < p.npass; ++i) {
+    p.bits[i] = (total + p.npass - 1 - i) / p.npass;   // spread the bits evenly over the passes
+    p.shift[i] = shift;
+    shift += p.bits[i];
   }
-  __syncthreads();
-  if (threadIdx.x < radix) ghist[(uint64_t)threadIdx.x * nblocks + blockIdx.x] = hist[threadIdx.x];
+  return p;
 }
 
 template <typename KeyT>
 __global__ void __launch_bounds__(RS_THREADS)
-k_radix_scatter(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
-                uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ gbase,
-                int shift, int bits, uint32_t nblocks) {
-  __shared__ uint32_t whist[RS_WARPS][256];
-  __shared__ uint32_t dbase[256];
+k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t* __restrict__ ghist /*[npass][256]*/,
+                 PassPlan plan) {
+  __shared__ uint32_t hist[MAX_PASSES][256];
   const uint64_t n = *n_ptr;
   const uint64_t start = (uint64_t)blockIdx.x * RS_TILE;
   if (start >= n) return;
-  const uint32_t radix = 1u << bits, mask = radix - 1;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int p = 0; p < MAX_PASSES; ++p) hist[p][threadIdx.x] = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+#pragma unroll 4
+  for (int it = 0; it < RS_IPT; ++it) {
+    const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
+    const bool valid = idx < n;
+    const unsigned vm = __ballot_sync(0xffffffffu, valid);
+    if (valid) {
+      const KeyT key = keys[idx];
+      for (int p = 0; p < plan.npass; ++p) {
+        const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
+        const unsigned peers = __match_any_sync(vm, d);   // aggregate equal digits in the warp
+        if (lane == __ffs(peers) - 1) atomicAdd(&hist[p][d], __popc(peers));
+      }
+    }
+  }
+  __syncthreads();
+  for (int p = 0; p < plan.npass; ++p) {
+    const uint32_t c = hist[p][threadIdx.x];
+    if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c);
+  }
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
+             uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
+             uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits) {
+  __shared__ uint32_t whist[RS_WARPS][256];
+  __shared__ uint32_t dbase[256];
+  __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_tile;
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
 #pragma unroll
   for (int w = 0; w < RS_WARPS; ++w) whist[w][threadIdx.x] = 0;
-  if (threadIdx.x < radix) dbase[threadIdx.x] = gbase[(uint64_t)threadIdx.x * nblocks + blockIdx.x];
   __syncthreads();
+  const uint32_t t = s_tile;
+  const uint64_t n = *n_ptr;
+  const uint64_t start = (uint64_t)t * RS_TILE;
+  if (start >= n) return;
+  const uint32_t mask = (1u << bits) - 1u;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   // warp w owns the contiguous segment [start + w*512, +512); iteration `it` covers 32 consecutive
   // positions, so (it, lane) is the input order and the ranks below are stable.
   const uint64_t seg = start + (uint64_t)warp * (32 * RS_IPT);
@@ -193,11 +234,15 @@ k_radix_scatter(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, 
 #pragma unroll
   for (int it = 0; it < RS_IPT; ++it) {
     const uint64_t idx = seg + (uint64_t)it * 32 + lane;
+    key[it] = idx < n ? kin[idx] : (KeyT)0;
+  }
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    const uint64_t idx = seg + (uint64_t)it * 32 + lane;
     const bool valid = idx < n;
     const unsigned vm = __ballot_sync(0xffffffffu, valid);
-    key[it] = 0; rank[it] = 0;
+    rank[it] = 0;
     if (valid) {
-      key[it] = kin[idx];
       const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
       const unsigned peers = __match_any_sync(vm, d);
       const int leader = __ffs(peers) - 1;
@@ -209,11 +254,19 @@ k_radix_scatter(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, 
     __syncwarp();
   }
   __syncthreads();
-  {  // exclusive prefix over the warps, per digit
+  {  // per digit: exclusive prefix over the warps, tile total, chained prefix over the tiles
     const int d = threadIdx.x;
     uint32_t run = 0;
 #pragma unroll
     for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
+    // exclusive scan of the global digit histogram = first output position of digit d
+    uint32_t tot;
+    const uint32_t gexcl = block_exclusive_scan(ghist[d], sm, tot);
+    uint64_t excl = 0;
+    uint64_t* st = status + d;
+    if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
+    else excl = lookback(st, t, 256, run);
+    dbase[d] = gexcl + (uint32_t)excl;
   }
   __syncthreads();
 #pragma unroll
@@ -228,28 +281,22 @@ k_radix_scatter(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, 
   }
 }
 
-// Sorts bits [begin_bit, end_bit) in passes of <= 8 bits.  Input in (ka, va); buffers alternate;
-// returns the number of passes (result is in (ka, va) if even, (kb, vb) if odd).
-static int radix_passes(int begin_bit, int end_bit) { return (end_bit - begin_bit + 7) / 8; }
-
+// Sorts bits [begin_bit, end_bit) in passes of <= 8 bits.  Input in (ka, va); buffers alternate
+// (result in (ka, va) after an even number of passes, (kb, vb) after an odd number).
+// ghist: [MAX_PASSES][256] u32, status: [npass][tiles][256] u64, both zeroed by the caller.
 template <typename KeyT>
 int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
-               const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* hist, uint32_t* sums) {
+               const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets) {
   const uint32_t nblocks = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
   if (nblocks == 0) return SPLX_OK;
-  const int passes = radix_passes(begin_bit, end_bit);
-  const int total = end_bit - begin_bit;
-  int shift = begin_bit;
-  for (int p = 0; p < passes; ++p) {
-    const int bits = (total + passes - 1 - p) / passes;  // spread the bits evenly over the passes
-    k_radix_hist<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, hist, shift, bits, nblocks);
-    SPLX_LAUNCH_CHECK(ctx, "k_radix_hist");
-    PlainOp op{hist, (uint64_t)nblocks << bits};
-    int rc = scan_exclusive(ctx, op, op.n, nullptr, sums, nullptr, nullptr, 0);
-    if (rc) return rc;
-    k_radix_scatter<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, hist, shift, bits, nblocks);
-    SPLX_LAUNCH_CHECK(ctx, "k_radix_scatter");
-    shift += bits;
+  const PassPlan plan = plan_passes(begin_bit, end_bit);
+  k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, plan);
+  SPLX_LAUNCH_CHECK(ctx, "k_radix_hist_all");
+  for (int p = 0; p < plan.npass; ++p) {
+    k_radix_pass<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
+                                                               status + (size_t)p * nblocks * 256, tickets + p,
+                                                               plan.shift[p], plan.bits[p]);
+    SPLX_LAUNCH_CHECK(ctx, "k_radix_pass");
     KeyT* tk = ka; ka = kb; kb = tk;
     uint32_t* tv = va; va = vb; vb = tv;
   }
@@ -323,8 +370,11 @@ k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, uint32_t* 
 
 __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_total; }
 
+// Workspace: a zero-initialised control region (counters, tickets, digit histograms, look-back
+// status words: one memset per call) followed by the sort buffers.
 struct Layout {
-  size_t counters, ckeys_a, cvals_a, ckeys_b, cvals_b, offs, keys_tmp, vals_tmp, hist, sums, total;
+  size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes;
+  size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, keys_tmp, vals_tmp, total;
 };
 
 static int slot_bits(int K, int TX, int TY) {
@@ -334,20 +384,24 @@ static int slot_bits(int K, int TX, int TY) {
   return b;
 }
 
-static Layout make_layout(int64_t n, uint64_t capacity) {
+static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   Layout L;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  const size_t tiles_n = ((size_t)n + RS_TILE - 1) / RS_TILE, tiles_m = ((size_t)capacity + RS_TILE - 1) / RS_TILE;
+  const size_t scan_n = ((size_t)n + SCAN_TILE - 1) / SCAN_TILE;
   L.counters = take(sizeof(Counters));
+  L.ghist_d = take(MAX_PASSES * 256 * 4);
+  L.ghist_s = take(MAX_PASSES * 256 * 4);
+  L.st_scan_v = take(scan_n * 8);
+  L.st_scan_t = take(scan_n * 8);
+  L.st_depth = take(4 * tiles_n * 256 * 8);
+  L.st_slot = take((size_t)((sbits + 7) / 8) * tiles_m * 256 * 8);
+  L.zero_bytes = off;
   L.ckeys_a = take((size_t)n * 4); L.cvals_a = take((size_t)n * 4);
   L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
   L.offs = take((size_t)n * 4);
   L.keys_tmp = take((size_t)capacity * 8); L.vals_tmp = take((size_t)capacity * 4);
-  const uint64_t big = (uint64_t)n > capacity ? (uint64_t)n : capacity;
-  const uint64_t nblocks = (big + RS_TILE - 1) / RS_TILE;
-  L.hist = take((size_t)nblocks * 256 * 4);
-  const uint64_t scan_len = nblocks * 256 > big ? nblocks * 256 : big;
-  L.sums = take(((size_t)(scan_len + SCAN_TILE - 1) / SCAN_TILE + 1) * 4);
   L.total = off;
   return L;
 }
@@ -355,13 +409,14 @@ static Layout make_layout(int64_t n, uint64_t capacity) {
 }  // namespace
 
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY) {
-  (void)K; (void)TX; (void)TY;
-  return make_layout(n, capacity).total;
+  return make_layout(n, capacity, slot_bits(K, TX, TY)).total;
 }
 
 int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, const int64_t* part_offsets,
                     const CamDev& cam, const splx_binning* out, void* ws, size_t ws_bytes) {
-  const Layout L = make_layout(n, out->capacity);
+  const int sbits = slot_bits(K, cam.TX, cam.TY);
+  if (sbits > 8 * MAX_PASSES) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles needs %d key bits (max 32)", sbits);
+  const Layout L = make_layout(n, out->capacity, sbits);
   if (ws_bytes < L.total)
     SPLX_FAIL(ctx, SPLX_ERR_WORKSPACE, "splx_bin_sort: workspace %zu B < required %zu B", ws_bytes, L.total);
   char* base = (char*)ws;
@@ -370,10 +425,9 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, c
   uint32_t* ckeys_b = (uint32_t*)(base + L.ckeys_b); uint32_t* cvals_b = (uint32_t*)(base + L.cvals_b);
   uint32_t* offs = (uint32_t*)(base + L.offs);
   uint64_t* keys_tmp = (uint64_t*)(base + L.keys_tmp); uint32_t* vals_tmp = (uint32_t*)(base + L.vals_tmp);
-  uint32_t* hist = (uint32_t*)(base + L.hist); uint32_t* sums = (uint32_t*)(base + L.sums);
   const int ntiles = cam.TX * cam.TY;
 
-  SPLX_CUDA_OK(ctx, cudaMemsetAsync(cnt, 0, sizeof(Counters), ctx->stream));
+  SPLX_CUDA_OK(ctx, cudaMemsetAsync(base, 0, L.zero_bytes, ctx->stream));
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->tile_ranges, 0, (size_t)K * ntiles * 2 * sizeof(uint32_t), ctx->stream));
   if (n == 0 || out->capacity == 0) {
     k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
@@ -383,14 +437,16 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, c
   int rc;
   // 1. visible Gaussians, index order
   VisibleOp vop{pr->tiles_touched, pr->depth, ckeys_a, cvals_a, (uint64_t)n};
-  if ((rc = scan_exclusive(ctx, vop, (uint64_t)n, nullptr, sums, &cnt->n_visible, nullptr, 0))) return rc;
+  if ((rc = scan_exclusive(ctx, vop, (uint64_t)n, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
+                           &cnt->n_visible, nullptr, 0))) return rc;
   // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers)
-  if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n, &cnt->n_visible, 0, 32, hist, sums))) return rc;
+  if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n, &cnt->n_visible, 0, 32,
+                                 (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2]))) return rc;
   // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
-  if ((rc = scan_exclusive(ctx, top, (uint64_t)n, &cnt->n_visible, sums, &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
-  const int sbits = slot_bits(K, cam.TX, cam.TY);
-  const int passes = radix_passes(32, 32 + sbits);
+  if ((rc = scan_exclusive(ctx, top, (uint64_t)n, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
+                           &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
+  const int passes = (sbits + 7) / 8;
   uint64_t* k0 = (passes & 1) ? keys_tmp : out->keys;   // so that the last pass lands in out->keys
   uint32_t* v0 = (passes & 1) ? vals_tmp : out->vals;
   uint64_t* k1 = (passes & 1) ? out->keys : keys_tmp;
@@ -402,7 +458,8 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, c
       pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
   // 4. stable sort on the slot bits
-  if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits, hist, sums))) return rc;
+  if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
+                                 (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6]))) return rc;
   // 5. ranges
   k_tile_ranges<<<(unsigned)((out->capacity + 255) / 256), 256, 0, ctx->stream>>>(out->keys, cnt, out->tile_ranges);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
