@@ -37,6 +37,11 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ float lg2_approx(float x) {
   float y;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -317,7 +322,7 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
                         eval_alpha(dx, dy, adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min, cfg.alpha_max, G, alpha, clamped);
         if (on) {
           any = true;
-          const float rom = __fdividef(1.0f, 1.0f - alpha);
+          const float rom = rcp_approx(1.0f - alpha);          // 1 - alpha >= 1 - alpha_max > 0
           T[s] *= rom;                              // T_i = T_{i+1} / (1 - alpha_i)
           const float w = alpha * T[s];
           q0 = fmaf(w, gC0[s], q0); q1 = fmaf(w, gC1[s], q1); q2 = fmaf(w, gC2[s], q2);     // dL/dc_i

@@ -17,8 +17,8 @@
 
 namespace {
 
-constexpr int SCAN_THREADS = 512, SCAN_IPT = 8, SCAN_TILE = SCAN_THREADS * SCAN_IPT;    // 4096
-constexpr int RS_THREADS = 256, RS_IPT = 16, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 4096
+constexpr int SCAN_THREADS = 512, SCAN_IPT = 4, SCAN_TILE = SCAN_THREADS * SCAN_IPT;
+constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
 
 struct Counters {   // device-resident counts, written by kernels, read by later kernels
@@ -45,15 +45,31 @@ __device__ __forceinline__ uint64_t ld_status(const uint64_t* p) {
 __device__ __forceinline__ void st_status(uint64_t* p, uint64_t v) {
   asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-// exclusive prefix of tile t (t > 0) given its own total: publish, look back, publish again
+// exclusive prefix of tile t (t > 0) given its own total: publish, look back, publish again.
+// The walk reads W predecessors per round trip (independent loads), consumes them nearest first
+// and stops at the first PREFIX; a predecessor that has published nothing yet ends the round.
+template <int W>
 __device__ __forceinline__ uint64_t lookback(uint64_t* status, uint32_t t, uint32_t stride, uint64_t total) {
   st_status(status + (uint64_t)t * stride, ST_AGG | total);
   uint64_t excl = 0;
-  for (int64_t p = (int64_t)t - 1; p >= 0; --p) {
-    uint64_t v;
-    do { v = ld_status(status + (uint64_t)p * stride); } while ((v & ST_MASK) == 0);
-    excl += v & ~ST_MASK;
-    if ((v & ST_MASK) == ST_PREFIX) break;
+  int64_t p = (int64_t)t - 1;
+  while (p >= 0) {
+    uint64_t v[W];
+#pragma unroll
+    for (int i = 0; i < W; ++i) v[i] = (p - i >= 0) ? ld_status(status + (uint64_t)(p - i) * stride) : ST_PREFIX;
+    bool done = false;
+    int used = 0;
+#pragma unroll
+    for (int i = 0; i < W; ++i) {
+      if (!done && used == i && (v[i] & ST_MASK) != 0) {
+        excl += v[i] & ~ST_MASK;
+        ++used;
+        if ((v[i] & ST_MASK) == ST_PREFIX) done = true;
+      }
+    }
+    if (done) break;
+    p -= used;
+    if (used == 0) __nanosleep(20);
   }
   st_status(status + (uint64_t)t * stride, ST_PREFIX | (excl + total));
   return excl;
@@ -112,7 +128,7 @@ k_scan(Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_
   if (threadIdx.x == 0) {
     uint64_t excl = 0;
     if (t == 0) st_status(status, ST_PREFIX | (uint64_t)total);
-    else excl = lookback(status, t, 1, total);
+    else excl = lookback<16>(status, t, 1, total);
     s_excl = excl;
     if (t + 1 == ntiles) {
       const uint64_t grand = excl + total;
@@ -173,35 +189,51 @@ static PassPlan plan_passes(int begin_bit, int end_bit) {
   return p;
 }
 
+// Lanes of the warp whose 8-bit digit equals this lane's, among the lanes of `vm`: eight ballots.
+// (Constant cost; the hardware MATCH.ANY serialises over the distinct values and the shared-memory
+// atomic unit over the lanes -- profiles/r01c.)
+__device__ __forceinline__ unsigned digit_peers(uint32_t d, unsigned vm) {
+  unsigned peers = vm;
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    const bool bit = (d >> b) & 1u;
+    const unsigned bal = __ballot_sync(0xffffffffu, bit);
+    peers &= bit ? bal : ~bal;
+  }
+  return peers;
+}
+
 template <typename KeyT>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t* __restrict__ ghist /*[npass][256]*/,
                  PassPlan plan) {
-  __shared__ uint32_t hist[MAX_PASSES][256];
+  __shared__ uint32_t hist[RS_WARPS][MAX_PASSES][256];   // warp-private: plain read-modify-write by group leaders
   const uint64_t n = *n_ptr;
   const uint64_t start = (uint64_t)blockIdx.x * RS_TILE;
   if (start >= n) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int p = 0; p < plan.npass; ++p)
 #pragma unroll
-  for (int p = 0; p < MAX_PASSES; ++p) hist[p][threadIdx.x] = 0;
+    for (int w = 0; w < RS_WARPS; ++w) hist[w][p][threadIdx.x] = 0;
   __syncthreads();
-  const int lane = threadIdx.x & 31;
-#pragma unroll 4
+#pragma unroll 2
   for (int it = 0; it < RS_IPT; ++it) {
     const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
     const bool valid = idx < n;
     const unsigned vm = __ballot_sync(0xffffffffu, valid);
-    if (valid) {
-      const KeyT key = keys[idx];
-      for (int p = 0; p < plan.npass; ++p) {
-        const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
-        const unsigned peers = __match_any_sync(vm, d);   // aggregate equal digits in the warp
-        if (lane == __ffs(peers) - 1) atomicAdd(&hist[p][d], __popc(peers));
-      }
+    const KeyT key = valid ? keys[idx] : (KeyT)0;
+    for (int p = 0; p < plan.npass; ++p) {
+      const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
+      const unsigned peers = digit_peers(d, vm);
+      if (valid && lane == __ffs(peers) - 1) hist[warp][p][d] += __popc(peers);
+      __syncwarp();
     }
   }
   __syncthreads();
   for (int p = 0; p < plan.npass; ++p) {
-    const uint32_t c = hist[p][threadIdx.x];
+    uint32_t c = 0;
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; ++w) c += hist[w][p][threadIdx.x];
     if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c);
   }
 }
@@ -241,16 +273,13 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
     const uint64_t idx = seg + (uint64_t)it * 32 + lane;
     const bool valid = idx < n;
     const unsigned vm = __ballot_sync(0xffffffffu, valid);
-    rank[it] = 0;
-    if (valid) {
-      const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
-      const unsigned peers = __match_any_sync(vm, d);
-      const int leader = __ffs(peers) - 1;
-      uint32_t old = 0;
-      if (lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
-      old = __shfl_sync(peers, old, leader);
-      rank[it] = old + __popc(peers & lt);
-    }
+    const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
+    const unsigned peers = digit_peers(d, vm);
+    const int leader = valid ? __ffs(peers) - 1 : lane;
+    uint32_t old = 0;
+    if (valid && lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
+    old = __shfl_sync(0xffffffffu, old, leader);
+    rank[it] = old + __popc(peers & lt);
     __syncwarp();
   }
   __syncthreads();
@@ -265,7 +294,7 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
     uint64_t excl = 0;
     uint64_t* st = status + d;
     if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
-    else excl = lookback(st, t, 256, run);
+    else excl = lookback<8>(st, t, 256, run);
     dbase[d] = gexcl + (uint32_t)excl;
   }
   __syncthreads();
