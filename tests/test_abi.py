@@ -45,7 +45,7 @@ def test_struct_sizes_match_the_header(libpath):
     from paper_2606_18588_b200 import binding as b
     assert ctypes.sizeof(b.Config) == 24
     assert ctypes.sizeof(b.CameraS) == 4 * (9 + 3 + 4) + 8 + 4
-    assert ctypes.sizeof(b.GaussiansS) == 48 and ctypes.sizeof(b.ProjectedS) == 56
+    assert ctypes.sizeof(b.GaussiansS) == 48 and ctypes.sizeof(b.ProjectedS) == 64
     assert ctypes.sizeof(b.BinningS) == 40 and ctypes.sizeof(b.PartialS) == 24
 
 
