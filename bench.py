@@ -36,6 +36,9 @@ FLOPS_BLEND_FWD = 12  # one contributing pair in the forward: Eq.3-4 accumulatio
 FLOPS_BLEND_BWD = 55  # one contributing pair in the backward incl. its 9 reduction adds
 FP32_LANES_PER_SM = 128
 SM_COUNT = 148
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on aerial_1M, from the `ncu --set full` capture summarised in
+# profiles/r01b_ncu_full.csv (a profiler number, copied here by hand; null for other workloads)
+NCU_TRAFFIC_BYTES = {"aerial_1M": {"k_raster_bwd": 218.1e6, "k_render_fwd": 211.3e6, "adam": 1596.8e6, "project_backward": 520.4e6}}
 
 
 def workload(name):
@@ -316,16 +319,16 @@ def run_ours(args):
     if dom == "raster_backward":
         ach = flops_bwd / (stage_ms[dom] * 1e-3) / 1e12
         roof = dict(kernel="k_raster_bwd", bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak,
-                    traffic=None, peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} clock)")
+                    traffic=NCU_TRAFFIC_BYTES.get(args.workload, {}).get("k_raster_bwd"), peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} clock)")
     elif dom == "render_partial":
         ach = flops_fwd / (stage_ms[dom] * 1e-3) / 1e12
         roof = dict(kernel="k_render_fwd", bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak,
-                    traffic=None, peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} clock)")
+                    traffic=NCU_TRAFFIC_BYTES.get(args.workload, {}).get("k_render_fwd"), peak_source=f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['source']} clock)")
     else:
         b = hbm_bytes.get(dom, 0)
         ach = b / (stage_ms[dom] * 1e-3) / 1e9
         roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
-                    traffic=None, peak_source=pk["source"])
+                    traffic=NCU_TRAFFIC_BYTES.get(args.workload, {}).get(dom), peak_source=pk["source"])
     per_kernel = {}
     for n, b in hbm_bytes.items():
         gbs = b / (stage_ms[n] * 1e-3) / 1e9
