@@ -190,20 +190,21 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------- CUDA path --
 def run_ours(args):
     import torch
-    import torch.distributed as dist
+    from paper_2606_18588_b200 import replicas
     from paper_2606_18588_b200.engine import Trainer
-    from paper_2606_18588_b200.scenes import PARAM_KEYS
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = replicas.world_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    replicas.init("nccl", local)
     sc = workload(args.workload)
     cam = sc.cameras[0]
+    if world > 1:   # every replica trains on its own seeded view of the same scene (weak scaling)
+        from paper_2606_18588_b200 import scenes as _sc
+        yaw = float(np.random.default_rng(replicas.replica_view_seed(2, rank)).uniform(0, 360))
+        if args.workload == "aerial_1M":
+            cam = _sc.aerial_camera(cam.width, cam.height, 60.0, 80.0, 45.0, yaw)
     W, H = cam.width, cam.height
     cap = {"aerial_1M": 6_000_000}.get(args.workload)
     tr = Trainer(sc.params, sc.part_offsets, W, H, sc.sh_degree, sc.bg, capacity=cap, device=local)
@@ -232,10 +233,7 @@ def run_ours(args):
         rec(9)
 
     def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(cuda=True)
 
     # unit counts of this view (outside the timed region): pair evaluations and intersections
     tr.pairs.zero_()
@@ -267,10 +265,7 @@ def run_ours(args):
     if sampler: sampler.mark()
     launches = c.launch_count() - l0
     ms_total = e0.elapsed_time(e1)
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_step = float(tmax.item()) / args.steps
+    ms_step = replicas.max_over_ranks(ms_total, cuda=True) / args.steps
     stage_ms = {n: statistics.mean(evs[s][i].elapsed_time(evs[s][i + 1]) for s in range(args.steps))
                 for i, n in enumerate(STAGES)}
     clocks = sampler.stop() if sampler else None
@@ -297,13 +292,9 @@ def run_ours(args):
     for _ in range(n_e2e):
         step_e2e()
     barrier()
-    e2e_ms = torch.tensor([(time.perf_counter() - t0) * 1e3 / n_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
-    e2e_ms = float(e2e_ms.item())
+    e2e_ms = replicas.max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e, cuda=True)
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        replicas.finish()
         return
 
     pk = peaks()
@@ -364,8 +355,7 @@ def run_ours(args):
                          h2d_bytes_per_step=int(tgt_host.numel() * 4),
                          d2h_bytes_per_step=int(img_host.numel() * 4 + 8)))
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.finish()
 
 
 def main():

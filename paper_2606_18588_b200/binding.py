@@ -146,6 +146,8 @@ def gaussians_struct(p: dict, cls=GaussiansS):
 class Projected:
     def __init__(self, n, device):
         f = dict(dtype=torch.float32, device=device)
+        self.n = n
+        n = max(n, 1)            # keep every pointer non-null for an empty scene
         self.means2d = torch.empty((n, 2), **f)
         self.depth = torch.empty(n, **f)
         self.conic_opacity = torch.empty((n, 4), **f)
@@ -154,7 +156,6 @@ class Projected:
         self.tiles_touched = torch.empty(n, dtype=torch.int32, device=device)  # uint32 bits
         self.clamp = torch.empty(n, dtype=torch.uint8, device=device)
         self.blend = torch.empty((n, BLEND_STRIDE), **f)
-        self.n = n
 
     def struct(self):
         return ProjectedS(_ptr(self.means2d), _ptr(self.depth), _ptr(self.conic_opacity), _ptr(self.rgb),

@@ -38,7 +38,7 @@ class Trainer:
         self.lr = dict(DEFAULT_LR if lr is None else lr)
         offs, total = _flat_layout(self.n)
         self._offs, self._total = offs, total
-        self.flat = {name: torch.zeros(total, dtype=torch.float32, device=dev) for name in ("param", "grad", "m", "v")}
+        self.flat = {name: torch.zeros(max(total, 4), dtype=torch.float32, device=dev) for name in ("param", "grad", "m", "v")}
         self.params, self.grads, self.m, self.v = ({}, {}, {}, {})
         for name, views in (("param", self.params), ("grad", self.grads), ("m", self.m), ("v", self.v)):
             for k in PARAM_KEYS:

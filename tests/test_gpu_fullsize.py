@@ -1,0 +1,131 @@
+"""-m gpu parity at BASELINE.json's full size, in the launch configuration bench.py times
+(aerial_1M = configs[1]: 1M Gaussians, SH3, 1920x1080, K = 4, capacity 6M).  The oracle cannot
+render the whole frame in seconds, so: the integer stages are compared in full (bit-exact keys,
+values, ranges: the oracle's bin_sort on 1M Gaussians takes seconds), the pixel stages on a seeded
+sample of tiles (teacher-forced lists), the gradients on every Gaussian those tiles touch."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_18588_b200 import scenes
+from paper_2606_18588_b200.engine import Trainer
+from tests import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+N_TILES = 48
+
+
+@pytest.fixture(scope="module")
+def full():
+    sc = scenes.aerial()
+    cam = sc.cameras[0]
+    tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=6_000_000)
+    tr.forward(cam, count_pairs=True)
+    torch.cuda.synchronize()
+    return sc, cam, tr
+
+
+def _tile_mask(tiles, W, H):
+    TX = (W + 15) // 16
+    m = np.zeros((H, W), bool)
+    for t in tiles:
+        y0, x0 = (t // TX) * 16, (t % TX) * 16
+        m[y0:y0 + 16, x0:x0 + 16] = True
+    return m
+
+
+def test_fullsize_binning_bit_exact(full):
+    sc, cam, tr = full
+    pr = G.gpu_projected(tr)
+    M, keys, vals, ranges = G.gpu_bins(tr)
+    M_ref, tt_ref = oracle.count_tiles(pr.means2d, pr.radius, cam.width, cam.height)
+    assert M == M_ref and np.array_equal(pr.tiles_touched, tt_ref)
+    ntiles = ranges.shape[1]
+    pos = 0
+    for k in range(tr.K):
+        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        ob = oracle.bin_sort(pr.means2d[a:b], pr.radius[a:b], pr.depth[a:b], cam.width, cam.height)
+        seg = keys[pos:pos + ob.M]
+        assert np.array_equal(seg, ob.keys + (np.uint64(k * ntiles) << np.uint64(32)))
+        assert np.array_equal(vals[pos:pos + ob.M], ob.vals + np.uint32(a))
+        live = ob.ranges[:, 1] > ob.ranges[:, 0]
+        assert np.array_equal(ranges[k][live], ob.ranges[live] + np.uint32(pos))
+        assert not ranges[k][~live].any()
+        pos += ob.M
+    assert pos == M
+
+
+def test_fullsize_projection_sampled(full):
+    sc, cam, tr = full
+    rng = np.random.default_rng(21)
+    idx = np.sort(rng.choice(sc.N, 20000, replace=False))
+    p = {k: sc.params[k][idx] for k in scenes.PARAM_KEYS}
+    ref = oracle.project(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sc.sh_degree, cam.as_array())
+    pr = G.gpu_projected(tr)
+    m = (ref.radius > 0) & (pr.radius[idx] == ref.radius)
+    assert m.sum() >= 0.999 * (ref.radius > 0).sum()
+    assert G.close(pr.depth[idx][m], ref.depth[m]).all()
+    assert G.close(pr.rgb[idx][m], ref.rgb[m]).all()
+    assert (np.abs(pr.means2d[idx][m] - ref.means2d[m]) <= 4 * 2.0 ** -23 * 1920 + 1e-5 * np.abs(ref.means2d[m])).all()
+
+
+def test_fullsize_pixels_and_gradients_on_sampled_tiles(full):
+    sc, cam, tr = full
+    W, H = cam.width, cam.height
+    TX, TY = (W + 15) // 16, (H + 15) // 16
+    tiles = np.sort(np.random.default_rng(22).choice(TX * TY, N_TILES, replace=False)).astype(np.int32)
+    mask = _tile_mask(tiles, W, H)
+    pr = G.gpu_projected(tr)
+    M, keys, vals, ranges = G.gpu_bins(tr)
+    ct_gpu = G.np32(tr.partials.ct).astype(np.float64)
+    d_gpu = G.np32(tr.partials.d).astype(np.float64)
+    # a5 on the sampled tiles, lists teacher-forced from the GPU binning (checked bit-exact above)
+    refs, frag = [], np.zeros((H, W), bool)
+    for k in range(tr.K):
+        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        lv = (vals - np.uint32(a)).astype(np.uint32)      # local indices; entries of other partitions are never addressed
+        ref = oracle.render_partial(pr.means2d[a:b], pr.conic_opacity[a:b], pr.rgb[a:b], pr.depth[a:b], lv, ranges[k],
+                                    W, H, tile_list=tiles)
+        refs.append(ref)
+        fk = (ref.margin < G.FRAGILE_MARGIN) & mask
+        frag |= fk
+        ok = G.close(ct_gpu[k], ref.ct).all(-1) & G.close(d_gpu[k], ref.d)
+        assert (ok | fk | ~mask).all(), f"partition {k}"
+    assert frag.sum() <= 4e-3 * mask.sum() * tr.K
+    # a6 / a8 on the same tiles from the GPU partials
+    img, Tt, _, om = oracle.compose(ct_gpu, d_gpu, tr.bg, tiles)
+    robust = mask & ~(om < 1e-6)
+    assert G.close(G.np32(tr.image), img).all(-1)[robust].all()
+    assert G.close(G.np32(tr.T_total), Tt)[robust].all()
+    # backward: dL/dimage non-zero on the sampled tiles only (robust, non-fragile pixels)
+    g_img = np.zeros((H, W, 3), np.float32)
+    sel = robust & ~frag
+    g_img[sel] = np.random.default_rng(23).standard_normal((int(sel.sum()), 3)).astype(np.float32)
+    tr.backward(g_image=torch.from_numpy(g_img).cuda(), overwrite=True)
+    torch.cuda.synchronize()
+    g_ct = oracle.compose_bwd(ct_gpu, d_gpu, g_img, tr.bg, None, tiles)
+    for k in range(tr.K):
+        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        lv = (vals - np.uint32(a)).astype(np.uint32)
+        g2 = oracle.raster_bwd(pr.means2d[a:b], pr.conic_opacity[a:b], pr.rgb[a:b], lv, ranges[k], W, H, g_ct[k],
+                               tile_list=tiles)
+        p = sc.partition(k)
+        ref = oracle.project_bwd(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sc.sh_degree,
+                                 cam.as_array(), pr.radius[a:b], pr.clamp[a:b], *g2)
+        for key in scenes.PARAM_KEYS:
+            w = scenes.PARAM_WIDTH[key]
+            got = G.np32(tr.grads[key]).reshape(-1, w)[a:b].astype(np.float64)
+            r = ref[key].reshape(-1, w)
+            assert np.abs(r).max() > 0, key
+            assert G.rel_l2(got, r) <= 1e-3, (k, key, G.rel_l2(got, r))
+            assert G.grad_close(got, r) <= 5e-3, (k, key)
+
+
+def test_fullsize_work_counters(full):
+    sc, cam, tr = full
+    walked, blended, evaluated, items = [int(x) for x in tr.pairs.tolist()]
+    assert walked > 5e8 and 0 < blended < evaluated <= walked and items > 0
+    n_contrib = tr.partials.n_contrib.to(torch.int64)
+    assert int(n_contrib.sum().item()) <= walked
