@@ -77,6 +77,7 @@ int64_t splx_launch_count(const splx_ctx* ctx) { return ctx ? ctx->launches : -1
 int splx_project(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
                  const splx_projected* out) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (g && g->n == 0) return SPLX_OK;   // empty scene: nothing to write
   if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: null/misaligned argument");
   if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: sh_degree %d not in [0,3]", sh_degree);
   return launch_project_fwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, out);
@@ -164,6 +165,7 @@ int splx_raster_backward(splx_ctx* ctx, const splx_projected* proj, const splx_b
 int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
                           const splx_projected* proj, float* g2d, int flags, const splx_gaussian_grads* grads) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (g && grads && g->n == 0 && grads->n == 0) return SPLX_OK;   // empty scene: nothing to write
   if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(proj) || !g2d || !aligned16(g2d) || !grads || !grads->mean ||
       !grads->log_scale || !grads->quat || !grads->opacity_logit || !grads->sh || !aligned16(grads->quat) ||
       !aligned16(grads->mean) || !aligned16(grads->log_scale) || !aligned16(grads->sh) || !aligned16(grads->opacity_logit) ||

@@ -173,20 +173,18 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
           float G, alpha; bool clamped;
           const bool ok = eval_alpha(dxs[s & 1], dys[s >> 1], adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min,
                                      cfg.alpha_max, G, alpha, clamped);
-          if (ok && !((done >> s) & 1)) {
-            const float Tn = T[s] * (1.0f - alpha);
-            if (Tn < cfg.T_eps) {
-              done |= 1u << s;
-              wdone[s] = pos;
-            } else {
-              const float w = alpha * T[s];
-              C0[s] = fmaf(w, c.x, C0[s]); C1[s] = fmaf(w, c.y, C1[s]); C2[s] = fmaf(w, c.z, C2[s]);
-              D[s] = fmaf(w, a.w, D[s]);
-              T[s] = Tn;
-              last[s] = pos;
-              if (COUNT) ++blended;
-            }
-          }
+          // branch-free: a pixel that skips the entry blends it with weight 0
+          const bool live_px = ok && !((done >> s) & 1);
+          const float Tn = T[s] * (1.0f - alpha);
+          const bool stop = live_px && (Tn < cfg.T_eps);      // the exit rule fires BEFORE this entry is applied
+          const bool take = live_px && !(Tn < cfg.T_eps);
+          const float w = take ? alpha * T[s] : 0.0f;
+          C0[s] = fmaf(w, c.x, C0[s]); C1[s] = fmaf(w, c.y, C1[s]); C2[s] = fmaf(w, c.z, C2[s]);
+          D[s] = fmaf(w, a.w, D[s]);
+          T[s] = take ? Tn : T[s];
+          last[s] = take ? pos : last[s];
+          if (stop) done |= 1u << s;
+          if (COUNT) { if (stop) wdone[s] = pos; if (take) ++blended; }
         }
       }
       __syncwarp();
@@ -218,31 +216,37 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
   }
 }
 
-// Reduce 9 per-lane values over the warp with 14 shuffles instead of 45: at each butterfly step a
-// lane keeps one half of its values and hands the other half to its partner.  Afterwards lane
-// 4*j (j = 0..7) holds the warp total of v[j] and every lane holds the total of v8.
-__device__ __forceinline__ float warp_reduce9(float (&v)[8], float& v8, int lane) {
-  const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+// Reduce 9 per-lane values over the warp with 12 shuffles instead of 45: at each butterfly step a
+// lane keeps one half of its values and hands the other half to its partner; the ninth value rides
+// along as a plain butterfly until only two values are left, which then share the last two steps.
+// Afterwards lane L with (L & 2) == 0 holds the warp total of v[4*bit4 + 2*bit3 + bit2] and every
+// lane with (L & 2) != 0 holds the total of v8.
+__device__ __forceinline__ float warp_reduce9(const float (&v)[8], float v8, int lane) {
+  const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4, h2 = lane & 2;
   float a[4], b[2], c;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const float send = h16 ? v[i] : v[i + 4], keep = h16 ? v[i + 4] : v[i];
     a[i] = keep + __shfl_xor_sync(FULL, send, 16);
   }
+  v8 += __shfl_xor_sync(FULL, v8, 16);
 #pragma unroll
   for (int i = 0; i < 2; ++i) {
     const float send = h8 ? a[i] : a[i + 2], keep = h8 ? a[i + 2] : a[i];
     b[i] = keep + __shfl_xor_sync(FULL, send, 8);
   }
+  v8 += __shfl_xor_sync(FULL, v8, 8);
   {
     const float send = h4 ? b[0] : b[1], keep = h4 ? b[1] : b[0];
     c = keep + __shfl_xor_sync(FULL, send, 4);
   }
-  c += __shfl_xor_sync(FULL, c, 2);
+  v8 += __shfl_xor_sync(FULL, v8, 4);
+  {
+    const float send = h2 ? c : v8, keep = h2 ? v8 : c;
+    c = keep + __shfl_xor_sync(FULL, send, 2);
+  }
   c += __shfl_xor_sync(FULL, c, 1);
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v8 += __shfl_xor_sync(FULL, v8, o);
-  return c;   // lane L: total of v[((L>>4)&1)*4 + ((L>>3)&1)*2 + ((L>>2)&1)]
+  return c;
 }
 
 __global__ void __launch_bounds__(BLOCK)
@@ -260,19 +264,23 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
   const float px0 = (float)pxi + 0.5f, px1 = px0 + 8.0f, py0 = (float)pyi + 0.5f, py1 = py0 + 4.0f;
   const float log2_amin = cfg.alpha_min > 0.f ? log2f(cfg.alpha_min) : -INFINITY;
 
+  // Per pixel: T = transmittance in front of the entry being visited (starts from the final one);
+  // Q = <dL/dC, colour composited from everything behind> + dL/dT * (transmittance behind), so that
+  // dL/dalpha_i = T_i (<dL/dC, c_i> - Q_{i+1}) and Q_i = Q_{i+1} + alpha_i (<dL/dC, c_i> - Q_{i+1}); the walk
+  // starts behind the last contributor, where the colour behind is 0 and the transmittance behind is 1.
   uint32_t last[4];
-  float T[4], S0[4], S1[4], S2[4], gC0[4], gC1[4], gC2[4], gTfin[4];
+  float T[4], Q[4], gC0[4], gC1[4], gC2[4];
   uint32_t lmax = 0;
 #pragma unroll
   for (int s = 0; s < 4; ++s) {
     const int x = pxi + 8 * (s & 1), y = pyi + 4 * (s >> 1);
-    last[s] = 0; T[s] = 1.f; S0[s] = S1[s] = S2[s] = 0.f; gC0[s] = gC1[s] = gC2[s] = gTfin[s] = 0.f;
+    last[s] = 0; T[s] = 1.f; Q[s] = 0.f; gC0[s] = gC1[s] = gC2[s] = 0.f;
     if (x < W && y < H) {
       const size_t pix = ((size_t)k * H + y) * W + x;
       last[s] = n_contrib[pix];
-      T[s] = ct[4 * pix + 3];                // the walk starts from the final transmittance
+      T[s] = ct[4 * pix + 3];
       const float4 g = *reinterpret_cast<const float4*>(g_ct + 4 * pix);
-      gC0[s] = g.x; gC1[s] = g.y; gC2[s] = g.z; gTfin[s] = g.w * T[s];
+      gC0[s] = g.x; gC1[s] = g.y; gC2[s] = g.z; Q[s] = g.w;
     }
     lmax = max(lmax, last[s]);
   }
@@ -310,7 +318,9 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
       const float adx[2] = {__fmul_rn(b.x, dxs[0]), __fmul_rn(b.x, dxs[1])};
       const float bdx[2] = {__fmul_rn(b.y, dxs[0]), __fmul_rn(b.y, dxs[1])};
       const float cdy[2] = {__fmul_rn(b.z, dys[0]), __fmul_rn(b.z, dys[1])};
-      // moments of dL/dG over this lane's pixels, and the colour sums
+      // moments of dL/dG over this lane's pixels, and the colour sums.  Branch-free per slot: a pixel
+      // that does not blend this entry runs the same arithmetic with alpha = 0 (T, Q unchanged, every
+      // contribution exactly 0), so the four slots interleave in the pipeline.
       float n0 = 0.f, nx = 0.f, ny = 0.f, nxx = 0.f, nxy = 0.f, nyy = 0.f, q0 = 0.f, q1 = 0.f, q2 = 0.f;
       bool any = false;
 #pragma unroll
@@ -318,28 +328,26 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
         if (!((mj >> s) & 1)) continue;     // warp-uniform
         const float dx = dxs[s & 1], dy = dys[s >> 1];
         float G, alpha; bool clamped;
-        const bool on = (c1 <= last[s]) &&
-                        eval_alpha(dx, dy, adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min, cfg.alpha_max, G, alpha, clamped);
-        if (on) {
-          any = true;
-          const float rom = rcp_approx(1.0f - alpha);          // 1 - alpha >= 1 - alpha_max > 0
-          T[s] *= rom;                              // T_i = T_{i+1} / (1 - alpha_i)
-          const float w = alpha * T[s];
-          q0 = fmaf(w, gC0[s], q0); q1 = fmaf(w, gC1[s], q1); q2 = fmaf(w, gC2[s], q2);     // dL/dc_i
-          const float dLda = T[s] * (gC0[s] * (c.x - S0[s]) + gC1[s] * (c.y - S1[s]) + gC2[s] * (c.z - S2[s])) - gTfin[s] * rom;
-          S0[s] = fmaf(alpha, c.x - S0[s], S0[s]); S1[s] = fmaf(alpha, c.y - S1[s], S1[s]); S2[s] = fmaf(alpha, c.z - S2[s], S2[s]);
-          if (!clamped) {
-            const float gG = dLda * G;              // dL/dG-weight of this pixel (dL/do contribution)
-            const float t1 = gG * dx, t2 = gG * dy;
-            n0 += gG; nx += t1; ny += t2;
-            nxx = fmaf(t1, dx, nxx); nxy = fmaf(t1, dy, nxy); nyy = fmaf(t2, dy, nyy);
-          }
-        }
+        const bool on = eval_alpha(dx, dy, adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min, cfg.alpha_max, G, alpha, clamped) &&
+                        (c1 <= last[s]);
+        any |= on;
+        const float al = on ? alpha : 0.0f;
+        const float rom = rcp_approx(1.0f - al);             // 1 - alpha >= 1 - alpha_max > 0
+        const float Ti = on ? T[s] * rom : T[s];             // T_i = T_{i+1} / (1 - alpha_i)
+        T[s] = Ti;
+        const float w = al * Ti;
+        q0 = fmaf(w, gC0[s], q0); q1 = fmaf(w, gC1[s], q1); q2 = fmaf(w, gC2[s], q2);     // dL/dc_i
+        const float diff = fmaf(gC0[s], c.x, fmaf(gC1[s], c.y, gC2[s] * c.z)) - Q[s];
+        Q[s] = fmaf(al, diff, Q[s]);
+        const float gG = (on && !clamped) ? Ti * diff * G : 0.0f;   // dL/dG-weight of this pixel (dL/do contribution)
+        const float t1 = gG * dx, t2 = gG * dy;
+        n0 += gG; nx += t1; ny += t2;
+        nxx = fmaf(t1, dx, nxx); nxy = fmaf(t1, dy, nxy); nyy = fmaf(t2, dy, nyy);
       }
       if (!__any_sync(FULL, any)) continue;
       // linear map from the moments to the gradients of (u, v, A, B, C, o); alpha = o 2^(A' dx^2 + B' dx dy + C' dy^2)
       const float go = a.z * LN2;
-      float v[8], v8 = q2;
+      float v[8];
       v[0] = go * fmaf(2.0f * b.x, nx, b.y * ny);    // dL/du
       v[1] = go * fmaf(2.0f * b.z, ny, b.y * nx);    // dL/dv
       v[2] = -0.5f * a.z * nxx;                      // dL/dA
@@ -347,13 +355,13 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
       v[4] = -0.5f * a.z * nyy;                      // dL/dC
       v[5] = n0;                                     // dL/do
       v[6] = q0; v[7] = q1;
-      const float tot = warp_reduce9(v, v8, lane);
+      const float tot = warp_reduce9(v, q2, lane);
       float* dst = g2d + (size_t)SPLX_G2D_STRIDE * __float_as_uint(b.w);
       if ((lane & 3) == 0) {
         const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
         atomicAdd(dst + idx, tot);
-      } else if (lane == 1) {
-        atomicAdd(dst + 8, v8);
+      } else if (lane == 2) {
+        atomicAdd(dst + 8, tot);
       }
     }
     __syncwarp();
