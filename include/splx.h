@@ -40,6 +40,7 @@ extern "C" {
 #define SPLX_MAX_K 64
 #define SPLX_TILE 16
 #define SPLX_ADAM_MAX_GROUPS 8
+#define SPLX_MAX_VIEWS 8 /* views consolidated into one launch (splx_plan) */
 #define SPLX_BLEND_STRIDE 12 /* floats per Gaussian in splx_projected.blend */
 #define SPLX_G2D_STRIDE 12 /* floats per Gaussian in the 2-D gradient buffer, see splx_raster_backward */
 
@@ -217,6 +218,86 @@ int splx_adam(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int6
 int splx_adam_groups(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int n_groups,
                      const int64_t *group_offsets, const float *lr, float beta1, float beta2,
                      float eps, int step, float grad_scale, int zero_grad);
+
+/* ==== Optional subsystems (BASELINE.json north_star): visibility prediction
+ * and conflict-free consolidation of B views into one launch.  Additive:
+ * the single-view calls above are the same code run with a one-view plan. ==================== */
+
+/* Per-(partition, tile) visibility state, one byte per slot k*tiles + tile.  A slot whose state
+ * is non-zero is SKIPPED: its list is dropped in splx_bin_sort_plan (tile range = (0,0)), so it is
+ * neither rendered, composed nor back-propagated (it behaves as the identity partial C=0, T=1). */
+#define SPLX_TILE_INVISIBLE 1 /* outside Omega_v^k, the projection of frustum(v) ^ AABB_k (L212, L227) */
+#define SPLX_TILE_SATURATED 2 /* every pixel of the tile has prod_{j in front of k} T^j < eps (L213, L231) */
+
+/* splx_plan.flags */
+#define SPLX_PLAN_SPARSE 1 /* partial pixels and g_ct of a (partition, tile) slot with an EMPTY list are
+                              neither written nor read (exact: such a partial is the identity); compose calls
+                              then need the binning.  Without it every slot of a participating partition is
+                              written, as in the single-view calls. */
+
+/* One launch = B views of identical size, each partition rendering (at most) one of them.  A
+ * conflict-free bucket (L249) maps disjoint partition sets to its views; a single view maps every
+ * participating partition to view 0.  Read on the HOST at call time. */
+typedef struct {
+  int32_t n_views;             /* B in [1, SPLX_MAX_VIEWS] */
+  const splx_camera *cams;     /* HOST [B]; identical width and height */
+  const int32_t *view_of_part; /* HOST [K]: view index of partition k, or -1 = not a participant of this launch
+                                  (its Gaussians are not projected, binned, rendered or differentiated) */
+  const uint8_t *tile_state;   /* DEVICE [K*tiles] or NULL (nothing skipped) */
+  int32_t flags;
+} splx_plan;
+
+/* Geometric visibility (L212, L227): HOST computation, no device work, ctx not needed.  For each of
+ * the K axis-aligned boxes [aabb_lo[k], aabb_hi[k]] (HOST float[K][3], world space) the convex
+ * polyhedron box ^ frustum (the four side planes through the image border and z >= near_z; no far
+ * plane) is projected; tile_state[k*tiles + t] (HOST out) = 0 if tile t's pixel-area
+ * rectangle meets that convex region, else SPLX_TILE_INVISIBLE.  participants (HOST out, may be
+ * NULL): bit k set iff partition k has at least one visible tile (GetParticipants, L249).
+ * Double precision.  Returns SPLX_OK or SPLX_ERR_INVALID_ARG (K > 64, null pointers, lo > hi). */
+int splx_visible_regions(int K, const float *aabb_lo, const float *aabb_hi, const splx_camera *cam,
+                         uint8_t *tile_state, uint64_t *participants);
+
+/* Conflict-free view consolidation (L249): greedy bucketing in view order.  View v goes to the first
+ * bucket none of whose views shares a partition with participants[v] and that holds fewer than
+ * max_views_per_bucket views (<= SPLX_MAX_VIEWS), else opens a new bucket.  HOST in/out.
+ * bucket_of_view[n_views] and *n_buckets are written. */
+int splx_schedule_views(int n_views, const uint64_t *participants, int max_views_per_bucket,
+                        int32_t *bucket_of_view, int32_t *n_buckets);
+
+/* The stages under a plan.  part_offsets: HOST [K+1] as in splx_bin_sort.  Arrays indexed by view
+ * have a leading dimension B = plan->n_views: image[B,H,W,3], T_total[B,H,W], dL_dimage[B,H,W,3].
+ * Arrays indexed by partition keep their [K,...] layout (a partition belongs to one view). */
+int splx_project_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                      const splx_plan *plan, int sh_degree, const splx_projected *out);
+int splx_bin_sort_plan(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
+                       const int64_t *part_offsets, const splx_plan *plan, const splx_binning *out,
+                       void *ws, size_t ws_bytes);
+int splx_render_partial_plan(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins, int K,
+                             const splx_plan *plan, const splx_partial *out, uint64_t *pairs);
+/* bins: needed with SPLX_PLAN_SPARSE or tile_state_out, else may be NULL.  tile_state_out (DEVICE
+ * [K*tiles], may be NULL, may alias plan->tile_state): saturation detection "at no additional
+ * cost" during composition (L231): for every participating partition k and tile t,
+ * out = (in & SPLX_TILE_INVISIBLE) | (SPLX_TILE_SATURATED if at EVERY pixel of the tile the product
+ * of the T^j composited in front of k is < sat_eps); `in` = plan->tile_state or 0.  A partition
+ * that is the identity at a pixel stands behind all others there (its front product is T_total). */
+int splx_compose_plan(splx_ctx *ctx, int K, const splx_partial *partials, const splx_binning *bins,
+                      const splx_plan *plan, const float bg[3], float *image, float *T_total,
+                      float sat_eps, uint8_t *tile_state_out);
+int splx_compose_backward_plan(splx_ctx *ctx, int K, const splx_partial *partials,
+                               const splx_binning *bins, const splx_plan *plan, const float bg[3],
+                               const float *dL_dimage, const float *dL_dT_total, float *g_ct);
+int splx_raster_backward_plan(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins, int K,
+                              const splx_plan *plan, const splx_partial *partials, const float *g_ct,
+                              float *g2d);
+/* With SPLX_PB_OVERWRITE the gradient rows of NON-participating partitions are written as zeros. */
+int splx_project_backward_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                               const splx_plan *plan, int sh_degree, const splx_projected *proj,
+                               float *g2d, int flags, const splx_gaussian_grads *grads);
+int splx_backward_plan(splx_ctx *ctx, int K, const int64_t *part_offsets, const splx_plan *plan,
+                       const splx_partial *partials, const float bg[3], const float *dL_dimage,
+                       const float *dL_dT_total, const splx_gaussians *g, const splx_projected *proj,
+                       const splx_binning *bins, int sh_degree, const splx_gaussian_grads *grads,
+                       void *ws, size_t ws_bytes, int flags);
 
 #ifdef __cplusplus
 }

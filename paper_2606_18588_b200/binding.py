@@ -29,7 +29,13 @@ EXPORTS = [
     "splx_render_partial", "splx_compose", "splx_l1_loss_grad", "splx_compose_backward",
     "splx_raster_backward", "splx_project_backward", "splx_backward_ws_bytes", "splx_backward",
     "splx_adam", "splx_adam_groups",
+    "splx_visible_regions", "splx_schedule_views", "splx_project_plan", "splx_bin_sort_plan",
+    "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
+    "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
 ]
+MAX_VIEWS = 8
+TILE_INVISIBLE, TILE_SATURATED = 1, 2
+PLAN_SPARSE = 1
 
 
 class SplxError(RuntimeError):
@@ -67,6 +73,11 @@ class BinningS(C.Structure):
 
 class PartialS(C.Structure):
     _fields_ = [("ct", C.c_void_p), ("d", C.c_void_p), ("n_contrib", C.c_void_p)]
+
+
+class PlanS(C.Structure):
+    _fields_ = [("n_views", C.c_int32), ("cams", C.c_void_p), ("view_of_part", C.c_void_p),
+                ("tile_state", C.c_void_p), ("flags", C.c_int32)]
 
 
 def lib():
@@ -112,6 +123,18 @@ def lib():
         L.splx_adam_groups.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                                        C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int,
                                        C.c_float, C.c_int]
+        vp = C.c_void_p
+        L.splx_visible_regions.argtypes = [C.c_int, vp, vp, vp, vp, vp]
+        L.splx_schedule_views.argtypes = [C.c_int, vp, C.c_int, vp, vp]
+        L.splx_project_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp]
+        L.splx_bin_sort_plan.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp, vp, vp, C.c_size_t]
+        L.splx_render_partial_plan.argtypes = [vp, vp, vp, C.c_int, vp, vp, vp]
+        L.splx_compose_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, C.c_float, vp]
+        L.splx_compose_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp]
+        L.splx_raster_backward_plan.argtypes = [vp, vp, vp, C.c_int, vp, vp, vp, vp]
+        L.splx_project_backward_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp]
+        L.splx_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp, vp,
+                                         C.c_size_t, C.c_int]
         _lib = L
     return _lib
 
@@ -133,6 +156,60 @@ def camera_struct(cam) -> CameraS:
     s.fx, s.fy, s.cx, s.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
     s.width, s.height, s.near_z = int(cam.width), int(cam.height), float(cam.near_z)
     return s
+
+
+class Plan:
+    """splx_plan: B views of one size, the view each partition renders (-1 = not a participant), the
+    optional device tile-state bytes [K*tiles] and the flags.  Keeps the ctypes storage alive."""
+
+    def __init__(self, cams, view_of_part, tile_state=None, sparse=False):
+        self.cams = list(cams)
+        self.view_of_part = [int(v) for v in view_of_part]
+        self.tile_state = tile_state
+        self.flags = PLAN_SPARSE if sparse else 0
+        self._cams = (CameraS * len(self.cams))(*[camera_struct(c) for c in self.cams])
+        self._vop = (C.c_int32 * len(self.view_of_part))(*self.view_of_part)
+        self._s = PlanS(len(self.cams), C.cast(self._cams, C.c_void_p), C.cast(self._vop, C.c_void_p),
+                        _ptr(tile_state), self.flags)
+
+    @property
+    def K(self):
+        return len(self.view_of_part)
+
+    @property
+    def B(self):
+        return len(self.cams)
+
+    def ref(self):
+        return C.byref(self._s)
+
+
+def visible_regions(aabb_lo, aabb_hi, cam):
+    """splx_visible_regions (host computation): returns (tile_state uint8 numpy [K, tiles], participants bitmask)."""
+    import numpy as np
+    lo = np.ascontiguousarray(aabb_lo, np.float32).reshape(-1, 3)
+    hi = np.ascontiguousarray(aabb_hi, np.float32).reshape(-1, 3)
+    K = lo.shape[0]
+    TX, TY = (int(cam.width) + TILE - 1) // TILE, (int(cam.height) + TILE - 1) // TILE
+    out = np.empty((K, TX * TY), np.uint8)
+    part = C.c_uint64(0)
+    cs = camera_struct(cam)
+    rc = lib().splx_visible_regions(K, lo.ctypes.data, hi.ctypes.data, C.byref(cs), out.ctypes.data, C.byref(part))
+    if rc != OK:
+        raise SplxError(rc, "splx_visible_regions: invalid argument")
+    return out, int(part.value)
+
+
+def schedule_views(participants, max_views_per_bucket=MAX_VIEWS):
+    """splx_schedule_views (host computation): greedy conflict-free bucketing; returns bucket index per view."""
+    n = len(participants)
+    pa = (C.c_uint64 * max(n, 1))(*[int(x) for x in participants])
+    out = (C.c_int32 * max(n, 1))()
+    nb = C.c_int32(0)
+    rc = lib().splx_schedule_views(n, pa, int(max_views_per_bucket), out, C.byref(nb))
+    if rc != OK:
+        raise SplxError(rc, "splx_schedule_views: invalid argument")
+    return [int(out[i]) for i in range(n)], int(nb.value)
 
 
 def gaussians_struct(p: dict, cls=GaussiansS):
@@ -312,3 +389,64 @@ class Context:
         lr = (C.c_float * n)(*[float(x) for x in lrs])
         self._check(lib().splx_adam_groups(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, lr,
                                            beta1, beta2, eps, step, grad_scale, int(zero_grad)))
+
+    # ---- the same stages under a launch plan (visibility prediction, consolidated views) ---------
+    visible_regions = staticmethod(visible_regions)     # host computations: no context needed
+    schedule_views = staticmethod(schedule_views)
+
+    @staticmethod
+    def _offs(part_offsets):
+        return (C.c_int64 * len(part_offsets))(*[int(x) for x in part_offsets])
+
+    def project_plan(self, params: dict, part_offsets, plan: Plan, sh_degree: int, out: Projected):
+        g, ps = gaussians_struct(params), out.struct()
+        self._check(lib().splx_project_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
+                                            sh_degree, C.byref(ps)))
+
+    def bin_sort_plan(self, proj: Projected, part_offsets, plan: Plan, out: Binning, ws: torch.Tensor):
+        ps, bs = proj.struct(), out.struct()
+        self._check(lib().splx_bin_sort_plan(self._h, C.byref(ps), proj.n, plan.K, self._offs(part_offsets), plan.ref(),
+                                             C.byref(bs), _ptr(ws), ws.numel() * ws.element_size()))
+
+    def render_partial_plan(self, proj: Projected, bins: Binning, plan: Plan, out: Partial, pairs=None):
+        ps, bs, os_ = proj.struct(), bins.struct(), out.struct()
+        self._check(lib().splx_render_partial_plan(self._h, C.byref(ps), C.byref(bs), plan.K, plan.ref(), C.byref(os_),
+                                                   _ptr(pairs)))
+
+    def compose_plan(self, partials: Partial, bins, plan: Plan, bg, image, T_total=None, sat_eps=1e-4,
+                     tile_state_out=None):
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        ps = partials.struct()
+        bs = bins.struct() if bins is not None else None
+        self._check(lib().splx_compose_plan(self._h, plan.K, C.byref(ps), C.byref(bs) if bs is not None else None,
+                                            plan.ref(), b, _ptr(image), _ptr(T_total), float(sat_eps),
+                                            _ptr(tile_state_out)))
+
+    def compose_backward_plan(self, partials: Partial, bins, plan: Plan, bg, g_image, g_T_total, g_ct):
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        ps = partials.struct()
+        bs = bins.struct() if bins is not None else None
+        self._check(lib().splx_compose_backward_plan(self._h, plan.K, C.byref(ps), C.byref(bs) if bs is not None else None,
+                                                     plan.ref(), b, _ptr(g_image), _ptr(g_T_total), _ptr(g_ct)))
+
+    def raster_backward_plan(self, proj: Projected, bins: Binning, plan: Plan, partials: Partial, g_ct, g2d):
+        ps, bs, pa = proj.struct(), bins.struct(), partials.struct()
+        self._check(lib().splx_raster_backward_plan(self._h, C.byref(ps), C.byref(bs), plan.K, plan.ref(), C.byref(pa),
+                                                    _ptr(g_ct), _ptr(g2d)))
+
+    def project_backward_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
+                              grads: dict, clear_g2d=False, overwrite=False):
+        g, gg, ps = gaussians_struct(params), gaussians_struct(grads), proj.struct()
+        flags = (PB_CLEAR_G2D if clear_g2d else 0) | (PB_OVERWRITE if overwrite else 0)
+        self._check(lib().splx_project_backward_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
+                                                     sh_degree, C.byref(ps), _ptr(g2d), flags, C.byref(gg)))
+
+    def backward_plan(self, part_offsets, plan: Plan, partials: Partial, bg, g_image, g_T_total, params: dict,
+                      proj: Projected, bins: Binning, sh_degree, grads: dict, ws: torch.Tensor, overwrite=False):
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        pa, ps, bs = partials.struct(), proj.struct(), bins.struct()
+        g, gg = gaussians_struct(params), gaussians_struct(grads)
+        self._check(lib().splx_backward_plan(self._h, plan.K, self._offs(part_offsets), plan.ref(), C.byref(pa), b,
+                                             _ptr(g_image), _ptr(g_T_total), C.byref(g), C.byref(ps), C.byref(bs),
+                                             sh_degree, C.byref(gg), _ptr(ws), ws.numel() * ws.element_size(),
+                                             PB_OVERWRITE if overwrite else 0))

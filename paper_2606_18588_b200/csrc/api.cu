@@ -22,6 +22,51 @@ static bool bins_ok(const splx_binning* b) {
   return b && b->keys && b->vals && b->tile_ranges && b->num_intersections && aligned16(b->keys);
 }
 
+// ---- launch plans ---------------------------------------------------------------------------
+// Validates a splx_plan against K and builds the device-side copy.  All views must share one image size.
+static int make_plan(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, PlanDev* out) {
+  if (!plan || !plan->cams || !plan->view_of_part) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: plan, cams or view_of_part is NULL", who);
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: K=%d not in [1,%d]", who, K, SPLX_MAX_K);
+  if (plan->n_views < 1 || plan->n_views > SPLX_MAX_VIEWS)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: n_views=%d not in [1,%d]", who, plan->n_views, SPLX_MAX_VIEWS);
+  if (plan->flags & ~SPLX_PLAN_SPARSE) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: unknown plan flags %d", who, plan->flags);
+  memset(out, 0, sizeof *out);
+  for (int b = 0; b < plan->n_views; ++b) {
+    if (!cam_ok(&plan->cams[b])) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: camera %d invalid", who, b);
+    if (plan->cams[b].width != plan->cams[0].width || plan->cams[b].height != plan->cams[0].height)
+      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: all views of a plan must have the same size", who);
+    out->cam[b] = make_camdev(&plan->cams[b], ctx->cfg);
+  }
+  for (int k = 0; k < K; ++k) {
+    const int v = plan->view_of_part[k];
+    if (v < -1 || v >= plan->n_views) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: view_of_part[%d]=%d out of range", who, k, v);
+    out->pv.v[k] = (signed char)v;
+  }
+  for (int k = K; k < SPLX_MAX_K; ++k) out->pv.v[k] = -1;
+  out->B = plan->n_views; out->K = K;
+  out->W = out->cam[0].W; out->H = out->cam[0].H; out->TX = out->cam[0].TX; out->TY = out->cam[0].TY;
+  out->ntiles = out->TX * out->TY;
+  out->flags = plan->flags;
+  out->tile_state = plan->tile_state;
+  return SPLX_OK;
+}
+
+static bool offsets_ok(const int64_t* po, int K, int64_t n) {
+  if (!po || po[0] != 0 || po[K] != n) return false;
+  for (int k = 0; k < K; ++k) if (po[k + 1] < po[k]) return false;
+  return true;
+}
+
+// One view, every partition renders it: the plan behind the single-view calls.
+struct SinglePlan {
+  int32_t views[SPLX_MAX_K];
+  splx_plan plan;
+  explicit SinglePlan(const splx_camera* cam) {
+    for (int k = 0; k < SPLX_MAX_K; ++k) views[k] = 0;
+    plan.n_views = 1; plan.cams = cam; plan.view_of_part = views; plan.tile_state = nullptr; plan.flags = 0;
+  }
+};
+
 extern "C" {
 
 int splx_create(splx_ctx** out, int device, void* cuda_stream, const splx_config* cfg) {
@@ -74,13 +119,27 @@ int splx_set_stream(splx_ctx* ctx, void* cuda_stream) {
 
 int64_t splx_launch_count(const splx_ctx* ctx) { return ctx ? ctx->launches : -1; }
 
+int splx_project_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const splx_plan* plan,
+                      int sh_degree, const splx_projected* out) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (g && g->n == 0) return SPLX_OK;   // empty scene: nothing to write
+  if (!gauss_ok(g) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: null/misaligned argument");
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: sh_degree %d not in [0,3]", sh_degree);
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_project", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: part_offsets must run monotonically from 0 to n");
+  return launch_project_fwd(ctx, g, pd, part_offsets, sh_degree, out);
+}
+
 int splx_project(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
                  const splx_projected* out) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (g && g->n == 0) return SPLX_OK;   // empty scene: nothing to write
-  if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: null/misaligned argument");
-  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: sh_degree %d not in [0,3]", sh_degree);
-  return launch_project_fwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, out);
+  if (g && g->n == 0) return SPLX_OK;
+  if (!gauss_ok(g) || !cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: null/misaligned argument");
+  const SinglePlan sp(cam);
+  const int64_t po[2] = {0, g->n};
+  return splx_project_plan(ctx, g, 1, po, &sp.plan, sh_degree, out);
 }
 
 size_t splx_bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, const splx_camera* cam) {
@@ -89,21 +148,28 @@ size_t splx_bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, const splx_ca
   return bin_sort_ws_bytes(n, capacity, K, TX, TY);
 }
 
+int splx_bin_sort_plan(splx_ctx* ctx, const splx_projected* proj, int64_t n, int K, const int64_t* part_offsets,
+                       const splx_plan* plan, const splx_binning* out, void* ws, size_t ws_bytes) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !bins_ok(out) || n < 0 || (!ws && ws_bytes))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_bin_sort", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: part_offsets must run monotonically from 0 to n");
+  if (n >= ((int64_t)1 << 32) || out->capacity >= ((uint64_t)1 << 32))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: n and capacity must be < 2^32");
+  if ((uint64_t)K * pd.ntiles >= ((uint64_t)1 << 31)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles too large");
+  if (!aligned16(ws)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: workspace not 16-byte aligned");
+  return launch_bin_sort(ctx, proj, n, pd, part_offsets, out, ws, ws_bytes);
+}
+
 int splx_bin_sort(splx_ctx* ctx, const splx_projected* proj, int64_t n, int K, const int64_t* part_offsets,
                   const splx_camera* cam, const splx_binning* out, void* ws, size_t ws_bytes) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!proj_ok(proj) || !cam_ok(cam) || !bins_ok(out) || !part_offsets || n < 0 || (!ws && ws_bytes))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: null/misaligned argument");
-  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K=%d not in [1,%d]", K, SPLX_MAX_K);
-  if (part_offsets[0] != 0 || part_offsets[K] != n) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: part_offsets must run from 0 to n");
-  for (int k = 0; k < K; ++k)
-    if (part_offsets[k + 1] < part_offsets[k]) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: part_offsets not monotone");
-  if (n >= ((int64_t)1 << 32) || out->capacity >= ((uint64_t)1 << 32))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: n and capacity must be < 2^32");
-  const CamDev cd = make_camdev(cam, ctx->cfg);
-  if ((uint64_t)K * cd.TX * cd.TY >= ((uint64_t)1 << 31)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles too large");
-  if (!aligned16(ws)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: workspace not 16-byte aligned");
-  return launch_bin_sort(ctx, proj, n, K, part_offsets, cd, out, ws, ws_bytes);
+  if (!cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: null/misaligned argument");
+  const SinglePlan sp(cam);
+  return splx_bin_sort_plan(ctx, proj, n, K, part_offsets, &sp.plan, out, ws, ws_bytes);
 }
 
 int splx_check_capacity(splx_ctx* ctx, const splx_binning* bins, uint64_t* m_host) {
@@ -118,21 +184,44 @@ int splx_check_capacity(splx_ctx* ctx, const splx_binning* bins, uint64_t* m_hos
   return SPLX_OK;
 }
 
+int splx_render_partial_plan(splx_ctx* ctx, const splx_projected* proj, const splx_binning* bins, int K,
+                             const splx_plan* plan, const splx_partial* out, uint64_t* pairs) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !bins_ok(bins) || !partial_ok(out))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_render_partial", K, plan, &pd))) return rc;
+  return launch_render_fwd(ctx, proj, bins, pd, out, pairs);
+}
+
 int splx_render_partial(splx_ctx* ctx, const splx_projected* proj, const splx_binning* bins, int K,
                         const splx_camera* cam, const splx_partial* out, uint64_t* pairs) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!proj_ok(proj) || !bins_ok(bins) || !cam_ok(cam) || !partial_ok(out))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: null/misaligned argument");
-  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: K=%d not in [1,%d]", K, SPLX_MAX_K);
-  return launch_render_fwd(ctx, proj, bins, K, make_camdev(cam, ctx->cfg), out, pairs);
+  if (!cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: null/misaligned argument");
+  const SinglePlan sp(cam);
+  return splx_render_partial_plan(ctx, proj, bins, K, &sp.plan, out, pairs);
+}
+
+int splx_compose_plan(splx_ctx* ctx, int K, const splx_partial* partials, const splx_binning* bins, const splx_plan* plan,
+                      const float bg[3], float* image, float* T_total, float sat_eps, uint8_t* tile_state_out) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!partial_ok(partials) || !bg || !image) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_compose", K, plan, &pd))) return rc;
+  if ((pd.flags & SPLX_PLAN_SPARSE) && !bins_ok(bins))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: SPLX_PLAN_SPARSE needs the binning");
+  if (tile_state_out && !(sat_eps >= 0.f)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: sat_eps must be >= 0");
+  return launch_compose_fwd(ctx, partials, bins, pd, bg, image, T_total, sat_eps, tile_state_out);
 }
 
 int splx_compose(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
                  float* image, float* T_total) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!partial_ok(partials) || !cam_ok(cam) || !bg || !image) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: null/misaligned argument");
-  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: K=%d not in [1,%d]", K, SPLX_MAX_K);
-  return launch_compose_fwd(ctx, K, partials, make_camdev(cam, ctx->cfg), bg, image, T_total);
+  if (!cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: null/misaligned argument");
+  const SinglePlan sp(cam);
+  return splx_compose_plan(ctx, K, partials, nullptr, &sp.plan, bg, image, T_total, 0.f, nullptr);
 }
 
 int splx_l1_loss_grad(splx_ctx* ctx, const float* image, const float* target, int64_t count, float scale,
@@ -143,37 +232,74 @@ int splx_l1_loss_grad(splx_ctx* ctx, const float* image, const float* target, in
   return launch_l1(ctx, image, target, count, scale, dL_dimage, loss_sum);
 }
 
+int splx_compose_backward_plan(splx_ctx* ctx, int K, const splx_partial* partials, const splx_binning* bins,
+                               const splx_plan* plan, const float bg[3], const float* dL_dimage,
+                               const float* dL_dT_total, float* g_ct) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!partial_ok(partials) || !bg || !dL_dimage || !g_ct || !aligned16(g_ct))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_compose_backward", K, plan, &pd))) return rc;
+  if ((pd.flags & SPLX_PLAN_SPARSE) && !bins_ok(bins))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: SPLX_PLAN_SPARSE needs the binning");
+  return launch_compose_bwd(ctx, partials, bins, pd, bg, dL_dimage, dL_dT_total, g_ct);
+}
+
 int splx_compose_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam,
                           const float bg[3], const float* dL_dimage, const float* dL_dT_total, float* g_ct) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!partial_ok(partials) || !cam_ok(cam) || !bg || !dL_dimage || !g_ct || !aligned16(g_ct))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: null/misaligned argument");
-  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: K=%d not in [1,%d]", K, SPLX_MAX_K);
-  return launch_compose_bwd(ctx, K, partials, make_camdev(cam, ctx->cfg), bg, dL_dimage, dL_dT_total, g_ct);
+  if (!cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: null/misaligned argument");
+  const SinglePlan sp(cam);
+  return splx_compose_backward_plan(ctx, K, partials, nullptr, &sp.plan, bg, dL_dimage, dL_dT_total, g_ct);
+}
+
+int splx_raster_backward_plan(splx_ctx* ctx, const splx_projected* proj, const splx_binning* bins, int K,
+                              const splx_plan* plan, const splx_partial* partials, const float* g_ct, float* g2d) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !bins_ok(bins) || !partial_ok(partials) || !g_ct || !g2d || !aligned16(g_ct) || !aligned16(g2d))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_raster_backward", K, plan, &pd))) return rc;
+  return launch_raster_bwd(ctx, proj, bins, pd, partials, g_ct, g2d);
 }
 
 int splx_raster_backward(splx_ctx* ctx, const splx_projected* proj, const splx_binning* bins, int K,
                          const splx_camera* cam, const splx_partial* partials, const float* g_ct, float* g2d) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!proj_ok(proj) || !bins_ok(bins) || !cam_ok(cam) || !partial_ok(partials) || !g_ct || !g2d ||
-      !aligned16(g_ct) || !aligned16(g2d))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: null/misaligned argument");
-  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: K=%d not in [1,%d]", K, SPLX_MAX_K);
-  return launch_raster_bwd(ctx, proj, bins, K, make_camdev(cam, ctx->cfg), partials, g_ct, g2d);
+  if (!cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: null/misaligned argument");
+  const SinglePlan sp(cam);
+  return splx_raster_backward_plan(ctx, proj, bins, K, &sp.plan, partials, g_ct, g2d);
 }
 
-int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
-                          const splx_projected* proj, float* g2d, int flags, const splx_gaussian_grads* grads) {
+int splx_project_backward_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets,
+                               const splx_plan* plan, int sh_degree, const splx_projected* proj, float* g2d, int flags,
+                               const splx_gaussian_grads* grads) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (g && grads && g->n == 0 && grads->n == 0) return SPLX_OK;   // empty scene: nothing to write
-  if (!gauss_ok(g) || !cam_ok(cam) || !proj_ok(proj) || !g2d || !aligned16(g2d) || !grads || !grads->mean ||
+  if (!gauss_ok(g) || !proj_ok(proj) || !g2d || !aligned16(g2d) || !grads || !grads->mean ||
       !grads->log_scale || !grads->quat || !grads->opacity_logit || !grads->sh || !aligned16(grads->quat) ||
       !aligned16(grads->mean) || !aligned16(grads->log_scale) || !aligned16(grads->sh) || !aligned16(grads->opacity_logit) ||
       grads->n != g->n)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: null/misaligned argument");
   if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: sh_degree %d not in [0,3]", sh_degree);
   if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: unknown flags %d", flags);
-  return launch_project_bwd(ctx, g, make_camdev(cam, ctx->cfg), sh_degree, proj, g2d, flags, grads);
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_project_backward", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: part_offsets must run monotonically from 0 to n");
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads);
+}
+
+int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
+                          const splx_projected* proj, float* g2d, int flags, const splx_gaussian_grads* grads) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (g && grads && g->n == 0 && grads->n == 0) return SPLX_OK;
+  if (!gauss_ok(g) || !cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: null/misaligned argument");
+  const SinglePlan sp(cam);
+  const int64_t po[2] = {0, g->n};
+  return splx_project_backward_plan(ctx, g, 1, po, &sp.plan, sh_degree, proj, g2d, flags, grads);
 }
 
 size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera* cam) {
@@ -183,13 +309,16 @@ size_t splx_backward_ws_bytes(int64_t n, int K, const splx_camera* cam) {
   return g_ct + g2d;
 }
 
-int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
-                  const float* dL_dimage, const float* dL_dT_total, const splx_gaussians* g,
-                  const splx_projected* proj, const splx_binning* bins, int sh_degree,
-                  const splx_gaussian_grads* grads, void* ws, size_t ws_bytes, int flags) {
+int splx_backward_plan(splx_ctx* ctx, int K, const int64_t* part_offsets, const splx_plan* plan,
+                       const splx_partial* partials, const float bg[3], const float* dL_dimage,
+                       const float* dL_dT_total, const splx_gaussians* g, const splx_projected* proj,
+                       const splx_binning* bins, int sh_degree, const splx_gaussian_grads* grads, void* ws,
+                       size_t ws_bytes, int flags) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (flags & ~SPLX_PB_OVERWRITE) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: unknown flags %d", flags);
-  if (!gauss_ok(g) || !cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: null/misaligned argument");
+  if (!gauss_ok(g) || !plan || !plan->cams || plan->n_views < 1 || !cam_ok(&plan->cams[0]))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: null/misaligned argument");
+  const splx_camera* cam = &plan->cams[0];
   const size_t need = splx_backward_ws_bytes(g->n, K, cam);
   if (!ws || !aligned16(ws) || ws_bytes < need)
     SPLX_FAIL(ctx, SPLX_ERR_WORKSPACE, "splx_backward: workspace %zu B < required %zu B", ws_bytes, need);
@@ -197,12 +326,28 @@ int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx
   float* g2d = (float*)((char*)ws + align_up((size_t)K * cam->width * cam->height * 4 * sizeof(float), 256));
   int rc;
   // a8: Eq.6-7 hand dL/dC^k, dL/dT^k to every partition's rasteriser backward
-  if ((rc = splx_compose_backward(ctx, K, partials, cam, bg, dL_dimage, dL_dT_total, g_ct))) return rc;
+  if ((rc = splx_compose_backward_plan(ctx, K, partials, bins, plan, bg, dL_dimage, dL_dT_total, g_ct))) return rc;
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(g2d, 0, (size_t)g->n * SPLX_G2D_STRIDE * sizeof(float), ctx->stream));
   // a9: reverse-order blend gradients into means2D, conic, opacity, colour
-  if ((rc = splx_raster_backward(ctx, proj, bins, K, cam, partials, g_ct, g2d))) return rc;
+  if ((rc = splx_raster_backward_plan(ctx, proj, bins, K, plan, partials, g_ct, g2d))) return rc;
   // a10: projection backward to the 3-D parameters
-  return splx_project_backward(ctx, g, cam, sh_degree, proj, g2d, flags, grads);
+  return splx_project_backward_plan(ctx, g, K, part_offsets, plan, sh_degree, proj, g2d, flags, grads);
+}
+
+int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
+                  const float* dL_dimage, const float* dL_dT_total, const splx_gaussians* g,
+                  const splx_projected* proj, const splx_binning* bins, int sh_degree,
+                  const splx_gaussian_grads* grads, void* ws, size_t ws_bytes, int flags) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!gauss_ok(g) || !cam_ok(cam)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: null/misaligned argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_backward: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  const SinglePlan sp(cam);
+  // the projection backward needs no partition structure for a single view: one run over all Gaussians
+  int64_t po[SPLX_MAX_K + 1];
+  po[0] = 0;
+  for (int k = 1; k <= K; ++k) po[k] = g->n;
+  return splx_backward_plan(ctx, K, po, &sp.plan, partials, bg, dL_dimage, dL_dT_total, g, proj, bins, sh_degree, grads,
+                            ws, ws_bytes, flags);
 }
 
 int splx_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr, float beta1,

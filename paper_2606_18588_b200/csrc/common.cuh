@@ -44,6 +44,46 @@ static inline CamDev make_camdev(const splx_camera* c, const splx_config& cfg) {
   return d;
 }
 
+// Launch plan on the device side (splx_plan): B views of identical size, the view each partition
+// renders in this launch (-1 = the partition does not participate), the optional per-(partition,
+// tile) visibility state and the flags.  Passed to kernels as a __grid_constant__ parameter so that
+// the per-partition camera is an indexed constant-bank load.
+struct PartView { signed char v[SPLX_MAX_K]; };
+
+struct PlanDev {
+  int B, K, W, H, TX, TY, ntiles, flags;
+  const uint8_t* tile_state;
+  PartView pv;
+  CamDev cam[SPLX_MAX_VIEWS];
+};
+
+// Contiguous runs of Gaussians (one per participating partition) covered by ONE launch of a
+// per-Gaussian kernel: block b works on run r with block_prefix[r] <= b < block_prefix[r+1].
+// view[r] < 0 marks a run of a non-participating partition (only present when its outputs must
+// be cleared).  jprefix = running count of Gaussians, for kernels indexed by element.
+struct RunTable {
+  int n, blocks_total;
+  int64_t begin[SPLX_MAX_K], end[SPLX_MAX_K], jprefix[SPLX_MAX_K + 1];
+  int block_prefix[SPLX_MAX_K + 1];
+  signed char view[SPLX_MAX_K];
+};
+
+static inline RunTable make_runs(const PlanDev& plan, const int64_t* part_offsets, int block, bool with_inactive) {
+  RunTable rt;
+  memset(&rt, 0, sizeof rt);
+  for (int k = 0; k < plan.K; ++k) {
+    const int v = plan.pv.v[k];
+    const int64_t b = part_offsets[k], e = part_offsets[k + 1];
+    if (e <= b || (v < 0 && !with_inactive)) continue;
+    const int r = rt.n++;
+    rt.begin[r] = b; rt.end[r] = e; rt.view[r] = (signed char)v;
+    rt.jprefix[r + 1] = rt.jprefix[r] + (e - b);
+    rt.block_prefix[r + 1] = rt.block_prefix[r] + (int)((e - b + block - 1) / block);
+  }
+  rt.blocks_total = rt.block_prefix[rt.n];
+  return rt;
+}
+
 #define SPLX_FAIL(ctx, code, ...)                                  \
   do {                                                             \
     snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__);         \
@@ -86,20 +126,20 @@ __device__ __forceinline__ void tile_rect(float u, float v, int radius, int TX, 
 }
 
 // ---- stage launchers (defined one per .cu file, called from api.cu) ----------------------
-int launch_project_fwd(splx_ctx*, const splx_gaussians*, const CamDev&, int sh_degree,
+int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*);
-int launch_project_bwd(splx_ctx*, const splx_gaussians*, const CamDev&, int sh_degree,
+int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
-int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, int K, const int64_t* part_offsets,
-                    const CamDev&, const splx_binning*, void* ws, size_t ws_bytes);
-int launch_render_fwd(splx_ctx*, const splx_projected*, const splx_binning*, int K, const CamDev&,
+int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, const PlanDev&, const int64_t* part_offsets,
+                    const splx_binning*, void* ws, size_t ws_bytes);
+int launch_render_fwd(splx_ctx*, const splx_projected*, const splx_binning*, const PlanDev&,
                       const splx_partial*, uint64_t* pairs);
-int launch_raster_bwd(splx_ctx*, const splx_projected*, const splx_binning*, int K, const CamDev&,
+int launch_raster_bwd(splx_ctx*, const splx_projected*, const splx_binning*, const PlanDev&,
                       const splx_partial*, const float* g_ct, float* g2d);
-int launch_compose_fwd(splx_ctx*, int K, const splx_partial*, const CamDev&, const float* bg,
-                       float* image, float* T_total);
-int launch_compose_bwd(splx_ctx*, int K, const splx_partial*, const CamDev&, const float* bg,
+int launch_compose_fwd(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
+                       float* image, float* T_total, float sat_eps, uint8_t* tile_state_out);
+int launch_compose_bwd(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
                        const float* g_image, const float* g_T_total, float* g_ct);
 int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count, float scale,
               float* g_image, double* loss_sum);

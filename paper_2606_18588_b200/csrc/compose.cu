@@ -6,23 +6,40 @@
 // Readings: s3 ordering key D/(1-T); s4 ties by partition index, an empty partial
 // (T == 1) is the identity and sorts last; s7 background blended behind everything.
 //
-// HBM-bound streaming kernels: one thread per pixel, float4 (C,T) + float D per partition.
-// Only the live partials (T < 1) of a pixel are ordered: an empty one contributes nothing
-// wherever it stands, so the insertion sort runs over ~1-2 entries instead of K.
+// HBM-bound streaming kernels.  Grid = (tiles, B views), CTA = one 16 x 16 tile, one thread per pixel,
+// float4 (C,T) + float D per partition.  A view composes only the partitions that render it
+// (splx_plan.view_of_part); with SPLX_PLAN_SPARSE a (partition, tile) slot whose list is empty is
+// the identity and is not even read -- the tile's participant flags are looked up once per CTA.
+// Only the live partials (T < 1) of a pixel are ordered: an empty one contributes nothing wherever
+// it stands, so the insertion sort runs over ~1-2 entries instead of K.
 #include "common.cuh"
 
 namespace {
 
-constexpr int CB = 256;
+constexpr int CB = SPLX_TILE * SPLX_TILE;
 
-struct PartialPtrs { const float* ct; const float* d; };
+// s_use[k] = 1 iff partition k is composed into view b on this tile.
+__device__ __forceinline__ void tile_participants(const PartView& pv, int K, int b, int tile, int ntiles, int sparse,
+                                                  const uint32_t* __restrict__ ranges, uint8_t* s_use) {
+  for (int k = threadIdx.x; k < K; k += CB) {
+    bool use = pv.v[k] == b;
+    if (use && sparse) {
+      const uint2 r = *reinterpret_cast<const uint2*>(ranges + 2 * ((size_t)k * ntiles + tile));
+      use = r.x < r.y;
+    }
+    s_use[k] = use ? 1 : 0;
+  }
+  __syncthreads();
+}
 
 // Collect the live partials of one pixel, sorted by (key, k).  Returns the count.
 template <int KMAX>
-__device__ __forceinline__ int ordered_live(const float* __restrict__ ct, const float* __restrict__ d,
-                                            int K, size_t HW, size_t pix, float (&key)[KMAX], int (&idx)[KMAX]) {
+__device__ __forceinline__ int ordered_live(const float* __restrict__ ct, const float* __restrict__ d, int K,
+                                            const uint8_t* s_use, size_t HW, size_t pix, float (&key)[KMAX],
+                                            int (&idx)[KMAX]) {
   int L = 0;
   for (int k = 0; k < K; ++k) {
+    if (!s_use[k]) continue;
     const float T = __ldg(ct + 4 * ((size_t)k * HW + pix) + 3);
     if (T < 1.0f) {
       const float kk = __fdiv_rn(__ldg(d + (size_t)k * HW + pix), __fsub_rn(1.0f, T));
@@ -34,43 +51,80 @@ __device__ __forceinline__ int ordered_live(const float* __restrict__ ct, const 
   return L;
 }
 
-template <int KMAX>
+template <int KMAX, bool SAT>
 __global__ void __launch_bounds__(CB)
-k_compose_fwd(const float* __restrict__ ct, const float* __restrict__ d, int K, size_t HW, float bg0, float bg1,
-              float bg2, float* __restrict__ image, float* __restrict__ T_total) {
-  const size_t pix = (size_t)blockIdx.x * CB + threadIdx.x;
-  if (pix >= HW) return;
-  float key[KMAX]; int idx[KMAX];
-  const int L = ordered_live<KMAX>(ct, d, K, HW, pix, key, idx);
-  float Tacc = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-  for (int m = 0; m < L; ++m) {
-    const float4 p = __ldg(reinterpret_cast<const float4*>(ct) + (size_t)idx[m] * HW + pix);
-    C0 = fmaf(Tacc, p.x, C0); C1 = fmaf(Tacc, p.y, C1); C2 = fmaf(Tacc, p.z, C2);
-    Tacc *= p.w;
+k_compose_fwd(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
+              const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
+              float bg1, float bg2, float* __restrict__ image, float* __restrict__ T_total, float sat_eps,
+              const uint8_t* __restrict__ state_in, uint8_t* __restrict__ state_out) {
+  __shared__ uint8_t s_use[SPLX_MAX_K];
+  __shared__ unsigned s_unsat[2];
+  const int tile = blockIdx.x, b = blockIdx.y;
+  if (SAT && threadIdx.x < 2) s_unsat[threadIdx.x] = 0u;
+  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
+  const int x = (tile % TX) * SPLX_TILE + (threadIdx.x & 15), y = (tile / TX) * SPLX_TILE + (threadIdx.x >> 4);
+  const size_t HW = (size_t)W * H;
+  const bool inside = x < W && y < H;
+  unsigned long long unsat = 0ull;
+  if (inside) {
+    const size_t pix = (size_t)y * W + x;
+    float key[KMAX]; int idx[KMAX];
+    const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
+    float Tacc = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+    unsigned long long live = 0ull;
+    for (int m = 0; m < L; ++m) {
+      const float4 p = __ldg(reinterpret_cast<const float4*>(ct) + (size_t)idx[m] * HW + pix);
+      if (SAT) { live |= 1ull << idx[m]; if (!(Tacc < sat_eps)) unsat |= 1ull << idx[m]; }
+      C0 = fmaf(Tacc, p.x, C0); C1 = fmaf(Tacc, p.y, C1); C2 = fmaf(Tacc, p.z, C2);
+      Tacc *= p.w;
+    }
+    float* im = image + 3 * ((size_t)b * HW + pix);
+    im[0] = fmaf(Tacc, bg0, C0);
+    im[1] = fmaf(Tacc, bg1, C1);
+    im[2] = fmaf(Tacc, bg2, C2);
+    if (T_total) T_total[(size_t)b * HW + pix] = Tacc;
+    // a partition that is the identity at this pixel stands behind all live ones: its front product is T_total
+    if (SAT && !(Tacc < sat_eps)) unsat |= ~live;
   }
-  image[3 * pix] = fmaf(Tacc, bg0, C0);
-  image[3 * pix + 1] = fmaf(Tacc, bg1, C1);
-  image[3 * pix + 2] = fmaf(Tacc, bg2, C2);
-  if (T_total) T_total[pix] = Tacc;
+  if (SAT) {
+    const unsigned lo = __reduce_or_sync(0xffffffffu, (unsigned)unsat);
+    const unsigned hi = __reduce_or_sync(0xffffffffu, (unsigned)(unsat >> 32));
+    if ((threadIdx.x & 31) == 0) { if (lo) atomicOr(&s_unsat[0], lo); if (hi) atomicOr(&s_unsat[1], hi); }
+    __syncthreads();
+    for (int k = threadIdx.x; k < K; k += CB) {
+      if (pv.v[k] != b) continue;
+      const size_t slot = (size_t)k * ntiles + tile;
+      const uint8_t in = state_in ? state_in[slot] : (uint8_t)0;
+      const bool u = (s_unsat[k >> 5] >> (k & 31)) & 1u;
+      state_out[slot] = (uint8_t)((in & SPLX_TILE_INVISIBLE) | (u ? 0 : SPLX_TILE_SATURATED));
+    }
+  }
 }
 
 template <int KMAX>
 __global__ void __launch_bounds__(CB)
-k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, int K, size_t HW, float bg0, float bg1,
-              float bg2, const float* __restrict__ g_image, const float* __restrict__ g_T_total,
+k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
+              const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
+              float bg1, float bg2, const float* __restrict__ g_image, const float* __restrict__ g_T_total,
               float* __restrict__ g_ct) {
-  const size_t pix = (size_t)blockIdx.x * CB + threadIdx.x;
-  if (pix >= HW) return;
+  __shared__ uint8_t s_use[SPLX_MAX_K];
+  const int tile = blockIdx.x, b = blockIdx.y;
+  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
+  const int x = (tile % TX) * SPLX_TILE + (threadIdx.x & 15), y = (tile / TX) * SPLX_TILE + (threadIdx.x >> 4);
+  if (x >= W || y >= H) return;
+  const size_t HW = (size_t)W * H, pix = (size_t)y * W + x;
   float key[KMAX]; int idx[KMAX];
-  const int L = ordered_live<KMAX>(ct, d, K, HW, pix, key, idx);
-  const float g0 = g_image[3 * pix], g1 = g_image[3 * pix + 1], g2 = g_image[3 * pix + 2];
-  const float gT = g_T_total ? g_T_total[pix] : 0.f;
+  const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
+  const float* gi = g_image + 3 * ((size_t)b * HW + pix);
+  const float g0 = gi[0], g1 = gi[1], g2 = gi[2];
+  const float gT = g_T_total ? g_T_total[(size_t)b * HW + pix] : 0.f;
   // T_total = product over the live partials in order (the empty ones multiply by 1)
   float Ttot = 1.f;
   for (int m = 0; m < L; ++m) Ttot *= __ldg(ct + 4 * ((size_t)idx[m] * HW + pix) + 3);
   // Empty partials stand behind all live ones: Tfront = T_total, Behind = bg, BehindT = 1.
   const float4 ge = make_float4(Ttot * g0, Ttot * g1, Ttot * g2, Ttot * (g0 * bg0 + g1 * bg1 + g2 * bg2 + gT));
   for (int k = 0; k < K; ++k) {
+    if (!s_use[k]) continue;
     const float T = __ldg(ct + 4 * ((size_t)k * HW + pix) + 3);
     if (!(T < 1.0f)) reinterpret_cast<float4*>(g_ct)[(size_t)k * HW + pix] = ge;
   }
@@ -123,26 +177,48 @@ k_l1(const float* __restrict__ image, const float* __restrict__ target, int64_t 
 }  // namespace
 
 // The K partials are required to be one [K,H,W,*] allocation (splx_partial describes all K).
-int launch_compose_fwd(splx_ctx* ctx, int K, const splx_partial* p, const CamDev& cam, const float* bg,
-                       float* image, float* T_total) {
-  const size_t HW = (size_t)cam.W * cam.H;
-  const unsigned grid = (unsigned)((HW + CB - 1) / CB);
-  if (K <= 8)
-    k_compose_fwd<8><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, K, HW, bg[0], bg[1], bg[2], image, T_total);
+template <int KMAX>
+static void compose_fwd_k(splx_ctx* ctx, const splx_partial* p, const uint32_t* ranges, const PlanDev& plan, int sparse,
+                          const float* bg, float* image, float* T_total, float sat_eps, uint8_t* state_out) {
+  dim3 grid(plan.ntiles, plan.B);
+  if (state_out)
+    k_compose_fwd<KMAX, true><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
+                                                           plan.ntiles, sparse, bg[0], bg[1], bg[2], image, T_total,
+                                                           sat_eps, plan.tile_state, state_out);
   else
-    k_compose_fwd<SPLX_MAX_K><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, K, HW, bg[0], bg[1], bg[2], image, T_total);
+    k_compose_fwd<KMAX, false><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
+                                                            plan.ntiles, sparse, bg[0], bg[1], bg[2], image, T_total,
+                                                            sat_eps, nullptr, nullptr);
+}
+
+int launch_compose_fwd(splx_ctx* ctx, const splx_partial* p, const splx_binning* bins, const PlanDev& plan,
+                       const float* bg, float* image, float* T_total, float sat_eps, uint8_t* state_out) {
+  const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
+  const uint32_t* ranges = bins ? bins->tile_ranges : nullptr;
+  if (plan.K <= 8) compose_fwd_k<8>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
+  else if (plan.K <= 16) compose_fwd_k<16>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
+  else if (plan.K <= 32) compose_fwd_k<32>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
+  else compose_fwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
   SPLX_LAUNCH_CHECK(ctx, "k_compose_fwd");
   return SPLX_OK;
 }
 
-int launch_compose_bwd(splx_ctx* ctx, int K, const splx_partial* p, const CamDev& cam, const float* bg,
-                       const float* g_image, const float* g_T_total, float* g_ct) {
-  const size_t HW = (size_t)cam.W * cam.H;
-  const unsigned grid = (unsigned)((HW + CB - 1) / CB);
-  if (K <= 8)
-    k_compose_bwd<8><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, K, HW, bg[0], bg[1], bg[2], g_image, g_T_total, g_ct);
-  else
-    k_compose_bwd<SPLX_MAX_K><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, K, HW, bg[0], bg[1], bg[2], g_image, g_T_total, g_ct);
+template <int KMAX>
+static void compose_bwd_k(splx_ctx* ctx, const splx_partial* p, const uint32_t* ranges, const PlanDev& plan, int sparse,
+                          const float* bg, const float* g_image, const float* g_T_total, float* g_ct) {
+  dim3 grid(plan.ntiles, plan.B);
+  k_compose_bwd<KMAX><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
+                                                   plan.ntiles, sparse, bg[0], bg[1], bg[2], g_image, g_T_total, g_ct);
+}
+
+int launch_compose_bwd(splx_ctx* ctx, const splx_partial* p, const splx_binning* bins, const PlanDev& plan,
+                       const float* bg, const float* g_image, const float* g_T_total, float* g_ct) {
+  const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
+  const uint32_t* ranges = bins ? bins->tile_ranges : nullptr;
+  if (plan.K <= 8) compose_bwd_k<8>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
+  else if (plan.K <= 16) compose_bwd_k<16>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
+  else if (plan.K <= 32) compose_bwd_k<32>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
+  else compose_bwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
   SPLX_LAUNCH_CHECK(ctx, "k_compose_bwd");
   return SPLX_OK;
 }

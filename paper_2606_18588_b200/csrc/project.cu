@@ -107,11 +107,24 @@ __device__ __forceinline__ void sh_eval(int deg, float x, float y, float z, floa
   Y[15] = -kK3a * x * (xx - 3.f * yy);
 }
 
+// Run of the launch this block works on (warp-uniform binary search over <= 64 entries).
+__device__ __forceinline__ int find_run(const RunTable& rt, int b) {
+  int lo = 0, hi = rt.n - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (rt.block_prefix[mid] <= b) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
 template <int DEG>
 __global__ void __launch_bounds__(PROJ_THREADS)
-k_project_fwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected out) {
-  const int64_t i = (int64_t)blockIdx.x * PROJ_THREADS + threadIdx.x;
-  if (i >= g.n) return;
+k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
+              splx_config cfg, splx_projected out) {
+  const int r = find_run(rt, (int)blockIdx.x);
+  const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
+  if (i >= rt.end[r]) return;
+  const CamDev& cam = plan.cam[rt.view[r]];   // the view this partition renders (indexed constant-bank loads)
   Geo G;
   bool vis = geometry(g, i, cam, cfg.dilation, G);
   float u = 0.f, v = 0.f;
@@ -224,20 +237,24 @@ __device__ __forceinline__ void cp_async_wait_all() {
 
 template <int DEG, bool ACC>
 __global__ void __launch_bounds__(PB_THREADS)
-k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, float* __restrict__ g2d,
-              int clear_g2d, splx_gaussian_grads out) {
+k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
+              splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out) {
   extern __shared__ __align__(16) float s_dyn[];
   float* s_sh = s_dyn;                                   // [128][52] sh in, SH gradient out
   float* s_old = s_dyn + PB_THREADS * PB_STRIDE;         // [128][52] previous SH gradient (ACC only)
   __shared__ __align__(16) float s_m[PB_THREADS * 3];    // mean gradient tile
   __shared__ __align__(16) float s_s[PB_THREADS * 3];    // log_scale gradient tile
   __shared__ uint8_t s_vis[PB_THREADS];
-  const int64_t base = (int64_t)blockIdx.x * PB_THREADS;
+  const int run = find_run(rt, (int)blockIdx.x);
+  const int64_t base = rt.begin[run] + (int64_t)((int)blockIdx.x - rt.block_prefix[run]) * PB_THREADS;
+  const int64_t run_end = rt.end[run];
   const int64_t i = base + threadIdx.x;
-  const int nrows = (int)min((int64_t)PB_THREADS, g.n - base);
+  const int nrows = (int)min((int64_t)PB_THREADS, run_end - base);
+  const int view = rt.view[run];                          // < 0: a non-participating partition (OVERWRITE only): zeros
+  const CamDev& cam = plan.cam[view < 0 ? 0 : view];
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;        // float4 chunks of a row that hold used coefficients
-  const bool vis = (i < g.n) && (pr.radius[i] > 0);
+  const bool vis = (i < run_end) && (view >= 0) && (pr.radius[i] > 0);
   s_vis[threadIdx.x] = vis ? 1 : 0;
   __syncthreads();
 #pragma unroll
@@ -378,7 +395,7 @@ k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, 
   }
 #pragma unroll
   for (int k = 0; k < 3; ++k) { s_m[3 * threadIdx.x + k] = dmu[k]; s_s[3 * threadIdx.x + k] = dls[k]; }
-  if (i < g.n) {
+  if (i < run_end) {
     float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
     if (ACC) {
       if (vis) {
@@ -412,8 +429,9 @@ k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, 
       }
     }
   }
-  // mean / log_scale gradient tiles: 96 float4 each; a partial last block falls back to scalars
-  if (nrows == PB_THREADS) {
+  // mean / log_scale gradient tiles: 96 float4 each; a partial last block, or a run that does not start
+  // on a multiple of 4 Gaussians (12-byte rows: 16-byte alignment needs base % 4 == 0), falls back to scalars
+  if (nrows == PB_THREADS && (base & 3) == 0) {
     if (threadIdx.x < 96) {
       float4* dm = reinterpret_cast<float4*>(out.mean + 3 * base) + threadIdx.x;
       float4* ds = reinterpret_cast<float4*>(out.log_scale + 3 * base) + threadIdx.x;
@@ -425,7 +443,7 @@ k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, 
       }
       *dm = a; *ds = b;
     }
-  } else if (i < g.n) {
+  } else if (i < run_end) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       if (ACC) { out.mean[3 * i + k] += dmu[k]; out.log_scale[3 * i + k] += dls[k]; }
@@ -435,47 +453,51 @@ k_project_bwd(splx_gaussians g, CamDev cam, splx_config cfg, splx_projected pr, 
 }
 
 template <int DEG, bool ACC>
-static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, const splx_projected* pr, float* g2d,
-                      int clear_g2d, const splx_gaussian_grads* grads) {
-  const unsigned grid = (unsigned)((g->n + PB_THREADS - 1) / PB_THREADS);
+static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
+                      const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
   cudaFuncSetAttribute(k_project_bwd<DEG, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  k_project_bwd<DEG, ACC><<<grid, PB_THREADS, smem, ctx->stream>>>(*g, cam, ctx->cfg, *pr, g2d, clear_g2d, *grads);
+  k_project_bwd<DEG, ACC><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(*g, plan, rt, ctx->cfg, *pr, g2d,
+                                                                                      clear_g2d, *grads);
 }
 
 }  // namespace
 
-int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, int deg,
+int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
                        const splx_projected* out) {
-  if (g->n == 0) return SPLX_OK;
-  const unsigned grid = (unsigned)((g->n + PROJ_THREADS - 1) / PROJ_THREADS);
+  const RunTable rt = make_runs(plan, part_offsets, PROJ_THREADS, false);
+  if (rt.blocks_total == 0) return SPLX_OK;
+  const unsigned grid = (unsigned)rt.blocks_total;
   switch (deg) {
-    case 0: k_project_fwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
-    case 1: k_project_fwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
-    case 2: k_project_fwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
-    default: k_project_fwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, cam, ctx->cfg, *out); break;
+    case 0: k_project_fwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 1: k_project_fwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 2: k_project_fwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    default: k_project_fwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
   }
   SPLX_LAUNCH_CHECK(ctx, "k_project_fwd");
   return SPLX_OK;
 }
 
-int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const CamDev& cam, int deg,
+int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
                        const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads) {
-  if (g->n == 0) return SPLX_OK;
   const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
-  if (flags & SPLX_PB_OVERWRITE) {
+  const bool overwrite = (flags & SPLX_PB_OVERWRITE) != 0;
+  // "=" must also clear the rows of partitions that do not participate in this launch
+  const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, overwrite);
+  if (rt.blocks_total == 0) return SPLX_OK;
+  if (overwrite) {
     switch (deg) {
-      case 0: launch_pb<0, false>(ctx, g, cam, pr, g2d, clr, grads); break;
-      case 1: launch_pb<1, false>(ctx, g, cam, pr, g2d, clr, grads); break;
-      case 2: launch_pb<2, false>(ctx, g, cam, pr, g2d, clr, grads); break;
-      default: launch_pb<3, false>(ctx, g, cam, pr, g2d, clr, grads); break;
+      case 0: launch_pb<0, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
+      case 1: launch_pb<1, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
+      case 2: launch_pb<2, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
+      default: launch_pb<3, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
     }
   } else {
     switch (deg) {
-      case 0: launch_pb<0, true>(ctx, g, cam, pr, g2d, clr, grads); break;
-      case 1: launch_pb<1, true>(ctx, g, cam, pr, g2d, clr, grads); break;
-      case 2: launch_pb<2, true>(ctx, g, cam, pr, g2d, clr, grads); break;
-      default: launch_pb<3, true>(ctx, g, cam, pr, g2d, clr, grads); break;
+      case 0: launch_pb<0, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
+      case 1: launch_pb<1, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
+      case 2: launch_pb<2, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
+      default: launch_pb<3, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
     }
   }
   SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");

@@ -119,16 +119,19 @@ __device__ __forceinline__ bool eval_alpha(float dx, float dy, float adx, float 
 template <bool COUNT>
 __global__ void __launch_bounds__(BLOCK)
 k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
-             int W, int H, int TX, int ntiles, splx_config cfg, float* __restrict__ out_ct,
-             float* __restrict__ out_d, uint32_t* __restrict__ out_n, unsigned long long* pairs) {
+             int W, int H, int TX, int ntiles, splx_config cfg, const __grid_constant__ PartView pv, int sparse,
+             float* __restrict__ out_ct, float* __restrict__ out_d, uint32_t* __restrict__ out_n,
+             unsigned long long* pairs) {
   __shared__ Ring rings[WARPS];
   const int tile = blockIdx.x, k = blockIdx.y;
+  if (pv.v[k] < 0) return;                 // the partition does not participate in this launch
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   Ring& ring = rings[warp];
   const int X0 = (tile % TX) * SPLX_TILE, Y0 = (tile / TX) * SPLX_TILE + 8 * warp;
   const int pxi = X0 + (lane & 7), pyi = Y0 + (lane >> 3);          // slot 0 pixel; slot s adds (8(s&1), 4(s>>1))
   const float px0 = (float)pxi + 0.5f, px1 = px0 + 8.0f, py0 = (float)pyi + 0.5f, py1 = py0 + 4.0f;
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
+  if (sparse && r0 == r1) return;          // SPLX_PLAN_SPARSE: an empty list is the identity partial, never stored
   const float log2_amin = cfg.alpha_min > 0.f ? log2f(cfg.alpha_min) : -INFINITY;
 
   float T[4], C0[4], C1[4], C2[4], D[4];
@@ -371,26 +374,27 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 
 }  // namespace
 
-int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, int K,
-                      const CamDev& cam, const splx_partial* out, uint64_t* pairs) {
-  const int ntiles = cam.TX * cam.TY;
-  dim3 grid(ntiles, K);
+int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, const PlanDev& plan,
+                      const splx_partial* out, uint64_t* pairs) {
+  dim3 grid(plan.ntiles, plan.K);
+  const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
   if (pairs)
-    k_render_fwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles,
-                                                        ctx->cfg, out->ct, out->d, out->n_contrib, (unsigned long long*)pairs);
+    k_render_fwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
+                                                        plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d,
+                                                        out->n_contrib, (unsigned long long*)pairs);
   else
-    k_render_fwd<false><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles,
-                                                         ctx->cfg, out->ct, out->d, out->n_contrib, nullptr);
+    k_render_fwd<false><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
+                                                         plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d,
+                                                         out->n_contrib, nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_render_fwd");
   return SPLX_OK;
 }
 
-int launch_raster_bwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, int K,
-                      const CamDev& cam, const splx_partial* part, const float* g_ct, float* g2d) {
-  const int ntiles = cam.TX * cam.TY;
-  dim3 grid(ntiles, K);
-  k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, cam.W, cam.H, cam.TX, ntiles,
-                                                ctx->cfg, part->ct, part->n_contrib, g_ct, g2d);
+int launch_raster_bwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, const PlanDev& plan,
+                      const splx_partial* part, const float* g_ct, float* g2d) {
+  dim3 grid(plan.ntiles, plan.K);   // slots of non-participating partitions have empty ranges and exit at once
+  k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
+                                                plan.ntiles, ctx->cfg, part->ct, part->n_contrib, g_ct, g2d);
   SPLX_LAUNCH_CHECK(ctx, "k_raster_bwd");
   return SPLX_OK;
 }

@@ -102,7 +102,7 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
 
 template <class Op>
 __global__ void __launch_bounds__(SCAN_THREADS)
-k_scan(Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
+k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
        uint64_t clamp_to) {
   __shared__ uint32_t sm[33];
   __shared__ uint32_t s_tile;
@@ -142,12 +142,27 @@ k_scan(Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_
   for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex); ex += v[k]; }
 }
 
+// Element j of the launch -> Gaussian index, through the runs of the participating partitions
+// (non-participants are never read: their tiles_touched may be stale).
+struct RunMap {
+  int n;
+  int64_t begin[SPLX_MAX_K], jprefix[SPLX_MAX_K + 1];
+  __device__ uint64_t operator()(uint64_t j) const {
+    int lo = 0, hi = n - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if ((uint64_t)jprefix[mid] <= j) lo = mid; else hi = mid - 1;
+    }
+    return (uint64_t)begin[lo] + (j - (uint64_t)jprefix[lo]);
+  }
+};
+
 struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order preserved
-  const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n;
+  const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n; RunMap map;
   __device__ uint64_t count(const uint64_t*) const { return n; }
-  __device__ uint32_t load(uint64_t i) const { return tiles_touched[i] > 0 ? 1u : 0u; }
-  __device__ void store(uint64_t i, uint32_t v, uint32_t ex) const {
-    if (v) { ckeys[ex] = __float_as_uint(depth[i]); cvals[ex] = (uint32_t)i; }
+  __device__ uint32_t load(uint64_t j) const { return tiles_touched[map(j)] > 0 ? 1u : 0u; }
+  __device__ void store(uint64_t j, uint32_t v, uint32_t ex) const {
+    if (v) { const uint64_t i = map(j); ckeys[ex] = __float_as_uint(depth[i]); cvals[ex] = (uint32_t)i; }
   }
 };
 struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, depth order
@@ -388,11 +403,13 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
 }
 
 __global__ void __launch_bounds__(256)
-k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, uint32_t* __restrict__ ranges) {
+k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint8_t* __restrict__ tile_state,
+              uint32_t* __restrict__ ranges) {
   const uint64_t m = cnt->m_sorted;
   const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= m) return;
   const uint32_t s = (uint32_t)(keys[j] >> 32);
+  if (tile_state && tile_state[s]) return;   // a skipped (partition, tile) slot keeps the empty range (0,0)
   if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
   if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
 }
@@ -441,8 +458,10 @@ size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY) {
   return make_layout(n, capacity, slot_bits(K, TX, TY)).total;
 }
 
-int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, const int64_t* part_offsets,
-                    const CamDev& cam, const splx_binning* out, void* ws, size_t ws_bytes) {
+int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const PlanDev& plan, const int64_t* part_offsets,
+                    const splx_binning* out, void* ws, size_t ws_bytes) {
+  const int K = plan.K;
+  const PlanDev& cam = plan;   // TX, TY
   const int sbits = slot_bits(K, cam.TX, cam.TY);
   if (sbits > 8 * MAX_PASSES) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles needs %d key bits (max 32)", sbits);
   const Layout L = make_layout(n, out->capacity, sbits);
@@ -458,22 +477,27 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, c
 
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(base, 0, L.zero_bytes, ctx->stream));
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->tile_ranges, 0, (size_t)K * ntiles * 2 * sizeof(uint32_t), ctx->stream));
-  if (n == 0 || out->capacity == 0) {
+  const RunTable rt = make_runs(plan, part_offsets, 1, false);
+  const int64_t n_act = rt.jprefix[rt.n];    // Gaussians of the participating partitions
+  if (n_act == 0 || out->capacity == 0) {
     k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
     SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
     return SPLX_OK;
   }
   int rc;
   // 1. visible Gaussians, index order
-  VisibleOp vop{pr->tiles_touched, pr->depth, ckeys_a, cvals_a, (uint64_t)n};
-  if ((rc = scan_exclusive(ctx, vop, (uint64_t)n, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
+  VisibleOp vop{pr->tiles_touched, pr->depth, ckeys_a, cvals_a, (uint64_t)n_act, {}};
+  vop.map.n = rt.n;
+  for (int r = 0; r < rt.n; ++r) { vop.map.begin[r] = rt.begin[r]; vop.map.jprefix[r] = rt.jprefix[r]; }
+  vop.map.jprefix[rt.n] = rt.jprefix[rt.n];
+  if ((rc = scan_exclusive(ctx, vop, (uint64_t)n_act, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
                            &cnt->n_visible, nullptr, 0))) return rc;
   // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers)
-  if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n, &cnt->n_visible, 0, 32,
+  if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n_act, &cnt->n_visible, 0, 32,
                                  (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2]))) return rc;
   // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
-  if ((rc = scan_exclusive(ctx, top, (uint64_t)n, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
+  if ((rc = scan_exclusive(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
                            &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
   const int passes = (sbits + 7) / 8;
   uint64_t* k0 = (passes & 1) ? keys_tmp : out->keys;   // so that the last pass lands in out->keys
@@ -483,14 +507,15 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, int K, c
   PartOffs parts;
   parts.K = K;
   for (int k = 0; k <= K; ++k) parts.off[k] = part_offsets[k];
-  k_emit_keys<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(
+  k_emit_keys<<<(unsigned)((n_act + 255) / 256), 256, 0, ctx->stream>>>(
       pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
   // 4. stable sort on the slot bits
   if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
                                  (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6]))) return rc;
   // 5. ranges
-  k_tile_ranges<<<(unsigned)((out->capacity + 255) / 256), 256, 0, ctx->stream>>>(out->keys, cnt, out->tile_ranges);
+  k_tile_ranges<<<(unsigned)((out->capacity + 255) / 256), 256, 0, ctx->stream>>>(out->keys, cnt, plan.tile_state,
+                                                                                         out->tile_ranges);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
   k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
   SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
