@@ -59,6 +59,12 @@ class Trainer:
         self._cam = None
         self._ws_sort = None
         self._ws_bwd = None
+        # plan path (visibility prediction / consolidated views): buffers with a leading view dimension
+        self._images = self._T_totals = self._g_images = None
+        self._plan = None
+        self._participants = {}     # view id -> partition bitmask (splx_visible_regions)
+        self._geom_state = {}       # view id -> host uint8 [K, tiles]
+        self._bucket_state = {}     # tuple of view ids -> device uint8 [K * tiles] (geometric | saturated bits)
 
     # -- workspaces are sized per camera resolution (constant here) ----------------------------
     def _workspaces(self, cam):
@@ -111,3 +117,106 @@ class Trainer:
 
     def zero_grad(self):
         self.flat["grad"].zero_()
+
+    # ---- launch plans: visibility prediction and consolidated views (L247-L249) ----
+    def _view_buffers(self, B):
+        if self._images is None or self._images.shape[0] < B:
+            dev = self.ctx.device
+            self._images = torch.empty((B, self.H, self.W, 3), dtype=torch.float32, device=dev)
+            self._T_totals = torch.empty((B, self.H, self.W), dtype=torch.float32, device=dev)
+            self._g_images = torch.empty((B, self.H, self.W, 3), dtype=torch.float32, device=dev)
+        return self._images[:B], self._T_totals[:B], self._g_images[:B]
+
+    def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True) -> binding.Plan:
+        if view_of_part is None:
+            view_of_part = [0] * self.K
+        return binding.Plan(cams, view_of_part, tile_state, sparse)
+
+    def forward_plan(self, plan: binding.Plan, sat_eps=None, tile_state_out=None, count_pairs=False):
+        """a1-a6 for all views of the plan in one launch per stage; returns images[B,H,W,3]."""
+        self._workspaces(plan.cams[0])
+        self._plan = plan
+        c = self.ctx
+        images, T_totals, _ = self._view_buffers(plan.B)
+        c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
+        c.bin_sort_plan(self.proj, self.part_offsets, plan, self.bins, self._ws_sort)
+        c.render_partial_plan(self.proj, self.bins, plan, self.partials, self.pairs if count_pairs else None)
+        c.compose_plan(self.partials, self.bins, plan, self.bg, images, T_totals,
+                       sat_eps if sat_eps is not None else 0.0, tile_state_out)
+        return images
+
+    def loss_grad_plan(self, targets):
+        """a7 for B views at once: targets[B,H,W,3]; every view's loss is its own mean (scale = B)."""
+        B = self._plan.B
+        images, _, g_images = self._view_buffers(B)
+        self.ctx.l1_loss_grad(images, targets, g_images, self.loss_sum, float(B))
+
+    def backward_plan(self, overwrite=False, g_images=None):
+        plan = self._plan
+        _, _, gi = self._view_buffers(plan.B)
+        self.ctx.backward_plan(self.part_offsets, plan, self.partials, self.bg, gi if g_images is None else g_images,
+                               None, self.params, self.proj, self.bins, self.sh_degree, self.grads, self._ws_bwd,
+                               overwrite=overwrite)
+
+    def set_aabbs(self, lo, hi):
+        """Static partition boxes (scenes.partition_aabbs) for the geometric visibility prediction."""
+        self._aabb = (np.ascontiguousarray(lo, np.float32), np.ascontiguousarray(hi, np.float32))
+        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear()
+
+    def participants(self, view_id, cam) -> int:
+        """GetParticipants(v) (L249): partitions whose box meets the view frustum; cached per view id."""
+        if view_id not in self._participants:
+            state, part = binding.visible_regions(self._aabb[0], self._aabb[1], cam)
+            for k in range(self.K):                       # an empty partition never participates
+                if self.part_offsets[k + 1] == self.part_offsets[k]:
+                    part &= ~(1 << k)
+                    state[k] = binding.TILE_INVISIBLE
+            self._participants[view_id] = part
+            self._geom_state[view_id] = state
+        return self._participants[view_id]
+
+    def buckets(self, view_ids, cams, consolidate=True, max_views=binding.MAX_VIEWS):
+        """Conflict-free buckets (L249) over the given views: list of lists of positions into view_ids."""
+        parts = [self.participants(v, c) for v, c in zip(view_ids, cams)]
+        if not consolidate:
+            return [[i] for i in range(len(view_ids))]
+        bucket_of, nb = binding.schedule_views(parts, max_views)
+        out = [[] for _ in range(nb)]
+        for i, b in enumerate(bucket_of):
+            out[b].append(i)
+        return out
+
+    def bucket_plan(self, view_ids, cams, saturation=True, sparse=True):
+        """Plan of one conflict-free bucket: every partition renders the view it participates in; the tile state
+        (geometric bits now, saturated bits as compose detects them) persists per bucket across iterations."""
+        key = tuple(view_ids)
+        vop = [-1] * self.K
+        for j, (v, cam) in enumerate(zip(view_ids, cams)):
+            part = self.participants(v, cam)
+            for k in range(self.K):
+                if (part >> k) & 1:
+                    assert vop[k] < 0, "views of a bucket must not share a partition"
+                    vop[k] = j
+        if key not in self._bucket_state:
+            st = np.full((self.K, self._geom_state[view_ids[0]].shape[1]), binding.TILE_INVISIBLE, np.uint8)
+            for k in range(self.K):
+                if vop[k] >= 0:
+                    st[k] = self._geom_state[view_ids[vop[k]]][k]
+            self._bucket_state[key] = torch.from_numpy(st.reshape(-1)).to(self.ctx.device)
+        state = self._bucket_state[key]
+        return self.make_plan(cams, vop, state, sparse), (state if saturation else None)
+
+    def iteration_views(self, view_ids, cams, targets, consolidate=True, saturation=True, sat_eps=1e-4, sparse=True):
+        """One training iteration over B views with visibility prediction: geometric participants and tile
+        regions, saturated tiles skipped from the previous visit of the same bucket on, conflict-free views
+        consolidated into one launch per stage.  targets: device tensor [B,H,W,3].  Returns the number of launches
+        of the forward (= buckets)."""
+        groups = self.buckets(view_ids, cams, consolidate)
+        for gi, grp in enumerate(groups):
+            plan, state_out = self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse)
+            self.forward_plan(plan, sat_eps, state_out)
+            tg = targets[grp[0]:grp[0] + 1] if len(grp) == 1 else targets[torch.as_tensor(grp, device=targets.device)]
+            self.loss_grad_plan(tg)
+            self.backward_plan(overwrite=(gi == 0))
+        self.adam_step(len(view_ids))
+        return len(groups)

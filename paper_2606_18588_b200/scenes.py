@@ -118,6 +118,24 @@ def grid_partition(mean, lo, hi, gx, gy):
     return iy * gx + ix
 
 
+def partition_aabbs(params, part_offsets, inflate_sigma=3.0):
+    """Axis-aligned box of every partition (partitions are AABBs): the bounding box of
+    its Gaussians' supports, a Gaussian's support being its mean +- inflate_sigma x its largest scale (reading
+    s21; inflate_sigma = 0 gives the box of the means).  Static input of the geometric visibility
+    prediction; an empty partition gets the degenerate box lo = hi = 0 (callers drop it from the participants)."""
+    K = len(part_offsets) - 1
+    lo = np.zeros((K, 3), np.float32)
+    hi = np.zeros((K, 3), np.float32)
+    for k in range(K):
+        a, b = int(part_offsets[k]), int(part_offsets[k + 1])
+        if b > a:
+            m = params["mean"][a:b].astype(np.float64)
+            r = inflate_sigma * np.exp(params["log_scale"][a:b].astype(np.float64).max(1))[:, None]
+            lo[k] = np.floor((m - r).min(0) * 1024) / 1024        # outward rounding to a float32-exact grid
+            hi[k] = np.ceil((m + r).max(0) * 1024) / 1024
+    return lo, hi
+
+
 def tiny(seed=0, n=4096, size=128, f=150.0, K=2, sh_degree=0):
     """BASELINE.json configs[0]: world frame = camera frame, K contiguous depth chunks."""
     rng = np.random.default_rng(seed)
@@ -242,3 +260,26 @@ def small_aerial(seed=0, n=20_000, width=320, height=176, K=(2, 2), sh_degree=3)
     and scales enlarged so the per-pixel list lengths stay comparable."""
     return aerial(seed=seed, n=n, width=width, height=height, grid=K, sh_degree=sh_degree,
                   log_scale_mu=-0.9, fov_deg=60.0, name=f"aerial_{n}")
+
+
+def small_city(seed=0, n=30_000, width=320, height=176, n_views=4, grid=(4, 2)):
+    """configs[2] shrunk for CPU tests and element-by-element parity: same recipe on a 120 m block with 12
+    buildings, B views looking at different parts of it (so that a view touches only some partitions)."""
+    return city(seed=seed, n=n, width=width, height=height, extent=120.0, n_buildings=12, grid=grid,
+                altitude=35.0, height_range=(5.0, 25.0), n_views=n_views, name=f"city_{n}")
+
+
+def small_blocks(seed=0, n=24_000, width=320, height=176, n_views=6, grid=(4, 2), extent=(240.0, 120.0, 6.0),
+                 altitude=22.0, pitch_deg=62.0):
+    """A wide, flat configs[1]-style box cut into grid cells, seen by B low cameras that each look at a
+    different spot: a view touches only one to three partitions, so conflict-free buckets
+    with several views exist.  Scales are set from the point spacing so that lists stay short."""
+    sc = aerial(seed=seed, n=n, width=width, height=height, extent=extent, grid=grid, sh_degree=3, n_views=0,
+                log_scale_mu=float(np.log(0.9 * np.sqrt(extent[0] * extent[1] / n))), log_scale_sigma=0.25,
+                name=f"blocks_{n}")
+    crng = np.random.default_rng(seed + 2)
+    for v in range(n_views):
+        tgt = (crng.uniform(-0.42, 0.42) * extent[0], crng.uniform(-0.35, 0.35) * extent[1], 0.0)
+        sc.cameras.append(aerial_camera(width, height, 60.0, altitude, pitch_deg, crng.uniform(0, 360), tgt))
+        sc.targets.append(np.random.default_rng(seed + 1 + 1000 * v).uniform(0, 1, (height, width, 3)).astype(np.float32))
+    return sc

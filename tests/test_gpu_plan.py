@@ -1,0 +1,281 @@
+"""-m gpu parity tests of the two optional subsystems through the C ABI (the *_plan calls): visibility
+prediction and conflict-free consolidation of B views (L247-L249), against
+oracle/visibility.py.  Same bars as the core: integers bit-exact, images 1e-5, gradients 1e-3."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import visibility as ov
+from paper_2606_18588_b200 import binding, scenes
+from tests import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+
+def _trainer(sc):
+    tr = G.make_trainer(sc)
+    tr.set_aabbs(*scenes.partition_aabbs(sc.params, sc.part_offsets))
+    return tr
+
+
+def _grads_np(tr):
+    return {k: G.np32(tr.grads[k]).astype(np.float64) for k in scenes.PARAM_KEYS}
+
+
+def _check_grads(tr, ref_grads, exclude=None):
+    for key in scenes.PARAM_KEYS:
+        got = G.np32(tr.grads[key]).astype(np.float64)
+        ref = np.concatenate([g[key].reshape(-1) for g in ref_grads])
+        assert G.rel_l2(got, ref) <= 1e-3, (key, G.rel_l2(got, ref))
+        assert G.grad_close(got, ref) <= 5e-3, (key, G.grad_close(got, ref))
+
+
+def _fragile(res):
+    frag = np.zeros(res.image.shape[:2], bool)
+    for pa in res.partials:
+        frag |= pa.margin < G.FRAGILE_MARGIN
+    if res.order_margin is not None:
+        frag |= res.order_margin < 1e-6
+    return frag
+
+
+@pytest.fixture(scope="module")
+def aerial():
+    return scenes.small_aerial()
+
+
+@pytest.fixture(scope="module")
+def city():
+    return scenes.small_city()       # every view sees every partition; opaque: saturation everywhere
+
+
+@pytest.fixture(scope="module")
+def blocks():
+    return scenes.small_blocks()     # a view sees 2-4 of the 8 partitions: conflict-free buckets exist
+
+
+def test_sparse_partials_change_nothing(aerial):
+    """SPLX_PLAN_SPARSE only avoids storing and loading identity partials: image bit-equal, gradients equal."""
+    sc = aerial
+    cam = sc.cameras[0]
+    target = torch.from_numpy(sc.targets[0]).cuda()[None]
+    out = []
+    for sparse in (False, True):
+        tr = _trainer(sc)
+        tr.partials.ct.fill_(float("nan")); tr.partials.d.fill_(float("nan"))   # unread slots may hold anything
+        plan = tr.make_plan([cam], None, None, sparse)
+        img = tr.forward_plan(plan).clone()
+        tr.loss_grad_plan(target)
+        tr.backward_plan(overwrite=True)
+        torch.cuda.synchronize()
+        out.append((img, _grads_np(tr), tr))
+    assert torch.equal(out[0][0], out[1][0])
+    assert not torch.isnan(out[1][0]).any()
+    for key in scenes.PARAM_KEYS:
+        assert G.grad_close(out[1][1][key], out[0][1][key]) <= 1e-4, key
+    # and the dense plan is the single-view call
+    tr = out[0][2]
+    tr.forward(cam)
+    assert torch.equal(tr.image, out[0][0][0])
+
+
+def test_geometric_state_and_masked_binning(city):
+    """splx_visible_regions == LP oracle on the scene's own boxes; bin_sort under the state keeps keys/vals and
+    zeroes exactly the ranges of the skipped slots (bit-exact, teacher-forced)."""
+    sc = city
+    cam = sc.cameras[1]
+    lo, hi = scenes.partition_aabbs(sc.params, sc.part_offsets, inflate_sigma=0.0)   # tight boxes: some lists are cut
+    tr = G.make_trainer(sc)
+    state, part = binding.visible_regions(lo, hi, cam)
+    ref, part_ref, margin = ov.visible_regions(lo, hi, cam.as_array())
+    robust = np.abs(margin) > 1e-6
+    assert np.array_equal(state[robust], ref[robust]) and part == part_ref and robust.mean() > 0.98
+    assert 0 < (state == 0).mean() < 1
+    vop = [0 if (part >> k) & 1 else -1 for k in range(sc.K)]
+    dev_state = torch.from_numpy(state.reshape(-1)).cuda()
+    c = tr.ctx
+    tr._workspaces(cam)
+    # unmasked reference binning on the GPU
+    plan0 = tr.make_plan([cam], vop, None, False)
+    c.project_plan(tr.params, tr.part_offsets, plan0, tr.sh_degree, tr.proj)
+    c.bin_sort_plan(tr.proj, tr.part_offsets, plan0, tr.bins, tr._ws_sort)
+    M0, keys0, vals0, ranges0 = G.gpu_bins(tr)
+    keys0, vals0, ranges0 = keys0.copy(), vals0.copy(), ranges0.copy()
+    plan1 = tr.make_plan([cam], vop, dev_state, False)
+    c.bin_sort_plan(tr.proj, tr.part_offsets, plan1, tr.bins, tr._ws_sort)
+    M1, keys1, vals1, ranges1 = G.gpu_bins(tr)
+    assert M1 == M0 and np.array_equal(keys1, keys0) and np.array_equal(vals1, vals0)
+    n_cut = 0
+    pr = G.gpu_projected(tr)
+    pos = 0
+    for k in range(sc.K):
+        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        if vop[k] < 0:
+            assert not ranges1[k].any()
+            continue
+        bn = oracle.bin_sort(pr.means2d[a:b], pr.radius[a:b], pr.depth[a:b], cam.width, cam.height)
+        want = ov.apply_tile_state(bn.ranges, state[k]).astype(np.int64)
+        live = want[:, 1] > want[:, 0]
+        assert np.array_equal(ranges1[k][live].astype(np.int64), want[live] + pos)
+        assert not ranges1[k][~live].any()
+        n_cut += int(((bn.ranges[:, 1] > bn.ranges[:, 0]) & ~live).sum())
+        pos += bn.M
+    assert pos == M1 and n_cut > 0, "tight boxes must cut some boundary lists"
+
+
+def test_non_participants_are_skipped_and_cleared(blocks):
+    """A partition with view -1 is not projected (its projected rows keep stale values), gets no keys, and
+    SPLX_PB_OVERWRITE writes zeros into its gradient rows."""
+    sc = blocks
+    cam = sc.cameras[1]
+    tr = _trainer(sc)
+    part = tr.participants(1, cam)
+    vop = [0 if (part >> k) & 1 else -1 for k in range(sc.K)]
+    assert 0 < sum(v == 0 for v in vop) < sc.K
+    tr.proj.tiles_touched.fill_(7); tr.proj.radius.fill_(9)
+    for v in tr.grads.values():
+        v.fill_(5.0)
+    plan = tr.make_plan([cam], vop, None, True)
+    tr.forward_plan(plan)
+    tr.loss_grad_plan(torch.from_numpy(sc.targets[0]).cuda()[None])
+    tr.backward_plan(overwrite=True)
+    torch.cuda.synchronize()
+    tt = G.u32(tr.proj.tiles_touched)
+    vals = G.u32(tr.bins.vals)[:tr.num_intersections()]
+    for k in range(sc.K):
+        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        inside = ((vals >= a) & (vals < b)).sum()
+        if vop[k] < 0:
+            assert (tt[a:b] == 7).all() and inside == 0
+            for key in scenes.PARAM_KEYS:
+                w = scenes.PARAM_WIDTH[key]
+                assert not G.np32(tr.grads[key])[a * w:b * w].any(), key
+        else:
+            assert (tt[a:b] != 7).any()
+    # against the oracle on the participating partitions only, and against the oracle on ALL partitions: the
+    # boxes contain every 3-sigma support, so dropping the non-participants changes nothing
+    views, grads = ov.iteration_plan(sc.partitions(), [cam.as_array()], vop, sc.sh_degree, [sc.targets[0]], sc.bg)
+    res_all = oracle.forward(sc.partitions(), cam.as_array(), sc.sh_degree, sc.bg)
+    assert np.array_equal(res_all.image, views[0].image)
+    frag = _fragile(views[0])
+    img = G.np32(tr._images[0]).astype(np.float64)
+    assert (G.close(img, views[0].image).all(-1) | frag).mean() >= 1 - 1e-4
+    _check_grads(tr, grads)
+
+
+def test_saturation_detection_teacher_forced(city):
+    """compose's tile_state_out against the oracle's front products computed from the GPU's own partials."""
+    sc = city
+    cam = sc.cameras[0]
+    for eps in (1e-4, 1e-2):
+        tr = _trainer(sc)
+        part = tr.participants(0, cam)
+        vop = [0 if (part >> k) & 1 else -1 for k in range(sc.K)]
+        members = [k for k in range(sc.K) if vop[k] == 0]
+        geom = tr._geom_state[0]
+        state_dev = torch.from_numpy(geom.reshape(-1).copy()).cuda()
+        plan = tr.make_plan([cam], vop, state_dev, False)          # dense: every participant's partial is stored
+        out = torch.full_like(state_dev, 77)
+        tr.forward_plan(plan, eps, out)
+        torch.cuda.synchronize()
+        ct = G.np32(tr.partials.ct).astype(np.float64); d = G.np32(tr.partials.d).astype(np.float64)
+        ref, margin = ov.saturation(ct, d, eps, geom, members)
+        got = G.np32(out).reshape(sc.K, -1)
+        for k in range(sc.K):
+            if vop[k] < 0:
+                assert (got[k] == 77).all()          # rows of non-participants are not touched
+                continue
+            robust = margin[k] > 1e-5
+            assert np.array_equal(got[k][robust], ref[k][robust]), (eps, k)
+            assert robust.mean() > 0.99
+        if eps == 1e-2:
+            assert (ref[members] & ov.TILE_SATURATED).any(), "the city scene must saturate somewhere at eps = 1e-2"
+
+
+def test_consolidated_bucket_against_the_oracle(blocks):
+    """B views of a conflict-free bucket in ONE launch per stage: images per view and the summed gradients
+    against the oracle's plan iteration, and against the same views run one by one on the GPU."""
+    sc = blocks
+    tr = _trainer(sc)
+    ids = list(range(len(sc.cameras)))
+    groups = tr.buckets(ids, sc.cameras, consolidate=True)
+    parts = [tr.participants(v, sc.cameras[v]) for v in ids]
+    ref_b, nb = ov.schedule_views(parts)
+    assert [sorted(g) for g in groups] == [sorted(i for i in ids if ref_b[i] == b) for b in range(nb)]
+    multi = [g for g in groups if len(g) > 1]
+    assert multi, "the test scene must have a bucket with more than one view"
+    grp = multi[0]
+    cams = [sc.cameras[i] for i in grp]
+    plan, _ = tr.bucket_plan(grp, cams, saturation=False)
+    targets = torch.from_numpy(np.stack([sc.targets[i] for i in grp])).cuda()
+    imgs = tr.forward_plan(plan).clone()
+    tr.loss_grad_plan(targets)
+    tr.backward_plan(overwrite=True)
+    torch.cuda.synchronize()
+    state = G.np32(plan.tile_state).reshape(sc.K, -1)
+    views, grads = ov.iteration_plan(sc.partitions(), [c.as_array() for c in cams], plan.view_of_part, sc.sh_degree,
+                                     [sc.targets[i] for i in grp], sc.bg, tile_state=state)
+    for j, res in enumerate(views):
+        frag = _fragile(res)
+        img = G.np32(imgs[j]).astype(np.float64)
+        ok = G.close(img, res.image).all(-1)
+        assert (~(ok | frag)).sum() <= 1e-4 * frag.size, j
+        assert np.abs(img - res.image).max() <= G.FRAGILE_TOL
+    _check_grads(tr, grads)
+    g_multi = _grads_np(tr)
+    # the same views one after the other (one-view plans, gradients accumulated): same images, same sum
+    tr2 = _trainer(sc)
+    for j, i in enumerate(grp):
+        vop = [0 if plan.view_of_part[k] == j else -1 for k in range(sc.K)]
+        p1 = tr2.make_plan([sc.cameras[i]], vop, plan.tile_state, True)
+        img1 = tr2.forward_plan(p1)
+        assert torch.equal(img1[0], imgs[j])
+        tr2.loss_grad_plan(targets[j:j + 1])
+        tr2.backward_plan(overwrite=(j == 0))
+    torch.cuda.synchronize()
+    g_seq = _grads_np(tr2)
+    for key in scenes.PARAM_KEYS:
+        assert G.grad_close(g_multi[key], g_seq[key]) <= 1e-4, key
+
+
+def test_iteration_views_with_visibility_prediction(city):
+    """The whole subsystem: two iterations over B views; the second applies the saturated tiles the first
+    detected.  Every skipped slot has (oracle) front product < eps, and the image stays within eps * max rgb of
+    the oracle that skips nothing (SURVEY s8(f) agreement rule)."""
+    sc = city
+    eps = 1e-2
+    tr = _trainer(sc)
+    ids = list(range(len(sc.cameras)))
+    targets = torch.from_numpy(np.stack(sc.targets)).cuda()
+    lr0 = dict(tr.lr)
+    tr.lr = {k: 0.0 for k in lr0}          # keep the parameters fixed so that both iterations see the same scene
+    n_launch = tr.iteration_views(ids, sc.cameras, targets, sat_eps=eps)
+    assert n_launch == len(tr.buckets(ids, sc.cameras))
+    # second visit: saturated slots are skipped
+    groups = tr.buckets(ids, sc.cameras)
+    skipped = 0
+    for grp in groups:
+        cams = [sc.cameras[i] for i in grp]
+        plan, state_out = tr.bucket_plan(grp, cams)
+        state = G.np32(plan.tile_state).reshape(sc.K, -1).copy()
+        imgs = tr.forward_plan(plan, eps, state_out).clone()
+        torch.cuda.synchronize()
+        full, _ = ov.iteration_plan(sc.partitions(), [c.as_array() for c in cams], plan.view_of_part, sc.sh_degree,
+                                    [sc.targets[i] for i in grp], sc.bg)
+        for j, res in enumerate(full):
+            members = res.members
+            ct = np.stack([p.ct for p in res.partials]); d = np.stack([p.d for p in res.partials])
+            front = ov.front_products(ct, res.order)
+            TX = (cams[j].width + 15) // 16
+            for jj, k in enumerate(members):
+                for t in np.nonzero(state[k] & ov.TILE_SATURATED)[0]:
+                    x0, y0 = (t % TX) * 16, (t // TX) * 16
+                    assert np.all(front[jj, y0:y0 + 16, x0:x0 + 16] < eps * (1 + 1e-3)), (k, t)
+                    skipped += 1
+            rgb_max = max(float(p.rgb.max()) for p in res.proj)
+            frag = _fragile(res)
+            img = G.np32(imgs[j]).astype(np.float64)
+            err = np.abs(img - res.image).max(-1)
+            assert (err[~frag] <= eps * rgb_max + 1e-5).all()
+    assert skipped > 0

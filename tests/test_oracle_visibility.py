@@ -1,0 +1,169 @@
+"""Pins of the oracle for the two optional subsystems (oracle/visibility.py) and of the product's HOST logic
+(splx_visible_regions, splx_schedule_views need no GPU): PAPER.md L212-L231 (visibility prediction),
+L247-L249 (conflict-free consolidation)."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import visibility as ov
+from paper_2606_18588_b200 import binding, scenes
+
+from .common import cam64, random_scene
+
+
+def _cam(width=96, height=80, pitch=40.0, yaw=30.0, alt=30.0, target=(1.3, -0.7, 0.0)):
+    return scenes.aerial_camera(width, height, 60.0, alt, pitch, yaw, target)
+
+
+BOXES_LO = np.array([[-20, -20, 0], [0, -20, 0], [-20, 0, 0], [0, 0, 0], [200, 200, 0], [-3, -3, 0]], np.float32)
+BOXES_HI = np.array([[0, 0, 8], [20, 0, 8], [0, 20, 8], [20, 20, 8], [220, 220, 8], [3, 3, 0]], np.float32)
+
+
+def test_region_lp_agrees_with_ray_brute_force():
+    """The LP statement against geometry done the slow way: every sampled image point whose ray meets the
+    box lies in a visible tile, and a robustly visible tile contains a point whose ray meets the box."""
+    cam = _cam()
+    c64 = cam.as_array()
+    state, part, margin = ov.visible_regions(BOXES_LO, BOXES_HI, c64)
+    W, H = cam.width, cam.height
+    TX = (W + 15) // 16
+    us = np.arange(0.125, W, 0.25); vs = np.arange(0.125, H, 0.25)
+    for k in range(len(BOXES_LO)):
+        hit_tiles = set()
+        for v in vs:
+            for u in us:
+                if ov.ray_hits_box(BOXES_LO[k].astype(np.float64), BOXES_HI[k].astype(np.float64), c64, u, v):
+                    hit_tiles.add(int(v // 16) * TX + int(u // 16))
+        vis_tiles = set(np.nonzero(state[k] == 0)[0].tolist())
+        assert hit_tiles <= vis_tiles, k
+        for t in vis_tiles - hit_tiles:          # only slivers thinner than the sampling pitch may be missed
+            assert margin[k, t] < 0.2, (k, t, margin[k, t])
+    assert part & 0b1111 == 0b1111 and not (part >> 4) & 1   # the four central boxes are seen, the far one is not
+
+
+def test_region_of_a_box_that_fills_the_view_or_lies_behind_the_camera():
+    cam = _cam()
+    c64 = cam.as_array()
+    state, part, _ = ov.visible_regions(np.array([[-500, -500, -5]], np.float32), np.array([[500, 500, 5]], np.float32), c64)
+    assert part == 1 and np.all(state == 0)                   # the ground slab covers every tile
+    o = -cam.R.T.astype(np.float64) @ cam.t.astype(np.float64)
+    fwd = cam.R[2].astype(np.float64)
+    behind = o - 50.0 * fwd
+    state, part, _ = ov.visible_regions((behind - 1).astype(np.float32)[None], (behind + 1).astype(np.float32)[None], c64)
+    assert part == 0 and np.all(state == ov.TILE_INVISIBLE)
+
+
+def test_library_host_geometry_equals_the_lp_oracle():
+    """splx_visible_regions (clip + hull + separating axes, host C++) against the LP, on every tile whose
+    LP margin is not within rounding of zero."""
+    for yaw, pitch in ((30.0, 40.0), (200.0, 25.0), (95.0, 70.0)):
+        cam = _cam(yaw=yaw, pitch=pitch)
+        ref, part_ref, margin = ov.visible_regions(BOXES_LO, BOXES_HI, cam.as_array())
+        got, part = binding.visible_regions(BOXES_LO, BOXES_HI, cam)
+        robust = np.abs(margin) > 1e-6
+        assert robust.mean() > 0.98
+        assert np.array_equal(got[robust], ref[robust])
+        assert part == part_ref
+
+
+def test_schedule_views_is_greedy_and_conflict_free():
+    rng = np.random.default_rng(3)
+    for trial in range(20):
+        n = int(rng.integers(1, 30))
+        parts = [int(rng.integers(1, 1 << 8)) & int(rng.integers(1, 1 << 8)) or 1 for _ in range(n)]
+        cap = int(rng.integers(1, 9))
+        ref, nb_ref = ov.schedule_views(parts, cap)
+        got, nb = binding.schedule_views(parts, cap)
+        assert got == ref and nb == nb_ref
+        for b in range(nb):
+            members = [parts[i] for i in range(n) if got[i] == b]
+            assert 1 <= len(members) <= cap
+            acc = 0
+            for m in members:
+                assert acc & m == 0
+                acc |= m
+    # Fig. 15 of the paper: V0 needs GPUs {0,2}, V2 needs {1,3}: one slot; a view on {0,1} conflicts with both
+    assert ov.schedule_views([0b0101, 0b0011, 0b1010])[0] == [0, 1, 0]
+
+
+def _two_layer_partials(H=32, W=32):
+    """K = 3 hand-made partials: partition 0 in front (D/(1-T) = 1), 1 behind it (2), 2 empty."""
+    ct = np.zeros((3, H, W, 4)); d = np.zeros((3, H, W))
+    ct[..., 3] = 1.0
+    ct[0, ..., :3] = 0.3; ct[0, ..., 3] = 5e-5; d[0] = 1.0 * (1 - 5e-5)
+    ct[1, ..., :3] = 0.2; ct[1, ..., 3] = 0.5; d[1] = 2.0 * 0.5
+    return ct, d
+
+
+def test_saturation_closed_forms():
+    ct, d = _two_layer_partials()
+    ct[0, 0:16, 0:16, 3] = 0.5; d[0, 0:16, 0:16] = 0.5          # tile 0: front partition is half transparent
+    ct[0, 20, 20, 3] = 0.9; d[0, 20, 20] = 0.1                   # tile 3: one unsaturated pixel
+    state, margin = ov.saturation(ct, d, 1e-4)
+    # partition 0 is in front everywhere: never saturated.  1 is behind T = 5e-5 < eps except tile 0 and the
+    # pixel in tile 3.  2 (empty) stands behind both: 5e-5 * 0.5 < eps except tile 0 (0.25) and that pixel.
+    assert state[0].tolist() == [0, 0, 0, 0]
+    assert state[1].tolist() == [0, 2, 2, 0]
+    assert state[2].tolist() == [0, 2, 2, 0]
+    # geometric bit is preserved, saturated bit recomputed
+    s_in = np.array([[1, 0, 0, 0], [0, 0, 2, 2], [1, 1, 0, 0]], np.uint8)
+    state2, _ = ov.saturation(ct, d, 1e-4, s_in)
+    assert state2.tolist() == [[1, 0, 0, 0], [0, 2, 2, 0], [1, 3, 2, 0]]
+    # a larger threshold saturates more (Table 4 sweeps eps): with eps = 0.3, 0.25 < eps on tile 0 for partition 2
+    state3, _ = ov.saturation(ct, d, 0.3)
+    assert state3[2].tolist() == [2, 2, 2, 0] and state3[1, 0] == 0
+
+
+def test_skipping_saturated_tiles_changes_the_image_by_at_most_eps():
+    """every skipped slot has front product < eps, so dropping it moves a pixel by <= eps * max rgb."""
+    sc = scenes.small_city(n=6000, width=96, height=80, n_views=1)
+    cam = sc.cameras[0].as_array()
+    parts = sc.partitions()
+    eps = 1e-2
+    views, _ = ov.iteration_plan(parts, [cam], [0] * sc.K, sc.sh_degree, sc.targets)
+    res = views[0]
+    ct = np.stack([p.ct for p in res.partials]); d = np.stack([p.d for p in res.partials])
+    state, _ = ov.saturation(ct, d, eps)
+    front = ov.front_products(ct, res.order)
+    TX = (sc.cameras[0].width + 15) // 16
+    n_skipped = 0
+    for k in range(sc.K):
+        for t in np.nonzero(state[k])[0]:
+            x0, y0 = (t % TX) * 16, (t // TX) * 16
+            assert np.all(front[k, y0:y0 + 16, x0:x0 + 16] < eps)
+            n_skipped += int(res.bins[k].ranges.reshape(-1, 2)[t, 1] > res.bins[k].ranges.reshape(-1, 2)[t, 0])
+    views2, _ = ov.iteration_plan(parts, [cam], [0] * sc.K, sc.sh_degree, sc.targets, tile_state=state)
+    rgb_max = max(float(p.rgb.max()) for p in res.proj)
+    assert np.abs(views2[0].image - res.image).max() <= eps * rgb_max * (1 + 1e-9)
+    assert n_skipped > 0, "the test scene must saturate somewhere"
+
+
+def test_plan_with_one_view_is_the_plain_iteration():
+    rng = np.random.default_rng(5)
+    p, cam = random_scene(rng, 60, size=48, f=60.0)
+    parts = [{k: v[:30] for k, v in p.items()}, {k: v[30:] for k, v in p.items()}]
+    target = rng.uniform(0, 1, (48, 48, 3))
+    ref = oracle.iteration(parts, cam64(cam), 3, target)
+    views, grads = ov.iteration_plan(parts, [cam64(cam)], [0, 0], 3, [target])
+    assert np.array_equal(views[0].image, ref.image)
+    for k in range(2):
+        for key in oracle.PARAM_KEYS:
+            assert np.array_equal(grads[k][key], ref.grads[k][key])
+
+
+def test_consolidated_views_equal_the_views_one_by_one():
+    """L249: views of a conflict-free bucket touch disjoint partitions, so one consolidated pass = the two
+    single-view passes over their own partitions; a non-participant gets no gradient."""
+    rng = np.random.default_rng(6)
+    p, cam_a = random_scene(rng, 90, size=48, f=60.0)
+    cam_b = scenes.Camera(cam_a.R, cam_a.t + np.array([0.3, -0.2, 0.5]), 55.0, 55.0, 24.0, 24.0, 48, 48)
+    parts = [{k: v[i:i + 30] for k, v in p.items()} for i in (0, 30, 60)]
+    ta, tb = rng.uniform(0, 1, (48, 48, 3)), rng.uniform(0, 1, (48, 48, 3))
+    views, grads = ov.iteration_plan(parts, [cam64(cam_a), cam64(cam_b)], [1, -1, 0], 3, [ta, tb])
+    ra = oracle.iteration([parts[2]], cam64(cam_a), 3, ta)
+    rb = oracle.iteration([parts[0]], cam64(cam_b), 3, tb)
+    assert np.array_equal(views[0].image, ra.image) and np.array_equal(views[1].image, rb.image)
+    for key in oracle.PARAM_KEYS:
+        assert np.array_equal(grads[2][key], ra.grads[0][key])
+        assert np.array_equal(grads[0][key], rb.grads[0][key])
+        assert not grads[1][key].any()
