@@ -49,6 +49,12 @@ def workload(name):
         return scenes.tiny()                         # configs[0]
     if name == "aerial_small":
         return scenes.small_aerial()
+    if name == "city_10M":
+        return scenes.city()                         # configs[2]: 10M Gaussians, K=8, B=4 views
+    if name == "city_small":
+        return scenes.small_city()
+    if name == "blocks_small":
+        return scenes.small_blocks()
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -217,7 +223,33 @@ def run_ours(args):
     STAGES = ["project", "bin_sort", "render_partial", "compose", "l1_loss_grad", "compose_backward",
               "raster_backward", "project_backward", "adam"]
 
-    def step(ev=None):
+    # The step runs under a one-view launch plan (include/splx.h, splx_plan): sparse partial pixels and the
+    # geometric visibility state from the partitions' 3-sigma boxes -- both leave every result unchanged
+    # (tests/test_gpu_plan.py); --dense times the plain single-view calls instead.
+    from paper_2606_18588_b200 import scenes as _scn
+    tr.set_aabbs(*_scn.partition_aabbs(sc.params, sc.part_offsets))
+    plan, state = tr.bucket_plan([0], [cam], saturation=args.saturation, sparse=True)
+    images, T_totals, g_images = tr._view_buffers(1)
+    target1 = target[None]
+
+    def step_plan(ev=None):
+        def rec(i):
+            if ev is not None:
+                ev[i].record()
+        po = tr.part_offsets
+        rec(0); c.project_plan(tr.params, po, plan, tr.sh_degree, tr.proj)
+        rec(1); c.bin_sort_plan(tr.proj, po, plan, tr.bins, tr._ws_sort)
+        rec(2); c.render_partial_plan(tr.proj, tr.bins, plan, tr.partials)
+        rec(3); c.compose_plan(tr.partials, tr.bins, plan, tr.bg, images, T_totals, args.sat_eps, state)
+        rec(4); c.l1_loss_grad(images, target1, g_images, tr.loss_sum)
+        rec(5); c.compose_backward_plan(tr.partials, tr.bins, plan, tr.bg, g_images, None, g_ct)
+        rec(6); c.raster_backward_plan(tr.proj, tr.bins, plan, tr.partials, g_ct, g2d)
+        rec(7); c.project_backward_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True,
+                                        overwrite=True)
+        rec(8); tr.adam_step(1)
+        rec(9)
+
+    def step_dense(ev=None):
         def rec(i):
             if ev is not None:
                 ev[i].record()
@@ -231,6 +263,9 @@ def run_ours(args):
         rec(7); c.project_backward(tr.params, cam, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True, overwrite=True)
         rec(8); tr.adam_step(1)
         rec(9)
+
+    step = step_dense if args.dense else step_plan
+    result_image = tr.image if args.dense else images[0]
 
     def barrier():
         replicas.barrier(cuda=True)
@@ -248,6 +283,8 @@ def run_ours(args):
     n_contrib = tr.partials.n_contrib
     pairs_bwd = int(n_contrib.to(torch.int64).sum().item())       # list entries the backward re-evaluates
     n_visible = int((tr.proj.radius > 0).sum().item())
+    rng_ = tr.bins.tile_ranges
+    live_slots = int((rng_[:, 1] > rng_[:, 0]).sum().item())     # (partition, tile) slots with a non-empty list
 
     sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(max(args.warmup, 3)):
@@ -280,7 +317,7 @@ def run_ours(args):
         target.copy_(tgt_host, non_blocking=True)
         tr.loss_sum.zero_()
         step()
-        img_host.copy_(tr.image, non_blocking=True)
+        img_host.copy_(result_image, non_blocking=True)
         loss_host.copy_(tr.loss_sum, non_blocking=True)
         torch.cuda.current_stream().synchronize()
 
@@ -305,7 +342,8 @@ def run_ours(args):
     flops_bwd = pairs_bwd * FLOPS_EVAL + pairs_blend * FLOPS_BLEND_BWD
     flops_fwd = pairs_fwd * FLOPS_EVAL + pairs_blend * FLOPS_BLEND_FWD
     hbm_bytes = dict(project=n_visible * 285 + (tr.n - n_visible) * 93, adam=28 * 59 * tr.n,
-                     compose=(20 * K + 16) * W * H, compose_backward=(12 + 36 * K) * W * H,
+                     compose=(20 * K + 16) * W * H if args.dense else 20 * 256 * live_slots + 16 * W * H,
+                     compose_backward=(12 + 36 * K) * W * H if args.dense else 36 * 256 * live_slots + 12 * W * H,
                      project_backward=n_visible * 740, l1_loss_grad=36 * W * H)
     if dom == "raster_backward":
         ach = flops_bwd / (stage_ms[dom] * 1e-3) / 1e12
@@ -346,6 +384,10 @@ def run_ours(args):
                 data="synthetic",
                 config=dict(workload=args.workload, gaussians=tr.n, K=K, width=W, height=H, sh_degree=sc.sh_degree,
                             views_per_step=1, parallelism=f"replicas x{world} (one GPU per replica, no collective)",
+                            path="dense single-view calls" if args.dense else
+                                 "one-view launch plan: sparse partials + geometric tile state (results unchanged)",
+                            saturation_skipping=bool(args.saturation and not args.dense), live_slots=live_slots,
+                            slots=K * ((W + 15) // 16) * ((H + 15) // 16),
                             l2="working set (params+grads+moments 944 MB at 1M) is larger than the 126 MB L2",
                             intersections=M, visible=n_visible, pairs_fwd=pairs_fwd, pairs_bwd=pairs_bwd,
                             pairs_blended=pairs_blend, pairs_evaluated_fwd=pairs_eval, half_tile_items_fwd=items_fwd),
@@ -358,6 +400,70 @@ def run_ours(args):
     replicas.finish()
 
 
+# ------------------------------------------------------- optional subsystems: B views per step --
+def run_views(args):
+    """`--views B`: one step = one training iteration over B views of the workload (configs[2]-[4] style) through
+    Trainer.iteration_views: geometric participants, conflict-free buckets (one launch per stage per bucket),
+    saturated-tile skipping.  --no-visibility renders every partition for every view, --no-consolidate runs one
+    view per launch, --saturation/--sat-eps as above.  A secondary line: same JSON keys, config.views_per_step = B."""
+    import torch
+    from paper_2606_18588_b200 import binding, scenes
+    from paper_2606_18588_b200.engine import Trainer
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    sc = workload(args.workload)
+    B = min(args.views, len(sc.cameras))
+    cams = sc.cameras[:B]
+    W, H = cams[0].width, cams[0].height
+    cap = {"city_10M": 64_000_000}.get(args.workload)
+    tr = Trainer(sc.params, sc.part_offsets, W, H, sc.sh_degree, sc.bg, capacity=cap)
+    if args.no_visibility:   # boxes that contain everything: every partition participates in every view, no tile is invisible
+        big = np.float32(1e6)
+        tr.set_aabbs(np.full((tr.K, 3), -big), np.full((tr.K, 3), big))
+    else:
+        tr.set_aabbs(*scenes.partition_aabbs(sc.params, sc.part_offsets))
+    targets = torch.from_numpy(np.stack(sc.targets[:B])).cuda()
+    ids = list(range(B))
+    kw = dict(consolidate=not args.no_consolidate, saturation=args.saturation, sat_eps=args.sat_eps)
+    parts = [tr.participants(v, c) for v, c in zip(ids, cams)]
+    groups = tr.buckets(ids, cams, consolidate=not args.no_consolidate)
+    sampler = ClockSampler(0)
+    for _ in range(max(args.warmup, 3)):
+        tr.iteration_views(ids, cams, targets, **kw)
+    torch.cuda.synchronize()
+    M = tr.num_intersections()
+    l0 = tr.ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.mark()
+    e0.record()
+    for _ in range(args.steps):
+        tr.iteration_views(ids, cams, targets, **kw)
+    e1.record()
+    torch.cuda.synchronize()
+    sampler.mark()
+    ms = e0.elapsed_time(e1) / args.steps
+    launches = tr.ctx.launch_count() - l0
+    clocks = sampler.stop()
+    skipped = {}
+    for key, st in tr._bucket_state.items():
+        st = st.cpu().numpy()
+        skipped[str(list(key))] = dict(invisible=int((st & binding.TILE_INVISIBLE != 0).sum()),
+                                       saturated=int((st & binding.TILE_SATURATED != 0).sum()), slots=int(st.size))
+    line = dict(metric=METRIC, value=B * W * H / (ms * 1e-3) / 1e6, unit=UNIT, n_gpus=1, steps=args.steps,
+                warmup=max(args.warmup, 3), ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f32", data="synthetic",
+                config=dict(workload=args.workload, gaussians=tr.n, K=tr.K, width=W, height=H, sh_degree=sc.sh_degree,
+                            views_per_step=B, visibility_prediction=not args.no_visibility,
+                            consolidation=not args.no_consolidate, saturation_skipping=bool(args.saturation),
+                            sat_eps=args.sat_eps, participants=[bin(p) for p in parts], buckets=groups,
+                            tile_state=skipped, intersections_last_bucket=M,
+                            l2="working set (params+grads+moments) is larger than the 126 MB L2"),
+                iters_per_s=1e3 / ms, clocks=clocks, gpu_launches=int(launches))
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -366,6 +472,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="aerial_1M")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense", action="store_true", help="time the plain single-view calls (dense partial buffers)")
+    ap.add_argument("--saturation", action="store_true", help="skip tiles detected as saturated (PAPER.md L231)")
+    ap.add_argument("--sat-eps", type=float, default=1e-4)
+    ap.add_argument("--views", type=int, default=0, help="B > 0: time iterations over B views (optional subsystems)")
+    ap.add_argument("--no-visibility", action="store_true")
+    ap.add_argument("--no-consolidate", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 2 if args.steps is None else min(args.steps, 4)
@@ -374,7 +486,11 @@ def main():
     else:
         args.steps = 50 if args.steps is None else args.steps
         args.warmup = 5 if args.warmup is None else args.warmup
-        run_ours(args)
+        if args.views > 0:
+            args.steps = min(args.steps, 20)
+            run_views(args)
+        else:
+            run_ours(args)
 
 
 if __name__ == "__main__":

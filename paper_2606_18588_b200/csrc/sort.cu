@@ -20,6 +20,7 @@ namespace {
 constexpr int SCAN_THREADS = 512, SCAN_IPT = 4, SCAN_TILE = SCAN_THREADS * SCAN_IPT;
 constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
+constexpr uint32_t PERSISTENT_CTAS = SPLX_SM_COUNT * 8;   // grid of the persistent kernels: 8 CTAs per SM
 
 struct Counters {   // device-resident counts, written by kernels, read by later kernels
   uint64_t n_visible;
@@ -100,6 +101,8 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
   return res;
 }
 
+// Persistent: a CTA keeps taking tiles from the ticket counter until the (device-side) element count is
+// exhausted, so the grid is sized for the machine, not for the caller's capacity.
 template <class Op>
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
@@ -107,43 +110,45 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
   __shared__ uint32_t sm[33];
   __shared__ uint32_t s_tile;
   __shared__ uint64_t s_excl;
-  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
-  __syncthreads();
-  const uint32_t t = s_tile;
   const uint64_t n = op.count(n_ptr);
   const uint64_t ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
-  if (t >= ntiles) {
-    if (n == 0 && t == 0 && threadIdx.x == 0) {
+  if (n == 0) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
       if (total_out) *total_out = 0;
       if (clamp_out) *clamp_out = 0;
     }
     return;
   }
-  const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
-  uint32_t v[SCAN_IPT], s = 0;
+  for (;;) {
+    __syncthreads();                       // s_tile / s_excl of the previous round are no longer read
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const uint32_t t = s_tile;
+    if (t >= ntiles) return;
+    const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
+    uint32_t v[SCAN_IPT], s = 0;
 #pragma unroll
-  for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(base + k) : 0; s += v[k]; }
-  uint32_t total;
-  uint32_t ex = block_exclusive_scan(s, sm, total);
-  if (threadIdx.x == 0) {
-    uint64_t excl = 0;
-    if (t == 0) st_status(status, ST_PREFIX | (uint64_t)total);
-    else excl = lookback<16>(status, t, 1, total);
-    s_excl = excl;
-    if (t + 1 == ntiles) {
-      const uint64_t grand = excl + total;
-      if (total_out) *total_out = grand;
-      if (clamp_out) *clamp_out = grand < clamp_to ? grand : clamp_to;
+    for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(base + k) : 0; s += v[k]; }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(s, sm, total);
+    if (threadIdx.x == 0) {
+      uint64_t excl = 0;
+      if (t == 0) st_status(status, ST_PREFIX | (uint64_t)total);
+      else excl = lookback<16>(status, t, 1, total);
+      s_excl = excl;
+      if (t + 1 == ntiles) {
+        const uint64_t grand = excl + total;
+        if (total_out) *total_out = grand;
+        if (clamp_out) *clamp_out = grand < clamp_to ? grand : clamp_to;
+      }
     }
-  }
-  __syncthreads();
-  ex += (uint32_t)s_excl;
+    __syncthreads();
+    ex += (uint32_t)s_excl;
 #pragma unroll
-  for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex); ex += v[k]; }
+    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex); ex += v[k]; }
+  }
 }
 
-// Element j of the launch -> Gaussian index, through the runs of the participating partitions
-// (non-participants are never read: their tiles_touched may be stale).
 struct RunMap {
   int n;
   int64_t begin[SPLX_MAX_K], jprefix[SPLX_MAX_K + 1];
@@ -175,8 +180,9 @@ struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, d
 template <class Op>
 int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket,
                    uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to) {
-  const uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
+  uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
   if (nb == 0) return SPLX_OK;
+  if (nb > PERSISTENT_CTAS) nb = PERSISTENT_CTAS;
   k_scan<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to);
   SPLX_LAUNCH_CHECK(ctx, "k_scan");
   return SPLX_OK;
@@ -218,30 +224,37 @@ __device__ __forceinline__ unsigned digit_peers(uint32_t d, unsigned vm) {
   return peers;
 }
 
+// Grid-stride over the tiles (sized for the machine, not for the capacity).  The CTA that counts tile t also
+// clears the look-back status words of tile t for every pass, so the status arrays -- sized by the caller's
+// capacity -- never need a memset: only the part the actual count reaches is ever touched.
 template <typename KeyT>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t* __restrict__ ghist /*[npass][256]*/,
-                 PassPlan plan) {
+                 uint64_t* __restrict__ status, size_t status_stride, PassPlan plan) {
   __shared__ uint32_t hist[RS_WARPS][MAX_PASSES][256];   // warp-private: plain read-modify-write by group leaders
   const uint64_t n = *n_ptr;
-  const uint64_t start = (uint64_t)blockIdx.x * RS_TILE;
-  if (start >= n) return;
+  const uint64_t ntiles = (n + RS_TILE - 1) / RS_TILE;
+  if (blockIdx.x >= ntiles) return;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int p = 0; p < plan.npass; ++p)
 #pragma unroll
     for (int w = 0; w < RS_WARPS; ++w) hist[w][p][threadIdx.x] = 0;
   __syncthreads();
+  for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    for (int p = 0; p < plan.npass; ++p) status[(size_t)p * status_stride + t * 256 + threadIdx.x] = 0;
+    const uint64_t start = t * RS_TILE;
 #pragma unroll 2
-  for (int it = 0; it < RS_IPT; ++it) {
-    const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
-    const bool valid = idx < n;
-    const unsigned vm = __ballot_sync(0xffffffffu, valid);
-    const KeyT key = valid ? keys[idx] : (KeyT)0;
-    for (int p = 0; p < plan.npass; ++p) {
-      const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
-      const unsigned peers = digit_peers(d, vm);
-      if (valid && lane == __ffs(peers) - 1) hist[warp][p][d] += __popc(peers);
-      __syncwarp();
+    for (int it = 0; it < RS_IPT; ++it) {
+      const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
+      const bool valid = idx < n;
+      const unsigned vm = __ballot_sync(0xffffffffu, valid);
+      const KeyT key = valid ? keys[idx] : (KeyT)0;
+      for (int p = 0; p < plan.npass; ++p) {
+        const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
+        const unsigned peers = digit_peers(d, vm);
+        if (valid && lane == __ffs(peers) - 1) hist[warp][p][d] += __popc(peers);
+        __syncwarp();
+      }
     }
   }
   __syncthreads();
@@ -253,6 +266,8 @@ k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t*
   }
 }
 
+// Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
+// started and the look-back spin cannot wait on a CTA that was never scheduled.
 template <typename KeyT>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
@@ -260,67 +275,76 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
              uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits) {
   __shared__ uint32_t whist[RS_WARPS][256];
   __shared__ uint32_t dbase[256];
+  __shared__ uint32_t gbase[256];
   __shared__ uint32_t sm[33];
   __shared__ uint32_t s_tile;
-  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
-#pragma unroll
-  for (int w = 0; w < RS_WARPS; ++w) whist[w][threadIdx.x] = 0;
-  __syncthreads();
-  const uint32_t t = s_tile;
   const uint64_t n = *n_ptr;
-  const uint64_t start = (uint64_t)t * RS_TILE;
-  if (start >= n) return;
+  const uint64_t ntiles = (n + RS_TILE - 1) / RS_TILE;
+  if (blockIdx.x >= ntiles) return;
   const uint32_t mask = (1u << bits) - 1u;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  // warp w owns the contiguous segment [start + w*512, +512); iteration `it` covers 32 consecutive
-  // positions, so (it, lane) is the input order and the ranks below are stable.
-  const uint64_t seg = start + (uint64_t)warp * (32 * RS_IPT);
-  KeyT key[RS_IPT];
-  uint32_t rank[RS_IPT];
   const unsigned lt = (1u << lane) - 1u;
-#pragma unroll
-  for (int it = 0; it < RS_IPT; ++it) {
-    const uint64_t idx = seg + (uint64_t)it * 32 + lane;
-    key[it] = idx < n ? kin[idx] : (KeyT)0;
-  }
-#pragma unroll
-  for (int it = 0; it < RS_IPT; ++it) {
-    const uint64_t idx = seg + (uint64_t)it * 32 + lane;
-    const bool valid = idx < n;
-    const unsigned vm = __ballot_sync(0xffffffffu, valid);
-    const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
-    const unsigned peers = digit_peers(d, vm);
-    const int leader = valid ? __ffs(peers) - 1 : lane;
-    uint32_t old = 0;
-    if (valid && lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
-    old = __shfl_sync(0xffffffffu, old, leader);
-    rank[it] = old + __popc(peers & lt);
-    __syncwarp();
-  }
-  __syncthreads();
-  {  // per digit: exclusive prefix over the warps, tile total, chained prefix over the tiles
-    const int d = threadIdx.x;
-    uint32_t run = 0;
-#pragma unroll
-    for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
-    // exclusive scan of the global digit histogram = first output position of digit d
+  {  // exclusive scan of the global digit histogram = first output position of each digit (once per CTA)
     uint32_t tot;
-    const uint32_t gexcl = block_exclusive_scan(ghist[d], sm, tot);
-    uint64_t excl = 0;
-    uint64_t* st = status + d;
-    if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
-    else excl = lookback<8>(st, t, 256, run);
-    dbase[d] = gexcl + (uint32_t)excl;
+    gbase[threadIdx.x] = block_exclusive_scan(ghist[threadIdx.x], sm, tot);
   }
-  __syncthreads();
+  for (;;) {
+    __syncthreads();                       // the previous round no longer reads whist / dbase / s_tile
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
 #pragma unroll
-  for (int it = 0; it < RS_IPT; ++it) {
-    const uint64_t idx = seg + (uint64_t)it * 32 + lane;
-    if (idx < n) {
+    for (int w = 0; w < RS_WARPS; ++w) whist[w][threadIdx.x] = 0;
+    __syncthreads();
+    const uint32_t t = s_tile;
+    if (t >= ntiles) return;
+    const uint64_t start = (uint64_t)t * RS_TILE;
+    // warp w owns the contiguous segment [start + w*256, +256); iteration `it` covers 32 consecutive
+    // positions, so (it, lane) is the input order and the ranks below are stable.
+    const uint64_t seg = start + (uint64_t)warp * (32 * RS_IPT);
+    KeyT key[RS_IPT];
+    uint32_t val[RS_IPT];
+    uint32_t rank[RS_IPT];
+#pragma unroll
+    for (int it = 0; it < RS_IPT; ++it) {
+      const uint64_t idx = seg + (uint64_t)it * 32 + lane;
+      key[it] = idx < n ? kin[idx] : (KeyT)0;
+      val[it] = idx < n ? vin[idx] : 0u;
+    }
+#pragma unroll
+    for (int it = 0; it < RS_IPT; ++it) {
+      const uint64_t idx = seg + (uint64_t)it * 32 + lane;
+      const bool valid = idx < n;
+      const unsigned vm = __ballot_sync(0xffffffffu, valid);
       const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
-      const uint32_t pos = dbase[d] + whist[warp][d] + rank[it];
-      kout[pos] = key[it];
-      vout[pos] = vin[idx];
+      const unsigned peers = digit_peers(d, vm);
+      const int leader = valid ? __ffs(peers) - 1 : lane;
+      uint32_t old = 0;
+      if (valid && lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
+      old = __shfl_sync(0xffffffffu, old, leader);
+      rank[it] = old + __popc(peers & lt);
+      __syncwarp();
+    }
+    __syncthreads();
+    {  // per digit: exclusive prefix over the warps, tile total, chained prefix over the tiles
+      const int d = threadIdx.x;
+      uint32_t run = 0;
+#pragma unroll
+      for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
+      uint64_t excl = 0;
+      uint64_t* st = status + d;
+      if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
+      else excl = lookback<8>(st, t, 256, run);
+      dbase[d] = gbase[d] + (uint32_t)excl;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < RS_IPT; ++it) {
+      const uint64_t idx = seg + (uint64_t)it * 32 + lane;
+      if (idx < n) {
+        const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
+        const uint32_t pos = dbase[d] + whist[warp][d] + rank[it];
+        kout[pos] = key[it];
+        vout[pos] = val[it];
+      }
     }
   }
 }
@@ -331,14 +355,16 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
 template <typename KeyT>
 int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
                const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets) {
-  const uint32_t nblocks = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
-  if (nblocks == 0) return SPLX_OK;
+  const uint32_t ntiles_cap = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
+  if (ntiles_cap == 0) return SPLX_OK;
+  const uint32_t nblocks = ntiles_cap < PERSISTENT_CTAS ? ntiles_cap : PERSISTENT_CTAS;
+  const size_t stride = (size_t)ntiles_cap * 256;     // status words per pass
   const PassPlan plan = plan_passes(begin_bit, end_bit);
-  k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, plan);
+  k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, status, stride, plan);
   SPLX_LAUNCH_CHECK(ctx, "k_radix_hist_all");
   for (int p = 0; p < plan.npass; ++p) {
     k_radix_pass<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
-                                                               status + (size_t)p * nblocks * 256, tickets + p,
+                                                               status + (size_t)p * stride, tickets + p,
                                                                plan.shift[p], plan.bits[p]);
     SPLX_LAUNCH_CHECK(ctx, "k_radix_pass");
     KeyT* tk = ka; ka = kb; kb = tk;
@@ -354,8 +380,10 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
             uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
   const uint64_t nvis = cnt->n_visible;
-  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31;
+  // grid-stride over blocks of 256 visible Gaussians (the grid is sized for the machine; nvis lives on the device)
+  for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < nvis; base += (uint64_t)gridDim.x * blockDim.x) {
+  const uint64_t j = base + threadIdx.x;
   int x0 = 0, y0 = 0, w = 0, tt = 0;
   uint32_t i = 0, o = 0, dbits = 0, slot0 = 0;
   if (j < nvis) {
@@ -400,24 +428,26 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       }
     }
   }
+  }
 }
 
 __global__ void __launch_bounds__(256)
 k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint8_t* __restrict__ tile_state,
               uint32_t* __restrict__ ranges) {
   const uint64_t m = cnt->m_sorted;
-  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= m) return;
-  const uint32_t s = (uint32_t)(keys[j] >> 32);
-  if (tile_state && tile_state[s]) return;   // a skipped (partition, tile) slot keeps the empty range (0,0)
-  if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
-  if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
+  for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j < m; j += (uint64_t)gridDim.x * blockDim.x) {
+    const uint32_t s = (uint32_t)(keys[j] >> 32);
+    if (tile_state && tile_state[s]) continue;   // a skipped (partition, tile) slot keeps the empty range (0,0)
+    if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
+    if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
+  }
 }
 
 __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_total; }
 
-// Workspace: a zero-initialised control region (counters, tickets, digit histograms, look-back
-// status words: one memset per call) followed by the sort buffers.
+// Workspace: a small zero-initialised control region (counters, tickets, digit histograms, the scans' status
+// words: one memset per call), the radix passes' status words (cleared on the device, only as far as the
+// actual counts reach) and the sort buffers.
 struct Layout {
   size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes;
   size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, keys_tmp, vals_tmp, total;
@@ -441,9 +471,9 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   L.ghist_s = take(MAX_PASSES * 256 * 4);
   L.st_scan_v = take(scan_n * 8);
   L.st_scan_t = take(scan_n * 8);
-  L.st_depth = take(4 * tiles_n * 256 * 8);
-  L.st_slot = take((size_t)((sbits + 7) / 8) * tiles_m * 256 * 8);
   L.zero_bytes = off;
+  L.st_depth = take(4 * tiles_n * 256 * 8);                                   // cleared tile by tile by k_radix_hist_all
+  L.st_slot = take((size_t)((sbits + 7) / 8) * tiles_m * 256 * 8);
   L.ckeys_a = take((size_t)n * 4); L.cvals_a = take((size_t)n * 4);
   L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
   L.offs = take((size_t)n * 4);
@@ -507,15 +537,16 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   PartOffs parts;
   parts.K = K;
   for (int k = 0; k <= K; ++k) parts.off[k] = part_offsets[k];
-  k_emit_keys<<<(unsigned)((n_act + 255) / 256), 256, 0, ctx->stream>>>(
+  const uint64_t emit_blocks = ((uint64_t)n_act + 255) / 256, range_blocks = (out->capacity + 255) / 256;
+  k_emit_keys<<<(unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
       pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
   // 4. stable sort on the slot bits
   if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
                                  (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6]))) return rc;
   // 5. ranges
-  k_tile_ranges<<<(unsigned)((out->capacity + 255) / 256), 256, 0, ctx->stream>>>(out->keys, cnt, plan.tile_state,
-                                                                                         out->tile_ranges);
+  k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
+      out->keys, cnt, plan.tile_state, out->tile_ranges);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
   k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
   SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
