@@ -42,16 +42,26 @@ __device__ __forceinline__ float det2_accurate(float a, float c, float b) {
   return f + e;
 }
 
-__device__ __forceinline__ bool geometry(const splx_gaussians& g, int64_t i, const CamDev& cam,
-                                         float dilation, Geo& G) {
-  const float mx = g.mean[3 * i], my = g.mean[3 * i + 1], mz = g.mean[3 * i + 2];
+// Raw per-Gaussian inputs of the geometry chain, loaded up front so that the loads are independent.
+struct GeoIn { float m[3], ls[3]; float4 q; };
+
+__device__ __forceinline__ GeoIn load_geo(const splx_gaussians& g, int64_t i) {
+  GeoIn in;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { in.m[k] = g.mean[3 * i + k]; in.ls[k] = g.log_scale[3 * i + k]; }
+  in.q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
+  return in;
+}
+
+__device__ __forceinline__ bool geometry(const GeoIn& in, const CamDev& cam, float dilation, Geo& G) {
+  const float mx = in.m[0], my = in.m[1], mz = in.m[2];
 #pragma unroll
   for (int r = 0; r < 3; ++r)
     G.p[r] = cam.R[3 * r] * mx + cam.R[3 * r + 1] * my + cam.R[3 * r + 2] * mz + cam.t[r];
   if (!(G.p[2] > cam.near_z)) return false;
 #pragma unroll
-  for (int k = 0; k < 3; ++k) G.s[k] = expf(g.log_scale[3 * i + k]);
-  const float4 q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
+  for (int k = 0; k < 3; ++k) G.s[k] = expf(in.ls[k]);
+  const float4 q = in.q;
   G.qn = sqrtf(q.x * q.x + q.y * q.y + q.z * q.z + q.w * q.w);
   const float inv = 1.0f / G.qn;
   const float w = q.x * inv, x = q.y * inv, y = q.z * inv, z = q.w * inv;
@@ -126,7 +136,8 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   if (i >= rt.end[r]) return;
   const CamDev& cam = plan.cam[rt.view[r]];   // the view this partition renders (indexed constant-bank loads)
   Geo G;
-  bool vis = geometry(g, i, cam, cfg.dilation, G);
+  const GeoIn gin = load_geo(g, i);
+  bool vis = geometry(gin, cam, cfg.dilation, G);
   float u = 0.f, v = 0.f;
   int rad = 0, tt = 0;
   if (vis) {
@@ -165,7 +176,7 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
 
   // colour: SH along the direction from the camera centre to the mean (s13)
-  float dx = g.mean[3 * i] - cam.o[0], dy = g.mean[3 * i + 1] - cam.o[1], dz = g.mean[3 * i + 2] - cam.o[2];
+  float dx = gin.m[0] - cam.o[0], dy = gin.m[1] - cam.o[1], dz = gin.m[2] - cam.o[2];
   const float dinv = rsqrtf(dx * dx + dy * dy + dz * dz);
   dx *= dinv; dy *= dinv; dz *= dinv;
   constexpr int NSH = (DEG + 1) * (DEG + 1);
@@ -254,7 +265,23 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   const CamDev& cam = plan.cam[view < 0 ? 0 : view];
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;        // float4 chunks of a row that hold used coefficients
-  const bool vis = (i < run_end) && (view >= 0) && (pr.radius[i] > 0);
+  // every per-Gaussian input is requested up front (independent loads in flight together; a culled row costs
+  // ~100 B more, but the kernel was stalled on these dependent loads: profiles/r01k)
+  const bool inr = (i < run_end) && (view >= 0);
+  int rad = 0;
+  GeoIn gin;
+  float4 g0 = make_float4(0.f, 0.f, 0.f, 0.f), g1 = g0, g2 = g0;
+  float op = 0.f;
+  uint8_t cl = 0;
+  float4* gp = reinterpret_cast<float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
+  if (inr) {
+    rad = pr.radius[i];
+    gin = load_geo(g, i);
+    g0 = gp[0]; g1 = gp[1]; g2 = gp[2];
+    op = pr.conic_opacity[4 * i + 3];
+    cl = pr.clamp[i];
+  }
+  const bool vis = inr && rad > 0;
   s_vis[threadIdx.x] = vis ? 1 : 0;
   __syncthreads();
 #pragma unroll
@@ -271,18 +298,14 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   float dlogit = 0.f;
   float grgb[3] = {0.f, 0.f, 0.f};
   Geo G;
-  if (vis && geometry(g, i, cam, cfg.dilation, G)) {
-    float4* gp = reinterpret_cast<float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
-    const float4 g0 = gp[0], g1 = gp[1], g2 = gp[2];
+  if (vis && geometry(gin, cam, cfg.dilation, G)) {
     if (clear_g2d) { const float4 zz = make_float4(0.f, 0.f, 0.f, 0.f); gp[0] = zz; gp[1] = zz; gp[2] = zz; }
     const float gu = g0.x, gv = g0.y, gA = g0.z, gB = g0.w, gC = g1.x, gop = g1.y;
     grgb[0] = g1.z; grgb[1] = g1.w; grgb[2] = g2.x;
-    const uint8_t cl = pr.clamp[i];
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) if ((cl >> ch) & 1) grgb[ch] = 0.f;
 
     // opacity: o = sigmoid(logit)
-    const float op = pr.conic_opacity[4 * i + 3];
     dlogit = op * (1.f - op) * gop;
 
     // conic Q = P^-1 (P = Sigma2D):  dL/dP = -Q Gm Q,  Gm = [[gA, gB/2],[gB/2, gC]]
@@ -355,7 +378,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   __syncthreads();
   if (vis) {
     // colour: rgb = max(0, 0.5 + sum_l Y_l(dir) sh_l), dir = (mu - o)/|mu - o|
-    float dv[3] = {g.mean[3 * i] - cam.o[0], g.mean[3 * i + 1] - cam.o[1], g.mean[3 * i + 2] - cam.o[2]};
+    float dv[3] = {gin.m[0] - cam.o[0], gin.m[1] - cam.o[1], gin.m[2] - cam.o[2]};
     const float dinv = rsqrtf(dv[0] * dv[0] + dv[1] * dv[1] + dv[2] * dv[2]);
     const float dir[3] = {dv[0] * dinv, dv[1] * dinv, dv[2] * dinv};
     float Y[NSH];
@@ -457,6 +480,7 @@ static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pla
                       const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
   cudaFuncSetAttribute(k_project_bwd<DEG, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   k_project_bwd<DEG, ACC><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(*g, plan, rt, ctx->cfg, *pr, g2d,
                                                                                       clear_g2d, *grads);
 }
