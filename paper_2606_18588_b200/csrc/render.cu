@@ -19,8 +19,10 @@
 //     whose best pixel stays below alpha_min is skipped for that Gaussian.  Only pairs that the
 //     alpha_min rule would skip anyway are dropped, so results are bit-identical to walking the list.
 //   * backward: a lane accumulates the six moments of dL/dG over its 4 pixels and the colour sums in
-//     registers; ONE warp reduction (14 shuffles for 9 values) and one set of atomics per
-//     (Gaussian, half tile) that has a contributor.
+//     registers and stores its nine partial gradients to a shared staging block (9 conflict-free
+//     stores per (Gaussian, half tile) item); every seven items the 63 rows are summed over the lanes
+//     (one row per lane, rotating column: no bank conflict) and leave as two rounds of 32 distinct
+//     atomics.  ~28 instructions per item instead of ~75 for a shuffle tree + selects (profiles/r01k).
 #include "common.cuh"
 
 namespace {
@@ -219,37 +221,35 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
   }
 }
 
-// Reduce 9 per-lane values over the warp with 12 shuffles instead of 45: at each butterfly step a
-// lane keeps one half of its values and hands the other half to its partner; the ninth value rides
-// along as a plain butterfly until only two values are left, which then share the last two steps.
-// Afterwards lane L with (L & 2) == 0 holds the warp total of v[4*bit4 + 2*bit3 + bit2] and every
-// lane with (L & 2) != 0 holds the total of v8.
-__device__ __forceinline__ float warp_reduce9(const float (&v)[8], float v8, int lane) {
-  const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4, h2 = lane & 2;
-  float a[4], b[2], c;
+// Staging block of one warp in the backward: STAGE_ITEMS (Gaussian, half tile) items x 9 gradient values x 32
+// lane partials.  63 rows = two rounds of 32 row sums; a lane sums its row with a rotating column so that the
+// 32 lanes hit 32 different banks.
+constexpr int STAGE_ITEMS = 7;
+struct __align__(128) Stage { float v[STAGE_ITEMS * 9][32]; };
+
+// Sum the staged rows over the lanes: lane L sums row r*32 + L with eight 16-byte loads whose chunk index is
+// XOR-swizzled by L & 7, so that the eight lanes of a quarter warp (one LDS.128 wavefront) read eight
+// different 16-byte bank groups.  The XOR is applied to the byte address (rows are 128-byte aligned).
+__device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int lane, float* __restrict__ g2d) {
+  __syncwarp();
+  const int rows = nb * 9;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const float send = h16 ? v[i] : v[i + 4], keep = h16 ? v[i + 4] : v[i];
-    a[i] = keep + __shfl_xor_sync(FULL, send, 16);
-  }
-  v8 += __shfl_xor_sync(FULL, v8, 16);
+  for (int r = 0; r < 2; ++r) {
+    const int p = r * 32 + lane;
+    const int pc = p < rows ? p : 0;
+    const unsigned base = (unsigned)__cvta_generic_to_shared(st.v[pc]) + 16u * (unsigned)(lane & 7);
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
 #pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const float send = h8 ? a[i] : a[i + 2], keep = h8 ? a[i + 2] : a[i];
-    b[i] = keep + __shfl_xor_sync(FULL, send, 8);
+    for (int q = 0; q < 8; ++q) {
+      float4 f;
+      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(f.x), "=f"(f.y), "=f"(f.z), "=f"(f.w) : "r"(base ^ (16u * q)));
+      s0 += f.x; s1 += f.y; s2 += f.z; s3 += f.w;
+    }
+    const int item = pc / 9, val = pc - 9 * item;
+    const uint32_t idx = __shfl_sync(FULL, gid, item);
+    if (p < rows) atomicAdd(g2d + (size_t)SPLX_G2D_STRIDE * idx + val, (s0 + s1) + (s2 + s3));
   }
-  v8 += __shfl_xor_sync(FULL, v8, 8);
-  {
-    const float send = h4 ? b[0] : b[1], keep = h4 ? b[1] : b[0];
-    c = keep + __shfl_xor_sync(FULL, send, 4);
-  }
-  v8 += __shfl_xor_sync(FULL, v8, 4);
-  {
-    const float send = h2 ? c : v8, keep = h2 ? v8 : c;
-    c = keep + __shfl_xor_sync(FULL, send, 2);
-  }
-  c += __shfl_xor_sync(FULL, c, 1);
-  return c;
+  __syncwarp();
 }
 
 __global__ void __launch_bounds__(BLOCK)
@@ -257,6 +257,7 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
              int W, int H, int TX, int ntiles, splx_config cfg, const float* __restrict__ ct,
              const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d) {
   __shared__ Ring rings[WARPS];
+  __shared__ Stage stages[WARPS];
   const int tile = blockIdx.x, k = blockIdx.y;
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
   if (r0 == r1) return;
@@ -294,10 +295,13 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 #pragma unroll
   for (int s = 0; s < 4; ++s) smax[s] = __reduce_max_sync(FULL, last[s]);
 
-  const int nb = (int)((bmax + 31) / 32);
+  Stage& stage = stages[warp];
+  int nb = 0;                 // items staged so far (warp-uniform)
+  uint32_t gid = 0;           // lane b keeps the Gaussian index of staged item b
+  const int nbatch = (int)((bmax + 31) / 32);
   int buf = 0;
-  stage_issue(ring, 0, lane, blend, vals, r0 + 32u * (uint32_t)(nb - 1) + lane, r0 + bmax);
-  for (int bi = nb - 1; bi >= 0; --bi, buf ^= 1) {
+  stage_issue(ring, 0, lane, blend, vals, r0 + 32u * (uint32_t)(nbatch - 1) + lane, r0 + bmax);
+  for (int bi = nbatch - 1; bi >= 0; --bi, buf ^= 1) {
     const uint32_t start = 32u * (uint32_t)bi;      // list position (0-based) of entry 0 of this batch
     if (bi > 0) stage_issue(ring, buf ^ 1, lane, blend, vals, r0 + start - 32 + lane, r0 + bmax);
     else cp_async_commit();
@@ -325,7 +329,6 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
       // that does not blend this entry runs the same arithmetic with alpha = 0 (T, Q unchanged, every
       // contribution exactly 0), so the four slots interleave in the pipeline.
       float n0 = 0.f, nx = 0.f, ny = 0.f, nxx = 0.f, nxy = 0.f, nyy = 0.f, q0 = 0.f, q1 = 0.f, q2 = 0.f;
-      bool any = false;
 #pragma unroll
       for (int s = 0; s < 4; ++s) {
         if (!((mj >> s) & 1)) continue;     // warp-uniform
@@ -333,7 +336,6 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
         float G, alpha; bool clamped;
         const bool on = eval_alpha(dx, dy, adx[s & 1], bdx[s & 1], cdy[s >> 1], a.z, cfg.alpha_min, cfg.alpha_max, G, alpha, clamped) &&
                         (c1 <= last[s]);
-        any |= on;
         const float al = on ? alpha : 0.0f;
         const float rom = rcp_approx(1.0f - al);             // 1 - alpha >= 1 - alpha_max > 0
         const float Ti = on ? T[s] * rom : T[s];             // T_i = T_{i+1} / (1 - alpha_i)
@@ -342,33 +344,30 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
         q0 = fmaf(w, gC0[s], q0); q1 = fmaf(w, gC1[s], q1); q2 = fmaf(w, gC2[s], q2);     // dL/dc_i
         const float diff = fmaf(gC0[s], c.x, fmaf(gC1[s], c.y, gC2[s] * c.z)) - Q[s];
         Q[s] = fmaf(al, diff, Q[s]);
-        const float gG = (on && !clamped) ? Ti * diff * G : 0.0f;   // dL/dG-weight of this pixel (dL/do contribution)
+        // o * dL/dG-weight of this pixel: T_i diff G o = w diff where alpha is not clamped (w = alpha_i T_i is 0
+        // for a pixel that does not blend the entry); the factor 1/o is applied once per item below
+        const float gG = clamped ? 0.0f : w * diff;
         const float t1 = gG * dx, t2 = gG * dy;
         n0 += gG; nx += t1; ny += t2;
         nxx = fmaf(t1, dx, nxx); nxy = fmaf(t1, dy, nxy); nyy = fmaf(t2, dy, nyy);
       }
-      if (!__any_sync(FULL, any)) continue;
-      // linear map from the moments to the gradients of (u, v, A, B, C, o); alpha = o 2^(A' dx^2 + B' dx dy + C' dy^2)
-      const float go = a.z * LN2;
-      float v[8];
-      v[0] = go * fmaf(2.0f * b.x, nx, b.y * ny);    // dL/du
-      v[1] = go * fmaf(2.0f * b.z, ny, b.y * nx);    // dL/dv
-      v[2] = -0.5f * a.z * nxx;                      // dL/dA
-      v[3] = -a.z * nxy;                             // dL/dB
-      v[4] = -0.5f * a.z * nyy;                      // dL/dC
-      v[5] = n0;                                     // dL/do
-      v[6] = q0; v[7] = q1;
-      const float tot = warp_reduce9(v, q2, lane);
-      float* dst = g2d + (size_t)SPLX_G2D_STRIDE * __float_as_uint(b.w);
-      if ((lane & 3) == 0) {
-        const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-        atomicAdd(dst + idx, tot);
-      } else if (lane == 2) {
-        atomicAdd(dst + 8, tot);
-      }
+      // linear map from the moments to the gradients of (u, v, A, B, C, o); alpha = o 2^(A' dx^2 + B' dx dy + C' dy^2).
+      // The lane's nine partial sums go to row (item, value) of the staging block; rows are summed over the
+      // lanes seven items at a time (flush_stage): 9 conflict-free stores per item here instead of a shuffle tree.
+      float* row = stage.v[nb * 9];
+      row[lane] = LN2 * fmaf(2.0f * b.x, nx, b.y * ny);         // dL/du   (moments carry the factor o)
+      row[32 + lane] = LN2 * fmaf(2.0f * b.z, ny, b.y * nx);    // dL/dv
+      row[64 + lane] = -0.5f * nxx;                             // dL/dA
+      row[96 + lane] = -nxy;                                    // dL/dB
+      row[128 + lane] = -0.5f * nyy;                            // dL/dC
+      row[160 + lane] = n0 * rcp_approx(fmaxf(a.z, 1e-30f));    // dL/do (o == 0 blends nothing: 0, not NaN)
+      row[192 + lane] = q0; row[224 + lane] = q1; row[256 + lane] = q2;
+      if (lane == nb) gid = __float_as_uint(b.w);
+      if (++nb == STAGE_ITEMS) { flush_stage(stage, nb, gid, lane, g2d); nb = 0; }
     }
     __syncwarp();
   }
+  if (nb) flush_stage(stage, nb, gid, lane, g2d);
   cp_async_wait<0>();
 }
 
