@@ -20,6 +20,7 @@ namespace {
 constexpr int SCAN_THREADS = 512, SCAN_IPT = 4, SCAN_TILE = SCAN_THREADS * SCAN_IPT;
 constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
+static_assert(SCAN_TILE == RS_TILE, "the compaction scan clears the radix status words tile by tile");
 constexpr uint32_t PERSISTENT_CTAS = SPLX_SM_COUNT * 8;   // grid of the persistent kernels: 8 CTAs per SM
 
 struct Counters {   // device-resident counts, written by kernels, read by later kernels
@@ -103,13 +104,20 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
 
 // Persistent: a CTA keeps taking tiles from the ticket counter until the (device-side) element count is
 // exhausted, so the grid is sized for the machine, not for the caller's capacity.
-template <class Op>
+// HIST (the compaction scan): the CTA also counts the four 8-bit digit histograms of the keys it stores (shared
+// atomics, flushed once per CTA) and clears the radix passes' look-back status words of tile t -- output tile t of
+// the depth sort can only hold elements of input tiles <= t -- so the depth sort needs no histogram kernel.
+template <class Op, bool HIST>
 __global__ void __launch_bounds__(SCAN_THREADS)
 k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
-       uint64_t clamp_to) {
+       uint64_t clamp_to, uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
   __shared__ uint32_t sm[33];
   __shared__ uint32_t s_tile;
   __shared__ uint64_t s_excl;
+  __shared__ uint32_t s_hist[HIST ? 4 * 256 : 1];
+  if (HIST) {
+    for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) s_hist[x] = 0;
+  }
   const uint64_t n = op.count(n_ptr);
   const uint64_t ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
   if (n == 0) {
@@ -124,7 +132,11 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
     __syncthreads();
     const uint32_t t = s_tile;
-    if (t >= ntiles) return;
+    if (t >= ntiles) break;
+    if (HIST) {
+#pragma unroll
+      for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) rstatus[(size_t)(x >> 8) * rstride + (size_t)t * 256 + (x & 255)] = 0;
+    }
     const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
     uint32_t v[SCAN_IPT], s = 0;
 #pragma unroll
@@ -145,7 +157,11 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     __syncthreads();
     ex += (uint32_t)s_excl;
 #pragma unroll
-    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex); ex += v[k]; }
+    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex, s_hist); ex += v[k]; }
+  }
+  if (HIST) {
+    __syncthreads();
+    for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
   }
 }
 
@@ -166,24 +182,32 @@ struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order 
   const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n; RunMap map;
   __device__ uint64_t count(const uint64_t*) const { return n; }
   __device__ uint32_t load(uint64_t j) const { return tiles_touched[map(j)] > 0 ? 1u : 0u; }
-  __device__ void store(uint64_t j, uint32_t v, uint32_t ex) const {
-    if (v) { const uint64_t i = map(j); ckeys[ex] = __float_as_uint(depth[i]); cvals[ex] = (uint32_t)i; }
+  __device__ void store(uint64_t j, uint32_t v, uint32_t ex, uint32_t* hist) const {
+    if (v) {
+      const uint64_t i = map(j);
+      const uint32_t key = __float_as_uint(depth[i]);
+      ckeys[ex] = key; cvals[ex] = (uint32_t)i;
+#pragma unroll
+      for (int p = 0; p < 4; ++p) atomicAdd(&hist[p * 256 + ((key >> (8 * p)) & 255u)], 1u);
+    }
   }
 };
 struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, depth order
   const uint32_t* tiles_touched; const uint32_t* cvals; uint32_t* offs;
   __device__ uint64_t count(const uint64_t* n_ptr) const { return *n_ptr; }
   __device__ uint32_t load(uint64_t j) const { return tiles_touched[cvals[j]]; }
-  __device__ void store(uint64_t j, uint32_t, uint32_t ex) const { offs[j] = ex; }
+  __device__ void store(uint64_t j, uint32_t, uint32_t ex, uint32_t*) const { offs[j] = ex; }
 };
 
-template <class Op>
+template <class Op, bool HIST>
 int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket,
-                   uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to) {
+                   uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to, uint32_t* ghist = nullptr,
+                   uint64_t* rstatus = nullptr, size_t rstride = 0) {
   uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
   if (nb == 0) return SPLX_OK;
   if (nb > PERSISTENT_CTAS) nb = PERSISTENT_CTAS;
-  k_scan<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to);
+  k_scan<Op, HIST><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to, ghist,
+                                                         rstatus, rstride);
   SPLX_LAUNCH_CHECK(ctx, "k_scan");
   return SPLX_OK;
 }
@@ -276,6 +300,9 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
   __shared__ uint32_t whist[RS_WARPS][256];
   __shared__ uint32_t dbase[256];
   __shared__ uint32_t gbase[256];
+  __shared__ uint32_t lbase[256];
+  __shared__ KeyT skey[RS_TILE];
+  __shared__ uint32_t sval[RS_TILE];
   __shared__ uint32_t sm[33];
   __shared__ uint32_t s_tile;
   const uint64_t n = *n_ptr;
@@ -324,26 +351,48 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
       __syncwarp();
     }
     __syncthreads();
-    {  // per digit: exclusive prefix over the warps, tile total, chained prefix over the tiles
+    uint32_t run = 0;   // per digit (thread d): exclusive prefix over the warps, tile total
+    {
       const int d = threadIdx.x;
-      uint32_t run = 0;
 #pragma unroll
       for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
-      uint64_t excl = 0;
-      uint64_t* st = status + d;
-      if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
-      else excl = lookback<8>(st, t, 256, run);
-      dbase[d] = gbase[d] + (uint32_t)excl;
+    }
+    {  // position of digit d's first key inside the tile, in digit order
+      uint32_t tot;
+      lbase[threadIdx.x] = block_exclusive_scan(run, sm, tot);
     }
     __syncthreads();
+    // the tile's keys go to shared memory in digit order, so that the scatter below writes runs of consecutive
+    // addresses (one run per digit) instead of 2048 isolated 8- or 12-byte items
 #pragma unroll
     for (int it = 0; it < RS_IPT; ++it) {
       const uint64_t idx = seg + (uint64_t)it * 32 + lane;
       if (idx < n) {
         const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
-        const uint32_t pos = dbase[d] + whist[warp][d] + rank[it];
-        kout[pos] = key[it];
-        vout[pos] = val[it];
+        const uint32_t lp = lbase[d] + whist[warp][d] + rank[it];
+        skey[lp] = key[it];
+        sval[lp] = val[it];
+      }
+    }
+    {  // chained prefix over the tiles (look-back), one chain per digit
+      const int d = threadIdx.x;
+      uint64_t excl = 0;
+      uint64_t* st = status + d;
+      if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
+      else excl = lookback<8>(st, t, 256, run);
+      dbase[d] = gbase[d] + (uint32_t)excl - lbase[d];      // global position = dbase[d] + position in the tile
+    }
+    __syncthreads();
+    const uint32_t nv = (uint32_t)((n - start) < (uint64_t)RS_TILE ? (n - start) : (uint64_t)RS_TILE);
+#pragma unroll
+    for (int it = 0; it < RS_IPT; ++it) {
+      const uint32_t j = (uint32_t)it * RS_THREADS + threadIdx.x;
+      if (j < nv) {
+        const KeyT k = skey[j];
+        const uint32_t d = (uint32_t)(k >> shift) & mask;
+        const uint32_t pos = dbase[d] + j;
+        kout[pos] = k;
+        vout[pos] = sval[j];
       }
     }
   }
@@ -354,14 +403,17 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
 // ghist: [MAX_PASSES][256] u32, status: [npass][tiles][256] u64, both zeroed by the caller.
 template <typename KeyT>
 int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
-               const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets) {
+               const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets,
+               bool have_hist /* histograms counted and status cleared by the producer of the keys */) {
   const uint32_t ntiles_cap = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
   if (ntiles_cap == 0) return SPLX_OK;
   const uint32_t nblocks = ntiles_cap < PERSISTENT_CTAS ? ntiles_cap : PERSISTENT_CTAS;
   const size_t stride = (size_t)ntiles_cap * 256;     // status words per pass
   const PassPlan plan = plan_passes(begin_bit, end_bit);
-  k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, status, stride, plan);
-  SPLX_LAUNCH_CHECK(ctx, "k_radix_hist_all");
+  if (!have_hist) {
+    k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, status, stride, plan);
+    SPLX_LAUNCH_CHECK(ctx, "k_radix_hist_all");
+  }
   for (int p = 0; p < plan.npass; ++p) {
     k_radix_pass<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
                                                                status + (size_t)p * stride, tickets + p,
@@ -378,7 +430,19 @@ __global__ void __launch_bounds__(256)
 k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
-            uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+            uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
+            uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+  // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
+  // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
+  __shared__ uint32_t s_hist[MAX_PASSES * 256];
+  for (int x = threadIdx.x; x < MAX_PASSES * 256; x += blockDim.x) s_hist[x] = 0;
+  {
+    const uint64_t words = ((cnt->m_sorted + RS_TILE - 1) / RS_TILE) * 256;
+    for (int p = 0; p < plan.npass; ++p)
+      for (uint64_t x = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; x < words; x += (uint64_t)gridDim.x * blockDim.x)
+        rstatus[(size_t)p * rstride + x] = 0;
+  }
+  __syncthreads();
   const uint64_t nvis = cnt->n_visible;
   const int lane = threadIdx.x & 31;
   // grid-stride over blocks of 256 visible Gaussians (the grid is sized for the machine; nvis lives on the device)
@@ -407,6 +471,8 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
         const uint32_t slot = slot0 + (uint32_t)((y0 + t / w) * TX + x0 + t % w);
         keys[pos] = ((uint64_t)slot << 32) | dbits;
         vals[pos] = i;
+        for (int p = 0; p < plan.npass; ++p)
+          atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
       }
     }
   }
@@ -425,16 +491,21 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
         const uint32_t slot = ss + (uint32_t)((sy0 + t / sw) * TX + sx0 + t % sw);
         keys[pos] = ((uint64_t)slot << 32) | sd;
         vals[pos] = si;
+        for (int p = 0; p < plan.npass; ++p)
+          atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
       }
     }
   }
   }
+  __syncthreads();
+  for (int x = threadIdx.x; x < plan.npass * 256; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
 }
 
 __global__ void __launch_bounds__(256)
 k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint8_t* __restrict__ tile_state,
-              uint32_t* __restrict__ ranges) {
+              uint32_t* __restrict__ ranges, uint64_t* __restrict__ m_out) {
   const uint64_t m = cnt->m_sorted;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *m_out = cnt->m_total;
   for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j < m; j += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t s = (uint32_t)(keys[j] >> 32);
     if (tile_state && tile_state[s]) continue;   // a skipped (partition, tile) slot keeps the empty range (0,0)
@@ -520,14 +591,16 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   vop.map.n = rt.n;
   for (int r = 0; r < rt.n; ++r) { vop.map.begin[r] = rt.begin[r]; vop.map.jprefix[r] = rt.jprefix[r]; }
   vop.map.jprefix[rt.n] = rt.jprefix[rt.n];
-  if ((rc = scan_exclusive(ctx, vop, (uint64_t)n_act, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
-                           &cnt->n_visible, nullptr, 0))) return rc;
-  // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers)
+  const size_t stride_d = (((size_t)n_act + RS_TILE - 1) / RS_TILE) * 256;   // status words per pass, depth sort
+  if ((rc = scan_exclusive<VisibleOp, true>(ctx, vop, (uint64_t)n_act, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
+                                            &cnt->n_visible, nullptr, 0, (uint32_t*)(base + L.ghist_d),
+                                            (uint64_t*)(base + L.st_depth), stride_d))) return rc;
+  // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers); histograms came with step 1
   if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n_act, &cnt->n_visible, 0, 32,
-                                 (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2]))) return rc;
+                                 (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2], true))) return rc;
   // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
-  if ((rc = scan_exclusive(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
+  if ((rc = scan_exclusive<TouchedOp, false>(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
                            &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
   const int passes = (sbits + 7) / 8;
   uint64_t* k0 = (passes & 1) ? keys_tmp : out->keys;   // so that the last pass lands in out->keys
@@ -539,16 +612,16 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   for (int k = 0; k <= K; ++k) parts.off[k] = part_offsets[k];
   const uint64_t emit_blocks = ((uint64_t)n_act + 255) / 256, range_blocks = (out->capacity + 255) / 256;
   k_emit_keys<<<(unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
-      pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0);
+      pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0,
+      plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
+      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
   // 4. stable sort on the slot bits
   if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
-                                 (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6]))) return rc;
+                                 (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6], true))) return rc;
   // 5. ranges
   k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
-      out->keys, cnt, plan.tile_state, out->tile_ranges);
+      out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
-  k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
-  SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
   return SPLX_OK;
 }
