@@ -307,6 +307,20 @@ def run_ours(args):
                 for i, n in enumerate(STAGES)}
     clocks = sampler.stop() if sampler else None
 
+    # the same iteration replayed from a CUDA graph (a1-a10 captured once, Adam outside): no per-stage events
+    graph_ms = None
+    if not args.dense:
+        for _ in range(3):
+            tr.step_graph(0, cam, target1, saturation=args.saturation, sat_eps=args.sat_eps)
+        barrier()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for s in range(args.steps):
+            tr.step_graph(0, cam, target1, saturation=args.saturation, sat_eps=args.sat_eps)
+        g1.record()
+        barrier()
+        graph_ms = replicas.max_over_ranks(g0.elapsed_time(g1), cuda=True) / args.steps
+
     # end to end through the public API with HOST buffers: the step's input (target image) comes from
     # pinned host memory, the result (rendered image + loss) goes back to pinned host memory, every step
     tgt_host = torch.from_numpy(sc.targets[0]).pin_memory()
@@ -314,12 +328,15 @@ def run_ours(args):
     loss_host = torch.empty(1, dtype=torch.float64).pin_memory()
 
     def step_e2e():
-        target.copy_(tgt_host, non_blocking=True)
-        tr.loss_sum.zero_()
-        step()
-        img_host.copy_(result_image, non_blocking=True)
-        loss_host.copy_(tr.loss_sum, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
+        if args.dense:
+            target.copy_(tgt_host, non_blocking=True)
+            tr.loss_sum.zero_()
+            step()
+            img_host.copy_(result_image, non_blocking=True)
+            loss_host.copy_(tr.loss_sum, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+        else:   # the public call: Trainer.step_host (copies on a side stream, overlapped with the kernels)
+            tr.step_host(0, cam, tgt_host, img_host, loss_host, saturation=args.saturation, sat_eps=args.sat_eps)
 
     for _ in range(3):
         step_e2e()
@@ -335,6 +352,11 @@ def run_ours(args):
         return
 
     pk = peaks()
+    # `value`: the iteration as a user runs it (Trainer.step_graph: a1-a10 replayed from a CUDA graph, then Adam), K
+    # steps between two events; the eager pass above (10 event records per step) gives the per-stage times
+    ms_eager = ms_step
+    if graph_ms:
+        ms_step = graph_ms
     mpix = world * W * H / (ms_step * 1e-3) / 1e6
     # dominant kernel: the rasteriser backward (FP32 issue + shuffles + atomics): algorithmic flops
     dom = max(stage_ms, key=stage_ms.get)
@@ -393,6 +415,10 @@ def run_ours(args):
                             pairs_blended=pairs_blend, pairs_evaluated_fwd=pairs_eval, half_tile_items_fwd=items_fwd),
                 iters_per_s=world * 1e3 / ms_step, stages_ms=stage_ms, per_kernel=per_kernel, roofline=roof,
                 cpu_baseline=cpu, clocks=clocks, gpu_launches=int(launches),
+                timing=dict(value_from=("K steps of Trainer.step_graph (CUDA-graph replay of a1-a10 + Adam)" if graph_ms
+                                        else "K eager steps with per-stage events"),
+                            ms_per_step_eager_with_stage_events=ms_eager,
+                            stages_ms_from="a separate pass of K eager steps with a CUDA event between stages"),
                 e2e=dict(value=world * W * H / (e2e_ms * 1e-3) / 1e6, unit=UNIT, ms_per_step=e2e_ms,
                          h2d_bytes_per_step=int(tgt_host.numel() * 4),
                          d2h_bytes_per_step=int(img_host.numel() * 4 + 8)))

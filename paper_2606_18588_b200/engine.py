@@ -57,6 +57,8 @@ class Trainer:
         self.pairs = torch.zeros(4, dtype=torch.int64, device=dev)
         self.step_count = 0
         self._cam = None
+        self._aabb = None
+        self._side = None
         self._ws_sort = None
         self._ws_bwd = None
         # plan path (visibility prediction / consolidated views): buffers with a leading view dimension
@@ -220,3 +222,93 @@ class Trainer:
             self.backward_plan(overwrite=(gi == 0))
         self.adam_step(len(view_ids))
         return len(groups)
+
+    # ---- end to end from HOST buffers ---------------------------------------------------------------
+    def _host_body(self, main, side, plan, state, target_host, image_host, loss_host, sat_eps):
+        """a1-a10 with the host copies on the side stream: the target travels while the forward renders (it is
+        first needed by the loss), the image travels while the backward runs."""
+        side.wait_stream(main)
+        with torch.cuda.stream(side):
+            self._target_dev[0].copy_(target_host, non_blocking=True)
+            self._ev_target.record(side)
+        self.loss_sum.zero_()
+        images = self.forward_plan(plan, sat_eps, state)
+        if image_host is not None:
+            side.wait_stream(main)
+            with torch.cuda.stream(side):
+                image_host.copy_(images[0], non_blocking=True)
+        main.wait_event(self._ev_target)
+        self.loss_grad_plan(self._target_dev)
+        self.backward_plan(overwrite=True)
+        main.wait_stream(side)
+        if loss_host is not None:    # after the image has left: the two copies share one device-to-host engine, and
+            loss_host.copy_(self.loss_sum, non_blocking=True)   # 8 bytes queued behind 25 MB would stall this stream
+
+    def step_host(self, view_id, cam, target_host, image_host=None, loss_host=None, saturation=False, sat_eps=1e-4,
+                  graph=True):
+        """One whole training iteration (a1-a11) on one view whose target image lives in pinned HOST memory; the
+        rendered image and the loss go back to pinned host memory.  With graph=True the launches of a1-a10 and the
+        copies are captured once per (view, buffers) into a CUDA graph and replayed (one launch per step instead of
+        ~25); Adam stays outside the graph because its bias correction depends on the step number.  Returns after
+        the device has drained, so the host buffers are valid."""
+        dev = self.ctx.device
+        main = torch.cuda.current_stream(dev)
+        if self._side is None:
+            self._side = torch.cuda.Stream(dev)
+            self._ev_target = torch.cuda.Event()
+            self._target_dev = torch.empty((1, self.H, self.W, 3), dtype=torch.float32, device=dev)
+            self._graphs = {}
+        if not graph:
+            plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
+                           else (self.make_plan([cam]), None))
+            self._host_body(main, self._side, plan, state, target_host, image_host, loss_host, sat_eps)
+        else:
+            key = (view_id, target_host.data_ptr(), image_host.data_ptr() if image_host is not None else 0,
+                   loss_host.data_ptr() if loss_host is not None else 0, bool(saturation), float(sat_eps))
+            if key not in self._graphs:
+                plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
+                               else (self.make_plan([cam]), None))
+                self._workspaces(cam)
+                self._view_buffers(1)
+                torch.cuda.synchronize(dev)
+                g = torch.cuda.CUDAGraph()
+                old = main.cuda_stream
+                with torch.cuda.graph(g):
+                    cap = torch.cuda.current_stream(dev)
+                    self.ctx.set_stream(cap.cuda_stream)
+                    try:
+                        self._host_body(cap, self._side, plan, state, target_host, image_host, loss_host, sat_eps)
+                    finally:
+                        self.ctx.set_stream(old)
+                self._graphs[key] = (g, plan)          # the plan owns the host arrays the capture read
+            self._graphs[key][0].replay()
+        self.adam_step(1)
+        main.synchronize()
+
+    def step_graph(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
+        """One whole training iteration on one view with the target already on the device ([1,H,W,3]): a1-a10
+        replayed from a CUDA graph captured at the first call for this (view, target), then Adam.  Asynchronous."""
+        dev = self.ctx.device
+        if getattr(self, "_dgraphs", None) is None:
+            self._dgraphs = {}
+        key = (view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps))
+        if key not in self._dgraphs:
+            plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
+                           else (self.make_plan([cam]), None))
+            self._workspaces(cam)
+            self._view_buffers(1)
+            main = torch.cuda.current_stream(dev)
+            torch.cuda.synchronize(dev)
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                self.ctx.set_stream(torch.cuda.current_stream(dev).cuda_stream)
+                try:
+                    self.loss_sum.zero_()
+                    self.forward_plan(plan, sat_eps, state)
+                    self.loss_grad_plan(target_dev)
+                    self.backward_plan(overwrite=True)
+                finally:
+                    self.ctx.set_stream(main.cuda_stream)
+            self._dgraphs[key] = (g, plan)
+        self._dgraphs[key][0].replay()
+        self.adam_step(1)

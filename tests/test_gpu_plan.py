@@ -279,3 +279,31 @@ def test_iteration_views_with_visibility_prediction(city):
             err = np.abs(img - res.image).max(-1)
             assert (err[~frag] <= eps * rgb_max + 1e-5).all()
     assert skipped > 0
+
+
+def test_step_host_equals_the_stage_calls(aerial):
+    """Trainer.step_host (the end-to-end call bench.py times: host buffers, copies overlapped on a side stream)
+    produces the image, loss and parameter update of the plain stage-by-stage iteration."""
+    sc = aerial
+    cam = sc.cameras[0]
+    a, b = _trainer(sc), _trainer(sc)
+    tgt_host = torch.from_numpy(sc.targets[0]).pin_memory()
+    img_host = torch.empty((cam.height, cam.width, 3), dtype=torch.float32).pin_memory()
+    loss_host = torch.zeros(1, dtype=torch.float64).pin_memory()
+    target = torch.from_numpy(sc.targets[0]).cuda()
+    for it in range(2):
+        a.step_host(0, cam, tgt_host, img_host, loss_host)
+        b.loss_sum.zero_()
+        b.forward(cam)
+        b.loss_grad(target)
+        b.backward(overwrite=True)
+        b.adam_step()
+        torch.cuda.synchronize()
+        if it == 0:   # same parameters in: bit-equal image (later steps differ by the atomics' summation order)
+            assert torch.equal(img_host.cuda(), b.image)
+            assert float(loss_host.item()) == pytest.approx(float(b.loss_sum.item()), rel=1e-12)
+        else:
+            assert torch.allclose(img_host.cuda(), b.image, rtol=0, atol=1e-5)
+            assert float(loss_host.item()) == pytest.approx(float(b.loss_sum.item()), rel=1e-6)
+    for key in scenes.PARAM_KEYS:
+        assert torch.allclose(a.params[key], b.params[key], rtol=1e-3, atol=1e-6), key
