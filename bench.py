@@ -51,6 +51,12 @@ def workload(name):
         return scenes.small_aerial()
     if name == "city_10M":
         return scenes.city()                         # configs[2]: 10M Gaussians, K=8, B=4 views
+    if name == "city_40M":                           # configs[3]: 40M Gaussians, 1000 m, 4K views, K=16, B=4 (device generator)
+        return scenes.city_device(n=40_000_000, width=3840, height=2160, extent=1000.0, n_buildings=800, grid=(4, 4),
+                                  altitude=200.0, height_range=(5.0, 60.0), n_views=4, name="city_40M")
+    if name == "city_100M":                          # configs[4]: 100M Gaussians, 2000 m, 1080p, K=32, B=8
+        return scenes.city_device(n=100_000_000, width=1920, height=1080, extent=2000.0, n_buildings=3200, grid=(8, 4),
+                                  altitude=200.0, height_range=(5.0, 80.0), n_views=8, name="city_100M")
     if name == "city_small":
         return scenes.small_city()
     if name == "blocks_small":
@@ -443,13 +449,16 @@ def run_views(args):
     B = min(args.views, len(sc.cameras))
     cams = sc.cameras[:B]
     W, H = cams[0].width, cams[0].height
-    cap = {"city_10M": 64_000_000}.get(args.workload)
+    cap = {"city_10M": 64_000_000, "city_40M": 160_000_000, "city_100M": 96_000_000}.get(args.workload)
     tr = Trainer(sc.params, sc.part_offsets, W, H, sc.sh_degree, sc.bg, capacity=cap)
+    aabbs = scenes.partition_aabbs(sc.params, sc.part_offsets)
+    sc.params = None                                   # a device-generated scene: release the generator's copy
+    torch.cuda.empty_cache()
     if args.no_visibility:   # boxes that contain everything: every partition participates in every view, no tile is invisible
         big = np.float32(1e6)
         tr.set_aabbs(np.full((tr.K, 3), -big), np.full((tr.K, 3), big))
     else:
-        tr.set_aabbs(*scenes.partition_aabbs(sc.params, sc.part_offsets))
+        tr.set_aabbs(*aabbs)
     targets = torch.from_numpy(np.stack(sc.targets[:B])).cuda()
     ids = list(range(B))
     kw = dict(consolidate=not args.no_consolidate, saturation=args.saturation, sat_eps=args.sat_eps)
@@ -486,7 +495,9 @@ def run_views(args):
                             sat_eps=args.sat_eps, participants=[bin(p) for p in parts], buckets=groups,
                             tile_state=skipped, intersections_last_bucket=M,
                             l2="working set (params+grads+moments) is larger than the 126 MB L2"),
-                iters_per_s=1e3 / ms, clocks=clocks, gpu_launches=int(launches))
+                iters_per_s=1e3 / ms, clocks=clocks, gpu_launches=int(launches),
+                peak_device_memory_GB=torch.cuda.max_memory_allocated() / 1e9,
+                capacity_ok=bool(M <= tr.capacity))
     print(json.dumps(line))
 
 

@@ -31,7 +31,7 @@ class Trainer:
                  capacity=None, device=0, cfg=None, lr=None):
         self.ctx = binding.Context(device, cfg=cfg)
         dev = self.ctx.device
-        self.n = int(params["mean"].shape[0])
+        self.n = int(params["opacity_logit"].shape[0])
         self.K = len(part_offsets) - 1
         self.part_offsets = [int(x) for x in part_offsets]
         self.W, self.H, self.sh_degree, self.bg = int(width), int(height), int(sh_degree), tuple(bg)
@@ -44,7 +44,11 @@ class Trainer:
             for k in PARAM_KEYS:
                 views[k] = self.flat[name][offs[k]:offs[k] + self.n * PARAM_WIDTH[k]]
         for k in PARAM_KEYS:
-            self.params[k].copy_(torch.from_numpy(np.ascontiguousarray(params[k], np.float32).reshape(-1)))
+            src = params[k]
+            if isinstance(src, torch.Tensor):       # a device-generated scene (scenes.city_device)
+                self.params[k].copy_(src.reshape(-1))
+            else:
+                self.params[k].copy_(torch.from_numpy(np.ascontiguousarray(src, np.float32).reshape(-1)))
         self.proj = binding.Projected(self.n, dev)
         # capacity for the tile intersections: caller's bound, else a generous default
         self.capacity = int(capacity) if capacity is not None else max(1 << 16, 24 * self.n)

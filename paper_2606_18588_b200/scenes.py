@@ -126,9 +126,15 @@ def partition_aabbs(params, part_offsets, inflate_sigma=3.0):
     K = len(part_offsets) - 1
     lo = np.zeros((K, 3), np.float32)
     hi = np.zeros((K, 3), np.float32)
+    on_device = not isinstance(params["mean"], np.ndarray)      # torch tensors of a device-generated scene
     for k in range(K):
         a, b = int(part_offsets[k]), int(part_offsets[k + 1])
-        if b > a:
+        if b > a and on_device:
+            m = params["mean"].reshape(-1, 3)[a:b].double()
+            r = inflate_sigma * params["log_scale"].reshape(-1, 3)[a:b].double().max(1).values.exp()[:, None]
+            lo[k] = np.floor((m - r).min(0).values.cpu().numpy() * 1024) / 1024
+            hi[k] = np.ceil((m + r).max(0).values.cpu().numpy() * 1024) / 1024
+        elif b > a:
             m = params["mean"][a:b].astype(np.float64)
             r = inflate_sigma * np.exp(params["log_scale"][a:b].astype(np.float64).max(1))[:, None]
             lo[k] = np.floor((m - r).min(0) * 1024) / 1024        # outward rounding to a float32-exact grid
@@ -283,3 +289,68 @@ def small_blocks(seed=0, n=24_000, width=320, height=176, n_views=6, grid=(4, 2)
         sc.cameras.append(aerial_camera(width, height, 60.0, altitude, pitch_deg, crng.uniform(0, 360), tgt))
         sc.targets.append(np.random.default_rng(seed + 1 + 1000 * v).uniform(0, 1, (height, width, 3)).astype(np.float32))
     return sc
+
+
+def city_device(seed=0, n=40_000_000, width=3840, height=2160, extent=1000.0, n_buildings=800, grid=(4, 4),
+                altitude=200.0, pitch_deg=45.0, fov_deg=60.0, height_range=(5.0, 60.0), sh_degree=3, n_views=4,
+                name="city_40M", device="cuda"):
+    """The configs[2] recipe drawn ON THE DEVICE with a seeded torch generator, for BASELINE.json configs[3]
+    (40M Gaussians, 1000 m, 4K views, K = 16) and configs[4] (100M, 2000 m, K = 32): the host arrays would be
+    9-24 GB.  Same distributions as `city`; the random streams differ from numpy's, so `city_device(n=10M)` is
+    a different (equally distributed) scene than `city()`.  params are CUDA tensors ordered by partition;
+    slices are copied back to the host where a test needs them."""
+    import torch
+    g = torch.Generator(device=device); g.manual_seed(seed)
+    f32 = dict(dtype=torch.float32, device=device)
+    U = lambda *shape: torch.rand(*shape, generator=g, **f32)
+    Nrm = lambda *shape: torch.randn(*shape, generator=g, **f32)
+    half = extent / 2
+    nb = n_buildings
+    bc = (U(nb, 2) * 2 - 1) * half
+    bs = 10.0 + 30.0 * U(nb, 2)
+    bh = height_range[0] + (height_range[1] - height_range[0]) * U(nb)
+    n_b = int(0.7 * n); n_g = n - n_b
+    area = torch.stack([bs[:, 0] * bs[:, 1], bs[:, 1] * bh, bs[:, 1] * bh, bs[:, 0] * bh, bs[:, 0] * bh], 1)
+    prob = (area / area.sum()).reshape(-1)
+    face = torch.multinomial(prob, n_b, replacement=True, generator=g)
+    b, f = face // 5, face % 5
+    a = U(n_b) - 0.5
+    c = U(n_b)
+    bsx, bsy, bhh = bs[b, 0], bs[b, 1], bh[b]
+    x = torch.where(f == 0, a * bsx, torch.where(f == 1, 0.5 * bsx, torch.where(f == 2, -0.5 * bsx, a * bsx)))
+    y = torch.where(f == 0, (c - 0.5) * bsy, torch.where(f <= 2, a * bsy, torch.where(f == 3, 0.5 * bsy, -0.5 * bsy)))
+    z = torch.where(f == 0, bhh, c * bhh)
+    mean = torch.empty((n, 3), **f32)
+    mean[:n_b, 0] = bc[b, 0] + x; mean[:n_b, 1] = bc[b, 1] + y; mean[:n_b, 2] = z
+    mean[:n_b] += 0.1 * Nrm(n_b, 3)
+    mean[n_b:, 0:2] = (U(n_g, 2) * 2 - 1) * half
+    mean[n_b:, 2] = 0.05 * Nrm(n_g)
+    del b, f, a, c, x, y, z, bsx, bsy, bhh, face
+    sp_b = float(1.0 / np.sqrt(n_b / float(area.sum())))
+    sp_g = float(1.0 / np.sqrt(n_g / (extent * extent)))
+    log_scale = torch.empty((n, 3), **f32)
+    log_scale[:n_b] = np.log(1.5 * sp_b) + 0.5 * Nrm(n_b, 3)
+    log_scale[n_b:] = np.log(1.0 * sp_g) + 0.5 * Nrm(n_g, 3)
+    logit = torch.empty(n, **f32)
+    logit[:n_b] = 2.0 + Nrm(n_b); logit[n_b:] = Nrm(n_g)
+    quat = Nrm(n, 4); quat /= quat.norm(dim=1, keepdim=True)
+    K = grid[0] * grid[1]
+    ix = torch.clamp(torch.floor((mean[:, 0] + half) / extent * grid[0]).long(), 0, grid[0] - 1)
+    iy = torch.clamp(torch.floor((mean[:, 1] + half) / extent * grid[1]).long(), 0, grid[1] - 1)
+    part_id = iy * grid[0] + ix
+    order = torch.argsort(part_id, stable=True)
+    counts = torch.bincount(part_id, minlength=K).cpu().numpy()
+    offs = np.zeros(K + 1, np.int64); offs[1:] = np.cumsum(counts)
+    del ix, iy, part_id
+    params = dict(mean=mean[order].contiguous(), log_scale=log_scale[order].contiguous(), quat=quat[order].contiguous(),
+                  opacity_logit=logit[order].contiguous())
+    del mean, log_scale, quat, logit, order
+    params["sh"] = 0.2 * Nrm(n, 16, 3)          # i.i.d.: needs no reordering
+    crng = np.random.default_rng(seed + 2)
+    cams, targets = [], []
+    for v in range(n_views):
+        tgt = np.append(crng.uniform(-0.4 * extent, 0.4 * extent, 2), 0.0)
+        cams.append(aerial_camera(width, height, fov_deg, altitude, pitch_deg, crng.uniform(0, 360), tgt))
+        targets.append(np.random.default_rng(seed + 1 + 1000 * v).uniform(0, 1, (height, width, 3)).astype(np.float32))
+    return Scene(name, params, offs, cams, targets, sh_degree,
+                 meta=dict(seed=seed, config="configs[3]/[4] recipe, device generator", grid=grid, extent=extent))
