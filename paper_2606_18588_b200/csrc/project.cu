@@ -265,17 +265,18 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   const CamDev& cam = plan.cam[view < 0 ? 0 : view];
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;        // float4 chunks of a row that hold used coefficients
-  // every per-Gaussian input is requested up front (independent loads in flight together; a culled row costs
-  // ~100 B more, but the kernel was stalled on these dependent loads: profiles/r01k)
+  // Two dependent rounds of loads: the radius (4 B per row, decides visibility), then -- for visible rows only --
+  // every other per-Gaussian input at once (independent loads in flight together).  Requesting them inside the
+  // geometry chain stalled the kernel on dependent loads (profiles/r01k); requesting them for culled rows too
+  // moved ~100 B per culled row, which is most rows on the city scenes (profiles/r01n).
   const bool inr = (i < run_end) && (view >= 0);
-  int rad = 0;
+  const int rad = inr ? pr.radius[i] : 0;
   GeoIn gin;
   float4 g0 = make_float4(0.f, 0.f, 0.f, 0.f), g1 = g0, g2 = g0;
   float op = 0.f;
   uint8_t cl = 0;
   float4* gp = reinterpret_cast<float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
-  if (inr) {
-    rad = pr.radius[i];
+  if (rad > 0) {
     gin = load_geo(g, i);
     g0 = gp[0]; g1 = gp[1]; g2 = gp[2];
     op = pr.conic_opacity[4 * i + 3];

@@ -463,37 +463,38 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
     }
     slot0 = (uint32_t)lo * (uint32_t)(TX * TY);
   }
-  const bool big = tt > 32;
-  if (!big) {
-    for (int t = 0; t < tt; ++t) {
-      const uint64_t pos = (uint64_t)o + t;
-      if (pos < capacity) {
-        const uint32_t slot = slot0 + (uint32_t)((y0 + t / w) * TX + x0 + t % w);
-        keys[pos] = ((uint64_t)slot << 32) | dbits;
-        vals[pos] = i;
-        for (int p = 0; p < plan.npass; ++p)
-          atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
-      }
+  // The 32 runs of a warp are adjacent in the output (offs is the running sum of tiles_touched in this very
+  // order), so the warp writes its whole range [o_0, o_0 + T) cooperatively: lane l produces output slot
+  // s0 + l, finds the owning Gaussian by a binary search over the lanes' run starts (5 shuffles) and fetches its
+  // rectangle (6 shuffles).  Every store instruction covers 32 consecutive keys / values.
+  uint32_t pre = (uint32_t)tt;                      // exclusive prefix of tt over the warp
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, pre, d); if (lane >= d) pre += v; }
+  const uint32_t T = __shfl_sync(0xffffffffu, pre, 31);
+  pre -= (uint32_t)tt;
+  const uint32_t o0 = __shfl_sync(0xffffffffu, o, 0);
+  for (uint32_t s0 = 0; s0 < T; s0 += 32) {
+    const uint32_t sidx = s0 + lane;
+    int own = 0;
+#pragma unroll
+    for (int step = 16; step >= 1; step >>= 1) {
+      const int cand = own + step;
+      const uint32_t pc = __shfl_sync(0xffffffffu, pre, cand & 31);
+      if (cand < 32 && pc <= sidx) own = cand;
     }
-  }
-  // footprints covering many tiles are emitted by the whole warp (coalesced, no long serial tail)
-  unsigned bm = __ballot_sync(0xffffffffu, big);
-  while (bm) {
-    const int src = __ffs(bm) - 1;
-    bm &= bm - 1;
-    const int sx0 = __shfl_sync(0xffffffffu, x0, src), sy0 = __shfl_sync(0xffffffffu, y0, src);
-    const int sw = __shfl_sync(0xffffffffu, w, src), stt = __shfl_sync(0xffffffffu, tt, src);
-    const uint32_t so = __shfl_sync(0xffffffffu, o, src), si = __shfl_sync(0xffffffffu, i, src);
-    const uint32_t sd = __shfl_sync(0xffffffffu, dbits, src), ss = __shfl_sync(0xffffffffu, slot0, src);
-    for (int t = lane; t < stt; t += 32) {
-      const uint64_t pos = (uint64_t)so + t;
-      if (pos < capacity) {
-        const uint32_t slot = ss + (uint32_t)((sy0 + t / sw) * TX + sx0 + t % sw);
-        keys[pos] = ((uint64_t)slot << 32) | sd;
-        vals[pos] = si;
-        for (int p = 0; p < plan.npass; ++p)
-          atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
-      }
+    const uint32_t t = sidx - __shfl_sync(0xffffffffu, pre, own);
+    const int sx0 = __shfl_sync(0xffffffffu, x0, own), sy0 = __shfl_sync(0xffffffffu, y0, own);
+    const int sw = __shfl_sync(0xffffffffu, w, own);
+    const uint32_t si = __shfl_sync(0xffffffffu, i, own), sd = __shfl_sync(0xffffffffu, dbits, own);
+    const uint32_t ss = __shfl_sync(0xffffffffu, slot0, own);
+    const uint64_t pos = (uint64_t)o0 + sidx;
+    if (sidx < T && pos < capacity) {
+      const uint32_t ty = t / (uint32_t)sw;
+      const uint32_t slot = ss + (uint32_t)((sy0 + (int)ty) * TX + sx0 + (int)(t - ty * (uint32_t)sw));
+      keys[pos] = ((uint64_t)slot << 32) | sd;
+      vals[pos] = si;
+      for (int p = 0; p < plan.npass; ++p)
+        atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
     }
   }
   }
