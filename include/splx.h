@@ -283,6 +283,16 @@ int splx_render_partial_plan(splx_ctx *ctx, const splx_projected *proj, const sp
 int splx_compose_plan(splx_ctx *ctx, int K, const splx_partial *partials, const splx_binning *bins,
                       const splx_plan *plan, const float bg[3], float *image, float *T_total,
                       float sat_eps, uint8_t *tile_state_out);
+/* a6 + a7 + a8 in one pass over the partial pixels: splx_compose_plan, then the mean-L1 gradient of
+ * splx_l1_loss_grad over the B*H*W*3 values of `image` against `targets` [B,H,W,3] (scale as there: pass B to
+ * give every view its own mean), then splx_compose_backward_plan with dL_dT_total = NULL -- statement by
+ * statement the same arithmetic, without the second read of the partials and without dL/dimage ever leaving
+ * the SM.  image, T_total (may be NULL), g_ct, loss_sum (device double, += sum|.|, may be NULL) and
+ * tile_state_out are written as by the three staged calls. */
+int splx_compose_l1_backward_plan(splx_ctx *ctx, int K, const splx_partial *partials,
+                                  const splx_binning *bins, const splx_plan *plan, const float bg[3],
+                                  const float *targets, float scale, float *image, float *T_total,
+                                  double *loss_sum, float *g_ct, float sat_eps, uint8_t *tile_state_out);
 int splx_compose_backward_plan(splx_ctx *ctx, int K, const splx_partial *partials,
                                const splx_binning *bins, const splx_plan *plan, const float bg[3],
                                const float *dL_dimage, const float *dL_dT_total, float *g_ct);

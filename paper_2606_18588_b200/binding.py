@@ -32,6 +32,7 @@ EXPORTS = [
     "splx_visible_regions", "splx_schedule_views", "splx_project_plan", "splx_bin_sort_plan",
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
+    "splx_compose_l1_backward_plan",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -131,6 +132,8 @@ def lib():
         L.splx_render_partial_plan.argtypes = [vp, vp, vp, C.c_int, vp, vp, vp]
         L.splx_compose_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, C.c_float, vp]
         L.splx_compose_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp]
+        L.splx_compose_l1_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, C.c_float, vp, vp, vp, vp,
+                                                    C.c_float, vp]
         L.splx_raster_backward_plan.argtypes = [vp, vp, vp, C.c_int, vp, vp, vp, vp]
         L.splx_project_backward_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp]
         L.splx_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp, vp,
@@ -421,6 +424,16 @@ class Context:
         self._check(lib().splx_compose_plan(self._h, plan.K, C.byref(ps), C.byref(bs) if bs is not None else None,
                                             plan.ref(), b, _ptr(image), _ptr(T_total), float(sat_eps),
                                             _ptr(tile_state_out)))
+
+    def compose_l1_backward_plan(self, partials: Partial, bins, plan: Plan, bg, targets, image, T_total, loss_sum, g_ct,
+                                 scale=1.0, sat_eps=1e-4, tile_state_out=None):
+        b = (C.c_float * 3)(*[float(x) for x in bg])
+        ps = partials.struct()
+        bs = bins.struct() if bins is not None else None
+        self._check(lib().splx_compose_l1_backward_plan(self._h, plan.K, C.byref(ps), C.byref(bs) if bs is not None else None,
+                                                        plan.ref(), b, _ptr(targets), float(scale), _ptr(image),
+                                                        _ptr(T_total), _ptr(loss_sum), _ptr(g_ct), float(sat_eps),
+                                                        _ptr(tile_state_out)))
 
     def compose_backward_plan(self, partials: Partial, bins, plan: Plan, bg, g_image, g_T_total, g_ct):
         b = (C.c_float * 3)(*[float(x) for x in bg])

@@ -216,6 +216,23 @@ int splx_compose_plan(splx_ctx* ctx, int K, const splx_partial* partials, const 
   return launch_compose_fwd(ctx, partials, bins, pd, bg, image, T_total, sat_eps, tile_state_out);
 }
 
+int splx_compose_l1_backward_plan(splx_ctx* ctx, int K, const splx_partial* partials, const splx_binning* bins,
+                                  const splx_plan* plan, const float bg[3], const float* targets, float scale,
+                                  float* image, float* T_total, double* loss_sum, float* g_ct, float sat_eps,
+                                  uint8_t* tile_state_out) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!partial_ok(partials) || !bg || !image || !targets || !g_ct || !aligned16(g_ct))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_l1_backward: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_compose_l1_backward", K, plan, &pd))) return rc;
+  if ((pd.flags & SPLX_PLAN_SPARSE) && !bins_ok(bins))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_l1_backward: SPLX_PLAN_SPARSE needs the binning");
+  if (tile_state_out && !(sat_eps >= 0.f)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_l1_backward: sat_eps must be >= 0");
+  return launch_compose_fused(ctx, partials, bins, pd, bg, targets, scale, image, T_total, loss_sum, g_ct, sat_eps,
+                              tile_state_out);
+}
+
 int splx_compose(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
                  float* image, float* T_total) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;

@@ -141,6 +141,9 @@ int launch_compose_fwd(splx_ctx*, const splx_partial*, const splx_binning* bins,
                        float* image, float* T_total, float sat_eps, uint8_t* tile_state_out);
 int launch_compose_bwd(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
                        const float* g_image, const float* g_T_total, float* g_ct);
+int launch_compose_fused(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
+                         const float* target, float scale, float* image, float* T_total, double* loss_sum, float* g_ct,
+                         float sat_eps, uint8_t* tile_state_out);
 int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count, float scale,
               float* g_image, double* loss_sum);
 int launch_adam_groups(splx_ctx*, float* param, float* grad, float* m, float* v, int n_groups,

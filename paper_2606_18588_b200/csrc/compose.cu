@@ -143,6 +143,96 @@ k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, const u
   }
 }
 
+// a6 + a7 + a8 in ONE pass over the partial pixels (splx_compose_l1_backward_plan): the forward composite, the
+// mean-L1 loss gradient against the view's target and the composition backward all need the same ordered
+// partials of the pixel, so the staged path's second read of the partials and the image / dL/dimage round
+// trip through HBM disappear.  Arithmetic is the staged kernels', statement by statement.
+template <int KMAX, bool SAT>
+__global__ void __launch_bounds__(CB)
+k_compose_fused(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
+                const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
+                float bg1, float bg2, const float* __restrict__ target, float gscale, float* __restrict__ image,
+                float* __restrict__ T_total, double* loss_sum, float* __restrict__ g_ct, float sat_eps,
+                const uint8_t* __restrict__ state_in, uint8_t* __restrict__ state_out) {
+  __shared__ uint8_t s_use[SPLX_MAX_K];
+  __shared__ unsigned s_unsat[2];
+  __shared__ float s_loss[CB / 32];
+  const int tile = blockIdx.x, b = blockIdx.y;
+  if (SAT && threadIdx.x < 2) s_unsat[threadIdx.x] = 0u;
+  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
+  const int x = (tile % TX) * SPLX_TILE + (threadIdx.x & 15), y = (tile / TX) * SPLX_TILE + (threadIdx.x >> 4);
+  const size_t HW = (size_t)W * H;
+  const bool inside = x < W && y < H;
+  unsigned long long unsat = 0ull;
+  float lacc = 0.f;
+  if (inside) {
+    const size_t pix = (size_t)y * W + x;
+    float key[KMAX]; int idx[KMAX];
+    const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
+    float Tacc = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+    unsigned long long live = 0ull;
+    for (int m = 0; m < L; ++m) {
+      const float4 p = __ldg(reinterpret_cast<const float4*>(ct) + (size_t)idx[m] * HW + pix);
+      live |= 1ull << idx[m];
+      if (SAT && !(Tacc < sat_eps)) unsat |= 1ull << idx[m];
+      key[m] = Tacc;                                   // T in front of the m-th partial (the keys are spent)
+      C0 = fmaf(Tacc, p.x, C0); C1 = fmaf(Tacc, p.y, C1); C2 = fmaf(Tacc, p.z, C2);
+      Tacc *= p.w;
+    }
+    const float Ttot = Tacc;
+    const float i0 = fmaf(Ttot, bg0, C0), i1 = fmaf(Ttot, bg1, C1), i2 = fmaf(Ttot, bg2, C2);
+    float* im = image + 3 * ((size_t)b * HW + pix);
+    im[0] = i0; im[1] = i1; im[2] = i2;
+    if (T_total) T_total[(size_t)b * HW + pix] = Ttot;
+    if (SAT && !(Ttot < sat_eps)) unsat |= ~live;
+    // a7: mean L1 against the target of view b
+    const float* tg = target + 3 * ((size_t)b * HW + pix);
+    const float e0 = i0 - tg[0], e1 = i1 - tg[1], e2 = i2 - tg[2];
+    lacc = fabsf(e0) + fabsf(e1) + fabsf(e2);
+    const float g0 = e0 > 0.f ? gscale : (e0 < 0.f ? -gscale : 0.f);
+    const float g1 = e1 > 0.f ? gscale : (e1 < 0.f ? -gscale : 0.f);
+    const float g2 = e2 > 0.f ? gscale : (e2 < 0.f ? -gscale : 0.f);
+    // a8: identity partials stand behind all live ones
+    const float4 ge = make_float4(Ttot * g0, Ttot * g1, Ttot * g2, Ttot * (g0 * bg0 + g1 * bg1 + g2 * bg2));
+    for (int k = 0; k < K; ++k)
+      if (s_use[k] && !((live >> k) & 1ull)) reinterpret_cast<float4*>(g_ct)[(size_t)k * HW + pix] = ge;
+    float B0 = bg0, B1 = bg1, B2 = bg2;
+    for (int m = L - 1; m >= 0; --m) {
+      const float4 p = __ldg(reinterpret_cast<const float4*>(ct) + (size_t)idx[m] * HW + pix);
+      const float Tf = key[m];
+      reinterpret_cast<float4*>(g_ct)[(size_t)idx[m] * HW + pix] =
+          make_float4(Tf * g0, Tf * g1, Tf * g2, Tf * (g0 * B0 + g1 * B1 + g2 * B2));
+      B0 = fmaf(p.w, B0, p.x); B1 = fmaf(p.w, B1, p.y); B2 = fmaf(p.w, B2, p.z);
+    }
+  }
+  if (loss_sum) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) lacc += __shfl_xor_sync(0xffffffffu, lacc, o);
+    if ((threadIdx.x & 31) == 0) s_loss[threadIdx.x >> 5] = lacc;
+  }
+  if (SAT) {
+    const unsigned lo = __reduce_or_sync(0xffffffffu, (unsigned)unsat);
+    const unsigned hi = __reduce_or_sync(0xffffffffu, (unsigned)(unsat >> 32));
+    if ((threadIdx.x & 31) == 0) { if (lo) atomicOr(&s_unsat[0], lo); if (hi) atomicOr(&s_unsat[1], hi); }
+  }
+  __syncthreads();
+  if (loss_sum && threadIdx.x == 0) {
+    float t = 0.f;
+#pragma unroll
+    for (int w = 0; w < CB / 32; ++w) t += s_loss[w];
+    atomicAdd(loss_sum, (double)t);
+  }
+  if (SAT) {
+    for (int k = threadIdx.x; k < K; k += CB) {
+      if (pv.v[k] != b) continue;
+      const size_t slot = (size_t)k * ntiles + tile;
+      const uint8_t in = state_in ? state_in[slot] : (uint8_t)0;
+      const bool u = (s_unsat[k >> 5] >> (k & 31)) & 1u;
+      state_out[slot] = (uint8_t)((in & SPLX_TILE_INVISIBLE) | (u ? 0 : SPLX_TILE_SATURATED));
+    }
+  }
+}
+
 // mean-L1 gradient; float4-vectorised body with a scalar tail
 __global__ void __launch_bounds__(CB)
 k_l1(const float* __restrict__ image, const float* __restrict__ target, int64_t count, float gscale,
@@ -220,6 +310,35 @@ int launch_compose_bwd(splx_ctx* ctx, const splx_partial* p, const splx_binning*
   else if (plan.K <= 32) compose_bwd_k<32>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
   else compose_bwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
   SPLX_LAUNCH_CHECK(ctx, "k_compose_bwd");
+  return SPLX_OK;
+}
+
+template <int KMAX>
+static void compose_fused_k(splx_ctx* ctx, const splx_partial* p, const uint32_t* ranges, const PlanDev& plan, int sparse,
+                            const float* bg, const float* target, float gscale, float* image, float* T_total,
+                            double* loss_sum, float* g_ct, float sat_eps, uint8_t* state_out) {
+  dim3 grid(plan.ntiles, plan.B);
+  if (state_out)
+    k_compose_fused<KMAX, true><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
+                                                             plan.ntiles, sparse, bg[0], bg[1], bg[2], target, gscale, image,
+                                                             T_total, loss_sum, g_ct, sat_eps, plan.tile_state, state_out);
+  else
+    k_compose_fused<KMAX, false><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
+                                                              plan.ntiles, sparse, bg[0], bg[1], bg[2], target, gscale, image,
+                                                              T_total, loss_sum, g_ct, sat_eps, nullptr, nullptr);
+}
+
+int launch_compose_fused(splx_ctx* ctx, const splx_partial* p, const splx_binning* bins, const PlanDev& plan,
+                         const float* bg, const float* target, float scale, float* image, float* T_total,
+                         double* loss_sum, float* g_ct, float sat_eps, uint8_t* state_out) {
+  const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
+  const uint32_t* ranges = bins ? bins->tile_ranges : nullptr;
+  const float gscale = scale / (float)((int64_t)plan.B * plan.W * plan.H * 3);   // as splx_l1_loss_grad over B*H*W*3 values
+  if (plan.K <= 8) compose_fused_k<8>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
+  else if (plan.K <= 16) compose_fused_k<16>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
+  else if (plan.K <= 32) compose_fused_k<32>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
+  else compose_fused_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
+  SPLX_LAUNCH_CHECK(ctx, "k_compose_fused");
   return SPLX_OK;
 }
 

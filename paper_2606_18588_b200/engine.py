@@ -151,6 +151,35 @@ class Trainer:
                        sat_eps if sat_eps is not None else 0.0, tile_state_out)
         return images
 
+    def fused_buffers(self):
+        """g_ct [K,H,W,4] and g2d [n,12] of the fused path (g2d starts zeroed and is kept zero by
+        splx_project_backward's SPLX_PB_CLEAR_G2D)."""
+        if getattr(self, "_g_ct", None) is None:
+            dev = self.ctx.device
+            self._g_ct = torch.empty((self.K, self.H, self.W, 4), dtype=torch.float32, device=dev)
+            self._g2d = torch.zeros((max(self.n, 1), binding.G2D_STRIDE), dtype=torch.float32, device=dev)
+        return self._g_ct, self._g2d
+
+    def iteration_fused(self, plan: binding.Plan, targets, overwrite=True, sat_eps=None, tile_state_out=None):
+        """a1-a10 under a plan with composition, mean-L1 loss and composition backward in ONE kernel
+        (splx_compose_l1_backward_plan) -- the training path; the staged calls remain for stage-wise parity.
+        targets: device [B,H,W,3].  Returns images[B,H,W,3]."""
+        self._workspaces(plan.cams[0])
+        self._plan = plan
+        c = self.ctx
+        images, T_totals, _ = self._view_buffers(plan.B)
+        g_ct, g2d = self.fused_buffers()
+        c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
+        c.bin_sort_plan(self.proj, self.part_offsets, plan, self.bins, self._ws_sort)
+        c.render_partial_plan(self.proj, self.bins, plan, self.partials)
+        c.compose_l1_backward_plan(self.partials, self.bins, plan, self.bg, targets, images, T_totals, self.loss_sum, g_ct,
+                                   scale=float(plan.B), sat_eps=sat_eps if sat_eps is not None else 0.0,
+                                   tile_state_out=tile_state_out)
+        c.raster_backward_plan(self.proj, self.bins, plan, self.partials, g_ct, g2d)
+        c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                clear_g2d=True, overwrite=overwrite)
+        return images
+
     def loss_grad_plan(self, targets):
         """a7 for B views at once: targets[B,H,W,3]; every view's loss is its own mean (scale = B)."""
         B = self._plan.B
@@ -220,10 +249,8 @@ class Trainer:
         groups = self.buckets(view_ids, cams, consolidate)
         for gi, grp in enumerate(groups):
             plan, state_out = self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse)
-            self.forward_plan(plan, sat_eps, state_out)
             tg = targets[grp[0]:grp[0] + 1] if len(grp) == 1 else targets[torch.as_tensor(grp, device=targets.device)]
-            self.loss_grad_plan(tg)
-            self.backward_plan(overwrite=(gi == 0))
+            self.iteration_fused(plan, tg, overwrite=(gi == 0), sat_eps=sat_eps, tile_state_out=state_out)
         self.adam_step(len(view_ids))
         return len(groups)
 
@@ -236,14 +263,24 @@ class Trainer:
             self._target_dev[0].copy_(target_host, non_blocking=True)
             self._ev_target.record(side)
         self.loss_sum.zero_()
-        images = self.forward_plan(plan, sat_eps, state)
+        self._workspaces(plan.cams[0])
+        self._plan = plan
+        c = self.ctx
+        images, T_totals, _ = self._view_buffers(1)
+        g_ct, g2d = self.fused_buffers()
+        c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
+        c.bin_sort_plan(self.proj, self.part_offsets, plan, self.bins, self._ws_sort)
+        c.render_partial_plan(self.proj, self.bins, plan, self.partials)
+        main.wait_event(self._ev_target)            # the target is first needed by the fused composition + loss
+        c.compose_l1_backward_plan(self.partials, self.bins, plan, self.bg, self._target_dev, images, T_totals,
+                                   self.loss_sum, g_ct, scale=1.0, sat_eps=sat_eps, tile_state_out=state)
         if image_host is not None:
             side.wait_stream(main)
             with torch.cuda.stream(side):
                 image_host.copy_(images[0], non_blocking=True)
-        main.wait_event(self._ev_target)
-        self.loss_grad_plan(self._target_dev)
-        self.backward_plan(overwrite=True)
+        c.raster_backward_plan(self.proj, self.bins, plan, self.partials, g_ct, g2d)
+        c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                clear_g2d=True, overwrite=True)
         main.wait_stream(side)
         if loss_host is not None:    # after the image has left: the two copies share one device-to-host engine, and
             loss_host.copy_(self.loss_sum, non_blocking=True)   # 8 bytes queued behind 25 MB would stall this stream
@@ -274,6 +311,7 @@ class Trainer:
                                else (self.make_plan([cam]), None))
                 self._workspaces(cam)
                 self._view_buffers(1)
+                self.fused_buffers()
                 torch.cuda.synchronize(dev)
                 g = torch.cuda.CUDAGraph()
                 old = main.cuda_stream
@@ -301,6 +339,7 @@ class Trainer:
                            else (self.make_plan([cam]), None))
             self._workspaces(cam)
             self._view_buffers(1)
+            self.fused_buffers()
             main = torch.cuda.current_stream(dev)
             torch.cuda.synchronize(dev)
             g = torch.cuda.CUDAGraph()
@@ -308,9 +347,7 @@ class Trainer:
                 self.ctx.set_stream(torch.cuda.current_stream(dev).cuda_stream)
                 try:
                     self.loss_sum.zero_()
-                    self.forward_plan(plan, sat_eps, state)
-                    self.loss_grad_plan(target_dev)
-                    self.backward_plan(overwrite=True)
+                    self.iteration_fused(plan, target_dev, overwrite=True, sat_eps=sat_eps, tile_state_out=state)
                 finally:
                     self.ctx.set_stream(main.cuda_stream)
             self._dgraphs[key] = (g, plan)
