@@ -303,6 +303,25 @@ int splx_raster_backward_plan(splx_ctx *ctx, const splx_projected *proj, const s
 int splx_project_backward_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                                const splx_plan *plan, int sh_degree, const splx_projected *proj,
                                float *g2d, int flags, const splx_gaussian_grads *grads);
+/* a10 + a11 fused: the LAST projection backward of an iteration also takes the Adam step of splx_adam on every
+ * row of every partition (participating or not), reading the gradient it has just formed -- plus, without
+ * SPLX_PB_OVERWRITE, the gradient earlier launches of the iteration left in `grads` -- instead of storing it:
+ * `grads` is only read (never written), Adam never re-reads it.  params / m / v: the parameter set (updated in
+ * place: the const of splx_gaussians does not apply here), first and second moments, same SoA layout as
+ * splx_gaussian_grads.  lr: HOST float[5] for mean, log_scale, quat, opacity_logit, sh.  bias_corr: DEVICE
+ * float[2] = 1/(1-beta1^t), 1/(1-beta2^t) (on the device so that a captured CUDA graph can be replayed with
+ * the next step's values).  Elementwise the arithmetic of splx_project_backward_plan followed by splx_adam
+ * with grad_scale. */
+int splx_project_backward_adam_plan(splx_ctx *ctx, const splx_gaussian_grads *params, int K,
+                                    const int64_t *part_offsets, const splx_plan *plan, int sh_degree,
+                                    const splx_projected *proj, float *g2d, int flags,
+                                    const splx_gaussian_grads *grads, const splx_gaussian_grads *m,
+                                    const splx_gaussian_grads *v, const float lr[5], float beta1, float beta2,
+                                    float eps, const float *bias_corr, float grad_scale);
+/* Advance the DEVICE-resident Adam step counter (*step_dev += 1, a device int32 the caller zero-initialises) and
+ * write bias_corr (device float[2]) = 1/(1-beta1^t), 1/(1-beta2^t) for the new t: the producer of
+ * splx_project_backward_adam_plan's bias_corr that can live inside a captured CUDA graph. */
+int splx_adam_bias_step(splx_ctx *ctx, float beta1, float beta2, int32_t *step_dev, float *bias_corr);
 int splx_backward_plan(splx_ctx *ctx, int K, const int64_t *part_offsets, const splx_plan *plan,
                        const splx_partial *partials, const float bg[3], const float *dL_dimage,
                        const float *dL_dT_total, const splx_gaussians *g, const splx_projected *proj,

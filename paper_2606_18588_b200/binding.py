@@ -32,7 +32,7 @@ EXPORTS = [
     "splx_visible_regions", "splx_schedule_views", "splx_project_plan", "splx_bin_sort_plan",
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
-    "splx_compose_l1_backward_plan",
+    "splx_compose_l1_backward_plan", "splx_project_backward_adam_plan", "splx_adam_bias_step",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -138,6 +138,9 @@ def lib():
         L.splx_project_backward_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp]
         L.splx_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp, vp,
                                          C.c_size_t, C.c_int]
+        L.splx_project_backward_adam_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp,
+                                                      C.c_float, C.c_float, C.c_float, vp, C.c_float]
+        L.splx_adam_bias_step.argtypes = [vp, C.c_float, C.c_float, vp, vp]
         _lib = L
     return _lib
 
@@ -453,6 +456,22 @@ class Context:
         flags = (PB_CLEAR_G2D if clear_g2d else 0) | (PB_OVERWRITE if overwrite else 0)
         self._check(lib().splx_project_backward_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
                                                      sh_degree, C.byref(ps), _ptr(g2d), flags, C.byref(gg)))
+
+    def project_backward_adam_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
+                                   grads: dict, m: dict, v: dict, lrs, bias_corr, beta1=0.9, beta2=0.999, eps=1e-15,
+                                   grad_scale=1.0, clear_g2d=False, overwrite=False):
+        """lrs: five learning rates in PARAM order (mean, log_scale, quat, opacity_logit, sh); bias_corr: device float[2]."""
+        sets = [gaussians_struct(x) for x in (params, grads, m, v)]
+        ps = proj.struct()
+        lr = (C.c_float * 5)(*[float(x) for x in lrs])
+        flags = (PB_CLEAR_G2D if clear_g2d else 0) | (PB_OVERWRITE if overwrite else 0)
+        self._check(lib().splx_project_backward_adam_plan(
+            self._h, C.byref(sets[0]), plan.K, self._offs(part_offsets), plan.ref(), sh_degree, C.byref(ps), _ptr(g2d),
+            flags, C.byref(sets[1]), C.byref(sets[2]), C.byref(sets[3]), lr, beta1, beta2, eps, _ptr(bias_corr),
+            float(grad_scale)))
+
+    def adam_bias_step(self, step_dev, bias_corr, beta1=0.9, beta2=0.999):
+        self._check(lib().splx_adam_bias_step(self._h, beta1, beta2, _ptr(step_dev), _ptr(bias_corr)))
 
     def backward_plan(self, part_offsets, plan: Plan, partials: Partial, bg, g_image, g_T_total, params: dict,
                       proj: Projected, bins: Binning, sh_degree, grads: dict, ws: torch.Tensor, overwrite=False):

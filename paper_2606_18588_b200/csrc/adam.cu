@@ -73,7 +73,23 @@ k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __rest
   }
 }
 
+// Device-resident step counter of the fused optimiser path: t = ++(*step); bc = 1/(1-b1^t), 1/(1-b2^t) formed in
+// double as launch_adam does on the host.  One thread; lives inside captured CUDA graphs, where a host-side step
+// number would be frozen at capture time.
+__global__ void k_adam_bias_step(int32_t* step, float* bc, double b1, double b2) {
+  const int t = *step + 1;
+  *step = t;
+  bc[0] = (float)(1.0 / (1.0 - pow(b1, (double)t)));
+  bc[1] = (float)(1.0 / (1.0 - pow(b2, (double)t)));
+}
+
 }  // namespace
+
+int launch_adam_bias_step(splx_ctx* ctx, float beta1, float beta2, int32_t* step_dev, float* bias_corr) {
+  k_adam_bias_step<<<1, 1, 0, ctx->stream>>>(step_dev, bias_corr, (double)beta1, (double)beta2);
+  SPLX_LAUNCH_CHECK(ctx, "k_adam_bias_step");
+  return SPLX_OK;
+}
 
 int launch_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int n_groups,
                        const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,

@@ -306,7 +306,41 @@ int splx_project_backward_plan(splx_ctx* ctx, const splx_gaussians* g, int K, co
   int rc;
   if ((rc = make_plan(ctx, "splx_project_backward", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: part_offsets must run monotonically from 0 to n");
-  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads);
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr);
+}
+
+int splx_project_backward_adam_plan(splx_ctx* ctx, const splx_gaussian_grads* params, int K, const int64_t* part_offsets,
+                                    const splx_plan* plan, int sh_degree, const splx_projected* proj, float* g2d, int flags,
+                                    const splx_gaussian_grads* grads, const splx_gaussian_grads* m,
+                                    const splx_gaussian_grads* v, const float lr[5], float beta1, float beta2, float eps,
+                                    const float* bias_corr, float grad_scale) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!params || !grads || !m || !v || !lr || !bias_corr || !proj_ok(proj) || !g2d || !aligned16(g2d))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: null/misaligned argument");
+  const splx_gaussian_grads* sets[4] = {params, grads, m, v};
+  for (const splx_gaussian_grads* s : sets) {
+    if (s->n != params->n || (s->n > 0 && (!s->mean || !s->log_scale || !s->quat || !s->opacity_logit || !s->sh ||
+                                           !aligned16(s->mean) || !aligned16(s->log_scale) || !aligned16(s->quat) ||
+                                           !aligned16(s->opacity_logit) || !aligned16(s->sh))))
+      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: params, grads, m, v must be four aligned sets of n rows");
+  }
+  if (params->n == 0) return SPLX_OK;
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: sh_degree %d not in [0,3]", sh_degree);
+  if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: unknown flags %d", flags);
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_project_backward_adam", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, params->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: part_offsets must run monotonically from 0 to n");
+  AdamFuse af;
+  af.p[0] = params->mean; af.p[1] = params->log_scale; af.p[2] = params->quat; af.p[3] = params->opacity_logit; af.p[4] = params->sh;
+  af.m[0] = m->mean; af.m[1] = m->log_scale; af.m[2] = m->quat; af.m[3] = m->opacity_logit; af.m[4] = m->sh;
+  af.v[0] = v->mean; af.v[1] = v->log_scale; af.v[2] = v->quat; af.v[3] = v->opacity_logit; af.v[4] = v->sh;
+  for (int j = 0; j < 5; ++j) af.lr[j] = lr[j];
+  af.b1 = beta1; af.b2 = beta2;
+  af.omb1 = (float)(1.0 - (double)beta1); af.omb2 = (float)(1.0 - (double)beta2);   // as splx_adam forms them
+  af.eps = eps; af.gscale = grad_scale; af.bc = bias_corr;
+  const splx_gaussians g{params->mean, params->log_scale, params->quat, params->opacity_logit, params->sh, params->n};
+  return launch_project_bwd(ctx, &g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, &af);
 }
 
 int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
@@ -365,6 +399,13 @@ int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx
   for (int k = 1; k <= K; ++k) po[k] = g->n;
   return splx_backward_plan(ctx, K, po, &sp.plan, partials, bg, dL_dimage, dL_dT_total, g, proj, bins, sh_degree, grads,
                             ws, ws_bytes, flags);
+}
+
+int splx_adam_bias_step(splx_ctx* ctx, float beta1, float beta2, int32_t* step_dev, float* bias_corr) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!step_dev || !bias_corr || !(beta1 >= 0.f && beta1 < 1.f) || !(beta2 >= 0.f && beta2 < 1.f))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_bias_step: null pointer or beta not in [0,1)");
+  return launch_adam_bias_step(ctx, beta1, beta2, step_dev, bias_corr);
 }
 
 int splx_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr, float beta1,

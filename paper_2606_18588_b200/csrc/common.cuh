@@ -125,11 +125,20 @@ __device__ __forceinline__ void tile_rect(float u, float v, int radius, int TX, 
   y1 = !(y1f > 0.0f) ? 0 : (y1f >= (float)TY ? TY : (int)y1f);
 }
 
+// Optional optimiser fusion of the projection backward (splx_project_backward_adam_plan).
+struct AdamFuse {
+  float *p[5], *m[5], *v[5];          // mean, log_scale, quat, opacity_logit, sh
+  float lr[5];
+  float b1, b2, omb1, omb2, eps, gscale;
+  const float* bc;                    // device float[2]: 1/(1-b1^t), 1/(1-b2^t)
+};
+
+
 // ---- stage launchers (defined one per .cu file, called from api.cu) ----------------------
 int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
-                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*);
+                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*, const AdamFuse* adam);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
 int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, const PlanDev&, const int64_t* part_offsets,
                     const splx_binning*, void* ws, size_t ws_bytes);
@@ -149,5 +158,6 @@ int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count,
 int launch_adam_groups(splx_ctx*, float* param, float* grad, float* m, float* v, int n_groups,
                        const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
                        float grad_scale, int zero_grad);
+int launch_adam_bias_step(splx_ctx*, float beta1, float beta2, int32_t* step_dev, float* bias_corr);
 int launch_adam(splx_ctx*, float* param, float* grad, float* m, float* v, int64_t count, float lr,
                 float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad);

@@ -246,10 +246,37 @@ __device__ __forceinline__ void cp_async_wait_all() {
   asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
 }
 
-template <int DEG, bool ACC>
+// Optional optimiser fusion (splx_project_backward_adam_plan): the LAST projection backward of an iteration
+// applies Adam to every row it owns straight from the gradient it has just formed (plus, when accumulating, the
+// gradient the earlier views left in memory), so the gradient is never written and Adam never re-reads it:
+// 24 B per parameter (28 accumulating) instead of 8 + 28.  Same statements as adam.cu's adam1.
+__device__ __forceinline__ void adam_step1(float& p, float g, float& m, float& v, const AdamFuse& a, float lr, float ibc1,
+                                           float ibc2) {
+  m = fmaf(a.b1, m, a.omb1 * g);
+  v = fmaf(a.b2, v, a.omb2 * g * g);
+  p -= lr * (m * ibc1) / (sqrtf(v * ibc2) + a.eps);
+}
+__device__ __forceinline__ void adam_vec4(float* pp, float* pm, float* pv, float4 g, const AdamFuse& a, float lr, float ibc1,
+                                          float ibc2) {
+  float4 p = *reinterpret_cast<float4*>(pp), m = *reinterpret_cast<float4*>(pm), v = *reinterpret_cast<float4*>(pv);
+  adam_step1(p.x, g.x * a.gscale, m.x, v.x, a, lr, ibc1, ibc2);
+  adam_step1(p.y, g.y * a.gscale, m.y, v.y, a, lr, ibc1, ibc2);
+  adam_step1(p.z, g.z * a.gscale, m.z, v.z, a, lr, ibc1, ibc2);
+  adam_step1(p.w, g.w * a.gscale, m.w, v.w, a, lr, ibc1, ibc2);
+  *reinterpret_cast<float4*>(pp) = p; *reinterpret_cast<float4*>(pm) = m; *reinterpret_cast<float4*>(pv) = v;
+}
+__device__ __forceinline__ void adam_scalar(float* pp, float* pm, float* pv, float g, const AdamFuse& a, float lr, float ibc1,
+                                            float ibc2) {
+  float p = *pp, m = *pm, v = *pv;
+  adam_step1(p, g * a.gscale, m, v, a, lr, ibc1, ibc2);
+  *pp = p; *pm = m; *pv = v;
+}
+
+template <int DEG, bool ACC, bool ADAM>
 __global__ void __launch_bounds__(PB_THREADS)
 k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
-              splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out) {
+              splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out,
+              const __grid_constant__ AdamFuse af) {
   extern __shared__ __align__(16) float s_dyn[];
   float* s_sh = s_dyn;                                   // [128][52] sh in, SH gradient out
   float* s_old = s_dyn + PB_THREADS * PB_STRIDE;         // [128][52] previous SH gradient (ACC only)
@@ -419,9 +446,17 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   }
 #pragma unroll
   for (int k = 0; k < 3; ++k) { s_m[3 * threadIdx.x + k] = dmu[k]; s_s[3 * threadIdx.x + k] = dls[k]; }
+  float ibc1 = 0.f, ibc2 = 0.f;
+  if (ADAM) { ibc1 = af.bc[0]; ibc2 = af.bc[1]; }
   if (i < run_end) {
     float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
-    if (ACC) {
+    if (ADAM) {
+      float4 gq = dq;                     // zeros for a culled row
+      float gl = dlogit;
+      if (ACC) { const float4 cur = *oq; gq.x += cur.x; gq.y += cur.y; gq.z += cur.z; gq.w += cur.w; gl += out.opacity_logit[i]; }
+      adam_vec4(af.p[2] + 4 * i, af.m[2] + 4 * i, af.v[2] + 4 * i, gq, af, af.lr[2], ibc1, ibc2);
+      adam_scalar(af.p[3] + i, af.m[3] + i, af.v[3] + i, gl, af, af.lr[3], ibc1, ibc2);
+    } else if (ACC) {
       if (vis) {
         float4 cur = *oq;
         cur.x += dq.x; cur.y += dq.y; cur.z += dq.z; cur.w += dq.w;
@@ -434,7 +469,51 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     }
   }
   __syncthreads();
-  // coalesced write-back of the SH-gradient tile (+= needs visible rows only; = writes every row)
+  // coalesced write-back of the SH-gradient tile (+= needs visible rows only; = writes every row; with ADAM the
+  // gradient is consumed here instead: every row of the tile takes its optimiser step)
+  if (ADAM) {
+    // four chunks at a time: all of their parameter / moment (/ old gradient) loads are requested before the first
+    // store, because the compiler cannot move a load above a store that may alias it -- 12-16 independent 16-byte
+    // loads per thread keep enough bytes in flight for this low-occupancy kernel to stream
+#pragma unroll
+    for (int c0 = 0; c0 < 12; c0 += 4) {
+      float4 P[4], M[4], V[4], Gr[4];
+      int64_t off[4];
+      bool ok[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int q = (c0 + u) * PB_THREADS + threadIdx.x;
+        const int row = q / 12, c4 = q - row * 12;
+        ok[u] = row < nrows;
+        off[u] = 48 * (base + row) + 4 * c4;
+        Gr[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok[u]) {
+          const bool live = s_vis[row] && c4 < NV;
+          P[u] = *reinterpret_cast<const float4*>(af.p[4] + off[u]);
+          M[u] = *reinterpret_cast<const float4*>(af.m[4] + off[u]);
+          V[u] = *reinterpret_cast<const float4*>(af.v[4] + off[u]);
+          if (live) Gr[u] = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
+          if (ACC) {
+            const float4 o = live ? *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4)
+                                  : *reinterpret_cast<const float4*>(out.sh + off[u]);
+            Gr[u].x += o.x; Gr[u].y += o.y; Gr[u].z += o.z; Gr[u].w += o.w;
+          }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (ok[u]) {
+          adam_step1(P[u].x, Gr[u].x * af.gscale, M[u].x, V[u].x, af, af.lr[4], ibc1, ibc2);
+          adam_step1(P[u].y, Gr[u].y * af.gscale, M[u].y, V[u].y, af, af.lr[4], ibc1, ibc2);
+          adam_step1(P[u].z, Gr[u].z * af.gscale, M[u].z, V[u].z, af, af.lr[4], ibc1, ibc2);
+          adam_step1(P[u].w, Gr[u].w * af.gscale, M[u].w, V[u].w, af, af.lr[4], ibc1, ibc2);
+          *reinterpret_cast<float4*>(af.p[4] + off[u]) = P[u];
+          *reinterpret_cast<float4*>(af.m[4] + off[u]) = M[u];
+          *reinterpret_cast<float4*>(af.v[4] + off[u]) = V[u];
+        }
+      }
+    }
+  } else {
 #pragma unroll
   for (int c = 0; c < 12; ++c) {
     const int q = c * PB_THREADS + threadIdx.x;
@@ -453,6 +532,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       }
     }
   }
+  }
   // mean / log_scale gradient tiles: 96 float4 each; a partial last block, or a run that does not start
   // on a multiple of 4 Gaussians (12-byte rows: 16-byte alignment needs base % 4 == 0), falls back to scalars
   if (nrows == PB_THREADS && (base & 3) == 0) {
@@ -465,25 +545,47 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
         a.x += om.x; a.y += om.y; a.z += om.z; a.w += om.w;
         b.x += os.x; b.y += os.y; b.z += os.z; b.w += os.w;
       }
-      *dm = a; *ds = b;
+      if (ADAM) {
+        const int64_t off = 3 * base + 4 * threadIdx.x;
+        adam_vec4(af.p[0] + off, af.m[0] + off, af.v[0] + off, a, af, af.lr[0], ibc1, ibc2);
+        adam_vec4(af.p[1] + off, af.m[1] + off, af.v[1] + off, b, af, af.lr[1], ibc1, ibc2);
+      } else {
+        *dm = a; *ds = b;
+      }
     }
   } else if (i < run_end) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      if (ACC) { out.mean[3 * i + k] += dmu[k]; out.log_scale[3 * i + k] += dls[k]; }
+      if (ADAM) {
+        const float gm = dmu[k] + (ACC ? out.mean[3 * i + k] : 0.f), gs = dls[k] + (ACC ? out.log_scale[3 * i + k] : 0.f);
+        adam_scalar(af.p[0] + 3 * i + k, af.m[0] + 3 * i + k, af.v[0] + 3 * i + k, gm, af, af.lr[0], ibc1, ibc2);
+        adam_scalar(af.p[1] + 3 * i + k, af.m[1] + 3 * i + k, af.v[1] + 3 * i + k, gs, af, af.lr[1], ibc1, ibc2);
+      } else if (ACC) { out.mean[3 * i + k] += dmu[k]; out.log_scale[3 * i + k] += dls[k]; }
       else     { out.mean[3 * i + k] = dmu[k]; out.log_scale[3 * i + k] = dls[k]; }
     }
   }
 }
 
-template <int DEG, bool ACC>
+template <int DEG, bool ACC, bool ADAM>
 static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
-                      const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads) {
+                      const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
+                      const AdamFuse& af) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  k_project_bwd<DEG, ACC><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(*g, plan, rt, ctx->cfg, *pr, g2d,
-                                                                                      clear_g2d, *grads);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  k_project_bwd<DEG, ACC, ADAM><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(*g, plan, rt, ctx->cfg, *pr, g2d,
+                                                                                            clear_g2d, *grads, af);
+}
+
+template <bool ACC, bool ADAM>
+static void launch_pb_deg(splx_ctx* ctx, int deg, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
+                          const splx_projected* pr, float* g2d, int clr, const splx_gaussian_grads* grads, const AdamFuse& af) {
+  switch (deg) {
+    case 0: launch_pb<0, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
+    case 1: launch_pb<1, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
+    case 2: launch_pb<2, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
+    default: launch_pb<3, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
+  }
 }
 
 }  // namespace
@@ -504,26 +606,22 @@ int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pl
 }
 
 int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
-                       const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads) {
+                       const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads,
+                       const AdamFuse* adam) {
   const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
   const bool overwrite = (flags & SPLX_PB_OVERWRITE) != 0;
-  // "=" must also clear the rows of partitions that do not participate in this launch
-  const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, overwrite);
+  // "=" must also clear the rows of partitions that do not participate in this launch; the fused optimiser
+  // step must reach every row of every partition
+  const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, overwrite || adam != nullptr);
   if (rt.blocks_total == 0) return SPLX_OK;
-  if (overwrite) {
-    switch (deg) {
-      case 0: launch_pb<0, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-      case 1: launch_pb<1, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-      case 2: launch_pb<2, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-      default: launch_pb<3, false>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-    }
+  AdamFuse none;
+  memset(&none, 0, sizeof none);
+  if (adam) {
+    if (overwrite) launch_pb_deg<false, true>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, *adam);
+    else launch_pb_deg<true, true>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, *adam);
   } else {
-    switch (deg) {
-      case 0: launch_pb<0, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-      case 1: launch_pb<1, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-      case 2: launch_pb<2, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-      default: launch_pb<3, true>(ctx, g, plan, rt, pr, g2d, clr, grads); break;
-    }
+    if (overwrite) launch_pb_deg<false, false>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, none);
+    else launch_pb_deg<true, false>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, none);
   }
   SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
   return SPLX_OK;

@@ -60,6 +60,10 @@ class Trainer:
         self.loss_sum = torch.zeros(1, dtype=torch.float64, device=dev)
         self.pairs = torch.zeros(4, dtype=torch.int64, device=dev)
         self.step_count = 0
+        #: fuse the Adam step into the last projection backward (splx_project_backward_adam_plan).  Off by default:
+        #: at 4 CTAs/SM (124 registers) the fused kernel streams the moments at ~4 TB/s, while the stand-alone Adam
+        #: kernel runs at 95 % of the HBM roof -- measured 0.44 ms fused against 0.11 + 0.27 ms
+        self.fuse_adam = False
         self._cam = None
         self._aabb = None
         self._side = None
@@ -160,7 +164,18 @@ class Trainer:
             self._g2d = torch.zeros((max(self.n, 1), binding.G2D_STRIDE), dtype=torch.float32, device=dev)
         return self._g_ct, self._g2d
 
-    def iteration_fused(self, plan: binding.Plan, targets, overwrite=True, sat_eps=None, tile_state_out=None):
+    def prepare_adam(self):
+        """Host side of the fused optimiser step: count the step.  The bias corrections themselves come from the
+        DEVICE-resident counter (splx_adam_bias_step, launched by iteration_fused(adam=True)), so that a captured graph
+        advances them at every replay and no host value is read by work that is still in flight."""
+        if getattr(self, "_bc_dev", None) is None:
+            dev = self.ctx.device
+            self._bc_dev = torch.empty(2, dtype=torch.float32, device=dev)
+            self._step_dev = torch.full((1,), self.step_count, dtype=torch.int32, device=dev)
+        self.step_count += 1
+
+    def iteration_fused(self, plan: binding.Plan, targets, overwrite=True, sat_eps=None, tile_state_out=None, adam=False,
+                        n_views=1):
         """a1-a10 under a plan with composition, mean-L1 loss and composition backward in ONE kernel
         (splx_compose_l1_backward_plan) -- the training path; the staged calls remain for stage-wise parity.
         targets: device [B,H,W,3].  Returns images[B,H,W,3]."""
@@ -176,8 +191,14 @@ class Trainer:
                                    scale=float(plan.B), sat_eps=sat_eps if sat_eps is not None else 0.0,
                                    tile_state_out=tile_state_out)
         c.raster_backward_plan(self.proj, self.bins, plan, self.partials, g_ct, g2d)
-        c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                clear_g2d=True, overwrite=overwrite)
+        if adam:     # the last backward of the iteration takes the optimiser step too (call prepare_adam() first)
+            c.adam_bias_step(self._step_dev, self._bc_dev)
+            c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                         self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev,
+                                         grad_scale=1.0 / n_views, clear_g2d=True, overwrite=overwrite)
+        else:
+            c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                    clear_g2d=True, overwrite=overwrite)
         return images
 
     def loss_grad_plan(self, targets):
@@ -247,11 +268,15 @@ class Trainer:
         consolidated into one launch per stage.  targets: device tensor [B,H,W,3].  Returns the number of launches
         of the forward (= buckets)."""
         groups = self.buckets(view_ids, cams, consolidate)
+        if self.fuse_adam:
+            self.prepare_adam()
         for gi, grp in enumerate(groups):
             plan, state_out = self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse)
             tg = targets[grp[0]:grp[0] + 1] if len(grp) == 1 else targets[torch.as_tensor(grp, device=targets.device)]
-            self.iteration_fused(plan, tg, overwrite=(gi == 0), sat_eps=sat_eps, tile_state_out=state_out)
-        self.adam_step(len(view_ids))
+            self.iteration_fused(plan, tg, overwrite=(gi == 0), sat_eps=sat_eps, tile_state_out=state_out,
+                                 adam=(self.fuse_adam and gi == len(groups) - 1), n_views=len(view_ids))
+        if not self.fuse_adam:
+            self.adam_step(len(view_ids))
         return len(groups)
 
     # ---- end to end from HOST buffers ---------------------------------------------------------------
@@ -279,8 +304,14 @@ class Trainer:
             with torch.cuda.stream(side):
                 image_host.copy_(images[0], non_blocking=True)
         c.raster_backward_plan(self.proj, self.bins, plan, self.partials, g_ct, g2d)
-        c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                clear_g2d=True, overwrite=True)
+        if self.fuse_adam:
+            c.adam_bias_step(self._step_dev, self._bc_dev)
+            c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                         self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev, grad_scale=1.0,
+                                         clear_g2d=True, overwrite=True)
+        else:
+            c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                    clear_g2d=True, overwrite=True)
         main.wait_stream(side)
         if loss_host is not None:    # after the image has left: the two copies share one device-to-host engine, and
             loss_host.copy_(self.loss_sum, non_blocking=True)   # 8 bytes queued behind 25 MB would stall this stream
@@ -290,10 +321,13 @@ class Trainer:
         """One whole training iteration (a1-a11) on one view whose target image lives in pinned HOST memory; the
         rendered image and the loss go back to pinned host memory.  With graph=True the launches of a1-a10 and the
         copies are captured once per (view, buffers) into a CUDA graph and replayed (one launch per step instead of
-        ~25); Adam stays outside the graph because its bias correction depends on the step number.  Returns after
-        the device has drained, so the host buffers are valid."""
+        ~20); the Adam step is fused into the projection backward, its bias corrections travel through a pinned
+        host pair that the graph's copy node reads at replay time.  Returns after the device has drained, so the host
+        buffers are valid."""
         dev = self.ctx.device
         main = torch.cuda.current_stream(dev)
+        if self.fuse_adam:
+            self.prepare_adam()
         if self._side is None:
             self._side = torch.cuda.Stream(dev)
             self._ev_target = torch.cuda.Event()
@@ -305,7 +339,7 @@ class Trainer:
             self._host_body(main, self._side, plan, state, target_host, image_host, loss_host, sat_eps)
         else:
             key = (view_id, target_host.data_ptr(), image_host.data_ptr() if image_host is not None else 0,
-                   loss_host.data_ptr() if loss_host is not None else 0, bool(saturation), float(sat_eps))
+                   loss_host.data_ptr() if loss_host is not None else 0, bool(saturation), float(sat_eps), self.fuse_adam)
             if key not in self._graphs:
                 plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
                                else (self.make_plan([cam]), None))
@@ -324,16 +358,19 @@ class Trainer:
                         self.ctx.set_stream(old)
                 self._graphs[key] = (g, plan)          # the plan owns the host arrays the capture read
             self._graphs[key][0].replay()
-        self.adam_step(1)
+        if not self.fuse_adam:
+            self.adam_step(1)        # outside the graph: its bias correction is a launch argument
         main.synchronize()
 
     def step_graph(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
         """One whole training iteration on one view with the target already on the device ([1,H,W,3]): a1-a10
         replayed from a CUDA graph captured at the first call for this (view, target), then Adam.  Asynchronous."""
         dev = self.ctx.device
+        if self.fuse_adam:
+            self.prepare_adam()           # this step's bias corrections (the captured copy node reads them at replay)
         if getattr(self, "_dgraphs", None) is None:
             self._dgraphs = {}
-        key = (view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps))
+        key = (view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps), self.fuse_adam)
         if key not in self._dgraphs:
             plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
                            else (self.make_plan([cam]), None))
@@ -347,9 +384,11 @@ class Trainer:
                 self.ctx.set_stream(torch.cuda.current_stream(dev).cuda_stream)
                 try:
                     self.loss_sum.zero_()
-                    self.iteration_fused(plan, target_dev, overwrite=True, sat_eps=sat_eps, tile_state_out=state)
+                    self.iteration_fused(plan, target_dev, overwrite=True, sat_eps=sat_eps, tile_state_out=state,
+                                         adam=self.fuse_adam)
                 finally:
                     self.ctx.set_stream(main.cuda_stream)
             self._dgraphs[key] = (g, plan)
         self._dgraphs[key][0].replay()
-        self.adam_step(1)
+        if not self.fuse_adam:
+            self.adam_step(1)            # outside the graph: its bias correction is a launch argument

@@ -338,3 +338,65 @@ def test_fused_compose_loss_backward_equals_the_staged_calls(blocks):
     assert torch.equal(st_a, st_b)
     assert float(tr.loss_sum.item()) == pytest.approx(loss_a, rel=1e-6)
     assert g_ct_a.abs().max() > 0
+
+
+def test_fused_projection_backward_adam_equals_the_two_calls(blocks):
+    """splx_project_backward_adam_plan (a10 + a11 in one kernel) against splx_project_backward_plan followed by
+    splx_adam_groups: parameters and moments bit-equal, in '=' mode and in '+=' mode, non-participants included."""
+    sc = blocks
+    cam = sc.cameras[1]
+    rng = np.random.default_rng(41)
+    for overwrite in (True, False):
+        a, b = _trainer(sc), _trainer(sc)
+        part = a.participants(1, cam)
+        vop = [0 if (part >> k) & 1 else -1 for k in range(sc.K)]
+        g2d = np.zeros((a.n, 12), np.float32)
+        g2d[:, :9] = rng.standard_normal((a.n, 9))
+        old = rng.standard_normal(a.flat["grad"].shape).astype(np.float32) * 0.1
+        m0 = rng.standard_normal(a.flat["m"].shape).astype(np.float32) * 0.01
+        v0 = np.abs(rng.standard_normal(a.flat["v"].shape)).astype(np.float32) * 1e-4
+        for tr in (a, b):
+            plan = tr.make_plan([cam], vop, None, True)
+            tr._workspaces(cam)
+            tr.ctx.project_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj)
+            tr.flat["grad"].copy_(torch.from_numpy(old)); tr.flat["m"].copy_(torch.from_numpy(m0)); tr.flat["v"].copy_(torch.from_numpy(v0))
+            tr._plan = plan
+        # a: two calls
+        a.ctx.project_backward_plan(a.params, a.part_offsets, a._plan, a.sh_degree, a.proj, torch.from_numpy(g2d).cuda(),
+                                    a.grads, clear_g2d=True, overwrite=overwrite)
+        a.adam_step(n_views=2)
+        # b: fused
+        b.prepare_adam()
+        b.ctx.adam_bias_step(b._step_dev, b._bc_dev)       # device counter 0 -> 1, bias corrections of step 1
+        b.ctx.project_backward_adam_plan(b.params, b.part_offsets, b._plan, b.sh_degree, b.proj, torch.from_numpy(g2d).cuda(),
+                                         b.grads, b.m, b.v, [b.lr[k] for k in scenes.PARAM_KEYS], b._bc_dev,
+                                         grad_scale=0.5, clear_g2d=True, overwrite=overwrite)
+        torch.cuda.synchronize()
+        for name in ("param", "m", "v"):
+            x, y = a.flat[name], b.flat[name]
+            assert torch.equal(x, y), (overwrite, name, float((x - y).abs().max()))
+        assert not torch.equal(a.flat["param"], torch.from_numpy(np.zeros(1, np.float32)).cuda().expand_as(a.flat["param"]))
+
+
+def test_training_paths_agree_with_and_without_the_fused_optimiser(aerial):
+    """Three steps of Trainer.step_graph with fuse_adam on / off (CUDA-graph replays; the fused variant reads its
+    bias corrections from the pinned pair at replay time) and of the plain stage calls land on the same parameters."""
+    sc = aerial
+    cam = sc.cameras[0]
+    target = torch.from_numpy(sc.targets[0]).cuda()
+    trs = [_trainer(sc), _trainer(sc), _trainer(sc)]
+    trs[1].fuse_adam = True
+    for _ in range(3):
+        trs[0].step_graph(0, cam, target[None])
+        trs[1].step_graph(0, cam, target[None])
+        trs[2].forward(cam); trs[2].loss_grad(target); trs[2].backward(overwrite=True); trs[2].adam_step()
+    torch.cuda.synchronize()
+    assert trs[0].step_count == trs[1].step_count == trs[2].step_count == 3
+    for key in scenes.PARAM_KEYS:
+        for t in trs[:2]:
+            # Adam normalises the gradient: where it is ~0 the atomics' summation order decides its sign and the
+            # parameter moves by +-lr either way -- those few elements aside, the three paths agree
+            ref = trs[2].params[key]
+            close = (t.params[key] - ref).abs() <= 1e-3 * ref.abs() + 2e-6
+            assert close.float().mean().item() > 0.999, (key, close.float().mean().item())
+    assert not torch.equal(trs[0].params["mean"], torch.from_numpy(sc.params["mean"].reshape(-1)).cuda())
