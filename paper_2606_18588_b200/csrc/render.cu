@@ -224,7 +224,14 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 // Staging block of one warp in the backward: STAGE_ITEMS (Gaussian, half tile) items x 9 gradient values x 32
 // lane partials.  63 rows = two rounds of 32 row sums; a lane sums its row with a rotating column so that the
 // 32 lanes hit 32 different banks.
-constexpr int STAGE_ITEMS = 7;
+#ifndef SPLX_STAGE_ITEMS
+#define SPLX_STAGE_ITEMS 7
+#endif
+#ifndef SPLX_BWD_MIN_CTAS
+#define SPLX_BWD_MIN_CTAS 10   /* 92 registers; higher occupancy targets measured slower (profiles/r01c) */
+#endif
+constexpr int STAGE_ITEMS = SPLX_STAGE_ITEMS;
+constexpr int STAGE_ROUNDS = (STAGE_ITEMS * 9 + 31) / 32;
 struct __align__(128) Stage { float v[STAGE_ITEMS * 9][32]; };
 
 // Sum the staged rows over the lanes: lane L sums row r*32 + L with eight 16-byte loads whose chunk index is
@@ -234,7 +241,7 @@ __device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int la
   __syncwarp();
   const int rows = nb * 9;
 #pragma unroll
-  for (int r = 0; r < 2; ++r) {
+  for (int r = 0; r < STAGE_ROUNDS; ++r) {
     const int p = r * 32 + lane;
     const int pc = p < rows ? p : 0;
     const unsigned base = (unsigned)__cvta_generic_to_shared(st.v[pc]) + 16u * (unsigned)(lane & 7);
@@ -252,7 +259,7 @@ __device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int la
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(BLOCK)
+__global__ void __launch_bounds__(BLOCK, SPLX_BWD_MIN_CTAS)
 k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const float* __restrict__ ct,
              const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d) {

@@ -292,8 +292,11 @@ k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t*
 
 // Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
 // started and the look-back spin cannot wait on a CTA that was never scheduled.
+#ifndef SPLX_RS_MIN_CTAS
+#define SPLX_RS_MIN_CTAS 4
+#endif
 template <typename KeyT>
-__global__ void __launch_bounds__(RS_THREADS)
+__global__ void __launch_bounds__(RS_THREADS, SPLX_RS_MIN_CTAS)
 k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
              uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
              uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits) {
