@@ -293,7 +293,23 @@ def run_ours(args):
     rng_ = tr.bins.tile_ranges
     live_slots = int((rng_[:, 1] > rng_[:, 0]).sum().item())     # (partition, tile) slots with a non-empty list
 
+    # Every timed pass (eager with stage events, graph replay, end to end) starts from the SAME training state: the
+    # parameters and moments are restored first, then W warm-up steps, then K timed steps -- the work of a step
+    # drifts as training moves the Gaussians, so passes run one after the other would time different scenes.
+    snap = {k: tr.flat[k].clone() for k in ("param", "m", "v")}
+    snap_count = tr.step_count
+
+    def restore():
+        for k, v in snap.items():
+            tr.flat[k].copy_(v)
+        tr.step_count = snap_count
+        if getattr(tr, "_step_dev", None) is not None:
+            tr._step_dev.fill_(snap_count)
+        if state is not None:
+            pass   # the saturation bytes are rebuilt by the first composition
+
     sampler = ClockSampler(local) if rank == 0 else None
+    restore()
     for _ in range(max(args.warmup, 3)):
         step()
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(10)] for _ in range(args.steps)]
@@ -317,7 +333,8 @@ def run_ours(args):
     # the same iteration replayed from a CUDA graph (a1-a10 captured once, Adam outside): no per-stage events
     graph_ms = None
     if not args.dense:
-        for _ in range(3):
+        restore()
+        for _ in range(max(args.warmup, 3)):
             tr.step_graph(0, cam, target1, saturation=args.saturation, sat_eps=args.sat_eps)
         barrier()
         g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -345,10 +362,11 @@ def run_ours(args):
         else:   # the public call: Trainer.step_host (copies on a side stream, overlapped with the kernels)
             tr.step_host(0, cam, tgt_host, img_host, loss_host, saturation=args.saturation, sat_eps=args.sat_eps)
 
-    for _ in range(3):
+    restore()
+    for _ in range(max(args.warmup, 3)):
         step_e2e()
     barrier()
-    n_e2e = max(3, args.steps // 2)
+    n_e2e = args.steps
     t0 = time.perf_counter()
     for _ in range(n_e2e):
         step_e2e()
