@@ -118,6 +118,38 @@ def grid_partition(mean, lo, hi, gx, gy):
     return iy * gx + ix
 
 
+def kd_partition(mean, K):
+    """"recursive binary splitting akin to a KD-tree, selecting the axis with the largest extent and
+    splitting at the median Gaussian position at each level so that the Gaussian counts across partitions remain
+    balanced".  K must be a power of two.  Returns part_id[n] in [0, K); leaves are numbered left to right, the lower
+    half of a split (ties by index, so the counts of the two halves differ by at most one) first."""
+    assert K >= 1 and (K & (K - 1)) == 0, "KD partitions come in powers of two"
+    mean = np.asarray(mean)
+    part_id = np.zeros(mean.shape[0], np.int64)
+    cells = [np.arange(mean.shape[0])]
+    while len(cells) < K:
+        nxt = []
+        for idx in cells:
+            if idx.size == 0:
+                nxt += [idx, idx]
+                continue
+            pts = mean[idx]
+            axis = int(np.argmax(pts.max(0) - pts.min(0)))
+            order = np.argsort(pts[:, axis], kind="stable")
+            half = (idx.size + 1) // 2
+            nxt += [idx[order[:half]], idx[order[half:]]]
+        cells = nxt
+    for k, idx in enumerate(cells):
+        part_id[idx] = k
+    return part_id
+
+
+def imbalance_ratio(part_offsets):
+    """N_max / N_mean - 1 over the partitions."""
+    counts = np.diff(np.asarray(part_offsets, np.float64))
+    return float(counts.max() / counts.mean() - 1.0)
+
+
 def partition_aabbs(params, part_offsets, inflate_sigma=3.0):
     """Axis-aligned box of every partition (partitions are AABBs): the bounding box of
     its Gaussians' supports, a Gaussian's support being its mean +- inflate_sigma x its largest scale (reading
@@ -177,7 +209,7 @@ def tiny(seed=0, n=4096, size=128, f=150.0, K=2, sh_degree=0):
 
 def aerial(seed=0, n=1_000_000, width=1920, height=1080, extent=(100.0, 100.0, 20.0), grid=(2, 2),
            altitude=80.0, pitch_deg=45.0, fov_deg=60.0, log_scale_mu=-2.5, log_scale_sigma=0.5,
-           sh_degree=3, n_views=1, name="aerial_1M"):
+           sh_degree=3, n_views=1, name="aerial_1M", partition="grid"):
     """BASELINE.json configs[1]: uniform box, K = grid xy partitions, aerial camera."""
     rng = np.random.default_rng(seed)
     ex, ey, ez = extent
@@ -193,7 +225,10 @@ def aerial(seed=0, n=1_000_000, width=1920, height=1080, extent=(100.0, 100.0, 2
         sh=rng.normal(0.0, 0.2, (n, 16, 3)).astype(np.float32),
     )
     K = grid[0] * grid[1]
-    part_id = grid_partition(mean, (-ex / 2, -ey / 2), (ex / 2, ey / 2), grid[0], grid[1])
+    if partition == "kd":        # the paper's own partitioner (L480) instead of BASELINE.json's uniform grid
+        part_id = kd_partition(mean, K)
+    else:
+        part_id = grid_partition(mean, (-ex / 2, -ey / 2), (ex / 2, ey / 2), grid[0], grid[1])
     params, offs = _order_by_partition(params, part_id, K)
     crng = np.random.default_rng(seed + 2)
     cams, targets = [], []

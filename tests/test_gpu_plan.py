@@ -400,3 +400,25 @@ def test_training_paths_agree_with_and_without_the_fused_optimiser(aerial):
             close = (t.params[key] - ref).abs() <= 1e-3 * ref.abs() + 2e-6
             assert close.float().mean().item() > 0.999, (key, close.float().mean().item())
     assert not torch.equal(trs[0].params["mean"], torch.from_numpy(sc.params["mean"].reshape(-1)).cuda())
+
+
+def test_kd_partitions_under_the_plan():
+    """The paper's own partitioner (KD median splits, L480) instead of the uniform grid: the plan path takes any
+    boxes.  One view, geometric state from the KD cells' 3-sigma boxes, against the oracle."""
+    sc = scenes.aerial(n=20_000, width=320, height=176, grid=(2, 2), log_scale_mu=-0.9, partition="kd", name="aerial_kd")
+    assert scenes.imbalance_ratio(sc.part_offsets) < 1e-3
+    cam = sc.cameras[0]
+    tr = _trainer(sc)
+    plan, _ = tr.bucket_plan([0], [cam], saturation=False)
+    target = torch.from_numpy(sc.targets[0]).cuda()[None]
+    imgs = tr.iteration_fused(plan, target, overwrite=True).clone()
+    torch.cuda.synchronize()
+    state = G.np32(plan.tile_state).reshape(sc.K, -1)
+    views, grads = ov.iteration_plan(sc.partitions(), [cam.as_array()], plan.view_of_part, sc.sh_degree, [sc.targets[0]],
+                                     sc.bg, tile_state=state)
+    frag = _fragile(views[0])
+    ok = G.close(G.np32(imgs[0]).astype(np.float64), views[0].image).all(-1)
+    assert (~(ok | frag)).sum() <= 1e-4 * frag.size
+    _check_grads(tr, grads)
+    full = oracle.forward(sc.partitions(), cam.as_array(), sc.sh_degree, sc.bg)     # no state at all
+    assert np.array_equal(full.image, views[0].image)

@@ -167,3 +167,30 @@ def test_consolidated_views_equal_the_views_one_by_one():
         assert np.array_equal(grads[2][key], ra.grads[0][key])
         assert np.array_equal(grads[0][key], rb.grads[0][key])
         assert not grads[1][key].any()
+
+
+def test_kd_partition_is_balanced_and_axis_aligned():
+    """median splits along the widest axis: counts differ by at most one per level, the cells are
+    disjoint axis-aligned boxes, the imbalance ratio N_max / N_mean - 1 is ~0; a skewed cloud stays balanced where
+    a uniform grid does not."""
+    rng = np.random.default_rng(8)
+    pts = np.concatenate([rng.normal(0, 1, (7001, 3)) * (5, 1, 0.2), rng.normal((30, 4, 0), 0.5, (3000, 3))]).astype(np.float32)
+    for K in (1, 2, 8, 16):
+        pid = scenes.kd_partition(pts, K)
+        counts = np.bincount(pid, minlength=K)
+        assert counts.sum() == len(pts) and counts.max() - counts.min() <= 1
+        offs = np.concatenate([[0], np.cumsum(counts)])
+        assert scenes.imbalance_ratio(offs) <= K / len(pts) + 1e-12       # at most one Gaussian above the mean
+        lo = np.array([pts[pid == k].min(0) for k in range(K)]); hi = np.array([pts[pid == k].max(0) for k in range(K)])
+        for a in range(K):
+            for b in range(a + 1, K):      # boxes of two leaves are separated along some axis (touching at most)
+                assert np.any(lo[a] >= hi[b]) or np.any(lo[b] >= hi[a]), (K, a, b)
+    first = scenes.kd_partition(pts, 2)
+    ext = pts.max(0) - pts.min(0)
+    axis = int(np.argmax(ext))
+    assert pts[first == 0][:, axis].max() <= pts[first == 1][:, axis].min()        # split along the widest axis
+    gid = scenes.grid_partition(pts, pts.min(0)[:2], pts.max(0)[:2], 4, 2)
+    g_offs = np.concatenate([[0], np.cumsum(np.bincount(gid, minlength=8))])
+    assert scenes.imbalance_ratio(g_offs) > 1.0
+    sc = scenes.aerial(n=5000, width=64, height=48, grid=(2, 2), partition="kd", name="kd")
+    assert np.diff(sc.part_offsets).tolist() == [1250, 1250, 1250, 1250]
