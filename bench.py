@@ -51,6 +51,8 @@ def workload(name):
         return scenes.small_aerial()
     if name == "city_10M":
         return scenes.city()                         # configs[2]: 10M Gaussians, K=8, B=4 views
+    if name == "street_10M":                         # the configs[2] scene seen from street level
+        return scenes.city(street=True, name="street_10M")
     if name == "city_40M":                           # configs[3]: 40M Gaussians, 1000 m, 4K views, K=16, B=4 (device generator)
         return scenes.city_device(n=40_000_000, width=3840, height=2160, extent=1000.0, n_buildings=800, grid=(4, 4),
                                   altitude=200.0, height_range=(5.0, 60.0), n_views=4, name="city_40M")
@@ -471,7 +473,8 @@ def run_views(args):
     B = min(args.views, len(sc.cameras))
     cams = sc.cameras[:B]
     W, H = cams[0].width, cams[0].height
-    cap = {"city_10M": 64_000_000, "city_40M": 160_000_000, "city_100M": 96_000_000}.get(args.workload)
+    cap = {"city_10M": 64_000_000, "street_10M": 200_000_000, "city_40M": 160_000_000,
+           "city_100M": 96_000_000}.get(args.workload)
     tr = Trainer(sc.params, sc.part_offsets, W, H, sc.sh_degree, sc.bg, capacity=cap)
     aabbs = scenes.partition_aabbs(sc.params, sc.part_offsets)
     sc.params = None                                   # a device-generated scene: release the generator's copy

@@ -97,6 +97,17 @@ def aerial_camera(width, height, fov_deg, altitude, pitch_deg, yaw_deg, target=(
     return Camera(R, t, f, f, width / 2.0, height / 2.0, width, height)
 
 
+def street_camera(width, height, fov_deg, position, yaw_deg, pitch_deg=0.0):
+    """Street-level camera (the street scenes, where walls saturate whole partitions): at `position`,
+    looking along `yaw` at `pitch` above the horizon."""
+    ps, th = np.deg2rad(yaw_deg), np.deg2rad(pitch_deg)
+    pos = np.asarray(position, np.float64)
+    tgt = pos + np.array([np.cos(th) * np.cos(ps), np.cos(th) * np.sin(ps), np.sin(th)])
+    R, t = look_at(pos, tgt)
+    f = 0.5 * width / np.tan(0.5 * np.deg2rad(fov_deg))
+    return Camera(R, t, f, f, width / 2.0, height / 2.0, width, height)
+
+
 def _rand_quat(rng, n):
     q = rng.standard_normal((n, 4)).astype(np.float32)
     q /= np.linalg.norm(q, axis=1, keepdims=True)
@@ -243,7 +254,7 @@ def aerial(seed=0, n=1_000_000, width=1920, height=1080, extent=(100.0, 100.0, 2
 
 def city(seed=0, n=10_000_000, width=1920, height=1080, extent=500.0, n_buildings=200, grid=(4, 2),
          altitude=120.0, pitch_deg=45.0, fov_deg=60.0, height_range=(5.0, 50.0), sh_degree=3,
-         n_views=4, name="city_10M"):
+         n_views=4, name="city_10M", street=False):
     """BASELINE.json configs[2]: 70 % of the means on building surfaces (roof + 4 walls,
     area-weighted, N(0, 0.1 m) jitter), 30 % on the ground plane; K = grid partitions."""
     rng = np.random.default_rng(seed)
@@ -288,11 +299,17 @@ def city(seed=0, n=10_000_000, width=1920, height=1080, extent=500.0, n_building
     cams, targets = [], []
     for v in range(n_views):
         tgt = np.append(crng.uniform(-0.4 * extent, 0.4 * extent, 2), 0.0)
-        cams.append(aerial_camera(width, height, fov_deg, altitude, pitch_deg, crng.uniform(0, 360), tgt))
+        yaw = crng.uniform(0, 360)
+        if street:   # the same seeded spots, seen from 1.7 m above the ground looking along the yaw (street scenes, L296)
+            while np.any((np.abs(tgt[:2] - bc) < 0.5 * bs + 2.0).all(1)):      # not inside (or 2 m from) a building
+                tgt = np.append(crng.uniform(-0.4 * extent, 0.4 * extent, 2), 0.0)
+            cams.append(street_camera(width, height, fov_deg, (tgt[0], tgt[1], 1.7), yaw, 5.0))
+        else:
+            cams.append(aerial_camera(width, height, fov_deg, altitude, pitch_deg, yaw, tgt))
         targets.append(np.random.default_rng(seed + 1 + 1000 * v)
                        .uniform(0, 1, (height, width, 3)).astype(np.float32))
     return Scene(name, params, offs, cams, targets, sh_degree,
-                 meta=dict(seed=seed, config="configs[2]", grid=grid, extent=extent))
+                 meta=dict(seed=seed, config="configs[2]", grid=grid, extent=extent, street=street))
 
 
 def small_aerial(seed=0, n=20_000, width=320, height=176, K=(2, 2), sh_degree=3):
