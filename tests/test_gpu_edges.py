@@ -118,3 +118,73 @@ def test_argument_validation():
     p = torch.zeros(16, device="cuda")
     with pytest.raises(binding.SplxError):
         tr.ctx.adam(p, p.clone(), p.clone(), p.clone(), lr=1e-3, step=0)         # step is 1-based
+
+
+# ---- the same edges under launch plans ------------------------------------------------------------------
+def test_plan_without_participants_gives_background():
+    """Every partition at view -1: nothing is projected, binned or rendered; Eq.5 with no partial = background for
+    every view; '=' mode writes an all-zero gradient."""
+    sc = scenes.tiny(n=600, size=48, f=60.0, K=2, seed=7)
+    cam = sc.cameras[0]
+    bg = (0.1, 0.2, 0.3)
+    tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, bg)
+    for v in tr.grads.values():
+        v.fill_(3.0)
+    plan = tr.make_plan([cam, cam], [-1, -1], None, True)
+    target = torch.from_numpy(np.stack([sc.targets[0], sc.targets[0]])).cuda()
+    imgs = tr.iteration_fused(plan, target, overwrite=True)
+    torch.cuda.synchronize()
+    assert tr.num_intersections() == 0
+    assert np.allclose(G.np32(imgs), np.asarray(bg, np.float32), atol=0)
+    assert (G.np32(tr._T_totals[:2]) == 1).all()
+    assert not tr.flat["grad"].any()
+
+
+def test_plan_with_64_partitions_and_8_views():
+    """The limits of the plan: K = SPLX_MAX_K = 64 partitions, B = SPLX_MAX_VIEWS = 8 views (each rendering 8 of
+    them), against the oracle's plan iteration."""
+    sc = scenes.tiny(n=3200, size=64, f=75.0, K=64, seed=8, sh_degree=1)
+    base = sc.cameras[0]
+    cams = []
+    for b in range(8):
+        t = base.t + np.array([0.05 * b, -0.03 * b, 0.1 * b], np.float32)
+        cams.append(scenes.Camera(base.R, t, base.fx, base.fy, base.cx, base.cy, base.width, base.height))
+    vop = [k % 8 for k in range(64)]
+    rng = np.random.default_rng(9)
+    targets = rng.uniform(0, 1, (8, 64, 64, 3)).astype(np.float32)
+    tr = Trainer(sc.params, sc.part_offsets, 64, 64, sc.sh_degree, sc.bg)
+    plan = tr.make_plan(cams, vop, None, True)
+    imgs = tr.iteration_fused(plan, torch.from_numpy(targets).cuda(), overwrite=True).clone()
+    torch.cuda.synchronize()
+    from oracle import visibility as ov
+    views, grads = ov.iteration_plan(sc.partitions(), [c.as_array() for c in cams], vop, sc.sh_degree, list(targets), sc.bg)
+    for b, res in enumerate(views):
+        frag = np.zeros((64, 64), bool)
+        for pa in res.partials:
+            frag |= pa.margin < G.FRAGILE_MARGIN
+        frag |= res.order_margin < 1e-6
+        ok = G.close(G.np32(imgs[b]).astype(np.float64), res.image).all(-1)
+        assert (ok | frag).all(), b
+    for key in scenes.PARAM_KEYS:
+        ref = np.concatenate([g[key].reshape(-1) for g in grads])
+        assert G.rel_l2(G.np32(tr.grads[key]), ref) <= 1e-3, key
+
+
+def test_plan_capacity_overflow_and_bad_plans_are_reported():
+    sc = scenes.tiny(n=2000, size=64, f=75.0, K=2, seed=10)
+    cam = sc.cameras[0]
+    tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=1000)
+    plan = tr.make_plan([cam], [0, 0], None, True)
+    tr.forward_plan(plan)
+    with pytest.raises(binding.SplxError) as e:
+        tr.num_intersections()
+    assert e.value.code == binding.ERR_CAPACITY
+    other = scenes.Camera(cam.R, cam.t, cam.fx, cam.fy, cam.cx, cam.cy, cam.width * 2, cam.height)
+    for bad in (lambda: tr.make_plan([cam, other], [0, 1]),          # views of different sizes
+                lambda: tr.make_plan([cam], [0, 1]),                 # view index out of range
+                lambda: tr.make_plan([cam] * 9, [0, 0])):            # more than SPLX_MAX_VIEWS views
+        with pytest.raises(binding.SplxError) as e:
+            tr.ctx.project_plan(tr.params, tr.part_offsets, bad(), tr.sh_degree, tr.proj)
+        assert e.value.code == binding.ERR_INVALID_ARG
+    with pytest.raises(binding.SplxError):                            # sparse compose without the binning
+        tr.ctx.compose_plan(tr.partials, None, plan, tr.bg, tr._images[:1])
