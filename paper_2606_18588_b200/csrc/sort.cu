@@ -17,10 +17,14 @@
 
 namespace {
 
-constexpr int SCAN_THREADS = 512, SCAN_IPT = 4, SCAN_TILE = SCAN_THREADS * SCAN_IPT;
+#ifndef SPLX_SCAN_IPT
+#define SPLX_SCAN_IPT 16
+#endif
+constexpr int SCAN_THREADS = 512, SCAN_IPT = SPLX_SCAN_IPT, SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // 8192 elements per tile
 constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
-static_assert(SCAN_TILE == RS_TILE, "the compaction scan clears the radix status words tile by tile");
+static_assert(SCAN_TILE % RS_TILE == 0, "the compaction scan clears the radix status words of the tiles it covers");
+constexpr int SCAN_RS = SCAN_TILE / RS_TILE;
 constexpr uint32_t PERSISTENT_CTAS = SPLX_SM_COUNT * 8;   // grid of the persistent kernels: 8 CTAs per SM
 
 struct Counters {   // device-resident counts, written by kernels, read by later kernels
@@ -135,12 +139,16 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     if (t >= ntiles) break;
     if (HIST) {
 #pragma unroll
-      for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) rstatus[(size_t)(x >> 8) * rstride + (size_t)t * 256 + (x & 255)] = 0;
+      for (int x = threadIdx.x; x < 4 * 256 * SCAN_RS; x += SCAN_THREADS) {   // pass x / (256 SCAN_RS), radix tiles SCAN_RS t ..
+        const int pass = x / (256 * SCAN_RS), w = x - pass * (256 * SCAN_RS);
+        rstatus[(size_t)pass * rstride + (size_t)t * (256 * SCAN_RS) + w] = 0;
+      }
     }
     const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
     uint32_t v[SCAN_IPT], s = 0;
+    const typename Op::Cursor cur = op.cursor(base < n ? base : 0);      // the thread's 16 elements are consecutive
 #pragma unroll
-    for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(base + k) : 0; s += v[k]; }
+    for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(cur, base, k) : 0; s += v[k]; }
     uint32_t total;
     uint32_t ex = block_exclusive_scan(s, sm, total);
     if (threadIdx.x == 0) {
@@ -157,7 +165,7 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     __syncthreads();
     ex += (uint32_t)s_excl;
 #pragma unroll
-    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(base + k, v[k], ex, s_hist); ex += v[k]; }
+    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(cur, base, k, v[k], ex, s_hist); ex += v[k]; }
   }
   if (HIST) {
     __syncthreads();
@@ -180,11 +188,16 @@ struct RunMap {
 
 struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order preserved
   const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n; RunMap map;
+  struct Cursor {};
   __device__ uint64_t count(const uint64_t*) const { return n; }
-  __device__ uint32_t load(uint64_t j) const { return tiles_touched[map(j)] > 0 ? 1u : 0u; }
-  __device__ void store(uint64_t j, uint32_t v, uint32_t ex, uint32_t* hist) const {
+  __device__ Cursor cursor(uint64_t) const { return Cursor{}; }
+  __device__ uint64_t index(const Cursor& c, uint64_t base, int k) const {
+    return map(base + k);     // a <= 6-step search over the run starts (uniform across a warp: constant-bank loads)
+  }
+  __device__ uint32_t load(const Cursor& c, uint64_t base, int k) const { return tiles_touched[index(c, base, k)] > 0 ? 1u : 0u; }
+  __device__ void store(const Cursor& c, uint64_t base, int k, uint32_t v, uint32_t ex, uint32_t* hist) const {
     if (v) {
-      const uint64_t i = map(j);
+      const uint64_t i = index(c, base, k);
       const uint32_t key = __float_as_uint(depth[i]);
       ckeys[ex] = key; cvals[ex] = (uint32_t)i;
 #pragma unroll
@@ -195,8 +208,10 @@ struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order 
 struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, depth order
   const uint32_t* tiles_touched; const uint32_t* cvals; uint32_t* offs;
   __device__ uint64_t count(const uint64_t* n_ptr) const { return *n_ptr; }
-  __device__ uint32_t load(uint64_t j) const { return tiles_touched[cvals[j]]; }
-  __device__ void store(uint64_t j, uint32_t, uint32_t ex, uint32_t*) const { offs[j] = ex; }
+  struct Cursor {};
+  __device__ Cursor cursor(uint64_t) const { return Cursor{}; }
+  __device__ uint32_t load(const Cursor&, uint64_t base, int k) const { return tiles_touched[cvals[base + k]]; }
+  __device__ void store(const Cursor&, uint64_t base, int k, uint32_t, uint32_t ex, uint32_t*) const { offs[base + k] = ex; }
 };
 
 template <class Op, bool HIST>
@@ -407,11 +422,12 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
 template <typename KeyT>
 int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
                const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets,
-               bool have_hist /* histograms counted and status cleared by the producer of the keys */) {
+               bool have_hist /* histograms counted and status cleared by the producer of the keys */,
+               size_t stride_words = 0 /* status words per pass; 0 = tiles(capacity) * 256 */) {
   const uint32_t ntiles_cap = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
   if (ntiles_cap == 0) return SPLX_OK;
   const uint32_t nblocks = ntiles_cap < PERSISTENT_CTAS ? ntiles_cap : PERSISTENT_CTAS;
-  const size_t stride = (size_t)ntiles_cap * 256;     // status words per pass
+  const size_t stride = stride_words ? stride_words : (size_t)ntiles_cap * 256;     // status words per pass
   const PassPlan plan = plan_passes(begin_bit, end_bit);
   if (!have_hist) {
     k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, status, stride, plan);
@@ -539,7 +555,7 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   Layout L;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
-  const size_t tiles_n = ((size_t)n + RS_TILE - 1) / RS_TILE, tiles_m = ((size_t)capacity + RS_TILE - 1) / RS_TILE;
+  const size_t tiles_m = ((size_t)capacity + RS_TILE - 1) / RS_TILE;
   const size_t scan_n = ((size_t)n + SCAN_TILE - 1) / SCAN_TILE;
   L.counters = take(sizeof(Counters));
   L.ghist_d = take(MAX_PASSES * 256 * 4);
@@ -547,7 +563,7 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   L.st_scan_v = take(scan_n * 8);
   L.st_scan_t = take(scan_n * 8);
   L.zero_bytes = off;
-  L.st_depth = take(4 * tiles_n * 256 * 8);                                   // cleared tile by tile by k_radix_hist_all
+  L.st_depth = take(4 * scan_n * SCAN_RS * 256 * 8);                          // cleared by the compaction scan, whole scan tiles
   L.st_slot = take((size_t)((sbits + 7) / 8) * tiles_m * 256 * 8);
   L.ckeys_a = take((size_t)n * 4); L.cvals_a = take((size_t)n * 4);
   L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
@@ -595,13 +611,15 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   vop.map.n = rt.n;
   for (int r = 0; r < rt.n; ++r) { vop.map.begin[r] = rt.begin[r]; vop.map.jprefix[r] = rt.jprefix[r]; }
   vop.map.jprefix[rt.n] = rt.jprefix[rt.n];
-  const size_t stride_d = (((size_t)n_act + RS_TILE - 1) / RS_TILE) * 256;   // status words per pass, depth sort
+  // status words per pass of the depth sort: whole scan tiles (the compaction scan clears SCAN_RS radix tiles at a time)
+  const size_t stride_d = (((size_t)n_act + SCAN_TILE - 1) / SCAN_TILE) * SCAN_RS * 256;
   if ((rc = scan_exclusive<VisibleOp, true>(ctx, vop, (uint64_t)n_act, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
                                             &cnt->n_visible, nullptr, 0, (uint32_t*)(base + L.ghist_d),
                                             (uint64_t*)(base + L.st_depth), stride_d))) return rc;
   // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers); histograms came with step 1
   if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n_act, &cnt->n_visible, 0, 32,
-                                 (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2], true))) return rc;
+                                 (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2], true,
+                                 stride_d))) return rc;
   // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
   if ((rc = scan_exclusive<TouchedOp, false>(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
