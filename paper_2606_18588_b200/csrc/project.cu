@@ -272,8 +272,11 @@ __device__ __forceinline__ void adam_scalar(float* pp, float* pm, float* pv, flo
   *pp = p; *pm = m; *pv = v;
 }
 
+#ifndef SPLX_PB_MIN_CTAS
+#define SPLX_PB_MIN_CTAS 5   /* 96 registers, no spills; 6 spills and is not faster (measured) */
+#endif
 template <int DEG, bool ACC, bool ADAM>
-__global__ void __launch_bounds__(PB_THREADS)
+__global__ void __launch_bounds__(PB_THREADS, SPLX_PB_MIN_CTAS)
 k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out,
               const __grid_constant__ AdamFuse af) {
