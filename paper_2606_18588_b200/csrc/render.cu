@@ -118,8 +118,11 @@ __device__ __forceinline__ bool eval_alpha(float dx, float dy, float adx, float 
   return (p2 <= 0.0f) && (alpha >= amin);
 }
 
+#ifndef SPLX_FWD_MIN_CTAS
+#define SPLX_FWD_MIN_CTAS 14   /* 71 registers; the sweep 12..20 shows no effect below spilling: issue-bound */
+#endif
 template <bool COUNT>
-__global__ void __launch_bounds__(BLOCK)
+__global__ void __launch_bounds__(BLOCK, SPLX_FWD_MIN_CTAS)
 k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const __grid_constant__ PartView pv, int sparse,
              float* __restrict__ out_ct, float* __restrict__ out_d, uint32_t* __restrict__ out_n,
