@@ -37,8 +37,8 @@ FLOPS_BLEND_BWD = 55  # one contributing pair in the backward incl. its 9 reduct
 FP32_LANES_PER_SM = 128
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on aerial_1M, from the `ncu --set full` capture summarised in
-# profiles/r01c_ncu_full.csv (a profiler number, copied here by hand; null for other workloads)
-NCU_TRAFFIC_BYTES = {"aerial_1M": {"k_raster_bwd": 220.8e6, "k_render_fwd": 88.8e6, "adam": 1596.8e6, "project_backward": 522.9e6}}
+# profiles/r01d_ncu_full.csv (a profiler number, copied here by hand; null for other workloads)
+NCU_TRAFFIC_BYTES = {"aerial_1M": {"k_raster_bwd": 217.5e6, "k_render_fwd": 89.1e6, "adam": 1597.4e6, "project_backward": 520.4e6}}
 
 
 def workload(name):
