@@ -303,6 +303,19 @@ int splx_raster_backward_plan(splx_ctx *ctx, const splx_projected *proj, const s
 int splx_project_backward_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                                const splx_plan *plan, int sh_degree, const splx_projected *proj,
                                float *g2d, int flags, const splx_gaussian_grads *grads);
+/* The list of VISIBLE Gaussians (global indices, ascending) that the last splx_bin_sort[_plan] on workspace `ws`
+ * left there, and its device-side count: pointers INTO the workspace (device memory), valid until the next
+ * splx_bin_sort on it.  Same n, capacity, K, cam as that call.  Host computation only. */
+int splx_bin_sort_visible(const void *ws, int64_t n, uint64_t capacity, int K, const splx_camera *cam,
+                          const uint32_t **visible, const uint64_t **num_visible);
+/* splx_project_backward_plan in += mode over the visible Gaussians only: the rows processed are the entries of
+ * `visible` (device uint32[*num_visible], *num_visible a device uint64) instead of every Gaussian of the
+ * participating partitions -- same result (a culled Gaussian has no gradient), work proportional to the visible
+ * count.  flags: SPLX_PB_CLEAR_G2D or 0. */
+int splx_project_backward_list_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                                    const splx_plan *plan, int sh_degree, const splx_projected *proj,
+                                    float *g2d, int flags, const splx_gaussian_grads *grads,
+                                    const uint32_t *visible, const uint64_t *num_visible);
 /* a10 + a11 fused: the LAST projection backward of an iteration also takes the Adam step of splx_adam on every
  * row of every partition (participating or not), reading the gradient it has just formed -- plus, without
  * SPLX_PB_OVERWRITE, the gradient earlier launches of the iteration left in `grads` -- instead of storing it:

@@ -33,6 +33,7 @@ EXPORTS = [
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
     "splx_compose_l1_backward_plan", "splx_project_backward_adam_plan", "splx_adam_bias_step",
+    "splx_bin_sort_visible", "splx_project_backward_list_plan",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -141,6 +142,8 @@ def lib():
         L.splx_project_backward_adam_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp,
                                                       C.c_float, C.c_float, C.c_float, vp, C.c_float]
         L.splx_adam_bias_step.argtypes = [vp, C.c_float, C.c_float, vp, vp]
+        L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
+        L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -469,6 +472,23 @@ class Context:
             self._h, C.byref(sets[0]), plan.K, self._offs(part_offsets), plan.ref(), sh_degree, C.byref(ps), _ptr(g2d),
             flags, C.byref(sets[1]), C.byref(sets[2]), C.byref(sets[3]), lr, beta1, beta2, eps, _ptr(bias_corr),
             float(grad_scale)))
+
+    @staticmethod
+    def bin_sort_visible(ws: torch.Tensor, n, capacity, K, cam):
+        """Device pointers (ints) of the visible list and of its count inside the bin_sort workspace."""
+        cs = camera_struct(cam)
+        lst, cnt = C.c_void_p(), C.c_void_p()
+        rc = lib().splx_bin_sort_visible(_ptr(ws), n, capacity, K, C.byref(cs), C.byref(lst), C.byref(cnt))
+        if rc != OK:
+            raise SplxError(rc, "splx_bin_sort_visible: invalid argument")
+        return lst.value, cnt.value
+
+    def project_backward_list_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
+                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False):
+        g, gg, ps = gaussians_struct(params), gaussians_struct(grads), proj.struct()
+        self._check(lib().splx_project_backward_list_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
+                                                          sh_degree, C.byref(ps), _ptr(g2d), PB_CLEAR_G2D if clear_g2d else 0,
+                                                          C.byref(gg), C.c_void_p(visible_ptr), C.c_void_p(count_ptr)))
 
     def adam_bias_step(self, step_dev, bias_corr, beta1=0.9, beta2=0.999):
         self._check(lib().splx_adam_bias_step(self._h, beta1, beta2, _ptr(step_dev), _ptr(bias_corr)))

@@ -306,7 +306,35 @@ int splx_project_backward_plan(splx_ctx* ctx, const splx_gaussians* g, int K, co
   int rc;
   if ((rc = make_plan(ctx, "splx_project_backward", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: part_offsets must run monotonically from 0 to n");
-  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr);
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, nullptr, nullptr);
+}
+
+int splx_bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, const splx_camera* cam,
+                          const uint32_t** visible, const uint64_t** num_visible) {
+  if (!ws || n < 0 || K < 1 || K > SPLX_MAX_K || !cam_ok(cam) || !visible || !num_visible) return SPLX_ERR_INVALID_ARG;
+  const int TX = (cam->width + SPLX_TILE - 1) / SPLX_TILE, TY = (cam->height + SPLX_TILE - 1) / SPLX_TILE;
+  return bin_sort_visible(ws, n, capacity, K, TX, TY, visible, num_visible);
+}
+
+int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets,
+                                    const splx_plan* plan, int sh_degree, const splx_projected* proj, float* g2d, int flags,
+                                    const splx_gaussian_grads* grads, const uint32_t* visible, const uint64_t* num_visible) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!visible || !num_visible) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: visible list is NULL");
+  if (flags & SPLX_PB_OVERWRITE) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: accumulates only (no SPLX_PB_OVERWRITE)");
+  if (g && grads && g->n == 0 && grads->n == 0) return SPLX_OK;
+  if (!gauss_ok(g) || !proj_ok(proj) || !g2d || !aligned16(g2d) || !grads || !grads->mean ||
+      !grads->log_scale || !grads->quat || !grads->opacity_logit || !grads->sh || !aligned16(grads->quat) ||
+      !aligned16(grads->mean) || !aligned16(grads->log_scale) || !aligned16(grads->sh) || !aligned16(grads->opacity_logit) ||
+      grads->n != g->n)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: null/misaligned argument");
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: sh_degree %d not in [0,3]", sh_degree);
+  if (flags & ~SPLX_PB_CLEAR_G2D) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: unknown flags %d", flags);
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_project_backward_list", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: part_offsets must run monotonically from 0 to n");
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, visible, num_visible);
 }
 
 int splx_project_backward_adam_plan(splx_ctx* ctx, const splx_gaussian_grads* params, int K, const int64_t* part_offsets,
@@ -340,7 +368,7 @@ int splx_project_backward_adam_plan(splx_ctx* ctx, const splx_gaussian_grads* pa
   af.omb1 = (float)(1.0 - (double)beta1); af.omb2 = (float)(1.0 - (double)beta2);   // as splx_adam forms them
   af.eps = eps; af.gscale = grad_scale; af.bc = bias_corr;
   const splx_gaussians g{params->mean, params->log_scale, params->quat, params->opacity_logit, params->sh, params->n};
-  return launch_project_bwd(ctx, &g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, &af);
+  return launch_project_bwd(ctx, &g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, &af, nullptr, nullptr);
 }
 
 int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,

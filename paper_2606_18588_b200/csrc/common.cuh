@@ -138,7 +138,11 @@ struct AdamFuse {
 int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
-                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*, const AdamFuse* adam);
+                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*, const AdamFuse* adam,
+                       const uint32_t* visible_list, const uint64_t* num_visible);
+// the depth-sorted list of visible Gaussians a bin_sort leaves in its workspace, and its device-side count
+int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX, int TY, const uint32_t** list,
+                     const uint64_t** count);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
 int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, const PlanDev&, const int64_t* part_offsets,
                     const splx_binning*, void* ws, size_t ws_bytes);

@@ -275,23 +275,49 @@ __device__ __forceinline__ void adam_scalar(float* pp, float* pm, float* pv, flo
 #ifndef SPLX_PB_MIN_CTAS
 #define SPLX_PB_MIN_CTAS 5   /* 96 registers, no spills; 6 spills and is not faster (measured) */
 #endif
-template <int DEG, bool ACC, bool ADAM>
+// LIST (accumulating launches only): the rows of a block are 128 entries of the binning's list of VISIBLE Gaussians
+// (splx_bin_sort_visible) instead of 128 consecutive Gaussians, so the work follows the visible count -- on the
+// city scenes ~10 % of the participating Gaussians -- and not the partition sizes; the grid is persistent because
+// the count lives on the device.
+template <int DEG, bool ACC, bool ADAM, bool LIST>
 __global__ void __launch_bounds__(PB_THREADS, SPLX_PB_MIN_CTAS)
 k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out,
-              const __grid_constant__ AdamFuse af) {
+              const __grid_constant__ AdamFuse af, const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr) {
   extern __shared__ __align__(16) float s_dyn[];
   float* s_sh = s_dyn;                                   // [128][52] sh in, SH gradient out
   float* s_old = s_dyn + PB_THREADS * PB_STRIDE;         // [128][52] previous SH gradient (ACC only)
   __shared__ __align__(16) float s_m[PB_THREADS * 3];    // mean gradient tile
   __shared__ __align__(16) float s_s[PB_THREADS * 3];    // log_scale gradient tile
   __shared__ uint8_t s_vis[PB_THREADS];
-  const int run = find_run(rt, (int)blockIdx.x);
-  const int64_t base = rt.begin[run] + (int64_t)((int)blockIdx.x - rt.block_prefix[run]) * PB_THREADS;
-  const int64_t run_end = rt.end[run];
-  const int64_t i = base + threadIdx.x;
-  const int nrows = (int)min((int64_t)PB_THREADS, run_end - base);
-  const int view = rt.view[run];                          // < 0: a non-participating partition (OVERWRITE only): zeros
+  __shared__ int64_t s_idx[PB_THREADS];                  // Gaussian of each row of the block
+  const uint64_t nvis = LIST ? *nvis_ptr : 0;
+  for (uint64_t blk = blockIdx.x; LIST ? (blk * PB_THREADS < nvis) : (blk == blockIdx.x); blk += gridDim.x) {
+  int64_t base = 0, run_end = 0, i = 0;
+  int nrows, view;
+  if (LIST) {
+    const uint64_t j0 = blk * PB_THREADS;
+    nrows = (int)min((uint64_t)PB_THREADS, nvis - j0);
+    view = 0;
+    if ((int)threadIdx.x < nrows) {
+      i = (int64_t)vlist[j0 + threadIdx.x];
+      run_end = i + 1;
+      int lo = 0, hi = rt.n - 1;                          // the run (partition) of Gaussian i -> its view
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (rt.begin[mid] <= i) lo = mid; else hi = mid - 1;
+      }
+      view = rt.view[lo];
+    }
+  } else {
+    const int run = find_run(rt, (int)blockIdx.x);
+    base = rt.begin[run] + (int64_t)((int)blockIdx.x - rt.block_prefix[run]) * PB_THREADS;
+    run_end = rt.end[run];
+    i = base + threadIdx.x;
+    nrows = (int)min((int64_t)PB_THREADS, run_end - base);
+    view = rt.view[run];                                  // < 0: a non-participating partition (OVERWRITE only): zeros
+  }
+  s_idx[threadIdx.x] = i;
   const CamDev& cam = plan.cam[view < 0 ? 0 : view];
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;        // float4 chunks of a row that hold used coefficients
@@ -320,8 +346,8 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     const int q = c * PB_THREADS + threadIdx.x;
     const int row = q / NV, c4 = q - row * NV;
     if (row < nrows && s_vis[row]) {
-      cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * (base + row) + 4 * c4);
-      if (ACC) cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * (base + row) + 4 * c4);
+      cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * s_idx[row] + 4 * c4);
+      if (ACC) cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
     }
   }
   float dmu[3] = {0.f, 0.f, 0.f}, dls[3] = {0.f, 0.f, 0.f};
@@ -488,7 +514,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
         const int q = (c0 + u) * PB_THREADS + threadIdx.x;
         const int row = q / 12, c4 = q - row * 12;
         ok[u] = row < nrows;
-        off[u] = 48 * (base + row) + 4 * c4;
+        off[u] = 48 * (ok[u] ? s_idx[row] : 0) + 4 * c4;
         Gr[u] = make_float4(0.f, 0.f, 0.f, 0.f);
         if (ok[u]) {
           const bool live = s_vis[row] && c4 < NV;
@@ -522,7 +548,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     const int q = c * PB_THREADS + threadIdx.x;
     const int row = q / 12, c4 = q - row * 12;
     if (row < nrows) {
-      float4* dst = reinterpret_cast<float4*>(out.sh + 48 * (base + row)) + c4;
+      float4* dst = reinterpret_cast<float4*>(out.sh + 48 * s_idx[row]) + c4;
       const bool live = s_vis[row] && c4 < NV;
       if (ACC) {
         if (live) {
@@ -538,7 +564,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   }
   // mean / log_scale gradient tiles: 96 float4 each; a partial last block, or a run that does not start
   // on a multiple of 4 Gaussians (12-byte rows: 16-byte alignment needs base % 4 == 0), falls back to scalars
-  if (nrows == PB_THREADS && (base & 3) == 0) {
+  if (!LIST && nrows == PB_THREADS && (base & 3) == 0) {
     if (threadIdx.x < 96) {
       float4* dm = reinterpret_cast<float4*>(out.mean + 3 * base) + threadIdx.x;
       float4* ds = reinterpret_cast<float4*>(out.log_scale + 3 * base) + threadIdx.x;
@@ -567,6 +593,8 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       else     { out.mean[3 * i + k] = dmu[k]; out.log_scale[3 * i + k] = dls[k]; }
     }
   }
+  __syncthreads();      // LIST: the next block of rows reuses the shared tiles
+  }
 }
 
 template <int DEG, bool ACC, bool ADAM>
@@ -574,10 +602,24 @@ static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pla
                       const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
                       const AdamFuse& af) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  k_project_bwd<DEG, ACC, ADAM><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(*g, plan, rt, ctx->cfg, *pr, g2d,
-                                                                                            clear_g2d, *grads, af);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  k_project_bwd<DEG, ACC, ADAM, false><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(
+      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, nullptr, nullptr);
+}
+
+// accumulating launch over the list of visible Gaussians (persistent grid: the count lives on the device)
+template <int DEG>
+static void launch_pb_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
+                           const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
+                           const AdamFuse& af, const uint32_t* vlist, const uint64_t* nvis) {
+  const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * 2;
+  cudaFuncSetAttribute(k_project_bwd<DEG, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, true, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  const int64_t need = (rt.jprefix[rt.n] + PB_THREADS - 1) / PB_THREADS;
+  const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 4 ? need : (int64_t)SPLX_SM_COUNT * 4;
+  k_project_bwd<DEG, true, false, true><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
+      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis);
 }
 
 template <bool ACC, bool ADAM>
@@ -610,9 +652,23 @@ int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pl
 
 int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
                        const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads,
-                       const AdamFuse* adam) {
+                       const AdamFuse* adam, const uint32_t* vlist, const uint64_t* nvis) {
   const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
   const bool overwrite = (flags & SPLX_PB_OVERWRITE) != 0;
+  if (vlist && nvis && !overwrite && !adam) {      // += over the visible Gaussians only
+    const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, false);
+    if (rt.jprefix[rt.n] == 0) return SPLX_OK;
+    AdamFuse none;
+    memset(&none, 0, sizeof none);
+    switch (deg) {
+      case 0: launch_pb_list<0>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
+      case 1: launch_pb_list<1>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
+      case 2: launch_pb_list<2>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
+      default: launch_pb_list<3>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
+    }
+    SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
+    return SPLX_OK;
+  }
   // "=" must also clear the rows of partitions that do not participate in this launch; the fused optimiser
   // step must reach every row of every partition
   const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, overwrite || adam != nullptr);

@@ -187,7 +187,7 @@ struct RunMap {
 };
 
 struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order preserved
-  const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint64_t n; RunMap map;
+  const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint32_t* vis_list; uint64_t n; RunMap map;
   struct Cursor {};
   __device__ uint64_t count(const uint64_t*) const { return n; }
   __device__ Cursor cursor(uint64_t) const { return Cursor{}; }
@@ -200,6 +200,7 @@ struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order 
       const uint64_t i = index(c, base, k);
       const uint32_t key = __float_as_uint(depth[i]);
       ckeys[ex] = key; cvals[ex] = (uint32_t)i;
+      vis_list[ex] = (uint32_t)i;      // the visible Gaussians in INDEX order (kept: the depth sort permutes cvals)
 #pragma unroll
       for (int p = 0; p < 4; ++p) atomicAdd(&hist[p * 256 + ((key >> (8 * p)) & 255u)], 1u);
     }
@@ -541,7 +542,7 @@ __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_
 // actual counts reach) and the sort buffers.
 struct Layout {
   size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes;
-  size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, keys_tmp, vals_tmp, total;
+  size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, vis_list, keys_tmp, vals_tmp, total;
 };
 
 static int slot_bits(int K, int TX, int TY) {
@@ -568,6 +569,7 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   L.ckeys_a = take((size_t)n * 4); L.cvals_a = take((size_t)n * 4);
   L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
   L.offs = take((size_t)n * 4);
+  L.vis_list = take((size_t)n * 4);
   L.keys_tmp = take((size_t)capacity * 8); L.vals_tmp = take((size_t)capacity * 4);
   L.total = off;
   return L;
@@ -577,6 +579,15 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
 
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY) {
   return make_layout(n, capacity, slot_bits(K, TX, TY)).total;
+}
+
+int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX, int TY, const uint32_t** list,
+                     const uint64_t** count) {
+  const Layout L = make_layout(n, capacity, slot_bits(K, TX, TY));
+  const char* base = (const char*)ws;
+  *list = (const uint32_t*)(base + L.vis_list);       // index order: consecutive rows of the list are close in memory
+  *count = &((const Counters*)(base + L.counters))->n_visible;
+  return SPLX_OK;
 }
 
 int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const PlanDev& plan, const int64_t* part_offsets,
@@ -607,7 +618,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   }
   int rc;
   // 1. visible Gaussians, index order
-  VisibleOp vop{pr->tiles_touched, pr->depth, ckeys_a, cvals_a, (uint64_t)n_act, {}};
+  VisibleOp vop{pr->tiles_touched, pr->depth, ckeys_a, cvals_a, (uint32_t*)(base + L.vis_list), (uint64_t)n_act, {}};
   vop.map.n = rt.n;
   for (int r = 0; r < rt.n; ++r) { vop.map.begin[r] = rt.begin[r]; vop.map.jprefix[r] = rt.jprefix[r]; }
   vop.map.jprefix[rt.n] = rt.jprefix[rt.n];

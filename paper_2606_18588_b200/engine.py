@@ -7,6 +7,8 @@ CUDA kernels behind ``binding.Context``.  K partitions = K contiguous slices of 
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import torch
 
@@ -64,6 +66,9 @@ class Trainer:
         #: at 4 CTAs/SM (124 registers) the fused kernel streams the moments at ~4 TB/s, while the stand-alone Adam
         #: kernel runs at 95 % of the HBM roof -- measured 0.44 ms fused against 0.11 + 0.27 ms
         self.fuse_adam = False
+        #: accumulating projection backward over the binning's list of visible Gaussians
+        #: (splx_project_backward_list_plan) instead of all rows of the participating partitions
+        self.use_visible_list = os.environ.get("SPLX_VISIBLE_LIST", "1") == "1"
         self._cam = None
         self._aabb = None
         self._side = None
@@ -196,6 +201,10 @@ class Trainer:
             c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
                                          self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev,
                                          grad_scale=1.0 / n_views, clear_g2d=True, overwrite=overwrite)
+        elif not overwrite and self.use_visible_list:   # an accumulating launch over the binning's visible list only
+            lst, cnt = c.bin_sort_visible(self._ws_sort, self.n, self.capacity, self.K, plan.cams[0])
+            c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
+                                         lst, cnt, clear_g2d=True)
         else:
             c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
                                     clear_g2d=True, overwrite=overwrite)

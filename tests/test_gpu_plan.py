@@ -422,3 +422,36 @@ def test_kd_partitions_under_the_plan():
     _check_grads(tr, grads)
     full = oracle.forward(sc.partitions(), cam.as_array(), sc.sh_degree, sc.bg)     # no state at all
     assert np.array_equal(full.image, views[0].image)
+
+
+def test_projection_backward_over_the_visible_list(blocks):
+    """splx_project_backward_list_plan (+= over the binning's list of visible Gaussians) == the dense += call:
+    a culled Gaussian has no gradient, so only the rows touched differ, not the result."""
+    sc = blocks
+    cam = sc.cameras[1]
+    rng = np.random.default_rng(51)
+    a, b = _trainer(sc), _trainer(sc)
+    part = a.participants(1, cam)
+    vop = [0 if (part >> k) & 1 else -1 for k in range(sc.K)]
+    g2d = np.zeros((a.n, 12), np.float32)
+    g2d[:, :9] = rng.standard_normal((a.n, 9))
+    old = rng.standard_normal(a.flat["grad"].shape).astype(np.float32)
+    for tr in (a, b):
+        plan = tr.make_plan([cam], vop, None, True)
+        tr._workspaces(cam)
+        tr.ctx.project_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj)
+        tr.ctx.bin_sort_plan(tr.proj, tr.part_offsets, plan, tr.bins, tr._ws_sort)
+        tr.flat["grad"].copy_(torch.from_numpy(old))
+        tr._plan = plan
+    ga, gb = torch.from_numpy(g2d).cuda(), torch.from_numpy(g2d).cuda()
+    a.ctx.project_backward_plan(a.params, a.part_offsets, a._plan, a.sh_degree, a.proj, ga, a.grads, clear_g2d=True)
+    lst, cnt = b.ctx.bin_sort_visible(b._ws_sort, b.n, b.capacity, b.K, cam)
+    b.ctx.project_backward_list_plan(b.params, b.part_offsets, b._plan, b.sh_degree, b.proj, gb, b.grads, lst, cnt,
+                                     clear_g2d=True)
+    torch.cuda.synchronize()
+    assert torch.equal(a.flat["grad"], b.flat["grad"])
+    assert torch.equal(ga, gb)
+    assert not torch.equal(a.flat["grad"], torch.from_numpy(old).cuda())
+    n_vis = int((b.proj.radius[torch.as_tensor([i for k in range(sc.K) if vop[k] == 0
+                                                  for i in range(b.part_offsets[k], b.part_offsets[k + 1])]).cuda()] > 0).sum())
+    assert 0 < n_vis < b.n
