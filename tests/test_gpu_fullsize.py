@@ -245,3 +245,28 @@ def test_city_10M_pixels_and_gradients_on_sampled_tiles(full_city):
         if vop[k] < 0:
             a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
             assert not tr.grads["mean"][3 * a:3 * b].any()
+
+
+def test_three_pass_slot_sort_bit_exact():
+    """K * tiles > 65 536 slots (K = 16 at 1080p: 17 slot bits) takes three radix passes on the slot bits, as the
+    configs[3] / configs[4] benches do (19 / 18 bits): keys, values and ranges bit-exact against the oracle."""
+    sc = scenes.aerial(n=200_000, grid=(4, 4), log_scale_mu=-1.8, name="aerial_200k_k16")
+    cam = sc.cameras[0]
+    tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=8_000_000)
+    assert tr.K * ((cam.width + 15) // 16) * ((cam.height + 15) // 16) > 65536
+    tr.forward(cam)
+    torch.cuda.synchronize()
+    pr = G.gpu_projected(tr)
+    M, keys, vals, ranges = G.gpu_bins(tr)
+    ntiles = ranges.shape[1]
+    pos = 0
+    for k in range(tr.K):
+        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        ob = oracle.bin_sort(pr.means2d[a:b], pr.radius[a:b], pr.depth[a:b], cam.width, cam.height)
+        assert np.array_equal(keys[pos:pos + ob.M], ob.keys + (np.uint64(k * ntiles) << np.uint64(32))), k
+        assert np.array_equal(vals[pos:pos + ob.M], ob.vals + np.uint32(a)), k
+        live = ob.ranges[:, 1] > ob.ranges[:, 0]
+        assert np.array_equal(ranges[k][live], ob.ranges[live] + np.uint32(pos))
+        assert not ranges[k][~live].any()
+        pos += ob.M
+    assert pos == M and M > 1_000_000
