@@ -69,6 +69,8 @@ class Trainer:
         #: accumulating projection backward over the binning's list of visible Gaussians
         #: (splx_project_backward_list_plan) instead of all rows of the participating partitions
         self.use_visible_list = os.environ.get("SPLX_VISIBLE_LIST", "1") == "1"
+        #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
+        self.pipeline_buckets = os.environ.get("SPLX_PIPELINE", "1") == "1"
         self._cam = None
         self._aabb = None
         self._side = None
@@ -179,6 +181,48 @@ class Trainer:
             self._step_dev = torch.full((1,), self.step_count, dtype=torch.int32, device=dev)
         self.step_count += 1
 
+    def _bufs(self, which=0):
+        """(projected, binning, sort workspace) set `which`: set 1 is the double buffer of the pipelined multi-bucket
+        iteration (the next bucket is projected and binned while the current one is blended)."""
+        if which == 0:
+            return self.proj, self.bins, self._ws_sort
+        if getattr(self, "_alt", None) is None:
+            dev = self.ctx.device
+            self._alt = (binding.Projected(self.n, dev), binding.Binning(self.capacity, self.K, self.W, self.H, dev),
+                         torch.empty_like(self._ws_sort))
+        return self._alt
+
+    def _front(self, plan, bufs):
+        """a1-a4 of a bucket: project, bin/sort."""
+        proj, bins, ws = bufs
+        self.ctx.project_plan(self.params, self.part_offsets, plan, self.sh_degree, proj)
+        self.ctx.bin_sort_plan(proj, self.part_offsets, plan, bins, ws)
+
+    def _back(self, plan, bufs, targets, overwrite, sat_eps, tile_state_out, adam, n_views):
+        """a5-a10 of a bucket: render, fused composition + loss + composition backward, raster and projection backward."""
+        proj, bins, ws = bufs
+        c = self.ctx
+        images, T_totals, _ = self._view_buffers(plan.B)
+        g_ct, g2d = self.fused_buffers()
+        c.render_partial_plan(proj, bins, plan, self.partials)
+        c.compose_l1_backward_plan(self.partials, bins, plan, self.bg, targets, images, T_totals, self.loss_sum, g_ct,
+                                   scale=float(plan.B), sat_eps=sat_eps if sat_eps is not None else 0.0,
+                                   tile_state_out=tile_state_out)
+        c.raster_backward_plan(proj, bins, plan, self.partials, g_ct, g2d)
+        if adam:     # the last backward of the iteration takes the optimiser step too (call prepare_adam() first)
+            c.adam_bias_step(self._step_dev, self._bc_dev)
+            c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
+                                         self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev,
+                                         grad_scale=1.0 / n_views, clear_g2d=True, overwrite=overwrite)
+        elif not overwrite and self.use_visible_list:   # an accumulating launch over the binning's visible list only
+            lst, cnt = c.bin_sort_visible(ws, self.n, self.capacity, self.K, plan.cams[0])
+            c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
+                                         lst, cnt, clear_g2d=True)
+        else:
+            c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
+                                    clear_g2d=True, overwrite=overwrite)
+        return images
+
     def iteration_fused(self, plan: binding.Plan, targets, overwrite=True, sat_eps=None, tile_state_out=None, adam=False,
                         n_views=1):
         """a1-a10 under a plan with composition, mean-L1 loss and composition backward in ONE kernel
@@ -186,29 +230,9 @@ class Trainer:
         targets: device [B,H,W,3].  Returns images[B,H,W,3]."""
         self._workspaces(plan.cams[0])
         self._plan = plan
-        c = self.ctx
-        images, T_totals, _ = self._view_buffers(plan.B)
-        g_ct, g2d = self.fused_buffers()
-        c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
-        c.bin_sort_plan(self.proj, self.part_offsets, plan, self.bins, self._ws_sort)
-        c.render_partial_plan(self.proj, self.bins, plan, self.partials)
-        c.compose_l1_backward_plan(self.partials, self.bins, plan, self.bg, targets, images, T_totals, self.loss_sum, g_ct,
-                                   scale=float(plan.B), sat_eps=sat_eps if sat_eps is not None else 0.0,
-                                   tile_state_out=tile_state_out)
-        c.raster_backward_plan(self.proj, self.bins, plan, self.partials, g_ct, g2d)
-        if adam:     # the last backward of the iteration takes the optimiser step too (call prepare_adam() first)
-            c.adam_bias_step(self._step_dev, self._bc_dev)
-            c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                         self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev,
-                                         grad_scale=1.0 / n_views, clear_g2d=True, overwrite=overwrite)
-        elif not overwrite and self.use_visible_list:   # an accumulating launch over the binning's visible list only
-            lst, cnt = c.bin_sort_visible(self._ws_sort, self.n, self.capacity, self.K, plan.cams[0])
-            c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                         lst, cnt, clear_g2d=True)
-        else:
-            c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                    clear_g2d=True, overwrite=overwrite)
-        return images
+        bufs = self._bufs(0)
+        self._front(plan, bufs)
+        return self._back(plan, bufs, targets, overwrite, sat_eps, tile_state_out, adam, n_views)
 
     def loss_grad_plan(self, targets):
         """a7 for B views at once: targets[B,H,W,3]; every view's loss is its own mean (scale = B)."""
@@ -279,11 +303,44 @@ class Trainer:
         groups = self.buckets(view_ids, cams, consolidate)
         if self.fuse_adam:
             self.prepare_adam()
-        for gi, grp in enumerate(groups):
-            plan, state_out = self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse)
-            tg = targets[grp[0]:grp[0] + 1] if len(grp) == 1 else targets[torch.as_tensor(grp, device=targets.device)]
-            self.iteration_fused(plan, tg, overwrite=(gi == 0), sat_eps=sat_eps, tile_state_out=state_out,
-                                 adam=(self.fuse_adam and gi == len(groups) - 1), n_views=len(view_ids))
+        G = len(groups)
+        plans = [self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse) for grp in groups]
+        tgs = [targets[grp[0]:grp[0] + 1] if len(grp) == 1 else targets[torch.as_tensor(grp, device=targets.device)]
+               for grp in groups]
+        self._workspaces(cams[0])
+        if G == 1 or not self.pipeline_buckets:
+            for gi in range(G):
+                self.iteration_fused(plans[gi][0], tgs[gi], overwrite=(gi == 0), sat_eps=sat_eps, tile_state_out=plans[gi][1],
+                                     adam=(self.fuse_adam and gi == G - 1), n_views=len(view_ids))
+        else:
+            # Two streams, double-buffered projected / binning sets: bucket g+1 is projected and sorted (latency-bound
+            # kernels that leave most of the SMs idle) on the side stream while bucket g is blended on the main one.
+            dev = self.ctx.device
+            main = torch.cuda.current_stream(dev)
+            if getattr(self, "_front_stream", None) is None:
+                self._front_stream = torch.cuda.Stream(dev)
+            side = self._front_stream
+            ev_front = [torch.cuda.Event() for _ in range(G)]
+            ev_back = [torch.cuda.Event() for _ in range(G)]
+            side.wait_stream(main)                       # the parameters of the previous optimiser step
+            self.ctx.set_stream(side.cuda_stream)
+            self._front(plans[0][0], self._bufs(0))
+            ev_front[0].record(side)
+            self.ctx.set_stream(main.cuda_stream)
+            for gi in range(G):
+                if gi + 1 < G:
+                    if gi >= 1:
+                        side.wait_event(ev_back[gi - 1])  # buffer set (gi + 1) % 2 was last read by the back half of gi - 1
+                    self.ctx.set_stream(side.cuda_stream)
+                    self._front(plans[gi + 1][0], self._bufs((gi + 1) % 2))
+                    ev_front[gi + 1].record(side)
+                    self.ctx.set_stream(main.cuda_stream)
+                main.wait_event(ev_front[gi])
+                self._plan = plans[gi][0]
+                self._back(plans[gi][0], self._bufs(gi % 2), tgs[gi], gi == 0, sat_eps, plans[gi][1],
+                           self.fuse_adam and gi == G - 1, len(view_ids))
+                ev_back[gi].record(main)
+            side.wait_stream(main)
         if not self.fuse_adam:
             self.adam_step(len(view_ids))
         return len(groups)
