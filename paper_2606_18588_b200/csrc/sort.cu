@@ -446,12 +446,22 @@ int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, ui
 }
 
 // ------------------------------------------------------------------------- key emission --
+// Two kernels hand out the work in two ways; both are launched and the device-side counts decide which one works
+// (the other returns at once -- the host does not know M):
+//  * k_emit_keys, by Gaussian (a warp writes the 32 adjacent runs of its 32 Gaussians): cheapest when footprints are
+//    small and alike (aerial views: 3-12 tiles per Gaussian);
+//  * k_emit_keys_lb, by output position: when the mean footprint is large the sizes are very unequal as well
+//    (street-level views: a few Gaussians next to each other at the head of the depth order cover thousands of tiles
+//    each) and the first scheme leaves a handful of CTAs with all the work (1.5 ms on street_10M against 0.2 ms).
+__device__ __forceinline__ bool emit_by_output(const Counters* cnt) { return cnt->m_total > 16 * cnt->n_visible; }
+
 __global__ void __launch_bounds__(256)
 k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
             uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
             uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+  if (emit_by_output(cnt)) return;
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
   __shared__ uint32_t s_hist[MAX_PASSES * 256];
@@ -517,6 +527,96 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
         atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
     }
   }
+  }
+  __syncthreads();
+  for (int x = threadIdx.x; x < plan.npass * 256; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
+}
+
+__global__ void __launch_bounds__(256)
+k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
+            const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
+            const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
+            uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
+            uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+  if (!emit_by_output(cnt)) return;
+  // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
+  // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
+  __shared__ uint32_t s_hist[MAX_PASSES * 256];
+  for (int x = threadIdx.x; x < MAX_PASSES * 256; x += blockDim.x) s_hist[x] = 0;
+  {
+    const uint64_t words = ((cnt->m_sorted + RS_TILE - 1) / RS_TILE) * 256;
+    for (int p = 0; p < plan.npass; ++p)
+      for (uint64_t x = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; x < words; x += (uint64_t)gridDim.x * blockDim.x)
+        rstatus[(size_t)p * rstride + x] = 0;
+  }
+  __syncthreads();
+  // Load-balanced by OUTPUT position: a CTA produces tiles of EK_TILE consecutive keys, whatever the sizes of the
+  // footprints they belong to (street-level views put a few Gaussians that cover thousands of tiles next to each
+  // other at the head of the depth order: partitioning by Gaussian left a handful of CTAs with all the work,
+  // 1.5 ms on street_10M).  Per tile: a 256-ary search over offs finds the first owner, the owners' run starts and
+  // rectangles are staged in shared memory, every thread places EK_IPT keys by a binary search over the staged starts.
+  constexpr int EK_TILE = 1024, EK_IPT = EK_TILE / 256;
+  __shared__ uint32_t s_off[EK_TILE + 1], s_xy[EK_TILE + 1], s_w[EK_TILE + 1], s_slot0[EK_TILE + 1], s_db[EK_TILE + 1],
+      s_gi[EK_TILE + 1];
+  __shared__ uint32_t s_nown;
+  const uint64_t nvis = cnt->n_visible;
+  const uint64_t m = cnt->m_sorted;                       // min(M, capacity): positions beyond the capacity are dropped
+  for (uint64_t begin = (uint64_t)blockIdx.x * EK_TILE; begin < m; begin += (uint64_t)gridDim.x * EK_TILE) {
+    const uint64_t end = begin + EK_TILE < m ? begin + EK_TILE : m;
+    // last j with offs[j] <= begin (offs is strictly increasing, offs[0] == 0)
+    uint64_t lo = 0, hi = nvis;
+    while (hi - lo > 1) {
+      const uint64_t step = (hi - lo + 255) / 256;
+      const uint64_t pidx = lo + (uint64_t)threadIdx.x * step;
+      const bool ok = pidx < hi && (uint64_t)offs[pidx] <= begin;
+      const int c = __syncthreads_count(ok);             // the trues are a prefix; thread 0 is always true
+      lo = lo + (uint64_t)(c - 1) * step;
+      hi = lo + step < hi ? lo + step : hi;
+    }
+    const uint64_t j0 = lo;
+    if (threadIdx.x == 0) s_nown = 0;
+    __syncthreads();
+    // stage the owners j0, j0 + 1, ... whose runs start before `end` (at most EK_TILE + 1 of them)
+    for (int q = threadIdx.x; q <= EK_TILE; q += 256) {
+      const uint64_t j = j0 + q;
+      uint32_t o = 0xffffffffu;
+      if (j < nvis) o = offs[j];
+      if (j < nvis && (uint64_t)o < end) {
+        const uint32_t i = cvals[j];
+        const float2 mm = *reinterpret_cast<const float2*>(means2d + 2 * (uint64_t)i);
+        int x0, y0, x1, y1;
+        tile_rect(mm.x, mm.y, radius[i], TX, TY, x0, y0, x1, y1);
+        int plo = 0, phi = parts.K - 1;                   // partition of Gaussian i: last k with off[k] <= i
+        while (plo < phi) {
+          const int mid = (plo + phi + 1) >> 1;
+          if (parts.off[mid] <= (int64_t)i) plo = mid; else phi = mid - 1;
+        }
+        s_off[q] = o; s_xy[q] = ((uint32_t)y0 << 16) | (uint32_t)x0; s_w[q] = (uint32_t)(x1 - x0);
+        s_slot0[q] = (uint32_t)plo * (uint32_t)(TX * TY); s_db[q] = ckeys[j]; s_gi[q] = i;
+        atomicMax(&s_nown, (uint32_t)q + 1);
+      }
+    }
+    __syncthreads();
+    const uint32_t nown = s_nown;
+#pragma unroll
+    for (int k = 0; k < EK_IPT; ++k) {
+      const uint64_t pos = begin + (uint64_t)k * 256 + threadIdx.x;
+      if (pos < end) {
+        uint32_t ql = 0, qh = nown - 1;                   // last staged owner whose run starts at or before pos
+        while (ql < qh) {
+          const uint32_t mid = (ql + qh + 1) >> 1;
+          if ((uint64_t)s_off[mid] <= pos) ql = mid; else qh = mid - 1;
+        }
+        const uint32_t t = (uint32_t)(pos - s_off[ql]), w = s_w[ql], xy = s_xy[ql];
+        const uint32_t ty = t / w;
+        const uint32_t slot = s_slot0[ql] + ((xy >> 16) + ty) * (uint32_t)TX + (xy & 0xffffu) + (t - ty * w);
+        keys[pos] = ((uint64_t)slot << 32) | s_db[ql];
+        vals[pos] = s_gi[ql];
+        for (int p = 0; p < plan.npass; ++p)
+          atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
+      }
+    }
+    __syncthreads();
   }
   __syncthreads();
   for (int x = threadIdx.x; x < plan.npass * 256; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
@@ -649,6 +749,12 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
       plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
       (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
+  const uint64_t emit_tiles = (out->capacity + 1023) / 1024;     // output tiles of 1024 keys
+  k_emit_keys_lb<<<(unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
+      pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0,
+      plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
+      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256);
+  SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
   // 4. stable sort on the slot bits
   if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
                                  (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6], true))) return rc;
