@@ -13,10 +13,20 @@ from tests import gpu_common as G
 
 pytestmark = pytest.mark.gpu
 
+def _big_footprints():
+    """Footprints of ~20-60 tiles (mean > 16): takes the load-balanced key emission (k_emit_keys_lb) of street-level views."""
+    sc = scenes.tiny(n=700, size=176, f=200.0, K=3, sh_degree=1, seed=4)
+    sc.params["log_scale"] = (sc.params["log_scale"] + 1.6).astype(np.float32)
+    sc.params["opacity_logit"] = (sc.params["opacity_logit"] - 2.0).astype(np.float32)
+    sc.name = "tiny_big_footprints"
+    return sc
+
+
 SCENES = {
     "tiny": lambda: scenes.tiny(),                              # BASELINE configs[0]
     "aerial_small": lambda: scenes.small_aerial(),              # configs[1] recipe, ragged 320x176, K=4, SH3
     "tiny_k5_sh2": lambda: scenes.tiny(n=3000, size=72, f=84.0, K=5, sh_degree=2, seed=3),  # ragged both ways
+    "big_footprints": _big_footprints,
 }
 
 
@@ -104,6 +114,8 @@ def test_a1_projection(run):
 
 def test_a2_a4_binning_bit_exact(run):
     pr = run.proj
+    if run.sc.name == "tiny_big_footprints":
+        assert run.M > 16 * (pr.radius > 0).sum(), "this scene must take the load-balanced emission path"
     # teacher-forced: counts from the GPU's own (means2d, radius)
     M_ref, tt_ref = oracle.count_tiles(pr.means2d, pr.radius, run.W, run.H)
     assert np.array_equal(pr.tiles_touched, tt_ref)
