@@ -479,3 +479,32 @@ def test_pipelined_buckets_equal_the_sequential_iteration(city):
     assert close.float().mean().item() > 0.999
     for k in out[0][2]:
         assert (out[0][2][k] != out[1][2][k]).float().mean().item() < 1e-3, k     # a slot within rounding of eps may flip
+
+
+def test_iteration_views_gradients_against_the_oracle(blocks):
+    """A whole multi-bucket iteration (two consolidated two-view buckets + two single views; first bucket '=', later
+    buckets '+=' over the visible list with per-row cameras; pipelined over two streams): the accumulated gradient
+    against the sum of the oracle's plan iterations."""
+    sc = blocks
+    tr = _trainer(sc)
+    tr.lr = {k: 0.0 for k in tr.lr}
+    ids = list(range(len(sc.cameras)))
+    targets = torch.from_numpy(np.stack(sc.targets)).cuda()
+    groups = tr.buckets(ids, sc.cameras)
+    assert any(len(g) > 1 for g in groups[1:]), "a consolidated bucket must take the accumulating path"
+    tr.iteration_views(ids, sc.cameras, targets, saturation=False)
+    torch.cuda.synchronize()
+    total = None
+    for grp in groups:
+        cams = [sc.cameras[i] for i in grp]
+        plan, _ = tr.bucket_plan(grp, cams, saturation=False)
+        state = G.np32(plan.tile_state).reshape(sc.K, -1)
+        _, grads = ov.iteration_plan(sc.partitions(), [c.as_array() for c in cams], plan.view_of_part, sc.sh_degree,
+                                     [sc.targets[i] for i in grp], sc.bg, tile_state=state)
+        if total is None:
+            total = grads
+        else:
+            for k in range(sc.K):
+                for key in scenes.PARAM_KEYS:
+                    total[k][key] = total[k][key] + grads[k][key]
+    _check_grads(tr, total)
