@@ -231,7 +231,7 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 #define SPLX_STAGE_ITEMS 7
 #endif
 #ifndef SPLX_BWD_MIN_CTAS
-#define SPLX_BWD_MIN_CTAS 10   /* 92 registers; higher occupancy targets measured slower (profiles/r01c) */
+#define SPLX_BWD_MIN_CTAS 10   /* 92 registers; 12 and 14 CTAs/SM with a 3-item stage measured slower */
 #endif
 constexpr int STAGE_ITEMS = SPLX_STAGE_ITEMS;
 constexpr int STAGE_ROUNDS = (STAGE_ITEMS * 9 + 31) / 32;

@@ -82,7 +82,7 @@ __device__ __forceinline__ uint64_t lookback(uint64_t* status, uint32_t t, uint3
 }
 
 // ---------------------------------------------------------------- generic exclusive scan --
-// One launch: tiles of 4096 values, chained by look-back.  Op supplies count(), load(i) and
+// One launch: tiles of 8192 values, chained by look-back.  Op supplies count(), load(i) and
 // store(i, value, exclusive_prefix).  The grand total goes to *total_out (and, clamped, to *clamp_out).
 
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* smem /*>=33*/, uint32_t& total) {
@@ -252,7 +252,7 @@ static PassPlan plan_passes(int begin_bit, int end_bit) {
 
 // Lanes of the warp whose 8-bit digit equals this lane's, among the lanes of `vm`: eight ballots.
 // (Constant cost; the hardware MATCH.ANY serialises over the distinct values and the shared-memory
-// atomic unit over the lanes -- profiles/r01c.)
+// atomic unit over the lanes: measured mid-round.)
 __device__ __forceinline__ unsigned digit_peers(uint32_t d, unsigned vm) {
   unsigned peers = vm;
 #pragma unroll
