@@ -479,6 +479,7 @@ def run_views(args):
     aabbs = scenes.partition_aabbs(sc.params, sc.part_offsets)
     sc.params = None                                   # a device-generated scene: release the generator's copy
     torch.cuda.empty_cache()
+    tr.sparse_adam = bool(args.sparse_adam)
     if args.no_visibility:   # boxes that contain everything: every partition participates in every view, no tile is invisible
         big = np.float32(1e6)
         tr.set_aabbs(np.full((tr.K, 3), -big), np.full((tr.K, 3), big))
@@ -517,6 +518,7 @@ def run_views(args):
                 config=dict(workload=args.workload, gaussians=tr.n, K=tr.K, width=W, height=H, sh_degree=sc.sh_degree,
                             views_per_step=B, visibility_prediction=not args.no_visibility,
                             consolidation=not args.no_consolidate, saturation_skipping=bool(args.saturation),
+                            optimiser="visible-only Adam (option, not the paper's)" if args.sparse_adam else "dense Adam",
                             sat_eps=args.sat_eps, participants=[bin(p) for p in parts], buckets=groups,
                             tile_state=skipped, intersections_last_bucket=M,
                             l2="working set (params+grads+moments) is larger than the 126 MB L2"),
@@ -540,6 +542,8 @@ def main():
     ap.add_argument("--views", type=int, default=0, help="B > 0: time iterations over B views (optional subsystems)")
     ap.add_argument("--no-visibility", action="store_true")
     ap.add_argument("--no-consolidate", action="store_true")
+    ap.add_argument("--sparse-adam", action="store_true",
+                    help="--views only: visible-only Adam (an option outside the paper, DESIGN.md s31)")
     args = ap.parse_args()
     if args.impl == "reference":
         args.steps = 2 if args.steps is None else min(args.steps, 4)

@@ -315,7 +315,18 @@ int splx_bin_sort_visible(const void *ws, int64_t n, uint64_t capacity, int K, c
 int splx_project_backward_list_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                                     const splx_plan *plan, int sh_degree, const splx_projected *proj,
                                     float *g2d, int flags, const splx_gaussian_grads *grads,
-                                    const uint32_t *visible, const uint64_t *num_visible);
+                                    const uint32_t *visible, const uint64_t *num_visible, uint8_t *touched);
+/* touched (device uint8[n], may be NULL): the flags of the visible-only optimiser.  A row whose flag is clear has no
+ * gradient yet in this iteration: the call STORES its gradient (whatever the row held) and sets the flag; a row whose
+ * flag is set is accumulated into.  With it no gradient buffer is ever zeroed or overwritten wholesale.
+ *
+ * splx_adam_sparse -- an OPTION outside the paper (it changes the optimiser: DESIGN.md s31): the Adam step of
+ * splx_adam on the Gaussians whose flag is set only, all 59 parameters of a row with the learning rate of their
+ * group (lr: HOST float[5] for mean, log_scale, quat, opacity_logit, sh); the others keep parameters and both
+ * moments unchanged.  Clears the flags it consumes.  step is 1-based and global (bias correction as splx_adam). */
+int splx_adam_sparse(splx_ctx *ctx, const splx_gaussian_grads *params, const splx_gaussian_grads *grads,
+                     const splx_gaussian_grads *m, const splx_gaussian_grads *v, uint8_t *touched,
+                     const float lr[5], float beta1, float beta2, float eps, int step, float grad_scale);
 /* a10 + a11 fused: the LAST projection backward of an iteration also takes the Adam step of splx_adam on every
  * row of every partition (participating or not), reading the gradient it has just formed -- plus, without
  * SPLX_PB_OVERWRITE, the gradient earlier launches of the iteration left in `grads` -- instead of storing it:

@@ -205,3 +205,14 @@ def iteration_plan(parts, cams, view_of_part, sh_degree, targets, bg=(0.0, 0.0, 
             grads[k] = dict(mean=np.zeros((n, 3)), log_scale=np.zeros((n, 3)), quat=np.zeros((n, 4)),
                             opacity_logit=np.zeros(n), sh=np.zeros((n, 16, 3)))
     return views, grads
+
+
+def adam_rows(param, grad, m, v, rows, lr, beta1=0.9, beta2=0.999, eps=1e-15, step=1):
+    """Visible-only Adam (an option OUTSIDE the paper, SURVEY.md s8(f) NEXT 4 / DESIGN.md s31): the Adam step of
+    ``oracle.adam`` on the boolean-selected ``rows`` of [n, w] float64 arrays, in place; the other rows keep their
+    parameters and both moments (no decay).  The bias correction uses the global ``step``."""
+    from . import adam
+    rows = np.asarray(rows, bool)
+    p = np.ascontiguousarray(param[rows]); mm = np.ascontiguousarray(m[rows]); vv = np.ascontiguousarray(v[rows])
+    adam(p.reshape(-1), np.ascontiguousarray(grad[rows]).reshape(-1), mm.reshape(-1), vv.reshape(-1), lr, beta1, beta2, eps, step)
+    param[rows] = p; m[rows] = mm; v[rows] = vv

@@ -33,7 +33,7 @@ EXPORTS = [
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
     "splx_compose_l1_backward_plan", "splx_project_backward_adam_plan", "splx_adam_bias_step",
-    "splx_bin_sort_visible", "splx_project_backward_list_plan",
+    "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -143,7 +143,8 @@ def lib():
                                                       C.c_float, C.c_float, C.c_float, vp, C.c_float]
         L.splx_adam_bias_step.argtypes = [vp, C.c_float, C.c_float, vp, vp]
         L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
-        L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp]
+        L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp]
+        L.splx_adam_sparse.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float]
         _lib = L
     return _lib
 
@@ -484,11 +485,19 @@ class Context:
         return lst.value, cnt.value
 
     def project_backward_list_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
-                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False):
+                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False, touched=None):
         g, gg, ps = gaussians_struct(params), gaussians_struct(grads), proj.struct()
         self._check(lib().splx_project_backward_list_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
                                                           sh_degree, C.byref(ps), _ptr(g2d), PB_CLEAR_G2D if clear_g2d else 0,
-                                                          C.byref(gg), C.c_void_p(visible_ptr), C.c_void_p(count_ptr)))
+                                                          C.byref(gg), C.c_void_p(visible_ptr), C.c_void_p(count_ptr),
+                                                          _ptr(touched)))
+
+    def adam_sparse(self, params: dict, grads: dict, m: dict, v: dict, touched, lrs, beta1=0.9, beta2=0.999, eps=1e-15,
+                    step=1, grad_scale=1.0):
+        sets = [gaussians_struct(x) for x in (params, grads, m, v)]
+        lr = (C.c_float * 5)(*[float(x) for x in lrs])
+        self._check(lib().splx_adam_sparse(self._h, C.byref(sets[0]), C.byref(sets[1]), C.byref(sets[2]), C.byref(sets[3]),
+                                           _ptr(touched), lr, beta1, beta2, eps, int(step), float(grad_scale)))
 
     def adam_bias_step(self, step_dev, bias_corr, beta1=0.9, beta2=0.999):
         self._check(lib().splx_adam_bias_step(self._h, beta1, beta2, _ptr(step_dev), _ptr(bias_corr)))

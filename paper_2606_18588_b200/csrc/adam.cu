@@ -73,6 +73,60 @@ k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __rest
   }
 }
 
+// Visible-only ("sparse") Adam, an OPTION outside the paper: only Gaussians whose flag is set
+// -- they received a gradient in this iteration -- take the step, the others keep parameters AND moments untouched
+// (no decay); the flags are cleared on the way.  A block owns 128 consecutive Gaussians: it reads their 128 flag
+// bytes and walks the five parameter groups in coalesced 16-byte chunks, touching only flagged rows (a row's 48 SH
+// floats are 192 contiguous bytes).  A block without a flagged row leaves after the flag load.
+constexpr int SB = 128;
+struct SparseSets { float *p[5], *g[5], *m[5], *v[5]; float lr[5]; };
+
+__device__ __forceinline__ void adam4(float* pp, const float* pg, float* pm, float* pv, const AdamK& k, float lr, float gs) {
+  float4 p = *reinterpret_cast<float4*>(pp), g = *reinterpret_cast<const float4*>(pg);
+  float4 m = *reinterpret_cast<float4*>(pm), v = *reinterpret_cast<float4*>(pv);
+  AdamK kk = k; kk.lr = lr;
+  adam1(p.x, g.x * gs, m.x, v.x, kk); adam1(p.y, g.y * gs, m.y, v.y, kk);
+  adam1(p.z, g.z * gs, m.z, v.z, kk); adam1(p.w, g.w * gs, m.w, v.w, kk);
+  *reinterpret_cast<float4*>(pp) = p; *reinterpret_cast<float4*>(pm) = m; *reinterpret_cast<float4*>(pv) = v;
+}
+__device__ __forceinline__ void adam_s(float* pp, const float* pg, float* pm, float* pv, const AdamK& k, float lr, float gs) {
+  float p = *pp, m = *pm, v = *pv;
+  AdamK kk = k; kk.lr = lr;
+  adam1(p, *pg * gs, m, v, kk);
+  *pp = p; *pm = m; *pv = v;
+}
+
+__global__ void __launch_bounds__(SB)
+k_adam_sparse(const __grid_constant__ SparseSets S, uint8_t* __restrict__ touched, int64_t n, AdamK k, float gs) {
+  __shared__ uint8_t s_t[SB];
+  const int64_t base = (int64_t)blockIdx.x * SB;
+  const int64_t i = base + threadIdx.x;
+  const uint8_t t = i < n ? touched[i] : (uint8_t)0;
+  s_t[threadIdx.x] = t;
+  if (!__syncthreads_or(t)) return;
+  if (t) touched[i] = 0;
+  const int nrows = (int)min((int64_t)SB, n - base);
+  // sh: 12 float4 per row
+#pragma unroll 4
+  for (int c = 0; c < 12; ++c) {
+    const int q = c * SB + threadIdx.x;
+    const int row = q / 12, c4 = q - row * 12;
+    if (row < nrows && s_t[row]) {
+      const int64_t off = 48 * (base + row) + 4 * c4;
+      adam4(S.p[4] + off, S.g[4] + off, S.m[4] + off, S.v[4] + off, k, S.lr[4], gs);
+    }
+  }
+  if (t) {
+    adam4(S.p[2] + 4 * i, S.g[2] + 4 * i, S.m[2] + 4 * i, S.v[2] + 4 * i, k, S.lr[2], gs);      // quat
+    adam_s(S.p[3] + i, S.g[3] + i, S.m[3] + i, S.v[3] + i, k, S.lr[3], gs);                     // opacity logit
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      adam_s(S.p[0] + 3 * i + c, S.g[0] + 3 * i + c, S.m[0] + 3 * i + c, S.v[0] + 3 * i + c, k, S.lr[0], gs);   // mean
+      adam_s(S.p[1] + 3 * i + c, S.g[1] + 3 * i + c, S.m[1] + 3 * i + c, S.v[1] + 3 * i + c, k, S.lr[1], gs);   // log scale
+    }
+  }
+}
+
 // Device-resident step counter of the fused optimiser path: t = ++(*step); bc = 1/(1-b1^t), 1/(1-b2^t) formed in
 // double as launch_adam does on the host.  One thread; lives inside captured CUDA graphs, where a host-side step
 // number would be frozen at capture time.
@@ -84,6 +138,27 @@ __global__ void k_adam_bias_step(int32_t* step, float* bc, double b1, double b2)
 }
 
 }  // namespace
+
+int launch_adam_sparse(splx_ctx* ctx, const splx_gaussian_grads* P, const splx_gaussian_grads* Gr,
+                       const splx_gaussian_grads* M, const splx_gaussian_grads* V, uint8_t* touched, const float* lr,
+                       float beta1, float beta2, float eps, int step, float grad_scale) {
+  const int64_t n = P->n;
+  if (n <= 0) return SPLX_OK;
+  const double bc1 = 1.0 - pow((double)beta1, step), bc2 = 1.0 - pow((double)beta2, step);
+  const AdamK k{0.f, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps,
+                (float)(1.0 / bc1), (float)(1.0 / bc2)};
+  SparseSets S;
+  const splx_gaussian_grads* sets[4] = {P, Gr, M, V};
+  float** dst[4] = {S.p, S.g, S.m, S.v};
+  for (int a = 0; a < 4; ++a) {
+    dst[a][0] = sets[a]->mean; dst[a][1] = sets[a]->log_scale; dst[a][2] = sets[a]->quat;
+    dst[a][3] = sets[a]->opacity_logit; dst[a][4] = sets[a]->sh;
+  }
+  for (int j = 0; j < 5; ++j) S.lr[j] = lr[j];
+  k_adam_sparse<<<(unsigned)((n + SB - 1) / SB), SB, 0, ctx->stream>>>(S, touched, n, k, grad_scale);
+  SPLX_LAUNCH_CHECK(ctx, "k_adam_sparse");
+  return SPLX_OK;
+}
 
 int launch_adam_bias_step(splx_ctx* ctx, float beta1, float beta2, int32_t* step_dev, float* bias_corr) {
   k_adam_bias_step<<<1, 1, 0, ctx->stream>>>(step_dev, bias_corr, (double)beta1, (double)beta2);

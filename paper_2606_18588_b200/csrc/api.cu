@@ -306,7 +306,7 @@ int splx_project_backward_plan(splx_ctx* ctx, const splx_gaussians* g, int K, co
   int rc;
   if ((rc = make_plan(ctx, "splx_project_backward", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: part_offsets must run monotonically from 0 to n");
-  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, nullptr, nullptr);
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, nullptr, nullptr, nullptr);
 }
 
 int splx_bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, const splx_camera* cam,
@@ -318,7 +318,8 @@ int splx_bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, c
 
 int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets,
                                     const splx_plan* plan, int sh_degree, const splx_projected* proj, float* g2d, int flags,
-                                    const splx_gaussian_grads* grads, const uint32_t* visible, const uint64_t* num_visible) {
+                                    const splx_gaussian_grads* grads, const uint32_t* visible, const uint64_t* num_visible,
+                                    uint8_t* touched) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (!visible || !num_visible) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: visible list is NULL");
   if (flags & SPLX_PB_OVERWRITE) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: accumulates only (no SPLX_PB_OVERWRITE)");
@@ -334,7 +335,7 @@ int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int 
   int rc;
   if ((rc = make_plan(ctx, "splx_project_backward_list", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: part_offsets must run monotonically from 0 to n");
-  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, visible, num_visible);
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, visible, num_visible, touched);
 }
 
 int splx_project_backward_adam_plan(splx_ctx* ctx, const splx_gaussian_grads* params, int K, const int64_t* part_offsets,
@@ -368,7 +369,7 @@ int splx_project_backward_adam_plan(splx_ctx* ctx, const splx_gaussian_grads* pa
   af.omb1 = (float)(1.0 - (double)beta1); af.omb2 = (float)(1.0 - (double)beta2);   // as splx_adam forms them
   af.eps = eps; af.gscale = grad_scale; af.bc = bias_corr;
   const splx_gaussians g{params->mean, params->log_scale, params->quat, params->opacity_logit, params->sh, params->n};
-  return launch_project_bwd(ctx, &g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, &af, nullptr, nullptr);
+  return launch_project_bwd(ctx, &g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, &af, nullptr, nullptr, nullptr);
 }
 
 int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
@@ -427,6 +428,20 @@ int splx_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx
   for (int k = 1; k <= K; ++k) po[k] = g->n;
   return splx_backward_plan(ctx, K, po, &sp.plan, partials, bg, dL_dimage, dL_dT_total, g, proj, bins, sh_degree, grads,
                             ws, ws_bytes, flags);
+}
+
+int splx_adam_sparse(splx_ctx* ctx, const splx_gaussian_grads* params, const splx_gaussian_grads* grads,
+                     const splx_gaussian_grads* m, const splx_gaussian_grads* v, uint8_t* touched, const float lr[5],
+                     float beta1, float beta2, float eps, int step, float grad_scale) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!params || !grads || !m || !v || !touched || !lr || step < 1)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_sparse: null argument or step < 1");
+  const splx_gaussian_grads* sets[4] = {params, grads, m, v};
+  for (const splx_gaussian_grads* s : sets)
+    if (s->n != params->n || (s->n > 0 && (!s->mean || !s->log_scale || !s->quat || !s->opacity_logit || !s->sh ||
+                                           !aligned16(s->quat) || !aligned16(s->sh))))
+      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_sparse: params, grads, m, v must be four sets of n rows (quat, sh 16-byte aligned)");
+  return launch_adam_sparse(ctx, params, grads, m, v, touched, lr, beta1, beta2, eps, step, grad_scale);
 }
 
 int splx_adam_bias_step(splx_ctx* ctx, float beta1, float beta2, int32_t* step_dev, float* bias_corr) {

@@ -139,7 +139,10 @@ int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const i
                        const splx_projected*);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*, const AdamFuse* adam,
-                       const uint32_t* visible_list, const uint64_t* num_visible);
+                       const uint32_t* visible_list, const uint64_t* num_visible, uint8_t* touched);
+int launch_adam_sparse(splx_ctx*, const splx_gaussian_grads* params, const splx_gaussian_grads* grads,
+                       const splx_gaussian_grads* m, const splx_gaussian_grads* v, uint8_t* touched, const float* lr,
+                       float beta1, float beta2, float eps, int step, float grad_scale);
 // the depth-sorted list of visible Gaussians a bin_sort leaves in its workspace, and its device-side count
 int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX, int TY, const uint32_t** list,
                      const uint64_t** count);

@@ -283,7 +283,8 @@ template <int DEG, bool ACC, bool ADAM, bool LIST>
 __global__ void __launch_bounds__(PB_THREADS, SPLX_PB_MIN_CTAS)
 k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out,
-              const __grid_constant__ AdamFuse af, const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr) {
+              const __grid_constant__ AdamFuse af, const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr,
+              uint8_t* __restrict__ touched) {
   extern __shared__ __align__(16) float s_dyn[];
   float* s_sh = s_dyn;                                   // [128][52] sh in, SH gradient out
   float* s_old = s_dyn + PB_THREADS * PB_STRIDE;         // [128][52] previous SH gradient (ACC only)
@@ -291,6 +292,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   __shared__ __align__(16) float s_s[PB_THREADS * 3];    // log_scale gradient tile
   __shared__ uint8_t s_vis[PB_THREADS];
   __shared__ int64_t s_idx[PB_THREADS];                  // Gaussian of each row of the block
+  __shared__ uint8_t s_fresh[PB_THREADS];                // LIST + touched: first gradient of this row in the iteration ("=")
   const uint64_t nvis = LIST ? *nvis_ptr : 0;
   for (uint64_t blk = blockIdx.x; LIST ? (blk * PB_THREADS < nvis) : (blk == blockIdx.x); blk += gridDim.x) {
   int64_t base = 0, run_end = 0, i = 0;
@@ -340,6 +342,14 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   }
   const bool vis = inr && rad > 0;
   s_vis[threadIdx.x] = vis ? 1 : 0;
+  // sparse-optimiser mode: a row whose flag is still clear has no gradient yet in this iteration: its old content is
+  // garbage, this launch stores instead of accumulating and sets the flag (a list holds a Gaussian once: no race)
+  bool fresh = false;
+  if (LIST && touched != nullptr && vis) {
+    fresh = touched[i] == 0;
+    touched[i] = 1;
+  }
+  s_fresh[threadIdx.x] = fresh ? 1 : 0;
   __syncthreads();
 #pragma unroll
   for (int c = 0; c < NV; ++c) {
@@ -347,7 +357,10 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     const int row = q / NV, c4 = q - row * NV;
     if (row < nrows && s_vis[row]) {
       cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * s_idx[row] + 4 * c4);
-      if (ACC) cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
+      if (ACC) {
+        if (LIST && s_fresh[row]) *reinterpret_cast<float4*>(s_old + row * PB_STRIDE + 4 * c4) = make_float4(0.f, 0.f, 0.f, 0.f);
+        else cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
+      }
     }
   }
   float dmu[3] = {0.f, 0.f, 0.f}, dls[3] = {0.f, 0.f, 0.f};
@@ -487,10 +500,10 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       adam_scalar(af.p[3] + i, af.m[3] + i, af.v[3] + i, gl, af, af.lr[3], ibc1, ibc2);
     } else if (ACC) {
       if (vis) {
-        float4 cur = *oq;
+        float4 cur = fresh ? make_float4(0.f, 0.f, 0.f, 0.f) : *oq;
         cur.x += dq.x; cur.y += dq.y; cur.z += dq.z; cur.w += dq.w;
         *oq = cur;
-        out.opacity_logit[i] += dlogit;
+        out.opacity_logit[i] = (fresh ? 0.f : out.opacity_logit[i]) + dlogit;
       }
     } else {
       *oq = dq;
@@ -555,6 +568,8 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
           const float4 a = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
           const float4 o = *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
           *dst = make_float4(o.x + a.x, o.y + a.y, o.z + a.z, o.w + a.w);
+        } else if (LIST && s_fresh[row]) {
+          *dst = make_float4(0.f, 0.f, 0.f, 0.f);       // coefficients above sh_degree of a freshly stored row
         }
       } else {
         *dst = live ? *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4) : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -589,7 +604,10 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
         const float gm = dmu[k] + (ACC ? out.mean[3 * i + k] : 0.f), gs = dls[k] + (ACC ? out.log_scale[3 * i + k] : 0.f);
         adam_scalar(af.p[0] + 3 * i + k, af.m[0] + 3 * i + k, af.v[0] + 3 * i + k, gm, af, af.lr[0], ibc1, ibc2);
         adam_scalar(af.p[1] + 3 * i + k, af.m[1] + 3 * i + k, af.v[1] + 3 * i + k, gs, af, af.lr[1], ibc1, ibc2);
-      } else if (ACC) { out.mean[3 * i + k] += dmu[k]; out.log_scale[3 * i + k] += dls[k]; }
+      } else if (ACC) {
+        out.mean[3 * i + k] = (fresh ? 0.f : out.mean[3 * i + k]) + dmu[k];
+        out.log_scale[3 * i + k] = (fresh ? 0.f : out.log_scale[3 * i + k]) + dls[k];
+      }
       else     { out.mean[3 * i + k] = dmu[k]; out.log_scale[3 * i + k] = dls[k]; }
     }
   }
@@ -605,21 +623,21 @@ static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pla
   cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   k_project_bwd<DEG, ACC, ADAM, false><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(
-      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, nullptr, nullptr);
+      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, nullptr, nullptr, nullptr);
 }
 
 // accumulating launch over the list of visible Gaussians (persistent grid: the count lives on the device)
 template <int DEG>
 static void launch_pb_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
                            const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
-                           const AdamFuse& af, const uint32_t* vlist, const uint64_t* nvis) {
+                           const AdamFuse& af, const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * 2;
   cudaFuncSetAttribute(k_project_bwd<DEG, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   cudaFuncSetAttribute(k_project_bwd<DEG, true, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   const int64_t need = (rt.jprefix[rt.n] + PB_THREADS - 1) / PB_THREADS;
   const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 4 ? need : (int64_t)SPLX_SM_COUNT * 4;
   k_project_bwd<DEG, true, false, true><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
-      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis);
+      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis, touched);
 }
 
 template <bool ACC, bool ADAM>
@@ -652,7 +670,7 @@ int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pl
 
 int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
                        const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads,
-                       const AdamFuse* adam, const uint32_t* vlist, const uint64_t* nvis) {
+                       const AdamFuse* adam, const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
   const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
   const bool overwrite = (flags & SPLX_PB_OVERWRITE) != 0;
   if (vlist && nvis && !overwrite && !adam) {      // += over the visible Gaussians only
@@ -661,10 +679,10 @@ int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pl
     AdamFuse none;
     memset(&none, 0, sizeof none);
     switch (deg) {
-      case 0: launch_pb_list<0>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
-      case 1: launch_pb_list<1>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
-      case 2: launch_pb_list<2>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
-      default: launch_pb_list<3>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis); break;
+      case 0: launch_pb_list<0>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
+      case 1: launch_pb_list<1>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
+      case 2: launch_pb_list<2>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
+      default: launch_pb_list<3>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
     }
     SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
     return SPLX_OK;

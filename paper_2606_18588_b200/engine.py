@@ -69,6 +69,10 @@ class Trainer:
         #: accumulating projection backward over the binning's list of visible Gaussians
         #: (splx_project_backward_list_plan) instead of all rows of the participating partitions
         self.use_visible_list = os.environ.get("SPLX_VISIBLE_LIST", "1") == "1"
+        #: visible-only ("sparse") Adam -- an OPTION outside the paper: only Gaussians that received a gradient
+        #: in the iteration take the step (splx_adam_sparse); no gradient buffer is ever zeroed or overwritten wholesale
+        self.sparse_adam = os.environ.get("SPLX_SPARSE_ADAM", "0") == "1"
+        self._touched = None
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
         self.pipeline_buckets = os.environ.get("SPLX_PIPELINE", "1") == "1"
         self._cam = None
@@ -214,6 +218,12 @@ class Trainer:
             c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
                                          self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev,
                                          grad_scale=1.0 / n_views, clear_g2d=True, overwrite=overwrite)
+        elif self.sparse_adam:    # every launch walks the visible list; the flags say which rows to store and which to add to
+            if self._touched is None:
+                self._touched = torch.zeros(max(self.n, 1), dtype=torch.uint8, device=self.ctx.device)
+            lst, cnt = c.bin_sort_visible(ws, self.n, self.capacity, self.K, plan.cams[0])
+            c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
+                                         lst, cnt, clear_g2d=True, touched=self._touched)
         elif not overwrite and self.use_visible_list:   # an accumulating launch over the binning's visible list only
             lst, cnt = c.bin_sort_visible(ws, self.n, self.capacity, self.K, plan.cams[0])
             c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
@@ -341,7 +351,11 @@ class Trainer:
                            self.fuse_adam and gi == G - 1, len(view_ids))
                 ev_back[gi].record(main)
             side.wait_stream(main)
-        if not self.fuse_adam:
+        if self.sparse_adam:
+            self.step_count += 1
+            self.ctx.adam_sparse(self.params, self.grads, self.m, self.v, self._touched, [self.lr[k] for k in PARAM_KEYS],
+                                 step=self.step_count, grad_scale=1.0 / len(view_ids))
+        elif not self.fuse_adam:
             self.adam_step(len(view_ids))
         return len(groups)
 

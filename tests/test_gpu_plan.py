@@ -508,3 +508,65 @@ def test_iteration_views_gradients_against_the_oracle(blocks):
                 for key in scenes.PARAM_KEYS:
                     total[k][key] = total[k][key] + grads[k][key]
     _check_grads(tr, total)
+
+
+def test_sparse_adam_option(blocks):
+    """The visible-only optimiser (an option outside the paper): (1) splx_adam_sparse == splx_adam_groups on the flagged
+    rows, bit for bit, and leaves every other row of parameters and moments alone; it clears the flags; (2) the
+    flag-driven projection backward stores the first gradient of a row and adds the later ones, never touching the
+    rows no view sees; (3) a whole multi-bucket iteration moves exactly the Gaussians some view saw."""
+    sc = blocks
+    rng = np.random.default_rng(61)
+    a, b = _trainer(sc), _trainer(sc)
+    n = a.n
+    flags = (rng.uniform(size=n) < 0.3)
+    g = rng.standard_normal(a.flat["grad"].shape).astype(np.float32)
+    m0 = (rng.standard_normal(a.flat["m"].shape) * 0.01).astype(np.float32)
+    v0 = (np.abs(rng.standard_normal(a.flat["v"].shape)) * 1e-4).astype(np.float32)
+    for tr in (a, b):
+        tr.flat["grad"].copy_(torch.from_numpy(g)); tr.flat["m"].copy_(torch.from_numpy(m0)); tr.flat["v"].copy_(torch.from_numpy(v0))
+    a.adam_step(n_views=2)                                                   # dense
+    touched = torch.from_numpy(flags.astype(np.uint8)).cuda()
+    b.ctx.adam_sparse(b.params, b.grads, b.m, b.v, touched, [b.lr[k] for k in scenes.PARAM_KEYS], step=1, grad_scale=0.5)
+    torch.cuda.synchronize()
+    assert not touched.any()
+    fl = torch.from_numpy(flags).cuda()
+    for name, init in (("param", None), ("m", m0), ("v", v0)):
+        for key in scenes.PARAM_KEYS:
+            w = scenes.PARAM_WIDTH[key]
+            va = {"param": a.params, "m": a.m, "v": a.v}[name][key].reshape(n, w)
+            vb = {"param": b.params, "m": b.m, "v": b.v}[name][key].reshape(n, w)
+            assert torch.equal(va[fl], vb[fl]), (name, key)
+            orig = torch.from_numpy(np.asarray(sc.params[key], np.float32).reshape(n, w)).cuda() if init is None else None
+            if orig is not None:
+                assert torch.equal(vb[~fl], orig[~fl]), (name, key)
+    # (2) + (3): two iterations over all views with the sparse optimiser
+    tr = _trainer(sc)
+    tr.sparse_adam = True
+    tr.flat["grad"].fill_(float("nan"))                                      # never zeroed, never read where no view looks
+    ids = list(range(len(sc.cameras)))
+    targets = torch.from_numpy(np.stack(sc.targets)).cuda()
+    dense = _trainer(sc)
+    dense.lr = {k: 0.0 for k in dense.lr}
+    dense.iteration_views(ids, sc.cameras, targets, saturation=False)
+    p0 = tr.flat["param"].clone()
+    tr.iteration_views(ids, sc.cameras, targets, saturation=False)
+    torch.cuda.synchronize()
+    assert not tr._touched.any()
+    seen = torch.zeros(n, dtype=torch.bool, device="cuda")
+    for v_, cam in zip(ids, sc.cameras):
+        plan, _ = dense.bucket_plan([v_], [cam], saturation=False)
+        dense.forward_plan(plan)
+        part = dense.participants(v_, cam)
+        vis = dense.proj.radius > 0
+        for k in range(sc.K):
+            if (part >> k) & 1:
+                seen[dense.part_offsets[k]:dense.part_offsets[k + 1]] |= vis[dense.part_offsets[k]:dense.part_offsets[k + 1]]
+    assert 0 < int(seen.sum()) < n
+    moved = (tr.params["opacity_logit"] != p0[tr._offs["opacity_logit"]:tr._offs["opacity_logit"] + n])
+    assert not (moved & ~seen).any()                                         # what no view saw did not move
+    assert (moved & seen).float().sum() > 0.9 * seen.float().sum()
+    # the gradients of the seen rows are the dense iteration's
+    gs = tr.grads["sh"].reshape(n, 48)[seen]; gd = dense.grads["sh"].reshape(n, 48)[seen]
+    assert not torch.isnan(gs).any()
+    assert float((gs - gd).abs().max()) <= 1e-4 * float(gd.abs().max())

@@ -194,3 +194,26 @@ def test_kd_partition_is_balanced_and_axis_aligned():
     assert scenes.imbalance_ratio(g_offs) > 1.0
     sc = scenes.aerial(n=5000, width=64, height=48, grid=(2, 2), partition="kd", name="kd")
     assert np.diff(sc.part_offsets).tolist() == [1250, 1250, 1250, 1250]
+
+
+def test_adam_rows_is_adam_on_the_selected_rows():
+    """The visible-only option: all rows selected = dense Adam; no row selected = nothing moves; a partial selection
+    moves exactly the selected rows, with torch.optim.Adam's values on them (bias correction by the global step)."""
+    import torch
+    rng = np.random.default_rng(12)
+    p0 = rng.standard_normal((50, 3)); g = rng.standard_normal((50, 3))
+    rows = rng.uniform(size=50) < 0.4
+    p = p0.copy(); m = np.zeros_like(p); v = np.zeros_like(p)
+    ov.adam_rows(p, g, m, v, np.zeros(50, bool), 1e-2)
+    assert np.array_equal(p, p0) and not m.any() and not v.any()
+    pa = p0.copy(); ma = np.zeros_like(p); va = np.zeros_like(p)
+    ov.adam_rows(pa, g, ma, va, np.ones(50, bool), 1e-2)
+    pd = p0.copy().reshape(-1); md = np.zeros(150); vd = np.zeros(150)
+    oracle.adam(pd, g.reshape(-1), md, vd, 1e-2)
+    assert np.array_equal(pa.reshape(-1), pd)
+    ov.adam_rows(p, g, m, v, rows, 1e-2, step=1)
+    t = torch.tensor(p0[rows], dtype=torch.float64, requires_grad=True)
+    opt = torch.optim.Adam([t], lr=1e-2, eps=1e-15)
+    t.grad = torch.tensor(g[rows]); opt.step()
+    assert np.allclose(p[rows], t.detach().numpy(), rtol=1e-12, atol=1e-14)
+    assert np.array_equal(p[~rows], p0[~rows]) and not m[~rows].any()
