@@ -477,6 +477,7 @@ def run_views(args):
            "city_100M": 96_000_000}.get(args.workload)
     tr = Trainer(sc.params, sc.part_offsets, W, H, sc.sh_degree, sc.bg, capacity=cap)
     aabbs = scenes.partition_aabbs(sc.params, sc.part_offsets)
+    cells = scenes.partition_aabbs(sc.params, sc.part_offsets, inflate_sigma=0.0) if args.cross_filter else None
     sc.params = None                                   # a device-generated scene: release the generator's copy
     torch.cuda.empty_cache()
     tr.sparse_adam = bool(args.sparse_adam)
@@ -485,6 +486,15 @@ def run_views(args):
         tr.set_aabbs(np.full((tr.K, 3), -big), np.full((tr.K, 3), big))
     else:
         tr.set_aabbs(*aabbs)
+    cross = None
+    if args.cross_filter:    # Q_cross against the cell boxes (boxes of the means); timed once, it is view independent
+        tr.set_cross(*cells)
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(); tr.set_cross(*cells); c1.record()
+        torch.cuda.synchronize()
+        cross = dict(cross_sets_ms=c0.elapsed_time(c1),
+                     gaussians_in_Q_cross=int((tr._cross != 0).sum().item()))
     targets = torch.from_numpy(np.stack(sc.targets[:B])).cuda()
     ids = list(range(B))
     kw = dict(consolidate=not args.no_consolidate, saturation=args.saturation, sat_eps=args.sat_eps)
@@ -519,7 +529,7 @@ def run_views(args):
                             views_per_step=B, visibility_prediction=not args.no_visibility,
                             consolidation=not args.no_consolidate, saturation_skipping=bool(args.saturation),
                             optimiser="visible-only Adam (option, not the paper's)" if args.sparse_adam else "dense Adam",
-                            sat_eps=args.sat_eps, participants=[bin(p) for p in parts], buckets=groups,
+                            cross_boundary_filter=cross, sat_eps=args.sat_eps, participants=[bin(p) for p in parts], buckets=groups,
                             tile_state=skipped, intersections_last_bucket=M,
                             l2="working set (params+grads+moments) is larger than the 126 MB L2"),
                 iters_per_s=1e3 / ms, clocks=clocks, gpu_launches=int(launches),
@@ -542,6 +552,8 @@ def main():
     ap.add_argument("--views", type=int, default=0, help="B > 0: time iterations over B views (optional subsystems)")
     ap.add_argument("--no-visibility", action="store_true")
     ap.add_argument("--no-consolidate", action="store_true")
+    ap.add_argument("--cross-filter", action="store_true",
+                    help="--views only: cross-boundary per-ray filtering (PAPER.md L474-L476, DESIGN.md s32)")
     ap.add_argument("--sparse-adam", action="store_true",
                     help="--views only: visible-only Adam (an option outside the paper, DESIGN.md s31)")
     args = ap.parse_args()

@@ -308,6 +308,31 @@ int splx_project_backward_plan(splx_ctx *ctx, const splx_gaussians *g, int K, co
  * splx_bin_sort on it.  Same n, capacity, K, cam as that call.  Host computation only. */
 int splx_bin_sort_visible(const void *ws, int64_t n, uint64_t capacity, int K, const splx_camera *cam,
                           const uint32_t **visible, const uint64_t **num_visible);
+/* ---- cross-boundary per-ray filtering (appendix 8.1, Fig. 25; readings: DESIGN.md s32) ----
+ * "We remove a Gaussian G_i in Q_cross from the ray r of pixel p if and only if its depth d_i falls within the
+ * overlapped depth interval D_overlap and p lies in the overlapped pixel region Omega_v^k ^ Omega_v^s."
+ *
+ * splx_cross_sets (view independent; once per change of the Gaussians): cross_mask[i] (DEVICE uint64[n], out) gets
+ * bit s set iff Gaussian i of partition k != s is in Q_cross(k, s): the axis-aligned box around its
+ * support_sigma-sigma ellipsoid (half extent along axis a = support_sigma * sqrt(Sigma_aa), Sigma = R S^2 R^T)
+ * meets the closed CELL box [cell_lo[s], cell_hi[s]] (HOST float[K][3]).  fp32. */
+int splx_cross_sets(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                    const float *cell_lo, const float *cell_hi, float support_sigma, uint64_t *cross_mask);
+/* D^k of a plan (HOST computation, double precision rounded to float): part_depth_range[2k], [2k+1] (HOST out) =
+ * the smallest and largest camera-space z over the corners of box k under the view plan->view_of_part[k];
+ * (+inf, -inf) for a partition that renders no view. */
+int splx_cross_depth_ranges(int K, const float *aabb_lo, const float *aabb_hi, const splx_plan *plan,
+                            float *part_depth_range);
+/* splx_bin_sort_plan with the filter: the (Gaussian i of partition k, tile t) pair is left out of the list of
+ * (k, t) iff for some partition s: bit s of cross_mask[i], s renders the view k renders, depth[i] lies in the closed
+ * interval D^k ^ D^s of part_depth_range (HOST float[2K]), and tile t is in Omega^s (plan->tile_state[s, t] without
+ * SPLX_TILE_INVISIBLE; no tile_state = every tile).  The order of the remaining entries is unchanged, so every
+ * later stage (forward and backward) simply never sees the pair.  *num_intersections counts the pairs KEPT; the
+ * capacity must still hold the unfiltered count (removed pairs are sorted to the end of the key buffer: keys and
+ * vals beyond *num_intersections are scratch).  cross_mask NULL = splx_bin_sort_plan. */
+int splx_bin_sort_filtered_plan(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
+                                const int64_t *part_offsets, const splx_plan *plan, const uint64_t *cross_mask,
+                                const float *part_depth_range, const splx_binning *out, void *ws, size_t ws_bytes);
 /* splx_project_backward_plan in += mode over the visible Gaussians only: the rows processed are the entries of
  * `visible` (device uint32[*num_visible], *num_visible a device uint64) instead of every Gaussian of the
  * participating partitions -- same result (a culled Gaussian has no gradient), work proportional to the visible

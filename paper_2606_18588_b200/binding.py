@@ -34,6 +34,7 @@ EXPORTS = [
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
     "splx_compose_l1_backward_plan", "splx_project_backward_adam_plan", "splx_adam_bias_step",
     "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
+    "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -145,6 +146,9 @@ def lib():
         L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
         L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp]
         L.splx_adam_sparse.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float]
+        L.splx_cross_sets.argtypes = [vp, vp, C.c_int, vp, vp, vp, C.c_float, vp]
+        L.splx_cross_depth_ranges.argtypes = [C.c_int, vp, vp, vp, vp]
+        L.splx_bin_sort_filtered_plan.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp, vp, vp, vp, vp, C.c_size_t]
         _lib = L
     return _lib
 
@@ -208,6 +212,18 @@ def visible_regions(aabb_lo, aabb_hi, cam):
     if rc != OK:
         raise SplxError(rc, "splx_visible_regions: invalid argument")
     return out, int(part.value)
+
+
+def cross_depth_ranges(aabb_lo, aabb_hi, plan):
+    """splx_cross_depth_ranges (host computation): D^k of every partition under the view it renders, float32 [K, 2]."""
+    import numpy as np
+    lo = np.ascontiguousarray(aabb_lo, np.float32).reshape(-1, 3)
+    hi = np.ascontiguousarray(aabb_hi, np.float32).reshape(-1, 3)
+    out = np.empty((lo.shape[0], 2), np.float32)
+    rc = lib().splx_cross_depth_ranges(lo.shape[0], lo.ctypes.data, hi.ctypes.data, plan.ref(), out.ctypes.data)
+    if rc != OK:
+        raise SplxError(rc, "splx_cross_depth_ranges: invalid argument")
+    return out
 
 
 def schedule_views(participants, max_views_per_bucket=MAX_VIEWS):
@@ -417,6 +433,26 @@ class Context:
         ps, bs = proj.struct(), out.struct()
         self._check(lib().splx_bin_sort_plan(self._h, C.byref(ps), proj.n, plan.K, self._offs(part_offsets), plan.ref(),
                                              C.byref(bs), _ptr(ws), ws.numel() * ws.element_size()))
+
+    def cross_sets(self, params: dict, part_offsets, cell_lo, cell_hi, cross_mask: torch.Tensor, support_sigma=3.0):
+        """splx_cross_sets: cross_mask = device int64/uint64 [n] (bit s = in Q_cross against partition s)."""
+        import numpy as np
+        lo = np.ascontiguousarray(cell_lo, np.float32).reshape(-1, 3)
+        hi = np.ascontiguousarray(cell_hi, np.float32).reshape(-1, 3)
+        g = gaussians_struct(params)
+        self._check(lib().splx_cross_sets(self._h, C.byref(g), lo.shape[0], self._offs(part_offsets), lo.ctypes.data,
+                                          hi.ctypes.data, float(support_sigma), _ptr(cross_mask)))
+
+    def bin_sort_filtered_plan(self, proj: Projected, part_offsets, plan: Plan, cross_mask, part_depth_range, out: Binning,
+                               ws: torch.Tensor):
+        import numpy as np
+        ps, bs = proj.struct(), out.struct()
+        zr = np.ascontiguousarray(part_depth_range, np.float32).reshape(-1)
+        self._check(lib().splx_bin_sort_filtered_plan(self._h, C.byref(ps), proj.n, plan.K, self._offs(part_offsets),
+                                                      plan.ref(), _ptr(cross_mask), zr.ctypes.data, C.byref(bs), _ptr(ws),
+                                                      ws.numel() * ws.element_size()))
+
+    cross_depth_ranges = staticmethod(cross_depth_ranges)
 
     def render_partial_plan(self, proj: Projected, bins: Binning, plan: Plan, out: Partial, pairs=None):
         ps, bs, os_ = proj.struct(), bins.struct(), out.struct()

@@ -164,6 +164,43 @@ int splx_bin_sort_plan(splx_ctx* ctx, const splx_projected* proj, int64_t n, int
   return launch_bin_sort(ctx, proj, n, pd, part_offsets, out, ws, ws_bytes);
 }
 
+int splx_bin_sort_filtered_plan(splx_ctx* ctx, const splx_projected* proj, int64_t n, int K, const int64_t* part_offsets,
+                                const splx_plan* plan, const uint64_t* cross_mask, const float* part_depth_range,
+                                const splx_binning* out, void* ws, size_t ws_bytes) {
+  if (!cross_mask) return splx_bin_sort_plan(ctx, proj, n, K, part_offsets, plan, out, ws, ws_bytes);
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!proj_ok(proj) || !bins_ok(out) || n < 0 || (!ws && ws_bytes) || !part_depth_range)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_bin_sort_filtered", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: part_offsets must run monotonically from 0 to n");
+  if (n >= ((int64_t)1 << 32) || out->capacity >= ((uint64_t)1 << 32))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: n and capacity must be < 2^32");
+  if ((uint64_t)K * pd.ntiles >= ((uint64_t)1 << 31)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: K*tiles too large");
+  if (!aligned16(ws)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: workspace not 16-byte aligned");
+  CrossDev cd;
+  memset(&cd, 0, sizeof cd);
+  cd.mask = cross_mask;
+  for (int k = 0; k < K; ++k) { cd.zlo[k] = part_depth_range[2 * k]; cd.zhi[k] = part_depth_range[2 * k + 1]; }
+  return launch_bin_sort(ctx, proj, n, pd, part_offsets, out, ws, ws_bytes, &cd);
+}
+
+int splx_cross_sets(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const float* cell_lo,
+                    const float* cell_hi, float support_sigma, uint64_t* cross_mask) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!g || g->n < 0 || !cell_lo || !cell_hi || (g->n > 0 && (!g->mean || !g->log_scale || !g->quat || !cross_mask)))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_cross_sets: null argument");
+  if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_cross_sets: K=%d not in [1,%d]", K, SPLX_MAX_K);
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_cross_sets: part_offsets must run monotonically from 0 to n");
+  if (!(support_sigma >= 0.f)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_cross_sets: support_sigma must be >= 0");
+  if (((uintptr_t)g->quat & 15) || ((uintptr_t)cross_mask & 7)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_cross_sets: quat must be 16-byte, cross_mask 8-byte aligned");
+  for (int k = 0; k < K; ++k)
+    for (int a = 0; a < 3; ++a)
+      if (!(cell_lo[3 * k + a] <= cell_hi[3 * k + a])) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_cross_sets: box %d has lo > hi", k);
+  return launch_cross_sets(ctx, g, K, part_offsets, cell_lo, cell_hi, support_sigma, cross_mask);
+}
+
 int splx_bin_sort(splx_ctx* ctx, const splx_projected* proj, int64_t n, int K, const int64_t* part_offsets,
                   const splx_camera* cam, const splx_binning* out, void* ws, size_t ws_bytes) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;

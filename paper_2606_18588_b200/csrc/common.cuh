@@ -57,6 +57,13 @@ struct PlanDev {
   CamDev cam[SPLX_MAX_VIEWS];
 };
 
+// Cross-boundary per-ray filtering (L474-L476): the per-Gaussian Q_cross masks and the depth interval D^k of every
+// partition under the view it renders.  mask == nullptr = no filtering.
+struct CrossDev {
+  const uint64_t* mask;
+  float zlo[SPLX_MAX_K], zhi[SPLX_MAX_K];
+};
+
 // Contiguous runs of Gaussians (one per participating partition) covered by ONE launch of a
 // per-Gaussian kernel: block b works on run r with block_prefix[r] <= b < block_prefix[r+1].
 // view[r] < 0 marks a run of a non-participating partition (only present when its outputs must
@@ -148,7 +155,9 @@ int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX
                      const uint64_t** count);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
 int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, const PlanDev&, const int64_t* part_offsets,
-                    const splx_binning*, void* ws, size_t ws_bytes);
+                    const splx_binning*, void* ws, size_t ws_bytes, const CrossDev* cross = nullptr);
+int launch_cross_sets(splx_ctx*, const splx_gaussians*, int K, const int64_t* part_offsets, const float* cell_lo,
+                      const float* cell_hi, float support_sigma, uint64_t* cross_mask);
 int launch_render_fwd(splx_ctx*, const splx_projected*, const splx_binning*, const PlanDev&,
                       const splx_partial*, uint64_t* pairs);
 int launch_raster_bwd(splx_ctx*, const splx_projected*, const splx_binning*, const PlanDev&,

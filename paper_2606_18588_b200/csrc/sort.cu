@@ -455,12 +455,46 @@ int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, ui
 //    each) and the first scheme leaves a handful of CTAs with all the work (1.5 ms on street_10M against 0.2 ms).
 __device__ __forceinline__ bool emit_by_output(const Counters* cnt) { return cnt->m_total > 16 * cnt->n_visible; }
 
+// Cross-boundary per-ray filtering (L474-L476): a removed (Gaussian, tile) pair is emitted under the slot number
+// `nslots` (one past the last real slot), so the slot sort carries it behind every list and k_tile_ranges never
+// gives it a range; the rectangle arithmetic of the emission stays as it is.
+struct CrossEmit {
+  const uint64_t* mask;          // nullptr = no filtering
+  const uint8_t* tile_state;
+  uint32_t ntiles, nslots;
+  float zlo[SPLX_MAX_K], zhi[SPLX_MAX_K];
+  signed char view[SPLX_MAX_K];
+};
+
+// F_i: the partitions s whose visible tiles lose Gaussian i (partition k, depth d): i in Q_cross(k, s), same view,
+// d in D^k ^ D^s.
+__device__ __forceinline__ uint64_t cross_filter(const CrossEmit& cx, uint32_t i, int k, float d) {
+  uint64_t m = cx.mask[i], F = 0;
+  while (m) {
+    const int s = __ffsll((long long)m) - 1;
+    m &= m - 1;
+    if (cx.view[s] == cx.view[k] && d >= fmaxf(cx.zlo[k], cx.zlo[s]) && d <= fminf(cx.zhi[k], cx.zhi[s])) F |= 1ull << s;
+  }
+  return F;
+}
+
+// p in Omega^s for some s of F
+__device__ __forceinline__ bool cross_removed(const CrossEmit& cx, uint64_t F, uint32_t tile) {
+  while (F) {
+    const int s = __ffsll((long long)F) - 1;
+    F &= F - 1;
+    if (!cx.tile_state || !(cx.tile_state[(size_t)s * cx.ntiles + tile] & SPLX_TILE_INVISIBLE)) return true;
+  }
+  return false;
+}
+
 __global__ void __launch_bounds__(256)
 k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
             uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
-            uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+            uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride,
+            const __grid_constant__ CrossEmit cx) {
   if (emit_by_output(cnt)) return;
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
@@ -480,6 +514,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
   const uint64_t j = base + threadIdx.x;
   int x0 = 0, y0 = 0, w = 0, tt = 0;
   uint32_t i = 0, o = 0, dbits = 0, slot0 = 0;
+  uint64_t F = 0;
   if (j < nvis) {
     i = cvals[j]; dbits = ckeys[j]; o = offs[j];
     const float2 m = *reinterpret_cast<const float2*>(means2d + 2 * (uint64_t)i);
@@ -492,6 +527,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       if (parts.off[mid] <= (int64_t)i) lo = mid; else hi = mid - 1;
     }
     slot0 = (uint32_t)lo * (uint32_t)(TX * TY);
+    if (cx.mask) F = cross_filter(cx, i, lo, __uint_as_float(dbits));
   }
   // The 32 runs of a warp are adjacent in the output (offs is the running sum of tiles_touched in this very
   // order), so the warp writes its whole range [o_0, o_0 + T) cooperatively: lane l produces output slot
@@ -518,9 +554,13 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
     const uint32_t si = __shfl_sync(0xffffffffu, i, own), sd = __shfl_sync(0xffffffffu, dbits, own);
     const uint32_t ss = __shfl_sync(0xffffffffu, slot0, own);
     const uint64_t pos = (uint64_t)o0 + sidx;
+    uint64_t sF = 0;
+    if (cx.mask) sF = __shfl_sync(0xffffffffu, F, own);
     if (sidx < T && pos < capacity) {
       const uint32_t ty = t / (uint32_t)sw;
-      const uint32_t slot = ss + (uint32_t)((sy0 + (int)ty) * TX + sx0 + (int)(t - ty * (uint32_t)sw));
+      const uint32_t tile = (uint32_t)((sy0 + (int)ty) * TX + sx0 + (int)(t - ty * (uint32_t)sw));
+      uint32_t slot = ss + tile;
+      if (sF && cross_removed(cx, sF, tile)) slot = cx.nslots;
       keys[pos] = ((uint64_t)slot << 32) | sd;
       vals[pos] = si;
       for (int p = 0; p < plan.npass; ++p)
@@ -537,7 +577,8 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
             uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
-            uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+            uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride,
+            const __grid_constant__ CrossEmit cx) {
   if (!emit_by_output(cnt)) return;
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
@@ -558,6 +599,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
   constexpr int EK_TILE = 1024, EK_IPT = EK_TILE / 256;
   __shared__ uint32_t s_off[EK_TILE + 1], s_xy[EK_TILE + 1], s_w[EK_TILE + 1], s_slot0[EK_TILE + 1], s_db[EK_TILE + 1],
       s_gi[EK_TILE + 1];
+  __shared__ uint64_t s_F[EK_TILE + 1];
   __shared__ uint32_t s_nown;
   const uint64_t nvis = cnt->n_visible;
   const uint64_t m = cnt->m_sorted;                       // min(M, capacity): positions beyond the capacity are dropped
@@ -593,6 +635,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         }
         s_off[q] = o; s_xy[q] = ((uint32_t)y0 << 16) | (uint32_t)x0; s_w[q] = (uint32_t)(x1 - x0);
         s_slot0[q] = (uint32_t)plo * (uint32_t)(TX * TY); s_db[q] = ckeys[j]; s_gi[q] = i;
+        if (cx.mask) s_F[q] = cross_filter(cx, i, plo, __uint_as_float(s_db[q]));
         atomicMax(&s_nown, (uint32_t)q + 1);
       }
     }
@@ -609,7 +652,9 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         }
         const uint32_t t = (uint32_t)(pos - s_off[ql]), w = s_w[ql], xy = s_xy[ql];
         const uint32_t ty = t / w;
-        const uint32_t slot = s_slot0[ql] + ((xy >> 16) + ty) * (uint32_t)TX + (xy & 0xffffu) + (t - ty * w);
+        const uint32_t tile = ((xy >> 16) + ty) * (uint32_t)TX + (xy & 0xffffu) + (t - ty * w);
+        uint32_t slot = s_slot0[ql] + tile;
+        if (cx.mask) { const uint64_t F = s_F[ql]; if (F && cross_removed(cx, F, tile)) slot = cx.nslots; }
         keys[pos] = ((uint64_t)slot << 32) | s_db[ql];
         vals[pos] = s_gi[ql];
         for (int p = 0; p < plan.npass; ++p)
@@ -624,11 +669,20 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
 
 __global__ void __launch_bounds__(256)
 k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint8_t* __restrict__ tile_state,
-              uint32_t* __restrict__ ranges, uint64_t* __restrict__ m_out) {
+              uint32_t* __restrict__ ranges, uint64_t* __restrict__ m_out, uint32_t nslots, bool filtered) {
   const uint64_t m = cnt->m_sorted;
-  if (blockIdx.x == 0 && threadIdx.x == 0) *m_out = cnt->m_total;
+  // M as published: the unfiltered count (it is what the capacity must hold) unless the filter ran and everything
+  // fitted -- then the number of pairs kept, written by the thread that sees the first removed pair (or the last
+  // key, when nothing was removed).
+  const bool count_kept = filtered && cnt->m_total == m && m > 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0 && !count_kept) *m_out = cnt->m_total;
   for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j < m; j += (uint64_t)gridDim.x * blockDim.x) {
     const uint32_t s = (uint32_t)(keys[j] >> 32);
+    if (s >= nslots) {           // removed pairs: behind every list
+      if (count_kept && (j == 0 || (uint32_t)(keys[j - 1] >> 32) < nslots)) *m_out = j;
+      continue;
+    }
+    if (count_kept && j + 1 == m) *m_out = m;
     if (tile_state && tile_state[s]) continue;   // a skipped (partition, tile) slot keeps the empty range (0,0)
     if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
     if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
@@ -648,7 +702,7 @@ struct Layout {
 static int slot_bits(int K, int TX, int TY) {
   const uint64_t slots = (uint64_t)K * TX * TY;
   int b = 1;
-  while (((uint64_t)1 << b) < slots) ++b;
+  while (((uint64_t)1 << b) <= slots) ++b;   // the values 0..slots: `slots` itself marks a filtered pair
   return b;
 }
 
@@ -691,7 +745,7 @@ int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX
 }
 
 int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const PlanDev& plan, const int64_t* part_offsets,
-                    const splx_binning* out, void* ws, size_t ws_bytes) {
+                    const splx_binning* out, void* ws, size_t ws_bytes, const CrossDev* cross) {
   const int K = plan.K;
   const PlanDev& cam = plan;   // TX, TY
   const int sbits = slot_bits(K, cam.TX, cam.TY);
@@ -743,24 +797,31 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   PartOffs parts;
   parts.K = K;
   for (int k = 0; k <= K; ++k) parts.off[k] = part_offsets[k];
+  CrossEmit cx;
+  memset(&cx, 0, sizeof cx);
+  cx.ntiles = (uint32_t)ntiles; cx.nslots = (uint32_t)K * (uint32_t)ntiles;
+  if (cross && cross->mask) {
+    cx.mask = cross->mask; cx.tile_state = plan.tile_state;
+    for (int k = 0; k < K; ++k) { cx.zlo[k] = cross->zlo[k]; cx.zhi[k] = cross->zhi[k]; cx.view[k] = plan.pv.v[k]; }
+  }
   const uint64_t emit_blocks = ((uint64_t)n_act + 255) / 256, range_blocks = (out->capacity + 255) / 256;
   k_emit_keys<<<(unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
       pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0,
       plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
-      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256);
+      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256, cx);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
   const uint64_t emit_tiles = (out->capacity + 1023) / 1024;     // output tiles of 1024 keys
   k_emit_keys_lb<<<(unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
       pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0,
       plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
-      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256);
+      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256, cx);
   SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
   // 4. stable sort on the slot bits
   if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
                                  (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6], true))) return rc;
   // 5. ranges
   k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
-      out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections);
+      out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections, cx.nslots, cx.mask != nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
   return SPLX_OK;
 }

@@ -77,6 +77,7 @@ class Trainer:
         self.pipeline_buckets = os.environ.get("SPLX_PIPELINE", "1") == "1"
         self._cam = None
         self._aabb = None
+        self._cross = None          # Q_cross masks (set_cross): cross-boundary filtering on
         self._side = None
         self._ws_sort = None
         self._ws_bwd = None
@@ -160,7 +161,7 @@ class Trainer:
         c = self.ctx
         images, T_totals, _ = self._view_buffers(plan.B)
         c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
-        c.bin_sort_plan(self.proj, self.part_offsets, plan, self.bins, self._ws_sort)
+        self._bin_sort(self.proj, plan, self.bins, self._ws_sort)
         c.render_partial_plan(self.proj, self.bins, plan, self.partials, self.pairs if count_pairs else None)
         c.compose_plan(self.partials, self.bins, plan, self.bg, images, T_totals,
                        sat_eps if sat_eps is not None else 0.0, tile_state_out)
@@ -200,7 +201,7 @@ class Trainer:
         """a1-a4 of a bucket: project, bin/sort."""
         proj, bins, ws = bufs
         self.ctx.project_plan(self.params, self.part_offsets, plan, self.sh_degree, proj)
-        self.ctx.bin_sort_plan(proj, self.part_offsets, plan, bins, ws)
+        self._bin_sort(proj, plan, bins, ws)
 
     def _back(self, plan, bufs, targets, overwrite, sat_eps, tile_state_out, adam, n_views):
         """a5-a10 of a bucket: render, fused composition + loss + composition backward, raster and projection backward."""
@@ -256,6 +257,25 @@ class Trainer:
         self.ctx.backward_plan(self.part_offsets, plan, self.partials, self.bg, gi if g_images is None else g_images,
                                None, self.params, self.proj, self.bins, self.sh_degree, self.grads, self._ws_bwd,
                                overwrite=overwrite)
+
+    def set_cross(self, cell_lo, cell_hi, support_sigma=3.0):
+        """Cross-boundary per-ray filtering (L474-L476) on: Q_cross of every Gaussian against the cell
+        boxes (to be called again when the Gaussians change); the depth intervals and Omega come from set_aabbs.
+        cell_lo=None switches it off."""
+        if cell_lo is None:
+            self._cross = None
+            return
+        if self._cross is None:
+            self._cross = torch.empty(self.n, dtype=torch.int64, device=self.ctx.device)
+        self.ctx.cross_sets(self.params, self.part_offsets, cell_lo, cell_hi, self._cross, support_sigma)
+
+    def _bin_sort(self, proj, plan, bins, ws):
+        if self._cross is None:
+            self.ctx.bin_sort_plan(proj, self.part_offsets, plan, bins, ws)
+            return
+        if getattr(plan, "_zr", None) is None:
+            plan._zr = binding.cross_depth_ranges(self._aabb[0], self._aabb[1], plan)
+        self.ctx.bin_sort_filtered_plan(proj, self.part_offsets, plan, self._cross, plan._zr, bins, ws)
 
     def set_aabbs(self, lo, hi):
         """Static partition boxes (scenes.partition_aabbs) for the geometric visibility prediction."""
@@ -374,7 +394,7 @@ class Trainer:
         images, T_totals, _ = self._view_buffers(1)
         g_ct, g2d = self.fused_buffers()
         c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
-        c.bin_sort_plan(self.proj, self.part_offsets, plan, self.bins, self._ws_sort)
+        self._bin_sort(self.proj, plan, self.bins, self._ws_sort)
         c.render_partial_plan(self.proj, self.bins, plan, self.partials)
         main.wait_event(self._ev_target)            # the target is first needed by the fused composition + loss
         c.compose_l1_backward_plan(self.partials, self.bins, plan, self.bg, self._target_dev, images, T_totals,
