@@ -269,6 +269,16 @@ int splx_schedule_views(int n_views, const uint64_t *participants, int max_views
  * Arrays indexed by partition keep their [K,...] layout (a partition belongs to one view). */
 int splx_project_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                       const splx_plan *plan, int sh_degree, const splx_projected *out);
+/* splx_project_plan in two halves, so that a caller can overlap them with other work (the colour half needs nothing
+ * but tiles_touched of the geometry half and is not needed before splx_render_partial: it can run beside the
+ * binning, and -- across iterations -- the optimiser step of the SH coefficients can run beside the geometry half
+ * and the binning of the next iteration).  SPLX_PROJECT_GEOMETRY writes means2d, depth, conic_opacity, radius,
+ * tiles_touched and records 0-1 of `blend`; SPLX_PROJECT_COLOUR (after it) writes rgb, clamp and record 2.  Both
+ * bits = splx_project_plan; the results are bit-identical either way. */
+#define SPLX_PROJECT_GEOMETRY 1
+#define SPLX_PROJECT_COLOUR 2
+int splx_project_parts_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                            const splx_plan *plan, int sh_degree, const splx_projected *out, int parts);
 int splx_bin_sort_plan(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
                        const int64_t *part_offsets, const splx_plan *plan, const splx_binning *out,
                        void *ws, size_t ws_bytes);

@@ -34,11 +34,12 @@ EXPORTS = [
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
     "splx_compose_l1_backward_plan", "splx_project_backward_adam_plan", "splx_adam_bias_step",
     "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
-    "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
+    "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan", "splx_project_parts_plan",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
 PLAN_SPARSE = 1
+PROJECT_GEOMETRY, PROJECT_COLOUR = 1, 2
 
 
 class SplxError(RuntimeError):
@@ -146,6 +147,7 @@ def lib():
         L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
         L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp]
         L.splx_adam_sparse.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float]
+        L.splx_project_parts_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, C.c_int]
         L.splx_cross_sets.argtypes = [vp, vp, C.c_int, vp, vp, vp, C.c_float, vp]
         L.splx_cross_depth_ranges.argtypes = [C.c_int, vp, vp, vp, vp]
         L.splx_bin_sort_filtered_plan.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp, vp, vp, vp, vp, C.c_size_t]
@@ -428,6 +430,12 @@ class Context:
         g, ps = gaussians_struct(params), out.struct()
         self._check(lib().splx_project_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
                                             sh_degree, C.byref(ps)))
+
+    def project_parts_plan(self, params: dict, part_offsets, plan: Plan, sh_degree: int, out: Projected, parts: int):
+        """splx_project_parts_plan: parts = PROJECT_GEOMETRY (1), PROJECT_COLOUR (2) or both."""
+        g, ps = gaussians_struct(params), out.struct()
+        self._check(lib().splx_project_parts_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
+                                                  sh_degree, C.byref(ps), int(parts)))
 
     def bin_sort_plan(self, proj: Projected, part_offsets, plan: Plan, out: Binning, ws: torch.Tensor):
         ps, bs = proj.struct(), out.struct()

@@ -132,6 +132,21 @@ int splx_project_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64
   return launch_project_fwd(ctx, g, pd, part_offsets, sh_degree, out);
 }
 
+int splx_project_parts_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const splx_plan* plan,
+                            int sh_degree, const splx_projected* out, int parts) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (parts != SPLX_PROJECT_GEOMETRY && parts != SPLX_PROJECT_COLOUR && parts != (SPLX_PROJECT_GEOMETRY | SPLX_PROJECT_COLOUR))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: parts=%d", parts);
+  if (g && g->n == 0) return SPLX_OK;
+  if (!gauss_ok(g) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: null/misaligned argument");
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: sh_degree %d not in [0,3]", sh_degree);
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan(ctx, "splx_project_parts", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: part_offsets must run monotonically from 0 to n");
+  return launch_project_fwd(ctx, g, pd, part_offsets, sh_degree, out, parts);
+}
+
 int splx_project(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
                  const splx_projected* out) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;

@@ -143,7 +143,7 @@ struct AdamFuse {
 
 // ---- stage launchers (defined one per .cu file, called from api.cu) ----------------------
 int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
-                       const splx_projected*);
+                       const splx_projected*, int parts = 3);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*, const AdamFuse* adam,
                        const uint32_t* visible_list, const uint64_t* num_visible, uint8_t* touched);

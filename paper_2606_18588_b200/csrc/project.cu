@@ -127,56 +127,11 @@ __device__ __forceinline__ int find_run(const RunTable& rt, int b) {
   return lo;
 }
 
+// colour: SH along the direction from the camera centre to the mean (s13)
 template <int DEG>
-__global__ void __launch_bounds__(PROJ_THREADS)
-k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
-              splx_config cfg, splx_projected out) {
-  const int r = find_run(rt, (int)blockIdx.x);
-  const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
-  if (i >= rt.end[r]) return;
-  const CamDev& cam = plan.cam[rt.view[r]];   // the view this partition renders (indexed constant-bank loads)
-  Geo G;
-  const GeoIn gin = load_geo(g, i);
-  bool vis = geometry(gin, cam, cfg.dilation, G);
-  float u = 0.f, v = 0.f;
-  int rad = 0, tt = 0;
-  if (vis) {
-    const float mid = 0.5f * (G.a + G.c);
-    const float hd = 0.5f * (G.a - G.c);
-    const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
-    rad = (int)ceilf(3.0f * sqrtf(lam));
-    const float iz = 1.0f / G.p[2];
-    u = cam.fx * G.p[0] * iz + cam.cx;
-    v = cam.fy * G.p[1] * iz + cam.cy;
-    int x0, y0, x1, y1;
-    tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
-    tt = (x1 - x0) * (y1 - y0);
-    vis = tt > 0;
-  }
-  if (!vis) {
-    *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(0.f, 0.f);
-    out.depth[i] = 0.f;
-    *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
-    out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
-    out.radius[i] = 0; out.tiles_touched[i] = 0; out.clamp[i] = 0;
-    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-    bl[0] = bl[1] = bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
-    return;
-  }
-  const float idet = 1.0f / G.det;
-  const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
-  *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
-  out.depth[i] = G.p[2];
-  const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
-  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
-  out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
-  float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-  constexpr float kLog2e = 1.4426950408889634f;
-  bl[0] = make_float4(u, v, op, G.p[2]);
-  bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
-
-  // colour: SH along the direction from the camera centre to the mean (s13)
-  float dx = gin.m[0] - cam.o[0], dy = gin.m[1] - cam.o[1], dz = gin.m[2] - cam.o[2];
+__device__ __forceinline__ void colour(const splx_gaussians& g, const CamDev& cam, const float* m, int64_t i,
+                                       const splx_projected& out, float4* bl) {
+  float dx = m[0] - cam.o[0], dy = m[1] - cam.o[1], dz = m[2] - cam.o[2];
   const float dinv = rsqrtf(dx * dx + dy * dy + dz * dz);
   dx *= dinv; dy *= dinv; dz *= dinv;
   constexpr int NSH = (DEG + 1) * (DEG + 1);
@@ -203,6 +158,77 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   }
   bl[2] = make_float4(c[0], c[1], c[2], 0.f);
   out.clamp[i] = cl;
+}
+
+// PARTS: 1 = the geometry (everything the binning needs: 2-D mean, depth, conic, opacity, radius, tiles touched,
+// records 0-1 of the blend layout), 2 = the colour (SH -> rgb, clamp bits, record 2), 3 = both in one pass.  The
+// colour half reads tiles_touched written by the geometry half to know whether the Gaussian is visible; it depends
+// on nothing else of it, so a caller may run it beside the binning (splx_project_parts_plan).
+template <int DEG, int PARTS>
+__global__ void __launch_bounds__(PROJ_THREADS)
+k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
+              splx_config cfg, splx_projected out) {
+  const int r = find_run(rt, (int)blockIdx.x);
+  const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
+  if (i >= rt.end[r]) return;
+  const CamDev& cam = plan.cam[rt.view[r]];   // the view this partition renders (indexed constant-bank loads)
+  if (PARTS == 2) {
+    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+    if (out.tiles_touched[i] == 0) {
+      out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
+      out.clamp[i] = 0;
+      bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
+      return;
+    }
+    const float m[3] = {g.mean[3 * i], g.mean[3 * i + 1], g.mean[3 * i + 2]};
+    colour<DEG>(g, cam, m, i, out, bl);
+    return;
+  }
+  Geo G;
+  const GeoIn gin = load_geo(g, i);
+  bool vis = geometry(gin, cam, cfg.dilation, G);
+  float u = 0.f, v = 0.f;
+  int rad = 0, tt = 0;
+  if (vis) {
+    const float mid = 0.5f * (G.a + G.c);
+    const float hd = 0.5f * (G.a - G.c);
+    const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
+    rad = (int)ceilf(3.0f * sqrtf(lam));
+    const float iz = 1.0f / G.p[2];
+    u = cam.fx * G.p[0] * iz + cam.cx;
+    v = cam.fy * G.p[1] * iz + cam.cy;
+    int x0, y0, x1, y1;
+    tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
+    tt = (x1 - x0) * (y1 - y0);
+    vis = tt > 0;
+  }
+  if (!vis) {
+    *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(0.f, 0.f);
+    out.depth[i] = 0.f;
+    *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
+    out.radius[i] = 0; out.tiles_touched[i] = 0;
+    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+    bl[0] = bl[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (PARTS & 2) {
+      out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
+      out.clamp[i] = 0;
+      bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    return;
+  }
+  const float idet = 1.0f / G.det;
+  const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
+  *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
+  out.depth[i] = G.p[2];
+  const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
+  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
+  out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
+  float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+  constexpr float kLog2e = 1.4426950408889634f;
+  bl[0] = make_float4(u, v, op, G.p[2]);
+  bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
+
+  if (PARTS & 2) colour<DEG>(g, cam, gin.m, i, out, bl);
 }
 
 // Gradients of Y_l with respect to the (unconstrained) direction components.
@@ -653,17 +679,25 @@ static void launch_pb_deg(splx_ctx* ctx, int deg, const splx_gaussians* g, const
 
 }  // namespace
 
-int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
-                       const splx_projected* out) {
-  const RunTable rt = make_runs(plan, part_offsets, PROJ_THREADS, false);
-  if (rt.blocks_total == 0) return SPLX_OK;
+template <int PARTS>
+static void launch_pf(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt, int deg,
+                      const splx_projected* out) {
   const unsigned grid = (unsigned)rt.blocks_total;
   switch (deg) {
-    case 0: k_project_fwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    case 1: k_project_fwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    case 2: k_project_fwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    default: k_project_fwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 0: k_project_fwd<0, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 1: k_project_fwd<1, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 2: k_project_fwd<2, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    default: k_project_fwd<3, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
   }
+}
+
+int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
+                       const splx_projected* out, int parts) {
+  const RunTable rt = make_runs(plan, part_offsets, PROJ_THREADS, false);
+  if (rt.blocks_total == 0) return SPLX_OK;
+  if (parts == 1) launch_pf<1>(ctx, g, plan, rt, deg, out);
+  else if (parts == 2) launch_pf<2>(ctx, g, plan, rt, deg, out);
+  else launch_pf<3>(ctx, g, plan, rt, deg, out);
   SPLX_LAUNCH_CHECK(ctx, "k_project_fwd");
   return SPLX_OK;
 }

@@ -430,6 +430,7 @@ class Trainer:
             self.prepare_adam()
         if self._side is None:
             self._side = torch.cuda.Stream(dev)
+        if getattr(self, "_graphs", None) is None:
             self._ev_target = torch.cuda.Event()
             self._target_dev = torch.empty((1, self.H, self.W, 3), dtype=torch.float32, device=dev)
             self._graphs = {}
@@ -461,6 +462,94 @@ class Trainer:
         if not self.fuse_adam:
             self.adam_step(1)        # outside the graph: its bias correction is a launch argument
         main.synchronize()
+
+    # ---- the same iteration, scheduled so that HBM-bound and latency-bound stages overlap ----------------------
+    def _adam_part(self, sh: bool, step: int, n_views=1):
+        """Adam (a11) on the SH group only, or on the four geometry groups (mean, log_scale, quat, opacity) only."""
+        o = self._offs
+        if sh:
+            a, b = o["sh"], self._total
+            offs, lrs = [0, b - a], [self.lr["sh"]]
+        else:
+            a, b = 0, o["sh"]
+            keys = [k for k in PARAM_KEYS if k != "sh"]
+            offs, lrs = [o[k] for k in keys] + [b], [self.lr[k] for k in keys]
+        f = self.flat
+        self.ctx.adam_groups(f["param"][a:b], f["grad"][a:b], f["m"][a:b], f["v"][a:b], offs, lrs, step=step,
+                             grad_scale=1.0 / n_views)
+
+    def step_overlapped(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
+        """step_graph with the same kernels and the same arithmetic on a different schedule.  Two facts are used:
+        the binning needs only the GEOMETRY half of the projection (which reads 11 of a Gaussian's 59 parameters),
+        and the SH colour is not needed before the blend.  So the Adam step of the SH group -- 81 % of the
+        optimiser's bytes, bound by HBM -- is deferred to a second stream where it runs, followed by the colour half
+        of the next iteration's projection, beside that iteration's geometry half and binning (a chain of small,
+        latency-bound kernels that leaves the memory system idle).  Parameters are complete only after flush()."""
+        assert not self.fuse_adam and not self.sparse_adam
+        dev = self.ctx.device
+        c = self.ctx
+        main = torch.cuda.current_stream(dev)
+        if self._side is None:
+            self._side = torch.cuda.Stream(dev)
+        side = self._side
+        if getattr(self, "_ographs", None) is None:
+            self._ographs = {}
+            self._pending_sh = 0          # step number whose SH half of Adam has not run yet (0 = none)
+            self._ev = [torch.cuda.Event() for _ in range(3)]
+        key = (view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps))
+        if key not in self._ographs:
+            plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
+                           else (self.make_plan([cam]), None))
+            self._workspaces(cam)
+            self._view_buffers(1)
+            self.fused_buffers()
+            bufs = self._bufs(0)
+            torch.cuda.synchronize(dev)
+            graphs = []
+            for body in (lambda: self._bin_sort(self.proj, plan, self.bins, self._ws_sort),
+                         lambda: (self.loss_sum.zero_(), self._back(plan, bufs, target_dev, True, sat_eps, state, False, 1))):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    c.set_stream(torch.cuda.current_stream(dev).cuda_stream)
+                    try:
+                        body()
+                    finally:
+                        c.set_stream(main.cuda_stream)
+                graphs.append(g)
+            self._ographs[key] = (graphs[0], graphs[1], plan)
+        g_sort, g_back, plan = self._ographs[key]
+        self._plan = plan
+        ev_bwd, ev_geom, ev_col = self._ev
+        # main: geometry half (its parameters are final: the geometry groups were stepped on this stream)
+        c.project_parts_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, binding.PROJECT_GEOMETRY)
+        ev_geom.record(main)
+        # side: SH half of the previous step's Adam (after that step's backward), then the colour half
+        c.set_stream(side.cuda_stream)
+        try:
+            if self._pending_sh:
+                side.wait_event(ev_bwd)
+                self._adam_part(True, self._pending_sh)
+                self._pending_sh = 0
+            side.wait_event(ev_geom)
+            c.project_parts_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, binding.PROJECT_COLOUR)
+            ev_col.record(side)
+        finally:
+            c.set_stream(main.cuda_stream)
+        g_sort.replay()                     # a2-a4 beside the side stream's work
+        main.wait_event(ev_col)
+        g_back.replay()                     # a5-a10
+        ev_bwd.record(main)
+        self.step_count += 1
+        self._adam_part(False, self.step_count)
+        self._pending_sh = self.step_count
+
+    def flush(self):
+        """Run what step_overlapped deferred: afterwards every parameter has taken every step."""
+        if getattr(self, "_pending_sh", 0):
+            main = torch.cuda.current_stream(self.ctx.device)
+            main.wait_event(self._ev[0])
+            self._adam_part(True, self._pending_sh)
+            self._pending_sh = 0
 
     def step_graph(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
         """One whole training iteration on one view with the target already on the device ([1,H,W,3]): a1-a10

@@ -570,3 +570,55 @@ def test_sparse_adam_option(blocks):
     gs = tr.grads["sh"].reshape(n, 48)[seen]; gd = dense.grads["sh"].reshape(n, 48)[seen]
     assert not torch.isnan(gs).any()
     assert float((gs - gd).abs().max()) <= 1e-4 * float(gd.abs().max())
+
+
+def test_projection_halves_are_bit_identical(aerial):
+    """splx_project_parts_plan: geometry half then colour half == splx_project_plan, every output array bit for bit."""
+    sc = aerial
+    cam = sc.cameras[0]
+    tr = _trainer(sc)
+    plan = tr.make_plan([cam], [0, 0, -1, 0], None, True)
+    c = tr.ctx
+    names = ["means2d", "depth", "conic_opacity", "rgb", "radius", "tiles_touched", "clamp", "blend"]
+    for nm in names:
+        getattr(tr.proj, nm).fill_(7)
+    c.project_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj)
+    want = {nm: getattr(tr.proj, nm).clone() for nm in names}
+    for nm in names:
+        getattr(tr.proj, nm).fill_(7)
+    c.project_parts_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj, binding.PROJECT_GEOMETRY)
+    c.project_parts_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj, binding.PROJECT_COLOUR)
+    torch.cuda.synchronize()
+    for nm in names:
+        assert torch.equal(getattr(tr.proj, nm).view(torch.uint8), want[nm].view(torch.uint8)), nm
+    with pytest.raises(binding.SplxError):
+        c.project_parts_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj, 4)
+
+
+def test_step_overlapped_equals_step_graph(aerial):
+    """Trainer.step_overlapped (SH Adam deferred to a second stream beside the next geometry + binning) computes what
+    Trainer.step_graph computes: after the first step + flush the parameters and moments are bit-equal (same kernels,
+    same inputs; only g2d atomics could differ and they feed both alike to rounding), after three steps close."""
+    sc = aerial
+    cam = sc.cameras[0]
+    target = torch.from_numpy(sc.targets[0]).cuda()[None]
+    a, b = _trainer(sc), _trainer(sc)
+    for it in range(3):
+        a.step_overlapped(0, cam, target)
+        b.step_graph(0, cam, target)
+        if it == 0:
+            a.flush()
+            torch.cuda.synchronize()
+            assert float(a.loss_sum.item()) == pytest.approx(float(b.loss_sum.item()), rel=1e-6)
+            for key in scenes.PARAM_KEYS:
+                close = torch.isclose(a.params[key], b.params[key], rtol=1e-4, atol=1e-7)
+                assert close.float().mean().item() >= 0.999, key
+    a.flush()
+    torch.cuda.synchronize()
+    assert a.step_count == b.step_count == 3
+    for key in scenes.PARAM_KEYS:
+        close = torch.isclose(a.params[key], b.params[key], rtol=1e-3, atol=1e-6)
+        assert close.float().mean().item() >= 0.999, key
+        assert torch.isfinite(a.params[key]).all()
+    # the deferred half really ran: the SH moments of the third step are there
+    assert torch.allclose(a.m["sh"], b.m["sh"], rtol=1e-2, atol=1e-6)
