@@ -134,66 +134,110 @@ def test_fullsize_work_counters(full):
 
 
 # ---- configs[2]: 10M Gaussians under the launch plan ---------------------------------------------------
-@pytest.fixture(scope="module")
-def full_city():
-    sc = scenes.city()
+@pytest.fixture(scope="module", params=["city_10M", "city_40M", "city_100M"])
+def full_city(request):
+    """configs[2] (host-generated scene, 10M Gaussians, K = 8, 1080p), configs[3] (device-generated, 40M Gaussians,
+    K = 16, 4K views) and configs[4] (device-generated, 100M Gaussians, K = 32, 1080p): one view of the B under the
+    launch plan bench.py uses."""
+    if request.param == "city_10M":
+        sc, cap = scenes.city(), 64_000_000
+    elif request.param == "city_100M":    # configs[4]: 100M Gaussians, 2000 m, 1080p, K = 32, B = 8
+        sc = scenes.city_device(n=100_000_000, width=1920, height=1080, extent=2000.0, n_buildings=3200, grid=(8, 4),
+                                altitude=200.0, height_range=(5.0, 80.0), n_views=8, name="city_100M")
+        cap = 96_000_000
+    else:
+        sc = scenes.city_device(n=40_000_000, width=3840, height=2160, extent=1000.0, n_buildings=800, grid=(4, 4),
+                                altitude=200.0, height_range=(5.0, 60.0), n_views=4, name="city_40M")
+        cap = 160_000_000
     cam = sc.cameras[0]
-    tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=64_000_000)
+    tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=cap)
     tr.set_aabbs(*scenes.partition_aabbs(sc.params, sc.part_offsets))
+    sc.params = None                             # the tests read the trainer's copy (_partition_host)
+    torch.cuda.empty_cache()
     plan, _ = tr.bucket_plan([0], [cam], saturation=False, sparse=True)
     tr.partials.ct.fill_(float("nan"))          # slots the sparse plan never writes must never be read
     tr.forward_plan(plan, count_pairs=True)
     torch.cuda.synchronize()
-    return sc, cam, tr, plan
+    yield sc, cam, tr, plan
+    del tr, plan
+    torch.cuda.empty_cache()
 
 
-def test_city_10M_binning_bit_exact(full_city):
+def _partition_host(tr, k):
+    """Parameters of partition k from the trainer's device buffers, as float64 host arrays in the oracle's shapes."""
+    a, b = int(tr.part_offsets[k]), int(tr.part_offsets[k + 1])
+    out = {}
+    for key in scenes.PARAM_KEYS:
+        w = scenes.PARAM_WIDTH[key]
+        out[key] = tr.params[key].reshape(-1)[w * a:w * b].cpu().numpy().astype(np.float64)
+    out["mean"] = out["mean"].reshape(-1, 3); out["log_scale"] = out["log_scale"].reshape(-1, 3)
+    out["quat"] = out["quat"].reshape(-1, 4); out["sh"] = out["sh"].reshape(-1, 16, 3)
+    return out
+
+
+def _projected_slice(tr, a, b):
+    """oracle.Projected of Gaussians [a, b) from the GPU's projection (only the slice travels to the host)."""
+    p = tr.proj
+    f = lambda t, w: t.reshape(-1)[w * a:w * b].cpu().numpy()
+    return oracle.Projected(f(p.means2d, 2).astype(np.float64).reshape(-1, 2), f(p.depth, 1).astype(np.float64),
+                            f(p.conic_opacity, 4).astype(np.float64).reshape(-1, 4),
+                            f(p.rgb, 3).astype(np.float64).reshape(-1, 3), f(p.radius, 1).copy(),
+                            f(p.tiles_touched, 1).view(np.uint32).copy(), f(p.clamp, 1).copy())
+
+
+def test_city_binning_bit_exact(full_city):
     sc, cam, tr, plan = full_city
     vop = plan.view_of_part
     assert 0 < sum(v == 0 for v in vop) < sc.K, "the view must see some, not all, partitions"
     state = G.np32(plan.tile_state).reshape(sc.K, -1)
-    pr = G.gpu_projected(tr)
     M, keys, vals, ranges = G.gpu_bins(tr)
     ntiles = ranges.shape[1]
-    pos = 0
+    pos = n_cut = n_live = 0
     for k in range(tr.K):
-        a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
+        a, b = int(tr.part_offsets[k]), int(tr.part_offsets[k + 1])
         if vop[k] < 0:
             assert not ranges[k].any()
             continue
-        tt = oracle.count_tiles(pr.means2d[a:b], pr.radius[a:b], cam.width, cam.height)[1]
-        assert np.array_equal(pr.tiles_touched[a:b], tt)
-        ob = oracle.bin_sort(pr.means2d[a:b], pr.radius[a:b], pr.depth[a:b], cam.width, cam.height)
+        pk = _projected_slice(tr, a, b)
+        tt = oracle.count_tiles(pk.means2d, pk.radius, cam.width, cam.height)[1]
+        assert np.array_equal(pk.tiles_touched, tt)
+        ob = oracle.bin_sort(pk.means2d, pk.radius, pk.depth, cam.width, cam.height)
         assert np.array_equal(keys[pos:pos + ob.M], ob.keys + (np.uint64(k * ntiles) << np.uint64(32)))
         assert np.array_equal(vals[pos:pos + ob.M], ob.vals + np.uint32(a))
         want = ob.ranges.copy(); want[state[k] != 0] = 0       # skipped slots lose their list (DESIGN.md s28)
         live = want[:, 1] > want[:, 0]
         assert np.array_equal(ranges[k][live], want[live] + np.uint32(pos))
         assert not ranges[k][~live].any()
-        # the boxes hold every 3-sigma support: the geometric state cuts no list
-        assert np.array_equal(live, ob.ranges[:, 1] > ob.ranges[:, 0])
+        # the boxes hold every 3-sigma support in 3-D; the 2-D footprint (dilated, rounded up to whole pixels, a square
+        # around the ellipse) can still reach a tile the projected box does not: such a slot loses its list (s28, the
+        # oracle's `want` above does the same).  None at 1080p; a handful of border tiles at 4K.
+        ob_live = ob.ranges[:, 1] > ob.ranges[:, 0]
+        n_cut += int((ob_live & ~live).sum()); n_live += int(ob_live.sum())
         pos += ob.M
-    assert pos == M and M > 5_000_000
+    assert pos == M and M > 2_000_000
+    assert n_cut <= 2e-3 * n_live, (n_cut, n_live)
+    if tr.n == 10_000_000:
+        assert n_cut == 0
 
 
-def test_city_10M_pixels_and_gradients_on_sampled_tiles(full_city):
+def test_city_pixels_and_gradients_on_sampled_tiles(full_city):
     sc, cam, tr, plan = full_city
     vop = plan.view_of_part
     W, H = cam.width, cam.height
     TX, TY = (W + 15) // 16, (H + 15) // 16
     tiles = np.sort(np.random.default_rng(32).choice(TX * TY, 32, replace=False)).astype(np.int32)
     mask = _tile_mask(tiles, W, H)
-    pr = G.gpu_projected(tr)
     M, keys, vals, ranges = G.gpu_bins(tr)
     members = [k for k in range(tr.K) if vop[k] == 0]
+    prs = {k: _projected_slice(tr, int(tr.part_offsets[k]), int(tr.part_offsets[k + 1])) for k in members}
     ct_gpu = np.zeros((len(members), H, W, 4)); ct_gpu[..., 3] = 1.0
     d_gpu = np.zeros((len(members), H, W))
     frag = np.zeros((H, W), bool)
     for j, k in enumerate(members):
         a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
         lv = (vals - np.uint32(a)).astype(np.uint32)
-        ref = oracle.render_partial(pr.means2d[a:b], pr.conic_opacity[a:b], pr.rgb[a:b], pr.depth[a:b], lv, ranges[k],
-                                    W, H, tile_list=tiles)
+        pk = prs[k]
+        ref = oracle.render_partial(pk.means2d, pk.conic_opacity, pk.rgb, pk.depth, lv, ranges[k], W, H, tile_list=tiles)
         # the GPU's partial on the sampled tiles; a slot with an empty list was never written: it IS the identity
         ck = G.np32(tr.partials.ct[k]).astype(np.float64); dk = G.np32(tr.partials.d[k]).astype(np.float64)
         for t in tiles:
@@ -226,16 +270,16 @@ def test_city_10M_pixels_and_gradients_on_sampled_tiles(full_city):
     for j, k in enumerate(members):
         a, b = tr.part_offsets[k], tr.part_offsets[k + 1]
         lv = (vals - np.uint32(a)).astype(np.uint32)
-        g2 = oracle.raster_bwd(pr.means2d[a:b], pr.conic_opacity[a:b], pr.rgb[a:b], lv, ranges[k], W, H, g_ct[j],
-                               tile_list=tiles)
+        pk = prs[k]
+        g2 = oracle.raster_bwd(pk.means2d, pk.conic_opacity, pk.rgb, lv, ranges[k], W, H, g_ct[j], tile_list=tiles)
         if not any(np.abs(x).max() > 0 for x in g2):
             continue                                  # this partition has no list on the sampled tiles
-        p = sc.partition(k)
+        p = _partition_host(tr, k)
         ref = oracle.project_bwd(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sc.sh_degree,
-                                 cam.as_array(), pr.radius[a:b], pr.clamp[a:b], *g2)
+                                 cam.as_array(), pk.radius, pk.clamp, *g2)
         for key in scenes.PARAM_KEYS:
             w = scenes.PARAM_WIDTH[key]
-            got = G.np32(tr.grads[key]).reshape(-1, w)[a:b].astype(np.float64)
+            got = tr.grads[key].reshape(-1)[w * a:w * b].cpu().numpy().reshape(-1, w).astype(np.float64)
             r = ref[key].reshape(-1, w)
             assert G.rel_l2(got, r) <= 1e-3, (k, key, G.rel_l2(got, r))
             assert G.grad_close(got, r) <= 5e-3, (k, key)
