@@ -108,7 +108,15 @@ typedef struct {
   uint32_t *tile_ranges;
   uint64_t capacity;
   uint64_t *num_intersections;
+  /* Optional (NULL = off), DEVICE uint32[K*TX*TY + SPLX_ORDER_EXTRA], written by splx_bin_sort*: the slots with a
+   * non-empty list ordered by DESCENDING list length (to ~3 %: 1024 log-linear length classes, arbitrary order inside
+   * a class), then their count at index K*TX*TY, then scratch.  The blend kernels (render_partial with
+   * SPLX_PLAN_SPARSE, raster_backward) then hand out their CTAs in this order -- longest list first -- instead
+   * of tile order, which shortens the tail of the launch; results are unchanged (a slot's output does not depend on
+   * when it is computed). */
+  uint32_t *slot_order;
 } splx_binning;
+#define SPLX_ORDER_EXTRA 1025
 
 /* Partial pixels of all K partitions (Eq.3-4): ct[K,H,W,4] =
  * (premultiplied C^k rgb, T^k), d[K,H,W] = D^k = sum d_i alpha_i T_i, n_contrib[K,H,W] =

@@ -39,6 +39,7 @@ EXPORTS = [
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
 PLAN_SPARSE = 1
+ORDER_EXTRA = 1025
 PROJECT_GEOMETRY, PROJECT_COLOUR = 1, 2
 
 
@@ -72,7 +73,7 @@ class ProjectedS(C.Structure):
 
 class BinningS(C.Structure):
     _fields_ = [("keys", C.c_void_p), ("vals", C.c_void_p), ("tile_ranges", C.c_void_p),
-                ("capacity", C.c_uint64), ("num_intersections", C.c_void_p)]
+                ("capacity", C.c_uint64), ("num_intersections", C.c_void_p), ("slot_order", C.c_void_p)]
 
 
 class PartialS(C.Structure):
@@ -275,10 +276,13 @@ class Binning:
         self.vals = torch.empty(max(self.capacity, 4), dtype=torch.int32, device=device)     # uint32 bits
         self.tile_ranges = torch.zeros((K * self.TX * self.TY, 2), dtype=torch.int32, device=device)
         self.num_intersections = torch.zeros(2, dtype=torch.int64, device=device)
+        #: slots by descending list length (splx_binning.slot_order); set to None to hand out CTAs in tile order
+        self.slot_order = (torch.zeros(K * self.TX * self.TY + ORDER_EXTRA, dtype=torch.int32, device=device)
+                           if os.environ.get("SPLX_SLOT_ORDER", "1") == "1" else None)
 
     def struct(self):
         return BinningS(_ptr(self.keys), _ptr(self.vals), _ptr(self.tile_ranges), self.capacity,
-                        _ptr(self.num_intersections))
+                        _ptr(self.num_intersections), _ptr(self.slot_order))
 
 
 class Partial:

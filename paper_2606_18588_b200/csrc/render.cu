@@ -126,9 +126,14 @@ __global__ void __launch_bounds__(BLOCK, SPLX_FWD_MIN_CTAS)
 k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const __grid_constant__ PartView pv, int sparse,
              float* __restrict__ out_ct, float* __restrict__ out_d, uint32_t* __restrict__ out_n,
-             unsigned long long* pairs) {
+             unsigned long long* pairs, const uint32_t* __restrict__ order, uint32_t nslots) {
   __shared__ Ring rings[WARPS];
-  const int tile = blockIdx.x, k = blockIdx.y;
+  int tile = blockIdx.x, k = blockIdx.y;
+  if (order) {                             // CTAs handed out longest list first (splx_binning.slot_order)
+    if (blockIdx.x >= order[nslots]) return;
+    const uint32_t s = order[blockIdx.x];
+    k = (int)(s / (uint32_t)ntiles); tile = (int)(s - (uint32_t)k * (uint32_t)ntiles);
+  }
   if (pv.v[k] < 0) return;                 // the partition does not participate in this launch
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   Ring& ring = rings[warp];
@@ -265,10 +270,16 @@ __device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int la
 __global__ void __launch_bounds__(BLOCK, SPLX_BWD_MIN_CTAS)
 k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const float* __restrict__ ct,
-             const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d) {
+             const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d,
+             const uint32_t* __restrict__ order, uint32_t nslots) {
   __shared__ Ring rings[WARPS];
   __shared__ Stage stages[WARPS];
-  const int tile = blockIdx.x, k = blockIdx.y;
+  int tile = blockIdx.x, k = blockIdx.y;
+  if (order) {                             // CTAs handed out longest list first (splx_binning.slot_order)
+    if (blockIdx.x >= order[nslots]) return;
+    const uint32_t s = order[blockIdx.x];
+    k = (int)(s / (uint32_t)ntiles); tile = (int)(s - (uint32_t)k * (uint32_t)ntiles);
+  }
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
   if (r0 == r1) return;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -385,25 +396,31 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 
 int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, const PlanDev& plan,
                       const splx_partial* out, uint64_t* pairs) {
-  dim3 grid(plan.ntiles, plan.K);
   const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
+  const uint32_t nslots = (uint32_t)plan.ntiles * (uint32_t)plan.K;
+  // longest list first only where empty slots need no visit (without SPLX_PLAN_SPARSE they get the identity partial)
+  const uint32_t* order = sparse ? bins->slot_order : nullptr;
+  const dim3 grid = order ? dim3(nslots, 1) : dim3(plan.ntiles, plan.K);
   if (pairs)
     k_render_fwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
                                                         plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d,
-                                                        out->n_contrib, (unsigned long long*)pairs);
+                                                        out->n_contrib, (unsigned long long*)pairs, order, nslots);
   else
     k_render_fwd<false><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
                                                          plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d,
-                                                         out->n_contrib, nullptr);
+                                                         out->n_contrib, nullptr, order, nslots);
   SPLX_LAUNCH_CHECK(ctx, "k_render_fwd");
   return SPLX_OK;
 }
 
 int launch_raster_bwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, const PlanDev& plan,
                       const splx_partial* part, const float* g_ct, float* g2d) {
-  dim3 grid(plan.ntiles, plan.K);   // slots of non-participating partitions have empty ranges and exit at once
+  const uint32_t nslots = (uint32_t)plan.ntiles * (uint32_t)plan.K;
+  const uint32_t* order = bins->slot_order;
+  // slots of non-participating partitions have empty ranges: they exit at once / are not in the order
+  const dim3 grid = order ? dim3(nslots, 1) : dim3(plan.ntiles, plan.K);
   k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
-                                                plan.ntiles, ctx->cfg, part->ct, part->n_contrib, g_ct, g2d);
+                                                plan.ntiles, ctx->cfg, part->ct, part->n_contrib, g_ct, g2d, order, nslots);
   SPLX_LAUNCH_CHECK(ctx, "k_raster_bwd");
   return SPLX_OK;
 }

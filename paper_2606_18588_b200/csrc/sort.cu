@@ -689,6 +689,62 @@ k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint
   }
 }
 
+// ---- slots by descending list length (splx_binning.slot_order) ----------------------------------------------
+// The blend kernels' CTAs differ in work by two orders of magnitude (list lengths); handed out in tile order, a long
+// list that starts late is the tail of the launch.  Longest-first needs no exact sort: 1024 log-linear length classes
+// (5 mantissa bits: 3 % resolution), a histogram, a descending scan and a scatter with atomic cursors.
+constexpr int ORD_CLASSES = 1024;
+__device__ __forceinline__ uint32_t length_class(uint32_t len) {   // len >= 1; monotonic in len
+  const int e = 31 - __clz(len);
+  const uint32_t m = e >= 5 ? (len >> (e - 5)) & 31u : (len << (5 - e)) & 31u;
+  return (uint32_t)e * 32u + m;
+}
+
+__global__ void __launch_bounds__(256)
+k_order_hist(const uint32_t* __restrict__ ranges, uint32_t nslots, uint32_t* __restrict__ hist) {
+  __shared__ uint32_t s_h[ORD_CLASSES];
+  for (int x = threadIdx.x; x < ORD_CLASSES; x += 256) s_h[x] = 0;
+  __syncthreads();
+  for (uint32_t s = blockIdx.x * 256 + threadIdx.x; s < nslots; s += gridDim.x * 256) {
+    const uint2 r = reinterpret_cast<const uint2*>(ranges)[s];
+    if (r.y > r.x) atomicAdd(&s_h[length_class(r.y - r.x)], 1u);
+  }
+  __syncthreads();
+  for (int x = threadIdx.x; x < ORD_CLASSES; x += 256) if (s_h[x]) atomicAdd(&hist[x], s_h[x]);
+}
+
+// One CTA: class c (thread t = 1023 - c, so that the scan runs from the longest class down) gets the first output
+// position of its slots; the total is the number of live slots.
+__global__ void __launch_bounds__(ORD_CLASSES)
+k_order_scan(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_live) {
+  __shared__ uint32_t s_w[32];
+  const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+  const uint32_t c = hist[ORD_CLASSES - 1 - t];
+  uint32_t inc = c;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+  if (lane == 31) s_w[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t x = s_w[lane];
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += v; }
+    s_w[lane] = x;
+  }
+  __syncthreads();
+  const uint32_t before = (w ? s_w[w - 1] : 0u) + inc - c;
+  hist[ORD_CLASSES - 1 - t] = before;
+  if (t == ORD_CLASSES - 1) *n_live = before + c;
+}
+
+__global__ void __launch_bounds__(256)
+k_order_scatter(const uint32_t* __restrict__ ranges, uint32_t nslots, uint32_t* __restrict__ cursor, uint32_t* __restrict__ order) {
+  for (uint32_t s = blockIdx.x * 256 + threadIdx.x; s < nslots; s += gridDim.x * 256) {
+    const uint2 r = reinterpret_cast<const uint2*>(ranges)[s];
+    if (r.y > r.x) order[atomicAdd(&cursor[length_class(r.y - r.x)], 1u)] = s;
+  }
+}
+
 __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_total; }
 
 // Workspace: a small zero-initialised control region (counters, tickets, digit histograms, the scans' status
@@ -765,6 +821,8 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->tile_ranges, 0, (size_t)K * ntiles * 2 * sizeof(uint32_t), ctx->stream));
   const RunTable rt = make_runs(plan, part_offsets, 1, false);
   const int64_t n_act = rt.jprefix[rt.n];    // Gaussians of the participating partitions
+  if (out->slot_order)   // count of live slots and the class cursors
+    SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->slot_order + (size_t)K * ntiles, 0, SPLX_ORDER_EXTRA * sizeof(uint32_t), ctx->stream));
   if (n_act == 0 || out->capacity == 0) {
     k_publish_m<<<1, 1, 0, ctx->stream>>>(cnt, out->num_intersections);
     SPLX_LAUNCH_CHECK(ctx, "k_publish_m");
@@ -823,5 +881,17 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
       out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections, cx.nslots, cx.mask != nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
+  if (out->slot_order) {
+    const uint32_t nslots = (uint32_t)K * (uint32_t)ntiles;
+    uint32_t* n_live = out->slot_order + nslots;
+    uint32_t* cursor = n_live + 1;
+    const unsigned ob = (nslots + 255) / 256 < 2 * PERSISTENT_CTAS ? (nslots + 255) / 256 : 2 * PERSISTENT_CTAS;
+    k_order_hist<<<ob, 256, 0, ctx->stream>>>(out->tile_ranges, nslots, cursor);
+    SPLX_LAUNCH_CHECK(ctx, "k_order_hist");
+    k_order_scan<<<1, ORD_CLASSES, 0, ctx->stream>>>(cursor, n_live);
+    SPLX_LAUNCH_CHECK(ctx, "k_order_scan");
+    k_order_scatter<<<ob, 256, 0, ctx->stream>>>(out->tile_ranges, nslots, cursor, out->slot_order);
+    SPLX_LAUNCH_CHECK(ctx, "k_order_scatter");
+  }
   return SPLX_OK;
 }

@@ -46,7 +46,7 @@ def test_struct_sizes_match_the_header(libpath):
     assert ctypes.sizeof(b.Config) == 24
     assert ctypes.sizeof(b.CameraS) == 4 * (9 + 3 + 4) + 8 + 4
     assert ctypes.sizeof(b.GaussiansS) == 48 and ctypes.sizeof(b.ProjectedS) == 64
-    assert ctypes.sizeof(b.BinningS) == 40 and ctypes.sizeof(b.PartialS) == 24
+    assert ctypes.sizeof(b.BinningS) == 48 and ctypes.sizeof(b.PartialS) == 24
 
 
 def test_no_cpu_fallback_without_a_device(libpath):

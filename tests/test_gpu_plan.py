@@ -622,3 +622,38 @@ def test_step_overlapped_equals_step_graph(aerial):
         assert torch.isfinite(a.params[key]).all()
     # the deferred half really ran: the SH moments of the third step are there
     assert torch.allclose(a.m["sh"], b.m["sh"], rtol=1e-2, atol=1e-6)
+
+
+def test_slot_order_is_longest_first_and_changes_nothing(aerial):
+    """splx_binning.slot_order: a permutation of the slots with a non-empty list, list lengths descending up to the
+    3 % length classes; the blend kernels produce bit-equal partials with and without it, the backward equal gradients."""
+    sc = aerial
+    cam = sc.cameras[0]
+    target = torch.from_numpy(sc.targets[0]).cuda()[None]
+    a, b = _trainer(sc), _trainer(sc)
+    assert a.bins.slot_order is not None
+    b.bins.slot_order = None
+    out = []
+    for tr in (a, b):
+        tr.partials.ct.fill_(float("nan")); tr.partials.d.fill_(float("nan")); tr.partials.n_contrib.fill_(-1)
+        plan = tr.make_plan([cam], None, None, True)
+        img = tr.forward_plan(plan).clone()
+        tr.loss_grad_plan(target)
+        tr.backward_plan(overwrite=True)
+        torch.cuda.synchronize()
+        out.append((img, tr.partials.ct.clone(), tr.partials.d.clone(), tr.partials.n_contrib.clone(), _grads_np(tr)))
+    for x, y in zip(out[0][:4], out[1][:4]):
+        assert torch.equal(x.view(torch.int32), y.view(torch.int32))
+    for key in scenes.PARAM_KEYS:
+        assert G.grad_close(out[0][4][key], out[1][4][key]) <= 1e-4, key
+    ranges = G.u32(a.bins.tile_ranges).reshape(-1, 2).astype(np.int64)
+    length = ranges[:, 1] - ranges[:, 0]
+    nslots = length.shape[0]
+    order = G.u32(a.bins.slot_order)
+    n_live = int(order[nslots])
+    assert n_live == int((length > 0).sum())
+    assert np.array_equal(np.sort(order[:n_live]), np.nonzero(length > 0)[0])
+    ln = length[order[:n_live]].astype(np.float64)
+    # descending up to the class width (5 mantissa bits: a later slot is never more than 1/32 longer ... of its binade)
+    assert np.all(ln[1:] <= ln[:-1] * (1 + 1 / 16.0) + 1)
+    assert ln[0] == length.max()
