@@ -127,9 +127,20 @@ __device__ __forceinline__ int find_run(const RunTable& rt, int b) {
   return lo;
 }
 
-// colour: SH along the direction from the camera centre to the mean (s13)
-template <int DEG>
-__device__ __forceinline__ void colour(const splx_gaussians& g, const CamDev& cam, const float* m, int64_t i,
+// Position of chunk q of row `row` inside the row's NV chunks of the staged copy.  Degree 3 (12 chunks = 192 B, no
+// padding): XOR with the row so that the row-wise LDS.128 of a quarter warp spreads over the bank groups (chunks 0-7
+// conflict-free, chunks 8-11 two-way); smaller rows are left in place.
+template <int NV>
+__device__ __forceinline__ int sh_swz(int q, int row) {
+  if (NV == 12) return q < 8 ? (q ^ (row & 7)) : 8 + ((q - 8) ^ (row & 3));
+  return q;
+}
+
+// colour: SH along the direction from the camera centre to the mean (s13).  The coefficients come from `sh4`
+// (the Gaussian's row in global memory, chunk q at sh4[q]) or, STAGED, from the warp's shared-memory copy of its 32
+// rows (chunk q of row `lane` at sh4[lane * NV + sh_swz<NV>(q, lane)]).
+template <int DEG, bool STAGED>
+__device__ __forceinline__ void colour(const float4* sh4, int lane, const CamDev& cam, const float* m, int64_t i,
                                        const splx_projected& out, float4* bl) {
   float dx = m[0] - cam.o[0], dy = m[1] - cam.o[1], dz = m[2] - cam.o[2];
   const float dinv = rsqrtf(dx * dx + dy * dy + dz * dz);
@@ -137,12 +148,11 @@ __device__ __forceinline__ void colour(const splx_gaussians& g, const CamDev& ca
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   float Y[NSH];
   sh_eval(DEG, dx, dy, dz, Y);
-  const float4* sh4 = reinterpret_cast<const float4*>(g.sh + 48 * i);
   float c[3] = {0.5f, 0.5f, 0.5f};
   constexpr int NV = (NSH * 3 + 3) / 4;
 #pragma unroll
   for (int q = 0; q < NV; ++q) {
-    const float4 f = __ldg(sh4 + q);
+    const float4 f = STAGED ? sh4[lane * NV + sh_swz<NV>(q, lane)] : __ldg(sh4 + q);
     const float e[4] = {f.x, f.y, f.z, f.w};
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
@@ -164,71 +174,102 @@ __device__ __forceinline__ void colour(const splx_gaussians& g, const CamDev& ca
 // records 0-1 of the blend layout), 2 = the colour (SH -> rgb, clamp bits, record 2), 3 = both in one pass.  The
 // colour half reads tiles_touched written by the geometry half to know whether the Gaussian is visible; it depends
 // on nothing else of it, so a caller may run it beside the binning (splx_project_parts_plan).
+//
+// SH rows: a thread-per-Gaussian read of its 192-byte row is a 192-byte stride across the warp -- every 16-byte load
+// instruction touches 32 different lines (32 L1 wavefronts instead of 4) and the kernel ran at half the HBM roof,
+// bound by the L1's wavefront rate (profiles/r01e: lg_throttle + long_scoreboard).  The 32 rows of a warp are 6 KB of
+// CONTIGUOUS memory, so when at least SH_STAGE_MIN of them are visible the warp copies the block with coalesced
+// 16-byte cp.async into shared memory (chunk index XOR-swizzled by the row so that the row-wise LDS.128 of a quarter
+// warp hits eight different bank groups) and reads its rows from there; with fewer visible rows (the culled
+// partitions of a city view) the direct loads touch less memory and are kept.
+constexpr int SH_STAGE_MIN = 12;
 template <int DEG, int PARTS>
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected out) {
+  constexpr int NSH = (DEG + 1) * (DEG + 1);
+  constexpr int NV = (NSH * 3 + 3) / 4;
+  constexpr bool STAGE = (PARTS & 2) && DEG > 0;
+  __shared__ __align__(16) float4 s_sh[STAGE ? PROJ_THREADS * NV : 1];
   const int r = find_run(rt, (int)blockIdx.x);
   const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
-  if (i >= rt.end[r]) return;
+  const bool active = i < rt.end[r];
   const CamDev& cam = plan.cam[rt.view[r]];   // the view this partition renders (indexed constant-bank loads)
+  float m[3] = {0.f, 0.f, 0.f};
+  bool vis = false;
   if (PARTS == 2) {
-    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-    if (out.tiles_touched[i] == 0) {
-      out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
-      out.clamp[i] = 0;
-      bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
-      return;
+    if (active) {
+      vis = out.tiles_touched[i] != 0;
+      if (vis) { m[0] = g.mean[3 * i]; m[1] = g.mean[3 * i + 1]; m[2] = g.mean[3 * i + 2]; }
     }
-    const float m[3] = {g.mean[3 * i], g.mean[3 * i + 1], g.mean[3 * i + 2]};
-    colour<DEG>(g, cam, m, i, out, bl);
-    return;
-  }
-  Geo G;
-  const GeoIn gin = load_geo(g, i);
-  bool vis = geometry(gin, cam, cfg.dilation, G);
-  float u = 0.f, v = 0.f;
-  int rad = 0, tt = 0;
-  if (vis) {
-    const float mid = 0.5f * (G.a + G.c);
-    const float hd = 0.5f * (G.a - G.c);
-    const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
-    rad = (int)ceilf(3.0f * sqrtf(lam));
-    const float iz = 1.0f / G.p[2];
-    u = cam.fx * G.p[0] * iz + cam.cx;
-    v = cam.fy * G.p[1] * iz + cam.cy;
-    int x0, y0, x1, y1;
-    tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
-    tt = (x1 - x0) * (y1 - y0);
-    vis = tt > 0;
-  }
-  if (!vis) {
-    *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(0.f, 0.f);
-    out.depth[i] = 0.f;
-    *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
-    out.radius[i] = 0; out.tiles_touched[i] = 0;
-    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-    bl[0] = bl[1] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (PARTS & 2) {
-      out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
-      out.clamp[i] = 0;
-      bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
+  } else if (active) {
+    Geo G;
+    const GeoIn gin = load_geo(g, i);
+    vis = geometry(gin, cam, cfg.dilation, G);
+    float u = 0.f, v = 0.f;
+    int rad = 0, tt = 0;
+    if (vis) {
+      const float mid = 0.5f * (G.a + G.c);
+      const float hd = 0.5f * (G.a - G.c);
+      const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
+      rad = (int)ceilf(3.0f * sqrtf(lam));
+      const float iz = 1.0f / G.p[2];
+      u = cam.fx * G.p[0] * iz + cam.cx;
+      v = cam.fy * G.p[1] * iz + cam.cy;
+      int x0, y0, x1, y1;
+      tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
+      tt = (x1 - x0) * (y1 - y0);
+      vis = tt > 0;
     }
-    return;
+    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+    if (!vis) {
+      *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(0.f, 0.f);
+      out.depth[i] = 0.f;
+      *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
+      out.radius[i] = 0; out.tiles_touched[i] = 0;
+      bl[0] = bl[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {
+      const float idet = 1.0f / G.det;
+      const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
+      *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
+      out.depth[i] = G.p[2];
+      const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
+      *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
+      out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
+      constexpr float kLog2e = 1.4426950408889634f;
+      bl[0] = make_float4(u, v, op, G.p[2]);
+      bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
+      m[0] = gin.m[0]; m[1] = gin.m[1]; m[2] = gin.m[2];
+    }
   }
-  const float idet = 1.0f / G.det;
-  const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
-  *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
-  out.depth[i] = G.p[2];
-  const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
-  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
-  out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
+  if (!(PARTS & 2)) return;
   float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-  constexpr float kLog2e = 1.4426950408889634f;
-  bl[0] = make_float4(u, v, op, G.p[2]);
-  bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
-
-  if (PARTS & 2) colour<DEG>(g, cam, gin.m, i, out, bl);
+  if (active && !vis) {
+    out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
+    out.clamp[i] = 0;
+    bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  const int lane = threadIdx.x & 31;
+  const unsigned vmask = __ballot_sync(0xffffffffu, vis);
+  if (vmask == 0) return;
+  if (STAGE && __popc(vmask) >= SH_STAGE_MIN) {
+    float4* ws = s_sh + (threadIdx.x & ~31) * NV;                 // this warp's 32 rows
+    const int64_t i0 = i - lane;                                   // first Gaussian of the warp
+    const int64_t left = rt.end[r] - i0;
+    const int rows = (int)(left < 32 ? left : 32);
+    const float4* src = reinterpret_cast<const float4*>(g.sh + 48 * i0);
+    for (int c = lane; c < rows * NV; c += 32) {
+      const int row = c / NV, q = c - row * NV;
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(ws + row * NV + sh_swz<NV>(q, row));
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (size_t)row * 12 + q));
+    }
+    asm volatile("cp.async.commit_group;");
+    asm volatile("cp.async.wait_group 0;");
+    __syncwarp();
+    if (vis) colour<DEG, true>(ws, lane, cam, m, i, out, bl);
+    return;
+  }
+  if (vis) colour<DEG, false>(reinterpret_cast<const float4*>(g.sh + 48 * i), lane, cam, m, i, out, bl);
 }
 
 // Gradients of Y_l with respect to the (unconstrained) direction components.
