@@ -37,8 +37,8 @@ FLOPS_BLEND_BWD = 55  # one contributing pair in the backward incl. its 9 reduct
 FP32_LANES_PER_SM = 128
 SM_COUNT = 148
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on aerial_1M, from the `ncu --set full` capture summarised in
-# profiles/r01d_ncu_full.csv (a profiler number, copied here by hand; null for other workloads)
-NCU_TRAFFIC_BYTES = {"aerial_1M": {"k_raster_bwd": 217.5e6, "k_render_fwd": 89.1e6, "adam": 1597.4e6, "project_backward": 520.4e6}}
+# profiles/r01e_ncu_full.csv (a profiler number, copied here by hand; null for other workloads)
+NCU_TRAFFIC_BYTES = {"aerial_1M": {"k_raster_bwd": 250.9e6, "k_render_fwd": 86.7e6, "adam": 1598.0e6, "project_backward": 520.9e6}}
 
 
 def workload(name):
