@@ -188,3 +188,37 @@ def test_plan_capacity_overflow_and_bad_plans_are_reported():
         assert e.value.code == binding.ERR_INVALID_ARG
     with pytest.raises(binding.SplxError):                            # sparse compose without the binning
         tr.ctx.compose_plan(tr.partials, None, plan, tr.bg, tr._images[:1])
+
+
+def test_cross_boundary_argument_errors_and_degenerate_inputs():
+    """splx_cross_sets / splx_bin_sort_filtered_plan: invalid boxes and K are refused; one partition has no Q_cross;
+    a NULL mask is the unfiltered binning."""
+    import numpy as np
+    from paper_2606_18588_b200 import binding, scenes
+    sc = scenes.small_aerial(n=3000)
+    tr = G.make_trainer(sc)
+    lo, hi = scenes.partition_aabbs(sc.params, sc.part_offsets, inflate_sigma=0.0)
+    mask = torch.empty(tr.n, dtype=torch.int64, device="cuda")
+    bad_hi = hi.copy(); bad_hi[1, 0] = lo[1, 0] - 1.0
+    with pytest.raises(binding.SplxError):
+        tr.ctx.cross_sets(tr.params, tr.part_offsets, lo, bad_hi, mask)
+    with pytest.raises(binding.SplxError):
+        tr.ctx.cross_sets(tr.params, tr.part_offsets, lo, hi, mask, support_sigma=-1.0)
+    with pytest.raises(binding.SplxError):
+        tr.ctx.cross_sets(tr.params, tr.part_offsets, lo[:2], hi[:2], mask)      # K does not match part_offsets
+    # a single partition: nothing to cross into
+    one = np.array([0, tr.n], np.int64)
+    tr.ctx.cross_sets(tr.params, one, lo.min(0, keepdims=True), hi.max(0, keepdims=True), mask)
+    torch.cuda.synchronize()
+    assert not mask.any()
+    # NULL mask == splx_bin_sort_plan
+    cam = sc.cameras[0]
+    plan = tr.make_plan([cam], None, None, False)
+    tr._workspaces(cam)
+    tr.ctx.project_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj)
+    tr.ctx.bin_sort_plan(tr.proj, tr.part_offsets, plan, tr.bins, tr._ws_sort)
+    M0, k0, v0, r0 = G.gpu_bins(tr)
+    k0, v0, r0 = k0.copy(), v0.copy(), r0.copy()
+    tr.ctx.bin_sort_filtered_plan(tr.proj, tr.part_offsets, plan, None, np.zeros((tr.K, 2), np.float32), tr.bins, tr._ws_sort)
+    M1, k1, v1, r1 = G.gpu_bins(tr)
+    assert M1 == M0 and np.array_equal(k1, k0) and np.array_equal(v1, v0) and np.array_equal(r1, r0)

@@ -142,3 +142,22 @@ def test_fig25_worked_example():
     assert np.abs(unfiltered[r2] - ref4[r2]).max() > 1e-2
     np.testing.assert_allclose(filtered[r1], ref4[r1], rtol=0, atol=1e-12)
     assert np.abs(ref4[r1] - np.array([0.1, 0.2, 0.3])).max() > 1e-2     # G3 does show at r1
+
+
+def test_host_depth_ranges_match_the_oracle():
+    """splx_cross_depth_ranges is a HOST computation of the product: checked here without a GPU."""
+    from paper_2606_18588_b200 import binding, scenes
+    cams = [scenes.aerial_camera(96, 80, 60.0, 30.0, 40.0, 30.0, (1.0, 2.0, 0.0)),
+            scenes.aerial_camera(96, 80, 60.0, 25.0, 55.0, 200.0, (-3.0, 1.0, 0.0))]
+    lo = np.array([[-20.0, -20, 0], [0, -20, 0], [-20, 0, 0], [0, 0, 0]], np.float32)
+    hi = np.array([[0.0, 0, 8], [20, 0, 8], [0, 20, 8], [20, 20, 8]], np.float32)
+    vop = [0, 1, -1, 1]
+    plan = binding.Plan(cams, vop, None, False)
+    got = binding.cross_depth_ranges(lo, hi, plan)
+    ref = oc.depth_ranges(lo, hi, [c.as_array() for c in cams], vop)
+    assert got.dtype == np.float32 and got.shape == (4, 2)
+    assert got[2].tolist() == [np.inf, -np.inf]
+    np.testing.assert_allclose(got[[0, 1, 3]], ref[[0, 1, 3]], rtol=1e-6)
+    assert abs(got[1, 0] - got[0, 0]) > 1e-3          # the two views really differ
+    with np.testing.assert_raises(binding.SplxError):
+        binding.cross_depth_ranges(lo[:0], hi[:0], plan)
