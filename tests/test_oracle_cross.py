@@ -119,7 +119,21 @@ def test_fig25_worked_example():
         return v, r
 
     filtered, fbins = _render(parts, cam, lists)
-    # only G3 (partition 0, local index 1) is in Q_cross, against partition 1
+    # the paper's statements about the figure (tests/golden/fig25_cross_boundary.txt)
+    import os
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "fig25_cross_boundary.txt")):
+        if line.strip() and not line.startswith("#"):
+            w = line.split()
+            gold.setdefault(w[0], []).append(w[1:])
+    part_of = {g: int(k) for g, k in gold["partition_of"]}
+    assert part_of == {"G1": 0, "G2": 1, "G3": 0, "G4": 1}          # how _fig25 lays the scene out
+    local = {"G1": 0, "G3": 1, "G2": 0, "G4": 1}                    # index inside the partition (by depth)
+    in_cross = {g for (g,) in gold["q_cross"]}
+    for g in part_of:                                               # only G3 is in Q_cross, against partition 1
+        assert bool(Fs[part_of[g]][local[g]].any()) == (g in in_cross), g
+    assert gold["removed"] == [["r2", "G3"]] and gold["retained"] == [["r1", "G3"]]
+    assert gold["filtered_sequence"] == [["r2", "G1", "G2", "G4"]]
     assert Fs[0].tolist() == [[False, False], [False, True]] and not Fs[1].any()
     r1, r2 = (64, 24), (64, 64)                      # (row, column): r1 sees partition 0 only, r2 both
     t1, t2 = (r1[0] // 16) * TX + r1[1] // 16, (r2[0] // 16) * TX + r2[1] // 16
