@@ -64,6 +64,11 @@ struct CrossDev {
   float zlo[SPLX_MAX_K], zhi[SPLX_MAX_K];
 };
 
+// splx_binning.slot_order is built and used only where it pays: measured +1 % to +6 % at 1080p (8160 tiles, K = 4..32:
+// few waves of blend CTAs, the tail matters) and -0.5 % at 4K (32400 tiles, K = 16: many waves, and the order costs
+// locality in L2).  One rule for the producer (bin_sort) and the consumers (blend kernels).
+static inline bool slot_order_pays(const PlanDev& p) { return p.ntiles <= 16384; }
+
 // Contiguous runs of Gaussians (one per participating partition) covered by ONE launch of a
 // per-Gaussian kernel: block b works on run r with block_prefix[r] <= b < block_prefix[r+1].
 // view[r] < 0 marks a run of a non-participating partition (only present when its outputs must

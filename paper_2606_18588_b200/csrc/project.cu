@@ -182,6 +182,9 @@ __device__ __forceinline__ void colour(const float4* sh4, int lane, const CamDev
 // 16-byte cp.async into shared memory (chunk index XOR-swizzled by the row so that the row-wise LDS.128 of a quarter
 // warp hits eight different bank groups) and reads its rows from there; with fewer visible rows (the culled
 // partitions of a city view) the direct loads touch less memory and are kept.
+#ifndef SPLX_SH_STAGE
+#define SPLX_SH_STAGE 1
+#endif
 constexpr int SH_STAGE_MIN = 12;
 template <int DEG, int PARTS>
 __global__ void __launch_bounds__(PROJ_THREADS)
@@ -189,7 +192,7 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
               splx_config cfg, splx_projected out) {
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;
-  constexpr bool STAGE = (PARTS & 2) && DEG > 0;
+  constexpr bool STAGE = SPLX_SH_STAGE && (PARTS & 2) && DEG > 0;
   __shared__ __align__(16) float4 s_sh[STAGE ? PROJ_THREADS * NV : 1];
   const int r = find_run(rt, (int)blockIdx.x);
   const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
@@ -346,7 +349,7 @@ __device__ __forceinline__ void adam_scalar(float* pp, float* pm, float* pv, flo
 // (splx_bin_sort_visible) instead of 128 consecutive Gaussians, so the work follows the visible count -- on the
 // city scenes ~10 % of the participating Gaussians -- and not the partition sizes; the grid is persistent because
 // the count lives on the device.
-template <int DEG, bool ACC, bool ADAM, bool LIST>
+template <int DEG, bool ACC, bool ADAM, int LIST>   // LIST: 0 = every row of the runs, 1 = the visible list, 2 = the list + `touched` flags
 __global__ void __launch_bounds__(PB_THREADS, SPLX_PB_MIN_CTAS)
 k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out,
@@ -359,7 +362,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   __shared__ __align__(16) float s_s[PB_THREADS * 3];    // log_scale gradient tile
   __shared__ uint8_t s_vis[PB_THREADS];
   __shared__ int64_t s_idx[PB_THREADS];                  // Gaussian of each row of the block
-  __shared__ uint8_t s_fresh[PB_THREADS];                // LIST + touched: first gradient of this row in the iteration ("=")
+  __shared__ uint8_t s_fresh[LIST == 2 ? PB_THREADS : 1];                // LIST + touched: first gradient of this row in the iteration ("=")
   const uint64_t nvis = LIST ? *nvis_ptr : 0;
   for (uint64_t blk = blockIdx.x; LIST ? (blk * PB_THREADS < nvis) : (blk == blockIdx.x); blk += gridDim.x) {
   int64_t base = 0, run_end = 0, i = 0;
@@ -412,11 +415,11 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   // sparse-optimiser mode: a row whose flag is still clear has no gradient yet in this iteration: its old content is
   // garbage, this launch stores instead of accumulating and sets the flag (a list holds a Gaussian once: no race)
   bool fresh = false;
-  if (LIST && touched != nullptr && vis) {
+  if (LIST == 2 && vis) {
     fresh = touched[i] == 0;
     touched[i] = 1;
   }
-  s_fresh[threadIdx.x] = fresh ? 1 : 0;
+  if (LIST == 2) s_fresh[threadIdx.x] = fresh ? 1 : 0;
   __syncthreads();
 #pragma unroll
   for (int c = 0; c < NV; ++c) {
@@ -425,7 +428,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     if (row < nrows && s_vis[row]) {
       cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * s_idx[row] + 4 * c4);
       if (ACC) {
-        if (LIST && s_fresh[row]) *reinterpret_cast<float4*>(s_old + row * PB_STRIDE + 4 * c4) = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (LIST == 2 && s_fresh[row]) *reinterpret_cast<float4*>(s_old + row * PB_STRIDE + 4 * c4) = make_float4(0.f, 0.f, 0.f, 0.f);
         else cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
       }
     }
@@ -635,7 +638,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
           const float4 a = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
           const float4 o = *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
           *dst = make_float4(o.x + a.x, o.y + a.y, o.z + a.z, o.w + a.w);
-        } else if (LIST && s_fresh[row]) {
+        } else if (LIST == 2 && s_fresh[row]) {
           *dst = make_float4(0.f, 0.f, 0.f, 0.f);       // coefficients above sh_degree of a freshly stored row
         }
       } else {
@@ -687,9 +690,9 @@ static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pla
                       const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
                       const AdamFuse& af) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  k_project_bwd<DEG, ACC, ADAM, false><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, 0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  k_project_bwd<DEG, ACC, ADAM, 0><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(
       *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, nullptr, nullptr, nullptr);
 }
 
@@ -699,12 +702,19 @@ static void launch_pb_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev
                            const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
                            const AdamFuse& af, const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * 2;
-  cudaFuncSetAttribute(k_project_bwd<DEG, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(k_project_bwd<DEG, true, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   const int64_t need = (rt.jprefix[rt.n] + PB_THREADS - 1) / PB_THREADS;
   const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 4 ? need : (int64_t)SPLX_SM_COUNT * 4;
-  k_project_bwd<DEG, true, false, true><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
-      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis, touched);
+  if (touched) {
+    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    k_project_bwd<DEG, true, false, 2><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
+        *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis, touched);
+  } else {
+    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    k_project_bwd<DEG, true, false, 1><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
+        *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis, touched);
+  }
 }
 
 template <bool ACC, bool ADAM>

@@ -399,7 +399,7 @@ int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binnin
   const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
   const uint32_t nslots = (uint32_t)plan.ntiles * (uint32_t)plan.K;
   // longest list first only where empty slots need no visit (without SPLX_PLAN_SPARSE they get the identity partial)
-  const uint32_t* order = sparse ? bins->slot_order : nullptr;
+  const uint32_t* order = sparse && slot_order_pays(plan) ? bins->slot_order : nullptr;
   const dim3 grid = order ? dim3(nslots, 1) : dim3(plan.ntiles, plan.K);
   if (pairs)
     k_render_fwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
@@ -416,7 +416,7 @@ int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binnin
 int launch_raster_bwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, const PlanDev& plan,
                       const splx_partial* part, const float* g_ct, float* g2d) {
   const uint32_t nslots = (uint32_t)plan.ntiles * (uint32_t)plan.K;
-  const uint32_t* order = bins->slot_order;
+  const uint32_t* order = slot_order_pays(plan) ? bins->slot_order : nullptr;
   // slots of non-participating partitions have empty ranges: they exit at once / are not in the order
   const dim3 grid = order ? dim3(nslots, 1) : dim3(plan.ntiles, plan.K);
   k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,

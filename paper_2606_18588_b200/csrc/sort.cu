@@ -488,6 +488,7 @@ __device__ __forceinline__ bool cross_removed(const CrossEmit& cx, uint64_t F, u
   return false;
 }
 
+template <bool FILTER>     // FILTER: cross-boundary per-ray filtering on (cx.mask != nullptr)
 __global__ void __launch_bounds__(256)
 k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
@@ -527,7 +528,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       if (parts.off[mid] <= (int64_t)i) lo = mid; else hi = mid - 1;
     }
     slot0 = (uint32_t)lo * (uint32_t)(TX * TY);
-    if (cx.mask) F = cross_filter(cx, i, lo, __uint_as_float(dbits));
+    if (FILTER) F = cross_filter(cx, i, lo, __uint_as_float(dbits));
   }
   // The 32 runs of a warp are adjacent in the output (offs is the running sum of tiles_touched in this very
   // order), so the warp writes its whole range [o_0, o_0 + T) cooperatively: lane l produces output slot
@@ -555,12 +556,12 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
     const uint32_t ss = __shfl_sync(0xffffffffu, slot0, own);
     const uint64_t pos = (uint64_t)o0 + sidx;
     uint64_t sF = 0;
-    if (cx.mask) sF = __shfl_sync(0xffffffffu, F, own);
+    if (FILTER) sF = __shfl_sync(0xffffffffu, F, own);
     if (sidx < T && pos < capacity) {
       const uint32_t ty = t / (uint32_t)sw;
       const uint32_t tile = (uint32_t)((sy0 + (int)ty) * TX + sx0 + (int)(t - ty * (uint32_t)sw));
       uint32_t slot = ss + tile;
-      if (sF && cross_removed(cx, sF, tile)) slot = cx.nslots;
+      if (FILTER && sF && cross_removed(cx, sF, tile)) slot = cx.nslots;
       keys[pos] = ((uint64_t)slot << 32) | sd;
       vals[pos] = si;
       for (int p = 0; p < plan.npass; ++p)
@@ -572,6 +573,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
   for (int x = threadIdx.x; x < plan.npass * 256; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
 }
 
+template <bool FILTER>
 __global__ void __launch_bounds__(256)
 k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
@@ -599,7 +601,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
   constexpr int EK_TILE = 1024, EK_IPT = EK_TILE / 256;
   __shared__ uint32_t s_off[EK_TILE + 1], s_xy[EK_TILE + 1], s_w[EK_TILE + 1], s_slot0[EK_TILE + 1], s_db[EK_TILE + 1],
       s_gi[EK_TILE + 1];
-  __shared__ uint64_t s_F[EK_TILE + 1];
+  __shared__ uint64_t s_F[FILTER ? EK_TILE + 1 : 1];
   __shared__ uint32_t s_nown;
   const uint64_t nvis = cnt->n_visible;
   const uint64_t m = cnt->m_sorted;                       // min(M, capacity): positions beyond the capacity are dropped
@@ -635,7 +637,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         }
         s_off[q] = o; s_xy[q] = ((uint32_t)y0 << 16) | (uint32_t)x0; s_w[q] = (uint32_t)(x1 - x0);
         s_slot0[q] = (uint32_t)plo * (uint32_t)(TX * TY); s_db[q] = ckeys[j]; s_gi[q] = i;
-        if (cx.mask) s_F[q] = cross_filter(cx, i, plo, __uint_as_float(s_db[q]));
+        if (FILTER) s_F[q] = cross_filter(cx, i, plo, __uint_as_float(s_db[q]));
         atomicMax(&s_nown, (uint32_t)q + 1);
       }
     }
@@ -654,7 +656,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         const uint32_t ty = t / w;
         const uint32_t tile = ((xy >> 16) + ty) * (uint32_t)TX + (xy & 0xffffu) + (t - ty * w);
         uint32_t slot = s_slot0[ql] + tile;
-        if (cx.mask) { const uint64_t F = s_F[ql]; if (F && cross_removed(cx, F, tile)) slot = cx.nslots; }
+        if (FILTER) { const uint64_t F = s_F[ql]; if (F && cross_removed(cx, F, tile)) slot = cx.nslots; }
         keys[pos] = ((uint64_t)slot << 32) | s_db[ql];
         vals[pos] = s_gi[ql];
         for (int p = 0; p < plan.npass; ++p)
@@ -863,17 +865,28 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
     for (int k = 0; k < K; ++k) { cx.zlo[k] = cross->zlo[k]; cx.zhi[k] = cross->zhi[k]; cx.view[k] = plan.pv.v[k]; }
   }
   const uint64_t emit_blocks = ((uint64_t)n_act + 255) / 256, range_blocks = (out->capacity + 255) / 256;
-  k_emit_keys<<<(unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
-      pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0,
-      plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
-      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256, cx);
-  SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
+  const unsigned g_emit = (unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS);
   const uint64_t emit_tiles = (out->capacity + 1023) / 1024;     // output tiles of 1024 keys
-  k_emit_keys_lb<<<(unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
-      pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY, out->capacity, k0, v0,
-      plan_passes(32, 32 + sbits), (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot),
-      (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256, cx);
-  SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
+  const unsigned g_lb = (unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS);
+  const PassPlan spl = plan_passes(32, 32 + sbits);
+  uint32_t* gh = (uint32_t*)(base + L.ghist_s);
+  uint64_t* sst = (uint64_t*)(base + L.st_slot);
+  const size_t sstride = (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256;
+  if (cx.mask) {
+    k_emit_keys<true><<<g_emit, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
+                                                       out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+    SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
+    k_emit_keys_lb<true><<<g_lb, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
+                                                        out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+    SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
+  } else {
+    k_emit_keys<false><<<g_emit, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
+                                                        out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+    SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
+    k_emit_keys_lb<false><<<g_lb, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
+                                                         out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+    SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
+  }
   // 4. stable sort on the slot bits
   if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
                                  (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6], true))) return rc;
@@ -881,7 +894,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
       out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections, cx.nslots, cx.mask != nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
-  if (out->slot_order) {
+  if (out->slot_order && slot_order_pays(plan)) {
     const uint32_t nslots = (uint32_t)K * (uint32_t)ntiles;
     uint32_t* n_live = out->slot_order + nslots;
     uint32_t* cursor = n_live + 1;
