@@ -253,13 +253,18 @@ __device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int la
     const int p = r * 32 + lane;
     const int pc = p < rows ? p : 0;
     const unsigned base = (unsigned)__cvta_generic_to_shared(st.v[pc]) + 16u * (unsigned)(lane & 7);
-    float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+    // the four running sums as two packed pairs: FADD2 (sm_100a add.rn.f32x2) adds two independent IEEE floats per
+    // instruction -- same results, half the issue slots (the kernel is issue bound)
+    unsigned long long s01 = 0ull, s23 = 0ull;
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-      float4 f;
-      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(f.x), "=f"(f.y), "=f"(f.z), "=f"(f.w) : "r"(base ^ (16u * q)));
-      s0 += f.x; s1 += f.y; s2 += f.z; s3 += f.w;
+      unsigned long long f01, f23;
+      asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(f01), "=l"(f23) : "r"(base ^ (16u * q)));
+      asm("add.rn.f32x2 %0, %0, %1;" : "+l"(s01) : "l"(f01));
+      asm("add.rn.f32x2 %0, %0, %1;" : "+l"(s23) : "l"(f23));
     }
+    const float s0 = __uint_as_float((unsigned)s01), s1 = __uint_as_float((unsigned)(s01 >> 32));
+    const float s2 = __uint_as_float((unsigned)s23), s3 = __uint_as_float((unsigned)(s23 >> 32));
     const int item = pc / 9, val = pc - 9 * item;
     const uint32_t idx = __shfl_sync(FULL, gid, item);
     if (p < rows) atomicAdd(g2d + (size_t)SPLX_G2D_STRIDE * idx + val, (s0 + s1) + (s2 + s3));
