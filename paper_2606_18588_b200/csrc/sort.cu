@@ -18,9 +18,9 @@
 namespace {
 
 #ifndef SPLX_SCAN_IPT
-#define SPLX_SCAN_IPT 16
+#define SPLX_SCAN_IPT 8   /* 8 against 16, same session: city_10M 12.50 / 12.62 ms, street_10M 16.46 / 16.56, city_100M 66.8 / 67.2, others equal */
 #endif
-constexpr int SCAN_THREADS = 512, SCAN_IPT = SPLX_SCAN_IPT, SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // 8192 elements per tile
+constexpr int SCAN_THREADS = 512, SCAN_IPT = SPLX_SCAN_IPT, SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // 4096 elements per tile
 constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
 static_assert(SCAN_TILE % RS_TILE == 0, "the compaction scan clears the radix status words of the tiles it covers");
@@ -82,7 +82,7 @@ __device__ __forceinline__ uint64_t lookback(uint64_t* status, uint32_t t, uint3
 }
 
 // ---------------------------------------------------------------- generic exclusive scan --
-// One launch: tiles of 8192 values, chained by look-back.  Op supplies count(), load(i) and
+// One launch: tiles of SCAN_TILE values, chained by look-back.  Op supplies count(), load(i) and
 // store(i, value, exclusive_prefix).  The grand total goes to *total_out (and, clamped, to *clamp_out).
 
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* smem /*>=33*/, uint32_t& total) {
@@ -146,7 +146,7 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     }
     const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
     uint32_t v[SCAN_IPT], s = 0;
-    const typename Op::Cursor cur = op.cursor(base < n ? base : 0);      // the thread's 16 elements are consecutive
+    const typename Op::Cursor cur = op.cursor(base < n ? base : 0);      // the thread's SCAN_IPT elements are consecutive
 #pragma unroll
     for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(cur, base, k) : 0; s += v[k]; }
     uint32_t total;
