@@ -35,6 +35,8 @@ def build(force: bool = False) -> str:
         cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-ffp-contract=off",
                "-o", _LIB, _SRC]
         subprocess.check_call(cmd)
+    from . import dssim as _dssim      # the D-SSIM term has its own plain-C file
+    _dssim.build(force)
     return _LIB
 
 
