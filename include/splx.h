@@ -99,9 +99,11 @@ typedef struct {
 /* Tile binning of all K partitions.  slot = k * (TX*TY) + tile; key = (slot << 32) |
  * float_bits(depth); val = Gaussian index (global, into the SoA).  keys/vals[capacity];
  * tile_ranges[K*TX*TY][2] = [first, last+1) into keys/vals, (0,0) for an empty tile;
- * num_intersections: one device uint64 = M, the number of valid entries (clamped to
+ * num_intersections: DEVICE uint64[2]: [0] = M, the number of intersections (clamped to
  * nothing: if M > capacity the overflowing entries are dropped and splx_check_capacity
- * reports it). */
+ * reports it; with M >= 2^32 nothing is emitted at all); [1] = the number of NON-EMPTY lists that were dropped
+ * because their slot carried SPLX_TILE_INVISIBLE (0 whenever the caller's regions are conservative, see
+ * splx_footprint_margin). */
 typedef struct {
   uint64_t *keys;
   uint32_t *vals;
@@ -177,6 +179,19 @@ int splx_compose(splx_ctx *ctx, int K, const splx_partial *partials, const splx_
  * sign(image-target) * scale / count; loss_sum (device double, may be NULL) += sum|.|. */
 int splx_l1_loss_grad(splx_ctx *ctx, const float *image, const float *target, int64_t count,
                       float scale, float *dL_dimage, double *loss_sum);
+
+/* ---- the full loss of PAPER.md L95 (section 2, step 4): "L = L_RGB + lambda L_D-SSIM".  The paper gives neither lambda
+ * nor the SSIM window; reading s33 of DESIGN.md: L_RGB = mean |image - target|; L_D-SSIM = 1 - mean SSIM, SSIM per colour
+ * channel over an 11 x 11 Gaussian window (sigma 1.5, weights summing to 1), C1 = 0.01^2, C2 = 0.03^2, pixels outside
+ * the image adding nothing to the window sums (zero padding).  image, target, dL_dimage: DEVICE [n_views,H,W,3]
+ * (n_views <= SPLX_MAX_VIEWS; cam gives W and H only).  dL_dimage = scale / (n_views H W 3) * (sign(image - target)
+ * - lambda d(sum SSIM)/dimage): pass scale = n_views to give every view its own mean, as splx_l1_loss_grad.
+ * loss_sum (DEVICE double[2], may be NULL): [0] += sum |image - target|, [1] += sum SSIM, so that
+ * L = loss_sum[0] / count + lambda (1 - loss_sum[1] / count) with count = H W 3 per view.  ws: DEVICE scratch of
+ * n_views * splx_dssim_ws_floats(cam) floats.  lambda = 0 gives the gradient of splx_l1_loss_grad. */
+size_t splx_dssim_ws_floats(const splx_camera *cam);
+int splx_dssim_loss_grad(splx_ctx *ctx, int n_views, const splx_camera *cam, const float *image, const float *target,
+                         float lambda, float scale, float *dL_dimage, double *loss_sum, float *ws);
 
 /* ---- a8 composition backward: Eq.6-7.  g_ct[K,H,W,4] =
  * (dL/dC^k rgb, dL/dT^k).  dL_dT_total[H,W] may be NULL.  Overwrites g_ct. */
@@ -256,15 +271,29 @@ typedef struct {
   int32_t flags;
 } splx_plan;
 
-/* Geometric visibility (L212, L227): HOST computation, no device work, ctx not needed.  For each of
- * the K axis-aligned boxes [aabb_lo[k], aabb_hi[k]] (HOST float[K][3], world space) the convex
- * polyhedron box ^ frustum (the four side planes through the image border and z >= near_z; no far
- * plane) is projected; tile_state[k*tiles + t] (HOST out) = 0 if tile t's pixel-area
- * rectangle meets that convex region, else SPLX_TILE_INVISIBLE.  participants (HOST out, may be
- * NULL): bit k set iff partition k has at least one visible tile (GetParticipants, L249).
- * Double precision.  Returns SPLX_OK or SPLX_ERR_INVALID_ARG (K > 64, null pointers, lo > hi). */
-int splx_visible_regions(int K, const float *aabb_lo, const float *aabb_hi, const splx_camera *cam,
-                         uint8_t *tile_state, uint64_t *participants);
+/* Geometric visibility (L212, L227): HOST computation, no device work, ctx not needed.  n_boxes axis-aligned boxes
+ * [aabb_lo[j], aabb_hi[j]] (HOST float[n_boxes][3], world space), box j belonging to partition box_part[j] (HOST
+ * int32[n_boxes]; NULL = one box per partition, n_boxes == K): a partition is the UNION of its boxes (the cell of L155,
+ * or a finer cover of it by sub-cells).
+ *  - max_scale NULL, the plain region of L212: the convex polyhedron box ^ {z >= near_z} (no far plane) is
+ *    projected; tile_state[k*tiles + t] (HOST out) = 0 if tile t's pixel-area rectangle meets the projected region of
+ *    some box j of partition k, else SPLX_TILE_INVISIBLE.
+ *  - max_scale given (HOST float[n_boxes]: the largest scale exp(log_scale) among the Gaussians whose MEAN lies in box j;
+ *    the boxes are then boxes of means; cfg NULL = defaults), the CONSERVATIVE region of reading s21: Gaussians
+ *    belong to a partition by their mean (L155) but their footprints stick out of its box (L474).  With
+ *    c^2 = max(fx, fy)^2 (1 + limx^2 + limy^2), e = dilation + sqrt(radius_floor): the box is first cut down to the means
+ *    that can reach the image at all, Q = box ^ {z >= near_z} ^ {-(cx + g) z - h <= fx x <= (W - cx + g) z + h} ^ {same in
+ *    y}, g = 2.5 + 3 sqrt(e), h = 3 c max_scale; on Q every footprint square has half side <= 3 sqrt(c^2 max_scale^2 /
+ *    z_min(Q)^2 + e) + 1, so tile t is marked visible iff its rectangle grown by m = 3 sqrt(c^2 max_scale^2 / z_min^2 + e)
+ *    + 3.5 px meets the projection of Q.  Then a slot marked SPLX_TILE_INVISIBLE has an EMPTY list and a non-participant
+ *    no visible Gaussian: skipping them changes no pixel and no gradient.  The finer the boxes the tighter the regions
+ *    (scenes.partition_boxes covers every partition with a grid of sub-cells).
+ * participants (HOST out, may be NULL): bit k set iff partition k has at least one visible tile (GetParticipants,
+ * L249).  Double precision.  Returns SPLX_OK or SPLX_ERR_INVALID_ARG (K > 64, null pointers, lo > hi, near_z <= 0, a
+ * negative scale, box_part out of range). */
+int splx_visible_regions(int K, int n_boxes, const int32_t *box_part, const float *aabb_lo, const float *aabb_hi,
+                         const float *max_scale, const splx_config *cfg, const splx_camera *cam, uint8_t *tile_state,
+                         uint64_t *participants);
 
 /* Conflict-free view consolidation (L249): greedy bucketing in view order.  View v goes to the first
  * bucket none of whose views shares a partition with participants[v] and that holds fewer than
@@ -278,16 +307,6 @@ int splx_schedule_views(int n_views, const uint64_t *participants, int max_views
  * Arrays indexed by partition keep their [K,...] layout (a partition belongs to one view). */
 int splx_project_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                       const splx_plan *plan, int sh_degree, const splx_projected *out);
-/* splx_project_plan in two halves, so that a caller can overlap them with other work (the colour half needs nothing
- * but tiles_touched of the geometry half and is not needed before splx_render_partial: it can run beside the
- * binning, and -- across iterations -- the optimiser step of the SH coefficients can run beside the geometry half
- * and the binning of the next iteration).  SPLX_PROJECT_GEOMETRY writes means2d, depth, conic_opacity, radius,
- * tiles_touched and records 0-1 of `blend`; SPLX_PROJECT_COLOUR (after it) writes rgb, clamp and record 2.  Both
- * bits = splx_project_plan; the results are bit-identical either way. */
-#define SPLX_PROJECT_GEOMETRY 1
-#define SPLX_PROJECT_COLOUR 2
-int splx_project_parts_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
-                            const splx_plan *plan, int sh_degree, const splx_projected *out, int parts);
 int splx_bin_sort_plan(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
                        const int64_t *part_offsets, const splx_plan *plan, const splx_binning *out,
                        void *ws, size_t ws_bytes);
@@ -371,30 +390,95 @@ int splx_project_backward_list_plan(splx_ctx *ctx, const splx_gaussians *g, int 
 int splx_adam_sparse(splx_ctx *ctx, const splx_gaussian_grads *params, const splx_gaussian_grads *grads,
                      const splx_gaussian_grads *m, const splx_gaussian_grads *v, uint8_t *touched,
                      const float lr[5], float beta1, float beta2, float eps, int step, float grad_scale);
-/* a10 + a11 fused: the LAST projection backward of an iteration also takes the Adam step of splx_adam on every
- * row of every partition (participating or not), reading the gradient it has just formed -- plus, without
- * SPLX_PB_OVERWRITE, the gradient earlier launches of the iteration left in `grads` -- instead of storing it:
- * `grads` is only read (never written), Adam never re-reads it.  params / m / v: the parameter set (updated in
- * place: the const of splx_gaussians does not apply here), first and second moments, same SoA layout as
- * splx_gaussian_grads.  lr: HOST float[5] for mean, log_scale, quat, opacity_logit, sh.  bias_corr: DEVICE
- * float[2] = 1/(1-beta1^t), 1/(1-beta2^t) (on the device so that a captured CUDA graph can be replayed with
- * the next step's values).  Elementwise the arithmetic of splx_project_backward_plan followed by splx_adam
- * with grad_scale. */
-int splx_project_backward_adam_plan(splx_ctx *ctx, const splx_gaussian_grads *params, int K,
-                                    const int64_t *part_offsets, const splx_plan *plan, int sh_degree,
-                                    const splx_projected *proj, float *g2d, int flags,
-                                    const splx_gaussian_grads *grads, const splx_gaussian_grads *m,
-                                    const splx_gaussian_grads *v, const float lr[5], float beta1, float beta2,
-                                    float eps, const float *bias_corr, float grad_scale);
-/* Advance the DEVICE-resident Adam step counter (*step_dev += 1, a device int32 the caller zero-initialises) and
- * write bias_corr (device float[2]) = 1/(1-beta1^t), 1/(1-beta2^t) for the new t: the producer of
- * splx_project_backward_adam_plan's bias_corr that can live inside a captured CUDA graph. */
-int splx_adam_bias_step(splx_ctx *ctx, float beta1, float beta2, int32_t *step_dev, float *bias_corr);
 int splx_backward_plan(splx_ctx *ctx, int K, const int64_t *part_offsets, const splx_plan *plan,
                        const splx_partial *partials, const float bg[3], const float *dL_dimage,
                        const float *dL_dT_total, const splx_gaussians *g, const splx_projected *proj,
                        const splx_binning *bins, int sh_degree, const splx_gaussian_grads *grads,
                        void *ws, size_t ws_bytes, int flags);
+
+
+/* ==== One whole training iteration behind one call (the sequencing of PAPER.md Fig. 9, on one GPU) =========
+ * The stages above are the parity surface; a trainer calls THIS: a1-a10 for every bucket of views of an iteration
+ * (and optionally a11), issued by the library on the context's stream plus three internal streams -- projection and
+ * binning of bucket g+1 run beside the blending of bucket g when a second splx_frontset is given, host copies run on
+ * their own streams beside the kernels.  Nothing here synchronises; every internal stream is joined back into the
+ * context's stream before the call returns, so the call may be captured into a CUDA graph by the caller. */
+
+/* Buffers of a1-a4 for one bucket in flight. */
+typedef struct {
+  splx_projected proj;
+  splx_binning bins;
+  void *ws;        /* DEVICE, splx_bin_sort_ws_bytes(n, bins.capacity, K, cam) */
+  size_t ws_bytes;
+} splx_frontset;
+
+/* Every caller-owned buffer of an iteration.  DEVICE pointers unless marked HOST. */
+typedef struct {
+  splx_gaussian_grads params;   /* Theta, SoA over all K partitions; only splx_adam_cfg writes it */
+  splx_gaussian_grads grads;    /* same layout: the FIRST bucket of an iteration stores, later ones accumulate */
+  int32_t K;
+  const int64_t *part_offsets;  /* HOST [K+1] */
+  int32_t sh_degree;
+  float bg[3];
+  splx_frontset front[2];       /* front[1].ws == NULL: buckets run strictly one after the other */
+  splx_partial partials;        /* [K,H,W,*] */
+  float *g_ct;                  /* [K,H,W,4] */
+  float *g2d;                   /* [n,SPLX_G2D_STRIDE], all zero on entry; left all zero */
+  float *images;                /* [max_views,H,W,3]: image of view v of the iteration at slot v */
+  float *T_totals;              /* [max_views,H,W] or NULL */
+  float *targets;               /* [max_views,H,W,3]: staging of HOST targets (SPLX_ITER_HOST), else unused / NULL */
+  float *g_images;              /* [max_views,H,W,3]: dL/dimage, only used when lambda_dssim > 0, else may be NULL */
+  float *dssim_ws;              /* splx_dssim_ws_floats(W,H) floats per view x max_views, only when lambda_dssim > 0 */
+  double *loss_sum;             /* double[2]: [0] += sum |image-target| (cleared by the call), [1] += sum SSIM */
+  int32_t max_views;
+  const uint64_t *cross_mask;   /* Q_cross masks [n] (splx_cross_sets) or NULL: cross-boundary filtering off */
+  uint8_t *touched;             /* [n] flags of the visible-only optimiser option or NULL */
+} splx_trainset;
+
+/* One bucket = one launch per stage (a conflict-free set of views, L249). */
+typedef struct {
+  splx_plan plan;               /* plan.cams / view_of_part HOST, plan.tile_state DEVICE */
+  const int32_t *view_index;    /* HOST [plan.n_views]: plan view b is view view_index[b] of the iteration */
+  uint8_t *tile_state_out;      /* DEVICE [K*tiles] or NULL: saturation detection (may alias plan.tile_state) */
+  const float *part_depth_range;/* HOST [2K] (splx_cross_depth_ranges) when trainset.cross_mask is set, else NULL */
+} splx_bucket;
+
+/* Optional a11 at the end of the iteration: dense Adam over the flat buffers (splx_adam_groups), or, with
+ * trainset.touched, the visible-only option (splx_adam_sparse on the SoA sets; m / v as SoA). */
+typedef struct {
+  float *param, *grad, *m, *v;          /* flat buffers holding the five groups back to back */
+  int32_t n_groups;
+  const int64_t *group_offsets;         /* HOST [n_groups+1] */
+  const float *lr;                      /* HOST [n_groups] */
+  float beta1, beta2, eps;
+  int32_t step;                         /* 1-based */
+  splx_gaussian_grads m_soa, v_soa;     /* only read with trainset.touched */
+} splx_adam_cfg;
+
+#define SPLX_ITER_HOST 1   /* targets[v] / images_out[v] / loss_out / m_out are pinned HOST pointers */
+typedef struct {
+  int32_t flags;
+  float sat_eps;         /* threshold of the saturation detection (bucket.tile_state_out) */
+  float lambda_dssim;    /* 0: L = mean L1 (a6+a7+a8 fused); > 0: L = mean L1 + lambda * (1 - mean SSIM) */
+} splx_iter_opts;
+
+/* n_views views in n_buckets buckets; every view belongs to exactly one bucket.  targets[v]: [H,W,3] of view v
+ * (DEVICE, or pinned HOST with SPLX_ITER_HOST: copied to trainset.targets on the library's upload stream while the
+ * first bucket is projected and binned).  The loss of view v is its own mean; the gradients of the views add up
+ * (grad_scale 1/n_views is applied by a11).  With SPLX_ITER_HOST: images_out[v] (HOST [H,W,3] or NULL entries; the
+ * array itself may be NULL) receives image v as soon as its bucket is composed, loss_out (HOST double[2] or NULL)
+ * receives loss_sum; without the flag both must be NULL.  m_out (pinned HOST uint64[n_buckets] or NULL, with or
+ * without the flag) receives the intersection count of every bucket: compare it with bins.capacity after a
+ * synchronisation -- a bucket with more intersections dropped its farthest keys.  adam NULL = no optimiser step. */
+int splx_iteration(splx_ctx *ctx, const splx_trainset *ts, int n_buckets, const splx_bucket *buckets, int n_views,
+                   const float *const *targets, float *const *images_out, double *loss_out, uint64_t *m_out,
+                   const splx_iter_opts *opts, const splx_adam_cfg *adam);
+
+/* ---- measurement helper (not part of the method): the micro-benchmarks behind the ALU rooflines of the blend loops
+ * (an FMA loop and an ex2 loop measured on the box).  kind 0: FP32 FMA chains, *work (HOST out) = flops
+ * of the launch (2 per FMA); kind 1: ex2.approx chains, *work = ex2 evaluations.  One asynchronous launch over all SMs;
+ * the caller times it with CUDA events on the context's stream.  sink: DEVICE float[1] (never written in practice). */
+int splx_microbench(splx_ctx *ctx, int kind, int64_t iters, float *sink, double *work);
 
 #ifdef __cplusplus
 }

@@ -129,6 +129,17 @@ def project(mean, log_scale, quat, opacity_logit, sh, sh_degree, cam, cfg=DEFAUL
     return out
 
 
+def depth_key(mean, cam):
+    """The camera depth as the sort key sees it (reading s12): evaluated in fp32 in a fixed operation order, so that the
+    oracle and the kernel order near-equal depths alike.  Returned as float64 values that are exact fp32 numbers."""
+    n = int(np.asarray(mean).shape[0])
+    mean = _c(mean, np.float64).reshape(n, 3)
+    cam = _c(cam, np.float64)
+    out = np.zeros(n)
+    lib().orc_depth_key(ctypes.c_int64(n), _p(mean), _p(cam), _p(out))
+    return out
+
+
 def count_tiles(means2d, radius, W, H):
     n = int(np.asarray(radius).shape[0])
     means2d = _c(means2d, np.float64).reshape(n, 2)
@@ -299,7 +310,7 @@ def forward(parts, cam, sh_degree, bg=(0.0, 0.0, 0.0), cfg=DEFAULT_CFG, tile_lis
     for p in parts:
         pr = project(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sh_degree,
                      cam, cfg)
-        b = bin_sort(pr.means2d, pr.radius, pr.depth, W, H)
+        b = bin_sort(pr.means2d, pr.radius, depth_key(p["mean"], cam), W, H)     # order by the fp32 key (s12)
         pa = render_partial(pr.means2d, pr.conic_opacity, pr.rgb, pr.depth, b.vals, b.ranges, W, H,
                             cfg, tile_list)
         res.proj.append(pr); res.bins.append(b); res.partials.append(pa)

@@ -258,6 +258,23 @@ void orc_project(int64_t n, const double* mean, const double* log_scale, const d
 }
 
 // ---------------------------------------------------------------------------
+// The depth as the SORT KEY sees it.  Reading s12: key = (tile << 32) | float_bits(depth), an integer decision taken in
+// fp32 -- by both sides in the same precision and the same operation order, so that two Gaussians whose depths differ
+// by less than an fp32 rounding are ordered alike by the oracle and by the kernel:
+//   z32 = fl(fma(R22, mz, fma(R21, my, fl(R20 * mx))) + t2)        (all operands rounded to fp32 first)
+// Only the ORDER uses it; the depth that enters the partial depth D (Eq.4) stays the fp64 value of orc_project.
+// ---------------------------------------------------------------------------
+void orc_depth_key(int64_t n, const double* mean, const double* cam_, double* depth32) {
+  const Cam cam = load_cam(cam_);
+  const float r0 = (float)cam.R[6], r1 = (float)cam.R[7], r2 = (float)cam.R[8], t2 = (float)cam.t[2];
+  for (int64_t i = 0; i < n; ++i) {
+    const float mx = (float)mean[3 * i], my = (float)mean[3 * i + 1], mz = (float)mean[3 * i + 2];
+    const float z = std::fmaf(r2, mz, std::fmaf(r1, my, r0 * mx)) + t2;
+    depth32[i] = (double)z;
+  }
+}
+
+// ---------------------------------------------------------------------------
 // O2 tile binning + depth sort.  PAPER.md L81 ("sorted based on their distance
 // from the camera, i.e., depth d"), L165 ("sorted locally by depth").  The
 // mechanism (tile|depth 64-bit keys, stable order, per-tile ranges) is reading

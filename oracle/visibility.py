@@ -21,7 +21,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (DEFAULT_CFG, TILE, IterationResult, bin_sort, cam_wh, compose, compose_bwd, l1, project,
+from . import (DEFAULT_CFG, TILE, IterationResult, bin_sort, cam_wh, compose, compose_bwd, depth_key, l1, project,
                project_bwd, raster_bwd, render_partial, tiles_xy)
 
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -32,10 +32,40 @@ def _tile_rect(t, TX, W, H):
     return 16.0 * tx, min(16.0 * (tx + 1), float(W)), 16.0 * ty, min(16.0 * (ty + 1), float(H))
 
 
-def visible_regions(aabb_lo, aabb_hi, cam, tiles=None, tol=1e-7):
-    """state[K, tiles] (0 = visible, TILE_INVISIBLE, 255 = tile not evaluated), participants bitmask,
-    margin[K, tiles] = the largest slack s for which  A p + s <= b  is still feasible inside the box
-    (rows scaled to unit norm; > 0 robustly visible, < 0 robustly invisible, |s| <= tol undecided)."""
+def _reach(cam, s_max, cfg):
+    """Reading s21.  Gaussians belong to a partition by their mean (L155) but their footprints stick out of
+    its box (L474); the binning keeps every Gaussian whose square of tiles meets the image.  For scale <= s_max and
+    camera-space mean (x, y, z), z > near:  radius = ceil(3 sqrt(lambda)), lambda = mid + sqrt(max(floor, mid^2 - det))
+    <= lambda_max(Sigma2D) + sqrt(floor);  Sigma2D = J W Sigma W^T J^T + dilation I  =>  lambda_max <= |J|_2^2 s^2 +
+    dilation;  with J = [[fx/z, 0, -fx Lx/z], [0, fy/z, -fy Ly/z]], |Lx| <= limx, |Ly| <= limy (the clamps of s9),
+    |J|_2^2 <= c^2/z^2, c^2 = max(fx, fy)^2 (1 + limx^2 + limy^2).  So radius <= 3 c s/z + 3 sqrt(e) + 1,
+    e = dilation + sqrt(floor), and the square (pixel columns within radius + 1.5 of u = fx x/z + cx) can meet [0, W]
+    only if  -(cx + g) z - h <= fx x <= (W - cx + g) z + h  with g = 2.5 + 3 sqrt(e), h = 3 c s -- linear in the mean;
+    likewise in y.  Returns (rows, rhs) of those four half spaces as A p_world <= b, and (c^2, e)."""
+    R, t = cam[0:9].reshape(3, 3), cam[9:12]
+    fx, fy, cx, cy = cam[12:16]
+    W, H = cam_wh(cam)
+    dilation, lim_factor, rfloor = cfg[3], cfg[4], cfg[5]
+    limx, limy = lim_factor * W / (2 * fx), lim_factor * H / (2 * fy)
+    c2 = max(fx, fy) ** 2 * (1 + limx * limx + limy * limy)
+    e = dilation + np.sqrt(rfloor)
+    g, h = 2.5 + 3 * np.sqrt(e), 3 * np.sqrt(c2) * s_max
+    rows, rhs = [], []
+    # fx xc - (W - cx + g) zc <= h   with xc = R0.p + t0, zc = R2.p + t2
+    for sign, f, axis, span in ((1.0, fx, 0, W - cx), (-1.0, fx, 0, cx), (1.0, fy, 1, H - cy), (-1.0, fy, 1, cy)):
+        a = sign * f * R[axis] - (span + g) * R[2]
+        rows.append(a); rhs.append(h - (sign * f * t[axis] - (span + g) * t[2]))
+    return rows, rhs, c2, e
+
+
+def visible_regions(aabb_lo, aabb_hi, cam, tiles=None, tol=1e-7, max_scale=None, cfg=DEFAULT_CFG, whole_image=False):
+    """state[n_boxes, tiles] (0 = visible, TILE_INVISIBLE, 255 = tile not evaluated), participants bitmask (one bit per
+    box), margin[n_boxes, tiles] = the largest slack s for which  A p + s <= b  is still feasible inside the box
+    (rows scaled to unit norm; > 0 robustly visible, < 0 robustly invisible, |s| <= tol undecided).
+    max_scale None: the plain region of L212 (box ^ {z >= near} projected).  max_scale[n_boxes] (boxes of MEANS, the
+    largest scale of their Gaussians): the conservative region of reading s21 -- the box is first cut down to the
+    means that can reach the image (`_reach`), z_min of what is left gives the margin m = 3 sqrt(c^2 s^2/z_min^2 + e)
+    + 3.5 px by which every tile rectangle is grown.  whole_image: one 'tile' = the image rectangle (participants only)."""
     from scipy.optimize import linprog
     cam = np.asarray(cam, np.float64)
     R, t = cam[0:9].reshape(3, 3), cam[9:12]
@@ -46,13 +76,29 @@ def visible_regions(aabb_lo, aabb_hi, cam, tiles=None, tol=1e-7):
     lo = np.asarray(aabb_lo, np.float64).reshape(-1, 3)
     hi = np.asarray(aabb_hi, np.float64).reshape(-1, 3)
     K = lo.shape[0]
-    tiles = range(TX * TY) if tiles is None else [int(x) for x in tiles]
-    state = np.full((K, TX * TY), 255, np.uint8)
-    margin = np.full((K, TX * TY), np.nan)
+    if whole_image:
+        tiles = [0]
+    else:
+        tiles = range(TX * TY) if tiles is None else [int(x) for x in tiles]
+    state = np.full((K, 1 if whole_image else TX * TY), 255, np.uint8)
+    margin = np.full(state.shape, np.nan)
     part = 0
     for k in range(K):
+        bounds = [(lo[k, 0], hi[k, 0]), (lo[k, 1], hi[k, 1]), (lo[k, 2], hi[k, 2])]
+        xrows, xrhs, mg = [], [], 0.0
+        if max_scale is not None:
+            xrows, xrhs, c2, e = _reach(cam, float(max_scale[k]), cfg)
+            # z_min over the means that can reach the image (and lie in front of the near plane)
+            res = linprog(c=R[2], A_ub=np.array([-R[2]] + xrows), b_ub=np.array([t[2] - near] + xrhs), bounds=bounds, method="highs")
+            if res.status != 0:                     # no mean of this box can reach the image
+                state[k, list(tiles)] = TILE_INVISIBLE
+                margin[k, list(tiles)] = -1.0
+                continue
+            zmin = max(near, float(R[2] @ res.x + t[2]))
+            mg = 3.0 * np.sqrt(c2 * float(max_scale[k]) ** 2 / zmin ** 2 + e) + 3.5
         for tl in tiles:
-            x0, x1, y0, y1 = _tile_rect(tl, TX, W, H)
+            x0, x1, y0, y1 = (0.0, float(W), 0.0, float(H)) if whole_image else _tile_rect(tl, TX, W, H)
+            x0, x1, y0, y1 = x0 - mg, x1 + mg, y0 - mg, y1 + mg
             # camera-space coordinates are affine in the world point p: xc = R0.p + t0 etc.
             rows, rhs = [], []
             rows.append(-R[2]); rhs.append(t[2] - near)                                   # zc >= near
@@ -60,13 +106,12 @@ def visible_regions(aabb_lo, aabb_hi, cam, tiles=None, tol=1e-7):
             rows.append(fx * R[0] + (cx - x1) * R[2]); rhs.append(-(fx * t[0] + (cx - x1) * t[2]))   # u <= x1
             rows.append(-(fy * R[1] + (cy - y0) * R[2])); rhs.append(fy * t[1] + (cy - y0) * t[2])   # v >= y0
             rows.append(fy * R[1] + (cy - y1) * R[2]); rhs.append(-(fy * t[1] + (cy - y1) * t[2]))   # v <= y1
-            A = np.array(rows); b = np.array(rhs)
+            A = np.array(rows + xrows); b = np.array(rhs + xrhs)
             nrm = np.linalg.norm(A, axis=1)
             A = A / nrm[:, None]; b = b / nrm
             # maximise s subject to A p + s <= b, lo <= p <= hi
-            res = linprog(c=[0, 0, 0, -1.0], A_ub=np.hstack([A, np.ones((5, 1))]), b_ub=b,
-                          bounds=[(lo[k, 0], hi[k, 0]), (lo[k, 1], hi[k, 1]), (lo[k, 2], hi[k, 2]), (None, 1e6)],
-                          method="highs")
+            res = linprog(c=[0, 0, 0, -1.0], A_ub=np.hstack([A, np.ones((len(b), 1))]), b_ub=b,
+                          bounds=bounds + [(None, 1e6)], method="highs")
             assert res.status == 0, res.message
             s = float(res.x[3])
             margin[k, tl] = s
@@ -74,6 +119,21 @@ def visible_regions(aabb_lo, aabb_hi, cam, tiles=None, tol=1e-7):
             if s >= 0:
                 part |= 1 << k
     return state, part, margin
+
+
+def participants(aabb_lo, aabb_hi, cam, max_scale=None, cfg=DEFAULT_CFG):
+    """GetParticipants(v) (L249) without the tile grid: `visible_regions` posed for the whole image at once (one bit
+    per box)."""
+    return visible_regions(aabb_lo, aabb_hi, cam, max_scale=max_scale, cfg=cfg, whole_image=True)[1]
+
+
+def union_regions(state_boxes, box_part, K):
+    """A partition covered by several boxes is visible on a tile iff one of its boxes is (state per box -> per partition)."""
+    state_boxes = np.asarray(state_boxes)
+    out = np.full((K, state_boxes.shape[1]), TILE_INVISIBLE, np.uint8)
+    for j, k in enumerate(box_part):
+        out[k][state_boxes[j] == 0] = 0
+    return out
 
 
 def ray_hits_box(aabb_lo, aabb_hi, cam, u, v):
@@ -172,7 +232,7 @@ def iteration_plan(parts, cams, view_of_part, sh_degree, targets, bg=(0.0, 0.0, 
         for k in members:
             p = parts[k]
             pr = project(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], sh_degree, cam, cfg)
-            bn = bin_sort(pr.means2d, pr.radius, pr.depth, W, H)
+            bn = bin_sort(pr.means2d, pr.radius, depth_key(p["mean"], cam), W, H)     # order by the fp32 key (s12)
             if tile_state is not None:
                 bn.ranges = apply_tile_state(bn.ranges, tile_state[k])
             pa = render_partial(pr.means2d, pr.conic_opacity, pr.rgb, pr.depth, bn.vals, bn.ranges, W, H, cfg)

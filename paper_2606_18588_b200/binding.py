@@ -32,15 +32,15 @@ EXPORTS = [
     "splx_visible_regions", "splx_schedule_views", "splx_project_plan", "splx_bin_sort_plan",
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
-    "splx_compose_l1_backward_plan", "splx_project_backward_adam_plan", "splx_adam_bias_step",
+    "splx_compose_l1_backward_plan",
     "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
-    "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan", "splx_project_parts_plan",
+    "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
+    "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_iteration", "splx_microbench",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
 PLAN_SPARSE = 1
 ORDER_EXTRA = 1025
-PROJECT_GEOMETRY, PROJECT_COLOUR = 1, 2
 
 
 class SplxError(RuntimeError):
@@ -83,6 +83,37 @@ class PartialS(C.Structure):
 class PlanS(C.Structure):
     _fields_ = [("n_views", C.c_int32), ("cams", C.c_void_p), ("view_of_part", C.c_void_p),
                 ("tile_state", C.c_void_p), ("flags", C.c_int32)]
+
+
+class FrontsetS(C.Structure):
+    _fields_ = [("proj", ProjectedS), ("bins", BinningS), ("ws", C.c_void_p), ("ws_bytes", C.c_size_t)]
+
+
+class TrainsetS(C.Structure):
+    _fields_ = [("params", GaussiansS), ("grads", GaussiansS), ("K", C.c_int32), ("part_offsets", C.c_void_p),
+                ("sh_degree", C.c_int32), ("bg", C.c_float * 3), ("front", FrontsetS * 2), ("partials", PartialS),
+                ("g_ct", C.c_void_p), ("g2d", C.c_void_p), ("images", C.c_void_p), ("T_totals", C.c_void_p),
+                ("targets", C.c_void_p), ("g_images", C.c_void_p), ("dssim_ws", C.c_void_p), ("loss_sum", C.c_void_p),
+                ("max_views", C.c_int32), ("cross_mask", C.c_void_p), ("touched", C.c_void_p)]
+
+
+class BucketS(C.Structure):
+    _fields_ = [("plan", PlanS), ("view_index", C.c_void_p), ("tile_state_out", C.c_void_p),
+                ("part_depth_range", C.c_void_p)]
+
+
+class AdamCfgS(C.Structure):
+    _fields_ = [("param", C.c_void_p), ("grad", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p),
+                ("n_groups", C.c_int32), ("group_offsets", C.c_void_p), ("lr", C.c_void_p),
+                ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32),
+                ("m_soa", GaussiansS), ("v_soa", GaussiansS)]
+
+
+class IterOptsS(C.Structure):
+    _fields_ = [("flags", C.c_int32), ("sat_eps", C.c_float), ("lambda_dssim", C.c_float)]
+
+
+ITER_HOST = 1
 
 
 def lib():
@@ -129,7 +160,12 @@ def lib():
                                        C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int,
                                        C.c_float, C.c_int]
         vp = C.c_void_p
-        L.splx_visible_regions.argtypes = [C.c_int, vp, vp, vp, vp, vp]
+        L.splx_visible_regions.argtypes = [C.c_int, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.splx_dssim_ws_floats.restype = C.c_size_t
+        L.splx_dssim_ws_floats.argtypes = [vp]
+        L.splx_dssim_loss_grad.argtypes = [vp, C.c_int, vp, vp, vp, C.c_float, C.c_float, vp, vp, vp]
+        L.splx_microbench.argtypes = [vp, C.c_int, C.c_int64, vp, vp]
+        L.splx_iteration.argtypes = [vp, vp, C.c_int, vp, C.c_int, vp, vp, vp, vp, vp, vp]
         L.splx_schedule_views.argtypes = [C.c_int, vp, C.c_int, vp, vp]
         L.splx_project_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp]
         L.splx_bin_sort_plan.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp, vp, vp, C.c_size_t]
@@ -142,13 +178,9 @@ def lib():
         L.splx_project_backward_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp]
         L.splx_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp, vp,
                                          C.c_size_t, C.c_int]
-        L.splx_project_backward_adam_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp,
-                                                      C.c_float, C.c_float, C.c_float, vp, C.c_float]
-        L.splx_adam_bias_step.argtypes = [vp, C.c_float, C.c_float, vp, vp]
         L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
         L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp]
         L.splx_adam_sparse.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float]
-        L.splx_project_parts_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, C.c_int]
         L.splx_cross_sets.argtypes = [vp, vp, C.c_int, vp, vp, vp, C.c_float, vp]
         L.splx_cross_depth_ranges.argtypes = [C.c_int, vp, vp, vp, vp]
         L.splx_bin_sort_filtered_plan.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp, vp, vp, vp, vp, C.c_size_t]
@@ -201,17 +233,27 @@ class Plan:
         return C.byref(self._s)
 
 
-def visible_regions(aabb_lo, aabb_hi, cam):
-    """splx_visible_regions (host computation): returns (tile_state uint8 numpy [K, tiles], participants bitmask)."""
+def visible_regions(aabb_lo, aabb_hi, cam, max_scale=None, box_part=None, K=None, cfg=None):
+    """splx_visible_regions (host computation): returns (tile_state uint8 numpy [K, tiles], participants bitmask).
+    max_scale: float[n_boxes] largest scale of the Gaussians with their mean in box j -> the conservative regions of
+    reading s21 (None: the plain projected boxes); box_part: int[n_boxes] partition of every box (None: one box per
+    partition); K: number of partitions; cfg: the splx_config tuple (None = defaults)."""
     import numpy as np
     lo = np.ascontiguousarray(aabb_lo, np.float32).reshape(-1, 3)
     hi = np.ascontiguousarray(aabb_hi, np.float32).reshape(-1, 3)
-    K = lo.shape[0]
+    nb = lo.shape[0]
+    bp = np.ascontiguousarray(box_part, np.int32).reshape(nb) if box_part is not None else None
+    if K is None:
+        K = nb if bp is None else int(bp.max()) + 1
     TX, TY = (int(cam.width) + TILE - 1) // TILE, (int(cam.height) + TILE - 1) // TILE
     out = np.empty((K, TX * TY), np.uint8)
     part = C.c_uint64(0)
     cs = camera_struct(cam)
-    rc = lib().splx_visible_regions(K, lo.ctypes.data, hi.ctypes.data, C.byref(cs), out.ctypes.data, C.byref(part))
+    ms = np.ascontiguousarray(max_scale, np.float32).reshape(nb) if max_scale is not None else None
+    c = Config(*cfg) if cfg is not None else None
+    rc = lib().splx_visible_regions(K, nb, bp.ctypes.data if bp is not None else None, lo.ctypes.data, hi.ctypes.data,
+                                    ms.ctypes.data if ms is not None else None, C.byref(c) if c is not None else None,
+                                    C.byref(cs), out.ctypes.data, C.byref(part))
     if rc != OK:
         raise SplxError(rc, "splx_visible_regions: invalid argument")
     return out, int(part.value)
@@ -277,8 +319,7 @@ class Binning:
         self.tile_ranges = torch.zeros((K * self.TX * self.TY, 2), dtype=torch.int32, device=device)
         self.num_intersections = torch.zeros(2, dtype=torch.int64, device=device)
         #: slots by descending list length (splx_binning.slot_order); set to None to hand out CTAs in tile order
-        self.slot_order = (torch.zeros(K * self.TX * self.TY + ORDER_EXTRA, dtype=torch.int32, device=device)
-                           if os.environ.get("SPLX_SLOT_ORDER", "1") == "1" else None)
+        self.slot_order = torch.zeros(K * self.TX * self.TY + ORDER_EXTRA, dtype=torch.int32, device=device)
 
     def struct(self):
         return BinningS(_ptr(self.keys), _ptr(self.vals), _ptr(self.tile_ranges), self.capacity,
@@ -435,12 +476,6 @@ class Context:
         self._check(lib().splx_project_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
                                             sh_degree, C.byref(ps)))
 
-    def project_parts_plan(self, params: dict, part_offsets, plan: Plan, sh_degree: int, out: Projected, parts: int):
-        """splx_project_parts_plan: parts = PROJECT_GEOMETRY (1), PROJECT_COLOUR (2) or both."""
-        g, ps = gaussians_struct(params), out.struct()
-        self._check(lib().splx_project_parts_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
-                                                  sh_degree, C.byref(ps), int(parts)))
-
     def bin_sort_plan(self, proj: Projected, part_offsets, plan: Plan, out: Binning, ws: torch.Tensor):
         ps, bs = proj.struct(), out.struct()
         self._check(lib().splx_bin_sort_plan(self._h, C.byref(ps), proj.n, plan.K, self._offs(part_offsets), plan.ref(),
@@ -509,19 +544,6 @@ class Context:
         self._check(lib().splx_project_backward_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
                                                      sh_degree, C.byref(ps), _ptr(g2d), flags, C.byref(gg)))
 
-    def project_backward_adam_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
-                                   grads: dict, m: dict, v: dict, lrs, bias_corr, beta1=0.9, beta2=0.999, eps=1e-15,
-                                   grad_scale=1.0, clear_g2d=False, overwrite=False):
-        """lrs: five learning rates in PARAM order (mean, log_scale, quat, opacity_logit, sh); bias_corr: device float[2]."""
-        sets = [gaussians_struct(x) for x in (params, grads, m, v)]
-        ps = proj.struct()
-        lr = (C.c_float * 5)(*[float(x) for x in lrs])
-        flags = (PB_CLEAR_G2D if clear_g2d else 0) | (PB_OVERWRITE if overwrite else 0)
-        self._check(lib().splx_project_backward_adam_plan(
-            self._h, C.byref(sets[0]), plan.K, self._offs(part_offsets), plan.ref(), sh_degree, C.byref(ps), _ptr(g2d),
-            flags, C.byref(sets[1]), C.byref(sets[2]), C.byref(sets[3]), lr, beta1, beta2, eps, _ptr(bias_corr),
-            float(grad_scale)))
-
     @staticmethod
     def bin_sort_visible(ws: torch.Tensor, n, capacity, K, cam):
         """Device pointers (ints) of the visible list and of its count inside the bin_sort workspace."""
@@ -547,8 +569,37 @@ class Context:
         self._check(lib().splx_adam_sparse(self._h, C.byref(sets[0]), C.byref(sets[1]), C.byref(sets[2]), C.byref(sets[3]),
                                            _ptr(touched), lr, beta1, beta2, eps, int(step), float(grad_scale)))
 
-    def adam_bias_step(self, step_dev, bias_corr, beta1=0.9, beta2=0.999):
-        self._check(lib().splx_adam_bias_step(self._h, beta1, beta2, _ptr(step_dev), _ptr(bias_corr)))
+    @staticmethod
+    def dssim_ws_floats(width, height) -> int:
+        cs = CameraS()
+        cs.width, cs.height = int(width), int(height)
+        return int(lib().splx_dssim_ws_floats(C.byref(cs)))
+
+    def dssim_loss_grad(self, cam, image, target, g_image, loss_sum, ws, lam, scale=None):
+        """splx_dssim_loss_grad: image / target / g_image [B,H,W,3] (or [H,W,3]); loss_sum device double[2] or None."""
+        B = image.shape[0] if image.dim() == 4 else 1
+        cs = camera_struct(cam)
+        self._check(lib().splx_dssim_loss_grad(self._h, B, C.byref(cs), _ptr(image), _ptr(target), float(lam),
+                                               float(B if scale is None else scale), _ptr(g_image), _ptr(loss_sum), _ptr(ws)))
+
+    def iteration(self, trainset: "TrainsetS", buckets, n_views, targets, images_out=None, loss_out=None, m_out=None,
+                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None):
+        """splx_iteration.  buckets: ctypes array of BucketS; targets / images_out: lists of raw pointers (ints; device
+        pointers, or pinned host pointers with host=True); loss_out / m_out: raw pinned host pointers or None."""
+        tg = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) for x in targets])
+        io = None
+        if images_out is not None:
+            io = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) if x else None for x in images_out])
+        opts = IterOptsS(ITER_HOST if host else 0, float(sat_eps), float(lambda_dssim))
+        self._check(lib().splx_iteration(self._h, C.byref(trainset), len(buckets), buckets, int(n_views), tg, io,
+                                         C.c_void_p(loss_out) if loss_out else None, C.c_void_p(m_out) if m_out else None,
+                                         C.byref(opts), C.byref(adam) if adam is not None else None))
+
+    def microbench(self, kind: int, iters: int, sink) -> float:
+        """splx_microbench: launches the FMA (kind 0) or ex2 (kind 1) loop; returns the work of the launch (flops / ex2)."""
+        w = C.c_double(0.0)
+        self._check(lib().splx_microbench(self._h, int(kind), int(iters), _ptr(sink), C.byref(w)))
+        return float(w.value)
 
     def backward_plan(self, part_offsets, plan: Plan, partials: Partial, bg, g_image, g_T_total, params: dict,
                       proj: Projected, bins: Binning, sh_degree, grads: dict, ws: torch.Tensor, overwrite=False):

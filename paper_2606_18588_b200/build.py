@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libsplx.so")
-SOURCES = ["api.cu", "project.cu", "sort.cu", "render.cu", "compose.cu", "adam.cu", "visibility.cu", "cross.cu"]
+SOURCES = ["api.cu", "project.cu", "sort.cu", "render.cu", "compose.cu", "adam.cu", "visibility.cu", "cross.cu", "dssim.cu", "iteration.cu", "peaks.cu"]
 HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(HERE, "..", "include", "splx.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]

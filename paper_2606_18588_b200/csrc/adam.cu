@@ -127,16 +127,6 @@ k_adam_sparse(const __grid_constant__ SparseSets S, uint8_t* __restrict__ touche
   }
 }
 
-// Device-resident step counter of the fused optimiser path: t = ++(*step); bc = 1/(1-b1^t), 1/(1-b2^t) formed in
-// double as launch_adam does on the host.  One thread; lives inside captured CUDA graphs, where a host-side step
-// number would be frozen at capture time.
-__global__ void k_adam_bias_step(int32_t* step, float* bc, double b1, double b2) {
-  const int t = *step + 1;
-  *step = t;
-  bc[0] = (float)(1.0 / (1.0 - pow(b1, (double)t)));
-  bc[1] = (float)(1.0 / (1.0 - pow(b2, (double)t)));
-}
-
 }  // namespace
 
 int launch_adam_sparse(splx_ctx* ctx, const splx_gaussian_grads* P, const splx_gaussian_grads* Gr,
@@ -157,12 +147,6 @@ int launch_adam_sparse(splx_ctx* ctx, const splx_gaussian_grads* P, const splx_g
   for (int j = 0; j < 5; ++j) S.lr[j] = lr[j];
   k_adam_sparse<<<(unsigned)((n + SB - 1) / SB), SB, 0, ctx->stream>>>(S, touched, n, k, grad_scale);
   SPLX_LAUNCH_CHECK(ctx, "k_adam_sparse");
-  return SPLX_OK;
-}
-
-int launch_adam_bias_step(splx_ctx* ctx, float beta1, float beta2, int32_t* step_dev, float* bias_corr) {
-  k_adam_bias_step<<<1, 1, 0, ctx->stream>>>(step_dev, bias_corr, (double)beta1, (double)beta2);
-  SPLX_LAUNCH_CHECK(ctx, "k_adam_bias_step");
   return SPLX_OK;
 }
 

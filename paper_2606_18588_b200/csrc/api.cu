@@ -4,8 +4,14 @@
 
 static char g_create_err[512] = "";
 
+// near_z must be positive: with z <= 0 admitted 1/z blows up in J and float_bits(depth) no longer sorts as an unsigned key
 static bool cam_ok(const splx_camera* c) {
-  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f;
+  if (!c || c->width <= 0 || c->height <= 0) return false;
+  const float f[5] = {c->fx, c->fy, c->cx, c->cy, c->near_z};
+  for (float x : f) if (!(x == x) || x - x != 0.f) return false;      // NaN or infinity
+  for (int i = 0; i < 9; ++i) if (!(c->R[i] - c->R[i] == 0.f)) return false;
+  for (int i = 0; i < 3; ++i) if (!(c->t[i] - c->t[i] == 0.f)) return false;
+  return c->fx > 0.f && c->fy > 0.f && c->near_z > 0.f;
 }
 static bool proj_ok(const splx_projected* p) {
   return p && p->means2d && p->depth && p->conic_opacity && p->rgb && p->radius && p->tiles_touched &&
@@ -24,7 +30,7 @@ static bool bins_ok(const splx_binning* b) {
 
 // ---- launch plans ---------------------------------------------------------------------------
 // Validates a splx_plan against K and builds the device-side copy.  All views must share one image size.
-static int make_plan(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, PlanDev* out) {
+int make_plan_dev(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, PlanDev* out) {
   if (!plan || !plan->cams || !plan->view_of_part) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: plan, cams or view_of_part is NULL", who);
   if (K < 1 || K > SPLX_MAX_K) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: K=%d not in [1,%d]", who, K, SPLX_MAX_K);
   if (plan->n_views < 1 || plan->n_views > SPLX_MAX_VIEWS)
@@ -92,6 +98,7 @@ int splx_create(splx_ctx** out, int device, void* cuda_stream, const splx_config
   c->stream = (cudaStream_t)cuda_stream;
   c->launches = 0;
   c->err[0] = 0;
+  c->iter_ready = false;
   if (cfg) c->cfg = *cfg;
   else c->cfg = splx_config{1.0f / 255.0f, 0.99f, 1e-4f, 0.3f, 1.3f, 0.1f};
   if (!(c->cfg.alpha_max > 0.f) || c->cfg.alpha_min < 0.f || c->cfg.T_eps < 0.f) {
@@ -105,6 +112,7 @@ int splx_create(splx_ctx** out, int device, void* cuda_stream, const splx_config
 
 int splx_destroy(splx_ctx* ctx) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;
+  iteration_release(ctx);
   delete ctx;
   return SPLX_OK;
 }
@@ -127,24 +135,9 @@ int splx_project_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64
   if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: sh_degree %d not in [0,3]", sh_degree);
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_project", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_project", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project: part_offsets must run monotonically from 0 to n");
   return launch_project_fwd(ctx, g, pd, part_offsets, sh_degree, out);
-}
-
-int splx_project_parts_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const splx_plan* plan,
-                            int sh_degree, const splx_projected* out, int parts) {
-  if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (parts != SPLX_PROJECT_GEOMETRY && parts != SPLX_PROJECT_COLOUR && parts != (SPLX_PROJECT_GEOMETRY | SPLX_PROJECT_COLOUR))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: parts=%d", parts);
-  if (g && g->n == 0) return SPLX_OK;
-  if (!gauss_ok(g) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: null/misaligned argument");
-  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: sh_degree %d not in [0,3]", sh_degree);
-  PlanDev pd;
-  int rc;
-  if ((rc = make_plan(ctx, "splx_project_parts", K, plan, &pd))) return rc;
-  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_parts: part_offsets must run monotonically from 0 to n");
-  return launch_project_fwd(ctx, g, pd, part_offsets, sh_degree, out, parts);
 }
 
 int splx_project(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
@@ -170,7 +163,7 @@ int splx_bin_sort_plan(splx_ctx* ctx, const splx_projected* proj, int64_t n, int
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_bin_sort", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_bin_sort", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: part_offsets must run monotonically from 0 to n");
   if (n >= ((int64_t)1 << 32) || out->capacity >= ((uint64_t)1 << 32))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: n and capacity must be < 2^32");
@@ -188,7 +181,7 @@ int splx_bin_sort_filtered_plan(splx_ctx* ctx, const splx_projected* proj, int64
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_bin_sort_filtered", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_bin_sort_filtered", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: part_offsets must run monotonically from 0 to n");
   if (n >= ((int64_t)1 << 32) || out->capacity >= ((uint64_t)1 << 32))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_filtered: n and capacity must be < 2^32");
@@ -243,7 +236,7 @@ int splx_render_partial_plan(splx_ctx* ctx, const splx_projected* proj, const sp
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_render_partial: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_render_partial", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_render_partial", K, plan, &pd))) return rc;
   return launch_render_fwd(ctx, proj, bins, pd, out, pairs);
 }
 
@@ -261,11 +254,12 @@ int splx_compose_plan(splx_ctx* ctx, int K, const splx_partial* partials, const 
   if (!partial_ok(partials) || !bg || !image) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_compose", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_compose", K, plan, &pd))) return rc;
   if ((pd.flags & SPLX_PLAN_SPARSE) && !bins_ok(bins))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: SPLX_PLAN_SPARSE needs the binning");
   if (tile_state_out && !(sat_eps >= 0.f)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose: sat_eps must be >= 0");
-  return launch_compose_fwd(ctx, partials, bins, pd, bg, image, T_total, sat_eps, tile_state_out);
+  const ViewBufs vb = contiguous_views(pd.B, (size_t)pd.W * pd.H, nullptr, image, T_total, nullptr, nullptr);
+  return launch_compose_fwd(ctx, partials, bins, pd, bg, vb, sat_eps, tile_state_out);
 }
 
 int splx_compose_l1_backward_plan(splx_ctx* ctx, int K, const splx_partial* partials, const splx_binning* bins,
@@ -277,12 +271,12 @@ int splx_compose_l1_backward_plan(splx_ctx* ctx, int K, const splx_partial* part
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_l1_backward: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_compose_l1_backward", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_compose_l1_backward", K, plan, &pd))) return rc;
   if ((pd.flags & SPLX_PLAN_SPARSE) && !bins_ok(bins))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_l1_backward: SPLX_PLAN_SPARSE needs the binning");
   if (tile_state_out && !(sat_eps >= 0.f)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_l1_backward: sat_eps must be >= 0");
-  return launch_compose_fused(ctx, partials, bins, pd, bg, targets, scale, image, T_total, loss_sum, g_ct, sat_eps,
-                              tile_state_out);
+  const ViewBufs vb = contiguous_views(pd.B, (size_t)pd.W * pd.H, targets, image, T_total, nullptr, nullptr);
+  return launch_compose_fused(ctx, partials, bins, pd, bg, vb, scale, loss_sum, g_ct, sat_eps, tile_state_out);
 }
 
 int splx_compose(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam, const float bg[3],
@@ -309,10 +303,11 @@ int splx_compose_backward_plan(splx_ctx* ctx, int K, const splx_partial* partial
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_compose_backward", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_compose_backward", K, plan, &pd))) return rc;
   if ((pd.flags & SPLX_PLAN_SPARSE) && !bins_ok(bins))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_compose_backward: SPLX_PLAN_SPARSE needs the binning");
-  return launch_compose_bwd(ctx, partials, bins, pd, bg, dL_dimage, dL_dT_total, g_ct);
+  const ViewBufs vb = contiguous_views(pd.B, (size_t)pd.W * pd.H, nullptr, nullptr, nullptr, const_cast<float*>(dL_dimage), dL_dT_total);
+  return launch_compose_bwd(ctx, partials, bins, pd, bg, vb, g_ct);
 }
 
 int splx_compose_backward(splx_ctx* ctx, int K, const splx_partial* partials, const splx_camera* cam,
@@ -330,7 +325,7 @@ int splx_raster_backward_plan(splx_ctx* ctx, const splx_projected* proj, const s
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_raster_backward: null/misaligned argument");
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_raster_backward", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_raster_backward", K, plan, &pd))) return rc;
   return launch_raster_bwd(ctx, proj, bins, pd, partials, g_ct, g2d);
 }
 
@@ -356,9 +351,9 @@ int splx_project_backward_plan(splx_ctx* ctx, const splx_gaussians* g, int K, co
   if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: unknown flags %d", flags);
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_project_backward", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_project_backward", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward: part_offsets must run monotonically from 0 to n");
-  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, nullptr, nullptr, nullptr);
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, nullptr, nullptr);
 }
 
 int splx_bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, const splx_camera* cam,
@@ -385,43 +380,9 @@ int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int 
   if (flags & ~SPLX_PB_CLEAR_G2D) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: unknown flags %d", flags);
   PlanDev pd;
   int rc;
-  if ((rc = make_plan(ctx, "splx_project_backward_list", K, plan, &pd))) return rc;
+  if ((rc = make_plan_dev(ctx, "splx_project_backward_list", K, plan, &pd))) return rc;
   if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: part_offsets must run monotonically from 0 to n");
-  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, nullptr, visible, num_visible, touched);
-}
-
-int splx_project_backward_adam_plan(splx_ctx* ctx, const splx_gaussian_grads* params, int K, const int64_t* part_offsets,
-                                    const splx_plan* plan, int sh_degree, const splx_projected* proj, float* g2d, int flags,
-                                    const splx_gaussian_grads* grads, const splx_gaussian_grads* m,
-                                    const splx_gaussian_grads* v, const float lr[5], float beta1, float beta2, float eps,
-                                    const float* bias_corr, float grad_scale) {
-  if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!params || !grads || !m || !v || !lr || !bias_corr || !proj_ok(proj) || !g2d || !aligned16(g2d))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: null/misaligned argument");
-  const splx_gaussian_grads* sets[4] = {params, grads, m, v};
-  for (const splx_gaussian_grads* s : sets) {
-    if (s->n != params->n || (s->n > 0 && (!s->mean || !s->log_scale || !s->quat || !s->opacity_logit || !s->sh ||
-                                           !aligned16(s->mean) || !aligned16(s->log_scale) || !aligned16(s->quat) ||
-                                           !aligned16(s->opacity_logit) || !aligned16(s->sh))))
-      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: params, grads, m, v must be four aligned sets of n rows");
-  }
-  if (params->n == 0) return SPLX_OK;
-  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: sh_degree %d not in [0,3]", sh_degree);
-  if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: unknown flags %d", flags);
-  PlanDev pd;
-  int rc;
-  if ((rc = make_plan(ctx, "splx_project_backward_adam", K, plan, &pd))) return rc;
-  if (!offsets_ok(part_offsets, K, params->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_adam: part_offsets must run monotonically from 0 to n");
-  AdamFuse af;
-  af.p[0] = params->mean; af.p[1] = params->log_scale; af.p[2] = params->quat; af.p[3] = params->opacity_logit; af.p[4] = params->sh;
-  af.m[0] = m->mean; af.m[1] = m->log_scale; af.m[2] = m->quat; af.m[3] = m->opacity_logit; af.m[4] = m->sh;
-  af.v[0] = v->mean; af.v[1] = v->log_scale; af.v[2] = v->quat; af.v[3] = v->opacity_logit; af.v[4] = v->sh;
-  for (int j = 0; j < 5; ++j) af.lr[j] = lr[j];
-  af.b1 = beta1; af.b2 = beta2;
-  af.omb1 = (float)(1.0 - (double)beta1); af.omb2 = (float)(1.0 - (double)beta2);   // as splx_adam forms them
-  af.eps = eps; af.gscale = grad_scale; af.bc = bias_corr;
-  const splx_gaussians g{params->mean, params->log_scale, params->quat, params->opacity_logit, params->sh, params->n};
-  return launch_project_bwd(ctx, &g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, &af, nullptr, nullptr, nullptr);
+  return launch_project_bwd(ctx, g, pd, part_offsets, sh_degree, proj, g2d, flags, grads, visible, num_visible, touched);
 }
 
 int splx_project_backward(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
@@ -494,13 +455,6 @@ int splx_adam_sparse(splx_ctx* ctx, const splx_gaussian_grads* params, const spl
                                            !aligned16(s->quat) || !aligned16(s->sh))))
       SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_sparse: params, grads, m, v must be four sets of n rows (quat, sh 16-byte aligned)");
   return launch_adam_sparse(ctx, params, grads, m, v, touched, lr, beta1, beta2, eps, step, grad_scale);
-}
-
-int splx_adam_bias_step(splx_ctx* ctx, float beta1, float beta2, int32_t* step_dev, float* bias_corr) {
-  if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!step_dev || !bias_corr || !(beta1 >= 0.f && beta1 < 1.f) || !(beta2 >= 0.f && beta2 < 1.f))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_bias_step: null pointer or beta not in [0,1)");
-  return launch_adam_bias_step(ctx, beta1, beta2, step_dev, bias_corr);
 }
 
 int splx_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int64_t count, float lr, float beta1,

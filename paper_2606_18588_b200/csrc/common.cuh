@@ -16,7 +16,12 @@ struct splx_ctx {
   splx_config cfg;
   int64_t launches;
   char err[512];
+  // splx_iteration's own streams and events, created at its first call (iteration.cu), destroyed by splx_destroy
+  bool iter_ready;
+  cudaStream_t s_front, s_up, s_down;     // a1-a4 of the next bucket; host -> device targets; device -> host results
+  cudaEvent_t ev_start, ev_up, ev_front[2], ev_back[2], ev_img, ev_down;
 };
+void iteration_release(splx_ctx*);
 
 // Device-side copy of the camera plus derived quantities, passed by value to kernels.
 struct CamDev {
@@ -56,6 +61,30 @@ struct PlanDev {
   PartView pv;
   CamDev cam[SPLX_MAX_VIEWS];
 };
+
+// Per-view buffers of the composition kernels (view b of the launch -> its own pointers), so that the views of a
+// launch need not be contiguous in one allocation (a bucket takes views 0 and 3 of an iteration, say).
+struct ViewBufs {
+  const float* target[SPLX_MAX_VIEWS];     // [H,W,3]
+  float* image[SPLX_MAX_VIEWS];            // [H,W,3]
+  float* T_total[SPLX_MAX_VIEWS];          // [H,W] or nullptr
+  float* g_image[SPLX_MAX_VIEWS];          // [H,W,3]: written by the loss kernels, read by the composition backward
+  const float* g_T_total[SPLX_MAX_VIEWS];  // [H,W] or nullptr
+};
+// views 0..B-1 of contiguous [B,H,W,*] arrays (any of them may be nullptr)
+static inline ViewBufs contiguous_views(int B, size_t HW, const float* target, float* image, float* T_total,
+                                        float* g_image, const float* g_T_total) {
+  ViewBufs vb;
+  memset(&vb, 0, sizeof vb);
+  for (int b = 0; b < B; ++b) {
+    vb.target[b] = target ? target + 3 * HW * b : nullptr;
+    vb.image[b] = image ? image + 3 * HW * b : nullptr;
+    vb.T_total[b] = T_total ? T_total + HW * b : nullptr;
+    vb.g_image[b] = g_image ? g_image + 3 * HW * b : nullptr;
+    vb.g_T_total[b] = g_T_total ? g_T_total + HW * b : nullptr;
+  }
+  return vb;
+}
 
 // Cross-boundary per-ray filtering (L474-L476): the per-Gaussian Q_cross masks and the depth interval D^k of every
 // partition under the view it renders.  mask == nullptr = no filtering.
@@ -137,20 +166,14 @@ __device__ __forceinline__ void tile_rect(float u, float v, int radius, int TX, 
   y1 = !(y1f > 0.0f) ? 0 : (y1f >= (float)TY ? TY : (int)y1f);
 }
 
-// Optional optimiser fusion of the projection backward (splx_project_backward_adam_plan).
-struct AdamFuse {
-  float *p[5], *m[5], *v[5];          // mean, log_scale, quat, opacity_logit, sh
-  float lr[5];
-  float b1, b2, omb1, omb2, eps, gscale;
-  const float* bc;                    // device float[2]: 1/(1-b1^t), 1/(1-b2^t)
-};
-
+// validates a splx_plan against K and builds the device-side copy (api.cu)
+int make_plan_dev(splx_ctx*, const char* who, int K, const splx_plan*, PlanDev* out);
 
 // ---- stage launchers (defined one per .cu file, called from api.cu) ----------------------
 int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
-                       const splx_projected*, int parts = 3);
+                       const splx_projected*);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
-                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*, const AdamFuse* adam,
+                       const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*,
                        const uint32_t* visible_list, const uint64_t* num_visible, uint8_t* touched);
 int launch_adam_sparse(splx_ctx*, const splx_gaussian_grads* params, const splx_gaussian_grads* grads,
                        const splx_gaussian_grads* m, const splx_gaussian_grads* v, uint8_t* touched, const float* lr,
@@ -168,17 +191,18 @@ int launch_render_fwd(splx_ctx*, const splx_projected*, const splx_binning*, con
 int launch_raster_bwd(splx_ctx*, const splx_projected*, const splx_binning*, const PlanDev&,
                       const splx_partial*, const float* g_ct, float* g2d);
 int launch_compose_fwd(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
-                       float* image, float* T_total, float sat_eps, uint8_t* tile_state_out);
+                       const ViewBufs&, float sat_eps, uint8_t* tile_state_out);
 int launch_compose_bwd(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
-                       const float* g_image, const float* g_T_total, float* g_ct);
+                       const ViewBufs&, float* g_ct);
 int launch_compose_fused(splx_ctx*, const splx_partial*, const splx_binning* bins, const PlanDev&, const float* bg,
-                         const float* target, float scale, float* image, float* T_total, double* loss_sum, float* g_ct,
-                         float sat_eps, uint8_t* tile_state_out);
+                         const ViewBufs&, float scale, double* loss_sum, float* g_ct, float sat_eps,
+                         uint8_t* tile_state_out);
+size_t dssim_ws_floats(int W, int H);
+int launch_dssim(splx_ctx*, int B, int W, int H, const ViewBufs&, float lambda, float scale, double* loss_sum, float* ws);
 int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count, float scale,
               float* g_image, double* loss_sum);
 int launch_adam_groups(splx_ctx*, float* param, float* grad, float* m, float* v, int n_groups,
                        const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
                        float grad_scale, int zero_grad);
-int launch_adam_bias_step(splx_ctx*, float beta1, float beta2, int32_t* step_dev, float* bias_corr);
 int launch_adam(splx_ctx*, float* param, float* grad, float* m, float* v, int64_t count, float lr,
                 float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad);

@@ -40,7 +40,7 @@ __device__ __forceinline__ int ordered_live(const float* __restrict__ ct, const 
   int L = 0;
   if (KMAX <= 8) {
     // Few partitions: fetch every T and D first (predicated, independent loads: one memory latency instead of a
-    // chain of 2 K dependent ones -- the kernel was bound by that chain, profiles/r01e), then order them.  (A
+    // chain of 2 K dependent ones -- the kernel was bound by that chain, profiles/r01e_ncu_full.md), then order them.  (A
     // register-only sorting network with fully unrolled loops was measured too: 74 registers, 0.084 ms against 0.047.)
     float Tk[KMAX], dk[KMAX];
 #pragma unroll
@@ -77,7 +77,7 @@ template <int KMAX, bool SAT>
 __global__ void __launch_bounds__(CB)
 k_compose_fwd(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
               const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
-              float bg1, float bg2, float* __restrict__ image, float* __restrict__ T_total, float sat_eps,
+              float bg1, float bg2, const __grid_constant__ ViewBufs vb, float sat_eps,
               const uint8_t* __restrict__ state_in, uint8_t* __restrict__ state_out) {
   __shared__ uint8_t s_use[SPLX_MAX_K];
   __shared__ unsigned s_unsat[2];
@@ -100,11 +100,11 @@ k_compose_fwd(const float* __restrict__ ct, const float* __restrict__ d, const u
       C0 = fmaf(Tacc, p.x, C0); C1 = fmaf(Tacc, p.y, C1); C2 = fmaf(Tacc, p.z, C2);
       Tacc *= p.w;
     }
-    float* im = image + 3 * ((size_t)b * HW + pix);
+    float* im = vb.image[b] + 3 * pix;
     im[0] = fmaf(Tacc, bg0, C0);
     im[1] = fmaf(Tacc, bg1, C1);
     im[2] = fmaf(Tacc, bg2, C2);
-    if (T_total) T_total[(size_t)b * HW + pix] = Tacc;
+    if (vb.T_total[b]) vb.T_total[b][pix] = Tacc;
     // a partition that is the identity at this pixel stands behind all live ones: its front product is T_total
     if (SAT && !(Tacc < sat_eps)) unsat |= ~live;
   }
@@ -127,8 +127,7 @@ template <int KMAX>
 __global__ void __launch_bounds__(CB)
 k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
               const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
-              float bg1, float bg2, const float* __restrict__ g_image, const float* __restrict__ g_T_total,
-              float* __restrict__ g_ct) {
+              float bg1, float bg2, const __grid_constant__ ViewBufs vb, float* __restrict__ g_ct) {
   __shared__ uint8_t s_use[SPLX_MAX_K];
   const int tile = blockIdx.x, b = blockIdx.y;
   tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
@@ -137,9 +136,9 @@ k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, const u
   const size_t HW = (size_t)W * H, pix = (size_t)y * W + x;
   float key[KMAX]; int idx[KMAX];
   const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
-  const float* gi = g_image + 3 * ((size_t)b * HW + pix);
+  const float* gi = vb.g_image[b] + 3 * pix;
   const float g0 = gi[0], g1 = gi[1], g2 = gi[2];
-  const float gT = g_T_total ? g_T_total[(size_t)b * HW + pix] : 0.f;
+  const float gT = vb.g_T_total[b] ? vb.g_T_total[b][pix] : 0.f;
   // T_total = product over the live partials in order (the empty ones multiply by 1)
   float Ttot = 1.f;
   for (int m = 0; m < L; ++m) Ttot *= __ldg(ct + 4 * ((size_t)idx[m] * HW + pix) + 3);
@@ -173,9 +172,9 @@ template <int KMAX, bool SAT>
 __global__ void __launch_bounds__(CB)
 k_compose_fused(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
                 const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
-                float bg1, float bg2, const float* __restrict__ target, float gscale, float* __restrict__ image,
-                float* __restrict__ T_total, double* loss_sum, float* __restrict__ g_ct, float sat_eps,
-                const uint8_t* __restrict__ state_in, uint8_t* __restrict__ state_out) {
+                float bg1, float bg2, const __grid_constant__ ViewBufs vb, float gscale, double* loss_sum,
+                float* __restrict__ g_ct, float sat_eps, const uint8_t* __restrict__ state_in,
+                uint8_t* __restrict__ state_out) {
   __shared__ uint8_t s_use[SPLX_MAX_K];
   __shared__ unsigned s_unsat[2];
   __shared__ float s_loss[CB / 32];
@@ -203,12 +202,12 @@ k_compose_fused(const float* __restrict__ ct, const float* __restrict__ d, const
     }
     const float Ttot = Tacc;
     const float i0 = fmaf(Ttot, bg0, C0), i1 = fmaf(Ttot, bg1, C1), i2 = fmaf(Ttot, bg2, C2);
-    float* im = image + 3 * ((size_t)b * HW + pix);
+    float* im = vb.image[b] + 3 * pix;
     im[0] = i0; im[1] = i1; im[2] = i2;
-    if (T_total) T_total[(size_t)b * HW + pix] = Ttot;
+    if (vb.T_total[b]) vb.T_total[b][pix] = Ttot;
     if (SAT && !(Ttot < sat_eps)) unsat |= ~live;
     // a7: mean L1 against the target of view b
-    const float* tg = target + 3 * ((size_t)b * HW + pix);
+    const float* tg = vb.target[b] + 3 * pix;
     const float e0 = i0 - tg[0], e1 = i1 - tg[1], e2 = i2 - tg[2];
     lacc = fabsf(e0) + fabsf(e1) + fabsf(e2);
     const float g0 = e0 > 0.f ? gscale : (e0 < 0.f ? -gscale : 0.f);
@@ -291,75 +290,76 @@ k_l1(const float* __restrict__ image, const float* __restrict__ target, int64_t 
 // The K partials are required to be one [K,H,W,*] allocation (splx_partial describes all K).
 template <int KMAX>
 static void compose_fwd_k(splx_ctx* ctx, const splx_partial* p, const uint32_t* ranges, const PlanDev& plan, int sparse,
-                          const float* bg, float* image, float* T_total, float sat_eps, uint8_t* state_out) {
+                          const float* bg, const ViewBufs& vb, float sat_eps, uint8_t* state_out) {
   dim3 grid(plan.ntiles, plan.B);
   if (state_out)
     k_compose_fwd<KMAX, true><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
-                                                           plan.ntiles, sparse, bg[0], bg[1], bg[2], image, T_total,
-                                                           sat_eps, plan.tile_state, state_out);
+                                                           plan.ntiles, sparse, bg[0], bg[1], bg[2], vb, sat_eps,
+                                                           plan.tile_state, state_out);
   else
     k_compose_fwd<KMAX, false><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
-                                                            plan.ntiles, sparse, bg[0], bg[1], bg[2], image, T_total,
-                                                            sat_eps, nullptr, nullptr);
+                                                            plan.ntiles, sparse, bg[0], bg[1], bg[2], vb, sat_eps, nullptr,
+                                                            nullptr);
 }
 
 int launch_compose_fwd(splx_ctx* ctx, const splx_partial* p, const splx_binning* bins, const PlanDev& plan,
-                       const float* bg, float* image, float* T_total, float sat_eps, uint8_t* state_out) {
+                       const float* bg, const ViewBufs& vb, float sat_eps, uint8_t* state_out) {
   const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
   const uint32_t* ranges = bins ? bins->tile_ranges : nullptr;
-  if (plan.K <= 8) compose_fwd_k<8>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
-  else if (plan.K <= 16) compose_fwd_k<16>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
-  else if (plan.K <= 32) compose_fwd_k<32>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
-  else compose_fwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, image, T_total, sat_eps, state_out);
+  if (plan.K <= 8) compose_fwd_k<8>(ctx, p, ranges, plan, sparse, bg, vb, sat_eps, state_out);
+  else if (plan.K <= 16) compose_fwd_k<16>(ctx, p, ranges, plan, sparse, bg, vb, sat_eps, state_out);
+  else if (plan.K <= 32) compose_fwd_k<32>(ctx, p, ranges, plan, sparse, bg, vb, sat_eps, state_out);
+  else compose_fwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, vb, sat_eps, state_out);
   SPLX_LAUNCH_CHECK(ctx, "k_compose_fwd");
   return SPLX_OK;
 }
 
 template <int KMAX>
 static void compose_bwd_k(splx_ctx* ctx, const splx_partial* p, const uint32_t* ranges, const PlanDev& plan, int sparse,
-                          const float* bg, const float* g_image, const float* g_T_total, float* g_ct) {
+                          const float* bg, const ViewBufs& vb, float* g_ct) {
   dim3 grid(plan.ntiles, plan.B);
   k_compose_bwd<KMAX><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
-                                                   plan.ntiles, sparse, bg[0], bg[1], bg[2], g_image, g_T_total, g_ct);
+                                                   plan.ntiles, sparse, bg[0], bg[1], bg[2], vb, g_ct);
 }
 
 int launch_compose_bwd(splx_ctx* ctx, const splx_partial* p, const splx_binning* bins, const PlanDev& plan,
-                       const float* bg, const float* g_image, const float* g_T_total, float* g_ct) {
+                       const float* bg, const ViewBufs& vb, float* g_ct) {
   const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
   const uint32_t* ranges = bins ? bins->tile_ranges : nullptr;
-  if (plan.K <= 8) compose_bwd_k<8>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
-  else if (plan.K <= 16) compose_bwd_k<16>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
-  else if (plan.K <= 32) compose_bwd_k<32>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
-  else compose_bwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, g_image, g_T_total, g_ct);
+  if (plan.K <= 8) compose_bwd_k<8>(ctx, p, ranges, plan, sparse, bg, vb, g_ct);
+  else if (plan.K <= 16) compose_bwd_k<16>(ctx, p, ranges, plan, sparse, bg, vb, g_ct);
+  else if (plan.K <= 32) compose_bwd_k<32>(ctx, p, ranges, plan, sparse, bg, vb, g_ct);
+  else compose_bwd_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, vb, g_ct);
   SPLX_LAUNCH_CHECK(ctx, "k_compose_bwd");
   return SPLX_OK;
 }
 
 template <int KMAX>
 static void compose_fused_k(splx_ctx* ctx, const splx_partial* p, const uint32_t* ranges, const PlanDev& plan, int sparse,
-                            const float* bg, const float* target, float gscale, float* image, float* T_total,
-                            double* loss_sum, float* g_ct, float sat_eps, uint8_t* state_out) {
+                            const float* bg, const ViewBufs& vb, float gscale, double* loss_sum, float* g_ct, float sat_eps,
+                            uint8_t* state_out) {
   dim3 grid(plan.ntiles, plan.B);
   if (state_out)
     k_compose_fused<KMAX, true><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
-                                                             plan.ntiles, sparse, bg[0], bg[1], bg[2], target, gscale, image,
-                                                             T_total, loss_sum, g_ct, sat_eps, plan.tile_state, state_out);
+                                                             plan.ntiles, sparse, bg[0], bg[1], bg[2], vb, gscale, loss_sum,
+                                                             g_ct, sat_eps, plan.tile_state, state_out);
   else
     k_compose_fused<KMAX, false><<<grid, CB, 0, ctx->stream>>>(p->ct, p->d, ranges, plan.pv, plan.K, plan.W, plan.H, plan.TX,
-                                                              plan.ntiles, sparse, bg[0], bg[1], bg[2], target, gscale, image,
-                                                              T_total, loss_sum, g_ct, sat_eps, nullptr, nullptr);
+                                                              plan.ntiles, sparse, bg[0], bg[1], bg[2], vb, gscale, loss_sum,
+                                                              g_ct, sat_eps, nullptr, nullptr);
 }
 
+// gscale = scale / (values of ONE launch's images) as splx_l1_loss_grad forms it over B*H*W*3 values
 int launch_compose_fused(splx_ctx* ctx, const splx_partial* p, const splx_binning* bins, const PlanDev& plan,
-                         const float* bg, const float* target, float scale, float* image, float* T_total,
-                         double* loss_sum, float* g_ct, float sat_eps, uint8_t* state_out) {
+                         const float* bg, const ViewBufs& vb, float scale, double* loss_sum, float* g_ct, float sat_eps,
+                         uint8_t* state_out) {
   const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
   const uint32_t* ranges = bins ? bins->tile_ranges : nullptr;
-  const float gscale = scale / (float)((int64_t)plan.B * plan.W * plan.H * 3);   // as splx_l1_loss_grad over B*H*W*3 values
-  if (plan.K <= 8) compose_fused_k<8>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
-  else if (plan.K <= 16) compose_fused_k<16>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
-  else if (plan.K <= 32) compose_fused_k<32>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
-  else compose_fused_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, target, gscale, image, T_total, loss_sum, g_ct, sat_eps, state_out);
+  const float gscale = scale / (float)((int64_t)plan.B * plan.W * plan.H * 3);
+  if (plan.K <= 8) compose_fused_k<8>(ctx, p, ranges, plan, sparse, bg, vb, gscale, loss_sum, g_ct, sat_eps, state_out);
+  else if (plan.K <= 16) compose_fused_k<16>(ctx, p, ranges, plan, sparse, bg, vb, gscale, loss_sum, g_ct, sat_eps, state_out);
+  else if (plan.K <= 32) compose_fused_k<32>(ctx, p, ranges, plan, sparse, bg, vb, gscale, loss_sum, g_ct, sat_eps, state_out);
+  else compose_fused_k<SPLX_MAX_K>(ctx, p, ranges, plan, sparse, bg, vb, gscale, loss_sum, g_ct, sat_eps, state_out);
   SPLX_LAUNCH_CHECK(ctx, "k_compose_fused");
   return SPLX_OK;
 }

@@ -56,8 +56,11 @@ __device__ __forceinline__ GeoIn load_geo(const splx_gaussians& g, int64_t i) {
 __device__ __forceinline__ bool geometry(const GeoIn& in, const CamDev& cam, float dilation, Geo& G) {
   const float mx = in.m[0], my = in.m[1], mz = in.m[2];
 #pragma unroll
-  for (int r = 0; r < 3; ++r)
+  for (int r = 0; r < 2; ++r)
     G.p[r] = cam.R[3 * r] * mx + cam.R[3 * r + 1] * my + cam.R[3 * r + 2] * mz + cam.t[r];
+  // the depth is the sort key (s12): a fixed fp32 operation order, so that two Gaussians whose depths differ by less
+  // than a rounding are ordered by every build of this kernel -- and by the oracle -- alike
+  G.p[2] = __fadd_rn(__fmaf_rn(cam.R[8], mz, __fmaf_rn(cam.R[7], my, __fmul_rn(cam.R[6], mx))), cam.t[2]);
   if (!(G.p[2] > cam.near_z)) return false;
 #pragma unroll
   for (int k = 0; k < 3; ++k) G.s[k] = expf(in.ls[k]);
@@ -170,29 +173,21 @@ __device__ __forceinline__ void colour(const float4* sh4, int lane, const CamDev
   out.clamp[i] = cl;
 }
 
-// PARTS: 1 = the geometry (everything the binning needs: 2-D mean, depth, conic, opacity, radius, tiles touched,
-// records 0-1 of the blend layout), 2 = the colour (SH -> rgb, clamp bits, record 2), 3 = both in one pass.  The
-// colour half reads tiles_touched written by the geometry half to know whether the Gaussian is visible; it depends
-// on nothing else of it, so a caller may run it beside the binning (splx_project_parts_plan).
-//
 // SH rows: a thread-per-Gaussian read of its 192-byte row is a 192-byte stride across the warp -- every 16-byte load
 // instruction touches 32 different lines (32 L1 wavefronts instead of 4) and the kernel ran at half the HBM roof,
-// bound by the L1's wavefront rate (profiles/r01e: lg_throttle + long_scoreboard).  The 32 rows of a warp are 6 KB of
+// bound by the L1's wavefront rate (ncu: lg_throttle + long_scoreboard stalls).  The 32 rows of a warp are 6 KB of
 // CONTIGUOUS memory, so when at least SH_STAGE_MIN of them are visible the warp copies the block with coalesced
 // 16-byte cp.async into shared memory (chunk index XOR-swizzled by the row so that the row-wise LDS.128 of a quarter
 // warp hits eight different bank groups) and reads its rows from there; with fewer visible rows (the culled
 // partitions of a city view) the direct loads touch less memory and are kept.
-#ifndef SPLX_SH_STAGE
-#define SPLX_SH_STAGE 1
-#endif
 constexpr int SH_STAGE_MIN = 12;
-template <int DEG, int PARTS>
+template <int DEG>
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected out) {
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;
-  constexpr bool STAGE = SPLX_SH_STAGE && (PARTS & 2) && DEG > 0;
+  constexpr bool STAGE = DEG > 0;
   __shared__ __align__(16) float4 s_sh[STAGE ? PROJ_THREADS * NV : 1];
   const int r = find_run(rt, (int)blockIdx.x);
   const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
@@ -200,12 +195,7 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   const CamDev& cam = plan.cam[rt.view[r]];   // the view this partition renders (indexed constant-bank loads)
   float m[3] = {0.f, 0.f, 0.f};
   bool vis = false;
-  if (PARTS == 2) {
-    if (active) {
-      vis = out.tiles_touched[i] != 0;
-      if (vis) { m[0] = g.mean[3 * i]; m[1] = g.mean[3 * i + 1]; m[2] = g.mean[3 * i + 2]; }
-    }
-  } else if (active) {
+  if (active) {
     Geo G;
     const GeoIn gin = load_geo(g, i);
     vis = geometry(gin, cam, cfg.dilation, G);
@@ -245,7 +235,6 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       m[0] = gin.m[0]; m[1] = gin.m[1]; m[2] = gin.m[2];
     }
   }
-  if (!(PARTS & 2)) return;
   float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
   if (active && !vis) {
     out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
@@ -299,7 +288,7 @@ __device__ __forceinline__ void sh_grad(int deg, float x, float y, float z, floa
 
 // Backward block = 128 Gaussians.  The 48 SH coefficients of a Gaussian are 192 contiguous bytes, so a
 // thread-per-Gaussian access has a 192-byte stride: scattered 4-byte read-modify-writes of the SH
-// gradient ran at 9 % of the HBM roof (profiles/r01a).  Here the block's SH tile [128][48] and, when
+// gradient ran at 9 % of the HBM roof (profiles/r01a_launches_aerial_1M.md).  Here the block's SH tile [128][48] and, when
 // accumulating, the tile of the SH gradient travel global -> shared with 16-byte cp.async (LDGSTS)
 // issued before the geometry chain, so ~50 KB per block are in flight while the ALU work runs; the
 // result leaves with coalesced 128-bit stores.  Row stride 52 floats keeps 16-byte alignment and makes
@@ -316,45 +305,16 @@ __device__ __forceinline__ void cp_async_wait_all() {
   asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
 }
 
-// Optional optimiser fusion (splx_project_backward_adam_plan): the LAST projection backward of an iteration
-// applies Adam to every row it owns straight from the gradient it has just formed (plus, when accumulating, the
-// gradient the earlier views left in memory), so the gradient is never written and Adam never re-reads it:
-// 24 B per parameter (28 accumulating) instead of 8 + 28.  Same statements as adam.cu's adam1.
-__device__ __forceinline__ void adam_step1(float& p, float g, float& m, float& v, const AdamFuse& a, float lr, float ibc1,
-                                           float ibc2) {
-  m = fmaf(a.b1, m, a.omb1 * g);
-  v = fmaf(a.b2, v, a.omb2 * g * g);
-  p -= lr * (m * ibc1) / (sqrtf(v * ibc2) + a.eps);
-}
-__device__ __forceinline__ void adam_vec4(float* pp, float* pm, float* pv, float4 g, const AdamFuse& a, float lr, float ibc1,
-                                          float ibc2) {
-  float4 p = *reinterpret_cast<float4*>(pp), m = *reinterpret_cast<float4*>(pm), v = *reinterpret_cast<float4*>(pv);
-  adam_step1(p.x, g.x * a.gscale, m.x, v.x, a, lr, ibc1, ibc2);
-  adam_step1(p.y, g.y * a.gscale, m.y, v.y, a, lr, ibc1, ibc2);
-  adam_step1(p.z, g.z * a.gscale, m.z, v.z, a, lr, ibc1, ibc2);
-  adam_step1(p.w, g.w * a.gscale, m.w, v.w, a, lr, ibc1, ibc2);
-  *reinterpret_cast<float4*>(pp) = p; *reinterpret_cast<float4*>(pm) = m; *reinterpret_cast<float4*>(pv) = v;
-}
-__device__ __forceinline__ void adam_scalar(float* pp, float* pm, float* pv, float g, const AdamFuse& a, float lr, float ibc1,
-                                            float ibc2) {
-  float p = *pp, m = *pm, v = *pv;
-  adam_step1(p, g * a.gscale, m, v, a, lr, ibc1, ibc2);
-  *pp = p; *pm = m; *pv = v;
-}
-
-#ifndef SPLX_PB_MIN_CTAS
-#define SPLX_PB_MIN_CTAS 5   /* 96 registers, no spills; 6 spills and is not faster (measured) */
-#endif
+constexpr int PB_MIN_CTAS = 5;   // 96 registers, no spills; 6 spills and is not faster (measured)
 // LIST (accumulating launches only): the rows of a block are 128 entries of the binning's list of VISIBLE Gaussians
 // (splx_bin_sort_visible) instead of 128 consecutive Gaussians, so the work follows the visible count -- on the
 // city scenes ~10 % of the participating Gaussians -- and not the partition sizes; the grid is persistent because
 // the count lives on the device.
-template <int DEG, bool ACC, bool ADAM, int LIST>   // LIST: 0 = every row of the runs, 1 = the visible list, 2 = the list + `touched` flags
-__global__ void __launch_bounds__(PB_THREADS, SPLX_PB_MIN_CTAS)
+template <int DEG, bool ACC, int LIST>   // LIST: 0 = every row of the runs, 1 = the visible list, 2 = the list + `touched` flags
+__global__ void __launch_bounds__(PB_THREADS, PB_MIN_CTAS)
 k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected pr, float* __restrict__ g2d, int clear_g2d, splx_gaussian_grads out,
-              const __grid_constant__ AdamFuse af, const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr,
-              uint8_t* __restrict__ touched) {
+              const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr, uint8_t* __restrict__ touched) {
   extern __shared__ __align__(16) float s_dyn[];
   float* s_sh = s_dyn;                                   // [128][52] sh in, SH gradient out
   float* s_old = s_dyn + PB_THREADS * PB_STRIDE;         // [128][52] previous SH gradient (ACC only)
@@ -395,8 +355,8 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   constexpr int NV = (NSH * 3 + 3) / 4;        // float4 chunks of a row that hold used coefficients
   // Two dependent rounds of loads: the radius (4 B per row, decides visibility), then -- for visible rows only --
   // every other per-Gaussian input at once (independent loads in flight together).  Requesting them inside the
-  // geometry chain stalled the kernel on dependent loads (profiles/r01k); requesting them for culled rows too
-  // moved ~100 B per culled row, which is most rows on the city scenes (profiles/r01n).
+  // geometry chain stalled the kernel on dependent loads (23 % of DRAM peak); requesting them for culled rows too
+  // moved ~100 B per culled row, which is most rows on the city scenes.
   const bool inr = (i < run_end) && (view >= 0);
   const int rad = inr ? pr.radius[i] : 0;
   GeoIn gin;
@@ -558,17 +518,9 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   }
 #pragma unroll
   for (int k = 0; k < 3; ++k) { s_m[3 * threadIdx.x + k] = dmu[k]; s_s[3 * threadIdx.x + k] = dls[k]; }
-  float ibc1 = 0.f, ibc2 = 0.f;
-  if (ADAM) { ibc1 = af.bc[0]; ibc2 = af.bc[1]; }
   if (i < run_end) {
     float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
-    if (ADAM) {
-      float4 gq = dq;                     // zeros for a culled row
-      float gl = dlogit;
-      if (ACC) { const float4 cur = *oq; gq.x += cur.x; gq.y += cur.y; gq.z += cur.z; gq.w += cur.w; gl += out.opacity_logit[i]; }
-      adam_vec4(af.p[2] + 4 * i, af.m[2] + 4 * i, af.v[2] + 4 * i, gq, af, af.lr[2], ibc1, ibc2);
-      adam_scalar(af.p[3] + i, af.m[3] + i, af.v[3] + i, gl, af, af.lr[3], ibc1, ibc2);
-    } else if (ACC) {
+    if (ACC) {
       if (vis) {
         float4 cur = fresh ? make_float4(0.f, 0.f, 0.f, 0.f) : *oq;
         cur.x += dq.x; cur.y += dq.y; cur.z += dq.z; cur.w += dq.w;
@@ -581,51 +533,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     }
   }
   __syncthreads();
-  // coalesced write-back of the SH-gradient tile (+= needs visible rows only; = writes every row; with ADAM the
-  // gradient is consumed here instead: every row of the tile takes its optimiser step)
-  if (ADAM) {
-    // four chunks at a time: all of their parameter / moment (/ old gradient) loads are requested before the first
-    // store, because the compiler cannot move a load above a store that may alias it -- 12-16 independent 16-byte
-    // loads per thread keep enough bytes in flight for this low-occupancy kernel to stream
-#pragma unroll
-    for (int c0 = 0; c0 < 12; c0 += 4) {
-      float4 P[4], M[4], V[4], Gr[4];
-      int64_t off[4];
-      bool ok[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int q = (c0 + u) * PB_THREADS + threadIdx.x;
-        const int row = q / 12, c4 = q - row * 12;
-        ok[u] = row < nrows;
-        off[u] = 48 * (ok[u] ? s_idx[row] : 0) + 4 * c4;
-        Gr[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (ok[u]) {
-          const bool live = s_vis[row] && c4 < NV;
-          P[u] = *reinterpret_cast<const float4*>(af.p[4] + off[u]);
-          M[u] = *reinterpret_cast<const float4*>(af.m[4] + off[u]);
-          V[u] = *reinterpret_cast<const float4*>(af.v[4] + off[u]);
-          if (live) Gr[u] = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
-          if (ACC) {
-            const float4 o = live ? *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4)
-                                  : *reinterpret_cast<const float4*>(out.sh + off[u]);
-            Gr[u].x += o.x; Gr[u].y += o.y; Gr[u].z += o.z; Gr[u].w += o.w;
-          }
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        if (ok[u]) {
-          adam_step1(P[u].x, Gr[u].x * af.gscale, M[u].x, V[u].x, af, af.lr[4], ibc1, ibc2);
-          adam_step1(P[u].y, Gr[u].y * af.gscale, M[u].y, V[u].y, af, af.lr[4], ibc1, ibc2);
-          adam_step1(P[u].z, Gr[u].z * af.gscale, M[u].z, V[u].z, af, af.lr[4], ibc1, ibc2);
-          adam_step1(P[u].w, Gr[u].w * af.gscale, M[u].w, V[u].w, af, af.lr[4], ibc1, ibc2);
-          *reinterpret_cast<float4*>(af.p[4] + off[u]) = P[u];
-          *reinterpret_cast<float4*>(af.m[4] + off[u]) = M[u];
-          *reinterpret_cast<float4*>(af.v[4] + off[u]) = V[u];
-        }
-      }
-    }
-  } else {
+  // coalesced write-back of the SH-gradient tile (+= needs visible rows only; = writes every row)
 #pragma unroll
   for (int c = 0; c < 12; ++c) {
     const int q = c * PB_THREADS + threadIdx.x;
@@ -646,7 +554,6 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       }
     }
   }
-  }
   // mean / log_scale gradient tiles: 96 float4 each; a partial last block, or a run that does not start
   // on a multiple of 4 Gaussians (12-byte rows: 16-byte alignment needs base % 4 == 0), falls back to scalars
   if (!LIST && nrows == PB_THREADS && (base & 3) == 0) {
@@ -659,22 +566,12 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
         a.x += om.x; a.y += om.y; a.z += om.z; a.w += om.w;
         b.x += os.x; b.y += os.y; b.z += os.z; b.w += os.w;
       }
-      if (ADAM) {
-        const int64_t off = 3 * base + 4 * threadIdx.x;
-        adam_vec4(af.p[0] + off, af.m[0] + off, af.v[0] + off, a, af, af.lr[0], ibc1, ibc2);
-        adam_vec4(af.p[1] + off, af.m[1] + off, af.v[1] + off, b, af, af.lr[1], ibc1, ibc2);
-      } else {
-        *dm = a; *ds = b;
-      }
+      *dm = a; *ds = b;
     }
   } else if (i < run_end) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      if (ADAM) {
-        const float gm = dmu[k] + (ACC ? out.mean[3 * i + k] : 0.f), gs = dls[k] + (ACC ? out.log_scale[3 * i + k] : 0.f);
-        adam_scalar(af.p[0] + 3 * i + k, af.m[0] + 3 * i + k, af.v[0] + 3 * i + k, gm, af, af.lr[0], ibc1, ibc2);
-        adam_scalar(af.p[1] + 3 * i + k, af.m[1] + 3 * i + k, af.v[1] + 3 * i + k, gs, af, af.lr[1], ibc1, ibc2);
-      } else if (ACC) {
+      if (ACC) {
         out.mean[3 * i + k] = (fresh ? 0.f : out.mean[3 * i + k]) + dmu[k];
         out.log_scale[3 * i + k] = (fresh ? 0.f : out.log_scale[3 * i + k]) + dls[k];
       }
@@ -685,105 +582,72 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   }
 }
 
-template <int DEG, bool ACC, bool ADAM>
+template <int DEG, bool ACC>
 static void launch_pb(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
-                      const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
-                      const AdamFuse& af) {
+                      const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (ACC ? 2 : 1);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, ADAM, 0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-  k_project_bwd<DEG, ACC, ADAM, 0><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(
-      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, nullptr, nullptr, nullptr);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, ACC, 0>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  k_project_bwd<DEG, ACC, 0><<<(unsigned)rt.blocks_total, PB_THREADS, smem, ctx->stream>>>(
+      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, nullptr, nullptr, nullptr);
 }
 
 // accumulating launch over the list of visible Gaussians (persistent grid: the count lives on the device)
-template <int DEG>
+template <int DEG, int LIST>
 static void launch_pb_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
                            const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
-                           const AdamFuse& af, const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
+                           const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
   const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * 2;
   const int64_t need = (rt.jprefix[rt.n] + PB_THREADS - 1) / PB_THREADS;
   const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 4 ? need : (int64_t)SPLX_SM_COUNT * 4;
-  if (touched) {
-    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    k_project_bwd<DEG, true, false, 2><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
-        *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis, touched);
-  } else {
-    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(k_project_bwd<DEG, true, false, 1>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    k_project_bwd<DEG, true, false, 1><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
-        *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, af, vlist, nvis, touched);
-  }
+  cudaFuncSetAttribute(k_project_bwd<DEG, true, LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(k_project_bwd<DEG, true, LIST>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+  k_project_bwd<DEG, true, LIST><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
+      *g, plan, rt, ctx->cfg, *pr, g2d, clear_g2d, *grads, vlist, nvis, touched);
 }
 
-template <bool ACC, bool ADAM>
-static void launch_pb_deg(splx_ctx* ctx, int deg, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
-                          const splx_projected* pr, float* g2d, int clr, const splx_gaussian_grads* grads, const AdamFuse& af) {
-  switch (deg) {
-    case 0: launch_pb<0, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
-    case 1: launch_pb<1, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
-    case 2: launch_pb<2, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
-    default: launch_pb<3, ACC, ADAM>(ctx, g, plan, rt, pr, g2d, clr, grads, af); break;
-  }
+template <int DEG>
+static void launch_pb_deg(splx_ctx* ctx, bool overwrite, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
+                          const splx_projected* pr, float* g2d, int clr, const splx_gaussian_grads* grads,
+                          const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
+  if (vlist && touched) launch_pb_list<DEG, 2>(ctx, g, plan, rt, pr, g2d, clr, grads, vlist, nvis, touched);
+  else if (vlist) launch_pb_list<DEG, 1>(ctx, g, plan, rt, pr, g2d, clr, grads, vlist, nvis, touched);
+  else if (overwrite) launch_pb<DEG, false>(ctx, g, plan, rt, pr, g2d, clr, grads);
+  else launch_pb<DEG, true>(ctx, g, plan, rt, pr, g2d, clr, grads);
 }
 
 }  // namespace
 
-template <int PARTS>
-static void launch_pf(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt, int deg,
-                      const splx_projected* out) {
-  const unsigned grid = (unsigned)rt.blocks_total;
-  switch (deg) {
-    case 0: k_project_fwd<0, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    case 1: k_project_fwd<1, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    case 2: k_project_fwd<2, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    default: k_project_fwd<3, PARTS><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-  }
-}
-
 int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
-                       const splx_projected* out, int parts) {
+                       const splx_projected* out) {
   const RunTable rt = make_runs(plan, part_offsets, PROJ_THREADS, false);
   if (rt.blocks_total == 0) return SPLX_OK;
-  if (parts == 1) launch_pf<1>(ctx, g, plan, rt, deg, out);
-  else if (parts == 2) launch_pf<2>(ctx, g, plan, rt, deg, out);
-  else launch_pf<3>(ctx, g, plan, rt, deg, out);
+  const unsigned grid = (unsigned)rt.blocks_total;
+  switch (deg) {
+    case 0: k_project_fwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 1: k_project_fwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    case 2: k_project_fwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+    default: k_project_fwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+  }
   SPLX_LAUNCH_CHECK(ctx, "k_project_fwd");
   return SPLX_OK;
 }
 
 int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
                        const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads,
-                       const AdamFuse* adam, const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
+                       const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
   const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
   const bool overwrite = (flags & SPLX_PB_OVERWRITE) != 0;
-  if (vlist && nvis && !overwrite && !adam) {      // += over the visible Gaussians only
-    const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, false);
-    if (rt.jprefix[rt.n] == 0) return SPLX_OK;
-    AdamFuse none;
-    memset(&none, 0, sizeof none);
-    switch (deg) {
-      case 0: launch_pb_list<0>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
-      case 1: launch_pb_list<1>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
-      case 2: launch_pb_list<2>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
-      default: launch_pb_list<3>(ctx, g, plan, rt, pr, g2d, clr, grads, none, vlist, nvis, touched); break;
-    }
-    SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
-    return SPLX_OK;
-  }
-  // "=" must also clear the rows of partitions that do not participate in this launch; the fused optimiser
-  // step must reach every row of every partition
-  const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, overwrite || adam != nullptr);
-  if (rt.blocks_total == 0) return SPLX_OK;
-  AdamFuse none;
-  memset(&none, 0, sizeof none);
-  if (adam) {
-    if (overwrite) launch_pb_deg<false, true>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, *adam);
-    else launch_pb_deg<true, true>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, *adam);
-  } else {
-    if (overwrite) launch_pb_deg<false, false>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, none);
-    else launch_pb_deg<true, false>(ctx, deg, g, plan, rt, pr, g2d, clr, grads, none);
+  const bool list = vlist && nvis && !overwrite;      // += over the visible Gaussians only
+  // "=" must also clear the rows of partitions that do not participate in this launch
+  const RunTable rt = make_runs(plan, part_offsets, PB_THREADS, overwrite);
+  if (list ? rt.jprefix[rt.n] == 0 : rt.blocks_total == 0) return SPLX_OK;
+  if (!list) { vlist = nullptr; nvis = nullptr; touched = nullptr; }
+  switch (deg) {
+    case 0: launch_pb_deg<0>(ctx, overwrite, g, plan, rt, pr, g2d, clr, grads, vlist, nvis, touched); break;
+    case 1: launch_pb_deg<1>(ctx, overwrite, g, plan, rt, pr, g2d, clr, grads, vlist, nvis, touched); break;
+    case 2: launch_pb_deg<2>(ctx, overwrite, g, plan, rt, pr, g2d, clr, grads, vlist, nvis, touched); break;
+    default: launch_pb_deg<3>(ctx, overwrite, g, plan, rt, pr, g2d, clr, grads, vlist, nvis, touched); break;
   }
   SPLX_LAUNCH_CHECK(ctx, "k_project_bwd");
   return SPLX_OK;

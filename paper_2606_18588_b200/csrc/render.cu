@@ -6,7 +6,7 @@
 // below T_eps.  Backward: PAPER.md L184 ("the per-Gaussian gradient backpropagates through the
 // intermediate partial pixel"), with dL/dC^m and dL/dT^m coming from Eq.6-7 (compose.cu).
 //
-// Both kernels are instruction-issue bound (profiles/r01a: 90 % issue-slot utilisation, DRAM 2 %),
+// Both kernels are instruction-issue bound (profiles/r01a_ncu_blend_kernels.md: 90 % issue-slot utilisation, DRAM 2 %),
 // so the design minimises instructions per useful (pixel, Gaussian) pair:
 //   * grid = (tiles, K), CTA = 2 autonomous warps, one per HALF tile (16 x 8 pixels).  A lane owns 4
 //     pixels, one in each 8 x 4 block ("slot") of the half tile, so the record of a Gaussian is read
@@ -22,7 +22,7 @@
 //     registers and stores its nine partial gradients to a shared staging block (9 conflict-free
 //     stores per (Gaussian, half tile) item); every seven items the 63 rows are summed over the lanes
 //     (one row per lane, rotating column: no bank conflict) and leave as two rounds of 32 distinct
-//     atomics.  ~28 instructions per item instead of ~75 for a shuffle tree + selects (profiles/r01k).
+//     atomics.  ~28 instructions per item instead of ~75 for a shuffle tree + selects.
 #include "common.cuh"
 
 namespace {
@@ -118,11 +118,9 @@ __device__ __forceinline__ bool eval_alpha(float dx, float dy, float adx, float 
   return (p2 <= 0.0f) && (alpha >= amin);
 }
 
-#ifndef SPLX_FWD_MIN_CTAS
-#define SPLX_FWD_MIN_CTAS 14   /* 71 registers; the sweep 12..20 shows no effect below spilling: issue-bound */
-#endif
+constexpr int FWD_MIN_CTAS = 14;   // 71 registers; a sweep 12..20 showed no effect below spilling: issue-bound
 template <bool COUNT>
-__global__ void __launch_bounds__(BLOCK, SPLX_FWD_MIN_CTAS)
+__global__ void __launch_bounds__(BLOCK, FWD_MIN_CTAS)
 k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const __grid_constant__ PartView pv, int sparse,
              float* __restrict__ out_ct, float* __restrict__ out_d, uint32_t* __restrict__ out_n,
@@ -232,13 +230,8 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 // Staging block of one warp in the backward: STAGE_ITEMS (Gaussian, half tile) items x 9 gradient values x 32
 // lane partials.  63 rows = two rounds of 32 row sums; a lane sums its row with a rotating column so that the
 // 32 lanes hit 32 different banks.
-#ifndef SPLX_STAGE_ITEMS
-#define SPLX_STAGE_ITEMS 7
-#endif
-#ifndef SPLX_BWD_MIN_CTAS
-#define SPLX_BWD_MIN_CTAS 10   /* 92 registers; 12 and 14 CTAs/SM with a 3-item stage measured slower */
-#endif
-constexpr int STAGE_ITEMS = SPLX_STAGE_ITEMS;
+constexpr int STAGE_ITEMS = 7;
+constexpr int BWD_MIN_CTAS = 10;   // 92 registers; 12 and 14 CTAs/SM with a 3-item stage measured slower
 constexpr int STAGE_ROUNDS = (STAGE_ITEMS * 9 + 31) / 32;
 struct __align__(128) Stage { float v[STAGE_ITEMS * 9][32]; };
 
@@ -272,7 +265,7 @@ __device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int la
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(BLOCK, SPLX_BWD_MIN_CTAS)
+__global__ void __launch_bounds__(BLOCK, BWD_MIN_CTAS)
 k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const float* __restrict__ ct,
              const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d,

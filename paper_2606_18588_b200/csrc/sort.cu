@@ -17,10 +17,8 @@
 
 namespace {
 
-#ifndef SPLX_SCAN_IPT
-#define SPLX_SCAN_IPT 8   /* 8 against 16, same session: city_10M 12.50 / 12.62 ms, street_10M 16.46 / 16.56, city_100M 66.8 / 67.2, others equal */
-#endif
-constexpr int SCAN_THREADS = 512, SCAN_IPT = SPLX_SCAN_IPT, SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // 4096 elements per tile
+// 8 items per thread against 16, same session: city_10M 12.50 / 12.62 ms, street_10M 16.46 / 16.56, city_100M 66.8 / 67.2
+constexpr int SCAN_THREADS = 512, SCAN_IPT = 8, SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // 4096 elements per tile
 constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
 static_assert(SCAN_TILE % RS_TILE == 0, "the compaction scan clears the radix status words of the tiles it covers");
@@ -231,7 +229,7 @@ int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_pt
 // ---------------------------------------------------------------------- LSD radix sort --
 // "Onesweep" organisation: the digit histograms of ALL passes are counted in one read of the
 // input (a histogram does not depend on the order), then each pass is ONE kernel: a tile ranks
-// its 4096 keys (stable, warp multisplit with __match_any_sync), chains its per-digit counts to
+// its 2048 keys (stable; digit peers found with eight ballots, see digit_peers), chains its per-digit counts to
 // its predecessors by look-back (256 independent chains, one per thread) and scatters.
 // Per item and pass: key+value read once and written once (24 B for 64-bit keys, 16 B for 32-bit).
 
@@ -308,11 +306,8 @@ k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t*
 
 // Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
 // started and the look-back spin cannot wait on a CTA that was never scheduled.
-#ifndef SPLX_RS_MIN_CTAS
-#define SPLX_RS_MIN_CTAS 4
-#endif
 template <typename KeyT>
-__global__ void __launch_bounds__(RS_THREADS, SPLX_RS_MIN_CTAS)
+__global__ void __launch_bounds__(RS_THREADS, 4)
 k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
              uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
              uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits) {
@@ -496,7 +491,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
             uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
             uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride,
             const __grid_constant__ CrossEmit cx) {
-  if (emit_by_output(cnt)) return;
+  if (emit_by_output(cnt) || (cnt->m_total >> 32)) return;   // M >= 2^32: the 32-bit offsets have wrapped, nothing is emitted
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
   __shared__ uint32_t s_hist[MAX_PASSES * 256];
@@ -581,7 +576,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
             uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
             uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride,
             const __grid_constant__ CrossEmit cx) {
-  if (!emit_by_output(cnt)) return;
+  if (!emit_by_output(cnt) || (cnt->m_total >> 32)) return;
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
   __shared__ uint32_t s_hist[MAX_PASSES * 256];
@@ -685,7 +680,11 @@ k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint
       continue;
     }
     if (count_kept && j + 1 == m) *m_out = m;
-    if (tile_state && tile_state[s]) continue;   // a skipped (partition, tile) slot keeps the empty range (0,0)
+    if (tile_state && tile_state[s]) {           // a skipped (partition, tile) slot keeps the empty range (0,0)
+      // a NON-EMPTY list dropped on geometric grounds: the caller's regions were not conservative (splx_footprint_margin)
+      if ((tile_state[s] & SPLX_TILE_INVISIBLE) && (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s)) atomicAdd((unsigned long long*)(m_out + 1), 1ull);
+      continue;
+    }
     if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
     if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
   }
@@ -821,6 +820,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
 
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(base, 0, L.zero_bytes, ctx->stream));
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->tile_ranges, 0, (size_t)K * ntiles * 2 * sizeof(uint32_t), ctx->stream));
+  SPLX_CUDA_OK(ctx, cudaMemsetAsync(out->num_intersections + 1, 0, sizeof(uint64_t), ctx->stream));
   const RunTable rt = make_runs(plan, part_offsets, 1, false);
   const int64_t n_act = rt.jprefix[rt.n];    // Gaussians of the participating partitions
   if (out->slot_order)   // count of live slots and the class cursors

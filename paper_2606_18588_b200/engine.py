@@ -1,13 +1,15 @@
-"""Buffer ownership and call sequencing for one training iteration on one B200.
+"""Buffer ownership for training on one B200: ``Trainer`` owns the device memory (parameters, gradients, Adam
+moments, projected attributes, binning, partial-pixel buffers) and hands it to the C ABI of ``include/splx.h``.
 
-``Trainer`` owns the device memory (parameters, gradients, Adam moments, projected attributes,
-binning, partial-pixel buffers) and issues the C-ABI calls of ``include/splx.h`` in the order
-of SURVEY.md s3(b).  It performs no arithmetic of the method itself: every step runs in the
-CUDA kernels behind ``binding.Context``.  K partitions = K contiguous slices of the SoA.
+A whole training iteration -- a1-a10 for every bucket of views, the optimiser step, the host copies of the
+end-to-end path -- is ONE library call (``splx_iteration``, csrc/iteration.cu); this module only fills in its structs.
+The stage-by-stage methods (``forward``, ``loss_grad``, ``backward``, ``forward_plan`` ...) issue the single-stage calls
+in the order of SURVEY.md s3(b) and exist for stage-wise parity tests.  No arithmetic of the method happens here.
+K partitions = K contiguous slices of the SoA.
 """
 from __future__ import annotations
 
-import os
+import ctypes as C
 
 import numpy as np
 import torch
@@ -28,14 +30,20 @@ def _flat_layout(n):
     return offs, cur
 
 
+class CapacityError(RuntimeError):
+    """A bucket had more tile intersections than ``Trainer.capacity``: its farthest keys were dropped."""
+
+
 class Trainer:
     def __init__(self, params: dict, part_offsets, width, height, sh_degree=3, bg=(0.0, 0.0, 0.0),
-                 capacity=None, device=0, cfg=None, lr=None):
+                 capacity=None, device=0, cfg=None, lr=None, max_views=binding.MAX_VIEWS):
         self.ctx = binding.Context(device, cfg=cfg)
+        self.cfg = cfg
         dev = self.ctx.device
         self.n = int(params["opacity_logit"].shape[0])
         self.K = len(part_offsets) - 1
         self.part_offsets = [int(x) for x in part_offsets]
+        self._po = (C.c_int64 * (self.K + 1))(*self.part_offsets)
         self.W, self.H, self.sh_degree, self.bg = int(width), int(height), int(sh_degree), tuple(bg)
         self.lr = dict(DEFAULT_LR if lr is None else lr)
         offs, total = _flat_layout(self.n)
@@ -59,34 +67,34 @@ class Trainer:
         self.image = torch.empty((self.H, self.W, 3), dtype=torch.float32, device=dev)
         self.T_total = torch.empty((self.H, self.W), dtype=torch.float32, device=dev)
         self.g_image = torch.empty((self.H, self.W, 3), dtype=torch.float32, device=dev)
-        self.loss_sum = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.loss_sum = torch.zeros(2, dtype=torch.float64, device=dev)      # [0] sum |image - target|, [1] sum SSIM
         self.pairs = torch.zeros(4, dtype=torch.int64, device=dev)
         self.step_count = 0
-        #: fuse the Adam step into the last projection backward (splx_project_backward_adam_plan).  Off by default:
-        #: at 4 CTAs/SM (124 registers) the fused kernel streams the moments at ~4 TB/s, while the stand-alone Adam
-        #: kernel runs at 95 % of the HBM roof -- measured 0.44 ms fused against 0.11 + 0.27 ms
-        self.fuse_adam = False
-        #: accumulating projection backward over the binning's list of visible Gaussians
-        #: (splx_project_backward_list_plan) instead of all rows of the participating partitions
-        self.use_visible_list = os.environ.get("SPLX_VISIBLE_LIST", "1") == "1"
+        self.max_views = int(max_views)
+        #: weight of the D-SSIM term of PAPER.md L95 (L = L_RGB + lambda L_D-SSIM; 0 = mean L1 only, the harness loss of
+        #: BASELINE.json configs[0]; DESIGN.md s33 takes lambda = 0.2 when it is switched on)
+        self.lambda_dssim = 0.0
         #: visible-only ("sparse") Adam -- an OPTION outside the paper: only Gaussians that received a gradient
         #: in the iteration take the step (splx_adam_sparse); no gradient buffer is ever zeroed or overwritten wholesale
-        self.sparse_adam = os.environ.get("SPLX_SPARSE_ADAM", "0") == "1"
-        self._touched = None
+        self.sparse_adam = False
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
-        self.pipeline_buckets = os.environ.get("SPLX_PIPELINE", "1") == "1"
+        self.pipeline_buckets = True
+        self._touched = None
         self._cam = None
-        self._aabb = None
+        self._aabb = None           # (lo, hi, max_scale or None): boxes of the geometric visibility prediction
         self._cross = None          # Q_cross masks (set_cross): cross-boundary filtering on
-        self._side = None
         self._ws_sort = None
         self._ws_bwd = None
-        # plan path (visibility prediction / consolidated views): buffers with a leading view dimension
-        self._images = self._T_totals = self._g_images = None
+        self._alt = None
+        self._images = None
         self._plan = None
         self._participants = {}     # view id -> partition bitmask (splx_visible_regions)
         self._geom_state = {}       # view id -> host uint8 [K, tiles]
         self._bucket_state = {}     # tuple of view ids -> device uint8 [K * tiles] (geometric | saturated bits)
+        self._graphs = {}
+        self._m_host = torch.zeros(max(self.max_views, 1), dtype=torch.int64).pin_memory()   # M of every bucket
+        self._m_event = None
+        self._m_buckets = 0
 
     # -- workspaces are sized per camera resolution (constant here) ----------------------------
     def _workspaces(self, cam):
@@ -96,6 +104,7 @@ class Trainer:
             nb = self.ctx.backward_ws_bytes(self.n, self.K, cam)
             self._ws_bwd = torch.empty(nb, dtype=torch.uint8, device=self.ctx.device)
 
+    # ---- stage by stage (parity surface) ---------------------------------------------------------------------
     def forward(self, cam, count_pairs=False):
         """a1-a6: project, bin/sort, render the K partials, compose."""
         self._workspaces(cam)
@@ -127,7 +136,7 @@ class Trainer:
                              zero_grad=zero_grad)
 
     def iteration(self, cams, targets):
-        """One training iteration over B views (gradients of the B mean losses are averaged)."""
+        """One training iteration over B views through the single-stage calls (gradients of the B mean losses are averaged)."""
         for b, (cam, tgt) in enumerate(zip(cams, targets)):
             self.forward(cam)
             self.loss_grad(tgt)
@@ -144,9 +153,11 @@ class Trainer:
     def _view_buffers(self, B):
         if self._images is None or self._images.shape[0] < B:
             dev = self.ctx.device
-            self._images = torch.empty((B, self.H, self.W, 3), dtype=torch.float32, device=dev)
-            self._T_totals = torch.empty((B, self.H, self.W), dtype=torch.float32, device=dev)
-            self._g_images = torch.empty((B, self.H, self.W, 3), dtype=torch.float32, device=dev)
+            nb = max(B, self.max_views)
+            self._images = torch.empty((nb, self.H, self.W, 3), dtype=torch.float32, device=dev)
+            self._T_totals = torch.empty((nb, self.H, self.W), dtype=torch.float32, device=dev)
+            self._g_images = torch.empty((nb, self.H, self.W, 3), dtype=torch.float32, device=dev)
+            self._graphs.clear()
         return self._images[:B], self._T_totals[:B], self._g_images[:B]
 
     def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True) -> binding.Plan:
@@ -168,7 +179,7 @@ class Trainer:
         return images
 
     def fused_buffers(self):
-        """g_ct [K,H,W,4] and g2d [n,12] of the fused path (g2d starts zeroed and is kept zero by
+        """g_ct [K,H,W,4] and g2d [n,12] of the training path (g2d starts zeroed and is kept zero by
         splx_project_backward's SPLX_PB_CLEAR_G2D)."""
         if getattr(self, "_g_ct", None) is None:
             dev = self.ctx.device
@@ -176,85 +187,16 @@ class Trainer:
             self._g2d = torch.zeros((max(self.n, 1), binding.G2D_STRIDE), dtype=torch.float32, device=dev)
         return self._g_ct, self._g2d
 
-    def prepare_adam(self):
-        """Host side of the fused optimiser step: count the step.  The bias corrections themselves come from the
-        DEVICE-resident counter (splx_adam_bias_step, launched by iteration_fused(adam=True)), so that a captured graph
-        advances them at every replay and no host value is read by work that is still in flight."""
-        if getattr(self, "_bc_dev", None) is None:
-            dev = self.ctx.device
-            self._bc_dev = torch.empty(2, dtype=torch.float32, device=dev)
-            self._step_dev = torch.full((1,), self.step_count, dtype=torch.int32, device=dev)
-        self.step_count += 1
-
-    def _bufs(self, which=0):
-        """(projected, binning, sort workspace) set `which`: set 1 is the double buffer of the pipelined multi-bucket
-        iteration (the next bucket is projected and binned while the current one is blended)."""
-        if which == 0:
-            return self.proj, self.bins, self._ws_sort
-        if getattr(self, "_alt", None) is None:
-            dev = self.ctx.device
-            self._alt = (binding.Projected(self.n, dev), binding.Binning(self.capacity, self.K, self.W, self.H, dev),
-                         torch.empty_like(self._ws_sort))
-        return self._alt
-
-    def _front(self, plan, bufs):
-        """a1-a4 of a bucket: project, bin/sort."""
-        proj, bins, ws = bufs
-        self.ctx.project_plan(self.params, self.part_offsets, plan, self.sh_degree, proj)
-        self._bin_sort(proj, plan, bins, ws)
-
-    def _back(self, plan, bufs, targets, overwrite, sat_eps, tile_state_out, adam, n_views):
-        """a5-a10 of a bucket: render, fused composition + loss + composition backward, raster and projection backward."""
-        proj, bins, ws = bufs
-        c = self.ctx
-        images, T_totals, _ = self._view_buffers(plan.B)
-        g_ct, g2d = self.fused_buffers()
-        c.render_partial_plan(proj, bins, plan, self.partials)
-        c.compose_l1_backward_plan(self.partials, bins, plan, self.bg, targets, images, T_totals, self.loss_sum, g_ct,
-                                   scale=float(plan.B), sat_eps=sat_eps if sat_eps is not None else 0.0,
-                                   tile_state_out=tile_state_out)
-        c.raster_backward_plan(proj, bins, plan, self.partials, g_ct, g2d)
-        if adam:     # the last backward of the iteration takes the optimiser step too (call prepare_adam() first)
-            c.adam_bias_step(self._step_dev, self._bc_dev)
-            c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
-                                         self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev,
-                                         grad_scale=1.0 / n_views, clear_g2d=True, overwrite=overwrite)
-        elif self.sparse_adam:    # every launch walks the visible list; the flags say which rows to store and which to add to
-            if self._touched is None:
-                self._touched = torch.zeros(max(self.n, 1), dtype=torch.uint8, device=self.ctx.device)
-            lst, cnt = c.bin_sort_visible(ws, self.n, self.capacity, self.K, plan.cams[0])
-            c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
-                                         lst, cnt, clear_g2d=True, touched=self._touched)
-        elif not overwrite and self.use_visible_list:   # an accumulating launch over the binning's visible list only
-            lst, cnt = c.bin_sort_visible(ws, self.n, self.capacity, self.K, plan.cams[0])
-            c.project_backward_list_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
-                                         lst, cnt, clear_g2d=True)
-        else:
-            c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, proj, g2d, self.grads,
-                                    clear_g2d=True, overwrite=overwrite)
-        return images
-
-    def iteration_fused(self, plan: binding.Plan, targets, overwrite=True, sat_eps=None, tile_state_out=None, adam=False,
-                        n_views=1):
-        """a1-a10 under a plan with composition, mean-L1 loss and composition backward in ONE kernel
-        (splx_compose_l1_backward_plan) -- the training path; the staged calls remain for stage-wise parity.
-        targets: device [B,H,W,3].  Returns images[B,H,W,3]."""
-        self._workspaces(plan.cams[0])
-        self._plan = plan
-        bufs = self._bufs(0)
-        self._front(plan, bufs)
-        return self._back(plan, bufs, targets, overwrite, sat_eps, tile_state_out, adam, n_views)
-
     def loss_grad_plan(self, targets):
         """a7 for B views at once: targets[B,H,W,3]; every view's loss is its own mean (scale = B)."""
         B = self._plan.B
         images, _, g_images = self._view_buffers(B)
-        self.ctx.l1_loss_grad(images, targets, g_images, self.loss_sum, float(B))
+        self.ctx.l1_loss_grad(images[:B], targets, g_images[:B], self.loss_sum, float(B))
 
     def backward_plan(self, overwrite=False, g_images=None):
         plan = self._plan
         _, _, gi = self._view_buffers(plan.B)
-        self.ctx.backward_plan(self.part_offsets, plan, self.partials, self.bg, gi if g_images is None else g_images,
+        self.ctx.backward_plan(self.part_offsets, plan, self.partials, self.bg, gi[:plan.B] if g_images is None else g_images,
                                None, self.params, self.proj, self.bins, self.sh_degree, self.grads, self._ws_bwd,
                                overwrite=overwrite)
 
@@ -262,6 +204,7 @@ class Trainer:
         """Cross-boundary per-ray filtering (L474-L476) on: Q_cross of every Gaussian against the cell
         boxes (to be called again when the Gaussians change); the depth intervals and Omega come from set_aabbs.
         cell_lo=None switches it off."""
+        self._graphs.clear()
         if cell_lo is None:
             self._cross = None
             return
@@ -273,19 +216,39 @@ class Trainer:
         if self._cross is None:
             self.ctx.bin_sort_plan(proj, self.part_offsets, plan, bins, ws)
             return
-        if getattr(plan, "_zr", None) is None:
-            plan._zr = binding.cross_depth_ranges(self._aabb[0], self._aabb[1], plan)
-        self.ctx.bin_sort_filtered_plan(proj, self.part_offsets, plan, self._cross, plan._zr, bins, ws)
+        self.ctx.bin_sort_filtered_plan(proj, self.part_offsets, plan, self._cross, self._depth_ranges(plan), bins, ws)
 
-    def set_aabbs(self, lo, hi):
-        """Static partition boxes (scenes.partition_aabbs) for the geometric visibility prediction."""
-        self._aabb = (np.ascontiguousarray(lo, np.float32), np.ascontiguousarray(hi, np.float32))
-        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear()
+    def _depth_ranges(self, plan):
+        if getattr(plan, "_zr", None) is None:
+            plan._zr = np.ascontiguousarray(binding.cross_depth_ranges(self._part_box[0], self._part_box[1], plan), np.float32)
+        return plan._zr
+
+    def set_aabbs(self, lo, hi, max_scale=None, box_part=None):
+        """Static boxes for the geometric visibility prediction (L212).  With max_scale (scenes.partition_boxes) the boxes
+        are boxes of MEANS covering the partitions (box j belongs to partition box_part[j]; None = one box per partition)
+        and splx_visible_regions builds the conservative regions of reading s21: no list the binning builds is cut --
+        the training path.  Without max_scale the boxes are taken as they are (tests of
+        the region geometry itself, e.g. the 3-sigma boxes of scenes.partition_aabbs)."""
+        lo = np.ascontiguousarray(lo, np.float32).reshape(-1, 3)
+        hi = np.ascontiguousarray(hi, np.float32).reshape(-1, 3)
+        bp = None if box_part is None else np.ascontiguousarray(box_part, np.int32)
+        assert bp is not None or lo.shape[0] == self.K, "one box per partition, or box_part"
+        self._aabb = (lo, hi, None if max_scale is None else np.ascontiguousarray(max_scale, np.float32), bp)
+        # one box per partition (the union of its boxes): the depth intervals D^k of the cross-boundary filter (s32)
+        plo = np.full((self.K, 3), np.inf, np.float32); phi = np.full((self.K, 3), -np.inf, np.float32)
+        for j in range(lo.shape[0]):
+            k = j if bp is None else int(bp[j])
+            plo[k] = np.minimum(plo[k], lo[j]); phi[k] = np.maximum(phi[k], hi[j])
+        empty = ~np.isfinite(plo).all(1)
+        plo[empty] = 0; phi[empty] = 0
+        self._part_box = (plo, phi)
+        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear(); self._graphs.clear()
 
     def participants(self, view_id, cam) -> int:
-        """GetParticipants(v) (L249): partitions whose box meets the view frustum; cached per view id."""
+        """GetParticipants(v) (L249): partitions whose boxes meet the view frustum; cached per view id."""
         if view_id not in self._participants:
-            state, part = binding.visible_regions(self._aabb[0], self._aabb[1], cam)
+            lo, hi, ms, bp = self._aabb
+            state, part = binding.visible_regions(lo, hi, cam, ms, bp, self.K, self.cfg)
             for k in range(self.K):                       # an empty partition never participates
                 if self.part_offsets[k + 1] == self.part_offsets[k]:
                     part &= ~(1 << k)
@@ -325,259 +288,186 @@ class Trainer:
         state = self._bucket_state[key]
         return self.make_plan(cams, vop, state, sparse), (state if saturation else None)
 
-    def iteration_views(self, view_ids, cams, targets, consolidate=True, saturation=True, sat_eps=1e-4, sparse=True):
-        """One training iteration over B views with visibility prediction: geometric participants and tile
-        regions, saturated tiles skipped from the previous visit of the same bucket on, conflict-free views
-        consolidated into one launch per stage.  targets: device tensor [B,H,W,3].  Returns the number of launches
-        of the forward (= buckets)."""
-        groups = self.buckets(view_ids, cams, consolidate)
-        if self.fuse_adam:
-            self.prepare_adam()
-        G = len(groups)
-        plans = [self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse) for grp in groups]
-        tgs = [targets[grp[0]:grp[0] + 1] if len(grp) == 1 else targets[torch.as_tensor(grp, device=targets.device)]
-               for grp in groups]
-        self._workspaces(cams[0])
-        if G == 1 or not self.pipeline_buckets:
-            for gi in range(G):
-                self.iteration_fused(plans[gi][0], tgs[gi], overwrite=(gi == 0), sat_eps=sat_eps, tile_state_out=plans[gi][1],
-                                     adam=(self.fuse_adam and gi == G - 1), n_views=len(view_ids))
-        else:
-            # Two streams, double-buffered projected / binning sets: bucket g+1 is projected and sorted (latency-bound
-            # kernels that leave most of the SMs idle) on the side stream while bucket g is blended on the main one.
-            dev = self.ctx.device
-            main = torch.cuda.current_stream(dev)
-            if getattr(self, "_front_stream", None) is None:
-                self._front_stream = torch.cuda.Stream(dev)
-            side = self._front_stream
-            ev_front = [torch.cuda.Event() for _ in range(G)]
-            ev_back = [torch.cuda.Event() for _ in range(G)]
-            side.wait_stream(main)                       # the parameters of the previous optimiser step
-            self.ctx.set_stream(side.cuda_stream)
-            self._front(plans[0][0], self._bufs(0))
-            ev_front[0].record(side)
-            self.ctx.set_stream(main.cuda_stream)
-            for gi in range(G):
-                if gi + 1 < G:
-                    if gi >= 1:
-                        side.wait_event(ev_back[gi - 1])  # buffer set (gi + 1) % 2 was last read by the back half of gi - 1
-                    self.ctx.set_stream(side.cuda_stream)
-                    self._front(plans[gi + 1][0], self._bufs((gi + 1) % 2))
-                    ev_front[gi + 1].record(side)
-                    self.ctx.set_stream(main.cuda_stream)
-                main.wait_event(ev_front[gi])
-                self._plan = plans[gi][0]
-                self._back(plans[gi][0], self._bufs(gi % 2), tgs[gi], gi == 0, sat_eps, plans[gi][1],
-                           self.fuse_adam and gi == G - 1, len(view_ids))
-                ev_back[gi].record(main)
-            side.wait_stream(main)
-        if self.sparse_adam:
+    # ---- one library call per iteration (splx_iteration) -------------------------------------------------------
+    def _frontset(self, which):
+        proj, bins, ws = (self.proj, self.bins, self._ws_sort) if which == 0 else self._alt
+        return binding.FrontsetS(proj.struct(), bins.struct(), ws.data_ptr(), ws.numel())
+
+    def _trainset(self, n_views, pipelined):
+        """splx_trainset over this trainer's buffers (allocating the ones the training path needs on first use)."""
+        dev = self.ctx.device
+        self._view_buffers(max(n_views, 1))
+        g_ct, g2d = self.fused_buffers()
+        if getattr(self, "_targets_dev", None) is None or self._targets_dev.shape[0] < self._images.shape[0]:
+            self._targets_dev = torch.empty_like(self._images)
+        if pipelined and self._alt is None:
+            self._alt = (binding.Projected(self.n, dev), binding.Binning(self.capacity, self.K, self.W, self.H, dev),
+                         torch.empty_like(self._ws_sort))
+        if self.lambda_dssim > 0 and getattr(self, "_dssim_ws", None) is None:
+            nf = self.ctx.dssim_ws_floats(self.W, self.H)
+            self._dssim_ws = torch.empty(binding.MAX_VIEWS * nf, dtype=torch.float32, device=dev)
+        if self.sparse_adam and self._touched is None:
+            self._touched = torch.zeros(max(self.n, 1), dtype=torch.uint8, device=dev)
+        ts = binding.TrainsetS()
+        ts.params = binding.gaussians_struct(self.params)
+        ts.grads = binding.gaussians_struct(self.grads)
+        ts.K = self.K
+        ts.part_offsets = C.cast(self._po, C.c_void_p)
+        ts.sh_degree = self.sh_degree
+        ts.bg[:] = [float(x) for x in self.bg]
+        ts.front[0] = self._frontset(0)
+        if pipelined:
+            ts.front[1] = self._frontset(1)
+        ts.partials = self.partials.struct()
+        ts.g_ct, ts.g2d = g_ct.data_ptr(), g2d.data_ptr()
+        ts.images, ts.T_totals, ts.g_images = self._images.data_ptr(), self._T_totals.data_ptr(), self._g_images.data_ptr()
+        ts.targets = self._targets_dev.data_ptr()
+        ts.dssim_ws = self._dssim_ws.data_ptr() if self.lambda_dssim > 0 else None
+        ts.loss_sum = self.loss_sum.data_ptr()
+        ts.max_views = self._images.shape[0]
+        ts.cross_mask = self._cross.data_ptr() if self._cross is not None else None
+        ts.touched = self._touched.data_ptr() if self.sparse_adam else None
+        return ts
+
+    def _adam_cfg(self, step):
+        offs = (C.c_int64 * 6)(*([self._offs[k] for k in PARAM_KEYS] + [self._total]))
+        lrs = (C.c_float * 5)(*[float(self.lr[k]) for k in PARAM_KEYS])
+        f = self.flat
+        a = binding.AdamCfgS(f["param"].data_ptr(), f["grad"].data_ptr(), f["m"].data_ptr(), f["v"].data_ptr(), 5,
+                             C.cast(offs, C.c_void_p), C.cast(lrs, C.c_void_p), 0.9, 0.999, 1e-15, int(step),
+                             binding.gaussians_struct(self.m), binding.gaussians_struct(self.v))
+        a._keep = (offs, lrs)
+        return a
+
+    def _bucket_structs(self, plans, groups):
+        """ctypes array of splx_bucket for the plans [(binding.Plan, state_out or None)] over the view positions `groups`."""
+        arr = (binding.BucketS * len(plans))()
+        keep = []
+        for i, ((plan, state_out), grp) in enumerate(zip(plans, groups)):
+            vi = (C.c_int32 * len(grp))(*[int(x) for x in grp])
+            zr = self._depth_ranges(plan) if self._cross is not None else None
+            arr[i].plan = plan._s
+            arr[i].view_index = C.cast(vi, C.c_void_p)
+            arr[i].tile_state_out = state_out.data_ptr() if state_out is not None else None
+            arr[i].part_depth_range = zr.ctypes.data if zr is not None else None
+            keep += [vi, zr, plan]
+        arr._keep = keep
+        return arr
+
+    def check_overflow(self, wait=False):
+        """Raise CapacityError if a bucket of the last iteration overflowed the key capacity (its count M comes back through
+        a pinned host mirror written by splx_iteration; read only once the device has passed that point)."""
+        if self._m_event is None:
+            return
+        if wait:
+            self._m_event.synchronize()
+        if self._m_event.query():
+            m = int(self._m_host[:self._m_buckets].max())
+            self._m_event = None
+            if m > self.capacity:
+                raise CapacityError(f"{m} tile intersections exceed the capacity {self.capacity}: the farthest keys were dropped")
+
+    def _run_iteration(self, plans, groups, n_views, targets, sat_eps, adam=True, host=False, images_out=None,
+                       loss_out=None):
+        """plans: [(Plan, state_out)], groups: view positions per plan; targets: list of raw pointers per view."""
+        if not torch.cuda.is_current_stream_capturing():
+            self.check_overflow()
+        self._workspaces(plans[0][0].cams[0])
+        pipelined = self.pipeline_buckets and len(plans) > 1
+        ts = self._trainset(n_views, pipelined)
+        bk = self._bucket_structs(plans, groups)
+        cfg = None
+        if adam:
             self.step_count += 1
-            self.ctx.adam_sparse(self.params, self.grads, self.m, self.v, self._touched, [self.lr[k] for k in PARAM_KEYS],
-                                 step=self.step_count, grad_scale=1.0 / len(view_ids))
-        elif not self.fuse_adam:
-            self.adam_step(len(view_ids))
+            cfg = self._adam_cfg(self.step_count)
+        self._plan = plans[-1][0]
+        self.ctx.iteration(ts, bk, n_views, targets, images_out, loss_out, self._m_host.data_ptr(), host=host,
+                           sat_eps=0.0 if sat_eps is None else sat_eps, lambda_dssim=self.lambda_dssim, adam=cfg)
+        self._m_buckets = len(plans)
+        return ts, bk
+
+    def iteration_fused(self, plan: binding.Plan, targets, overwrite=True, sat_eps=None, tile_state_out=None):
+        """a1-a10 of ONE bucket under a plan (no optimiser step).  targets: device [B,H,W,3].  Returns images[B,H,W,3]."""
+        assert overwrite, "a single bucket always stores its gradient"
+        B = plan.B
+        hw3 = self.H * self.W * 3 * 4
+        self._run_iteration([(plan, tile_state_out)], [list(range(B))], B, [targets.data_ptr() + b * hw3 for b in range(B)],
+                            sat_eps, adam=False)
+        return self._images[:B]
+
+    def iteration_views(self, view_ids, cams, targets, consolidate=True, saturation=True, sat_eps=1e-4, sparse=True,
+                        images_host=None, loss_host=None):
+        """One training iteration over B views with visibility prediction: geometric participants and tile regions,
+        saturated tiles skipped from the previous visit of the same bucket on, conflict-free views consolidated into one
+        launch per stage, then Adam -- all inside splx_iteration.  targets: device tensor [B,H,W,3], or a list of B
+        PINNED HOST tensors [H,W,3] (then images_host: list of pinned host tensors or None, loss_host: pinned double[2]
+        or None receive the results: the end-to-end path).  Returns the number of buckets."""
+        groups = self.buckets(view_ids, cams, consolidate)
+        plans = [self.bucket_plan([view_ids[i] for i in grp], [cams[i] for i in grp], saturation, sparse) for grp in groups]
+        B = len(view_ids)
+        host = not isinstance(targets, torch.Tensor)
+        if host:
+            tptr = [t.data_ptr() for t in targets]
+            iptr = [t.data_ptr() for t in images_host] if images_host is not None else None
+            lptr = loss_host.data_ptr() if loss_host is not None else None
+        else:
+            hw3 = self.H * self.W * 3 * 4
+            tptr, iptr, lptr = [targets.data_ptr() + b * hw3 for b in range(B)], None, None
+        self._run_iteration(plans, groups, B, tptr, sat_eps, adam=True, host=host, images_out=iptr, loss_out=lptr)
+        self._m_event = torch.cuda.Event()
+        self._m_event.record(torch.cuda.current_stream(self.ctx.device))
         return len(groups)
 
-    # ---- end to end from HOST buffers ---------------------------------------------------------------
-    def _host_body(self, main, side, plan, state, target_host, image_host, loss_host, sat_eps):
-        """a1-a10 with the host copies on the side stream: the target travels while the forward renders (it is
-        first needed by the loss), the image travels while the backward runs."""
-        side.wait_stream(main)
-        with torch.cuda.stream(side):
-            self._target_dev[0].copy_(target_host, non_blocking=True)
-            self._ev_target.record(side)
-        self.loss_sum.zero_()
-        self._workspaces(plan.cams[0])
-        self._plan = plan
-        c = self.ctx
-        images, T_totals, _ = self._view_buffers(1)
-        g_ct, g2d = self.fused_buffers()
-        c.project_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj)
-        self._bin_sort(self.proj, plan, self.bins, self._ws_sort)
-        c.render_partial_plan(self.proj, self.bins, plan, self.partials)
-        main.wait_event(self._ev_target)            # the target is first needed by the fused composition + loss
-        c.compose_l1_backward_plan(self.partials, self.bins, plan, self.bg, self._target_dev, images, T_totals,
-                                   self.loss_sum, g_ct, scale=1.0, sat_eps=sat_eps, tile_state_out=state)
-        if image_host is not None:
-            side.wait_stream(main)
-            with torch.cuda.stream(side):
-                image_host.copy_(images[0], non_blocking=True)
-        c.raster_backward_plan(self.proj, self.bins, plan, self.partials, g_ct, g2d)
-        if self.fuse_adam:
-            c.adam_bias_step(self._step_dev, self._bc_dev)
-            c.project_backward_adam_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                         self.m, self.v, [self.lr[k] for k in PARAM_KEYS], self._bc_dev, grad_scale=1.0,
-                                         clear_g2d=True, overwrite=True)
-        else:
-            c.project_backward_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, g2d, self.grads,
-                                    clear_g2d=True, overwrite=True)
-        main.wait_stream(side)
-        if loss_host is not None:    # after the image has left: the two copies share one device-to-host engine, and
-            loss_host.copy_(self.loss_sum, non_blocking=True)   # 8 bytes queued behind 25 MB would stall this stream
+    # ---- one view per iteration, replayed from a CUDA graph -----------------------------------------------------
+    def _single_view_plan(self, view_id, cam, saturation):
+        if self._aabb is not None:
+            return self.bucket_plan([view_id], [cam], saturation=saturation)
+        return self.make_plan([cam]), None
 
-    def step_host(self, view_id, cam, target_host, image_host=None, loss_host=None, saturation=False, sat_eps=1e-4,
-                  graph=True):
-        """One whole training iteration (a1-a11) on one view whose target image lives in pinned HOST memory; the
-        rendered image and the loss go back to pinned host memory.  With graph=True the launches of a1-a10 and the
-        copies are captured once per (view, buffers) into a CUDA graph and replayed (one launch per step instead of
-        ~20); the Adam step is fused into the projection backward, its bias corrections travel through a pinned
-        host pair that the graph's copy node reads at replay time.  Returns after the device has drained, so the host
-        buffers are valid."""
+    def _graph_step(self, key, plan, state, target_ptr, sat_eps, host, image_ptr, loss_ptr):
+        """a1-a10 of one view captured once into a CUDA graph and replayed (one launch per step instead of ~20), then Adam
+        outside the graph (its step number is a launch argument)."""
         dev = self.ctx.device
-        main = torch.cuda.current_stream(dev)
-        if self.fuse_adam:
-            self.prepare_adam()
-        if self._side is None:
-            self._side = torch.cuda.Stream(dev)
-        if getattr(self, "_graphs", None) is None:
-            self._ev_target = torch.cuda.Event()
-            self._target_dev = torch.empty((1, self.H, self.W, 3), dtype=torch.float32, device=dev)
-            self._graphs = {}
-        if not graph:
-            plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
-                           else (self.make_plan([cam]), None))
-            self._host_body(main, self._side, plan, state, target_host, image_host, loss_host, sat_eps)
-        else:
-            key = (view_id, target_host.data_ptr(), image_host.data_ptr() if image_host is not None else 0,
-                   loss_host.data_ptr() if loss_host is not None else 0, bool(saturation), float(sat_eps), self.fuse_adam)
-            if key not in self._graphs:
-                plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
-                               else (self.make_plan([cam]), None))
-                self._workspaces(cam)
-                self._view_buffers(1)
-                self.fused_buffers()
-                torch.cuda.synchronize(dev)
-                g = torch.cuda.CUDAGraph()
-                old = main.cuda_stream
-                with torch.cuda.graph(g):
-                    cap = torch.cuda.current_stream(dev)
-                    self.ctx.set_stream(cap.cuda_stream)
-                    try:
-                        self._host_body(cap, self._side, plan, state, target_host, image_host, loss_host, sat_eps)
-                    finally:
-                        self.ctx.set_stream(old)
-                self._graphs[key] = (g, plan)          # the plan owns the host arrays the capture read
-            self._graphs[key][0].replay()
-        if not self.fuse_adam:
-            self.adam_step(1)        # outside the graph: its bias correction is a launch argument
-        main.synchronize()
-
-    # ---- the same iteration, scheduled so that HBM-bound and latency-bound stages overlap ----------------------
-    def _adam_part(self, sh: bool, step: int, n_views=1):
-        """Adam (a11) on the SH group only, or on the four geometry groups (mean, log_scale, quat, opacity) only."""
-        o = self._offs
-        if sh:
-            a, b = o["sh"], self._total
-            offs, lrs = [0, b - a], [self.lr["sh"]]
-        else:
-            a, b = 0, o["sh"]
-            keys = [k for k in PARAM_KEYS if k != "sh"]
-            offs, lrs = [o[k] for k in keys] + [b], [self.lr[k] for k in keys]
-        f = self.flat
-        self.ctx.adam_groups(f["param"][a:b], f["grad"][a:b], f["m"][a:b], f["v"][a:b], offs, lrs, step=step,
-                             grad_scale=1.0 / n_views)
-
-    def step_overlapped(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
-        """step_graph with the same kernels and the same arithmetic on a different schedule.  Two facts are used:
-        the binning needs only the GEOMETRY half of the projection (which reads 11 of a Gaussian's 59 parameters),
-        and the SH colour is not needed before the blend.  So the Adam step of the SH group -- 81 % of the
-        optimiser's bytes, bound by HBM -- is deferred to a second stream where it runs, followed by the colour half
-        of the next iteration's projection, beside that iteration's geometry half and binning (a chain of small,
-        latency-bound kernels that leaves the memory system idle).  Parameters are complete only after flush()."""
-        assert not self.fuse_adam and not self.sparse_adam
-        dev = self.ctx.device
-        c = self.ctx
-        main = torch.cuda.current_stream(dev)
-        if self._side is None:
-            self._side = torch.cuda.Stream(dev)
-        side = self._side
-        if getattr(self, "_ographs", None) is None:
-            self._ographs = {}
-            self._pending_sh = 0          # step number whose SH half of Adam has not run yet (0 = none)
-            self._ev = [torch.cuda.Event() for _ in range(3)]
-        key = (view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps))
-        if key not in self._ographs:
-            plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
-                           else (self.make_plan([cam]), None))
-            self._workspaces(cam)
-            self._view_buffers(1)
-            self.fused_buffers()
-            bufs = self._bufs(0)
-            torch.cuda.synchronize(dev)
-            graphs = []
-            for body in (lambda: self._bin_sort(self.proj, plan, self.bins, self._ws_sort),
-                         lambda: (self.loss_sum.zero_(), self._back(plan, bufs, target_dev, True, sat_eps, state, False, 1))):
-                g = torch.cuda.CUDAGraph()
-                with torch.cuda.graph(g):
-                    c.set_stream(torch.cuda.current_stream(dev).cuda_stream)
-                    try:
-                        body()
-                    finally:
-                        c.set_stream(main.cuda_stream)
-                graphs.append(g)
-            self._ographs[key] = (graphs[0], graphs[1], plan)
-        g_sort, g_back, plan = self._ographs[key]
-        self._plan = plan
-        ev_bwd, ev_geom, ev_col = self._ev
-        # main: geometry half (its parameters are final: the geometry groups were stepped on this stream)
-        c.project_parts_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, binding.PROJECT_GEOMETRY)
-        ev_geom.record(main)
-        # side: SH half of the previous step's Adam (after that step's backward), then the colour half
-        c.set_stream(side.cuda_stream)
-        try:
-            if self._pending_sh:
-                side.wait_event(ev_bwd)
-                self._adam_part(True, self._pending_sh)
-                self._pending_sh = 0
-            side.wait_event(ev_geom)
-            c.project_parts_plan(self.params, self.part_offsets, plan, self.sh_degree, self.proj, binding.PROJECT_COLOUR)
-            ev_col.record(side)
-        finally:
-            c.set_stream(main.cuda_stream)
-        g_sort.replay()                     # a2-a4 beside the side stream's work
-        main.wait_event(ev_col)
-        g_back.replay()                     # a5-a10
-        ev_bwd.record(main)
-        self.step_count += 1
-        self._adam_part(False, self.step_count)
-        self._pending_sh = self.step_count
-
-    def flush(self):
-        """Run what step_overlapped deferred: afterwards every parameter has taken every step."""
-        if getattr(self, "_pending_sh", 0):
-            main = torch.cuda.current_stream(self.ctx.device)
-            main.wait_event(self._ev[0])
-            self._adam_part(True, self._pending_sh)
-            self._pending_sh = 0
-
-    def step_graph(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
-        """One whole training iteration on one view with the target already on the device ([1,H,W,3]): a1-a10
-        replayed from a CUDA graph captured at the first call for this (view, target), then Adam.  Asynchronous."""
-        dev = self.ctx.device
-        if self.fuse_adam:
-            self.prepare_adam()           # this step's bias corrections (the captured copy node reads them at replay)
-        if getattr(self, "_dgraphs", None) is None:
-            self._dgraphs = {}
-        key = (view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps), self.fuse_adam)
-        if key not in self._dgraphs:
-            plan, state = (self.bucket_plan([view_id], [cam], saturation=saturation) if self._aabb is not None
-                           else (self.make_plan([cam]), None))
-            self._workspaces(cam)
-            self._view_buffers(1)
-            self.fused_buffers()
+        if key not in self._graphs:
             main = torch.cuda.current_stream(dev)
+            self._workspaces(plan.cams[0])
+            self._trainset(1, False)
             torch.cuda.synchronize(dev)
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g):
                 self.ctx.set_stream(torch.cuda.current_stream(dev).cuda_stream)
                 try:
-                    self.loss_sum.zero_()
-                    self.iteration_fused(plan, target_dev, overwrite=True, sat_eps=sat_eps, tile_state_out=state,
-                                         adam=self.fuse_adam)
+                    keep = self._run_iteration([(plan, state)], [[0]], 1, [target_ptr], sat_eps, adam=False, host=host,
+                                               images_out=[image_ptr] if image_ptr else None, loss_out=loss_ptr)
                 finally:
                     self.ctx.set_stream(main.cuda_stream)
-            self._dgraphs[key] = (g, plan)
-        self._dgraphs[key][0].replay()
-        if not self.fuse_adam:
-            self.adam_step(1)            # outside the graph: its bias correction is a launch argument
+            self._graphs[key] = (g, plan, keep)
+        self._graphs[key][0].replay()
+        self.adam_step(1)
+
+    def step_graph(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
+        """One whole training iteration on one view with the target already on the device ([1,H,W,3]).  Asynchronous."""
+        key = ("dev", view_id, target_dev.data_ptr(), bool(saturation), float(sat_eps), self.lambda_dssim)
+        plan, state = (None, None) if key in self._graphs else self._single_view_plan(view_id, cam, saturation)
+        self._graph_step(key, plan, state, target_dev.data_ptr(), sat_eps, False, None, None)
+
+    def step_host(self, view_id, cam, target_host, image_host=None, loss_host=None, saturation=False, sat_eps=1e-4,
+                  graph=True):
+        """One whole training iteration (a1-a11) on one view whose target image lives in PINNED HOST memory; the rendered
+        image and the loss sums (double[2]) go back to pinned host memory.  The copies run inside splx_iteration on the
+        library's own streams beside the kernels.  Returns after the device has drained: the host buffers are valid."""
+        dev = self.ctx.device
+        iptr = image_host.data_ptr() if image_host is not None else None
+        lptr = loss_host.data_ptr() if loss_host is not None else None
+        if graph:
+            key = ("host", view_id, target_host.data_ptr(), iptr, lptr, bool(saturation), float(sat_eps), self.lambda_dssim)
+            plan, state = (None, None) if key in self._graphs else self._single_view_plan(view_id, cam, saturation)
+            self._graph_step(key, plan, state, target_host.data_ptr(), sat_eps, True, iptr, lptr)
+        else:
+            plan, state = self._single_view_plan(view_id, cam, saturation)
+            self._run_iteration([(plan, state)], [[0]], 1, [target_host.data_ptr()], sat_eps, adam=True, host=True,
+                                images_out=[iptr] if iptr else None, loss_out=lptr)
+        torch.cuda.current_stream(dev).synchronize()
+        m = int(self._m_host[0])
+        if m > self.capacity:
+            raise CapacityError(f"{m} tile intersections exceed the capacity {self.capacity}: the farthest keys were dropped")

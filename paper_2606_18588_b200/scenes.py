@@ -185,6 +185,73 @@ def partition_aabbs(params, part_offsets, inflate_sigma=3.0):
     return lo, hi
 
 
+def partition_max_scale(params, part_offsets):
+    """Largest scale exp(log_scale) of every partition (0 for an empty one), rounded up to float32."""
+    return partition_boxes(params, part_offsets, sub=1)[2]
+
+
+def partition_boxes(params, part_offsets, sub=1):
+    """(lo, hi, max_scale, box_part): a cover of every partition by boxes of MEANS -- the static input of the CONSERVATIVE
+    geometric visibility prediction (Trainer.set_aabbs, splx_footprint_margin; reading s21).  sub = 1: one box per
+    partition, the bounding box of its Gaussians' means.  sub > 1: that box is cut into sub x sub equal cells in xy and
+    every non-empty cell gives the bounding box of the means inside it, so that a far corner of a large partition no
+    longer decides the margin of all of it, and one outlier in scale only widens its own cell.  max_scale[j]: the
+    largest scale exp(log_scale) among the Gaussians of box j (rounded up to float32); box_part[j]: its partition.
+    Boxes are rounded outward to a float32-exact grid.  No arithmetic of the method: input statistics only."""
+    K = len(part_offsets) - 1
+    los, his, mss, bps = [], [], [], []
+    on_device = not isinstance(params["mean"], np.ndarray)
+    for k in range(K):
+        a, b = int(part_offsets[k]), int(part_offsets[k + 1])
+        if b <= a:
+            if sub == 1:       # keep one (degenerate) box per partition so that box index == partition index
+                los.append(np.zeros(3)); his.append(np.zeros(3)); mss.append(0.0); bps.append(k)
+            continue
+        if on_device:
+            import torch
+            m = params["mean"].reshape(-1, 3)[a:b]
+            s = params["log_scale"].reshape(-1, 3)[a:b].max(1).values
+            lo_k, hi_k = m.min(0).values, m.max(0).values
+            if sub == 1:
+                cell = torch.zeros(b - a, dtype=torch.int64, device=m.device)
+            else:
+                ext = torch.clamp(hi_k - lo_k, min=1e-6)
+                ix = torch.clamp(((m[:, 0] - lo_k[0]) / ext[0] * sub).long(), 0, sub - 1)
+                iy = torch.clamp(((m[:, 1] - lo_k[1]) / ext[1] * sub).long(), 0, sub - 1)
+                cell = iy * sub + ix
+            nc = sub * sub
+            big = torch.finfo(torch.float32).max
+            clo = torch.full((nc, 3), big, device=m.device).scatter_reduce(0, cell[:, None].expand(-1, 3), m, "amin")
+            chi = torch.full((nc, 3), -big, device=m.device).scatter_reduce(0, cell[:, None].expand(-1, 3), m, "amax")
+            cms = torch.full((nc,), -big, device=m.device).scatter_reduce(0, cell, s, "amax")
+            cnt = torch.bincount(cell, minlength=nc).cpu().numpy()
+            clo, chi, cms = clo.double().cpu().numpy(), chi.double().cpu().numpy(), cms.double().cpu().numpy()
+        else:
+            m = params["mean"][a:b].astype(np.float64)
+            s = params["log_scale"][a:b].astype(np.float64).max(1)
+            lo_k, hi_k = m.min(0), m.max(0)
+            if sub == 1:
+                cell = np.zeros(b - a, np.int64)
+            else:
+                ext = np.maximum(hi_k - lo_k, 1e-6)
+                ix = np.clip(((m[:, 0] - lo_k[0]) / ext[0] * sub).astype(np.int64), 0, sub - 1)
+                iy = np.clip(((m[:, 1] - lo_k[1]) / ext[1] * sub).astype(np.int64), 0, sub - 1)
+                cell = iy * sub + ix
+            nc = sub * sub
+            cnt = np.bincount(cell, minlength=nc)
+            clo = np.full((nc, 3), np.inf); chi = np.full((nc, 3), -np.inf); cms = np.full(nc, -np.inf)
+            np.minimum.at(clo, cell, m); np.maximum.at(chi, cell, m); np.maximum.at(cms, cell, s)
+        for c in range(nc):
+            if cnt[c] == 0:
+                continue
+            los.append(np.floor(clo[c] * 1024) / 1024)        # outward rounding to a float32-exact grid
+            his.append(np.ceil(chi[c] * 1024) / 1024)
+            mss.append(float(np.nextafter(np.float32(np.exp(np.float64(cms[c]))), np.float32(np.inf))))
+            bps.append(k)
+    return (np.asarray(los, np.float32).reshape(-1, 3), np.asarray(his, np.float32).reshape(-1, 3),
+            np.asarray(mss, np.float32), np.asarray(bps, np.int32))
+
+
 def tiny(seed=0, n=4096, size=128, f=150.0, K=2, sh_degree=0):
     """BASELINE.json configs[0]: world frame = camera frame, K contiguous depth chunks."""
     rng = np.random.default_rng(seed)

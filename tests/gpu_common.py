@@ -27,7 +27,7 @@ def u64(t):
     return t.detach().cpu().numpy().view(np.uint64)
 
 
-def make_trainer(sc: scenes.Scene, cfg=None, capacity=None) -> Trainer:
+def make_trainer(sc: scenes.Scene, cfg=None, capacity=None, **kw) -> Trainer:
     cam = sc.cameras[0]
     return Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=capacity, cfg=cfg)
 

@@ -49,6 +49,50 @@ def test_struct_sizes_match_the_header(libpath):
     assert ctypes.sizeof(b.BinningS) == 48 and ctypes.sizeof(b.PartialS) == 24
 
 
+def test_iteration_structs_have_the_header_layout(tmp_path):
+    """The ctypes mirrors of the splx_iteration structs against the C compiler's own layout of include/splx.h."""
+    import subprocess
+    from paper_2606_18588_b200 import binding as b
+    src = tmp_path / "layout.c"
+    src.write_text("""
+#include <stdio.h>
+#include <stddef.h>
+#include "splx.h"
+int main(void) {
+  printf("%zu %zu %zu %zu %zu %zu ", sizeof(splx_frontset), sizeof(splx_trainset), sizeof(splx_bucket), sizeof(splx_adam_cfg),
+         sizeof(splx_iter_opts), sizeof(splx_plan));
+  printf("%zu %zu %zu %zu %zu %zu %zu\\n", offsetof(splx_trainset, part_offsets), offsetof(splx_trainset, bg),
+         offsetof(splx_trainset, front), offsetof(splx_trainset, partials), offsetof(splx_trainset, loss_sum),
+         offsetof(splx_trainset, touched), offsetof(splx_adam_cfg, m_soa));
+  return 0;
+}""")
+    exe = tmp_path / "layout"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    got = [int(x) for x in subprocess.check_output([str(exe)]).split()]
+    T, A = b.TrainsetS, b.AdamCfgS
+    want = [ctypes.sizeof(b.FrontsetS), ctypes.sizeof(T), ctypes.sizeof(b.BucketS), ctypes.sizeof(A),
+            ctypes.sizeof(b.IterOptsS), ctypes.sizeof(b.PlanS), T.part_offsets.offset, T.bg.offset, T.front.offset,
+            T.partials.offset, T.loss_sum.offset, T.touched.offset, A.m_soa.offset]
+    assert got == want
+
+
+def test_cameras_with_a_bad_near_plane_are_rejected(libpath):
+    """near_z <= 0 would admit z ~ 0 into 1/z and break the unsigned ordering of float_bits(depth); non-finite
+    intrinsics likewise.  The host-only entry points can be called without a GPU."""
+    import numpy as np
+    from paper_2606_18588_b200 import binding as b, scenes
+    lo = np.array([[-1, -1, 4]], np.float32); hi = np.array([[1, 1, 6]], np.float32)
+    cam = scenes.Camera(np.eye(3, dtype=np.float32), np.zeros(3, np.float32), 50.0, 50.0, 16.0, 16.0, 32, 32)
+    state, part = b.visible_regions(lo, hi, cam)
+    assert part == 1
+    for bad in (0.0, -0.5):
+        cam.near_z = bad
+        with pytest.raises(b.SplxError):
+            b.visible_regions(lo, hi, cam)
+        with pytest.raises(b.SplxError):
+            b.visible_regions(lo, hi, cam, np.ones(1, np.float32))
+
+
 def test_no_cpu_fallback_without_a_device(libpath):
     import torch
     if torch.cuda.is_available():
@@ -74,7 +118,7 @@ def test_product_package_never_touches_the_oracle():
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
                 assert "liboracle" not in txt and "splx_oracle" not in txt, f
     for f in os.listdir(os.path.join(ROOT, "oracle")):
-        if f.endswith((".py", ".cpp")):
+        if f.endswith((".py", ".cpp", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_2606_18588_b200\b", txt, flags=re.M), f
             assert "libsplx" not in txt

@@ -151,7 +151,7 @@ def full_city(request):
         cap = 160_000_000
     cam = sc.cameras[0]
     tr = Trainer(sc.params, sc.part_offsets, cam.width, cam.height, sc.sh_degree, sc.bg, capacity=cap)
-    tr.set_aabbs(*scenes.partition_aabbs(sc.params, sc.part_offsets))
+    tr.set_aabbs(*scenes.partition_boxes(sc.params, sc.part_offsets, sub=8))     # sub-cell boxes of means + footprint margin (s21)
     sc.params = None                             # the tests read the trainer's copy (_partition_host)
     torch.cuda.empty_cache()
     plan, _ = tr.bucket_plan([0], [cam], saturation=False, sparse=True)
@@ -188,11 +188,14 @@ def _projected_slice(tr, a, b):
 def test_city_binning_bit_exact(full_city):
     sc, cam, tr, plan = full_city
     vop = plan.view_of_part
-    assert 0 < sum(v == 0 for v in vop) < sc.K, "the view must see some, not all, partitions"
+    n_part = sum(v == 0 for v in vop)
+    assert 0 < n_part <= sc.K
+    if sc.K >= 16:
+        assert n_part <= sc.K // 2, "at K >= 16 the geometric prediction must drop most partitions of a view"
     state = G.np32(plan.tile_state).reshape(sc.K, -1)
     M, keys, vals, ranges = G.gpu_bins(tr)
     ntiles = ranges.shape[1]
-    pos = n_cut = n_live = 0
+    pos = n_live = 0
     for k in range(tr.K):
         a, b = int(tr.part_offsets[k]), int(tr.part_offsets[k + 1])
         if vop[k] < 0:
@@ -204,20 +207,20 @@ def test_city_binning_bit_exact(full_city):
         ob = oracle.bin_sort(pk.means2d, pk.radius, pk.depth, cam.width, cam.height)
         assert np.array_equal(keys[pos:pos + ob.M], ob.keys + (np.uint64(k * ntiles) << np.uint64(32)))
         assert np.array_equal(vals[pos:pos + ob.M], ob.vals + np.uint32(a))
-        want = ob.ranges.copy(); want[state[k] != 0] = 0       # skipped slots lose their list
+        # the oracle knows NOTHING of the geometric tile state: with conservative regions (reading s21) a slot marked
+        # invisible has an empty list, so the GPU's ranges equal the unrestricted binning
+        want = ob.ranges
         live = want[:, 1] > want[:, 0]
         assert np.array_equal(ranges[k][live], want[live] + np.uint32(pos))
         assert not ranges[k][~live].any()
-        # the boxes hold every 3-sigma support in 3-D; the 2-D footprint (dilated, rounded up to whole pixels, a square
-        # around the ellipse) can still reach a tile the projected box does not: such a slot loses its list (s28, the
-        # oracle's `want` above does the same).  None at 1080p; a handful of border tiles at 4K.
-        ob_live = ob.ranges[:, 1] > ob.ranges[:, 0]
-        n_cut += int((ob_live & ~live).sum()); n_live += int(ob_live.sum())
+        assert not (live & (state[k] != 0)).any()
+        n_live += int(live.sum())
         pos += ob.M
-    assert pos == M and M > 2_000_000
-    assert n_cut <= 2e-3 * n_live, (n_cut, n_live)
-    if tr.n == 10_000_000:
-        assert n_cut == 0
+    assert pos == M and M > 2_000_000 and n_live > 0
+    assert int(tr.bins.num_intersections[1].item()) == 0       # device counter: no non-empty list dropped as invisible
+    # ... and the prediction still does its job: most slots of the participants are marked invisible without a look
+    part_slots = sum(state[k].size for k in range(tr.K) if vop[k] == 0)
+    assert sum(int((state[k] != 0).sum()) for k in range(tr.K) if vop[k] == 0) > 0.2 * part_slots
 
 
 def test_city_pixels_and_gradients_on_sampled_tiles(full_city):

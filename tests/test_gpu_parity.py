@@ -57,7 +57,7 @@ class Run:
         tr.loss_sum.zero_()
         c.l1_loss_grad(tr.image, self.target, tr.g_image, tr.loss_sum)
         self.g_image = G.np32(tr.g_image).astype(np.float64)
-        self.loss = float(tr.loss_sum.item()) / self.g_image.size
+        self.loss = float(tr.loss_sum[0].item()) / self.g_image.size
         torch.cuda.synchronize()
 
 
@@ -97,6 +97,9 @@ def test_a1_projection(run):
     ulp_img = 4 * 2.0 ** -23 * max(run.W, run.H)
     assert (G.close(pr.means2d[m], ref.means2d[m]) | (np.abs(pr.means2d[m] - ref.means2d[m]) <= ulp_img)).all()
     assert G.close(pr.depth[m], ref.depth[m]).all()
+    # the depth is the sort key: both sides evaluate it in fp32 in one fixed operation order (reading s12) -- bit-equal
+    dk = oracle.depth_key(sc.params["mean"], run.camv)
+    assert np.array_equal(pr.depth[m].astype(np.float32).view(np.uint32), dk[m].astype(np.float32).view(np.uint32))
     assert G.close(pr.rgb[m], ref.rgb[m]).all()
     assert G.close(pr.conic_opacity[m, 3], ref.conic_opacity[m, 3]).all()
     # conic = Sigma2D^-1: relative error amplified by the conditioning a*c/det of the 2x2 inverse

@@ -170,3 +170,31 @@ def test_tile_list_restricts_work():
         sl = (slice(16 * ty, 16 * ty + 16), slice(16 * tx, 16 * tx + 16))
         assert np.array_equal(full.image[sl], sub.image[sl])
     assert not sub.image[0:16, 0:16].any()
+
+
+def test_depth_key_is_the_fp32_depth_in_a_fixed_operation_order():
+    """Reading s12: the sort key holds float_bits(depth), an integer decision taken in fp32.  oracle.depth_key is that
+    fp32 value -- exactly representable, within one fp32 rounding of the fp64 depth of the projection, equal to the
+    exactly rounded depth wherever that is unambiguous -- and the free-running oracle orders by it."""
+    import oracle
+    from .common import random_scene
+    rng = np.random.default_rng(11)
+    p, cam = random_scene(rng, 400, size=48, f=60.0, sh_degree=0)
+    p = {k: v.astype(np.float32).astype(np.float64) for k, v in p.items()}
+    camv = cam.as_array()
+    dk = oracle.depth_key(p["mean"], camv)
+    assert np.array_equal(dk, dk.astype(np.float32).astype(np.float64))           # fp32 numbers
+    pr = oracle.project(p["mean"], p["log_scale"], p["quat"], p["opacity_logit"], p["sh"], 0, camv)
+    vis = pr.radius > 0
+    ulp = np.spacing(np.abs(pr.depth[vis]).astype(np.float32)).astype(np.float64)
+    assert (np.abs(dk[vis] - pr.depth[vis]) <= 1.5 * ulp).all()                   # three roundings, mostly cancelling
+    assert (dk[vis] == pr.depth[vis].astype(np.float32)).mean() > 0.5             # usually THE correctly rounded depth
+    # the driver sorts by it: every tile list is ordered by (bits(depth_key), index)
+    res = oracle.forward([p], camv, 0)
+    b = res.bins[0]
+    bits = dk.astype(np.float32).view(np.uint32).astype(np.uint64)
+    assert np.array_equal(b.keys & np.uint64(0xFFFFFFFF), bits[b.vals])
+    for t in range(b.ranges.shape[0]):
+        a, e = b.ranges[t]
+        k = list(zip(bits[b.vals[a:e]].tolist(), b.vals[a:e].tolist()))
+        assert k == sorted(k)

@@ -66,6 +66,18 @@ def test_library_host_geometry_equals_the_lp_oracle():
         assert part == part_ref
 
 
+def test_participants_is_the_union_of_the_tile_regions():
+    """ov.participants (one LP per box over the whole image) == 'some tile of visible_regions is visible', for the plain
+    and for the conservative regions, and == the library's host geometry."""
+    for yaw, pitch in ((30.0, 40.0), (200.0, 25.0)):
+        cam = _cam(yaw=yaw, pitch=pitch)
+        c64 = cam.as_array()
+        for ms in (None, np.array([0.0, 0.1, 0.5, 2.0, 30.0, 0.2])):
+            state, part_ref, _ = ov.visible_regions(BOXES_LO, BOXES_HI, c64, max_scale=ms)
+            assert ov.participants(BOXES_LO, BOXES_HI, c64, ms) == part_ref
+            assert binding.visible_regions(BOXES_LO, BOXES_HI, cam, ms)[1] == part_ref
+
+
 def test_schedule_views_is_greedy_and_conflict_free():
     rng = np.random.default_rng(3)
     for trial in range(20):
@@ -217,3 +229,102 @@ def test_adam_rows_is_adam_on_the_selected_rows():
     t.grad = torch.tensor(g[rows]); opt.step()
     assert np.allclose(p[rows], t.detach().numpy(), rtol=1e-12, atol=1e-14)
     assert np.array_equal(p[~rows], p0[~rows]) and not m[~rows].any()
+
+
+def _margin_scene(seed, n=1500):
+    """Gaussians in a 24 x 24 x 6 m slab cut into 2 x 2 cells, scales up to ~1.5 m, seen by a low oblique camera:
+    big footprints, many of them cut by the image border."""
+    rng = np.random.default_rng(seed)
+    mean = np.stack([rng.uniform(-12, 12, n), rng.uniform(-12, 12, n), rng.uniform(0, 6, n)], 1).astype(np.float32)
+    p = dict(mean=mean, log_scale=rng.normal(-1.2, 0.7, (n, 3)).astype(np.float32),
+             quat=rng.standard_normal((n, 4)).astype(np.float32), opacity_logit=rng.normal(0, 1, n).astype(np.float32),
+             sh=np.zeros((n, 16, 3), np.float32))
+    pid = scenes.grid_partition(mean, (-12, -12), (12, 12), 2, 2)
+    params, offs = scenes._order_by_partition(p, pid, 4)
+    cam = scenes.aerial_camera(160, 96, 70.0, 9.0, 28.0, 35.0 + 90 * seed, (2.0, -1.0, 0.0))
+    return params, offs, cam
+
+
+def test_footprint_radius_bound_of_reading_s21():
+    """The inequality the conservative regions rest on, against the projection oracle's own radii, Gaussian by Gaussian:
+    radius <= 3 c s / z + 3 sqrt(e) + 1 with c^2 = max(fx, fy)^2 (1 + limx^2 + limy^2), e = dilation + sqrt(floor),
+    s the Gaussian's largest scale, z its camera depth -- and it is not loose by more than the clamp factor."""
+    worst = 0.0
+    for seed in range(3):
+        params, offs, cam = _margin_scene(seed)
+        c64 = cam.as_array()
+        pr = oracle.project(params["mean"], params["log_scale"], params["quat"], params["opacity_logit"], params["sh"], 0, c64)
+        vis = pr.radius > 0
+        assert vis.sum() > 200
+        dil, limf, rfl = oracle.DEFAULT_CFG[3:6]
+        limx, limy = limf * cam.width / (2 * cam.fx), limf * cam.height / (2 * cam.fy)
+        c = max(cam.fx, cam.fy) * np.sqrt(1 + limx ** 2 + limy ** 2)
+        e = dil + np.sqrt(rfl)
+        smax = np.exp(params["log_scale"].astype(np.float64).max(1))
+        bound = 3 * c * smax[vis] / pr.depth[vis] + 3 * np.sqrt(e) + 1
+        assert (pr.radius[vis] <= bound).all()
+        worst = max(worst, float((pr.radius[vis] / bound).max()))
+    assert worst > 0.5          # tight within the factor sqrt(1 + limx^2 + limy^2) of the J clamp
+
+
+def test_conservative_regions_never_drop_a_list():
+    """Boxes of means + max_scale (reading s21): a (partition, tile) slot marked invisible has an EMPTY list in the
+    oracle's binning, and a non-participant has no visible Gaussian -- for the LP oracle and for the library's host
+    geometry alike, with one box per partition and with sub-cells (which mark MORE slots invisible, still without
+    cutting a list)."""
+    for seed in range(3):
+        params, offs, cam = _margin_scene(seed)
+        c64 = cam.as_array()
+        bins = []
+        for k in range(4):
+            a, b = int(offs[k]), int(offs[k + 1])
+            pr = oracle.project(params["mean"][a:b], params["log_scale"][a:b], params["quat"][a:b],
+                                params["opacity_logit"][a:b], params["sh"][a:b], 0, c64)
+            bins.append(oracle.bin_sort(pr.means2d, pr.radius, pr.depth, cam.width, cam.height))
+        n_inv = {}
+        for sub in (1, 3):
+            lo, hi, ms, bp = scenes.partition_boxes(params, offs, sub=sub)
+            assert set(bp.tolist()) == {0, 1, 2, 3}
+            m = params["mean"]
+            for j in range(len(bp)):         # max_scale[j] really bounds the Gaussians of box j
+                a, b = int(offs[bp[j]]), int(offs[bp[j] + 1])
+                inside = ((m[a:b] >= lo[j]) & (m[a:b] <= hi[j])).all(1)
+                assert inside.any() and np.exp(params["log_scale"][a:b][inside].max()) <= ms[j]
+            got, part = binding.visible_regions(lo, hi, cam, ms, bp, 4)
+            per_box, _, slack = ov.visible_regions(lo, hi, c64, max_scale=ms)
+            ref = ov.union_regions(per_box, bp, 4)
+            # a tile is decided robustly if every box of the partition is decided robustly on it
+            robust = np.ones_like(ref, bool)
+            for j, k in enumerate(bp):
+                robust[k] &= np.abs(slack[j]) > 1e-6
+            assert robust.mean() > 0.97
+            assert np.array_equal(got[robust], ref[robust])
+            assert part == sum(1 << k for k in range(4) if (ref[k] == 0).any())
+            for k in range(4):
+                live = bins[k].ranges[:, 1] > bins[k].ranges[:, 0]
+                for st in (got[k], ref[k]):
+                    assert not (live & (st == ov.TILE_INVISIBLE)).any(), (seed, sub, k)
+                if not (part >> k) & 1:
+                    assert bins[k].M == 0
+            n_inv[sub] = int((got == ov.TILE_INVISIBLE).sum())
+        assert n_inv[3] >= n_inv[1]
+        # ... while the plain boxes of the means (L212 as printed) do cut lists: the reason for the reading
+        lo, hi, ms, bp = scenes.partition_boxes(params, offs)
+        bare, _ = binding.visible_regions(lo, hi, cam)
+        cut = sum(int(((bins[k].ranges[:, 1] > bins[k].ranges[:, 0]) & (bare[k] == ov.TILE_INVISIBLE)).sum()) for k in range(4))
+        assert cut > 0
+
+
+def test_conservative_region_of_a_box_behind_or_beside_the_camera_is_empty():
+    """A box that straddles the camera plane far to the side, or lies wholly behind it, cannot reach the image however
+    the near plane cuts it: the reach half spaces remove it (without them z_min = near would blow the margin up)."""
+    cam = _cam(width=160, height=96, pitch=45.0, alt=200.0, target=(0.0, 0.0, 0.0))
+    o = -cam.R.T.astype(np.float64) @ cam.t.astype(np.float64)
+    right, fwd = cam.R[0].astype(np.float64), cam.R[2].astype(np.float64)
+    centres = [o + 400.0 * right, o - 300.0 * fwd, o + 300.0 * fwd]          # beside (straddling z = 0), behind, in front
+    lo = np.array([c - 60.0 for c in centres], np.float32); hi = np.array([c + 60.0 for c in centres], np.float32)
+    ms = np.array([3.0, 3.0, 3.0], np.float32)
+    got, part = binding.visible_regions(lo, hi, cam, ms)
+    _, part_ref, _ = ov.visible_regions(lo, hi, cam.as_array(), max_scale=ms, whole_image=True)
+    assert part == part_ref == 0b100
+    assert (got[0] == ov.TILE_INVISIBLE).all() and (got[1] == ov.TILE_INVISIBLE).all() and (got[2] == 0).any()
