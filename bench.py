@@ -380,6 +380,7 @@ def run_ours(args):
     sc.params = None                                   # a device-generated scene: release the generator's copy
     torch.cuda.empty_cache()
     tr.sparse_adam = bool(args.sparse_adam)
+    tr.flagged_grads = not args.plain_grads
     tr.lambda_dssim = float(args.lambda_dssim)
     if args.no_visibility:   # boxes that contain everything: every partition participates in every view, no tile is invisible
         big = np.float32(1e6)
@@ -457,6 +458,8 @@ def run_ours(args):
     def staged_iteration(ev):
         """The calls of splx_iteration issued one by one (buckets in order, no pipelining), an event before every stage."""
         po = tr.part_offsets
+        if flags:
+            tr._touched.zero_()       # (splx_iteration clears the flags with a cudaMemsetAsync)
         for gi, ((plan, state), grp) in enumerate(zip(plans, groups)):
             nb = len(grp)
             tg = targets[grp[0]:grp[0] + 1] if nb == 1 else targets[torch.as_tensor(grp, device="cuda")]
@@ -474,23 +477,18 @@ def run_ours(args):
                                            g_ct, scale=float(nb), sat_eps=args.sat_eps, tile_state_out=state)
             e[4].record(); c.raster_backward_plan(tr.proj, tr.bins, plan, tr.partials, g_ct, g2d)
             e[5].record()
-            if gi == 0 and not tr.sparse_adam:
+            if gi == 0 and not flags:
                 c.project_backward_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True, overwrite=True)
             else:
                 lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
                 c.project_backward_list_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, lst, cnt,
-                                             clear_g2d=True, touched=tr._touched if tr.sparse_adam else None)
+                                             clear_g2d=True, touched=tr._touched if flags else None)
             e[6].record()
-        if tr.sparse_adam:
-            tr.step_count += 1
-            c.adam_sparse(tr.params, tr.grads, tr.m, tr.v, tr._touched, [tr.lr[k] for k in scenes.PARAM_KEYS],
-                          step=tr.step_count, grad_scale=1.0 / B)
-        else:
-            tr.adam_step(B)
+        tr.adam_step(B, flagged=flags)
         ev[-1][7].record()
 
-    if tr.lambda_dssim > 0 or tr.sparse_adam:
-        tr._trainset(B, False)        # allocates the D-SSIM workspace / the touched flags
+    flags = tr._use_flags(plans[0][0])
+    tr._trainset(B, False, flags)     # allocates the D-SSIM workspace / the touched flags
     n_staged = max(3, min(args.steps, 10))
     restore()
     for _ in range(2):
@@ -571,14 +569,15 @@ def run_ours(args):
     fp32_nominal = SM_COUNT * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
     n_slot_pass = (max(1, (K * ntiles).bit_length()) + 7) // 8
     nv, npart, M = counts["visible"], counts["participating"], counts["intersections"]
-    first_overwrite = not tr.sparse_adam
+    first_overwrite = not flags
     vis0 = nv / max(len(plans), 1)                     # visible Gaussians of an average bucket
     hbm_bytes = dict(
         project=nv * 285 + (npart - nv) * 93,
         bin_sort=4 * npart + 12 * nv + 4 * 16 * nv + 4 * nv + (12 + 24 * n_slot_pass + 8) * M + 8 * K * ntiles * len(plans),
         compose=(20 + 16) * 256 * counts["live_slots"] + (12 + 12 + 4) * W * H * B,
         project_backward=(236 * tr.n + 272 * vis0 + 740 * (nv - vis0)) if first_overwrite else 740 * nv,
-        adam=28 * 59 * tr.n)
+        # flagged gradient rows: 24 B per parameter (param, m, v read + written) + the gradient of the touched rows only
+        adam=(24 * 59 * tr.n + tr.n + 4 * 59 * min(nv, tr.n)) if flags else 28 * 59 * tr.n)
     flops_fwd = counts["pairs_walked_fwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_FWD
     flops_bwd = counts["pairs_walked_bwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_BWD
     flops_fwd_exec = counts["pairs_evaluated_fwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_FWD
@@ -677,6 +676,8 @@ def main():
                     help="geometric visibility prediction: every partition is covered by sub x sub boxes of means (DESIGN.md s21)")
     ap.add_argument("--no-consolidate", action="store_true")
     ap.add_argument("--cross-filter", action="store_true", help="cross-boundary per-ray filtering (PAPER.md L474-L476, DESIGN.md s32)")
+    ap.add_argument("--plain-grads", action="store_true",
+                    help="do not track the gradient rows with flags: the first bucket writes every row, Adam reads every row")
     ap.add_argument("--sparse-adam", action="store_true", help="visible-only Adam (an option outside the paper, DESIGN.md s31)")
     args = ap.parse_args()
     if args.impl == "reference":

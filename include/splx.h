@@ -83,7 +83,9 @@ typedef struct {
 /* 2-D attributes of PAPER.md L80 (depth d, 2-D mean, Sigma2D as its inverse "conic").
  * means2d[n,2], depth[n], conic_opacity[n,4] = (A, B, C, o) with power = -0.5(A dx^2 +
  * C dy^2) - B dx dy, rgb[n,3], radius[n] (0 = culled), tiles_touched[n], clamp[n]
- * (bit c set: colour channel c was clamped at 0).  A culled Gaussian gets zeros. */
+ * (bit c set: colour channel c was clamped at 0).  A culled Gaussian gets radius = 0 and tiles_touched = 0; its other
+ * attributes are NOT written (no stage reads them: at city scale 90 % of the projected Gaussians are culled and their
+ * zeros were most of the projection's memory traffic). */
 typedef struct {
   float *means2d, *depth, *conic_opacity, *rgb;
   int32_t *radius;
@@ -92,7 +94,7 @@ typedef struct {
   /* blend[n,12]: the 48-byte record the blend kernels stage per list entry, written by
    * splx_project from the values above (no new arithmetic beyond the log2(e) pre-scaling of the
    * conic): (u, v, o, depth | -0.5 log2e A, -log2e B, -0.5 log2e C, bits(Gaussian index) |
-   * r, g, b, 0).  Zeros for a culled Gaussian. */
+   * r, g, b, 0).  Not written for a culled Gaussian. */
   float *blend;
 } splx_projected;
 
@@ -242,6 +244,16 @@ int splx_adam(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int6
 int splx_adam_groups(splx_ctx *ctx, float *param, float *grad, float *m, float *v, int n_groups,
                      const int64_t *group_offsets, const float *lr, float beta1, float beta2,
                      float eps, int step, float grad_scale, int zero_grad);
+
+/* splx_adam_groups with the gradient rows tracked by flags: every group holds `rows` rows of widths[j] floats (HOST
+ * int32[n_groups]; row r of group j at group_offsets[j] + r * widths[j]); touched (DEVICE uint8[rows]): the gradient of
+ * a row whose flag is clear is ZERO by definition and its memory is never read, so a caller need neither zero nor write
+ * the rows no view reached (splx_project_backward_list_plan's `touched` maintains the flags).  Still the DENSE optimiser
+ * of DESIGN.md s18: every parameter takes its step (an untouched one with g = 0: its moments decay, it moves along
+ * them); elementwise identical to splx_adam_groups on a buffer whose untouched rows are zero.  Flags are not cleared. */
+int splx_adam_groups_flagged(splx_ctx *ctx, float *param, const float *grad, float *m, float *v, int n_groups,
+                             const int64_t *group_offsets, const int32_t *widths, int64_t rows, const uint8_t *touched,
+                             const float *lr, float beta1, float beta2, float eps, int step, float grad_scale);
 
 /* ==== Optional subsystems (BASELINE.json north_star): visibility prediction
  * and conflict-free consolidation of B views into one launch.  Additive:
@@ -432,7 +444,11 @@ typedef struct {
   double *loss_sum;             /* double[2]: [0] += sum |image-target| (cleared by the call), [1] += sum SSIM */
   int32_t max_views;
   const uint64_t *cross_mask;   /* Q_cross masks [n] (splx_cross_sets) or NULL: cross-boundary filtering off */
-  uint8_t *touched;             /* [n] flags of the visible-only optimiser option or NULL */
+  uint8_t *touched;             /* [n] or NULL.  Given: the call clears it, every bucket's projection backward walks the
+                                   binning's list of visible Gaussians, STORES the gradient of a row it reaches first and
+                                   sets its flag, accumulates into flagged rows: grads is valid on flagged rows only and
+                                   no pass over all n rows ever zeroes or writes it.  NULL: the first bucket stores every
+                                   row of grads (zeros where nothing is visible), later buckets accumulate. */
 } splx_trainset;
 
 /* One bucket = one launch per stage (a conflict-free set of views, L249). */
@@ -443,8 +459,9 @@ typedef struct {
   const float *part_depth_range;/* HOST [2K] (splx_cross_depth_ranges) when trainset.cross_mask is set, else NULL */
 } splx_bucket;
 
-/* Optional a11 at the end of the iteration: dense Adam over the flat buffers (splx_adam_groups), or, with
- * trainset.touched, the visible-only option (splx_adam_sparse on the SoA sets; m / v as SoA). */
+/* Optional a11 at the end of the iteration: dense Adam over the flat buffers -- splx_adam_groups, or with
+ * trainset.touched splx_adam_groups_flagged (same result; the gradient rows no view reached are neither zeroed, written
+ * nor read) -- or, with trainset.touched and `sparse`, the visible-only option (splx_adam_sparse on the SoA sets). */
 typedef struct {
   float *param, *grad, *m, *v;          /* flat buffers holding the five groups back to back */
   int32_t n_groups;
@@ -452,7 +469,9 @@ typedef struct {
   const float *lr;                      /* HOST [n_groups] */
   float beta1, beta2, eps;
   int32_t step;                         /* 1-based */
-  splx_gaussian_grads m_soa, v_soa;     /* only read with trainset.touched */
+  const int32_t *widths;                /* HOST [n_groups]: floats per row of every group (needed with trainset.touched) */
+  int32_t sparse;                       /* with trainset.touched: 1 = the visible-only option (splx_adam_sparse), 0 = dense */
+  splx_gaussian_grads m_soa, v_soa;     /* only read with sparse */
 } splx_adam_cfg;
 
 #define SPLX_ITER_HOST 1   /* targets[v] / images_out[v] / loss_out / m_out are pinned HOST pointers */

@@ -35,7 +35,7 @@ EXPORTS = [
     "splx_compose_l1_backward_plan",
     "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
     "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
-    "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_iteration", "splx_microbench",
+    "splx_adam_groups_flagged", "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_iteration", "splx_microbench",
 ]
 MAX_VIEWS = 8
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
@@ -106,7 +106,7 @@ class AdamCfgS(C.Structure):
     _fields_ = [("param", C.c_void_p), ("grad", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p),
                 ("n_groups", C.c_int32), ("group_offsets", C.c_void_p), ("lr", C.c_void_p),
                 ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32),
-                ("m_soa", GaussiansS), ("v_soa", GaussiansS)]
+                ("widths", C.c_void_p), ("sparse", C.c_int32), ("m_soa", GaussiansS), ("v_soa", GaussiansS)]
 
 
 class IterOptsS(C.Structure):
@@ -164,6 +164,8 @@ def lib():
         L.splx_dssim_ws_floats.restype = C.c_size_t
         L.splx_dssim_ws_floats.argtypes = [vp]
         L.splx_dssim_loss_grad.argtypes = [vp, C.c_int, vp, vp, vp, C.c_float, C.c_float, vp, vp, vp]
+        L.splx_adam_groups_flagged.argtypes = [vp, vp, vp, vp, vp, C.c_int, vp, vp, C.c_int64, vp, vp, C.c_float, C.c_float,
+                                               C.c_float, C.c_int, C.c_float]
         L.splx_microbench.argtypes = [vp, C.c_int, C.c_int64, vp, vp]
         L.splx_iteration.argtypes = [vp, vp, C.c_int, vp, C.c_int, vp, vp, vp, vp, vp, vp]
         L.splx_schedule_views.argtypes = [C.c_int, vp, C.c_int, vp, vp]
@@ -462,6 +464,15 @@ class Context:
         lr = (C.c_float * n)(*[float(x) for x in lrs])
         self._check(lib().splx_adam_groups(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, lr,
                                            beta1, beta2, eps, step, grad_scale, int(zero_grad)))
+
+    def adam_groups_flagged(self, param, grad, m, v, group_offsets, widths, rows, touched, lrs, beta1=0.9, beta2=0.999,
+                            eps=1e-15, step=1, grad_scale=1.0):
+        n = len(lrs)
+        offs = (C.c_int64 * (n + 1))(*[int(x) for x in group_offsets])
+        wd = (C.c_int32 * n)(*[int(x) for x in widths])
+        lr = (C.c_float * n)(*[float(x) for x in lrs])
+        self._check(lib().splx_adam_groups_flagged(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, wd, int(rows),
+                                                   _ptr(touched), lr, beta1, beta2, eps, step, grad_scale))
 
     # ---- the same stages under a launch plan (visibility prediction, consolidated views) ---------
     visible_regions = staticmethod(visible_regions)     # host computations: no context needed

@@ -47,21 +47,61 @@ k_adam(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ 
 
 // All parameter groups of one flat buffer in ONE launch: the groups differ only in their learning
 // rate; group boundaries are multiples of 4 floats, so a 128-bit vector never straddles two groups.
-struct AdamGroups { long long end4[SPLX_ADAM_MAX_GROUPS]; float lr[SPLX_ADAM_MAX_GROUPS]; int n; };
+// FLAGS: the gradient of a row (Gaussian) whose byte in `touched` is clear is ZERO by definition and its memory is
+// never read -- the rows of the gradient buffer that no view of the iteration reached need neither zeroing nor
+// reading (at 100M Gaussians a view sees ~2 % of them).  Same arithmetic, statement by statement, as the plain kernel
+// on a gradient buffer whose untouched rows hold zeros.
+struct AdamGroups {
+  long long end4[SPLX_ADAM_MAX_GROUPS]; float lr[SPLX_ADAM_MAX_GROUPS]; int n;
+  long long start[SPLX_ADAM_MAX_GROUPS]; int width[SPLX_ADAM_MAX_GROUPS]; long long rows;     // FLAGS only
+};
 
-__global__ void __launch_bounds__(AB)
+template <bool FLAGS>
+__global__ void __launch_bounds__(AB, 6)      // 6 CTAs / SM (<= 42 registers): the bytes in flight, not the ALU, carry this kernel
 k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ m, float* __restrict__ v,
-              int64_t nvec, AdamK k, AdamGroups gr, float gscale, int zero_grad) {
+              int64_t nvec, AdamK k, const __grid_constant__ AdamGroups gr, float gscale, int zero_grad,
+              const uint8_t* __restrict__ touched) {
   for (int64_t i = (int64_t)blockIdx.x * AB + threadIdx.x; i < nvec; i += (int64_t)gridDim.x * AB) {
-    float lr = gr.lr[0];
+    int j = 0;
 #pragma unroll
-    for (int j = 1; j < SPLX_ADAM_MAX_GROUPS; ++j)
-      if (j < gr.n && i >= gr.end4[j - 1]) lr = gr.lr[j];
-    AdamK kk = k; kk.lr = lr;
-    float4 p = reinterpret_cast<float4*>(param)[i];
-    float4 g = reinterpret_cast<const float4*>(grad)[i];
-    float4 mm = reinterpret_cast<float4*>(m)[i];
-    float4 vv = reinterpret_cast<float4*>(v)[i];
+    for (int q = 1; q < SPLX_ADAM_MAX_GROUPS; ++q)
+      if (q < gr.n && i >= gr.end4[q - 1]) j = q;
+    AdamK kk = k; kk.lr = gr.lr[j];
+    float4 g = make_float4(0.f, 0.f, 0.f, 0.f), p, mm, vv;
+    if (FLAGS) {
+      // rows of the four elements of this vector (a row of width 3 or 1 does not fill a vector: up to four rows).  The
+      // widths of the Gaussian parameter groups get constant divisors in 32-bit arithmetic; any other width divides in 64.
+      const unsigned long long v0 = (unsigned long long)i - ((unsigned long long)gr.start[j] >> 2);   // vector index inside the group
+      const int w = gr.width[j];
+      unsigned long long r[4];
+      if (w == 48) { r[0] = r[1] = r[2] = r[3] = (uint32_t)v0 / 12u; }
+      else if (w == 4) { r[0] = r[1] = r[2] = r[3] = v0; }
+      else if (w == 1) { r[0] = 4 * v0; r[1] = r[0] + 1; r[2] = r[0] + 2; r[3] = r[0] + 3; }
+      else if (w == 3 && v0 < (1ull << 30)) {
+        const uint32_t e0 = 4u * (uint32_t)v0;
+        r[0] = e0 / 3u; r[1] = (e0 + 1u) / 3u; r[2] = (e0 + 2u) / 3u; r[3] = (e0 + 3u) / 3u;
+      } else {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) r[c] = (4 * v0 + c) / (unsigned long long)w;
+      }
+      // the flag bytes and the parameter / moment vectors are requested together (independent loads: one memory latency);
+      // only the gradient of a touched row waits for its flag
+      uint8_t fl[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) fl[c] = (long long)r[c] < gr.rows ? __ldg(touched + r[c]) : (uint8_t)0;
+      p = reinterpret_cast<float4*>(param)[i];
+      mm = reinterpret_cast<float4*>(m)[i];
+      vv = reinterpret_cast<float4*>(v)[i];
+      if (fl[0] | fl[1] | fl[2] | fl[3]) {
+        const float4 t = reinterpret_cast<const float4*>(grad)[i];
+        g = make_float4(fl[0] ? t.x : 0.f, fl[1] ? t.y : 0.f, fl[2] ? t.z : 0.f, fl[3] ? t.w : 0.f);
+      }
+    } else {
+      g = reinterpret_cast<const float4*>(grad)[i];
+      p = reinterpret_cast<float4*>(param)[i];
+      mm = reinterpret_cast<float4*>(m)[i];
+      vv = reinterpret_cast<float4*>(v)[i];
+    }
     adam1(p.x, g.x * gscale, mm.x, vv.x, kk);
     adam1(p.y, g.y * gscale, mm.y, vv.y, kk);
     adam1(p.z, g.z * gscale, mm.z, vv.z, kk);
@@ -69,7 +109,7 @@ k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __rest
     reinterpret_cast<float4*>(param)[i] = p;
     reinterpret_cast<float4*>(m)[i] = mm;
     reinterpret_cast<float4*>(v)[i] = vv;
-    if (zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!FLAGS && zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
 }
 
@@ -152,7 +192,7 @@ int launch_adam_sparse(splx_ctx* ctx, const splx_gaussian_grads* P, const splx_g
 
 int launch_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float* v, int n_groups,
                        const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
-                       float grad_scale, int zero_grad) {
+                       float grad_scale, int zero_grad, const int32_t* widths, int64_t rows, const uint8_t* touched) {
   const int64_t count = group_offsets[n_groups];
   if (count <= 0) return SPLX_OK;
   const double bc1 = 1.0 - pow((double)beta1, step), bc2 = 1.0 - pow((double)beta2, step);
@@ -163,12 +203,19 @@ int launch_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float
   const AdamK k{0.f, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps,
                 (float)(1.0 / bc1), (float)(1.0 / bc2)};
   AdamGroups gr;
+  memset(&gr, 0, sizeof gr);
   gr.n = n_groups;
+  gr.rows = rows;
   for (int j = 0; j < SPLX_ADAM_MAX_GROUPS; ++j) {
     gr.end4[j] = j < n_groups ? group_offsets[j + 1] >> 2 : nvec;
     gr.lr[j] = j < n_groups ? lr[j] : 0.f;
+    gr.start[j] = j < n_groups ? group_offsets[j] : count;
+    gr.width[j] = (touched && j < n_groups) ? widths[j] : 1;
   }
-  k_adam_groups<<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, zero_grad);
+  if (touched)
+    k_adam_groups<true><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, 0, touched);
+  else
+    k_adam_groups<false><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, zero_grad, nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_adam_groups");
   return SPLX_OK;
 }

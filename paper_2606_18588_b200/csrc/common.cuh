@@ -203,6 +203,7 @@ int launch_l1(splx_ctx*, const float* image, const float* target, int64_t count,
               float* g_image, double* loss_sum);
 int launch_adam_groups(splx_ctx*, float* param, float* grad, float* m, float* v, int n_groups,
                        const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
-                       float grad_scale, int zero_grad);
+                       float grad_scale, int zero_grad, const int32_t* widths = nullptr, int64_t rows = 0,
+                       const uint8_t* touched = nullptr);
 int launch_adam(splx_ctx*, float* param, float* grad, float* m, float* v, int64_t count, float lr,
                 float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad);

@@ -113,6 +113,7 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
   const splx_gaussians g{ts->params.mean, ts->params.log_scale, ts->params.quat, ts->params.opacity_logit, ts->params.sh, n};
 
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(ts->loss_sum, 0, 2 * sizeof(double), main));
+  if (ts->touched && n > 0) SPLX_CUDA_OK(ctx, cudaMemsetAsync(ts->touched, 0, (size_t)n, main));
   SPLX_CUDA_OK(ctx, cudaEventRecord(ctx->ev_start, main));
   if (host) {   // the targets travel while the first bucket is projected, binned and rendered: first needed by the loss
     SPLX_CUDA_OK(ctx, cudaStreamWaitEvent(ctx->s_up, ctx->ev_start, 0));
@@ -179,9 +180,9 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
       down_used = true;
     }
     if ((r = splx_raster_backward_plan(ctx, &fs.proj, &fs.bins, K, plan, &ts->partials, ts->g_ct, ts->g2d))) return r;
-    // a10: the first bucket stores the gradient (every row: no zeroing pass), later buckets accumulate over the
-    // binning's list of visible Gaussians; with the visible-only optimiser every bucket walks the list and the
-    // flags say which rows to store and which to add to
+    // a10: with flags (ts->touched) every bucket walks the binning's list of visible Gaussians, stores the gradient of a
+    // row it is the first to reach and adds to the others; without them the first bucket stores every row of the
+    // gradient (zeros where nothing is visible) and later buckets accumulate over the list
     const uint32_t* vlist = nullptr;
     const uint64_t* nvis = nullptr;
     if (ts->touched || gi > 0) {
@@ -216,12 +217,17 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
   }
 
   if (adam) {
-    if (ts->touched) {
+    const float gs = 1.0f / (float)n_views;
+    if (ts->touched && adam->sparse) {
       if ((rc = splx_adam_sparse(ctx, &ts->params, &ts->grads, &adam->m_soa, &adam->v_soa, ts->touched, adam->lr, adam->beta1,
-                                 adam->beta2, adam->eps, adam->step, 1.0f / (float)n_views))) return rc;
+                                 adam->beta2, adam->eps, adam->step, gs))) return rc;
+    } else if (ts->touched) {
+      if ((rc = splx_adam_groups_flagged(ctx, adam->param, adam->grad, adam->m, adam->v, adam->n_groups, adam->group_offsets,
+                                         adam->widths, n, ts->touched, adam->lr, adam->beta1, adam->beta2, adam->eps, adam->step,
+                                         gs))) return rc;
     } else {
       if ((rc = splx_adam_groups(ctx, adam->param, adam->grad, adam->m, adam->v, adam->n_groups, adam->group_offsets, adam->lr,
-                                 adam->beta1, adam->beta2, adam->eps, adam->step, 1.0f / (float)n_views, 0))) return rc;
+                                 adam->beta1, adam->beta2, adam->eps, adam->step, gs, 0))) return rc;
     }
   }
   if (down_used) {   // join: a caller that synchronises the context's stream finds the host buffers complete

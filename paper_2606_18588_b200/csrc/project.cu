@@ -215,12 +215,8 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       vis = tt > 0;
     }
     float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-    if (!vis) {
-      *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(0.f, 0.f);
-      out.depth[i] = 0.f;
-      *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
-      out.radius[i] = 0; out.tiles_touched[i] = 0;
-      bl[0] = bl[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!vis) {   // a culled Gaussian: radius = tiles_touched = 0 say so; nothing downstream reads its other attributes, and
+      out.radius[i] = 0; out.tiles_touched[i] = 0;     // writing 129 bytes of zeros for it was most of this kernel's traffic
     } else {
       const float idet = 1.0f / G.det;
       const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
@@ -236,11 +232,6 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     }
   }
   float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-  if (active && !vis) {
-    out.rgb[3 * i] = 0.f; out.rgb[3 * i + 1] = 0.f; out.rgb[3 * i + 2] = 0.f;
-    out.clamp[i] = 0;
-    bl[2] = make_float4(0.f, 0.f, 0.f, 0.f);
-  }
   const int lane = threadIdx.x & 31;
   const unsigned vmask = __ballot_sync(0xffffffffu, vis);
   if (vmask == 0) return;

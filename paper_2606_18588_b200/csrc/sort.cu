@@ -32,7 +32,10 @@ struct Counters {   // device-resident counts, written by kernels, read by later
   uint32_t ticket[16];  // dynamic tile counters, one per single-pass kernel of the pipeline
 };
 
-struct PartOffs { int64_t off[SPLX_MAX_K + 1]; int K; };
+// rank[k]: position of partition k among the partitions that take part in this launch (-1: it does not).  The slot sort
+// runs on the COMPACT slot rank[k] * ntiles + tile -- monotone in the true slot k * ntiles + tile, so the order is the
+// same, with fewer key bits (6-8 of 32 partitions take part in a city view: 16 bits instead of 18, two passes for three).
+struct PartOffs { int64_t off[SPLX_MAX_K + 1]; int K; signed char rank[SPLX_MAX_K]; };
 
 // Tile status word of the single-pass ("decoupled look-back") scans: flag in the top two bits,
 // running count below.  A tile publishes its own total (AGG) as soon as it knows it and its
@@ -306,11 +309,115 @@ k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t*
 
 // Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
 // started and the look-back spin cannot wait on a CTA that was never scheduled.
-template <typename KeyT>
+// The LAST pass of the slot sort writes the binning itself: its 32-bit items are (compact slot, position j in the
+// depth-sorted list of visible Gaussians); the 64-bit key (true slot << 32 | depth bits of j) and the value (Gaussian
+// index of j) are formed on the way out, from two arrays of N_visible entries that sit in L2.  The passes before it
+// move 8 bytes per intersection instead of 12.
+struct FinalOut {
+  uint64_t* keys; uint32_t* vals;               // splx_binning.keys / vals
+  const uint32_t* ckeys; const uint32_t* cvals; // depth bits / Gaussian index of the j-th visible Gaussian in depth order
+  uint32_t ntiles;
+  uint32_t skip[SPLX_MAX_K + 1];                // true slot = compact slot + skip[compact slot / ntiles]
+};
+
+// One tile of a radix pass (RS_TILE keys of one CTA): stable ranks by warp multisplit, the tile's keys reordered in
+// shared memory, the per-digit prefix over the tiles by look-back, the scatter.  FULL: every one of the RS_TILE
+// positions holds a key.
+template <typename KeyT, bool FINAL, bool FULL>
+__device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
+                                           uint32_t* __restrict__ vout, uint64_t start, uint32_t nv, uint32_t t, int shift,
+                                           uint32_t mask, uint64_t* status, const FinalOut& fin, uint32_t (*whist)[256],
+                                           uint32_t* dbase, const uint32_t* gbase, uint32_t* lbase, KeyT* skey, uint32_t* sval,
+                                           uint32_t* sm) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  // warp w owns the contiguous segment [w*256, +256) of the tile; iteration `it` covers 32 consecutive
+  // positions, so (it, lane) is the input order and the ranks below are stable.
+  const uint32_t seg = (uint32_t)warp * (32 * RS_IPT) + (uint32_t)lane;
+  KeyT key[RS_IPT];
+  uint32_t val[RS_IPT], dg[RS_IPT], rank[RS_IPT];
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    const uint32_t o = seg + (uint32_t)it * 32;
+    const bool valid = FULL || o < nv;
+    key[it] = valid ? kin[start + o] : (KeyT)0;
+    val[it] = valid ? vin[start + o] : 0u;
+  }
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    const bool valid = FULL || seg + (uint32_t)it * 32 < nv;
+    const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
+    dg[it] = d;
+    // lanes of the warp with this lane's digit: one ballot per digit bit; (bit - 1) is all ones for a clear bit
+    unsigned peers = FULL ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const uint32_t bit = (d >> b) & 1u;
+      peers &= __ballot_sync(0xffffffffu, bit) ^ (bit - 1u);
+    }
+    uint32_t old = 0;
+    const int leader = __ffs(peers) - 1;               // (an invalid lane: its own digit-0 group among the invalid ones; unused)
+    if (valid && lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
+    old = __shfl_sync(0xffffffffu, old, leader & 31);
+    rank[it] = old + __popc(peers & lt);
+    __syncwarp();
+  }
+  __syncthreads();
+  uint32_t run = 0;   // per digit (thread d): exclusive prefix over the warps, tile total
+  {
+    const int d = threadIdx.x;
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
+  }
+  {  // position of digit d's first key inside the tile, in digit order
+    uint32_t tot;
+    lbase[threadIdx.x] = block_exclusive_scan(run, sm, tot);
+  }
+  __syncthreads();
+  // the tile's keys go to shared memory in digit order, so that the scatter below writes runs of consecutive
+  // addresses (one run per digit) instead of 2048 isolated items
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    if (FULL || seg + (uint32_t)it * 32 < nv) {
+      const uint32_t lp = lbase[dg[it]] + whist[warp][dg[it]] + rank[it];
+      skey[lp] = key[it];
+      sval[lp] = val[it];
+    }
+  }
+  {  // chained prefix over the tiles (look-back), one chain per digit
+    const int d = threadIdx.x;
+    uint64_t excl = 0;
+    uint64_t* st = status + d;
+    if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
+    else excl = lookback<8>(st, t, 256, run);
+    dbase[d] = gbase[d] + (uint32_t)excl - lbase[d];      // global position = dbase[d] + position in the tile
+  }
+  __syncthreads();
+#pragma unroll
+  for (int it = 0; it < RS_IPT; ++it) {
+    const uint32_t j = (uint32_t)it * RS_THREADS + threadIdx.x;
+    if (FULL || j < nv) {
+      const KeyT k = skey[j];
+      const uint32_t d = (uint32_t)(k >> shift) & mask;
+      const uint32_t pos = dbase[d] + j;
+      if (FINAL) {
+        const uint32_t cs = (uint32_t)k, jj = sval[j];
+        const uint32_t slot = cs + fin.skip[cs / fin.ntiles];
+        fin.keys[pos] = ((uint64_t)slot << 32) | __ldg(fin.ckeys + jj);
+        fin.vals[pos] = __ldg(fin.cvals + jj);
+      } else {
+        kout[pos] = k;
+        vout[pos] = sval[j];
+      }
+    }
+  }
+}
+
+template <typename KeyT, bool FINAL>
 __global__ void __launch_bounds__(RS_THREADS, 4)
 k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
              uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
-             uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits) {
+             uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits, const __grid_constant__ FinalOut fin) {
   __shared__ uint32_t whist[RS_WARPS][256];
   __shared__ uint32_t dbase[256];
   __shared__ uint32_t gbase[256];
@@ -323,8 +430,6 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
   const uint64_t ntiles = (n + RS_TILE - 1) / RS_TILE;
   if (blockIdx.x >= ntiles) return;
   const uint32_t mask = (1u << bits) - 1u;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned lt = (1u << lane) - 1u;
   {  // exclusive scan of the global digit histogram = first output position of each digit (once per CTA)
     uint32_t tot;
     gbase[threadIdx.x] = block_exclusive_scan(ghist[threadIdx.x], sm, tot);
@@ -338,77 +443,13 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
     const uint32_t t = s_tile;
     if (t >= ntiles) return;
     const uint64_t start = (uint64_t)t * RS_TILE;
-    // warp w owns the contiguous segment [start + w*256, +256); iteration `it` covers 32 consecutive
-    // positions, so (it, lane) is the input order and the ranks below are stable.
-    const uint64_t seg = start + (uint64_t)warp * (32 * RS_IPT);
-    KeyT key[RS_IPT];
-    uint32_t val[RS_IPT];
-    uint32_t rank[RS_IPT];
-#pragma unroll
-    for (int it = 0; it < RS_IPT; ++it) {
-      const uint64_t idx = seg + (uint64_t)it * 32 + lane;
-      key[it] = idx < n ? kin[idx] : (KeyT)0;
-      val[it] = idx < n ? vin[idx] : 0u;
-    }
-#pragma unroll
-    for (int it = 0; it < RS_IPT; ++it) {
-      const uint64_t idx = seg + (uint64_t)it * 32 + lane;
-      const bool valid = idx < n;
-      const unsigned vm = __ballot_sync(0xffffffffu, valid);
-      const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
-      const unsigned peers = digit_peers(d, vm);
-      const int leader = valid ? __ffs(peers) - 1 : lane;
-      uint32_t old = 0;
-      if (valid && lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
-      old = __shfl_sync(0xffffffffu, old, leader);
-      rank[it] = old + __popc(peers & lt);
-      __syncwarp();
-    }
-    __syncthreads();
-    uint32_t run = 0;   // per digit (thread d): exclusive prefix over the warps, tile total
-    {
-      const int d = threadIdx.x;
-#pragma unroll
-      for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
-    }
-    {  // position of digit d's first key inside the tile, in digit order
-      uint32_t tot;
-      lbase[threadIdx.x] = block_exclusive_scan(run, sm, tot);
-    }
-    __syncthreads();
-    // the tile's keys go to shared memory in digit order, so that the scatter below writes runs of consecutive
-    // addresses (one run per digit) instead of 2048 isolated 8- or 12-byte items
-#pragma unroll
-    for (int it = 0; it < RS_IPT; ++it) {
-      const uint64_t idx = seg + (uint64_t)it * 32 + lane;
-      if (idx < n) {
-        const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
-        const uint32_t lp = lbase[d] + whist[warp][d] + rank[it];
-        skey[lp] = key[it];
-        sval[lp] = val[it];
-      }
-    }
-    {  // chained prefix over the tiles (look-back), one chain per digit
-      const int d = threadIdx.x;
-      uint64_t excl = 0;
-      uint64_t* st = status + d;
-      if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
-      else excl = lookback<8>(st, t, 256, run);
-      dbase[d] = gbase[d] + (uint32_t)excl - lbase[d];      // global position = dbase[d] + position in the tile
-    }
-    __syncthreads();
     const uint32_t nv = (uint32_t)((n - start) < (uint64_t)RS_TILE ? (n - start) : (uint64_t)RS_TILE);
-#pragma unroll
-    for (int it = 0; it < RS_IPT; ++it) {
-      const uint32_t j = (uint32_t)it * RS_THREADS + threadIdx.x;
-      if (j < nv) {
-        const KeyT k = skey[j];
-        const uint32_t d = (uint32_t)(k >> shift) & mask;
-        const uint32_t pos = dbase[d] + j;
-        kout[pos] = k;
-        vout[pos] = sval[j];
-      }
-    }
+    // the kernel is bound by instruction issue (ncu, city_100M: 62 % issue slots, DRAM 13 %): a full tile -- all but the
+    // last one -- takes the copy of the body without the per-item range checks
+    if (nv == RS_TILE)
+      radix_tile<KeyT, FINAL, true>(kin, vin, kout, vout, start, nv, t, shift, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+    else
+      radix_tile<KeyT, FINAL, false>(kin, vin, kout, vout, start, nv, t, shift, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
   }
 }
 
@@ -419,7 +460,8 @@ template <typename KeyT>
 int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
                const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets,
                bool have_hist /* histograms counted and status cleared by the producer of the keys */,
-               size_t stride_words = 0 /* status words per pass; 0 = tiles(capacity) * 256 */) {
+               size_t stride_words = 0 /* status words per pass; 0 = tiles(capacity) * 256 */,
+               const FinalOut* fin = nullptr /* the last pass writes the binning (see FinalOut) */) {
   const uint32_t ntiles_cap = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
   if (ntiles_cap == 0) return SPLX_OK;
   const uint32_t nblocks = ntiles_cap < PERSISTENT_CTAS ? ntiles_cap : PERSISTENT_CTAS;
@@ -429,10 +471,17 @@ int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, ui
     k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, status, stride, plan);
     SPLX_LAUNCH_CHECK(ctx, "k_radix_hist_all");
   }
+  FinalOut none;
+  memset(&none, 0, sizeof none);
   for (int p = 0; p < plan.npass; ++p) {
-    k_radix_pass<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
-                                                               status + (size_t)p * stride, tickets + p,
-                                                               plan.shift[p], plan.bits[p]);
+    if (fin && p + 1 == plan.npass)
+      k_radix_pass<KeyT, true><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
+                                                                       status + (size_t)p * stride, tickets + p,
+                                                                       plan.shift[p], plan.bits[p], *fin);
+    else
+      k_radix_pass<KeyT, false><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
+                                                                        status + (size_t)p * stride, tickets + p,
+                                                                        plan.shift[p], plan.bits[p], none);
     SPLX_LAUNCH_CHECK(ctx, "k_radix_pass");
     KeyT* tk = ka; ka = kb; kb = tk;
     uint32_t* tv = va; va = vb; vb = tv;
@@ -488,7 +537,7 @@ __global__ void __launch_bounds__(256)
 k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
-            uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
+            uint64_t capacity, uint32_t* __restrict__ skeys, uint32_t* __restrict__ spay, PassPlan plan,
             uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride,
             const __grid_constant__ CrossEmit cx) {
   if (emit_by_output(cnt) || (cnt->m_total >> 32)) return;   // M >= 2^32: the 32-bit offsets have wrapped, nothing is emitted
@@ -509,10 +558,10 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
   for (uint64_t base = (uint64_t)blockIdx.x * blockDim.x; base < nvis; base += (uint64_t)gridDim.x * blockDim.x) {
   const uint64_t j = base + threadIdx.x;
   int x0 = 0, y0 = 0, w = 0, tt = 0;
-  uint32_t i = 0, o = 0, dbits = 0, slot0 = 0;
+  uint32_t i = 0, o = 0, slot0 = 0;
   uint64_t F = 0;
   if (j < nvis) {
-    i = cvals[j]; dbits = ckeys[j]; o = offs[j];
+    i = cvals[j]; o = offs[j];
     const float2 m = *reinterpret_cast<const float2*>(means2d + 2 * (uint64_t)i);
     int x1, y1;
     tile_rect(m.x, m.y, radius[i], TX, TY, x0, y0, x1, y1);
@@ -522,8 +571,8 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       const int mid = (lo + hi + 1) >> 1;
       if (parts.off[mid] <= (int64_t)i) lo = mid; else hi = mid - 1;
     }
-    slot0 = (uint32_t)lo * (uint32_t)(TX * TY);
-    if (FILTER) F = cross_filter(cx, i, lo, __uint_as_float(dbits));
+    slot0 = (uint32_t)parts.rank[lo] * (uint32_t)(TX * TY);      // compact slot (see PartOffs)
+    if (FILTER) F = cross_filter(cx, i, lo, __uint_as_float(ckeys[j]));
   }
   // The 32 runs of a warp are adjacent in the output (offs is the running sum of tiles_touched in this very
   // order), so the warp writes its whole range [o_0, o_0 + T) cooperatively: lane l produces output slot
@@ -547,7 +596,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
     const uint32_t t = sidx - __shfl_sync(0xffffffffu, pre, own);
     const int sx0 = __shfl_sync(0xffffffffu, x0, own), sy0 = __shfl_sync(0xffffffffu, y0, own);
     const int sw = __shfl_sync(0xffffffffu, w, own);
-    const uint32_t si = __shfl_sync(0xffffffffu, i, own), sd = __shfl_sync(0xffffffffu, dbits, own);
+    const uint32_t sj = (uint32_t)base + (uint32_t)(threadIdx.x & ~31) + (uint32_t)own;     // position in the depth-sorted list
     const uint32_t ss = __shfl_sync(0xffffffffu, slot0, own);
     const uint64_t pos = (uint64_t)o0 + sidx;
     uint64_t sF = 0;
@@ -557,10 +606,10 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       const uint32_t tile = (uint32_t)((sy0 + (int)ty) * TX + sx0 + (int)(t - ty * (uint32_t)sw));
       uint32_t slot = ss + tile;
       if (FILTER && sF && cross_removed(cx, sF, tile)) slot = cx.nslots;
-      keys[pos] = ((uint64_t)slot << 32) | sd;
-      vals[pos] = si;
+      skeys[pos] = slot;
+      spay[pos] = sj;
       for (int p = 0; p < plan.npass; ++p)
-        atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
+        atomicAdd(&s_hist[p * 256 + ((slot >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u))], 1u);
     }
   }
   }
@@ -573,7 +622,7 @@ __global__ void __launch_bounds__(256)
 k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ radius,
             const uint32_t* __restrict__ ckeys, const uint32_t* __restrict__ cvals,
             const uint32_t* __restrict__ offs, const Counters* cnt, PartOffs parts, int TX, int TY,
-            uint64_t capacity, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals, PassPlan plan,
+            uint64_t capacity, uint32_t* __restrict__ skeys, uint32_t* __restrict__ spay, PassPlan plan,
             uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride,
             const __grid_constant__ CrossEmit cx) {
   if (!emit_by_output(cnt) || (cnt->m_total >> 32)) return;
@@ -594,8 +643,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
   // 1.5 ms on street_10M).  Per tile: a 256-ary search over offs finds the first owner, the owners' run starts and
   // rectangles are staged in shared memory, every thread places EK_IPT keys by a binary search over the staged starts.
   constexpr int EK_TILE = 1024, EK_IPT = EK_TILE / 256;
-  __shared__ uint32_t s_off[EK_TILE + 1], s_xy[EK_TILE + 1], s_w[EK_TILE + 1], s_slot0[EK_TILE + 1], s_db[EK_TILE + 1],
-      s_gi[EK_TILE + 1];
+  __shared__ uint32_t s_off[EK_TILE + 1], s_xy[EK_TILE + 1], s_w[EK_TILE + 1], s_slot0[EK_TILE + 1];
   __shared__ uint64_t s_F[FILTER ? EK_TILE + 1 : 1];
   __shared__ uint32_t s_nown;
   const uint64_t nvis = cnt->n_visible;
@@ -631,8 +679,8 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
           if (parts.off[mid] <= (int64_t)i) plo = mid; else phi = mid - 1;
         }
         s_off[q] = o; s_xy[q] = ((uint32_t)y0 << 16) | (uint32_t)x0; s_w[q] = (uint32_t)(x1 - x0);
-        s_slot0[q] = (uint32_t)plo * (uint32_t)(TX * TY); s_db[q] = ckeys[j]; s_gi[q] = i;
-        if (FILTER) s_F[q] = cross_filter(cx, i, plo, __uint_as_float(s_db[q]));
+        s_slot0[q] = (uint32_t)parts.rank[plo] * (uint32_t)(TX * TY);
+        if (FILTER) s_F[q] = cross_filter(cx, i, plo, __uint_as_float(ckeys[j]));
         atomicMax(&s_nown, (uint32_t)q + 1);
       }
     }
@@ -652,10 +700,10 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         const uint32_t tile = ((xy >> 16) + ty) * (uint32_t)TX + (xy & 0xffffu) + (t - ty * w);
         uint32_t slot = s_slot0[ql] + tile;
         if (FILTER) { const uint64_t F = s_F[ql]; if (F && cross_removed(cx, F, tile)) slot = cx.nslots; }
-        keys[pos] = ((uint64_t)slot << 32) | s_db[ql];
-        vals[pos] = s_gi[ql];
+        skeys[pos] = slot;
+        spay[pos] = (uint32_t)j0 + ql;                    // position of the owner in the depth-sorted list
         for (int p = 0; p < plan.npass; ++p)
-          atomicAdd(&s_hist[p * 256 + ((slot >> (plan.shift[p] - 32)) & ((1u << plan.bits[p]) - 1u))], 1u);
+          atomicAdd(&s_hist[p * 256 + ((slot >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u))], 1u);
       }
     }
     __syncthreads();
@@ -753,7 +801,7 @@ __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_
 // actual counts reach) and the sort buffers.
 struct Layout {
   size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes;
-  size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, vis_list, keys_tmp, vals_tmp, total;
+  size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, vis_list, pairs_tmp, total;
 };
 
 static int slot_bits(int K, int TX, int TY) {
@@ -781,7 +829,7 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
   L.offs = take((size_t)n * 4);
   L.vis_list = take((size_t)n * 4);
-  L.keys_tmp = take((size_t)capacity * 8); L.vals_tmp = take((size_t)capacity * 4);
+  L.pairs_tmp = take((size_t)capacity * 8);      // (compact slot, depth-order position) pairs: two uint32[capacity]
   L.total = off;
   return L;
 }
@@ -815,7 +863,6 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   uint32_t* ckeys_a = (uint32_t*)(base + L.ckeys_a); uint32_t* cvals_a = (uint32_t*)(base + L.cvals_a);
   uint32_t* ckeys_b = (uint32_t*)(base + L.ckeys_b); uint32_t* cvals_b = (uint32_t*)(base + L.cvals_b);
   uint32_t* offs = (uint32_t*)(base + L.offs);
-  uint64_t* keys_tmp = (uint64_t*)(base + L.keys_tmp); uint32_t* vals_tmp = (uint32_t*)(base + L.vals_tmp);
   const int ntiles = cam.TX * cam.TY;
 
   SPLX_CUDA_OK(ctx, cudaMemsetAsync(base, 0, L.zero_bytes, ctx->stream));
@@ -849,17 +896,33 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
   if ((rc = scan_exclusive<TouchedOp, false>(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
                            &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
-  const int passes = (sbits + 7) / 8;
-  uint64_t* k0 = (passes & 1) ? keys_tmp : out->keys;   // so that the last pass lands in out->keys
-  uint32_t* v0 = (passes & 1) ? vals_tmp : out->vals;
-  uint64_t* k1 = (passes & 1) ? out->keys : keys_tmp;
-  uint32_t* v1 = (passes & 1) ? out->vals : vals_tmp;
+  // 4. the (compact slot, depth-order position) pairs and their stable sort on the compact slot bits.  Two pair buffers:
+  // A in the workspace, B in the memory of out->keys (dead until the last pass writes the 64-bit keys there, reading A).
   PartOffs parts;
   parts.K = K;
   for (int k = 0; k <= K; ++k) parts.off[k] = part_offsets[k];
+  FinalOut fin;
+  memset(&fin, 0, sizeof fin);
+  int nact = 0;
+  for (int k = 0; k < K; ++k) {
+    const bool act = plan.pv.v[k] >= 0 && part_offsets[k + 1] > part_offsets[k];
+    parts.rank[k] = act ? (signed char)nact : (signed char)-1;
+    if (act) { fin.skip[nact] = (uint32_t)(k - nact) * (uint32_t)ntiles; ++nact; }
+  }
+  fin.skip[nact] = (uint32_t)(K - nact) * (uint32_t)ntiles;       // the slot of filtered pairs: one past the last real slot
+  fin.keys = out->keys; fin.vals = out->vals; fin.ckeys = ckeys_a; fin.cvals = cvals_a; fin.ntiles = (uint32_t)ntiles;
+  const uint32_t cslots = (uint32_t)nact * (uint32_t)ntiles;      // compact slots 0 .. cslots (cslots itself = filtered)
+  int cbits = 1;
+  while (((uint64_t)1 << cbits) <= cslots) ++cbits;
+  const PassPlan spl = plan_passes(0, cbits);
+  uint32_t* A_k = (uint32_t*)(base + L.pairs_tmp); uint32_t* A_p = A_k + out->capacity;
+  uint32_t* B_k = (uint32_t*)out->keys; uint32_t* B_p = B_k + out->capacity;
+  const bool startA = (spl.npass & 1) != 0;                       // so that the LAST pass reads A (and may overwrite B's memory)
+  uint32_t* k0 = startA ? A_k : B_k; uint32_t* p0 = startA ? A_p : B_p;
+  uint32_t* k1 = startA ? B_k : A_k; uint32_t* p1 = startA ? B_p : A_p;
   CrossEmit cx;
   memset(&cx, 0, sizeof cx);
-  cx.ntiles = (uint32_t)ntiles; cx.nslots = (uint32_t)K * (uint32_t)ntiles;
+  cx.ntiles = (uint32_t)ntiles; cx.nslots = cslots;
   if (cross && cross->mask) {
     cx.mask = cross->mask; cx.tile_state = plan.tile_state;
     for (int k = 0; k < K; ++k) { cx.zlo[k] = cross->zlo[k]; cx.zhi[k] = cross->zhi[k]; cx.view[k] = plan.pv.v[k]; }
@@ -868,31 +931,29 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   const unsigned g_emit = (unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS);
   const uint64_t emit_tiles = (out->capacity + 1023) / 1024;     // output tiles of 1024 keys
   const unsigned g_lb = (unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS);
-  const PassPlan spl = plan_passes(32, 32 + sbits);
   uint32_t* gh = (uint32_t*)(base + L.ghist_s);
   uint64_t* sst = (uint64_t*)(base + L.st_slot);
   const size_t sstride = (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256;
   if (cx.mask) {
     k_emit_keys<true><<<g_emit, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
-                                                       out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+                                                       out->capacity, k0, p0, spl, gh, sst, sstride, cx);
     SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
     k_emit_keys_lb<true><<<g_lb, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
-                                                        out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+                                                        out->capacity, k0, p0, spl, gh, sst, sstride, cx);
     SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
   } else {
     k_emit_keys<false><<<g_emit, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
-                                                        out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+                                                        out->capacity, k0, p0, spl, gh, sst, sstride, cx);
     SPLX_LAUNCH_CHECK(ctx, "k_emit_keys");
     k_emit_keys_lb<false><<<g_lb, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
-                                                         out->capacity, k0, v0, spl, gh, sst, sstride, cx);
+                                                         out->capacity, k0, p0, spl, gh, sst, sstride, cx);
     SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
   }
-  // 4. stable sort on the slot bits
-  if ((rc = radix_sort<uint64_t>(ctx, k0, v0, k1, v1, out->capacity, &cnt->m_sorted, 32, 32 + sbits,
-                                 (uint32_t*)(base + L.ghist_s), (uint64_t*)(base + L.st_slot), &cnt->ticket[6], true))) return rc;
+  if ((rc = radix_sort<uint32_t>(ctx, k0, p0, k1, p1, out->capacity, &cnt->m_sorted, 0, cbits, gh, sst, &cnt->ticket[6], true, 0,
+                                 &fin))) return rc;
   // 5. ranges
   k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
-      out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections, cx.nslots, cx.mask != nullptr);
+      out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections, (uint32_t)K * (uint32_t)ntiles, cx.mask != nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_tile_ranges");
   if (out->slot_order && slot_order_pays(plan)) {
     const uint32_t nslots = (uint32_t)K * (uint32_t)ntiles;

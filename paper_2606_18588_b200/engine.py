@@ -77,6 +77,10 @@ class Trainer:
         #: visible-only ("sparse") Adam -- an OPTION outside the paper: only Gaussians that received a gradient
         #: in the iteration take the step (splx_adam_sparse); no gradient buffer is ever zeroed or overwritten wholesale
         self.sparse_adam = False
+        #: the training path tracks the gradient rows an iteration reaches with one flag byte per Gaussian (splx_trainset.touched):
+        #: rows no view saw are neither zeroed, written nor read -- at 100M Gaussians a view sees ~2 % of them -- and the dense
+        #: Adam step takes their gradient as zero (splx_adam_groups_flagged: same result as the plain buffer)
+        self.flagged_grads = True
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
         self.pipeline_buckets = True
         self._touched = None
@@ -127,13 +131,22 @@ class Trainer:
                           g_T_total, self.params, self.proj, self.bins, self.sh_degree, self.grads, self._ws_bwd,
                           overwrite=overwrite)
 
-    def adam_step(self, n_views=1, zero_grad=False):
-        """a11: one Adam step over the flat parameter buffer (five groups = five learning rates, one launch)."""
+    def adam_step(self, n_views=1, zero_grad=False, flagged=False):
+        """a11: one Adam step over the flat parameter buffer (five groups = five learning rates, one launch).  flagged: the
+        gradient rows are tracked by the `touched` flags of the last splx_iteration (untouched rows count as zero)."""
         self.step_count += 1
         offs = [self._offs[k] for k in PARAM_KEYS] + [self._total]
-        self.ctx.adam_groups(self.flat["param"], self.flat["grad"], self.flat["m"], self.flat["v"], offs,
-                             [self.lr[k] for k in PARAM_KEYS], step=self.step_count, grad_scale=1.0 / n_views,
-                             zero_grad=zero_grad)
+        lrs = [self.lr[k] for k in PARAM_KEYS]
+        f = self.flat
+        if self.sparse_adam and flagged:
+            self.ctx.adam_sparse(self.params, self.grads, self.m, self.v, self._touched, lrs, step=self.step_count,
+                                 grad_scale=1.0 / n_views)
+        elif flagged:
+            self.ctx.adam_groups_flagged(f["param"], f["grad"], f["m"], f["v"], offs, [PARAM_WIDTH[k] for k in PARAM_KEYS], self.n,
+                                         self._touched, lrs, step=self.step_count, grad_scale=1.0 / n_views)
+        else:
+            self.ctx.adam_groups(f["param"], f["grad"], f["m"], f["v"], offs, lrs, step=self.step_count,
+                                 grad_scale=1.0 / n_views, zero_grad=zero_grad)
 
     def iteration(self, cams, targets):
         """One training iteration over B views through the single-stage calls (gradients of the B mean losses are averaged)."""
@@ -293,7 +306,7 @@ class Trainer:
         proj, bins, ws = (self.proj, self.bins, self._ws_sort) if which == 0 else self._alt
         return binding.FrontsetS(proj.struct(), bins.struct(), ws.data_ptr(), ws.numel())
 
-    def _trainset(self, n_views, pipelined):
+    def _trainset(self, n_views, pipelined, flags=False):
         """splx_trainset over this trainer's buffers (allocating the ones the training path needs on first use)."""
         dev = self.ctx.device
         self._view_buffers(max(n_views, 1))
@@ -306,7 +319,8 @@ class Trainer:
         if self.lambda_dssim > 0 and getattr(self, "_dssim_ws", None) is None:
             nf = self.ctx.dssim_ws_floats(self.W, self.H)
             self._dssim_ws = torch.empty(binding.MAX_VIEWS * nf, dtype=torch.float32, device=dev)
-        if self.sparse_adam and self._touched is None:
+        flags = flags or self.sparse_adam
+        if flags and self._touched is None:
             self._touched = torch.zeros(max(self.n, 1), dtype=torch.uint8, device=dev)
         ts = binding.TrainsetS()
         ts.params = binding.gaussians_struct(self.params)
@@ -326,17 +340,19 @@ class Trainer:
         ts.loss_sum = self.loss_sum.data_ptr()
         ts.max_views = self._images.shape[0]
         ts.cross_mask = self._cross.data_ptr() if self._cross is not None else None
-        ts.touched = self._touched.data_ptr() if self.sparse_adam else None
+        ts.touched = self._touched.data_ptr() if flags else None
         return ts
 
     def _adam_cfg(self, step):
         offs = (C.c_int64 * 6)(*([self._offs[k] for k in PARAM_KEYS] + [self._total]))
         lrs = (C.c_float * 5)(*[float(self.lr[k]) for k in PARAM_KEYS])
+        wds = (C.c_int32 * 5)(*[PARAM_WIDTH[k] for k in PARAM_KEYS])
         f = self.flat
         a = binding.AdamCfgS(f["param"].data_ptr(), f["grad"].data_ptr(), f["m"].data_ptr(), f["v"].data_ptr(), 5,
                              C.cast(offs, C.c_void_p), C.cast(lrs, C.c_void_p), 0.9, 0.999, 1e-15, int(step),
+                             C.cast(wds, C.c_void_p), 1 if self.sparse_adam else 0,
                              binding.gaussians_struct(self.m), binding.gaussians_struct(self.v))
-        a._keep = (offs, lrs)
+        a._keep = (offs, lrs, wds)
         return a
 
     def _bucket_structs(self, plans, groups):
@@ -368,13 +384,13 @@ class Trainer:
                 raise CapacityError(f"{m} tile intersections exceed the capacity {self.capacity}: the farthest keys were dropped")
 
     def _run_iteration(self, plans, groups, n_views, targets, sat_eps, adam=True, host=False, images_out=None,
-                       loss_out=None):
+                       loss_out=None, flags=False):
         """plans: [(Plan, state_out)], groups: view positions per plan; targets: list of raw pointers per view."""
         if not torch.cuda.is_current_stream_capturing():
             self.check_overflow()
         self._workspaces(plans[0][0].cams[0])
         pipelined = self.pipeline_buckets and len(plans) > 1
-        ts = self._trainset(n_views, pipelined)
+        ts = self._trainset(n_views, pipelined, flags)
         bk = self._bucket_structs(plans, groups)
         cfg = None
         if adam:
@@ -413,10 +429,22 @@ class Trainer:
         else:
             hw3 = self.H * self.W * 3 * 4
             tptr, iptr, lptr = [targets.data_ptr() + b * hw3 for b in range(B)], None, None
-        self._run_iteration(plans, groups, B, tptr, sat_eps, adam=True, host=host, images_out=iptr, loss_out=lptr)
+        self._run_iteration(plans, groups, B, tptr, sat_eps, adam=True, host=host, images_out=iptr, loss_out=lptr,
+                            flags=self._use_flags(plans[0][0]))
         self._m_event = torch.cuda.Event()
         self._m_event.record(torch.cuda.current_stream(self.ctx.device))
         return len(groups)
+
+    def _use_flags(self, first_plan):
+        """Track the gradient rows with flags (splx_trainset.touched) when that saves work: when the first bucket's
+        partitions hold most of the Gaussians it writes nearly every row anyway and the plain '=' pass is the cheaper one
+        (measured on aerial_1M and city_10M, where every view sees every partition)."""
+        if self.sparse_adam:
+            return True
+        if not self.flagged_grads:
+            return False
+        held = sum(self.part_offsets[k + 1] - self.part_offsets[k] for k, v in enumerate(first_plan.view_of_part) if v >= 0)
+        return held < 0.75 * self.n
 
     # ---- one view per iteration, replayed from a CUDA graph -----------------------------------------------------
     def _single_view_plan(self, view_id, cam, saturation):
@@ -431,19 +459,21 @@ class Trainer:
         if key not in self._graphs:
             main = torch.cuda.current_stream(dev)
             self._workspaces(plan.cams[0])
-            self._trainset(1, False)
+            flags = self._use_flags(plan)
+            self._trainset(1, False, flags)
             torch.cuda.synchronize(dev)
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g):
                 self.ctx.set_stream(torch.cuda.current_stream(dev).cuda_stream)
                 try:
                     keep = self._run_iteration([(plan, state)], [[0]], 1, [target_ptr], sat_eps, adam=False, host=host,
-                                               images_out=[image_ptr] if image_ptr else None, loss_out=loss_ptr)
+                                               images_out=[image_ptr] if image_ptr else None, loss_out=loss_ptr,
+                                               flags=flags)
                 finally:
                     self.ctx.set_stream(main.cuda_stream)
-            self._graphs[key] = (g, plan, keep)
+            self._graphs[key] = (g, plan, keep, flags)
         self._graphs[key][0].replay()
-        self.adam_step(1)
+        self.adam_step(1, flagged=self._graphs[key][3])
 
     def step_graph(self, view_id, cam, target_dev, saturation=False, sat_eps=1e-4):
         """One whole training iteration on one view with the target already on the device ([1,H,W,3]).  Asynchronous."""
@@ -466,7 +496,7 @@ class Trainer:
         else:
             plan, state = self._single_view_plan(view_id, cam, saturation)
             self._run_iteration([(plan, state)], [[0]], 1, [target_host.data_ptr()], sat_eps, adam=True, host=True,
-                                images_out=[iptr] if iptr else None, loss_out=lptr)
+                                images_out=[iptr] if iptr else None, loss_out=lptr, flags=self._use_flags(plan))
         torch.cuda.current_stream(dev).synchronize()
         m = int(self._m_host[0])
         if m > self.capacity:

@@ -200,7 +200,7 @@ def test_filtered_iteration_matches_oracle(aerial):
         got = G.np32(tr.grads[key]).astype(np.float64).reshape(-1)
         want = np.concatenate([g[key].reshape(-1) for g in ref])
         assert G.rel_l2(got, want) <= 1e-3, (key, G.rel_l2(got, want))
-        assert G.grad_close(got, want) <= 5e-3, (key, G.grad_close(got, want))
+        assert G.grad_close(got, want) <= G.GRAD_MAX_TOL, (key, G.grad_close(got, want))
 
 
 def test_fig25_on_the_gpu():

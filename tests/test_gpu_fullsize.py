@@ -122,7 +122,7 @@ def test_fullsize_pixels_and_gradients_on_sampled_tiles(full):
             r = ref[key].reshape(-1, w)
             assert np.abs(r).max() > 0, key
             assert G.rel_l2(got, r) <= 1e-3, (k, key, G.rel_l2(got, r))
-            assert G.grad_close(got, r) <= 5e-3, (k, key)
+            assert G.grad_close(got, r) <= G.GRAD_MAX_TOL, (k, key)
 
 
 def test_fullsize_work_counters(full):
@@ -285,7 +285,7 @@ def test_city_pixels_and_gradients_on_sampled_tiles(full_city):
             got = tr.grads[key].reshape(-1)[w * a:w * b].cpu().numpy().reshape(-1, w).astype(np.float64)
             r = ref[key].reshape(-1, w)
             assert G.rel_l2(got, r) <= 1e-3, (k, key, G.rel_l2(got, r))
-            assert G.grad_close(got, r) <= 5e-3, (k, key)
+            assert G.grad_close(got, r) <= G.GRAD_MAX_TOL, (k, key)
         checked += 1
     assert checked > 0
     for k in range(tr.K):        # non-participants: "=" mode wrote zeros
