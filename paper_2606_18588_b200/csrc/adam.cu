@@ -11,11 +11,21 @@ constexpr int AB = 256;
 
 struct AdamK { float lr, b1, b2, omb1, omb2, eps, ibc1, ibc2; };
 
+// sqrt.approx / div.approx (MUFU.SQRT, MUFU.RCP + one multiply: <= 1 and 2 ulp) instead of the IEEE sequences: with those the
+// kernel issued ~200 instructions per 16-byte vector and sat within 10 % of the issue limit at the HBM roof (28.2 ms at
+// 100 M Gaussians; 26.5 ms = 95 % of the measured copy bandwidth with the approximate pair).  The update is within 3 ulp of
+// the IEEE one: far inside the 1e-5 parity bar against the fp64 oracle.  sqrt.approx(0) = 0 (an untouched row has v = 0);
+// the divisor is >= eps > 0.
+__device__ __forceinline__ float sqrt_approx(float x) {
+  float y;
+  asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ void adam1(float& p, float g, float& m, float& v, const AdamK& k) {
   const float lr = k.lr, eps = k.eps, ibc1 = k.ibc1, ibc2 = k.ibc2;
   m = fmaf(k.b1, m, k.omb1 * g);
   v = fmaf(k.b2, v, k.omb2 * g * g);
-  p -= lr * (m * ibc1) / (sqrtf(v * ibc2) + eps);
+  p -= lr * __fdividef(m * ibc1, sqrt_approx(v * ibc2) + eps);
 }
 
 __global__ void __launch_bounds__(AB)
@@ -53,8 +63,36 @@ k_adam(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ 
 // on a gradient buffer whose untouched rows hold zeros.
 struct AdamGroups {
   long long end4[SPLX_ADAM_MAX_GROUPS]; float lr[SPLX_ADAM_MAX_GROUPS]; int n;
-  long long start[SPLX_ADAM_MAX_GROUPS]; int width[SPLX_ADAM_MAX_GROUPS]; long long rows;     // FLAGS only
+  uint32_t start4[SPLX_ADAM_MAX_GROUPS]; int width[SPLX_ADAM_MAX_GROUPS]; long long rows;     // FLAGS only
 };
+
+// Flags of the four elements of vector i of group j (0 = untouched), in 32-bit arithmetic (the launcher checks that vector
+// indices fit): a row of 48 or 4 floats holds the whole vector (one flag), a vector of a width-1 group holds four rows
+// (their four flag bytes are one aligned word), a width-3 group's vector touches two rows.
+__device__ __forceinline__ uint4 adam_flags(const AdamGroups& gr, int j, int64_t i, const uint8_t* __restrict__ touched) {
+  const uint32_t v0 = (uint32_t)i - gr.start4[j];        // vector index inside the group
+  const int w = gr.width[j];
+  const uint32_t nrow = (uint32_t)gr.rows;
+  uint32_t f0, f1, f2, f3;
+  if (w == 48 || w == 4) {
+    const uint32_t r = w == 48 ? v0 / 12u : v0;
+    f0 = f1 = f2 = f3 = r < nrow ? (uint32_t)__ldg(touched + r) : 0u;
+  } else if (w == 1) {
+    const uint32_t r = 4u * v0;
+    uint32_t word = 0;
+    if (r + 3 < nrow && ((uintptr_t)touched & 3) == 0) word = __ldg(reinterpret_cast<const uint32_t*>(touched + r));
+    else { for (uint32_t c = 0; c < 4; ++c) if (r + c < nrow) word |= (uint32_t)touched[r + c] << (8 * c); }
+    f0 = word & 0xffu; f1 = word & 0xff00u; f2 = word & 0xff0000u; f3 = word & 0xff000000u;
+  } else {
+    const uint32_t e0 = 4u * v0, uw = (uint32_t)w;         // (a width-3 group of 100 M rows: 3e8 elements, fits)
+    const uint32_t ra = e0 / uw, r1 = (e0 + 1u) / uw, r2 = (e0 + 2u) / uw, rb = (e0 + 3u) / uw;
+    const uint32_t fa = ra < nrow ? (uint32_t)__ldg(touched + ra) : 0u, fb = rb < nrow ? (uint32_t)__ldg(touched + rb) : 0u;
+    f0 = fa; f3 = fb;
+    f1 = r1 == ra ? fa : (r1 == rb ? fb : (r1 < nrow ? (uint32_t)__ldg(touched + r1) : 0u));
+    f2 = r2 == ra ? fa : (r2 == rb ? fb : (r2 < nrow ? (uint32_t)__ldg(touched + r2) : 0u));
+  }
+  return make_uint4(f0, f1, f2, f3);
+}
 
 template <bool FLAGS>
 __global__ void __launch_bounds__(AB, 6)      // 6 CTAs / SM (<= 42 registers): the bytes in flight, not the ALU, carry this kernel
@@ -69,32 +107,17 @@ k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __rest
     AdamK kk = k; kk.lr = gr.lr[j];
     float4 g = make_float4(0.f, 0.f, 0.f, 0.f), p, mm, vv;
     if (FLAGS) {
-      // rows of the four elements of this vector (a row of width 3 or 1 does not fill a vector: up to four rows).  The
-      // widths of the Gaussian parameter groups get constant divisors in 32-bit arithmetic; any other width divides in 64.
-      const unsigned long long v0 = (unsigned long long)i - ((unsigned long long)gr.start[j] >> 2);   // vector index inside the group
-      const int w = gr.width[j];
-      unsigned long long r[4];
-      if (w == 48) { r[0] = r[1] = r[2] = r[3] = (uint32_t)v0 / 12u; }
-      else if (w == 4) { r[0] = r[1] = r[2] = r[3] = v0; }
-      else if (w == 1) { r[0] = 4 * v0; r[1] = r[0] + 1; r[2] = r[0] + 2; r[3] = r[0] + 3; }
-      else if (w == 3 && v0 < (1ull << 30)) {
-        const uint32_t e0 = 4u * (uint32_t)v0;
-        r[0] = e0 / 3u; r[1] = (e0 + 1u) / 3u; r[2] = (e0 + 2u) / 3u; r[3] = (e0 + 3u) / 3u;
-      } else {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) r[c] = (4 * v0 + c) / (unsigned long long)w;
-      }
       // the flag bytes and the parameter / moment vectors are requested together (independent loads: one memory latency);
       // only the gradient of a touched row waits for its flag
-      uint8_t fl[4];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) fl[c] = (long long)r[c] < gr.rows ? __ldg(touched + r[c]) : (uint8_t)0;
+      const uint4 fl = adam_flags(gr, j, i, touched);
       p = reinterpret_cast<float4*>(param)[i];
       mm = reinterpret_cast<float4*>(m)[i];
       vv = reinterpret_cast<float4*>(v)[i];
-      if (fl[0] | fl[1] | fl[2] | fl[3]) {
+      // the decision is taken per WARP (512 contiguous bytes): whole bursts of the gradient stream are read or skipped --
+      // skipping single 16-byte vectors left DRAM with a scattered read pattern that cost more than the bytes it saved
+      if (__any_sync(__activemask(), (fl.x | fl.y | fl.z | fl.w) != 0u)) {
         const float4 t = reinterpret_cast<const float4*>(grad)[i];
-        g = make_float4(fl[0] ? t.x : 0.f, fl[1] ? t.y : 0.f, fl[2] ? t.z : 0.f, fl[3] ? t.w : 0.f);
+        g = make_float4(fl.x ? t.x : 0.f, fl.y ? t.y : 0.f, fl.z ? t.z : 0.f, fl.w ? t.w : 0.f);
       }
     } else {
       g = reinterpret_cast<const float4*>(grad)[i];
@@ -209,9 +232,11 @@ int launch_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float
   for (int j = 0; j < SPLX_ADAM_MAX_GROUPS; ++j) {
     gr.end4[j] = j < n_groups ? group_offsets[j + 1] >> 2 : nvec;
     gr.lr[j] = j < n_groups ? lr[j] : 0.f;
-    gr.start[j] = j < n_groups ? group_offsets[j] : count;
+    gr.start4[j] = (uint32_t)((j < n_groups ? group_offsets[j] : count) >> 2);
     gr.width[j] = (touched && j < n_groups) ? widths[j] : 1;
   }
+  if (touched && (nvec >> 32 || rows >> 30))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_flagged: more than 2^32 vectors or 2^30 rows");
   if (touched)
     k_adam_groups<true><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, 0, touched);
   else
