@@ -147,9 +147,9 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     }
     const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
     uint32_t v[SCAN_IPT], s = 0;
-    const typename Op::Cursor cur = op.cursor(base < n ? base : 0);      // the thread's SCAN_IPT elements are consecutive
+    op.load_all(base, n, v);                 // the thread's SCAN_IPT elements are consecutive
 #pragma unroll
-    for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? op.load(cur, base, k) : 0; s += v[k]; }
+    for (int k = 0; k < SCAN_IPT; ++k) s += v[k];
     uint32_t total;
     uint32_t ex = block_exclusive_scan(s, sm, total);
     if (threadIdx.x == 0) {
@@ -165,8 +165,7 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     }
     __syncthreads();
     ex += (uint32_t)s_excl;
-#pragma unroll
-    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < n) op.store(cur, base, k, v[k], ex, s_hist); ex += v[k]; }
+    op.store_all(base, n, v, ex, s_hist);
   }
   if (HIST) {
     __syncthreads();
@@ -189,31 +188,57 @@ struct RunMap {
 
 struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order preserved
   const uint32_t* tiles_touched; const float* depth; uint32_t* ckeys; uint32_t* cvals; uint32_t* vis_list; uint64_t n; RunMap map;
-  struct Cursor {};
   __device__ uint64_t count(const uint64_t*) const { return n; }
-  __device__ Cursor cursor(uint64_t) const { return Cursor{}; }
-  __device__ uint64_t index(const Cursor& c, uint64_t base, int k) const {
-    return map(base + k);     // a <= 6-step search over the run starts (uniform across a warp: constant-bank loads)
+  // A thread's SCAN_IPT elements are consecutive positions j of the concatenated runs: the run of the first one is
+  // searched once (a <= 6-step search over the run starts: constant-bank loads), the Gaussian index then advances
+  // with j; only a thread that straddles two runs searches again.
+  __device__ void span(uint64_t base, uint64_t& gi0, uint32_t& rem) const {
+    int lo = 0, hi = map.n - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if ((uint64_t)map.jprefix[mid] <= base) lo = mid; else hi = mid - 1;
+    }
+    gi0 = (uint64_t)map.begin[lo] + (base - (uint64_t)map.jprefix[lo]);
+    const uint64_t left = (uint64_t)map.jprefix[lo + 1] - base;
+    rem = left < (uint64_t)SCAN_IPT ? (uint32_t)left : (uint32_t)SCAN_IPT;
   }
-  __device__ uint32_t load(const Cursor& c, uint64_t base, int k) const { return tiles_touched[index(c, base, k)] > 0 ? 1u : 0u; }
-  __device__ void store(const Cursor& c, uint64_t base, int k, uint32_t v, uint32_t ex, uint32_t* hist) const {
-    if (v) {
-      const uint64_t i = index(c, base, k);
-      const uint32_t key = __float_as_uint(depth[i]);
-      ckeys[ex] = key; cvals[ex] = (uint32_t)i;
-      vis_list[ex] = (uint32_t)i;      // the visible Gaussians in INDEX order (kept: the depth sort permutes cvals)
+  __device__ void load_all(uint64_t base, uint64_t cnt, uint32_t (&v)[SCAN_IPT]) const {
+    uint64_t gi0 = 0; uint32_t rem = 0;
+    if (base < cnt) span(base, gi0, rem);
 #pragma unroll
-      for (int p = 0; p < 4; ++p) atomicAdd(&hist[p * 256 + ((key >> (8 * p)) & 255u)], 1u);
+    for (int k = 0; k < SCAN_IPT; ++k) {
+      v[k] = 0;
+      if (base + k < cnt) v[k] = tiles_touched[(uint32_t)k < rem ? gi0 + k : map(base + k)] > 0 ? 1u : 0u;
+    }
+  }
+  __device__ void store_all(uint64_t base, uint64_t cnt, const uint32_t (&v)[SCAN_IPT], uint32_t ex, uint32_t* hist) const {
+    uint64_t gi0 = 0; uint32_t rem = 0;
+    if (base < cnt) span(base, gi0, rem);
+#pragma unroll
+    for (int k = 0; k < SCAN_IPT; ++k) {
+      if (base + k < cnt && v[k]) {
+        const uint64_t i = (uint32_t)k < rem ? gi0 + k : map(base + k);
+        const uint32_t key = __float_as_uint(depth[i]);
+        ckeys[ex] = key; cvals[ex] = (uint32_t)i;
+        vis_list[ex] = (uint32_t)i;      // the visible Gaussians in INDEX order (kept: the depth sort permutes cvals)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) atomicAdd(&hist[p * 256 + ((key >> (8 * p)) & 255u)], 1u);
+      }
+      ex += v[k];
     }
   }
 };
 struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, depth order
   const uint32_t* tiles_touched; const uint32_t* cvals; uint32_t* offs;
   __device__ uint64_t count(const uint64_t* n_ptr) const { return *n_ptr; }
-  struct Cursor {};
-  __device__ Cursor cursor(uint64_t) const { return Cursor{}; }
-  __device__ uint32_t load(const Cursor&, uint64_t base, int k) const { return tiles_touched[cvals[base + k]]; }
-  __device__ void store(const Cursor&, uint64_t base, int k, uint32_t, uint32_t ex, uint32_t*) const { offs[base + k] = ex; }
+  __device__ void load_all(uint64_t base, uint64_t cnt, uint32_t (&v)[SCAN_IPT]) const {
+#pragma unroll
+    for (int k = 0; k < SCAN_IPT; ++k) v[k] = base + k < cnt ? tiles_touched[cvals[base + k]] : 0u;
+  }
+  __device__ void store_all(uint64_t base, uint64_t cnt, const uint32_t (&v)[SCAN_IPT], uint32_t ex, uint32_t*) const {
+#pragma unroll
+    for (int k = 0; k < SCAN_IPT; ++k) { if (base + k < cnt) offs[base + k] = ex; ex += v[k]; }
+  }
 };
 
 template <class Op, bool HIST>
@@ -225,7 +250,7 @@ int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_pt
   if (nb > PERSISTENT_CTAS) nb = PERSISTENT_CTAS;
   k_scan<Op, HIST><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to, ghist,
                                                          rstatus, rstride);
-  SPLX_LAUNCH_CHECK(ctx, "k_scan");
+  SPLX_LAUNCH_CHECK(ctx, HIST ? "k_scan<VisibleOp>" : "k_scan<TouchedOp>");
   return SPLX_OK;
 }
 
@@ -326,7 +351,7 @@ struct FinalOut {
 template <typename KeyT, bool FINAL, bool FULL>
 __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
                                            uint32_t* __restrict__ vout, uint64_t start, uint32_t nv, uint32_t t, int shift,
-                                           uint32_t mask, uint64_t* status, const FinalOut& fin, uint32_t (*whist)[256],
+                                           int bits, uint32_t mask, uint64_t* status, const FinalOut& fin, uint32_t (*whist)[256],
                                            uint32_t* dbase, const uint32_t* gbase, uint32_t* lbase, KeyT* skey, uint32_t* sval,
                                            uint32_t* sm) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -352,8 +377,10 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
     unsigned peers = FULL ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
 #pragma unroll
     for (int b = 0; b < 8; ++b) {
-      const uint32_t bit = (d >> b) & 1u;
-      peers &= __ballot_sync(0xffffffffu, bit) ^ (bit - 1u);
+      if (b < bits) {            // (uniform) a pass of 5 or 6 bits -- 17 slot bits make passes of 6, 6, 5 -- votes on those only
+        const uint32_t bit = (d >> b) & 1u;
+        peers &= __ballot_sync(0xffffffffu, bit) ^ (bit - 1u);
+      }
     }
     uint32_t old = 0;
     const int leader = __ffs(peers) - 1;               // (an invalid lane: its own digit-0 group among the invalid ones; unused)
@@ -447,9 +474,9 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
     // the kernel is bound by instruction issue (ncu, city_100M: 62 % issue slots, DRAM 13 %): a full tile -- all but the
     // last one -- takes the copy of the body without the per-item range checks
     if (nv == RS_TILE)
-      radix_tile<KeyT, FINAL, true>(kin, vin, kout, vout, start, nv, t, shift, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+      radix_tile<KeyT, FINAL, true>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
     else
-      radix_tile<KeyT, FINAL, false>(kin, vin, kout, vout, start, nv, t, shift, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+      radix_tile<KeyT, FINAL, false>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
   }
 }
 
