@@ -281,6 +281,11 @@ typedef struct {
                                   (its Gaussians are not projected, binned, rendered or differentiated) */
   const uint8_t *tile_state;   /* DEVICE [K*tiles] or NULL (nothing skipped) */
   int32_t flags;
+  const float *max_scale;      /* HOST [K] or NULL: an upper bound of exp(log_scale) over the Gaussians of partition k.  Given,
+                                  splx_project_plan first tests a Gaussian's MEAN against the half spaces outside which no
+                                  Gaussian that small can reach the image (the cut of splx_visible_regions, reading s21) and
+                                  reads its scale and rotation only if it passes: 12 instead of 40 bytes for most culled
+                                  Gaussians.  Exact as long as the bound holds (a caller that trains refreshes it). */
 } splx_plan;
 
 /* Geometric visibility (L212, L227): HOST computation, no device work, ctx not needed.  n_boxes axis-aligned boxes

@@ -49,6 +49,10 @@ int make_plan_dev(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, 
     out->pv.v[k] = (signed char)v;
   }
   for (int k = K; k < SPLX_MAX_K; ++k) out->pv.v[k] = -1;
+  for (int k = 0; k < SPLX_MAX_K; ++k) {
+    out->max_scale[k] = (plan->max_scale && k < K) ? plan->max_scale[k] : -1.0f;
+    if (plan->max_scale && k < K && !(plan->max_scale[k] >= 0.f)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: max_scale[%d] must be >= 0", who, k);
+  }
   out->B = plan->n_views; out->K = K;
   out->W = out->cam[0].W; out->H = out->cam[0].H; out->TX = out->cam[0].TX; out->TY = out->cam[0].TY;
   out->ntiles = out->TX * out->TY;
@@ -70,6 +74,7 @@ struct SinglePlan {
   explicit SinglePlan(const splx_camera* cam) {
     for (int k = 0; k < SPLX_MAX_K; ++k) views[k] = 0;
     plan.n_views = 1; plan.cams = cam; plan.view_of_part = views; plan.tile_state = nullptr; plan.flags = 0;
+    plan.max_scale = nullptr;
   }
 };
 

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <math.h>
 #include <string.h>
 
 #include "../../include/splx.h"
@@ -31,6 +32,9 @@ struct CamDev {
   float near_z;
   float o[3];  // camera centre -R^T t
   float limx, limy;
+  // reach test of a mean (reading s21): a Gaussian of scale <= s can touch the image only if
+  //   -(reach_l z + 3 reach_c s) <= fx x <= reach_r z + 3 reach_c s   and the same with (reach_t, reach_b) for fy y
+  float reach_l, reach_r, reach_t, reach_b, reach_c;
 };
 
 static inline CamDev make_camdev(const splx_camera* c, const splx_config& cfg) {
@@ -46,6 +50,13 @@ static inline CamDev make_camdev(const splx_camera* c, const splx_config& cfg) {
     d.o[j] = -(c->R[0 * 3 + j] * c->t[0] + c->R[1 * 3 + j] * c->t[1] + c->R[2 * 3 + j] * c->t[2]);
   d.limx = cfg.lim_factor * (float)c->width / (2.0f * c->fx);
   d.limy = cfg.lim_factor * (float)c->height / (2.0f * c->fy);
+  {   // g = 2.5 + 3 sqrt(dilation + sqrt(radius_floor)) pixels, +0.5 and 1e-4 relative for the fp32 evaluation of the test
+    const double e = (double)cfg.dilation + sqrt((double)cfg.radius_floor), g = 3.0 + 3.0 * sqrt(e);
+    const double fm = c->fx > c->fy ? c->fx : c->fy;
+    d.reach_l = (float)((c->cx + g) * 1.0001); d.reach_r = (float)(((double)c->width - c->cx + g) * 1.0001);
+    d.reach_t = (float)((c->cy + g) * 1.0001); d.reach_b = (float)(((double)c->height - c->cy + g) * 1.0001);
+    d.reach_c = (float)(fm * sqrt(1.0 + (double)d.limx * d.limx + (double)d.limy * d.limy) * 1.0001);
+  }
   return d;
 }
 
@@ -60,6 +71,7 @@ struct PlanDev {
   const uint8_t* tile_state;
   PartView pv;
   CamDev cam[SPLX_MAX_VIEWS];
+  float max_scale[SPLX_MAX_K];   // splx_plan.max_scale, or < 0: no reach test
 };
 
 // Per-view buffers of the composition kernels (view b of the launch -> its own pointers), so that the views of a
@@ -107,6 +119,7 @@ struct RunTable {
   int64_t begin[SPLX_MAX_K], end[SPLX_MAX_K], jprefix[SPLX_MAX_K + 1];
   int block_prefix[SPLX_MAX_K + 1];
   signed char view[SPLX_MAX_K];
+  signed char part[SPLX_MAX_K];     // the partition of run r
 };
 
 static inline RunTable make_runs(const PlanDev& plan, const int64_t* part_offsets, int block, bool with_inactive) {
@@ -117,7 +130,7 @@ static inline RunTable make_runs(const PlanDev& plan, const int64_t* part_offset
     const int64_t b = part_offsets[k], e = part_offsets[k + 1];
     if (e <= b || (v < 0 && !with_inactive)) continue;
     const int r = rt.n++;
-    rt.begin[r] = b; rt.end[r] = e; rt.view[r] = (signed char)v;
+    rt.begin[r] = b; rt.end[r] = e; rt.view[r] = (signed char)v; rt.part[r] = (signed char)k;
     rt.jprefix[r + 1] = rt.jprefix[r] + (e - b);
     rt.block_prefix[r + 1] = rt.block_prefix[r] + (int)((e - b + block - 1) / block);
   }

@@ -18,56 +18,57 @@ namespace {
 
 constexpr int CB = SPLX_TILE * SPLX_TILE;
 
-// s_use[k] = 1 iff partition k is composed into view b on this tile.
+// s_list[0 .. *s_n) = the partitions composed into view b on this tile (they render view b and, with SPLX_PLAN_SPARSE, have a
+// non-empty list here), in ascending order.  Built by the first warp: lane l looks at partitions l and l + 32.
 __device__ __forceinline__ void tile_participants(const PartView& pv, int K, int b, int tile, int ntiles, int sparse,
-                                                  const uint32_t* __restrict__ ranges, uint8_t* s_use) {
-  for (int k = threadIdx.x; k < K; k += CB) {
-    bool use = pv.v[k] == b;
-    if (use && sparse) {
-      const uint2 r = *reinterpret_cast<const uint2*>(ranges + 2 * ((size_t)k * ntiles + tile));
-      use = r.x < r.y;
+                                                  const uint32_t* __restrict__ ranges, uint8_t* s_list, int* s_n) {
+  if (threadIdx.x < 32) {
+    const int lane = threadIdx.x;
+    bool use[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int k = lane + 32 * h;
+      use[h] = k < K && pv.v[k] == b;
+      if (use[h] && sparse) {
+        const uint2 r = *reinterpret_cast<const uint2*>(ranges + 2 * ((size_t)k * ntiles + tile));
+        use[h] = r.x < r.y;
+      }
     }
-    s_use[k] = use ? 1 : 0;
+    const unsigned b0 = __ballot_sync(0xffffffffu, use[0]), b1 = __ballot_sync(0xffffffffu, use[1]);
+    const unsigned lt = (1u << lane) - 1u;
+    if (use[0]) s_list[__popc(b0 & lt)] = (uint8_t)lane;
+    if (use[1]) s_list[__popc(b0) + __popc(b1 & lt)] = (uint8_t)(lane + 32);
+    if (lane == 0) *s_n = __popc(b0) + __popc(b1);
   }
   __syncthreads();
 }
 
-// Collect the live partials of one pixel, sorted by (key, k).  Returns the count.
+// Collect the live partials of one pixel, sorted by (key, k).  Returns the count.  The candidates (the tile's
+// participants: ~1-6 of up to 64 partitions) are fetched eight at a time, every T and D of a chunk first -- predicated,
+// independent loads: one memory latency per chunk instead of a chain of dependent ones (the kernel was bound by that
+// chain, profiles/r01e_ncu_full.md; round 1 had the up-front fetch for K <= 8 only, the city configurations run K = 16, 32).
 template <int KMAX>
-__device__ __forceinline__ int ordered_live(const float* __restrict__ ct, const float* __restrict__ d, int K,
-                                            const uint8_t* s_use, size_t HW, size_t pix, float (&key)[KMAX],
-                                            int (&idx)[KMAX]) {
+__device__ __forceinline__ int ordered_live(const float* __restrict__ ct, const float* __restrict__ d, const uint8_t* s_list,
+                                            int n_use, size_t HW, size_t pix, float (&key)[KMAX], int (&idx)[KMAX]) {
   int L = 0;
-  if (KMAX <= 8) {
-    // Few partitions: fetch every T and D first (predicated, independent loads: one memory latency instead of a
-    // chain of 2 K dependent ones -- the kernel was bound by that chain, profiles/r01e_ncu_full.md), then order them.  (A
-    // register-only sorting network with fully unrolled loops was measured too: 74 registers, 0.084 ms against 0.047.)
-    float Tk[KMAX], dk[KMAX];
+  for (int c0 = 0; c0 < n_use; c0 += 8) {
+    float Tk[8], dk[8];
+    int kk[8];
 #pragma unroll
-    for (int k = 0; k < KMAX; ++k) {
-      const bool u = k < K && s_use[k];
-      Tk[k] = u ? __ldg(ct + 4 * ((size_t)k * HW + pix) + 3) : 1.0f;
-      dk[k] = u ? __ldg(d + (size_t)k * HW + pix) : 0.0f;
+    for (int j = 0; j < 8; ++j) {
+      const bool u = c0 + j < n_use;
+      kk[j] = u ? (int)s_list[c0 + j] : 0;
+      Tk[j] = u ? __ldg(ct + 4 * ((size_t)kk[j] * HW + pix) + 3) : 1.0f;
+      dk[j] = u ? __ldg(d + (size_t)kk[j] * HW + pix) : 0.0f;
     }
 #pragma unroll
-    for (int k = 0; k < KMAX; ++k) {
-      if (Tk[k] < 1.0f) {
-        const float kk = __fdiv_rn(dk[k], __fsub_rn(1.0f, Tk[k]));
+    for (int j = 0; j < 8; ++j) {
+      if (Tk[j] < 1.0f) {
+        const float kv = __fdiv_rn(dk[j], __fsub_rn(1.0f, Tk[j]));
         int p = L++;
-        while (p > 0 && key[p - 1] > kk) { key[p] = key[p - 1]; idx[p] = idx[p - 1]; --p; }
-        key[p] = kk; idx[p] = k;
+        while (p > 0 && key[p - 1] > kv) { key[p] = key[p - 1]; idx[p] = idx[p - 1]; --p; }    // stable: '>' keeps smaller k first
+        key[p] = kv; idx[p] = kk[j];
       }
-    }
-    return L;
-  }
-  for (int k = 0; k < K; ++k) {
-    if (!s_use[k]) continue;
-    const float T = __ldg(ct + 4 * ((size_t)k * HW + pix) + 3);
-    if (T < 1.0f) {
-      const float kk = __fdiv_rn(__ldg(d + (size_t)k * HW + pix), __fsub_rn(1.0f, T));
-      int p = L++;
-      while (p > 0 && key[p - 1] > kk) { key[p] = key[p - 1]; idx[p] = idx[p - 1]; --p; }  // stable: '>' keeps smaller k first
-      key[p] = kk; idx[p] = k;
     }
   }
   return L;
@@ -79,11 +80,12 @@ k_compose_fwd(const float* __restrict__ ct, const float* __restrict__ d, const u
               const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
               float bg1, float bg2, const __grid_constant__ ViewBufs vb, float sat_eps,
               const uint8_t* __restrict__ state_in, uint8_t* __restrict__ state_out) {
-  __shared__ uint8_t s_use[SPLX_MAX_K];
+  __shared__ uint8_t s_list[SPLX_MAX_K];
+  __shared__ int s_n;
   __shared__ unsigned s_unsat[2];
   const int tile = blockIdx.x, b = blockIdx.y;
   if (SAT && threadIdx.x < 2) s_unsat[threadIdx.x] = 0u;
-  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
+  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_list, &s_n);
   const int x = (tile % TX) * SPLX_TILE + (threadIdx.x & 15), y = (tile / TX) * SPLX_TILE + (threadIdx.x >> 4);
   const size_t HW = (size_t)W * H;
   const bool inside = x < W && y < H;
@@ -91,7 +93,7 @@ k_compose_fwd(const float* __restrict__ ct, const float* __restrict__ d, const u
   if (inside) {
     const size_t pix = (size_t)y * W + x;
     float key[KMAX]; int idx[KMAX];
-    const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
+    const int L = ordered_live<KMAX>(ct, d, s_list, s_n, HW, pix, key, idx);
     float Tacc = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
     unsigned long long live = 0ull;
     for (int m = 0; m < L; ++m) {
@@ -128,14 +130,15 @@ __global__ void __launch_bounds__(CB)
 k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, const uint32_t* __restrict__ ranges,
               const __grid_constant__ PartView pv, int K, int W, int H, int TX, int ntiles, int sparse, float bg0,
               float bg1, float bg2, const __grid_constant__ ViewBufs vb, float* __restrict__ g_ct) {
-  __shared__ uint8_t s_use[SPLX_MAX_K];
+  __shared__ uint8_t s_list[SPLX_MAX_K];
+  __shared__ int s_n;
   const int tile = blockIdx.x, b = blockIdx.y;
-  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
+  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_list, &s_n);
   const int x = (tile % TX) * SPLX_TILE + (threadIdx.x & 15), y = (tile / TX) * SPLX_TILE + (threadIdx.x >> 4);
   if (x >= W || y >= H) return;
   const size_t HW = (size_t)W * H, pix = (size_t)y * W + x;
   float key[KMAX]; int idx[KMAX];
-  const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
+  const int L = ordered_live<KMAX>(ct, d, s_list, s_n, HW, pix, key, idx);
   const float* gi = vb.g_image[b] + 3 * pix;
   const float g0 = gi[0], g1 = gi[1], g2 = gi[2];
   const float gT = vb.g_T_total[b] ? vb.g_T_total[b][pix] : 0.f;
@@ -144,10 +147,11 @@ k_compose_bwd(const float* __restrict__ ct, const float* __restrict__ d, const u
   for (int m = 0; m < L; ++m) Ttot *= __ldg(ct + 4 * ((size_t)idx[m] * HW + pix) + 3);
   // Empty partials stand behind all live ones: Tfront = T_total, Behind = bg, BehindT = 1.
   const float4 ge = make_float4(Ttot * g0, Ttot * g1, Ttot * g2, Ttot * (g0 * bg0 + g1 * bg1 + g2 * bg2 + gT));
-  for (int k = 0; k < K; ++k) {
-    if (!s_use[k]) continue;
-    const float T = __ldg(ct + 4 * ((size_t)k * HW + pix) + 3);
-    if (!(T < 1.0f)) reinterpret_cast<float4*>(g_ct)[(size_t)k * HW + pix] = ge;
+  unsigned long long live = 0ull;
+  for (int m = 0; m < L; ++m) live |= 1ull << idx[m];
+  for (int j = 0; j < s_n; ++j) {
+    const int k = s_list[j];
+    if (!((live >> k) & 1ull)) reinterpret_cast<float4*>(g_ct)[(size_t)k * HW + pix] = ge;
   }
   // Live partials, back to front: Tfront_m = T_total / prod_{r>=m} T_r is avoided (no division):
   // recompute the prefix products front to back into key[] (the keys are no longer needed).
@@ -175,12 +179,13 @@ k_compose_fused(const float* __restrict__ ct, const float* __restrict__ d, const
                 float bg1, float bg2, const __grid_constant__ ViewBufs vb, float gscale, double* loss_sum,
                 float* __restrict__ g_ct, float sat_eps, const uint8_t* __restrict__ state_in,
                 uint8_t* __restrict__ state_out) {
-  __shared__ uint8_t s_use[SPLX_MAX_K];
+  __shared__ uint8_t s_list[SPLX_MAX_K];
+  __shared__ int s_n;
   __shared__ unsigned s_unsat[2];
   __shared__ float s_loss[CB / 32];
   const int tile = blockIdx.x, b = blockIdx.y;
   if (SAT && threadIdx.x < 2) s_unsat[threadIdx.x] = 0u;
-  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_use);
+  tile_participants(pv, K, b, tile, ntiles, sparse, ranges, s_list, &s_n);
   const int x = (tile % TX) * SPLX_TILE + (threadIdx.x & 15), y = (tile / TX) * SPLX_TILE + (threadIdx.x >> 4);
   const size_t HW = (size_t)W * H;
   const bool inside = x < W && y < H;
@@ -189,7 +194,7 @@ k_compose_fused(const float* __restrict__ ct, const float* __restrict__ d, const
   if (inside) {
     const size_t pix = (size_t)y * W + x;
     float key[KMAX]; int idx[KMAX];
-    const int L = ordered_live<KMAX>(ct, d, K, s_use, HW, pix, key, idx);
+    const int L = ordered_live<KMAX>(ct, d, s_list, s_n, HW, pix, key, idx);
     float Tacc = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
     unsigned long long live = 0ull;
     for (int m = 0; m < L; ++m) {
@@ -215,8 +220,10 @@ k_compose_fused(const float* __restrict__ ct, const float* __restrict__ d, const
     const float g2 = e2 > 0.f ? gscale : (e2 < 0.f ? -gscale : 0.f);
     // a8: identity partials stand behind all live ones
     const float4 ge = make_float4(Ttot * g0, Ttot * g1, Ttot * g2, Ttot * (g0 * bg0 + g1 * bg1 + g2 * bg2));
-    for (int k = 0; k < K; ++k)
-      if (s_use[k] && !((live >> k) & 1ull)) reinterpret_cast<float4*>(g_ct)[(size_t)k * HW + pix] = ge;
+    for (int j = 0; j < s_n; ++j) {
+      const int k = s_list[j];
+      if (!((live >> k) & 1ull)) reinterpret_cast<float4*>(g_ct)[(size_t)k * HW + pix] = ge;
+    }
     float B0 = bg0, B1 = bg1, B2 = bg2;
     for (int m = L - 1; m >= 0; --m) {
       const float4 p = __ldg(reinterpret_cast<const float4*>(ct) + (size_t)idx[m] * HW + pix);

@@ -197,8 +197,27 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   bool vis = false;
   if (active) {
     Geo G;
-    const GeoIn gin = load_geo(g, i);
-    vis = geometry(gin, cam, cfg.dilation, G);
+    GeoIn gin;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) gin.m[k] = g.mean[3 * i + k];
+    // reach test on the mean alone (splx_plan.max_scale, reading s21): most Gaussians of a city view fail it, and their
+    // scale and rotation (28 of the 40 bytes a culled Gaussian costs) are never read
+    bool reach = true;
+    const float smax = plan.max_scale[rt.part[r]];
+    if (smax >= 0.f) {
+      const float x = cam.R[0] * gin.m[0] + cam.R[1] * gin.m[1] + cam.R[2] * gin.m[2] + cam.t[0];
+      const float y = cam.R[3] * gin.m[0] + cam.R[4] * gin.m[1] + cam.R[5] * gin.m[2] + cam.t[1];
+      const float z = cam.R[6] * gin.m[0] + cam.R[7] * gin.m[1] + cam.R[8] * gin.m[2] + cam.t[2];
+      const float h = 3.0f * cam.reach_c * smax, fxx = cam.fx * x, fyy = cam.fy * y;
+      reach = z > cam.near_z * 0.999f && fxx <= cam.reach_r * z + h && -fxx <= cam.reach_l * z + h &&
+              fyy <= cam.reach_b * z + h && -fyy <= cam.reach_t * z + h;
+    }
+    if (reach) {
+#pragma unroll
+      for (int k = 0; k < 3; ++k) gin.ls[k] = g.log_scale[3 * i + k];
+      gin.q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
+      vis = geometry(gin, cam, cfg.dilation, G);
+    }
     float u = 0.f, v = 0.f;
     int rad = 0, tt = 0;
     if (vis) {

@@ -21,6 +21,13 @@ namespace {
 constexpr int SCAN_THREADS = 512, SCAN_IPT = 8, SCAN_TILE = SCAN_THREADS * SCAN_IPT;   // 4096 elements per tile
 constexpr int RS_THREADS = 256, RS_IPT = 8, RS_TILE = RS_THREADS * RS_IPT, RS_WARPS = 8;  // 2048
 constexpr int MAX_PASSES = 4;
+// Digit values of the slot sort.  512 (9-bit digits: <= 18 compact slot bits in two passes instead of three) is implemented
+// (radix_tile<..., 512>: two digits per thread in the per-digit phases) and was MEASURED SLOWER everywhere: bin/sort
+// 11.9 -> 12.8 ms on city_100M and 13.3 -> 15.0 ms on city_40M although a pass is saved there, 0.32 -> 0.37 ms on
+// aerial_1M and 2.8 -> 3.6 ms on city_10M where none is (twice the look-back chains per thread, 512 status words per
+// 2048-key tile, 39 KB of shared memory).  256 stays.
+constexpr int SLOT_NB = 256;
+constexpr int SLOT_BITS = SLOT_NB == 256 ? 8 : 9;
 static_assert(SCAN_TILE % RS_TILE == 0, "the compaction scan clears the radix status words of the tiles it covers");
 constexpr int SCAN_RS = SCAN_TILE / RS_TILE;
 constexpr uint32_t PERSISTENT_CTAS = SPLX_SM_COUNT * 8;   // grid of the persistent kernels: 8 CTAs per SM
@@ -263,10 +270,10 @@ int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_pt
 
 struct PassPlan { int npass; int shift[MAX_PASSES]; int bits[MAX_PASSES]; };
 
-static PassPlan plan_passes(int begin_bit, int end_bit) {
+static PassPlan plan_passes(int begin_bit, int end_bit, int max_bits = 8) {
   PassPlan p;
   const int total = end_bit - begin_bit;
-  p.npass = (total + 7) / 8;
+  p.npass = (total + max_bits - 1) / max_bits;
   int shift = begin_bit;
   for (int i = 0; i < p.npass; ++i) {
     p.bits[i] = (total + p.npass - 1 - i) / p.npass;   // spread the bits evenly over the passes
@@ -290,50 +297,6 @@ __device__ __forceinline__ unsigned digit_peers(uint32_t d, unsigned vm) {
   return peers;
 }
 
-// Grid-stride over the tiles (sized for the machine, not for the capacity).  The CTA that counts tile t also
-// clears the look-back status words of tile t for every pass, so the status arrays -- sized by the caller's
-// capacity -- never need a memset: only the part the actual count reaches is ever touched.
-template <typename KeyT>
-__global__ void __launch_bounds__(RS_THREADS)
-k_radix_hist_all(const KeyT* __restrict__ keys, const uint64_t* n_ptr, uint32_t* __restrict__ ghist /*[npass][256]*/,
-                 uint64_t* __restrict__ status, size_t status_stride, PassPlan plan) {
-  __shared__ uint32_t hist[RS_WARPS][MAX_PASSES][256];   // warp-private: plain read-modify-write by group leaders
-  const uint64_t n = *n_ptr;
-  const uint64_t ntiles = (n + RS_TILE - 1) / RS_TILE;
-  if (blockIdx.x >= ntiles) return;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int p = 0; p < plan.npass; ++p)
-#pragma unroll
-    for (int w = 0; w < RS_WARPS; ++w) hist[w][p][threadIdx.x] = 0;
-  __syncthreads();
-  for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
-    for (int p = 0; p < plan.npass; ++p) status[(size_t)p * status_stride + t * 256 + threadIdx.x] = 0;
-    const uint64_t start = t * RS_TILE;
-#pragma unroll 2
-    for (int it = 0; it < RS_IPT; ++it) {
-      const uint64_t idx = start + (uint64_t)it * RS_THREADS + threadIdx.x;
-      const bool valid = idx < n;
-      const unsigned vm = __ballot_sync(0xffffffffu, valid);
-      const KeyT key = valid ? keys[idx] : (KeyT)0;
-      for (int p = 0; p < plan.npass; ++p) {
-        const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
-        const unsigned peers = digit_peers(d, vm);
-        if (valid && lane == __ffs(peers) - 1) hist[warp][p][d] += __popc(peers);
-        __syncwarp();
-      }
-    }
-  }
-  __syncthreads();
-  for (int p = 0; p < plan.npass; ++p) {
-    uint32_t c = 0;
-#pragma unroll
-    for (int w = 0; w < RS_WARPS; ++w) c += hist[w][p][threadIdx.x];
-    if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c);
-  }
-}
-
-// Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
-// started and the look-back spin cannot wait on a CTA that was never scheduled.
 // The LAST pass of the slot sort writes the binning itself: its 32-bit items are (compact slot, position j in the
 // depth-sorted list of visible Gaussians); the 64-bit key (true slot << 32 | depth bits of j) and the value (Gaussian
 // index of j) are formed on the way out, from two arrays of N_visible entries that sit in L2.  The passes before it
@@ -347,13 +310,16 @@ struct FinalOut {
 
 // One tile of a radix pass (RS_TILE keys of one CTA): stable ranks by warp multisplit, the tile's keys reordered in
 // shared memory, the per-digit prefix over the tiles by look-back, the scatter.  FULL: every one of the RS_TILE
-// positions holds a key.
-template <typename KeyT, bool FINAL, bool FULL>
+// positions holds a key.  NB = number of digit values (256: 8-bit digits; 512: 9-bit digits, two per thread in the
+// per-digit phases -- 17 or 18 slot bits then take two passes instead of three).
+template <typename KeyT, bool FINAL, bool FULL, int NB>
 __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
                                            uint32_t* __restrict__ vout, uint64_t start, uint32_t nv, uint32_t t, int shift,
-                                           int bits, uint32_t mask, uint64_t* status, const FinalOut& fin, uint32_t (*whist)[256],
+                                           int bits, uint32_t mask, uint64_t* status, const FinalOut& fin, uint32_t (*whist)[NB],
                                            uint32_t* dbase, const uint32_t* gbase, uint32_t* lbase, KeyT* skey, uint32_t* sval,
                                            uint32_t* sm) {
+  constexpr int DPT = NB / RS_THREADS;      // digits per thread: thread x owns digits DPT x .. DPT x + DPT - 1
+  constexpr int MAXB = NB == 256 ? 8 : 9;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
   // warp w owns the contiguous segment [w*256, +256) of the tile; iteration `it` covers 32 consecutive
@@ -376,8 +342,8 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
     // lanes of the warp with this lane's digit: one ballot per digit bit; (bit - 1) is all ones for a clear bit
     unsigned peers = FULL ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
 #pragma unroll
-    for (int b = 0; b < 8; ++b) {
-      if (b < bits) {            // (uniform) a pass of 5 or 6 bits -- 17 slot bits make passes of 6, 6, 5 -- votes on those only
+    for (int b = 0; b < MAXB; ++b) {
+      if (b < bits) {            // (uniform) a pass of fewer bits votes on those only
         const uint32_t bit = (d >> b) & 1u;
         peers &= __ballot_sync(0xffffffffu, bit) ^ (bit - 1u);
       }
@@ -390,15 +356,21 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
     __syncwarp();
   }
   __syncthreads();
-  uint32_t run = 0;   // per digit (thread d): exclusive prefix over the warps, tile total
-  {
-    const int d = threadIdx.x;
+  uint32_t run[DPT];   // per digit: exclusive prefix over the warps (left in whist), tile total
+  uint32_t rsum = 0;
 #pragma unroll
-    for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
+  for (int q = 0; q < DPT; ++q) {
+    const int d = DPT * threadIdx.x + q;
+    run[q] = 0;
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run[q]; run[q] += c; }
+    rsum += run[q];
   }
   {  // position of digit d's first key inside the tile, in digit order
     uint32_t tot;
-    lbase[threadIdx.x] = block_exclusive_scan(run, sm, tot);
+    uint32_t ex = block_exclusive_scan(rsum, sm, tot);
+#pragma unroll
+    for (int q = 0; q < DPT; ++q) { lbase[DPT * threadIdx.x + q] = ex; ex += run[q]; }
   }
   __syncthreads();
   // the tile's keys go to shared memory in digit order, so that the scatter below writes runs of consecutive
@@ -411,12 +383,14 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
       sval[lp] = val[it];
     }
   }
-  {  // chained prefix over the tiles (look-back), one chain per digit
-    const int d = threadIdx.x;
+  // chained prefix over the tiles (look-back), one chain per digit
+#pragma unroll
+  for (int q = 0; q < DPT; ++q) {
+    const int d = DPT * threadIdx.x + q;
     uint64_t excl = 0;
     uint64_t* st = status + d;
-    if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run);
-    else excl = lookback<8>(st, t, 256, run);
+    if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run[q]);
+    else excl = lookback<8>(st, t, NB, run[q]);
     dbase[d] = gbase[d] + (uint32_t)excl - lbase[d];      // global position = dbase[d] + position in the tile
   }
   __syncthreads();
@@ -440,15 +414,18 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
   }
 }
 
-template <typename KeyT, bool FINAL>
+// Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
+// started and the look-back spin cannot wait on a CTA that was never scheduled.
+template <typename KeyT, bool FINAL, int NB>
 __global__ void __launch_bounds__(RS_THREADS, 4)
 k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
-             uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
-             uint64_t* status /*[tiles][256]*/, uint32_t* ticket, int shift, int bits, const __grid_constant__ FinalOut fin) {
-  __shared__ uint32_t whist[RS_WARPS][256];
-  __shared__ uint32_t dbase[256];
-  __shared__ uint32_t gbase[256];
-  __shared__ uint32_t lbase[256];
+             uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[NB] of this pass*/,
+             uint64_t* status /*[tiles][NB]*/, uint32_t* ticket, int shift, int bits, const __grid_constant__ FinalOut fin) {
+  constexpr int DPT = NB / RS_THREADS;
+  __shared__ uint32_t whist[RS_WARPS][NB];
+  __shared__ uint32_t dbase[NB];
+  __shared__ uint32_t gbase[NB];
+  __shared__ uint32_t lbase[NB];
   __shared__ KeyT skey[RS_TILE];
   __shared__ uint32_t sval[RS_TILE];
   __shared__ uint32_t sm[33];
@@ -458,14 +435,20 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
   if (blockIdx.x >= ntiles) return;
   const uint32_t mask = (1u << bits) - 1u;
   {  // exclusive scan of the global digit histogram = first output position of each digit (once per CTA)
-    uint32_t tot;
-    gbase[threadIdx.x] = block_exclusive_scan(ghist[threadIdx.x], sm, tot);
+    uint32_t g[DPT], gs = 0, tot;
+#pragma unroll
+    for (int q = 0; q < DPT; ++q) { g[q] = ghist[DPT * threadIdx.x + q]; gs += g[q]; }
+    uint32_t ex = block_exclusive_scan(gs, sm, tot);
+#pragma unroll
+    for (int q = 0; q < DPT; ++q) { gbase[DPT * threadIdx.x + q] = ex; ex += g[q]; }
   }
   for (;;) {
     __syncthreads();                       // the previous round no longer reads whist / dbase / s_tile
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
 #pragma unroll
-    for (int w = 0; w < RS_WARPS; ++w) whist[w][threadIdx.x] = 0;
+    for (int w = 0; w < RS_WARPS; ++w)
+#pragma unroll
+      for (int q = 0; q < DPT; ++q) whist[w][DPT * threadIdx.x + q] = 0;
     __syncthreads();
     const uint32_t t = s_tile;
     if (t >= ntiles) return;
@@ -474,41 +457,36 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
     // the kernel is bound by instruction issue (ncu, city_100M: 62 % issue slots, DRAM 13 %): a full tile -- all but the
     // last one -- takes the copy of the body without the per-item range checks
     if (nv == RS_TILE)
-      radix_tile<KeyT, FINAL, true>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+      radix_tile<KeyT, FINAL, true, NB>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
     else
-      radix_tile<KeyT, FINAL, false>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+      radix_tile<KeyT, FINAL, false, NB>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
   }
 }
 
-// Sorts bits [begin_bit, end_bit) in passes of <= 8 bits.  Input in (ka, va); buffers alternate
+// Sorts bits [begin_bit, end_bit) in passes of <= log2(NB) bits.  Input in (ka, va); buffers alternate
 // (result in (ka, va) after an even number of passes, (kb, vb) after an odd number).
-// ghist: [MAX_PASSES][256] u32, status: [npass][tiles][256] u64, both zeroed by the caller.
-template <typename KeyT>
+// ghist: [MAX_PASSES][NB] u32 counted by the producer of the keys, which also cleared status: [npass][tiles][NB] u64.
+template <typename KeyT, int NB>
 int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, uint64_t capacity,
                const uint64_t* n_ptr, int begin_bit, int end_bit, uint32_t* ghist, uint64_t* status, uint32_t* tickets,
-               bool have_hist /* histograms counted and status cleared by the producer of the keys */,
-               size_t stride_words = 0 /* status words per pass; 0 = tiles(capacity) * 256 */,
+               size_t stride_words = 0 /* status words per pass; 0 = tiles(capacity) * NB */,
                const FinalOut* fin = nullptr /* the last pass writes the binning (see FinalOut) */) {
   const uint32_t ntiles_cap = (uint32_t)((capacity + RS_TILE - 1) / RS_TILE);
   if (ntiles_cap == 0) return SPLX_OK;
   const uint32_t nblocks = ntiles_cap < PERSISTENT_CTAS ? ntiles_cap : PERSISTENT_CTAS;
-  const size_t stride = stride_words ? stride_words : (size_t)ntiles_cap * 256;     // status words per pass
-  const PassPlan plan = plan_passes(begin_bit, end_bit);
-  if (!have_hist) {
-    k_radix_hist_all<KeyT><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, n_ptr, ghist, status, stride, plan);
-    SPLX_LAUNCH_CHECK(ctx, "k_radix_hist_all");
-  }
+  const size_t stride = stride_words ? stride_words : (size_t)ntiles_cap * NB;     // status words per pass
+  const PassPlan plan = plan_passes(begin_bit, end_bit, NB == 256 ? 8 : 9);
   FinalOut none;
   memset(&none, 0, sizeof none);
   for (int p = 0; p < plan.npass; ++p) {
     if (fin && p + 1 == plan.npass)
-      k_radix_pass<KeyT, true><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
-                                                                       status + (size_t)p * stride, tickets + p,
-                                                                       plan.shift[p], plan.bits[p], *fin);
+      k_radix_pass<KeyT, true, NB><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + NB * p,
+                                                                           status + (size_t)p * stride, tickets + p,
+                                                                           plan.shift[p], plan.bits[p], *fin);
     else
-      k_radix_pass<KeyT, false><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + 256 * p,
-                                                                        status + (size_t)p * stride, tickets + p,
-                                                                        plan.shift[p], plan.bits[p], none);
+      k_radix_pass<KeyT, false, NB><<<nblocks, RS_THREADS, 0, ctx->stream>>>(ka, va, kb, vb, n_ptr, ghist + NB * p,
+                                                                            status + (size_t)p * stride, tickets + p,
+                                                                            plan.shift[p], plan.bits[p], none);
     SPLX_LAUNCH_CHECK(ctx, "k_radix_pass");
     KeyT* tk = ka; ka = kb; kb = tk;
     uint32_t* tv = va; va = vb; vb = tv;
@@ -570,10 +548,10 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
   if (emit_by_output(cnt) || (cnt->m_total >> 32)) return;   // M >= 2^32: the 32-bit offsets have wrapped, nothing is emitted
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
-  __shared__ uint32_t s_hist[MAX_PASSES * 256];
-  for (int x = threadIdx.x; x < MAX_PASSES * 256; x += blockDim.x) s_hist[x] = 0;
+  __shared__ uint32_t s_hist[MAX_PASSES * SLOT_NB];
+  for (int x = threadIdx.x; x < MAX_PASSES * SLOT_NB; x += blockDim.x) s_hist[x] = 0;
   {
-    const uint64_t words = ((cnt->m_sorted + RS_TILE - 1) / RS_TILE) * 256;
+    const uint64_t words = ((cnt->m_sorted + RS_TILE - 1) / RS_TILE) * SLOT_NB;
     for (int p = 0; p < plan.npass; ++p)
       for (uint64_t x = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; x < words; x += (uint64_t)gridDim.x * blockDim.x)
         rstatus[(size_t)p * rstride + x] = 0;
@@ -636,12 +614,12 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       skeys[pos] = slot;
       spay[pos] = sj;
       for (int p = 0; p < plan.npass; ++p)
-        atomicAdd(&s_hist[p * 256 + ((slot >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u))], 1u);
+        atomicAdd(&s_hist[p * SLOT_NB + ((slot >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u))], 1u);
     }
   }
   }
   __syncthreads();
-  for (int x = threadIdx.x; x < plan.npass * 256; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
+  for (int x = threadIdx.x; x < plan.npass * SLOT_NB; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
 }
 
 template <bool FILTER>
@@ -655,10 +633,10 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
   if (!emit_by_output(cnt) || (cnt->m_total >> 32)) return;
   // The producer of the keys also counts the digit histograms of the slot sort (shared atomics, one flush per
   // CTA) and clears the look-back status words of the tiles the M keys will occupy: no histogram kernel.
-  __shared__ uint32_t s_hist[MAX_PASSES * 256];
-  for (int x = threadIdx.x; x < MAX_PASSES * 256; x += blockDim.x) s_hist[x] = 0;
+  __shared__ uint32_t s_hist[MAX_PASSES * SLOT_NB];
+  for (int x = threadIdx.x; x < MAX_PASSES * SLOT_NB; x += blockDim.x) s_hist[x] = 0;
   {
-    const uint64_t words = ((cnt->m_sorted + RS_TILE - 1) / RS_TILE) * 256;
+    const uint64_t words = ((cnt->m_sorted + RS_TILE - 1) / RS_TILE) * SLOT_NB;
     for (int p = 0; p < plan.npass; ++p)
       for (uint64_t x = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; x < words; x += (uint64_t)gridDim.x * blockDim.x)
         rstatus[(size_t)p * rstride + x] = 0;
@@ -730,13 +708,13 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         skeys[pos] = slot;
         spay[pos] = (uint32_t)j0 + ql;                    // position of the owner in the depth-sorted list
         for (int p = 0; p < plan.npass; ++p)
-          atomicAdd(&s_hist[p * 256 + ((slot >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u))], 1u);
+          atomicAdd(&s_hist[p * SLOT_NB + ((slot >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u))], 1u);
       }
     }
     __syncthreads();
   }
   __syncthreads();
-  for (int x = threadIdx.x; x < plan.npass * 256; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
+  for (int x = threadIdx.x; x < plan.npass * SLOT_NB; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
 }
 
 __global__ void __launch_bounds__(256)
@@ -846,12 +824,12 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   const size_t scan_n = ((size_t)n + SCAN_TILE - 1) / SCAN_TILE;
   L.counters = take(sizeof(Counters));
   L.ghist_d = take(MAX_PASSES * 256 * 4);
-  L.ghist_s = take(MAX_PASSES * 256 * 4);
+  L.ghist_s = take(MAX_PASSES * SLOT_NB * 4);
   L.st_scan_v = take(scan_n * 8);
   L.st_scan_t = take(scan_n * 8);
   L.zero_bytes = off;
   L.st_depth = take(4 * scan_n * SCAN_RS * 256 * 8);                          // cleared by the compaction scan, whole scan tiles
-  L.st_slot = take((size_t)((sbits + 7) / 8) * tiles_m * 256 * 8);
+  L.st_slot = take((size_t)((sbits + SLOT_BITS - 1) / SLOT_BITS) * tiles_m * SLOT_NB * 8);
   L.ckeys_a = take((size_t)n * 4); L.cvals_a = take((size_t)n * 4);
   L.ckeys_b = take((size_t)n * 4); L.cvals_b = take((size_t)n * 4);
   L.offs = take((size_t)n * 4);
@@ -881,7 +859,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   const int K = plan.K;
   const PlanDev& cam = plan;   // TX, TY
   const int sbits = slot_bits(K, cam.TX, cam.TY);
-  if (sbits > 8 * MAX_PASSES) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles needs %d key bits (max 32)", sbits);
+  if (sbits > SLOT_BITS * MAX_PASSES) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort: K*tiles needs %d key bits (max 32)", sbits);
   const Layout L = make_layout(n, out->capacity, sbits);
   if (ws_bytes < L.total)
     SPLX_FAIL(ctx, SPLX_ERR_WORKSPACE, "splx_bin_sort: workspace %zu B < required %zu B", ws_bytes, L.total);
@@ -916,9 +894,9 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
                                             &cnt->n_visible, nullptr, 0, (uint32_t*)(base + L.ghist_d),
                                             (uint64_t*)(base + L.st_depth), stride_d))) return rc;
   // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers); histograms came with step 1
-  if ((rc = radix_sort<uint32_t>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n_act, &cnt->n_visible, 0, 32,
-                                 (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2], true,
-                                 stride_d))) return rc;
+  if ((rc = radix_sort<uint32_t, 256>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n_act, &cnt->n_visible, 0, 32,
+                                      (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2],
+                                      stride_d))) return rc;
   // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
   if ((rc = scan_exclusive<TouchedOp, false>(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
@@ -941,7 +919,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   const uint32_t cslots = (uint32_t)nact * (uint32_t)ntiles;      // compact slots 0 .. cslots (cslots itself = filtered)
   int cbits = 1;
   while (((uint64_t)1 << cbits) <= cslots) ++cbits;
-  const PassPlan spl = plan_passes(0, cbits);
+  const PassPlan spl = plan_passes(0, cbits, SLOT_BITS);
   uint32_t* A_k = (uint32_t*)(base + L.pairs_tmp); uint32_t* A_p = A_k + out->capacity;
   uint32_t* B_k = (uint32_t*)out->keys; uint32_t* B_p = B_k + out->capacity;
   const bool startA = (spl.npass & 1) != 0;                       // so that the LAST pass reads A (and may overwrite B's memory)
@@ -960,7 +938,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   const unsigned g_lb = (unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS);
   uint32_t* gh = (uint32_t*)(base + L.ghist_s);
   uint64_t* sst = (uint64_t*)(base + L.st_slot);
-  const size_t sstride = (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * 256;
+  const size_t sstride = (((size_t)out->capacity + RS_TILE - 1) / RS_TILE) * SLOT_NB;
   if (cx.mask) {
     k_emit_keys<true><<<g_emit, 256, 0, ctx->stream>>>(pr->means2d, pr->radius, ckeys_a, cvals_a, offs, cnt, parts, cam.TX, cam.TY,
                                                        out->capacity, k0, p0, spl, gh, sst, sstride, cx);
@@ -976,8 +954,8 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
                                                          out->capacity, k0, p0, spl, gh, sst, sstride, cx);
     SPLX_LAUNCH_CHECK(ctx, "k_emit_keys_lb");
   }
-  if ((rc = radix_sort<uint32_t>(ctx, k0, p0, k1, p1, out->capacity, &cnt->m_sorted, 0, cbits, gh, sst, &cnt->ticket[6], true, 0,
-                                 &fin))) return rc;
+  if ((rc = radix_sort<uint32_t, SLOT_NB>(ctx, k0, p0, k1, p1, out->capacity, &cnt->m_sorted, 0, cbits, gh, sst, &cnt->ticket[6], 0,
+                                          &fin))) return rc;
   // 5. ranges
   k_tile_ranges<<<(unsigned)(range_blocks < 4 * PERSISTENT_CTAS ? range_blocks : 4 * PERSISTENT_CTAS), 256, 0, ctx->stream>>>(
       out->keys, cnt, plan.tile_state, out->tile_ranges, out->num_intersections, (uint32_t)K * (uint32_t)ntiles, cx.mask != nullptr);

@@ -176,7 +176,7 @@ class Trainer:
     def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True) -> binding.Plan:
         if view_of_part is None:
             view_of_part = [0] * self.K
-        return binding.Plan(cams, view_of_part, tile_state, sparse)
+        return binding.Plan(cams, view_of_part, tile_state, sparse, getattr(self, "_part_max_scale", None))
 
     def forward_plan(self, plan: binding.Plan, sat_eps=None, tile_state_out=None, count_pairs=False):
         """a1-a6 for all views of the plan in one launch per stage; returns images[B,H,W,3]."""
@@ -255,6 +255,14 @@ class Trainer:
         empty = ~np.isfinite(plo).all(1)
         plo[empty] = 0; phi[empty] = 0
         self._part_box = (plo, phi)
+        # the largest scale of every partition: splx_plan.max_scale (the projection's reach test on the mean alone)
+        self._part_max_scale = None
+        if max_scale is not None:
+            pms = np.zeros(self.K, np.float32)
+            for j in range(lo.shape[0]):
+                k = j if bp is None else int(bp[j])
+                pms[k] = max(pms[k], float(self._aabb[2][j]))
+            self._part_max_scale = pms
         self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear(); self._graphs.clear()
 
     def participants(self, view_id, cam) -> int:

@@ -659,3 +659,24 @@ def test_flag_tracked_gradient_rows_equal_the_plain_buffer(blocks):
             assert torch.isfinite(x).all()
             close = torch.isclose(x, y, rtol=1e-3, atol=2e-6)
             assert close.float().mean().item() >= 0.999, key
+
+
+def test_reach_test_on_the_mean_culls_nothing_visible(city, blocks):
+    """splx_plan.max_scale: the projection tests a Gaussian's mean against the half spaces outside which nothing of
+    that scale reaches the image (reading s21) before it reads scale and rotation.  Same radius / tiles_touched for
+    every Gaussian, bit-equal attributes for the visible ones -- and most Gaussians of a view do fail the test."""
+    for sc in (city, blocks):
+        cam = sc.cameras[-1]
+        ms = scenes.partition_boxes(sc.params, sc.part_offsets)[2]
+        a, b = G.make_trainer(sc), G.make_trainer(sc)
+        pa = binding.Plan([cam], [0] * sc.K, None, True, max_scale=ms)
+        pb = binding.Plan([cam], [0] * sc.K, None, True)
+        a.ctx.project_plan(a.params, a.part_offsets, pa, a.sh_degree, a.proj)
+        b.ctx.project_plan(b.params, b.part_offsets, pb, b.sh_degree, b.proj)
+        torch.cuda.synchronize()
+        assert torch.equal(a.proj.radius, b.proj.radius) and torch.equal(a.proj.tiles_touched, b.proj.tiles_touched)
+        vis = b.proj.radius > 0
+        assert 0 < int(vis.sum()) < sc.N
+        for name in ("means2d", "depth", "conic_opacity", "rgb", "blend", "clamp"):
+            x, y = getattr(a.proj, name), getattr(b.proj, name)
+            assert torch.equal(x[vis], y[vis]), name
