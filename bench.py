@@ -87,9 +87,13 @@ def ncu_traffic(workload_name, kernel):
     if not os.path.exists(p):
         return None
     try:
-        return json.load(open(p)).get(workload_name, {}).get(kernel)
+        per_kernel = json.load(open(p)).get(workload_name, {})
     except Exception:
         return None
+    for name, v in per_kernel.items():      # the file names template instances ("k_adam_groups<1>")
+        if name == kernel or name.split("<")[0] == kernel:
+            return v
+    return None
 
 
 class ClockSampler:

@@ -327,6 +327,18 @@ int splx_project_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64
 int splx_bin_sort_plan(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
                        const int64_t *part_offsets, const splx_plan *plan, const splx_binning *out,
                        void *ws, size_t ws_bytes);
+/* splx_project_plan in two halves ("standard 3DGS rendering procedure", steps a1 and the colour of s13):
+ * splx_project_geometry_plan writes everything splx_project_plan writes EXCEPT the colour (rgb, clamp, blend[8..10]);
+ * splx_project_colour_list_plan then computes the colour of the entries of `visible` (DEVICE uint32[*num_visible],
+ * *num_visible a DEVICE uint64: the list splx_bin_sort_visible returns after splx_bin_sort_plan on the geometry).
+ * Together bit-equal to splx_project_plan on every visible Gaussian; the work of the colour follows the visible
+ * count, not the partition sizes (on a city view ~13 % of the participating Gaussians are visible, scattered over the
+ * warps).  The colour must be complete before splx_render_partial_plan / splx_project_backward_* read it. */
+int splx_project_geometry_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                               const splx_plan *plan, const splx_projected *out);
+int splx_project_colour_list_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
+                                  const splx_plan *plan, int sh_degree, const splx_projected *out,
+                                  const uint32_t *visible, const uint64_t *num_visible);
 int splx_render_partial_plan(splx_ctx *ctx, const splx_projected *proj, const splx_binning *bins, int K,
                              const splx_plan *plan, const splx_partial *out, uint64_t *pairs);
 /* bins: needed with SPLX_PLAN_SPARSE or tile_state_out, else may be NULL.  tile_state_out (DEVICE

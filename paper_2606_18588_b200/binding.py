@@ -171,6 +171,8 @@ def lib():
         L.splx_schedule_views.argtypes = [C.c_int, vp, C.c_int, vp, vp]
         L.splx_project_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp]
         L.splx_bin_sort_plan.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp, vp, vp, C.c_size_t]
+        L.splx_project_geometry_plan.argtypes = [vp, vp, C.c_int, vp, vp, vp]
+        L.splx_project_colour_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp]
         L.splx_render_partial_plan.argtypes = [vp, vp, vp, C.c_int, vp, vp, vp]
         L.splx_compose_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, C.c_float, vp]
         L.splx_compose_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp]
@@ -487,6 +489,16 @@ class Context:
         g, ps = gaussians_struct(params), out.struct()
         self._check(lib().splx_project_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
                                             sh_degree, C.byref(ps)))
+
+    def project_geometry_plan(self, params: dict, part_offsets, plan: Plan, out: Projected):
+        g, ps = gaussians_struct(params), out.struct()
+        self._check(lib().splx_project_geometry_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(), C.byref(ps)))
+
+    def project_colour_list_plan(self, params: dict, part_offsets, plan: Plan, sh_degree: int, out: Projected,
+                                 visible_ptr: int, count_ptr: int):
+        g, ps = gaussians_struct(params), out.struct()
+        self._check(lib().splx_project_colour_list_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(), sh_degree,
+                                                        C.byref(ps), C.c_void_p(visible_ptr), C.c_void_p(count_ptr)))
 
     def bin_sort_plan(self, proj: Projected, part_offsets, plan: Plan, out: Binning, ws: torch.Tensor):
         ps, bs = proj.struct(), out.struct()

@@ -145,6 +145,32 @@ int splx_project_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64
   return launch_project_fwd(ctx, g, pd, part_offsets, sh_degree, out);
 }
 
+int splx_project_geometry_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const splx_plan* plan,
+                               const splx_projected* out) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (g && g->n == 0) return SPLX_OK;
+  if (!gauss_ok(g) || !proj_ok(out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_geometry: null/misaligned argument");
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan_dev(ctx, "splx_project_geometry", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_geometry: part_offsets must run monotonically from 0 to n");
+  return launch_project_fwd(ctx, g, pd, part_offsets, 0, out, false);
+}
+
+int splx_project_colour_list_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const splx_plan* plan,
+                                  int sh_degree, const splx_projected* out, const uint32_t* visible, const uint64_t* num_visible) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (g && g->n == 0) return SPLX_OK;
+  if (!gauss_ok(g) || !proj_ok(out) || !visible || !num_visible)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_colour_list: null/misaligned argument");
+  if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_colour_list: sh_degree %d not in [0,3]", sh_degree);
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan_dev(ctx, "splx_project_colour_list", K, plan, &pd))) return rc;
+  if (!offsets_ok(part_offsets, K, g->n)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_colour_list: part_offsets must run monotonically from 0 to n");
+  return launch_project_colour_list(ctx, g, pd, part_offsets, sh_degree, out, visible, num_visible);
+}
+
 int splx_project(splx_ctx* ctx, const splx_gaussians* g, const splx_camera* cam, int sh_degree,
                  const splx_projected* out) {
   if (!ctx) return SPLX_ERR_INVALID_ARG;

@@ -184,7 +184,9 @@ int make_plan_dev(splx_ctx*, const char* who, int K, const splx_plan*, PlanDev* 
 
 // ---- stage launchers (defined one per .cu file, called from api.cu) ----------------------
 int launch_project_fwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
-                       const splx_projected*);
+                       const splx_projected*, bool with_colour = true);
+int launch_project_colour_list(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
+                               const splx_projected*, const uint32_t* visible_list, const uint64_t* num_visible);
 int launch_project_bwd(splx_ctx*, const splx_gaussians*, const PlanDev&, const int64_t* part_offsets, int sh_degree,
                        const splx_projected*, float* g2d, int flags, const splx_gaussian_grads*,
                        const uint32_t* visible_list, const uint64_t* num_visible, uint8_t* touched);

@@ -129,9 +129,15 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
     const splx_bucket& bk = buckets[gi];
     const splx_frontset& fs = ts->front[set];
     int r;
-    if ((r = splx_project_plan(ctx, &g, K, ts->part_offsets, &bk.plan, ts->sh_degree, &fs.proj))) return r;
-    return splx_bin_sort_filtered_plan(ctx, &fs.proj, n, K, ts->part_offsets, &bk.plan, ts->cross_mask, bk.part_depth_range,
-                                       &fs.bins, fs.ws, fs.ws_bytes);
+    // the colour only for the visible Gaussians, once the binning has compacted their list (the geometry alone decides
+    // visibility, depth and footprint: the binning does not read the colour)
+    if ((r = splx_project_geometry_plan(ctx, &g, K, ts->part_offsets, &bk.plan, &fs.proj))) return r;
+    if ((r = splx_bin_sort_filtered_plan(ctx, &fs.proj, n, K, ts->part_offsets, &bk.plan, ts->cross_mask, bk.part_depth_range,
+                                         &fs.bins, fs.ws, fs.ws_bytes))) return r;
+    const uint32_t* vlist = nullptr;
+    const uint64_t* nvis = nullptr;
+    if ((r = splx_bin_sort_visible(fs.ws, n, fs.bins.capacity, K, &bk.plan.cams[0], &vlist, &nvis))) SPLX_FAIL(ctx, r, "splx_iteration: visible list");
+    return splx_project_colour_list_plan(ctx, &g, K, ts->part_offsets, &bk.plan, ts->sh_degree, &fs.proj, vlist, nvis);
   };
 
   // a5-a10 of bucket gi from front set `set`, on the context's stream

@@ -181,13 +181,16 @@ __device__ __forceinline__ void colour(const float4* sh4, int lane, const CamDev
 // warp hits eight different bank groups) and reads its rows from there; with fewer visible rows (the culled
 // partitions of a city view) the direct loads touch less memory and are kept.
 constexpr int SH_STAGE_MIN = 12;
-template <int DEG>
+// COLOUR = false (splx_project_geometry_plan): everything but the colour, which k_colour_list then computes for the
+// VISIBLE Gaussians only.  On a city view ~13 % of the participating Gaussians are visible, scattered over the warps:
+// nearly every warp ran the whole colour path (a third of the kernel's instructions) for 4 of its 32 lanes.
+template <int DEG, bool COLOUR>
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt,
               splx_config cfg, splx_projected out) {
   constexpr int NSH = (DEG + 1) * (DEG + 1);
   constexpr int NV = (NSH * 3 + 3) / 4;
-  constexpr bool STAGE = DEG > 0;
+  constexpr bool STAGE = COLOUR && DEG > 0;
   __shared__ __align__(16) float4 s_sh[STAGE ? PROJ_THREADS * NV : 1];
   const int r = find_run(rt, (int)blockIdx.x);
   const int64_t i = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PROJ_THREADS + threadIdx.x;
@@ -250,6 +253,7 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       m[0] = gin.m[0]; m[1] = gin.m[1]; m[2] = gin.m[2];
     }
   }
+  if (!COLOUR) return;
   float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
   const int lane = threadIdx.x & 31;
   const unsigned vmask = __ballot_sync(0xffffffffu, vis);
@@ -272,6 +276,30 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     return;
   }
   if (vis) colour<DEG, false>(reinterpret_cast<const float4*>(g.sh + 48 * i), lane, cam, m, i, out, bl);
+}
+
+// The colour of the visible Gaussians (the binning's list, index order): one thread per entry, persistent grid because
+// the count lives on the device.  Same arithmetic as the colour half of k_project_fwd (bit-equal rgb, clamp, blend[2]).
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS)
+k_colour_list(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt, splx_projected out,
+              const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr) {
+  const uint64_t nvis = *nvis_ptr;
+  const int lane = threadIdx.x & 31;
+  for (uint64_t j = (uint64_t)blockIdx.x * PROJ_THREADS + threadIdx.x; j < nvis; j += (uint64_t)gridDim.x * PROJ_THREADS) {
+    const int64_t i = (int64_t)vlist[j];
+    int lo = 0, hi = rt.n - 1;                          // the run (partition) of Gaussian i -> its view
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (rt.begin[mid] <= i) lo = mid; else hi = mid - 1;
+    }
+    const CamDev& cam = plan.cam[rt.view[lo]];
+    float m[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) m[k] = g.mean[3 * i + k];
+    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+    colour<DEG, false>(reinterpret_cast<const float4*>(g.sh + 48 * i), lane, cam, m, i, out, bl);
+  }
 }
 
 // Gradients of Y_l with respect to the (unconstrained) direction components.
@@ -629,17 +657,33 @@ static void launch_pb_deg(splx_ctx* ctx, bool overwrite, const splx_gaussians* g
 }  // namespace
 
 int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
-                       const splx_projected* out) {
+                       const splx_projected* out, bool with_colour) {
   const RunTable rt = make_runs(plan, part_offsets, PROJ_THREADS, false);
   if (rt.blocks_total == 0) return SPLX_OK;
   const unsigned grid = (unsigned)rt.blocks_total;
-  switch (deg) {
-    case 0: k_project_fwd<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    case 1: k_project_fwd<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    case 2: k_project_fwd<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
-    default: k_project_fwd<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out); break;
+#define PF(D, C) k_project_fwd<D, C><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out)
+  if (with_colour) {
+    switch (deg) { case 0: PF(0, true); break; case 1: PF(1, true); break; case 2: PF(2, true); break; default: PF(3, true); break; }
+  } else {
+    PF(0, false);     // the degree only matters to the colour
   }
+#undef PF
   SPLX_LAUNCH_CHECK(ctx, "k_project_fwd");
+  return SPLX_OK;
+}
+
+int launch_project_colour_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
+                               const splx_projected* out, const uint32_t* vlist, const uint64_t* nvis) {
+  const RunTable rt = make_runs(plan, part_offsets, PROJ_THREADS, false);
+  if (rt.blocks_total == 0) return SPLX_OK;
+  const unsigned grid = SPLX_SM_COUNT * 8;     // persistent: the count lives on the device
+  switch (deg) {
+    case 0: k_colour_list<0><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, *out, vlist, nvis); break;
+    case 1: k_colour_list<1><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, *out, vlist, nvis); break;
+    case 2: k_colour_list<2><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, *out, vlist, nvis); break;
+    default: k_colour_list<3><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, *out, vlist, nvis); break;
+  }
+  SPLX_LAUNCH_CHECK(ctx, "k_colour_list");
   return SPLX_OK;
 }
 

@@ -398,6 +398,42 @@ def test_projection_backward_over_the_visible_list(blocks):
     assert 0 < n_vis < b.n
 
 
+def test_projection_in_two_halves_equals_the_single_call(blocks):
+    """splx_project_geometry_plan + (after the binning) splx_project_colour_list_plan == splx_project_plan: identical
+    bytes in every output of the participating partitions, the colour compared on the visible Gaussians (a culled
+    one has none), and the binning built on the geometry alone is the same binning."""
+    sc = blocks
+    cam = sc.cameras[1]
+    a, b = _trainer(sc), _trainer(sc)
+    part = a.participants(1, cam)
+    vop = [0 if (part >> k) & 1 else -1 for k in range(sc.K)]
+    for tr in (a, b):
+        tr._plan = tr.make_plan([cam], vop, None, True)
+        tr._workspaces(cam)
+        for t in (tr.proj.rgb, tr.proj.blend):
+            t.fill_(-7.0)
+        tr.proj.clamp.fill_(9)
+    a.ctx.project_plan(a.params, a.part_offsets, a._plan, a.sh_degree, a.proj)
+    a.ctx.bin_sort_plan(a.proj, a.part_offsets, a._plan, a.bins, a._ws_sort)
+    b.ctx.project_geometry_plan(b.params, b.part_offsets, b._plan, b.proj)
+    b.ctx.bin_sort_plan(b.proj, b.part_offsets, b._plan, b.bins, b._ws_sort)
+    lst, cnt = b.ctx.bin_sort_visible(b._ws_sort, b.n, b.capacity, b.K, cam)
+    b.ctx.project_colour_list_plan(b.params, b.part_offsets, b._plan, b.sh_degree, b.proj, lst, cnt)
+    torch.cuda.synchronize()
+    rows = torch.as_tensor([i for k in range(sc.K) if vop[k] == 0 for i in range(a.part_offsets[k], a.part_offsets[k + 1])]).cuda()
+    vis = rows[a.proj.radius[rows] > 0]
+    assert 0 < vis.numel() < a.n
+    for name in ("radius", "tiles_touched"):
+        assert torch.equal(getattr(a.proj, name)[rows], getattr(b.proj, name)[rows]), name
+    for name in ("means2d", "depth", "conic_opacity", "rgb", "clamp", "blend"):
+        x, y = getattr(a.proj, name), getattr(b.proj, name)
+        x, y = x.view(a.n, -1)[vis], y.view(b.n, -1)[vis]
+        assert torch.equal(x.view(torch.uint8), y.view(torch.uint8)), name
+    m = int(a.bins.num_intersections[0])
+    assert m == int(b.bins.num_intersections[0]) and m > 0
+    assert torch.equal(a.bins.keys[:m], b.bins.keys[:m]) and torch.equal(a.bins.vals[:m], b.bins.vals[:m])
+
+
 def test_pipelined_buckets_equal_the_sequential_iteration(city):
     """Multi-bucket iterations project and sort bucket g+1 on a second stream while bucket g is blended (double-buffered
     projected / binning sets): same gradients, same saturation bytes, same parameters as one bucket after the other."""
