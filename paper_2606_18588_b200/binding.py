@@ -29,7 +29,8 @@ EXPORTS = [
     "splx_render_partial", "splx_compose", "splx_l1_loss_grad", "splx_compose_backward",
     "splx_raster_backward", "splx_project_backward", "splx_backward_ws_bytes", "splx_backward",
     "splx_adam", "splx_adam_groups",
-    "splx_visible_regions", "splx_schedule_views", "splx_project_plan", "splx_bin_sort_plan",
+    "splx_visible_regions", "splx_schedule_views", "splx_project_plan", "splx_project_geometry_plan",
+    "splx_project_colour_list_plan", "splx_bin_sort_plan",
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
     "splx_compose_l1_backward_plan",
