@@ -59,47 +59,16 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 // Staging ring of one warp: [buffer][quarter of the record][entry].  Quarter 0 = (u, v, o, depth),
 // 1 = (A', B', C', bits(index)), 2 = (r, g, b, 0).
-struct Ring { float4 q[NBUF][96]; };
-// gather layout (cp.async): quarter-major; stream layout (bulk copy of 32 consecutive 48-byte records): entry-major
-template <bool STREAM>
-__device__ __forceinline__ int ridx(int quarter, int j) { return STREAM ? 3 * j + quarter : 32 * quarter + j; }
-
-// ---- experiment: contiguous sorted attribute stream fed by 1-D bulk copies (cp.async.bulk + mbarrier) ----
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void bulk_issue(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(
-          smem_u32(bar)),
-      "r"(parity)
-      : "memory");
-}
-// sorted[e] = blend[vals[e]]: the 48-byte records in list order
-__global__ void __launch_bounds__(256) k_gather_blend(const float4* __restrict__ blend, const uint32_t* __restrict__ vals,
-                                                      const uint64_t* __restrict__ m_ptr, float4* __restrict__ sorted) {
-  const uint64_t n = 3ull * m_ptr[0];
-  for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (uint64_t)gridDim.x * blockDim.x) {
-    const uint32_t e = (uint32_t)(t / 3ull), q = (uint32_t)(t - 3ull * e);
-    sorted[t] = __ldg(blend + 3ull * __ldg(vals + e) + q);
-  }
-}
+struct Ring { float4 q[NBUF][3][32]; };
 
 // Issue the copies of list entry `idx` (if inside [.., end)) into slot `lane` of ring buffer `buf`.
 __device__ __forceinline__ void stage_issue(Ring& ring, int buf, int lane, const float* __restrict__ blend,
                                             const uint32_t* __restrict__ vals, uint32_t idx, uint32_t end) {
   if (idx < end) {
     const float* src = blend + (size_t)SPLX_BLEND_STRIDE * __ldg(vals + idx);
-    cp_async16(&ring.q[buf][lane], src);
-    cp_async16(&ring.q[buf][32 + lane], src + 4);
-    cp_async16(&ring.q[buf][64 + lane], src + 8);
+    cp_async16(&ring.q[buf][0][lane], src);
+    cp_async16(&ring.q[buf][1][lane], src + 4);
+    cp_async16(&ring.q[buf][2][lane], src + 8);
   }
   cp_async_commit();
 }
@@ -122,15 +91,14 @@ __device__ __forceinline__ float quad_max_rect(float gx, float gy, float A, floa
 // 4-bit mask of the slots of this warp's half tile on which the Gaussian can reach alpha_min.
 // (X0, Y0) = pixel coordinates of the half tile's first pixel; slot s covers columns 8(s&1)..+7 and
 // rows 4(s>>1)..+3; pixel i samples i + 0.5.
-template <int NS = 4>
 __device__ __forceinline__ unsigned cull_mask(const float4 a, const float4 b, float X0, float Y0, float log2_amin) {
   const float A = b.x, B = b.y, C = b.z, o = a.z;
-  if (!(A < 0.f) || !(C < 0.f) || !(log2_amin > -1e30f)) return (1u << NS) - 1u;   // degenerate conic or alpha_min == 0: keep all
+  if (!(A < 0.f) || !(C < 0.f) || !(log2_amin > -1e30f)) return 0xFu;   // degenerate conic or alpha_min == 0: keep all
   const float tau = log2_amin - lg2_approx(o) - CULL_MARGIN;           // keep the slot if max exponent >= tau
   const float hBC = -0.5f * __fdividef(B, C), hBA = -0.5f * __fdividef(B, A);
   unsigned m = 0;
 #pragma unroll
-  for (int s = 0; s < NS; ++s) {
+  for (int s = 0; s < 4; ++s) {
     const float x0 = X0 + (float)(8 * (s & 1)) + 0.5f, y0 = Y0 + (float)(4 * (s >> 1)) + 0.5f;
     const float qm = quad_max_rect(a.x, a.y, A, B, C, hBC, hBA, x0, x0 + 7.0f, y0, y0 + 3.0f);
     if (!(qm < tau)) m |= 1u << s;
@@ -151,19 +119,13 @@ __device__ __forceinline__ bool eval_alpha(float dx, float dy, float adx, float 
 }
 
 constexpr int FWD_MIN_CTAS = 14;   // 71 registers; a sweep 12..20 showed no effect below spilling: issue-bound
-// NS = slots (8 x 4 pixel blocks) per lane: 4 = a warp per HALF tile, two warps per CTA (the product); 8 = a warp per whole tile
-// (experiment).  STREAM = the records come as a contiguous list-ordered stream through 1-D bulk copies (experiment).
-template <bool COUNT, int NS, bool STREAM, int MASK = 0>
-__global__ void __launch_bounds__(NS == 4 ? 64 : 32, NS == 4 ? (MASK == 2 ? 12 : FWD_MIN_CTAS) : 16)
+template <bool COUNT>
+__global__ void __launch_bounds__(BLOCK, FWD_MIN_CTAS)
 k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const __grid_constant__ PartView pv, int sparse,
              float* __restrict__ out_ct, float* __restrict__ out_d, uint32_t* __restrict__ out_n,
-             unsigned long long* pairs, const uint32_t* __restrict__ order, uint32_t nslots, int count_empty = 0,
-             uint8_t* __restrict__ item_mask = nullptr, uint64_t mask_stride = 0) {
-  constexpr int NW = NS == 4 ? 2 : 1;
-  constexpr unsigned ALL = (1u << NS) - 1u;
-  __shared__ Ring rings[NW];
-  __shared__ uint64_t bars[NW][NBUF];
+             unsigned long long* pairs, const uint32_t* __restrict__ order, uint32_t nslots) {
+  __shared__ Ring rings[WARPS];
   int tile = blockIdx.x, k = blockIdx.y;
   if (order) {                             // CTAs handed out longest list first (splx_binning.slot_order)
     if (blockIdx.x >= order[nslots]) return;
@@ -173,75 +135,50 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
   if (pv.v[k] < 0) return;                 // the partition does not participate in this launch
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   Ring& ring = rings[warp];
-  const int X0 = (tile % TX) * SPLX_TILE, Y0 = (tile / TX) * SPLX_TILE + (NS == 4 ? 8 * warp : 0);
+  const int X0 = (tile % TX) * SPLX_TILE, Y0 = (tile / TX) * SPLX_TILE + 8 * warp;
   const int pxi = X0 + (lane & 7), pyi = Y0 + (lane >> 3);          // slot 0 pixel; slot s adds (8(s&1), 4(s>>1))
-  const float px0 = (float)pxi + 0.5f, px1 = px0 + 8.0f;
-  float pys[NS / 2];
-#pragma unroll
-  for (int r = 0; r < NS / 2; ++r) pys[r] = (float)pyi + 0.5f + 4.0f * (float)r;
+  const float px0 = (float)pxi + 0.5f, px1 = px0 + 8.0f, py0 = (float)pyi + 0.5f, py1 = py0 + 4.0f;
   const uint32_t r0 = ranges[2 * ((size_t)k * ntiles + tile)], r1 = ranges[2 * ((size_t)k * ntiles + tile) + 1];
   if (sparse && r0 == r1) return;          // SPLX_PLAN_SPARSE: an empty list is the identity partial, never stored
   const float log2_amin = cfg.alpha_min > 0.f ? log2f(cfg.alpha_min) : -INFINITY;
 
-  float T[NS], C0[NS], C1[NS], C2[NS], D[NS];
-  uint32_t last[NS], wdone[COUNT ? NS : 1];
+  float T[4], C0[4], C1[4], C2[4], D[4];
+  uint32_t last[4], wdone[4];
   unsigned done = 0;                       // bit s: slot s finished (exit rule fired, or outside the image)
   uint32_t blended = 0, evaluated = 0, items = 0;
 #pragma unroll
-  for (int s = 0; s < NS; ++s) {
-    T[s] = 1.f; C0[s] = C1[s] = C2[s] = D[s] = 0.f; last[s] = 0;
-    if (COUNT) wdone[s] = 0;
+  for (int s = 0; s < 4; ++s) {
+    T[s] = 1.f; C0[s] = C1[s] = C2[s] = D[s] = 0.f; last[s] = 0; wdone[s] = 0;
     if (pxi + 8 * (s & 1) >= W || pyi + 4 * (s >> 1) >= H) done |= 1u << s;
   }
   const unsigned outside = done;
 
-  if (r0 < r1 && !__all_sync(FULL, done == ALL)) {
-    uint32_t phase = 0;
-    if (STREAM) {
-      if (lane == 0) { mbar_init(&bars[warp][0], 1); mbar_init(&bars[warp][1], 1); }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      __syncwarp();
-      if (lane == 0) bulk_issue(ring.q[0], blend + (size_t)SPLX_BLEND_STRIDE * r0, 48u * min(32u, r1 - r0), &bars[warp][0]);
-    } else {
-      stage_issue(ring, 0, lane, blend, vals, r0 + lane, r1);
-    }
+  if (r0 < r1 && !__all_sync(FULL, done == 0xFu)) {
+    stage_issue(ring, 0, lane, blend, vals, r0 + lane, r1);
     int buf = 0;
     for (uint32_t start = r0; start < r1; start += 32, buf ^= 1) {
-      if (STREAM) {
-        if (lane == 0 && start + 32 < r1)
-          bulk_issue(ring.q[buf ^ 1], blend + (size_t)SPLX_BLEND_STRIDE * (start + 32), 48u * min(32u, r1 - start - 32),
-                     &bars[warp][buf ^ 1]);
-        mbar_wait(&bars[warp][buf], (phase >> buf) & 1u);
-        phase ^= 1u << buf;
-      } else {
-        stage_issue(ring, buf ^ 1, lane, blend, vals, start + 32 + lane, r1);
-        cp_async_wait<1>();
-        __syncwarp();
-      }
+      stage_issue(ring, buf ^ 1, lane, blend, vals, start + 32 + lane, r1);
+      cp_async_wait<1>();
+      __syncwarp();
       unsigned m = 0;
-      if (start + lane < r1)
-        m = cull_mask<NS>(ring.q[buf][ridx<STREAM>(0, lane)], ring.q[buf][ridx<STREAM>(1, lane)], (float)X0, (float)Y0, log2_amin);
-      const unsigned open_slots = ~__reduce_and_sync(FULL, done) & ALL;   // slots not yet finished in every lane
+      if (start + lane < r1) m = cull_mask(ring.q[buf][0][lane], ring.q[buf][1][lane], (float)X0, (float)Y0, log2_amin);
+      const unsigned open_slots = ~__reduce_and_sync(FULL, done) & 0xFu;   // slots not yet finished in every lane
       m &= open_slots;
       unsigned live = __ballot_sync(FULL, m != 0);
-      unsigned myrec = 0;                   // experiment: slots of MY entry in which some pixel blended it
-      unsigned tk0 = 0, tk1 = 0, tk2 = 0, tk3 = 0;   // MASK 2: bit j of tk<s> = this lane blended entry j of the batch in slot s
       while (live) {
         const int j = __ffs(live) - 1;
         live &= live - 1;
         const unsigned mj = __shfl_sync(FULL, m, j);
-        const float4 a = ring.q[buf][ridx<STREAM>(0, j)], b = ring.q[buf][ridx<STREAM>(1, j)], c = ring.q[buf][ridx<STREAM>(2, j)];
+        const float4 a = ring.q[buf][0][j], b = ring.q[buf][1][j], c = ring.q[buf][2][j];
         const uint32_t pos = start - r0 + (uint32_t)j + 1;     // 1-based list position, as in n_contrib
         const float dxs[2] = {__fsub_rn(a.x, px0), __fsub_rn(a.x, px1)};
+        const float dys[2] = {__fsub_rn(a.y, py0), __fsub_rn(a.y, py1)};
         const float adx[2] = {__fmul_rn(b.x, dxs[0]), __fmul_rn(b.x, dxs[1])};
         const float bdx[2] = {__fmul_rn(b.y, dxs[0]), __fmul_rn(b.y, dxs[1])};
-        float dys[NS / 2], cdy[NS / 2];
+        const float cdy[2] = {__fmul_rn(b.z, dys[0]), __fmul_rn(b.z, dys[1])};
+        if (COUNT) ++items;
 #pragma unroll
-        for (int r = 0; r < NS / 2; ++r) { dys[r] = __fsub_rn(a.y, pys[r]); cdy[r] = __fmul_rn(b.z, dys[r]); }
-        if (COUNT && !count_empty) ++items;
-        unsigned took = 0;
-#pragma unroll
-        for (int s = 0; s < NS; ++s) {
+        for (int s = 0; s < 4; ++s) {
           if (!((mj >> s) & 1)) continue;     // warp-uniform
           if (COUNT) ++evaluated;
           float G, alpha; bool clamped;
@@ -258,26 +195,18 @@ k_render_fwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
           T[s] = take ? Tn : T[s];
           last[s] = take ? pos : last[s];
           if (stop) done |= 1u << s;
-          if (COUNT) { if (stop) wdone[s] = pos; if (take) ++blended; if (count_empty && !__any_sync(FULL, take)) ++items; }
-          if (MASK == 1 && __any_sync(FULL, take)) took |= 1u << s;
-          if (MASK == 2) { const unsigned bj = take ? 1u << j : 0u; if (s == 0) tk0 |= bj; else if (s == 1) tk1 |= bj; else if (s == 2) tk2 |= bj; else tk3 |= bj; }
+          if (COUNT) { if (stop) wdone[s] = pos; if (take) ++blended; }
         }
-        if (MASK == 1 && lane == j) myrec = took;
       }
-      if (MASK == 2) {
-        myrec = ((__reduce_or_sync(FULL, tk0) >> lane) & 1u) | (((__reduce_or_sync(FULL, tk1) >> lane) & 1u) << 1) |
-                (((__reduce_or_sync(FULL, tk2) >> lane) & 1u) << 2) | (((__reduce_or_sync(FULL, tk3) >> lane) & 1u) << 3);
-      }
-      if (MASK && start + lane < r1) item_mask[(size_t)warp * mask_stride + start + lane] = (uint8_t)myrec;
       __syncwarp();
-      if (__all_sync(FULL, done == ALL)) break;
+      if (__all_sync(FULL, done == 0xFu)) break;
     }
-    if (!STREAM) cp_async_wait<0>();
+    cp_async_wait<0>();
   }
 
   uint32_t walked = 0;
 #pragma unroll
-  for (int s = 0; s < NS; ++s) {
+  for (int s = 0; s < 4; ++s) {
     if ((outside >> s) & 1) continue;
     const int x = pxi + 8 * (s & 1), y = pyi + 4 * (s >> 1);
     const size_t pix = ((size_t)k * H + y) * W + x;
@@ -336,12 +265,11 @@ __device__ __noinline__ void flush_stage(Stage& st, int nb, uint32_t gid, int la
   __syncwarp();
 }
 
-template <bool MASK>
 __global__ void __launch_bounds__(BLOCK, BWD_MIN_CTAS)
 k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals, const uint32_t* __restrict__ ranges,
              int W, int H, int TX, int ntiles, splx_config cfg, const float* __restrict__ ct,
              const uint32_t* __restrict__ n_contrib, const float* __restrict__ g_ct, float* __restrict__ g2d,
-             const uint32_t* __restrict__ order, uint32_t nslots, const uint8_t* __restrict__ item_mask, uint64_t mask_stride) {
+             const uint32_t* __restrict__ order, uint32_t nslots) {
   __shared__ Ring rings[WARPS];
   __shared__ Stage stages[WARPS];
   int tile = blockIdx.x, k = blockIdx.y;
@@ -399,9 +327,7 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
     cp_async_wait<1>();
     __syncwarp();
     unsigned m = 0;
-    if (start + lane < bmax)
-      m = MASK ? (unsigned)item_mask[(size_t)warp * mask_stride + r0 + start + lane]
-                    : cull_mask(ring.q[buf][lane], ring.q[buf][32 + lane], (float)X0, (float)Y0, log2_amin);
+    if (start + lane < bmax) m = cull_mask(ring.q[buf][0][lane], ring.q[buf][1][lane], (float)X0, (float)Y0, log2_amin);
     unsigned reach = 0;                              // slots in which some pixel's walk reaches this batch
 #pragma unroll
     for (int s = 0; s < 4; ++s) if (smax[s] > start) reach |= 1u << s;
@@ -412,7 +338,7 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
       live &= ~(1u << j);
       const uint32_t c1 = start + (uint32_t)j + 1;    // 1-based list position
       const unsigned mj = __shfl_sync(FULL, m, j);
-      const float4 a = ring.q[buf][j], b = ring.q[buf][32 + j], c = ring.q[buf][64 + j];
+      const float4 a = ring.q[buf][0][j], b = ring.q[buf][1][j], c = ring.q[buf][2][j];
       const float dxs[2] = {__fsub_rn(a.x, px0), __fsub_rn(a.x, px1)};
       const float dys[2] = {__fsub_rn(a.y, py0), __fsub_rn(a.y, py1)};
       const float adx[2] = {__fmul_rn(b.x, dxs[0]), __fmul_rn(b.x, dxs[1])};
@@ -466,11 +392,6 @@ k_raster_bwd(const float* __restrict__ blend, const uint32_t* __restrict__ vals,
 
 }  // namespace
 
-// experiment state (variant 4): the forward's per-(half tile, entry) slot masks, valid for the binning they were written for
-static uint8_t* g_item_mask = nullptr;
-static uint64_t g_mask_cap = 0;
-static const void* g_mask_valid_for = nullptr;
-
 int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binning* bins, const PlanDev& plan,
                       const splx_partial* out, uint64_t* pairs) {
   const int sparse = (plan.flags & SPLX_PLAN_SPARSE) ? 1 : 0;
@@ -478,46 +399,14 @@ int launch_render_fwd(splx_ctx* ctx, const splx_projected* pr, const splx_binnin
   // longest list first only where empty slots need no visit (without SPLX_PLAN_SPARSE they get the identity partial)
   const uint32_t* order = sparse && slot_order_pays(plan) ? bins->slot_order : nullptr;
   const dim3 grid = order ? dim3(nslots, 1) : dim3(plan.ntiles, plan.K);
-  // EXPERIMENT switch (removed again once measured): 0 = product, 1 = 8 pixels per lane, 2 = bulk-copy stream
-  static const int variant = getenv("SPLX_RENDER_VARIANT") ? atoi(getenv("SPLX_RENDER_VARIANT")) : 0;
-  if ((variant == 4 || variant == 5) && !pairs) {
-    if (g_mask_cap < bins->capacity) {
-      if (g_item_mask) cudaFree(g_item_mask);
-      if (cudaMalloc(&g_item_mask, (size_t)bins->capacity * 2) != cudaSuccess) SPLX_FAIL(ctx, SPLX_ERR_CUDA, "item mask buffer");
-      g_mask_cap = bins->capacity;
-    }
-    g_mask_valid_for = bins->vals;
-    if (variant == 4)
-      k_render_fwd<false, 4, false, 1><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
-          plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d, out->n_contrib, nullptr, order, nslots, 0, g_item_mask, g_mask_cap);
-    else
-      k_render_fwd<false, 4, false, 2><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
-          plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d, out->n_contrib, nullptr, order, nslots, 0, g_item_mask, g_mask_cap);
-    SPLX_LAUNCH_CHECK(ctx, "k_render_fwd");
-    return SPLX_OK;
-  }
-  g_mask_valid_for = nullptr;
-#define RENDER_ARGS(BLEND)                                                                                                  \
-  BLEND, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX, plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d, \
-      out->n_contrib, (unsigned long long*)pairs, order, nslots
-  if (variant == 1 && !pairs) {
-    k_render_fwd<false, 8, false><<<grid, 32, 0, ctx->stream>>>(RENDER_ARGS(pr->blend));
-  } else if (variant == 2 && !pairs) {
-    static float4* sorted = nullptr;
-    static uint64_t sorted_cap = 0;
-    if (sorted_cap < bins->capacity) {
-      if (sorted) cudaFree(sorted);
-      if (cudaMalloc(&sorted, (size_t)bins->capacity * 48) != cudaSuccess) SPLX_FAIL(ctx, SPLX_ERR_CUDA, "stream buffer");
-      sorted_cap = bins->capacity;
-    }
-    k_gather_blend<<<148 * 8, 256, 0, ctx->stream>>>((const float4*)pr->blend, bins->vals, bins->num_intersections, sorted);
-    k_render_fwd<false, 4, true><<<grid, BLOCK, 0, ctx->stream>>>(RENDER_ARGS((const float*)sorted));
-  } else if (pairs) {
-    k_render_fwd<true, 4, false><<<grid, BLOCK, 0, ctx->stream>>>(RENDER_ARGS(pr->blend), variant == 3);
-  } else {
-    k_render_fwd<false, 4, false><<<grid, BLOCK, 0, ctx->stream>>>(RENDER_ARGS(pr->blend));
-  }
-#undef RENDER_ARGS
+  if (pairs)
+    k_render_fwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
+                                                        plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d,
+                                                        out->n_contrib, (unsigned long long*)pairs, order, nslots);
+  else
+    k_render_fwd<false><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
+                                                         plan.ntiles, ctx->cfg, plan.pv, sparse, out->ct, out->d,
+                                                         out->n_contrib, nullptr, order, nslots);
   SPLX_LAUNCH_CHECK(ctx, "k_render_fwd");
   return SPLX_OK;
 }
@@ -528,12 +417,8 @@ int launch_raster_bwd(splx_ctx* ctx, const splx_projected* pr, const splx_binnin
   const uint32_t* order = slot_order_pays(plan) ? bins->slot_order : nullptr;
   // slots of non-participating partitions have empty ranges: they exit at once / are not in the order
   const dim3 grid = order ? dim3(nslots, 1) : dim3(plan.ntiles, plan.K);
-  if (g_mask_valid_for == bins->vals)
-    k_raster_bwd<true><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX, plan.ntiles,
-                                                        ctx->cfg, part->ct, part->n_contrib, g_ct, g2d, order, nslots, g_item_mask, g_mask_cap);
-  else
-    k_raster_bwd<false><<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX, plan.ntiles,
-                                                         ctx->cfg, part->ct, part->n_contrib, g_ct, g2d, order, nslots, nullptr, 0);
+  k_raster_bwd<<<grid, BLOCK, 0, ctx->stream>>>(pr->blend, bins->vals, bins->tile_ranges, plan.W, plan.H, plan.TX,
+                                                plan.ntiles, ctx->cfg, part->ct, part->n_contrib, g_ct, g2d, order, nslots);
   SPLX_LAUNCH_CHECK(ctx, "k_raster_bwd");
   return SPLX_OK;
 }

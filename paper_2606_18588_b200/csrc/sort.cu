@@ -119,8 +119,8 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
 // HIST (the compaction scan): the CTA also counts the four 8-bit digit histograms of the keys it stores (shared
 // atomics, flushed once per CTA) and clears the radix passes' look-back status words of tile t -- output tile t of
 // the depth sort can only hold elements of input tiles <= t -- so the depth sort needs no histogram kernel.
-template <class Op, bool HIST, int MINB = 2>
-__global__ void __launch_bounds__(SCAN_THREADS, MINB)
+template <class Op, bool HIST>
+__global__ void __launch_bounds__(SCAN_THREADS, 2)
 k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
        uint64_t clamp_to, uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
   __shared__ uint32_t sm[33];
@@ -162,7 +162,7 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     if (threadIdx.x == 0) {
       uint64_t excl = 0;
       if (t == 0) st_status(status, ST_PREFIX | (uint64_t)total);
-      else excl = lookback<MINB == 2 ? 16 : 8>(status, t, 1, total);
+      else excl = lookback<16>(status, t, 1, total);
       s_excl = excl;
       if (t + 1 == ntiles) {
         const uint64_t grand = excl + total;
@@ -255,12 +255,6 @@ int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_pt
   uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
   if (nb == 0) return SPLX_OK;
   if (nb > PERSISTENT_CTAS) nb = PERSISTENT_CTAS;
-  static const int minb = getenv("SPLX_SCAN_MINB") ? atoi(getenv("SPLX_SCAN_MINB")) : 2;     // EXPERIMENT switch
-  if (minb == 3)
-    k_scan<Op, HIST, 3><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to, ghist, rstatus, rstride);
-  else if (minb == 4)
-    k_scan<Op, HIST, 4><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to, ghist, rstatus, rstride);
-  else
   k_scan<Op, HIST><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to, ghist,
                                                          rstatus, rstride);
   SPLX_LAUNCH_CHECK(ctx, HIST ? "k_scan<VisibleOp>" : "k_scan<TouchedOp>");
@@ -318,7 +312,7 @@ struct FinalOut {
 // shared memory, the per-digit prefix over the tiles by look-back, the scatter.  FULL: every one of the RS_TILE
 // positions holds a key.  NB = number of digit values (256: 8-bit digits; 512: 9-bit digits, two per thread in the
 // per-digit phases -- 17 or 18 slot bits then take two passes instead of three).
-template <typename KeyT, bool FINAL, bool FULL, int NB, bool MATCH = false>
+template <typename KeyT, bool FINAL, bool FULL, int NB>
 __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
                                            uint32_t* __restrict__ vout, uint64_t start, uint32_t nv, uint32_t t, int shift,
                                            int bits, uint32_t mask, uint64_t* status, const FinalOut& fin, uint32_t (*whist)[NB],
@@ -347,8 +341,6 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
     dg[it] = d;
     // lanes of the warp with this lane's digit: one ballot per digit bit; (bit - 1) is all ones for a clear bit
     unsigned peers = FULL ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
-    if (MATCH) peers = __match_any_sync(0xffffffffu, valid ? d : 0xffffffffu);     // experiment: MATCH.ANY instead of the votes
-    else
 #pragma unroll
     for (int b = 0; b < MAXB; ++b) {
       if (b < bits) {            // (uniform) a pass of fewer bits votes on those only
@@ -424,7 +416,7 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
 
 // Persistent: tiles are taken from the ticket counter in order, so every predecessor of a running tile has
 // started and the look-back spin cannot wait on a CTA that was never scheduled.
-template <typename KeyT, bool FINAL, int NB, bool MATCH = false>
+template <typename KeyT, bool FINAL, int NB>
 __global__ void __launch_bounds__(RS_THREADS, 4)
 k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, KeyT* __restrict__ kout,
              uint32_t* __restrict__ vout, const uint64_t* n_ptr, const uint32_t* __restrict__ ghist /*[NB] of this pass*/,
@@ -465,9 +457,9 @@ k_radix_pass(const KeyT* __restrict__ kin, const uint32_t* __restrict__ vin, Key
     // the kernel is bound by instruction issue (ncu, city_100M: 62 % issue slots, DRAM 13 %): a full tile -- all but the
     // last one -- takes the copy of the body without the per-item range checks
     if (nv == RS_TILE)
-      radix_tile<KeyT, FINAL, true, NB, MATCH>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+      radix_tile<KeyT, FINAL, true, NB>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
     else
-      radix_tile<KeyT, FINAL, false, NB, MATCH>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
+      radix_tile<KeyT, FINAL, false, NB>(kin, vin, kout, vout, start, nv, t, shift, bits, mask, status, fin, whist, dbase, gbase, lbase, skey, sval, sm);
   }
 }
 
@@ -486,14 +478,10 @@ int radix_sort(splx_ctx* ctx, KeyT* ka, uint32_t* va, KeyT* kb, uint32_t* vb, ui
   const PassPlan plan = plan_passes(begin_bit, end_bit, NB == 256 ? 8 : 9);
   FinalOut none;
   memset(&none, 0, sizeof none);
-  static const bool match = getenv("SPLX_SORT_MATCH") != nullptr;     // EXPERIMENT switch, removed once measured
   for (int p = 0; p < plan.npass; ++p) {
 #define PASS_ARGS(F) ka, va, kb, vb, n_ptr, ghist + NB * p, status + (size_t)p * stride, tickets + p, plan.shift[p], plan.bits[p], F
-    const bool last = fin && p + 1 == plan.npass;
-    if (last && match) k_radix_pass<KeyT, true, NB, true><<<nblocks, RS_THREADS, 0, ctx->stream>>>(PASS_ARGS(*fin));
-    else if (last) k_radix_pass<KeyT, true, NB, false><<<nblocks, RS_THREADS, 0, ctx->stream>>>(PASS_ARGS(*fin));
-    else if (match) k_radix_pass<KeyT, false, NB, true><<<nblocks, RS_THREADS, 0, ctx->stream>>>(PASS_ARGS(none));
-    else k_radix_pass<KeyT, false, NB, false><<<nblocks, RS_THREADS, 0, ctx->stream>>>(PASS_ARGS(none));
+    if (fin && p + 1 == plan.npass) k_radix_pass<KeyT, true, NB><<<nblocks, RS_THREADS, 0, ctx->stream>>>(PASS_ARGS(*fin));
+    else k_radix_pass<KeyT, false, NB><<<nblocks, RS_THREADS, 0, ctx->stream>>>(PASS_ARGS(none));
 #undef PASS_ARGS
     SPLX_LAUNCH_CHECK(ctx, "k_radix_pass");
     KeyT* tk = ka; ka = kb; kb = tk;
