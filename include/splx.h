@@ -195,6 +195,21 @@ size_t splx_dssim_ws_floats(const splx_camera *cam);
 int splx_dssim_loss_grad(splx_ctx *ctx, int n_views, const splx_camera *cam, const float *image, const float *target,
                          float lambda, float scale, float *dL_dimage, double *loss_sum, float *ws);
 
+/* The same loss and gradient for callers that MUST NOT allocate (code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc) and cannot bring a workspace: the scratch of the two kernels (the nine derivative
+ * planes that splx_dssim_loss_grad keeps in `ws`) lives in a file-scope `static __device__` array inside the library,
+ * SPLX_DSSIM_STATIC_MAX_PIXELS * 9 floats = 9 MiB, which every GPU that loads libsplx.so holds until the process exits.
+ * Same arguments, same kernels, same results as splx_dssim_loss_grad.  Limit: n_views * W * H <=
+ * SPLX_DSSIM_STATIC_MAX_PIXELS (e.g. one 512 x 512 view); beyond it the call returns SPLX_ERR_WORKSPACE with the two
+ * numbers in splx_last_error and launches nothing.  The call performs no cudaMalloc / cudaFree and calls no allocating
+ * library routine (the first call on a device looks the array's address up with cudaGetSymbolAddress).  ALL calls on a
+ * device share the one array, which keeps the previous call's contents: nothing in it needs to start at zero (the
+ * forward kernel writes every plane element the backward kernel reads), but two calls that OVERLAP on the GPU (different
+ * streams or contexts on one device) race on it -- serialise them, or use splx_dssim_loss_grad with separate workspaces. */
+#define SPLX_DSSIM_STATIC_MAX_PIXELS 262144
+int splx_dssim_loss_grad_static(splx_ctx *ctx, int n_views, const splx_camera *cam, const float *image, const float *target,
+                                float lambda, float scale, float *dL_dimage, double *loss_sum);
+
 /* ---- a8 composition backward: Eq.6-7.  g_ct[K,H,W,4] =
  * (dL/dC^k rgb, dL/dT^k).  dL_dT_total[H,W] may be NULL.  Overwrites g_ct. */
 int splx_compose_backward(splx_ctx *ctx, int K, const splx_partial *partials,

@@ -36,9 +36,10 @@ EXPORTS = [
     "splx_compose_l1_backward_plan",
     "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
     "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
-    "splx_adam_groups_flagged", "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_iteration", "splx_microbench",
+    "splx_adam_groups_flagged", "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_dssim_loss_grad_static", "splx_iteration", "splx_microbench",
 ]
 MAX_VIEWS = 8
+DSSIM_STATIC_MAX_PIXELS = 262144
 TILE_INVISIBLE, TILE_SATURATED = 1, 2
 PLAN_SPARSE = 1
 ORDER_EXTRA = 1025
@@ -165,6 +166,7 @@ def lib():
         L.splx_dssim_ws_floats.restype = C.c_size_t
         L.splx_dssim_ws_floats.argtypes = [vp]
         L.splx_dssim_loss_grad.argtypes = [vp, C.c_int, vp, vp, vp, C.c_float, C.c_float, vp, vp, vp]
+        L.splx_dssim_loss_grad_static.argtypes = [vp, C.c_int, vp, vp, vp, C.c_float, C.c_float, vp, vp]
         L.splx_adam_groups_flagged.argtypes = [vp, vp, vp, vp, vp, C.c_int, vp, vp, C.c_int64, vp, vp, C.c_float, C.c_float,
                                                C.c_float, C.c_int, C.c_float]
         L.splx_microbench.argtypes = [vp, C.c_int, C.c_int64, vp, vp]
@@ -606,6 +608,14 @@ class Context:
         cs = camera_struct(cam)
         self._check(lib().splx_dssim_loss_grad(self._h, B, C.byref(cs), _ptr(image), _ptr(target), float(lam),
                                                float(B if scale is None else scale), _ptr(g_image), _ptr(loss_sum), _ptr(ws)))
+
+    def dssim_loss_grad_static(self, cam, image, target, g_image, loss_sum, lam, scale=None):
+        """splx_dssim_loss_grad_static: the same with the scratch in the library's static device array (no allocation;
+        n_views * W * H <= DSSIM_STATIC_MAX_PIXELS)."""
+        B = image.shape[0] if image.dim() == 4 else 1
+        cs = camera_struct(cam)
+        self._check(lib().splx_dssim_loss_grad_static(self._h, B, C.byref(cs), _ptr(image), _ptr(target), float(lam),
+                                                      float(B if scale is None else scale), _ptr(g_image), _ptr(loss_sum)))
 
     def iteration(self, trainset: "TrainsetS", buckets, n_views, targets, images_out=None, loss_out=None, m_out=None,
                   host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None):

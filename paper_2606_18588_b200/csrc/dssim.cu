@@ -188,3 +188,41 @@ int launch_dssim(splx_ctx* ctx, int B, int W, int H, const ViewBufs& vb, float l
   SPLX_LAUNCH_CHECK(ctx, "k_dssim_bwd");
   return SPLX_OK;
 }
+
+// ---- splx_dssim_loss_grad_static: the entry point that allocates nothing (include/splx.h) ----------------------------
+// The scratch is a file-scope device array.  In HOST code its name is a host-side stand-in, not a device address: the
+// address comes from cudaGetSymbolAddress, looked up once per device with that device current, and only that pointer
+// is handed to the kernels.
+static __device__ __align__(256) float g_dssim_scratch[(size_t)9 * SPLX_DSSIM_STATIC_MAX_PIXELS];
+
+namespace {
+constexpr int MAX_DEVICES = 64;
+float* g_scratch_ptr[MAX_DEVICES];      // device address of g_dssim_scratch on device d, nullptr until looked up
+}  // namespace
+
+extern "C" int splx_dssim_loss_grad_static(splx_ctx* ctx, int n_views, const splx_camera* cam, const float* image,
+                                           const float* target, float lambda, float scale, float* dL_dimage, double* loss_sum) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!cam || cam->width <= 0 || cam->height <= 0 || n_views < 1 || n_views > SPLX_MAX_VIEWS || !image || !target ||
+      !dL_dimage || !(lambda >= 0.f))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_dssim_loss_grad_static: null argument, bad size, n_views not in [1,%d] or lambda < 0",
+              SPLX_MAX_VIEWS);
+  const long long pixels = (long long)n_views * cam->width * cam->height;
+  if (pixels > (long long)SPLX_DSSIM_STATIC_MAX_PIXELS)
+    SPLX_FAIL(ctx, SPLX_ERR_WORKSPACE, "splx_dssim_loss_grad_static: n_views * W * H = %lld pixels exceed the static scratch of %d "
+              "pixels (SPLX_DSSIM_STATIC_MAX_PIXELS); use splx_dssim_loss_grad with a workspace", pixels, SPLX_DSSIM_STATIC_MAX_PIXELS);
+  if (ctx->device < 0 || ctx->device >= MAX_DEVICES) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_dssim_loss_grad_static: device %d", ctx->device);
+  float* ws = g_scratch_ptr[ctx->device];
+  if (!ws) {   // set-up, once per device: the symbol's address ON THE CONTEXT'S DEVICE
+    int cur = -1;
+    SPLX_CUDA_OK(ctx, cudaGetDevice(&cur));
+    if (cur != ctx->device) SPLX_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+    const cudaError_t e = cudaGetSymbolAddress((void**)&ws, g_dssim_scratch);
+    if (cur != ctx->device) cudaSetDevice(cur);
+    if (e != cudaSuccess || !ws) SPLX_FAIL(ctx, SPLX_ERR_CUDA, "cudaGetSymbolAddress(g_dssim_scratch) failed: %s", cudaGetErrorString(e));
+    g_scratch_ptr[ctx->device] = ws;
+  }
+  const ViewBufs vb = contiguous_views(n_views, (size_t)cam->width * cam->height, target, const_cast<float*>(image), nullptr,
+                                       dL_dimage, nullptr);
+  return launch_dssim(ctx, n_views, cam->width, cam->height, vb, lambda, scale, loss_sum, ws);
+}
