@@ -173,6 +173,52 @@ __device__ __forceinline__ void colour(const float4* sh4, int lane, const CamDev
   out.clamp[i] = cl;
 }
 
+// Reach test of a mean (reading s21): can a Gaussian of scale <= smax at this mean touch the image at all?  smax < 0:
+// no bound is known, every Gaussian goes through the full test.
+__device__ __forceinline__ bool reaches(const float* m, const CamDev& cam, float smax) {
+  if (!(smax >= 0.f)) return true;
+  const float x = cam.R[0] * m[0] + cam.R[1] * m[1] + cam.R[2] * m[2] + cam.t[0];
+  const float y = cam.R[3] * m[0] + cam.R[4] * m[1] + cam.R[5] * m[2] + cam.t[1];
+  const float z = cam.R[6] * m[0] + cam.R[7] * m[1] + cam.R[8] * m[2] + cam.t[2];
+  const float h = 3.0f * cam.reach_c * smax, fxx = cam.fx * x, fyy = cam.fy * y;
+  return z > cam.near_z * 0.999f && fxx <= cam.reach_r * z + h && -fxx <= cam.reach_l * z + h &&
+         fyy <= cam.reach_b * z + h && -fyy <= cam.reach_t * z + h;
+}
+
+// The geometry half of Gaussian i (its mean already in gin.m): covariance, footprint, tile count; a visible one gets its
+// parity outputs and the first two quarters of its blend record.  Returns the visibility; writes nothing for a culled one.
+__device__ __forceinline__ bool project_one(const splx_gaussians& g, int64_t i, GeoIn& gin, const CamDev& cam,
+                                            const splx_config& cfg, const splx_projected& out) {
+  Geo G;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) gin.ls[k] = g.log_scale[3 * i + k];
+  gin.q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
+  if (!geometry(gin, cam, cfg.dilation, G)) return false;
+  const float mid = 0.5f * (G.a + G.c);
+  const float hd = 0.5f * (G.a - G.c);
+  const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
+  const int rad = (int)ceilf(3.0f * sqrtf(lam));
+  const float iz = 1.0f / G.p[2];
+  const float u = cam.fx * G.p[0] * iz + cam.cx;
+  const float v = cam.fy * G.p[1] * iz + cam.cy;
+  int x0, y0, x1, y1;
+  tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
+  const int tt = (x1 - x0) * (y1 - y0);
+  if (tt <= 0) return false;
+  float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+  const float idet = 1.0f / G.det;
+  const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
+  *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
+  out.depth[i] = G.p[2];
+  const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
+  *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
+  out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
+  constexpr float kLog2e = 1.4426950408889634f;
+  bl[0] = make_float4(u, v, op, G.p[2]);
+  bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
+  return true;
+}
+
 // SH rows: a thread-per-Gaussian read of its 192-byte row is a 192-byte stride across the warp -- every 16-byte load
 // instruction touches 32 different lines (32 L1 wavefronts instead of 4) and the kernel ran at half the HBM roof,
 // bound by the L1's wavefront rate (ncu: lg_throttle + long_scoreboard stalls).  The 32 rows of a warp are 6 KB of
@@ -199,57 +245,16 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   float m[3] = {0.f, 0.f, 0.f};
   bool vis = false;
   if (active) {
-    Geo G;
     GeoIn gin;
 #pragma unroll
     for (int k = 0; k < 3; ++k) gin.m[k] = g.mean[3 * i + k];
     // reach test on the mean alone (splx_plan.max_scale, reading s21): most Gaussians of a city view fail it, and their
     // scale and rotation (28 of the 40 bytes a culled Gaussian costs) are never read
-    bool reach = true;
-    const float smax = plan.max_scale[rt.part[r]];
-    if (smax >= 0.f) {
-      const float x = cam.R[0] * gin.m[0] + cam.R[1] * gin.m[1] + cam.R[2] * gin.m[2] + cam.t[0];
-      const float y = cam.R[3] * gin.m[0] + cam.R[4] * gin.m[1] + cam.R[5] * gin.m[2] + cam.t[1];
-      const float z = cam.R[6] * gin.m[0] + cam.R[7] * gin.m[1] + cam.R[8] * gin.m[2] + cam.t[2];
-      const float h = 3.0f * cam.reach_c * smax, fxx = cam.fx * x, fyy = cam.fy * y;
-      reach = z > cam.near_z * 0.999f && fxx <= cam.reach_r * z + h && -fxx <= cam.reach_l * z + h &&
-              fyy <= cam.reach_b * z + h && -fyy <= cam.reach_t * z + h;
-    }
-    if (reach) {
-#pragma unroll
-      for (int k = 0; k < 3; ++k) gin.ls[k] = g.log_scale[3 * i + k];
-      gin.q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
-      vis = geometry(gin, cam, cfg.dilation, G);
-    }
-    float u = 0.f, v = 0.f;
-    int rad = 0, tt = 0;
-    if (vis) {
-      const float mid = 0.5f * (G.a + G.c);
-      const float hd = 0.5f * (G.a - G.c);
-      const float lam = mid + sqrtf(fmaxf(cfg.radius_floor, hd * hd + G.b * G.b));  // mid^2 - det
-      rad = (int)ceilf(3.0f * sqrtf(lam));
-      const float iz = 1.0f / G.p[2];
-      u = cam.fx * G.p[0] * iz + cam.cx;
-      v = cam.fy * G.p[1] * iz + cam.cy;
-      int x0, y0, x1, y1;
-      tile_rect(u, v, rad, cam.TX, cam.TY, x0, y0, x1, y1);
-      tt = (x1 - x0) * (y1 - y0);
-      vis = tt > 0;
-    }
-    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+    const bool reach = reaches(gin.m, cam, plan.max_scale[rt.part[r]]);
+    vis = reach && project_one(g, i, gin, cam, cfg, out);
     if (!vis) {   // a culled Gaussian: radius = tiles_touched = 0 say so; nothing downstream reads its other attributes, and
       out.radius[i] = 0; out.tiles_touched[i] = 0;     // writing 129 bytes of zeros for it was most of this kernel's traffic
     } else {
-      const float idet = 1.0f / G.det;
-      const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
-      *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
-      out.depth[i] = G.p[2];
-      const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
-      *reinterpret_cast<float4*>(out.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
-      out.radius[i] = rad; out.tiles_touched[i] = (uint32_t)tt;
-      constexpr float kLog2e = 1.4426950408889634f;
-      bl[0] = make_float4(u, v, op, G.p[2]);
-      bl[1] = make_float4(cA * (-0.5f * kLog2e), cB * (-kLog2e), cC * (-0.5f * kLog2e), __uint_as_float((uint32_t)i));
       m[0] = gin.m[0]; m[1] = gin.m[1]; m[2] = gin.m[2];
     }
   }
@@ -276,6 +281,56 @@ k_project_fwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     return;
   }
   if (vis) colour<DEG, false>(reinterpret_cast<const float4*>(g.sh + 48 * i), lane, cam, m, i, out, bl);
+}
+
+// The geometry half alone (splx_project_geometry_plan), in two phases per block of PG_TILE consecutive Gaussians.  On a
+// city view ~85 % of the participating Gaussians fail the reach test on their mean and the few that pass are scattered
+// over the warps: in the thread-per-Gaussian kernel above nearly every warp then ran the whole covariance chain (~300
+// instructions) for 4 of its 32 lanes, and a thread had ONE mean in flight.  Phase 1: every thread tests PG_ITEMS means
+// (their loads issued together), marks the ones that fail and appends the others to a list in shared memory; phase 2:
+// the block walks the list with full warps.  Same arithmetic per Gaussian (project_one): bit-equal outputs.
+constexpr int PG_ITEMS = 4;
+constexpr int PG_TILE = PROJ_THREADS * PG_ITEMS;
+__global__ void __launch_bounds__(PROJ_THREADS)
+k_project_geo(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt, splx_config cfg,
+              splx_projected out) {
+  __shared__ uint32_t s_list[PG_TILE];
+  __shared__ uint32_t s_n;
+  const int r = find_run(rt, (int)blockIdx.x);
+  const int64_t base = rt.begin[r] + (int64_t)((int)blockIdx.x - rt.block_prefix[r]) * PG_TILE;
+  const int64_t end = rt.end[r];
+  const CamDev& cam = plan.cam[rt.view[r]];
+  const float smax = plan.max_scale[rt.part[r]];
+  if (threadIdx.x == 0) s_n = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  float m[PG_ITEMS][3];
+#pragma unroll
+  for (int it = 0; it < PG_ITEMS; ++it) {
+    const int64_t i = base + it * PROJ_THREADS + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) m[it][k] = i < end ? g.mean[3 * i + k] : 0.f;
+  }
+#pragma unroll
+  for (int it = 0; it < PG_ITEMS; ++it) {
+    const int64_t i = base + it * PROJ_THREADS + threadIdx.x;
+    const bool reach = i < end && reaches(m[it], cam, smax);
+    if (i < end && !reach) { out.radius[i] = 0; out.tiles_touched[i] = 0; }
+    const unsigned bal = __ballot_sync(0xffffffffu, reach);
+    uint32_t pos = 0;
+    if (lane == 0 && bal) pos = atomicAdd(&s_n, (uint32_t)__popc(bal));
+    pos = __shfl_sync(0xffffffffu, pos, 0);
+    if (reach) s_list[pos + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)(it * PROJ_THREADS + threadIdx.x);
+  }
+  __syncthreads();
+  const uint32_t cnt = s_n;
+  for (uint32_t j = threadIdx.x; j < cnt; j += PROJ_THREADS) {
+    const int64_t i = base + s_list[j];
+    GeoIn gin;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) gin.m[k] = g.mean[3 * i + k];
+    if (!project_one(g, i, gin, cam, cfg, out)) { out.radius[i] = 0; out.tiles_touched[i] = 0; }
+  }
 }
 
 // The colour of the visible Gaussians (the binning's list, index order): one thread per entry, persistent grid because
@@ -664,11 +719,12 @@ int launch_project_fwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& pl
 #define PF(D, C) k_project_fwd<D, C><<<grid, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rt, ctx->cfg, *out)
   if (with_colour) {
     switch (deg) { case 0: PF(0, true); break; case 1: PF(1, true); break; case 2: PF(2, true); break; default: PF(3, true); break; }
-  } else {
-    PF(0, false);     // the degree only matters to the colour
+  } else {               // the degree only matters to the colour
+    const RunTable rg = make_runs(plan, part_offsets, PG_TILE, false);
+    k_project_geo<<<(unsigned)rg.blocks_total, PROJ_THREADS, 0, ctx->stream>>>(*g, plan, rg, ctx->cfg, *out);
   }
 #undef PF
-  SPLX_LAUNCH_CHECK(ctx, "k_project_fwd");
+  SPLX_LAUNCH_CHECK(ctx, with_colour ? "k_project_fwd" : "k_project_geo");
   return SPLX_OK;
 }
 
