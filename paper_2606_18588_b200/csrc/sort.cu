@@ -116,20 +116,13 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s
 
 // Persistent: a CTA keeps taking tiles from the ticket counter until the (device-side) element count is
 // exhausted, so the grid is sized for the machine, not for the caller's capacity.
-// HIST (the compaction scan): the CTA also counts the four 8-bit digit histograms of the keys it stores (shared
-// atomics, flushed once per CTA) and clears the radix passes' look-back status words of tile t -- output tile t of
-// the depth sort can only hold elements of input tiles <= t -- so the depth sort needs no histogram kernel.
-template <class Op, bool HIST>
+template <class Op>
 __global__ void __launch_bounds__(SCAN_THREADS, 2)
 k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket, uint64_t* total_out, uint64_t* clamp_out,
-       uint64_t clamp_to, uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+       uint64_t clamp_to) {
   __shared__ uint32_t sm[33];
   __shared__ uint32_t s_tile;
   __shared__ uint64_t s_excl;
-  __shared__ uint32_t s_hist[HIST ? 4 * 256 : 1];
-  if (HIST) {
-    for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) s_hist[x] = 0;
-  }
   const uint64_t n = op.count(n_ptr);
   const uint64_t ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
   if (n == 0) {
@@ -145,13 +138,6 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     __syncthreads();
     const uint32_t t = s_tile;
     if (t >= ntiles) break;
-    if (HIST) {
-#pragma unroll
-      for (int x = threadIdx.x; x < 4 * 256 * SCAN_RS; x += SCAN_THREADS) {   // pass x / (256 SCAN_RS), radix tiles SCAN_RS t ..
-        const int pass = x / (256 * SCAN_RS), w = x - pass * (256 * SCAN_RS);
-        rstatus[(size_t)pass * rstride + (size_t)t * (256 * SCAN_RS) + w] = 0;
-      }
-    }
     const uint64_t base = (uint64_t)t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
     uint32_t v[SCAN_IPT], s = 0;
     op.load_all(base, n, v);                 // the thread's SCAN_IPT elements are consecutive
@@ -172,11 +158,7 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     }
     __syncthreads();
     ex += (uint32_t)s_excl;
-    op.store_all(base, n, v, ex, s_hist);
-  }
-  if (HIST) {
-    __syncthreads();
-    for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
+    op.store_all(base, n, v, ex, nullptr);
   }
 }
 
@@ -248,16 +230,102 @@ struct TouchedOp {  // step 3: offsets of each visible Gaussian's run of keys, d
   }
 };
 
-template <class Op, bool HIST>
+template <class Op>
 int scan_exclusive(splx_ctx* ctx, Op op, uint64_t capacity, const uint64_t* n_ptr, uint64_t* status, uint32_t* ticket,
-                   uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to, uint32_t* ghist = nullptr,
-                   uint64_t* rstatus = nullptr, size_t rstride = 0) {
+                   uint64_t* total_out, uint64_t* clamp_out, uint64_t clamp_to) {
   uint32_t nb = (uint32_t)((capacity + SCAN_TILE - 1) / SCAN_TILE);
   if (nb == 0) return SPLX_OK;
   if (nb > PERSISTENT_CTAS) nb = PERSISTENT_CTAS;
-  k_scan<Op, HIST><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to, ghist,
-                                                         rstatus, rstride);
-  SPLX_LAUNCH_CHECK(ctx, HIST ? "k_scan<VisibleOp>" : "k_scan<TouchedOp>");
+  k_scan<Op><<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, n_ptr, status, ticket, total_out, clamp_out, clamp_to);
+  SPLX_LAUNCH_CHECK(ctx, "k_scan<TouchedOp>");
+  return SPLX_OK;
+}
+
+// ------------------------------------------------- step 1: compaction of the visible Gaussians --
+// Count -> scan -> scatter in three launches.  (It used to be ONE decoupled look-back scan: at city scale -- 40-50 M
+// participating Gaussians per bucket, 13 % of them visible -- that kernel ran at 1 TB/s with its warps waiting at the
+// barrier behind the one thread that walks back over the predecessors' status words, 0.35-0.42 ms per bucket; and it
+// cleared the depth sort's look-back words for as many tiles as there are PARTICIPATING Gaussians, as many bytes as it
+// read.)  Nothing here waits on another CTA: k_vis_count streams tiles_touched once (a count per SCAN_TILE elements),
+// k_vis_offsets scans the counts in one CTA and publishes N_visible, k_vis_compact reads tiles_touched again, ranks
+// inside the tile and scatters (depth bits, index), the index-ordered list, the four digit histograms of the depth sort,
+// and clears the status words of the tiles the depth sort will really use.
+__global__ void __launch_bounds__(SCAN_THREADS)
+k_vis_count(const __grid_constant__ VisibleOp op, uint32_t* __restrict__ tile_counts) {
+  __shared__ uint32_t sm[SCAN_THREADS / 32];
+  const uint64_t n = op.n, ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+  for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const uint64_t base = t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
+    uint32_t v[SCAN_IPT], s = 0;
+    op.load_all(base, n, v);
+#pragma unroll
+    for (int k = 0; k < SCAN_IPT; ++k) s += v[k];
+    s = __reduce_add_sync(0xffffffffu, s);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+      uint32_t w = threadIdx.x < SCAN_THREADS / 32 ? sm[threadIdx.x] : 0u;
+      w = __reduce_add_sync(0xffffffffu, w);
+      if (threadIdx.x == 0) tile_counts[t] = w;
+    }
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(1024)
+k_vis_offsets(uint32_t* __restrict__ tile_counts, uint64_t ntiles, uint64_t* __restrict__ n_visible) {
+  __shared__ uint32_t sm[33];
+  uint32_t running = 0;
+  for (uint64_t b = 0; b < ntiles; b += 1024) {
+    const uint64_t t = b + threadIdx.x;
+    const uint32_t c = t < ntiles ? tile_counts[t] : 0u;
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(c, sm, total);
+    if (t < ntiles) tile_counts[t] = running + ex;
+    running += total;
+  }
+  if (threadIdx.x == 0) *n_visible = running;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS, 2)
+k_vis_compact(const __grid_constant__ VisibleOp op, const uint32_t* __restrict__ tile_offsets, const uint64_t* __restrict__ n_visible,
+              uint32_t* __restrict__ ghist, uint64_t* __restrict__ rstatus, size_t rstride) {
+  __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_hist[4 * 256];
+  for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) s_hist[x] = 0;
+  // look-back status words of the four passes of the depth sort: 256 per tile of RS_TILE visible Gaussians
+  const uint64_t words = ((*n_visible + RS_TILE - 1) / RS_TILE) * 256;
+  for (uint64_t x = (uint64_t)blockIdx.x * SCAN_THREADS + threadIdx.x; x < words; x += (uint64_t)gridDim.x * SCAN_THREADS) {
+#pragma unroll
+    for (int pass = 0; pass < 4; ++pass) rstatus[(size_t)pass * rstride + x] = 0;
+  }
+  __syncthreads();
+  const uint64_t n = op.n, ntiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+  for (uint64_t t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const uint64_t base = t * SCAN_TILE + (uint64_t)threadIdx.x * SCAN_IPT;
+    uint32_t v[SCAN_IPT], s = 0;
+    op.load_all(base, n, v);
+#pragma unroll
+    for (int k = 0; k < SCAN_IPT; ++k) s += v[k];
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(s, sm, total) + tile_offsets[t];
+    if (total) op.store_all(base, n, v, ex, s_hist);
+  }
+  __syncthreads();
+  for (int x = threadIdx.x; x < 4 * 256; x += SCAN_THREADS) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
+}
+
+static int compact_visible(splx_ctx* ctx, const VisibleOp& op, uint32_t* tile_counts, uint64_t* n_visible, uint32_t* ghist,
+                           uint64_t* rstatus, size_t rstride) {
+  const uint64_t ntiles = (op.n + SCAN_TILE - 1) / SCAN_TILE;
+  if (ntiles == 0) return SPLX_OK;
+  const unsigned nb = (unsigned)(ntiles < 4 * SPLX_SM_COUNT ? ntiles : 4 * SPLX_SM_COUNT);
+  k_vis_count<<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, tile_counts);
+  SPLX_LAUNCH_CHECK(ctx, "k_vis_count");
+  k_vis_offsets<<<1, 1024, 0, ctx->stream>>>(tile_counts, ntiles, n_visible);
+  SPLX_LAUNCH_CHECK(ctx, "k_vis_offsets");
+  k_vis_compact<<<nb, SCAN_THREADS, 0, ctx->stream>>>(op, tile_counts, n_visible, ghist, rstatus, rstride);
+  SPLX_LAUNCH_CHECK(ctx, "k_vis_compact");
   return SPLX_OK;
 }
 
@@ -884,18 +952,17 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   vop.map.n = rt.n;
   for (int r = 0; r < rt.n; ++r) { vop.map.begin[r] = rt.begin[r]; vop.map.jprefix[r] = rt.jprefix[r]; }
   vop.map.jprefix[rt.n] = rt.jprefix[rt.n];
-  // status words per pass of the depth sort: whole scan tiles (the compaction scan clears SCAN_RS radix tiles at a time)
+  // status words per pass of the depth sort (room for every participating Gaussian being visible)
   const size_t stride_d = (((size_t)n_act + SCAN_TILE - 1) / SCAN_TILE) * SCAN_RS * 256;
-  if ((rc = scan_exclusive<VisibleOp, true>(ctx, vop, (uint64_t)n_act, nullptr, (uint64_t*)(base + L.st_scan_v), &cnt->ticket[0],
-                                            &cnt->n_visible, nullptr, 0, (uint32_t*)(base + L.ghist_d),
-                                            (uint64_t*)(base + L.st_depth), stride_d))) return rc;
+  if ((rc = compact_visible(ctx, vop, (uint32_t*)(base + L.st_scan_v), &cnt->n_visible, (uint32_t*)(base + L.ghist_d),
+                            (uint64_t*)(base + L.st_depth), stride_d))) return rc;
   // 2. stable sort by depth bits (4 passes of 8 bits: result back in the a-buffers); histograms came with step 1
   if ((rc = radix_sort<uint32_t, 256>(ctx, ckeys_a, cvals_a, ckeys_b, cvals_b, (uint64_t)n_act, &cnt->n_visible, 0, 32,
                                       (uint32_t*)(base + L.ghist_d), (uint64_t*)(base + L.st_depth), &cnt->ticket[2],
                                       stride_d))) return rc;
   // 3. offsets of every visible Gaussian's run, M, and the keys in depth order
   TouchedOp top{pr->tiles_touched, cvals_a, offs};
-  if ((rc = scan_exclusive<TouchedOp, false>(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
+  if ((rc = scan_exclusive<TouchedOp>(ctx, top, (uint64_t)n_act, &cnt->n_visible, (uint64_t*)(base + L.st_scan_t), &cnt->ticket[1],
                            &cnt->m_total, &cnt->m_sorted, out->capacity))) return rc;
   // 4. the (compact slot, depth-order position) pairs and their stable sort on the compact slot bits.  Two pair buffers:
   // A in the workspace, B in the memory of out->keys (dead until the last pass writes the 64-bit keys there, reading A).
