@@ -468,8 +468,12 @@ def run_ours(args):
             nb = len(grp)
             tg = targets[grp[0]:grp[0] + 1] if nb == 1 else targets[torch.as_tensor(grp, device="cuda")]
             e = ev[gi]
-            e[0].record(); c.project_plan(tr.params, po, plan, tr.sh_degree, tr.proj)
+            # a1 as splx_iteration runs it: the geometry half, the binning, then the colour of the visible list (e[8] between)
+            e[0].record(); c.project_geometry_plan(tr.params, po, plan, tr.proj)
             e[1].record(); tr._bin_sort(tr.proj, plan, tr.bins, tr._ws_sort)
+            e[8].record()
+            lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
+            c.project_colour_list_plan(tr.params, po, plan, tr.sh_degree, tr.proj, lst, cnt)
             e[2].record(); c.render_partial_plan(tr.proj, tr.bins, plan, tr.partials)
             e[3].record()
             if tr.lambda_dssim > 0:
@@ -496,8 +500,8 @@ def run_ours(args):
     n_staged = max(3, min(args.steps, 10))
     restore()
     for _ in range(2):
-        staged_iteration([[torch.cuda.Event() for _ in range(8)] for _ in plans])
-    evs = [[[torch.cuda.Event(enable_timing=True) for _ in range(8)] for _ in plans] for _ in range(n_staged)]
+        staged_iteration([[torch.cuda.Event() for _ in range(9)] for _ in plans])
+    evs = [[[torch.cuda.Event(enable_timing=True) for _ in range(9)] for _ in plans] for _ in range(n_staged)]
     torch.cuda.synchronize()
     for s in range(n_staged):
         staged_iteration(evs[s])
@@ -508,6 +512,9 @@ def run_ours(args):
             e = evs[s][gi]
             for i, n in enumerate(STAGES[:6]):
                 stage_ms[n] += e[i].elapsed_time(e[i + 1]) / n_staged
+            colour = e[8].elapsed_time(e[2]) / n_staged           # inside [e1, e2): belongs to the projection, not the binning
+            stage_ms["project"] += colour
+            stage_ms["bin_sort"] -= colour
         stage_ms["adam"] += evs[s][-1][6].elapsed_time(evs[s][-1][7]) / n_staged
     eager_ms = sum(evs[s][0][0].elapsed_time(evs[s][-1][7]) for s in range(n_staged)) / n_staged
 

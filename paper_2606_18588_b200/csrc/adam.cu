@@ -94,45 +94,64 @@ __device__ __forceinline__ uint4 adam_flags(const AdamGroups& gr, int j, int64_t
   return make_uint4(f0, f1, f2, f3);
 }
 
-template <bool FLAGS>
-__global__ void __launch_bounds__(AB, 6)      // 6 CTAs / SM (<= 42 registers): the bytes in flight, not the ALU, carry this kernel
-k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ m, float* __restrict__ v,
-              int64_t nvec, AdamK k, const __grid_constant__ AdamGroups gr, float gscale, int zero_grad,
-              const uint8_t* __restrict__ touched) {
-  for (int64_t i = (int64_t)blockIdx.x * AB + threadIdx.x; i < nvec; i += (int64_t)gridDim.x * AB) {
-    int j = 0;
+// U vectors per thread and trip (their loads are issued together); CS: ld.global.cs / st.global.cs (evict-first) on the
+// four streams.  Measured on 30 M Gaussians (7.1 GB per buffer; a quarter of the million-row blocks 60 % flagged), median
+// of 7 launches, bytes as bench.py counts them: FLAGS 7.95 ms = 5.49 TB/s with plain accesses and one vector per thread
+// -> 7.05 ms = 6.19 TB/s with two vectors and the streaming hints (the one-pass streams no longer evict the flag bytes
+// and each other's open DRAM pages from L2; the same hints with ONE vector per thread: 6.97-7.87 ms depending on the grid;
+// four vectors: 9.3-10.1 ms at 111 registers).  Without flags: 8.07 ms = 6.14 TB/s as it is, 7.9-8.4 ms with any
+// variant: left alone.  So: FLAGS -> U = 2, CS; plain -> U = 1, no hints.
+template <bool CS> __device__ __forceinline__ float4 ldv(const float4* p) { return CS ? __ldcs(p) : *p; }
+template <bool CS> __device__ __forceinline__ void stv(float4* p, float4 v) { if (CS) __stcs(p, v); else *p = v; }
+template <bool FLAGS, int U, bool CS>
+__global__ void __launch_bounds__(AB, U == 1 ? 6 : 4)      // the bytes in flight, not the ALU, carry this kernel
+k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __restrict__ m, float* __restrict__ v, int64_t nvec,
+              AdamK k, const __grid_constant__ AdamGroups gr, float gscale, int zero_grad, const uint8_t* __restrict__ touched) {
+  const int64_t stride = (int64_t)gridDim.x * AB;
+  for (int64_t i0 = (int64_t)blockIdx.x * AB + threadIdx.x; i0 < nvec; i0 += U * stride) {
+    float4 p[U], g[U], mm[U], vv[U];
+    int jj[U];
 #pragma unroll
-    for (int q = 1; q < SPLX_ADAM_MAX_GROUPS; ++q)
-      if (q < gr.n && i >= gr.end4[q - 1]) j = q;
-    AdamK kk = k; kk.lr = gr.lr[j];
-    float4 g = make_float4(0.f, 0.f, 0.f, 0.f), p, mm, vv;
-    if (FLAGS) {
-      // the flag bytes and the parameter / moment vectors are requested together (independent loads: one memory latency);
-      // only the gradient of a touched row waits for its flag
-      const uint4 fl = adam_flags(gr, j, i, touched);
-      p = reinterpret_cast<float4*>(param)[i];
-      mm = reinterpret_cast<float4*>(m)[i];
-      vv = reinterpret_cast<float4*>(v)[i];
-      // the decision is taken per WARP (512 contiguous bytes): whole bursts of the gradient stream are read or skipped --
-      // skipping single 16-byte vectors left DRAM with a scattered read pattern that cost more than the bytes it saved
-      if (__any_sync(__activemask(), (fl.x | fl.y | fl.z | fl.w) != 0u)) {
-        const float4 t = reinterpret_cast<const float4*>(grad)[i];
-        g = make_float4(fl.x ? t.x : 0.f, fl.y ? t.y : 0.f, fl.z ? t.z : 0.f, fl.w ? t.w : 0.f);
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = i0 + u * stride;
+      g[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      jj[u] = 0;
+      if (i >= nvec) continue;
+      int j = 0;
+#pragma unroll
+      for (int q = 1; q < SPLX_ADAM_MAX_GROUPS; ++q)
+        if (q < gr.n && i >= gr.end4[q - 1]) j = q;
+      jj[u] = j;
+      if (FLAGS) {
+        const uint4 fl = adam_flags(gr, j, i, touched);
+        p[u] = ldv<CS>(reinterpret_cast<float4*>(param) + i);
+        mm[u] = ldv<CS>(reinterpret_cast<float4*>(m) + i);
+        vv[u] = ldv<CS>(reinterpret_cast<float4*>(v) + i);
+        if (__any_sync(__activemask(), (fl.x | fl.y | fl.z | fl.w) != 0u)) {
+          const float4 t = ldv<CS>(reinterpret_cast<const float4*>(grad) + i);
+          g[u] = make_float4(fl.x ? t.x : 0.f, fl.y ? t.y : 0.f, fl.z ? t.z : 0.f, fl.w ? t.w : 0.f);
+        }
+      } else {
+        g[u] = ldv<CS>(reinterpret_cast<const float4*>(grad) + i);
+        p[u] = ldv<CS>(reinterpret_cast<float4*>(param) + i);
+        mm[u] = ldv<CS>(reinterpret_cast<float4*>(m) + i);
+        vv[u] = ldv<CS>(reinterpret_cast<float4*>(v) + i);
       }
-    } else {
-      g = reinterpret_cast<const float4*>(grad)[i];
-      p = reinterpret_cast<float4*>(param)[i];
-      mm = reinterpret_cast<float4*>(m)[i];
-      vv = reinterpret_cast<float4*>(v)[i];
     }
-    adam1(p.x, g.x * gscale, mm.x, vv.x, kk);
-    adam1(p.y, g.y * gscale, mm.y, vv.y, kk);
-    adam1(p.z, g.z * gscale, mm.z, vv.z, kk);
-    adam1(p.w, g.w * gscale, mm.w, vv.w, kk);
-    reinterpret_cast<float4*>(param)[i] = p;
-    reinterpret_cast<float4*>(m)[i] = mm;
-    reinterpret_cast<float4*>(v)[i] = vv;
-    if (!FLAGS && zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int64_t i = i0 + u * stride;
+      if (i >= nvec) continue;
+      AdamK kk = k; kk.lr = gr.lr[jj[u]];
+      adam1(p[u].x, g[u].x * gscale, mm[u].x, vv[u].x, kk);
+      adam1(p[u].y, g[u].y * gscale, mm[u].y, vv[u].y, kk);
+      adam1(p[u].z, g[u].z * gscale, mm[u].z, vv[u].z, kk);
+      adam1(p[u].w, g[u].w * gscale, mm[u].w, vv[u].w, kk);
+      stv<CS>(reinterpret_cast<float4*>(param) + i, p[u]);
+      stv<CS>(reinterpret_cast<float4*>(m) + i, mm[u]);
+      stv<CS>(reinterpret_cast<float4*>(v) + i, vv[u]);
+      if (!FLAGS && zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
   }
 }
 
@@ -238,9 +257,9 @@ int launch_adam_groups(splx_ctx* ctx, float* param, float* grad, float* m, float
   if (touched && (nvec >> 32 || rows >> 30))
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_flagged: more than 2^32 vectors or 2^30 rows");
   if (touched)
-    k_adam_groups<true><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, 0, touched);
+    k_adam_groups<true, 2, true><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, 0, touched);
   else
-    k_adam_groups<false><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, zero_grad, nullptr);
+    k_adam_groups<false, 1, false><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, nvec, k, gr, grad_scale, zero_grad, nullptr);
   SPLX_LAUNCH_CHECK(ctx, "k_adam_groups");
   return SPLX_OK;
 }
