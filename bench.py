@@ -385,8 +385,6 @@ def run_ours(args):
     torch.cuda.empty_cache()
     tr.sparse_adam = bool(args.sparse_adam)
     tr.flagged_grads = not args.plain_grads
-    tr.adam_early = args.adam_sms > 0
-    tr.adam_sms = max(args.adam_sms, 0)
     tr.lambda_dssim = float(args.lambda_dssim)
     if args.no_visibility:   # boxes that contain everything: every partition participates in every view, no tile is invisible
         big = np.float32(1e6)
@@ -691,9 +689,6 @@ def main():
     ap.add_argument("--cross-filter", action="store_true", help="cross-boundary per-ray filtering (PAPER.md L474-L476, DESIGN.md s32)")
     ap.add_argument("--plain-grads", action="store_true",
                     help="do not track the gradient rows with flags: the first bucket writes every row, Adam reads every row")
-    ap.add_argument("--adam-sms", type=int, default=0,
-                    help="> 0: a partition's optimiser step runs beside the later buckets on that many SMs as soon as its gradients "
-                         "are complete (SPLX_ITER_ADAM_EARLY); 0: one launch after the last bucket")
     ap.add_argument("--sparse-adam", action="store_true", help="visible-only Adam (an option outside the paper, DESIGN.md s31)")
     args = ap.parse_args()
     if args.impl == "reference":

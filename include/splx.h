@@ -270,19 +270,6 @@ int splx_adam_groups_flagged(splx_ctx *ctx, float *param, const float *grad, flo
                              const int64_t *group_offsets, const int32_t *widths, int64_t rows, const uint8_t *touched,
                              const float *lr, float beta1, float beta2, float eps, int step, float grad_scale);
 
-/* splx_adam_groups / splx_adam_groups_flagged restricted to n_ranges ROW ranges (row_ranges: HOST int64[2*n_ranges],
- * rows row_ranges[2i] <= r < row_ranges[2i+1] of every group; ascending, disjoint): the optimiser step of the partitions
- * whose gradients are complete, which splx_iteration can issue on its own stream while later buckets still render the
- * other partitions (a rank owns the gradients of its partition and needs no exchange to step).  touched:
- * DEVICE uint8[rows] as in splx_adam_groups_flagged, or NULL = every gradient row is read.  Elementwise identical to the
- * whole-buffer calls on the rows it covers; elements outside the ranges are neither read nor written (a 16-byte vector
- * that straddles a range border is updated element by element), so calls over disjoint ranges may run concurrently.
- * background_sms > 0: the launch shape for running BESIDE other kernels: that many CTAs, each filling one SM. */
-int splx_adam_groups_rows(splx_ctx *ctx, float *param, const float *grad, float *m, float *v, int n_groups,
-                          const int64_t *group_offsets, const int32_t *widths, int64_t rows, const uint8_t *touched,
-                          const float *lr, float beta1, float beta2, float eps, int step, float grad_scale,
-                          int n_ranges, const int64_t *row_ranges, int background_sms);
-
 /* ==== Optional subsystems (BASELINE.json north_star): visibility prediction
  * and conflict-free consolidation of B views into one launch.  Additive:
  * the single-view calls above are the same code run with a one-view plan. ==================== */
@@ -520,17 +507,10 @@ typedef struct {
 } splx_adam_cfg;
 
 #define SPLX_ITER_HOST 1   /* targets[v] / images_out[v] / loss_out / m_out are pinned HOST pointers */
-#define SPLX_ITER_ADAM_EARLY 2  /* a11 partition by partition (dense optimiser, adam->widths given): the step of partition k
-                                   (splx_adam_groups_rows) is issued on the library's optimiser stream as soon as the last
-                                   bucket that renders k has finished its backward -- at once for a partition no view of
-                                   the iteration sees -- beside the blending of the later buckets, on adam_sms SMs of its
-                                   own; only the partitions of the last bucket step after it.  Same parameters and moments
-                                   bit for bit as the single launch after the last bucket (flag clear). */
 typedef struct {
   int32_t flags;
   float sat_eps;         /* threshold of the saturation detection (bucket.tile_state_out) */
   float lambda_dssim;    /* 0: L = mean L1 (a6+a7+a8 fused); > 0: L = mean L1 + lambda * (1 - mean SSIM) */
-  int32_t adam_sms;      /* SPLX_ITER_ADAM_EARLY: SMs given to an optimiser launch that runs beside other kernels (0 = 32) */
 } splx_iter_opts;
 
 /* n_views views in n_buckets buckets; every view belongs to exactly one bucket.  targets[v]: [H,W,3] of view v

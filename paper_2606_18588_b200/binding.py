@@ -36,7 +36,7 @@ EXPORTS = [
     "splx_compose_l1_backward_plan",
     "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
     "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
-    "splx_adam_groups_flagged", "splx_adam_groups_rows", "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_dssim_loss_grad_static", "splx_iteration", "splx_microbench",
+    "splx_adam_groups_flagged", "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_dssim_loss_grad_static", "splx_iteration", "splx_microbench",
 ]
 MAX_VIEWS = 8
 DSSIM_STATIC_MAX_PIXELS = 262144
@@ -112,11 +112,10 @@ class AdamCfgS(C.Structure):
 
 
 class IterOptsS(C.Structure):
-    _fields_ = [("flags", C.c_int32), ("sat_eps", C.c_float), ("lambda_dssim", C.c_float), ("adam_sms", C.c_int32)]
+    _fields_ = [("flags", C.c_int32), ("sat_eps", C.c_float), ("lambda_dssim", C.c_float)]
 
 
 ITER_HOST = 1
-ITER_ADAM_EARLY = 2
 
 
 def lib():
@@ -188,8 +187,6 @@ def lib():
                                          C.c_size_t, C.c_int]
         L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
         L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp]
-        L.splx_adam_groups_rows.argtypes = [vp, vp, vp, vp, vp, C.c_int, vp, vp, C.c_int64, vp, vp, C.c_float, C.c_float,
-                                            C.c_float, C.c_int, C.c_float, C.c_int, vp, C.c_int]
         L.splx_adam_sparse.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float]
         L.splx_cross_sets.argtypes = [vp, vp, C.c_int, vp, vp, vp, C.c_float, vp]
         L.splx_cross_depth_ranges.argtypes = [C.c_int, vp, vp, vp, vp]
@@ -483,19 +480,6 @@ class Context:
         self._check(lib().splx_adam_groups_flagged(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, wd, int(rows),
                                                    _ptr(touched), lr, beta1, beta2, eps, step, grad_scale))
 
-    def adam_groups_rows(self, param, grad, m, v, group_offsets, widths, rows, touched, lrs, row_ranges, beta1=0.9,
-                         beta2=0.999, eps=1e-15, step=1, grad_scale=1.0, background_sms=0):
-        """splx_adam_groups_rows.  row_ranges: [(begin, end), ...] ascending and disjoint; touched: uint8 tensor or None."""
-        n = len(lrs)
-        offs = (C.c_int64 * (n + 1))(*[int(x) for x in group_offsets])
-        wd = (C.c_int32 * n)(*[int(x) for x in widths])
-        lr = (C.c_float * n)(*[float(x) for x in lrs])
-        flat = [int(x) for r in row_ranges for x in r]
-        rr = (C.c_int64 * max(len(flat), 1))(*flat)
-        self._check(lib().splx_adam_groups_rows(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, wd, int(rows),
-                                                _ptr(touched), lr, beta1, beta2, eps, step, grad_scale, len(flat) // 2, rr,
-                                                int(background_sms)))
-
     # ---- the same stages under a launch plan (visibility prediction, consolidated views) ---------
     visible_regions = staticmethod(visible_regions)     # host computations: no context needed
     schedule_views = staticmethod(schedule_views)
@@ -634,15 +618,14 @@ class Context:
                                                       float(B if scale is None else scale), _ptr(g_image), _ptr(loss_sum)))
 
     def iteration(self, trainset: "TrainsetS", buckets, n_views, targets, images_out=None, loss_out=None, m_out=None,
-                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None, adam_early=False, adam_sms=0):
+                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None):
         """splx_iteration.  buckets: ctypes array of BucketS; targets / images_out: lists of raw pointers (ints; device
         pointers, or pinned host pointers with host=True); loss_out / m_out: raw pinned host pointers or None."""
         tg = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) for x in targets])
         io = None
         if images_out is not None:
             io = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) if x else None for x in images_out])
-        opts = IterOptsS((ITER_HOST if host else 0) | (ITER_ADAM_EARLY if adam_early else 0), float(sat_eps), float(lambda_dssim),
-                         int(adam_sms))
+        opts = IterOptsS(ITER_HOST if host else 0, float(sat_eps), float(lambda_dssim))
         self._check(lib().splx_iteration(self._h, C.byref(trainset), len(buckets), buckets, int(n_views), tg, io,
                                          C.c_void_p(loss_out) if loss_out else None, C.c_void_p(m_out) if m_out else None,
                                          C.byref(opts), C.byref(adam) if adam is not None else None))

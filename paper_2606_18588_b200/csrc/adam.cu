@@ -155,107 +155,6 @@ k_adam_groups(float* __restrict__ param, float* __restrict__ grad, float* __rest
   }
 }
 
-// The same update restricted to ROW RANGES (splx_adam_groups_rows): the rows of the partitions whose gradients are
-// complete, so that splx_iteration can run the optimiser of a partition on its own stream while later buckets still
-// render other partitions (the optimiser is HBM bound and leaves the issue slots idle, the blend kernels are issue
-// bound and leave HBM idle).  A range and a group give one SEGMENT of the flat buffer: its aligned interior goes
-// through the 16-byte vector path (same arithmetic and flag handling as k_adam_groups), the <= 3 elements in front
-// of and behind the interior are updated one by one -- a vector shared by two partitions is never touched as a
-// whole, so two launches over different ranges never write the same bytes.
-constexpr int ADAM_MAX_SEGS = 80;
-constexpr size_t BG_SMEM = 200 * 1024;    // dynamic shared memory a BACKGROUND CTA asks for: nothing else fits beside it on its SM
-struct AdamSegs {
-  int n;
-  uint32_t vprefix[ADAM_MAX_SEGS + 1];   // running count of interior vectors
-  uint32_t vbegin[ADAM_MAX_SEGS];        // first interior vector (index into the flat buffer / 4)
-  long long e0[ADAM_MAX_SEGS], e1[ADAM_MAX_SEGS];   // element range of the segment
-  unsigned char group[ADAM_MAX_SEGS];
-};
-
-// THREADS = 256: a launch that has the GPU to itself (the shape of k_adam_groups).  THREADS = 1024 with BG_SMEM bytes of
-// dynamic shared memory: a launch that runs BESIDE the blend kernels on a few SMs of its own -- one such CTA fills an SM
-// (thread slots and shared memory), so the kernels it overlaps keep the other SMs undisturbed and only HBM is shared.
-template <bool FLAGS, int THREADS>
-__global__ void __launch_bounds__(THREADS, THREADS == 1024 ? 1 : 4)
-k_adam_rows(float* __restrict__ param, const float* __restrict__ grad, float* __restrict__ m, float* __restrict__ v, AdamK k,
-            const __grid_constant__ AdamGroups gr, const __grid_constant__ AdamSegs sg, float gscale,
-            const uint8_t* __restrict__ touched) {
-  constexpr int U = 2;
-  const uint64_t total = sg.vprefix[sg.n];
-  const uint64_t stride = (uint64_t)gridDim.x * THREADS;
-  for (uint64_t t0 = (uint64_t)blockIdx.x * THREADS + threadIdx.x; t0 < total; t0 += U * stride) {
-    float4 p[U], g[U], mm[U], vv[U];
-    int64_t idx[U];
-    int jj[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const uint64_t t = t0 + (uint64_t)u * stride;
-      idx[u] = -1; jj[u] = 0;
-      g[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (t >= total) continue;
-      int lo = 0, hi = sg.n;               // segment lo: vprefix[lo] <= t < vprefix[lo + 1]
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (t >= sg.vprefix[mid]) lo = mid; else hi = mid;
-      }
-      const int j = sg.group[lo];
-      const int64_t i = (int64_t)sg.vbegin[lo] + (int64_t)(t - sg.vprefix[lo]);
-      idx[u] = i; jj[u] = j;
-      if (FLAGS) {
-        const uint4 fl = adam_flags(gr, j, i, touched);
-        p[u] = __ldcs(reinterpret_cast<const float4*>(param) + i);
-        mm[u] = __ldcs(reinterpret_cast<const float4*>(m) + i);
-        vv[u] = __ldcs(reinterpret_cast<const float4*>(v) + i);
-        if (__any_sync(__activemask(), (fl.x | fl.y | fl.z | fl.w) != 0u)) {
-          const float4 q = __ldcs(reinterpret_cast<const float4*>(grad) + i);
-          g[u] = make_float4(fl.x ? q.x : 0.f, fl.y ? q.y : 0.f, fl.z ? q.z : 0.f, fl.w ? q.w : 0.f);
-        }
-      } else {
-        g[u] = __ldcs(reinterpret_cast<const float4*>(grad) + i);
-        p[u] = __ldcs(reinterpret_cast<const float4*>(param) + i);
-        mm[u] = __ldcs(reinterpret_cast<const float4*>(m) + i);
-        vv[u] = __ldcs(reinterpret_cast<const float4*>(v) + i);
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      if (idx[u] < 0) continue;
-      AdamK kk = k; kk.lr = gr.lr[jj[u]];
-      adam1(p[u].x, g[u].x * gscale, mm[u].x, vv[u].x, kk);
-      adam1(p[u].y, g[u].y * gscale, mm[u].y, vv[u].y, kk);
-      adam1(p[u].z, g[u].z * gscale, mm[u].z, vv[u].z, kk);
-      adam1(p[u].w, g[u].w * gscale, mm[u].w, vv[u].w, kk);
-      __stcs(reinterpret_cast<float4*>(param) + idx[u], p[u]);
-      __stcs(reinterpret_cast<float4*>(m) + idx[u], mm[u]);
-      __stcs(reinterpret_cast<float4*>(v) + idx[u], vv[u]);
-    }
-  }
-  // the elements around the aligned interiors: <= 3 in front, <= 3 behind, per segment
-  if (blockIdx.x == 0) {
-    for (int q = threadIdx.x; q < 6 * sg.n; q += THREADS) {
-      const int s = q / 6, w = q - 6 * s;
-      const long long e0 = sg.e0[s], e1 = sg.e1[s];
-      const long long vb4 = 4ll * sg.vbegin[s], ve4 = vb4 + 4ll * (sg.vprefix[s + 1] - sg.vprefix[s]);
-      const long long head_end = e1 < vb4 ? e1 : vb4;                       // head = [e0, head_end)
-      const long long tail_begin = ve4 > head_end ? ve4 : head_end;         // tail = [tail_begin, e1)
-      const long long e = w < 3 ? e0 + w : tail_begin + (w - 3);
-      if (w < 3 ? e >= head_end : e >= e1) continue;
-      const int j = sg.group[s];
-      float gv;
-      if (FLAGS) {
-        const long long row = (e - 4ll * gr.start4[j]) / gr.width[j];
-        gv = (row < gr.rows && touched[row]) ? grad[e] : 0.f;
-      } else {
-        gv = grad[e];
-      }
-      AdamK kk = k; kk.lr = gr.lr[j];
-      float pp = param[e], ms = m[e], vs = v[e];
-      adam1(pp, gv * gscale, ms, vs, kk);
-      param[e] = pp; m[e] = ms; v[e] = vs;
-    }
-  }
-}
-
 // Visible-only ("sparse") Adam, an OPTION outside the paper: only Gaussians whose flag is set
 // -- they received a gradient in this iteration -- take the step, the others keep parameters AND moments untouched
 // (no decay); the flags are cleared on the way.  A block owns 128 consecutive Gaussians: it reads their 128 flag
@@ -379,71 +278,5 @@ int launch_adam(splx_ctx* ctx, float* param, float* grad, float* m, float* v, in
                 (float)(1.0 / bc1), (float)(1.0 / bc2)};
   k_adam<<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, count, k, grad_scale, zero_grad);
   SPLX_LAUNCH_CHECK(ctx, "k_adam");
-  return SPLX_OK;
-}
-
-int launch_adam_rows(splx_ctx* ctx, float* param, const float* grad, float* m, float* v, int n_groups,
-                     const int64_t* group_offsets, const int32_t* widths, int64_t rows, const uint8_t* touched,
-                     const float* lr, float beta1, float beta2, float eps, int step, float grad_scale, int n_ranges,
-                     const int64_t* row_ranges, int background_sms) {
-  const int64_t count = group_offsets[n_groups];
-  if (count <= 0 || n_ranges <= 0) return SPLX_OK;
-  if ((count >> 2) >> 32 || rows >> 30)
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: more than 2^32 vectors or 2^30 rows");
-  const double bc1 = 1.0 - pow((double)beta1, step), bc2 = 1.0 - pow((double)beta2, step);
-  const AdamK k{0.f, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps,
-                (float)(1.0 / bc1), (float)(1.0 / bc2)};
-  AdamGroups gr;
-  memset(&gr, 0, sizeof gr);
-  gr.n = n_groups;
-  gr.rows = rows;
-  for (int j = 0; j < SPLX_ADAM_MAX_GROUPS; ++j) {
-    gr.end4[j] = j < n_groups ? group_offsets[j + 1] >> 2 : count >> 2;
-    gr.lr[j] = j < n_groups ? lr[j] : 0.f;
-    gr.start4[j] = (uint32_t)((j < n_groups ? group_offsets[j] : count) >> 2);
-    gr.width[j] = j < n_groups ? widths[j] : 1;
-  }
-  const bool bg = background_sms > 0;
-  if (bg) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      SPLX_CUDA_OK(ctx, cudaFuncSetAttribute(k_adam_rows<true, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BG_SMEM));
-      SPLX_CUDA_OK(ctx, cudaFuncSetAttribute(k_adam_rows<false, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BG_SMEM));
-      attr_set = true;
-    }
-  }
-  const int per_launch = ADAM_MAX_SEGS / n_groups;       // ranges per launch
-  for (int r0 = 0; r0 < n_ranges; r0 += per_launch) {
-    AdamSegs sg;
-    memset(&sg, 0, sizeof sg);
-    const int r1 = r0 + per_launch < n_ranges ? r0 + per_launch : n_ranges;
-    for (int r = r0; r < r1; ++r) {
-      const int64_t a = row_ranges[2 * r], b = row_ranges[2 * r + 1];
-      if (b <= a) continue;
-      for (int j = 0; j < n_groups; ++j) {
-        const int s = sg.n++;
-        const long long e0 = group_offsets[j] + a * widths[j], e1 = group_offsets[j] + b * widths[j];
-        const long long vb = (e0 + 3) >> 2, ve = e1 >> 2;
-        sg.e0[s] = e0; sg.e1[s] = e1; sg.group[s] = (unsigned char)j;
-        sg.vbegin[s] = (uint32_t)vb;
-        sg.vprefix[s + 1] = sg.vprefix[s] + (uint32_t)(ve > vb ? ve - vb : 0);
-      }
-    }
-    if (!sg.n) continue;
-    const int64_t nvec = sg.vprefix[sg.n];
-    const int threads = bg ? 1024 : AB;
-    int64_t blocks = (nvec + 2ll * threads - 1) / (2ll * threads);
-    const int64_t cap = bg ? background_sms : (int64_t)SPLX_SM_COUNT * 8;
-    if (blocks > cap) blocks = cap;
-    if (blocks < 1) blocks = 1;
-    if (bg) {
-      if (touched) k_adam_rows<true, 1024><<<(unsigned)blocks, 1024, BG_SMEM, ctx->stream>>>(param, grad, m, v, k, gr, sg, grad_scale, touched);
-      else k_adam_rows<false, 1024><<<(unsigned)blocks, 1024, BG_SMEM, ctx->stream>>>(param, grad, m, v, k, gr, sg, grad_scale, touched);
-    } else {
-      if (touched) k_adam_rows<true, AB><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, k, gr, sg, grad_scale, touched);
-      else k_adam_rows<false, AB><<<(unsigned)blocks, AB, 0, ctx->stream>>>(param, grad, m, v, k, gr, sg, grad_scale, touched);
-    }
-    SPLX_LAUNCH_CHECK(ctx, "k_adam_rows");
-  }
   return SPLX_OK;
 }

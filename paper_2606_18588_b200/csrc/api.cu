@@ -534,29 +534,4 @@ int splx_adam_groups_flagged(splx_ctx* ctx, float* param, const float* grad, flo
                             grad_scale, 0, widths, rows, touched);
 }
 
-int splx_adam_groups_rows(splx_ctx* ctx, float* param, const float* grad, float* m, float* v, int n_groups,
-                          const int64_t* group_offsets, const int32_t* widths, int64_t rows, const uint8_t* touched,
-                          const float* lr, float beta1, float beta2, float eps, int step, float grad_scale, int n_ranges,
-                          const int64_t* row_ranges, int background_sms) {
-  if (!ctx) return SPLX_ERR_INVALID_ARG;
-  if (!param || !grad || !m || !v || !group_offsets || !widths || !lr || step < 1 || rows < 0 || n_ranges < 0 ||
-      (n_ranges && !row_ranges) || background_sms < 0 || !aligned16(param) || !aligned16(grad) || !aligned16(m) || !aligned16(v))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: null/misaligned argument or step < 1");
-  if (n_groups < 1 || n_groups > SPLX_ADAM_MAX_GROUPS)
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: n_groups=%d not in [1,%d]", n_groups, SPLX_ADAM_MAX_GROUPS);
-  if (group_offsets[0] != 0) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: group_offsets[0] must be 0");
-  for (int j = 0; j < n_groups; ++j) {
-    if (group_offsets[j + 1] < group_offsets[j] || (group_offsets[j + 1] & 3))
-      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: offsets must be monotone multiples of 4");
-    if (widths[j] < 1 || group_offsets[j + 1] - group_offsets[j] < rows * widths[j])
-      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: group %d does not hold rows x width floats", j);
-  }
-  for (int r = 0; r < n_ranges; ++r)
-    if (row_ranges[2 * r] < 0 || row_ranges[2 * r + 1] > rows || row_ranges[2 * r] > row_ranges[2 * r + 1] ||
-        (r && row_ranges[2 * r] < row_ranges[2 * r - 1]))
-      SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_adam_groups_rows: range %d outside [0, rows], reversed or not ascending", r);
-  return launch_adam_rows(ctx, param, grad, m, v, n_groups, group_offsets, widths, rows, touched, lr, beta1, beta2, eps, step,
-                          grad_scale, n_ranges, row_ranges, background_sms);
-}
-
 }  // extern "C"

@@ -20,8 +20,7 @@ struct splx_ctx {
   // splx_iteration's own streams and events, created at its first call (iteration.cu), destroyed by splx_destroy
   bool iter_ready;
   cudaStream_t s_front, s_up, s_down;     // a1-a4 of the next bucket; host -> device targets; device -> host results
-  cudaStream_t s_adam;                    // a11 of the partitions whose gradients are complete, beside later buckets
-  cudaEvent_t ev_start, ev_up, ev_front[2], ev_back[2], ev_img, ev_down, ev_grads, ev_adam;
+  cudaEvent_t ev_start, ev_up, ev_front[2], ev_back[2], ev_img, ev_down;
 };
 void iteration_release(splx_ctx*);
 
@@ -221,9 +220,5 @@ int launch_adam_groups(splx_ctx*, float* param, float* grad, float* m, float* v,
                        const int64_t* group_offsets, const float* lr, float beta1, float beta2, float eps, int step,
                        float grad_scale, int zero_grad, const int32_t* widths = nullptr, int64_t rows = 0,
                        const uint8_t* touched = nullptr);
-int launch_adam_rows(splx_ctx*, float* param, const float* grad, float* m, float* v, int n_groups,
-                     const int64_t* group_offsets, const int32_t* widths, int64_t rows, const uint8_t* touched,
-                     const float* lr, float beta1, float beta2, float eps, int step, float grad_scale, int n_ranges,
-                     const int64_t* row_ranges, int background_sms);
 int launch_adam(splx_ctx*, float* param, float* grad, float* m, float* v, int64_t count, float lr,
                 float beta1, float beta2, float eps, int step, float grad_scale, int zero_grad);

@@ -15,14 +15,8 @@ static int iteration_streams(splx_ctx* ctx) {
   SPLX_CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->s_front, cudaStreamNonBlocking));
   SPLX_CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->s_up, cudaStreamNonBlocking));
   SPLX_CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->s_down, cudaStreamNonBlocking));
-  {   // the optimiser stream has the HIGHEST priority: its few one-per-SM CTAs are placed as soon as SMs drain, the blend
-      // kernels of the lower-priority streams then fill the rest
-    int least = 0, greatest = 0;
-    SPLX_CUDA_OK(ctx, cudaDeviceGetStreamPriorityRange(&least, &greatest));
-    SPLX_CUDA_OK(ctx, cudaStreamCreateWithPriority(&ctx->s_adam, cudaStreamNonBlocking, greatest));
-  }
   cudaEvent_t* evs[] = {&ctx->ev_start, &ctx->ev_up, &ctx->ev_front[0], &ctx->ev_front[1], &ctx->ev_back[0],
-                        &ctx->ev_back[1], &ctx->ev_img, &ctx->ev_down, &ctx->ev_grads, &ctx->ev_adam};
+                        &ctx->ev_back[1], &ctx->ev_img, &ctx->ev_down};
   for (cudaEvent_t* e : evs) SPLX_CUDA_OK(ctx, cudaEventCreateWithFlags(e, cudaEventDisableTiming));
   ctx->iter_ready = true;
   return SPLX_OK;
@@ -30,9 +24,9 @@ static int iteration_streams(splx_ctx* ctx) {
 
 void iteration_release(splx_ctx* ctx) {
   if (!ctx->iter_ready) return;
-  cudaStreamDestroy(ctx->s_front); cudaStreamDestroy(ctx->s_up); cudaStreamDestroy(ctx->s_down); cudaStreamDestroy(ctx->s_adam);
+  cudaStreamDestroy(ctx->s_front); cudaStreamDestroy(ctx->s_up); cudaStreamDestroy(ctx->s_down);
   cudaEvent_t evs[] = {ctx->ev_start, ctx->ev_up, ctx->ev_front[0], ctx->ev_front[1], ctx->ev_back[0], ctx->ev_back[1],
-                       ctx->ev_img, ctx->ev_down, ctx->ev_grads, ctx->ev_adam};
+                       ctx->ev_img, ctx->ev_down};
   for (cudaEvent_t e : evs) cudaEventDestroy(e);
   ctx->iter_ready = false;
 }
@@ -77,7 +71,7 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (!ts || !buckets || !targets || !opts || n_buckets < 1 || n_views < 1)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: null argument or empty iteration");
-  if (opts->flags & ~(SPLX_ITER_HOST | SPLX_ITER_ADAM_EARLY) || opts->adam_sms < 0 || opts->adam_sms > SPLX_SM_COUNT) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: unknown flags %d", opts->flags);
+  if (opts->flags & ~SPLX_ITER_HOST) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: unknown flags %d", opts->flags);
   const bool host = (opts->flags & SPLX_ITER_HOST) != 0;
   if (!host && (images_out || loss_out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: images_out / loss_out need SPLX_ITER_HOST");
   const int64_t n = ts->params.n;
@@ -206,52 +200,10 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
                                       SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE, &ts->grads);
   };
 
-  // SPLX_ITER_ADAM_EARLY: a11 partition by partition (splx_adam_groups_rows).  Partition k steps once the last bucket
-  // that renders it has finished its backward -- nothing reads its parameters or writes its gradients after that (a
-  // launch under a plan never touches a non-participant).  last_bucket[k] = -1: no view of the iteration sees k; with
-  // flag-tracked gradients its rows count as zero and it steps from the start, without them bucket 0 writes their zeros first.
-  const bool adam_early = adam && (opts->flags & SPLX_ITER_ADAM_EARLY) && !(ts->touched && adam->sparse) && adam->widths &&
-                          adam->n_groups >= 1 && adam->n_groups <= SPLX_ADAM_MAX_GROUPS;
-  const int adam_sms = opts->adam_sms > 0 ? opts->adam_sms : 32;
-  int last_bucket[SPLX_MAX_K];
-  bool adam_side = false;
-  if (adam_early) {
-    for (int k = 0; k < K; ++k) {
-      last_bucket[k] = ts->touched ? -1 : 0;
-      for (int gi = 0; gi < n_buckets; ++gi)
-        if (buckets[gi].plan.view_of_part[k] >= 0) last_bucket[k] = gi;
-    }
-  }
-  // the optimiser step of the partitions with last_bucket == gi: on the optimiser stream behind `after` (an event of
-  // the context's stream), or -- the last bucket's -- on the context's stream itself with the whole GPU
-  auto adam_step = [&](int gi, cudaEvent_t after) -> int {
-    int64_t ranges[2 * SPLX_MAX_K];
-    int nr = 0;
-    for (int k = 0; k < K; ++k) {
-      if (last_bucket[k] != gi || ts->part_offsets[k + 1] <= ts->part_offsets[k]) continue;
-      if (nr && ranges[2 * nr - 1] == ts->part_offsets[k]) ranges[2 * nr - 1] = ts->part_offsets[k + 1];
-      else { ranges[2 * nr] = ts->part_offsets[k]; ranges[2 * nr + 1] = ts->part_offsets[k + 1]; ++nr; }
-    }
-    if (!nr) return SPLX_OK;
-    const bool side = gi < n_buckets - 1;
-    if (side) { SPLX_CUDA_OK(ctx, cudaStreamWaitEvent(ctx->s_adam, after, 0)); adam_side = true; }
-    StreamScope scope(ctx, side ? ctx->s_adam : main);
-    return splx_adam_groups_rows(ctx, adam->param, adam->grad, adam->m, adam->v, adam->n_groups, adam->group_offsets, adam->widths,
-                                 n, ts->touched, adam->lr, adam->beta1, adam->beta2, adam->eps, adam->step,
-                                 1.0f / (float)n_views, nr, ranges, side ? adam_sms : 0);
-  };
-  auto adam_after = [&](int gi) -> int {   // after the backward of bucket gi on the context's stream
-    if (!adam_early) return SPLX_OK;
-    if (gi < n_buckets - 1) SPLX_CUDA_OK(ctx, cudaEventRecord(ctx->ev_grads, main));
-    return adam_step(gi, ctx->ev_grads);
-  };
-  if (adam_early && (rc = adam_step(-1, ctx->ev_start))) return rc;
-
   if (!pipelined) {
     for (int gi = 0; gi < n_buckets; ++gi) {
       if ((rc = front(gi, 0, main))) return rc;
       if ((rc = back(gi, 0))) return rc;
-      if ((rc = adam_after(gi))) return rc;
     }
   } else {
     SPLX_CUDA_OK(ctx, cudaStreamWaitEvent(ctx->s_front, ctx->ev_start, 0));     // the parameters of the previous optimiser step
@@ -267,16 +219,10 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
       SPLX_CUDA_OK(ctx, cudaStreamWaitEvent(main, ctx->ev_front[gi % 2], 0));
       if ((rc = back(gi, gi % 2))) return rc;
       SPLX_CUDA_OK(ctx, cudaEventRecord(ctx->ev_back[gi % 2], main));
-      if ((rc = adam_after(gi))) return rc;
     }
   }
 
-  if (adam_early) {
-    if (adam_side) {
-      SPLX_CUDA_OK(ctx, cudaEventRecord(ctx->ev_adam, ctx->s_adam));
-      SPLX_CUDA_OK(ctx, cudaStreamWaitEvent(main, ctx->ev_adam, 0));
-    }
-  } else if (adam) {
+  if (adam) {
     const float gs = 1.0f / (float)n_views;
     if (ts->touched && adam->sparse) {
       if ((rc = splx_adam_sparse(ctx, &ts->params, &ts->grads, &adam->m_soa, &adam->v_soa, ts->touched, adam->lr, adam->beta1,

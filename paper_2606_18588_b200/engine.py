@@ -83,10 +83,6 @@ class Trainer:
         self.flagged_grads = True
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
         self.pipeline_buckets = True
-        #: SPLX_ITER_ADAM_EARLY: the optimiser step of a partition is issued beside the blending of later buckets, on
-        #: `adam_sms` SMs of its own, as soon as its gradients are complete (same parameters bit for bit)
-        self.adam_early = False
-        self.adam_sms = 32
         self._touched = None
         self._cam = None
         self._aabb = None           # (lo, hi, max_scale or None): boxes of the geometric visibility prediction
@@ -410,8 +406,7 @@ class Trainer:
             cfg = self._adam_cfg(self.step_count)
         self._plan = plans[-1][0]
         self.ctx.iteration(ts, bk, n_views, targets, images_out, loss_out, self._m_host.data_ptr(), host=host,
-                           sat_eps=0.0 if sat_eps is None else sat_eps, lambda_dssim=self.lambda_dssim, adam=cfg,
-                           adam_early=self.adam_early, adam_sms=self.adam_sms)
+                           sat_eps=0.0 if sat_eps is None else sat_eps, lambda_dssim=self.lambda_dssim, adam=cfg)
         self._m_buckets = len(plans)
         return ts, bk
 

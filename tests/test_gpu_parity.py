@@ -339,50 +339,3 @@ def test_a11_adam_groups_equals_per_group_calls(run):
                         beta2=float(np.float32(0.999)), eps=float(np.float32(1e-15)), step=step)
             P[s], Mo[s], Vo[s] = Ps, Ms, Vs
     assert np.abs(G.np32(a[0]) - P).max() <= 1e-5
-
-
-@pytest.mark.parametrize("flagged", [False, True])
-def test_a11_adam_rows_equals_the_whole_buffer_call(run, flagged):
-    """splx_adam_groups_rows (the optimiser step of some partitions, the form splx_iteration can issue beside later
-    buckets): equal to splx_adam_groups / splx_adam_groups_flagged on the rows it covers, not a byte changed outside them
-    -- with range borders that fall inside 16-byte vectors of the width-3 and width-1 groups, a range shorter than a
-    vector, an empty range, both launch shapes, and the union of two disjoint calls == the whole-buffer call."""
-    tr = run.tr
-    rng = np.random.default_rng(13)
-    rows = 10_007
-    widths = [3, 3, 4, 1, 48]
-    offs = [0]
-    for w in widths:
-        offs.append(offs[-1] + (rows * w + 3) // 4 * 4)
-    lrs = [1e-3, 7e-2, 3e-4, 5e-3, 2e-3]
-    n = offs[-1]
-    p0 = rng.standard_normal(n).astype(np.float32)
-    g0 = rng.standard_normal(n).astype(np.float32)
-    touched = torch.from_numpy((rng.random(rows) < 0.3).astype(np.uint8)).cuda() if flagged else None
-    if flagged:   # whatever the untouched rows hold must never be read
-        for j, w in enumerate(widths):
-            g0[offs[j]:offs[j] + rows * w].reshape(rows, w)[~touched.cpu().numpy().astype(bool)] = np.nan
-    mk = lambda: [torch.from_numpy(x.copy()).cuda() for x in (p0, g0, 0.1 * np.abs(p0), 0.01 * p0 * p0)]
-    whole, parts, some = mk(), mk(), mk()
-    first = [(0, 1), (1, 3), (5, 5), (1001, 4003), (4003, 4004), (7777, 9001)]
-    rest = [(3, 1001), (4004, 7777), (9001, rows)]
-    for step in (1, 2):
-        if flagged:
-            tr.ctx.adam_groups_flagged(*whole, offs, widths, rows, touched, lrs, step=step, grad_scale=0.25)
-        else:
-            tr.ctx.adam_groups(*whole, offs, lrs, step=step, grad_scale=0.25)
-        tr.ctx.adam_groups_rows(*parts, offs, widths, rows, touched, lrs, first, step=step, grad_scale=0.25, background_sms=3)
-        tr.ctx.adam_groups_rows(*parts, offs, widths, rows, touched, lrs, rest, step=step, grad_scale=0.25)
-        tr.ctx.adam_groups_rows(*some, offs, widths, rows, touched, lrs, first, step=step, grad_scale=0.25)
-    ins, real = np.zeros(n, bool), np.zeros(n, bool)      # elements of the ranges of `first`; elements of any row
-    for j, w in enumerate(widths):
-        real[offs[j]: offs[j] + rows * w] = True          # (the whole-buffer call also steps the padding between the groups)
-        for a, b in first:
-            ins[offs[j] + a * w: offs[j] + b * w] = True
-    start = mk()
-    for t in (0, 2, 3):
-        x, y, z, x0 = G.np32(whole[t]), G.np32(parts[t]), G.np32(some[t]), G.np32(start[t])
-        assert np.array_equal(x[real], y[real]), t                                         # two disjoint calls == one
-        assert np.array_equal(y[~real], x0[~real]), t
-        assert np.array_equal(z[ins], x[ins]), t                                           # covered rows: the same step
-        assert np.array_equal(z[~ins], x0[~ins]), t                                        # the rest: untouched

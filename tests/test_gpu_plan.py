@@ -458,32 +458,6 @@ def test_pipelined_buckets_equal_the_sequential_iteration(city):
         assert (out[0][2][k] != out[1][2][k]).float().mean().item() < 1e-3, k     # a slot within rounding of eps may flip
 
 
-def test_early_optimiser_steps_equal_the_single_launch(blocks, city):
-    """SPLX_ITER_ADAM_EARLY: a11 of a partition beside the later buckets as soon as its gradients are complete
-    (splx_adam_groups_rows on the optimiser stream) == one launch after the last bucket: same parameters and moments, with
-    and without flag-tracked gradient rows (the equality of the step itself is test_a11_adam_rows_equals_the_whole_buffer_call;
-    two RUNS of an iteration differ by the order of the fp32 atomics of the gradient sums)."""
-    for sc in (blocks, city):
-        ids = list(range(len(sc.cameras)))
-        targets = torch.from_numpy(np.stack(sc.targets)).cuda()
-        for flags in (True, False):
-            out = []
-            for early in (False, True):
-                tr = _trainer_conservative(sc)
-                tr.adam_early, tr.adam_sms = early, 8
-                tr._use_flags = lambda plan, f=flags: f
-                for _ in range(3):
-                    n_b = tr.iteration_views(ids, sc.cameras, targets, saturation=False)
-                torch.cuda.synchronize()
-                out.append({k: tr.flat[k].clone() for k in ("param", "m", "v")})
-            if sc is blocks:
-                assert n_b > 1
-            for k in out[0]:
-                a, b = out[0][k], out[1][k]
-                close = (a - b).abs() <= 1e-3 * b.abs() + 2e-6
-                assert close.float().mean().item() > 0.999, k
-
-
 def test_iteration_views_gradients_against_the_oracle(blocks):
     """A whole multi-bucket iteration (two consolidated two-view buckets + two single views; first bucket '=', later
     buckets '+=' over the visible list with per-row cameras; pipelined over two streams): the accumulated gradient
