@@ -301,6 +301,15 @@ typedef struct {
                                   Gaussian that small can reach the image (the cut of splx_visible_regions, reading s21) and
                                   reads its scale and rotation only if it passes: 12 instead of 40 bytes for most culled
                                   Gaussians.  Exact as long as the bound holds (a caller that trains refreshes it). */
+  int32_t open_slots;          /* 0, or an upper bound of the number of slots (k, t) with partition k participating and
+                                  tile_state[k*tiles+t] lacking SPLX_TILE_INVISIBLE, given by a caller who VOUCHES that an
+                                  INVISIBLE slot holds no intersection (the conservative regions of splx_visible_regions with
+                                  max_scale).  splx_bin_sort* then sorts on a renumbering of the open slots -- a city view
+                                  leaves 85-90 % of the slots invisible, and 16 bits instead of 17-18 are two radix passes
+                                  over the intersections instead of three -- with the same keys, vals and ranges.  Should a
+                                  key fall into an INVISIBLE slot all the same (or into an open slot beyond the bound), it is
+                                  carried behind every list under slot number K*tiles + 1, gets no range, and is counted in
+                                  num_intersections[1]. */
 } splx_plan;
 
 /* Geometric visibility (L212, L227): HOST computation, no device work, ctx not needed.  n_boxes axis-aligned boxes

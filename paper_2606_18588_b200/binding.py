@@ -84,7 +84,7 @@ class PartialS(C.Structure):
 
 class PlanS(C.Structure):
     _fields_ = [("n_views", C.c_int32), ("cams", C.c_void_p), ("view_of_part", C.c_void_p),
-                ("tile_state", C.c_void_p), ("flags", C.c_int32), ("max_scale", C.c_void_p)]
+                ("tile_state", C.c_void_p), ("flags", C.c_int32), ("max_scale", C.c_void_p), ("open_slots", C.c_int32)]
 
 
 class FrontsetS(C.Structure):
@@ -218,7 +218,7 @@ class Plan:
     """splx_plan: B views of one size, the view each partition renders (-1 = not a participant), the
     optional device tile-state bytes [K*tiles] and the flags.  Keeps the ctypes storage alive."""
 
-    def __init__(self, cams, view_of_part, tile_state=None, sparse=False, max_scale=None):
+    def __init__(self, cams, view_of_part, tile_state=None, sparse=False, max_scale=None, open_slots=0):
         self.cams = list(cams)
         self.view_of_part = [int(v) for v in view_of_part]
         self.tile_state = tile_state
@@ -227,7 +227,9 @@ class Plan:
         self._vop = (C.c_int32 * len(self.view_of_part))(*self.view_of_part)
         self._ms = None if max_scale is None else (C.c_float * len(self.view_of_part))(*[float(x) for x in max_scale])
         self._s = PlanS(len(self.cams), C.cast(self._cams, C.c_void_p), C.cast(self._vop, C.c_void_p),
-                        _ptr(tile_state), self.flags, C.cast(self._ms, C.c_void_p) if self._ms is not None else None)
+                        _ptr(tile_state), self.flags, C.cast(self._ms, C.c_void_p) if self._ms is not None else None,
+                        int(open_slots))
+        self.open_slots = int(open_slots)
 
     @property
     def K(self):

@@ -58,6 +58,9 @@ int make_plan_dev(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, 
   out->ntiles = out->TX * out->TY;
   out->flags = plan->flags;
   out->tile_state = plan->tile_state;
+  if (plan->open_slots < 0 || (plan->open_slots > 0 && !plan->tile_state))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: open_slots < 0, or > 0 without tile_state", who);
+  out->open_slots = (uint32_t)plan->open_slots;
   return SPLX_OK;
 }
 
@@ -74,7 +77,7 @@ struct SinglePlan {
   explicit SinglePlan(const splx_camera* cam) {
     for (int k = 0; k < SPLX_MAX_K; ++k) views[k] = 0;
     plan.n_views = 1; plan.cams = cam; plan.view_of_part = views; plan.tile_state = nullptr; plan.flags = 0;
-    plan.max_scale = nullptr;
+    plan.max_scale = nullptr; plan.open_slots = 0;
   }
 };
 

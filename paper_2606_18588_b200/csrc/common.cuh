@@ -72,6 +72,7 @@ struct PlanDev {
   PartView pv;
   CamDev cam[SPLX_MAX_VIEWS];
   float max_scale[SPLX_MAX_K];   // splx_plan.max_scale, or < 0: no reach test
+  uint32_t open_slots;           // splx_plan.open_slots
 };
 
 // Per-view buffers of the composition kernels (view b of the launch -> its own pointers), so that the views of a

@@ -374,6 +374,7 @@ struct FinalOut {
   const uint32_t* ckeys; const uint32_t* cvals; // depth bits / Gaussian index of the j-th visible Gaussian in depth order
   uint32_t ntiles;
   uint32_t skip[SPLX_MAX_K + 1];                // true slot = compact slot + skip[compact slot / ntiles]
+  const uint32_t* inv;                          // or (renumbered open slots, k_slot_map): true slot = inv[sort slot]
 };
 
 // One tile of a radix pass (RS_TILE keys of one CTA): stable ranks by warp multisplit, the tile's keys reordered in
@@ -471,7 +472,7 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
       const uint32_t pos = dbase[d] + j;
       if (FINAL) {
         const uint32_t cs = (uint32_t)k, jj = sval[j];
-        const uint32_t slot = cs + fin.skip[cs / fin.ntiles];
+        const uint32_t slot = fin.inv ? __ldg(fin.inv + cs) : cs + fin.skip[cs / fin.ntiles];
         fin.keys[pos] = ((uint64_t)slot << 32) | __ldg(fin.ckeys + jj);
         fin.vals[pos] = __ldg(fin.cvals + jj);
       } else {
@@ -574,6 +575,7 @@ __device__ __forceinline__ bool emit_by_output(const Counters* cnt) { return cnt
 struct CrossEmit {
   const uint64_t* mask;          // nullptr = no filtering
   const uint8_t* tile_state;
+  const uint32_t* cmap;          // nullptr, or the renumbering of the OPEN slots (k_slot_map): sort slot = cmap[true slot]
   uint32_t ntiles, nslots;
   float zlo[SPLX_MAX_K], zhi[SPLX_MAX_K];
   signed char view[SPLX_MAX_K];
@@ -640,7 +642,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       const int mid = (lo + hi + 1) >> 1;
       if (parts.off[mid] <= (int64_t)i) lo = mid; else hi = mid - 1;
     }
-    slot0 = (uint32_t)parts.rank[lo] * (uint32_t)(TX * TY);      // compact slot (see PartOffs)
+    slot0 = (uint32_t)(cx.cmap ? lo : (int)parts.rank[lo]) * (uint32_t)(TX * TY);      // compact slot (see PartOffs), or the true one
     if (FILTER) F = cross_filter(cx, i, lo, __uint_as_float(ckeys[j]));
   }
   // The 32 runs of a warp are adjacent in the output (offs is the running sum of tiles_touched in this very
@@ -674,6 +676,7 @@ k_emit_keys(const float* __restrict__ means2d, const int32_t* __restrict__ radiu
       const uint32_t ty = t / (uint32_t)sw;
       const uint32_t tile = (uint32_t)((sy0 + (int)ty) * TX + sx0 + (int)(t - ty * (uint32_t)sw));
       uint32_t slot = ss + tile;
+      if (cx.cmap) slot = __ldg(cx.cmap + slot);
       if (FILTER && sF && cross_removed(cx, sF, tile)) slot = cx.nslots;
       skeys[pos] = slot;
       spay[pos] = sj;
@@ -748,7 +751,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
           if (parts.off[mid] <= (int64_t)i) plo = mid; else phi = mid - 1;
         }
         s_off[q] = o; s_xy[q] = ((uint32_t)y0 << 16) | (uint32_t)x0; s_w[q] = (uint32_t)(x1 - x0);
-        s_slot0[q] = (uint32_t)parts.rank[plo] * (uint32_t)(TX * TY);
+        s_slot0[q] = (uint32_t)(cx.cmap ? plo : (int)parts.rank[plo]) * (uint32_t)(TX * TY);
         if (FILTER) s_F[q] = cross_filter(cx, i, plo, __uint_as_float(ckeys[j]));
         atomicMax(&s_nown, (uint32_t)q + 1);
       }
@@ -768,6 +771,7 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
         const uint32_t ty = t / w;
         const uint32_t tile = ((xy >> 16) + ty) * (uint32_t)TX + (xy & 0xffffu) + (t - ty * w);
         uint32_t slot = s_slot0[ql] + tile;
+        if (cx.cmap) slot = __ldg(cx.cmap + slot);
         if (FILTER) { const uint64_t F = s_F[ql]; if (F && cross_removed(cx, F, tile)) slot = cx.nslots; }
         skeys[pos] = slot;
         spay[pos] = (uint32_t)j0 + ql;                    // position of the owner in the depth-sorted list
@@ -779,6 +783,57 @@ k_emit_keys_lb(const float* __restrict__ means2d, const int32_t* __restrict__ ra
   }
   __syncthreads();
   for (int x = threadIdx.x; x < plan.npass * SLOT_NB; x += blockDim.x) { const uint32_t c = s_hist[x]; if (c) atomicAdd(&ghist[x], c); }
+}
+
+// Renumbering of the OPEN slots (splx_plan.open_slots > 0: the caller vouches that a slot whose state has
+// SPLX_TILE_INVISIBLE holds no key -- the conservative regions of reading s21).  A city view leaves 85-90 % of the
+// (partition, tile) slots invisible, so the open ones need 16 bits where all slots of the participating partitions need
+// 17 or 18: two radix passes over the intersections instead of three.  cmap[s] = number of open slot s in slot order
+// (monotone: the sort order is unchanged); every other slot -> cap + 1, carried behind every list and counted by
+// k_tile_ranges (num_intersections[1]); cap itself = the pairs removed by the cross-boundary filter.  inv = the way back.
+// One CTA: 32 slots per thread and round, K * tiles <= 2 M slots.
+__global__ void __launch_bounds__(1024)
+k_slot_map(const uint8_t* __restrict__ state, const __grid_constant__ PartView pv, uint32_t ntiles, uint32_t nslots, uint32_t cap,
+           uint32_t* __restrict__ cmap, uint32_t* __restrict__ inv) {
+  __shared__ uint32_t sm[33];
+  uint32_t running = 0;
+  for (uint32_t b = 0; b < nslots; b += 1024 * 32) {
+    const uint32_t s0 = b + threadIdx.x * 32;
+    uint32_t open = 0;
+    if (s0 < nslots) {
+      uint32_t w[8];
+      if (s0 + 32 <= nslots) {
+        const uint4 a = *reinterpret_cast<const uint4*>(state + s0), c = *reinterpret_cast<const uint4*>(state + s0 + 16);
+        w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w; w[4] = c.x; w[5] = c.y; w[6] = c.z; w[7] = c.w;
+      } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          w[q] = 0xffffffffu;
+          for (int c = 0; c < 4; ++c) if (s0 + 4 * q + c < nslots) w[q] = (w[q] & ~(0xffu << (8 * c))) | ((uint32_t)state[s0 + 4 * q + c] << (8 * c));
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 32; ++k) {
+        const uint32_t s = s0 + k;
+        const bool inv_bit = (w[k >> 2] >> (8 * (k & 3))) & SPLX_TILE_INVISIBLE;
+        if (s < nslots && !inv_bit && pv.v[s / ntiles] >= 0) open |= 1u << k;
+      }
+    }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan((uint32_t)__popc(open), sm, total) + running;
+    if (s0 < nslots) {
+#pragma unroll
+      for (int k = 0; k < 32; ++k) {
+        const uint32_t s = s0 + k;
+        if (s >= nslots) break;
+        uint32_t c = cap + 1;
+        if ((open >> k) & 1u) { if (ex < cap) { c = ex; inv[ex] = s; } ++ex; }
+        cmap[s] = c;
+      }
+    }
+    running += total;
+  }
+  if (threadIdx.x == 0) { inv[cap] = nslots; inv[cap + 1] = nslots + 1; }
 }
 
 __global__ void __launch_bounds__(256)
@@ -794,6 +849,8 @@ k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint
     const uint32_t s = (uint32_t)(keys[j] >> 32);
     if (s >= nslots) {           // removed pairs: behind every list
       if (count_kept && (j == 0 || (uint32_t)(keys[j - 1] >> 32) < nslots)) *m_out = j;
+      // renumbered open slots (splx_plan.open_slots): a key that landed in a slot the caller declared INVISIBLE
+      if (s == nslots + 1) atomicAdd((unsigned long long*)(m_out + 1), 1ull);
       continue;
     }
     if (count_kept && j + 1 == m) *m_out = m;
@@ -869,7 +926,7 @@ __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_
 // words: one memset per call), the radix passes' status words (cleared on the device, only as far as the
 // actual counts reach) and the sort buffers.
 struct Layout {
-  size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes;
+  size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes, cmap, inv;
   size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, vis_list, pairs_tmp, total;
 };
 
@@ -899,6 +956,8 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   L.offs = take((size_t)n * 4);
   L.vis_list = take((size_t)n * 4);
   L.pairs_tmp = take((size_t)capacity * 8);      // (compact slot, depth-order position) pairs: two uint32[capacity]
+  L.cmap = take(((size_t)1 << sbits) * 4);       // renumbering of the open slots (k_slot_map) and its inverse
+  L.inv = take((((size_t)1 << sbits) + 2) * 4);
   L.total = off;
   return L;
 }
@@ -982,15 +1041,28 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   const uint32_t cslots = (uint32_t)nact * (uint32_t)ntiles;      // compact slots 0 .. cslots (cslots itself = filtered)
   int cbits = 1;
   while (((uint64_t)1 << cbits) <= cslots) ++cbits;
+  // renumbered open slots (splx_plan.open_slots), where that saves a pass over the intersections
+  CrossEmit cx;
+  memset(&cx, 0, sizeof cx);
+  cx.ntiles = (uint32_t)ntiles; cx.nslots = cslots;
+  if (plan.open_slots > 0 && plan.tile_state && aligned16(plan.tile_state)) {
+    const uint32_t cap = plan.open_slots < cslots ? plan.open_slots : cslots;
+    int obits = 1;
+    while (((uint64_t)1 << obits) <= (uint64_t)cap + 1) ++obits;       // the values 0 .. cap + 1
+    if ((obits + SLOT_BITS - 1) / SLOT_BITS < (cbits + SLOT_BITS - 1) / SLOT_BITS) {
+      uint32_t* cmap = (uint32_t*)(base + L.cmap);
+      uint32_t* inv = (uint32_t*)(base + L.inv);
+      k_slot_map<<<1, 1024, 0, ctx->stream>>>(plan.tile_state, plan.pv, (uint32_t)ntiles, (uint32_t)K * (uint32_t)ntiles, cap, cmap, inv);
+      SPLX_LAUNCH_CHECK(ctx, "k_slot_map");
+      cx.cmap = cmap; cx.nslots = cap; fin.inv = inv; cbits = obits;
+    }
+  }
   const PassPlan spl = plan_passes(0, cbits, SLOT_BITS);
   uint32_t* A_k = (uint32_t*)(base + L.pairs_tmp); uint32_t* A_p = A_k + out->capacity;
   uint32_t* B_k = (uint32_t*)out->keys; uint32_t* B_p = B_k + out->capacity;
   const bool startA = (spl.npass & 1) != 0;                       // so that the LAST pass reads A (and may overwrite B's memory)
   uint32_t* k0 = startA ? A_k : B_k; uint32_t* p0 = startA ? A_p : B_p;
   uint32_t* k1 = startA ? B_k : A_k; uint32_t* p1 = startA ? B_p : A_p;
-  CrossEmit cx;
-  memset(&cx, 0, sizeof cx);
-  cx.ntiles = (uint32_t)ntiles; cx.nslots = cslots;
   if (cross && cross->mask) {
     cx.mask = cross->mask; cx.tile_state = plan.tile_state;
     for (int k = 0; k < K; ++k) { cx.zlo[k] = cross->zlo[k]; cx.zhi[k] = cross->zhi[k]; cx.view[k] = plan.pv.v[k]; }

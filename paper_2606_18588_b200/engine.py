@@ -95,6 +95,8 @@ class Trainer:
         self._participants = {}     # view id -> partition bitmask (splx_visible_regions)
         self._geom_state = {}       # view id -> host uint8 [K, tiles]
         self._bucket_state = {}     # tuple of view ids -> device uint8 [K * tiles] (geometric | saturated bits)
+        self._bucket_open = {}      # tuple of view ids -> number of slots without the INVISIBLE bit (conservative regions), else 0
+        self._part_max_scale = None
         self._graphs = {}
         self._m_host = torch.zeros(max(self.max_views, 1), dtype=torch.int64).pin_memory()   # M of every bucket
         self._m_event = None
@@ -173,10 +175,10 @@ class Trainer:
             self._graphs.clear()
         return self._images[:B], self._T_totals[:B], self._g_images[:B]
 
-    def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True) -> binding.Plan:
+    def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True, open_slots=0) -> binding.Plan:
         if view_of_part is None:
             view_of_part = [0] * self.K
-        return binding.Plan(cams, view_of_part, tile_state, sparse, getattr(self, "_part_max_scale", None))
+        return binding.Plan(cams, view_of_part, tile_state, sparse, getattr(self, "_part_max_scale", None), open_slots)
 
     def forward_plan(self, plan: binding.Plan, sat_eps=None, tile_state_out=None, count_pairs=False):
         """a1-a6 for all views of the plan in one launch per stage; returns images[B,H,W,3]."""
@@ -263,7 +265,7 @@ class Trainer:
                 k = j if bp is None else int(bp[j])
                 pms[k] = max(pms[k], float(self._aabb[2][j]))
             self._part_max_scale = pms
-        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear(); self._graphs.clear()
+        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear(); self._bucket_open.clear(); self._graphs.clear()
 
     def participants(self, view_id, cam) -> int:
         """GetParticipants(v) (L249): partitions whose boxes meet the view frustum; cached per view id."""
@@ -306,8 +308,11 @@ class Trainer:
                 if vop[k] >= 0:
                     st[k] = self._geom_state[view_ids[vop[k]]][k]
             self._bucket_state[key] = torch.from_numpy(st.reshape(-1)).to(self.ctx.device)
+            # conservative regions (boxes of means + max_scale, reading s21): an INVISIBLE slot holds no intersection, so
+            # the slot sort may renumber the open ones (splx_plan.open_slots); the geometric bits never change afterwards
+            self._bucket_open[key] = int((st & binding.TILE_INVISIBLE == 0).sum()) if self._part_max_scale is not None else 0
         state = self._bucket_state[key]
-        return self.make_plan(cams, vop, state, sparse), (state if saturation else None)
+        return self.make_plan(cams, vop, state, sparse, self._bucket_open.get(key, 0)), (state if saturation else None)
 
     # ---- one library call per iteration (splx_iteration) -------------------------------------------------------
     def _frontset(self, which):

@@ -716,3 +716,75 @@ def test_reach_test_on_the_mean_culls_nothing_visible(city, blocks):
         for name in ("means2d", "depth", "conic_opacity", "rgb", "blend", "clamp"):
             x, y = getattr(a.proj, name), getattr(b.proj, name)
             assert torch.equal(x[vis], y[vis]), name
+
+
+def _slot_passes(values):
+    bits = 1
+    while (1 << bits) <= values:
+        bits += 1
+    return (bits + 7) // 8
+
+
+def test_renumbered_open_slots_give_the_same_binning(blocks):
+    """splx_plan.open_slots (conservative regions: an INVISIBLE slot holds no intersection): the slot sort runs on a
+    renumbering of the open slots when that saves a radix pass -- M, keys, vals and ranges bit-equal to the plain plan.
+    And a caller whose promise does not hold: the keys that land in an INVISIBLE slot are carried behind every list,
+    get no range and are counted in num_intersections[1]; the lists of the open slots are unchanged."""
+    sc = blocks
+    tr = _trainer_conservative(sc)
+    ntiles = tr.bins.tile_ranges.numel() // (2 * tr.K)
+    saved = 0
+    tr._workspaces(sc.cameras[0])
+    for v, cam in enumerate(sc.cameras):
+        plan, _ = tr.bucket_plan([v], [cam], saturation=False)
+        assert plan.open_slots > 0
+        nact = sum(1 for k, x in enumerate(plan.view_of_part) if x >= 0 and tr.part_offsets[k + 1] > tr.part_offsets[k])
+        saves = _slot_passes(min(plan.open_slots, nact * ntiles) + 1) < _slot_passes(nact * ntiles)
+        saved += saves
+        plain = tr.make_plan(plan.cams, plan.view_of_part, plan.tile_state, True, 0)
+        tr.ctx.project_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj)
+        out = []
+        for p in (plain, plan):
+            tr.bins.keys.fill_(0); tr.bins.vals.fill_(0)
+            launches = tr.ctx.launch_count()
+            tr._bin_sort(tr.proj, p, tr.bins, tr._ws_sort)
+            M, keys, vals, ranges = G.gpu_bins(tr)
+            out.append((M, keys.copy(), vals.copy(), ranges.copy(), int(tr.bins.num_intersections[1]), tr.ctx.launch_count() - launches))
+        (M0, k0, v0, r0, d0, l0), (M1, k1, v1, r1, d1, l1) = out
+        assert M0 == M1 and M0 > 0 and d0 == 0 and d1 == 0
+        assert np.array_equal(k0, k1) and np.array_equal(v0, v1) and np.array_equal(r0, r1)
+        if saves:
+            assert l1 == l0          # one launch more for the map, one radix pass less
+    assert saved >= 1, "no view of the scene exercises the renumbering"
+
+    # a broken promise: every second tile of the participating partitions declared INVISIBLE although it holds keys
+    v, cam = 0, sc.cameras[0]
+    plan, _ = tr.bucket_plan([v], [cam], saturation=False)
+    st = plan.tile_state.cpu().numpy().reshape(tr.K, ntiles).copy()
+    tr.ctx.project_plan(tr.params, tr.part_offsets, plan, tr.sh_degree, tr.proj)
+    tr._bin_sort(tr.proj, tr.make_plan(plan.cams, plan.view_of_part, plan.tile_state, True, 0), tr.bins, tr._ws_sort)
+    M0, k0, v0, r0 = [np.copy(x) if isinstance(x, np.ndarray) else x for x in G.gpu_bins(tr)]
+    bad = st.copy()
+    bad[:, ::2] |= binding.TILE_INVISIBLE
+    n_open = int((bad & binding.TILE_INVISIBLE == 0).sum())
+    dev = torch.from_numpy(bad.reshape(-1)).cuda()
+    nact = sum(1 for k, x in enumerate(plan.view_of_part) if x >= 0 and tr.part_offsets[k + 1] > tr.part_offsets[k])
+    assert _slot_passes(n_open + 1) < _slot_passes(nact * ntiles), "the broken promise must take the renumbered path"
+    tr._bin_sort(tr.proj, tr.make_plan(plan.cams, plan.view_of_part, dev, True, n_open), tr.bins, tr._ws_sort)
+    torch.cuda.synchronize()
+    keys = G.u64(tr.bins.keys)[:M0]; vals = G.u32(tr.bins.vals)[:M0]
+    ranges = G.u32(tr.bins.tile_ranges).reshape(tr.K, ntiles, 2)
+    slot0 = (k0 >> np.uint64(32)).astype(np.int64)
+    lost = (bad.reshape(-1)[slot0] & binding.TILE_INVISIBLE) != 0            # keys of the reference that sit in a declared slot
+    assert lost.any() and int(tr.bins.num_intersections[1]) == int(lost.sum())
+    kept = int((~lost).sum())
+    assert np.array_equal(keys[:kept], k0[~lost]) and np.array_equal(vals[:kept], v0[~lost])     # the open lists, in order
+    assert ((keys[kept:] >> np.uint64(32)) == tr.K * ntiles + 1).all()
+    for k in range(tr.K):
+        for t in range(ntiles):
+            a, b = r0[k, t]
+            if bad[k, t] & binding.TILE_INVISIBLE or a == b:
+                assert ranges[k, t, 0] == ranges[k, t, 1] == 0 or ranges[k, t, 0] == ranges[k, t, 1]
+            else:
+                a1, b1 = ranges[k, t]
+                assert b1 - a1 == b - a and np.array_equal(vals[a1:b1], v0[a:b])
