@@ -469,11 +469,16 @@ def run_ours(args):
             tg = targets[grp[0]:grp[0] + 1] if nb == 1 else targets[torch.as_tensor(grp, device="cuda")]
             e = ev[gi]
             # a1 as splx_iteration runs it: the geometry half, the binning, then the colour of the visible list (e[8] between)
-            e[0].record(); c.project_geometry_plan(tr.params, po, plan, tr.proj)
-            e[1].record(); tr._bin_sort(tr.proj, plan, tr.bins, tr._ws_sort)
-            e[8].record()
-            lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
-            c.project_colour_list_plan(tr.params, po, plan, tr.sh_degree, tr.proj, lst, cnt)
+            if fused_proj:
+                e[0].record(); c.project_plan(tr.params, po, plan, tr.sh_degree, tr.proj)
+                e[1].record(); tr._bin_sort(tr.proj, plan, tr.bins, tr._ws_sort)
+                e[8].record()
+            else:
+                e[0].record(); c.project_geometry_plan(tr.params, po, plan, tr.proj)
+                e[1].record(); tr._bin_sort(tr.proj, plan, tr.bins, tr._ws_sort)
+                e[8].record()
+                lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
+                c.project_colour_list_plan(tr.params, po, plan, tr.sh_degree, tr.proj, lst, cnt)
             e[2].record(); c.render_partial_plan(tr.proj, tr.bins, plan, tr.partials)
             e[3].record()
             if tr.lambda_dssim > 0:
@@ -496,6 +501,7 @@ def run_ours(args):
         ev[-1][7].record()
 
     flags = tr._use_flags(plans[0][0])
+    fused_proj = tr.use_fused_projection([p for p, _ in plans])
     tr._trainset(B, False, flags)     # allocates the D-SSIM workspace / the touched flags
     n_staged = max(3, min(args.steps, 10))
     restore()

@@ -116,6 +116,7 @@ class IterOptsS(C.Structure):
 
 
 ITER_HOST = 1
+ITER_FUSED_PROJECTION = 4
 
 
 def lib():
@@ -620,14 +621,15 @@ class Context:
                                                       float(B if scale is None else scale), _ptr(g_image), _ptr(loss_sum)))
 
     def iteration(self, trainset: "TrainsetS", buckets, n_views, targets, images_out=None, loss_out=None, m_out=None,
-                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None):
+                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None, fused_projection=False):
         """splx_iteration.  buckets: ctypes array of BucketS; targets / images_out: lists of raw pointers (ints; device
         pointers, or pinned host pointers with host=True); loss_out / m_out: raw pinned host pointers or None."""
         tg = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) for x in targets])
         io = None
         if images_out is not None:
             io = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) if x else None for x in images_out])
-        opts = IterOptsS(ITER_HOST if host else 0, float(sat_eps), float(lambda_dssim))
+        opts = IterOptsS((ITER_HOST if host else 0) | (ITER_FUSED_PROJECTION if fused_projection else 0), float(sat_eps),
+                         float(lambda_dssim))
         self._check(lib().splx_iteration(self._h, C.byref(trainset), len(buckets), buckets, int(n_views), tg, io,
                                          C.c_void_p(loss_out) if loss_out else None, C.c_void_p(m_out) if m_out else None,
                                          C.byref(opts), C.byref(adam) if adam is not None else None))

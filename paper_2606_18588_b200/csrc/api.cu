@@ -58,9 +58,9 @@ int make_plan_dev(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, 
   out->ntiles = out->TX * out->TY;
   out->flags = plan->flags;
   out->tile_state = plan->tile_state;
-  if (plan->open_slots < 0 || (plan->open_slots > 0 && !plan->tile_state))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: open_slots < 0, or > 0 without tile_state", who);
-  out->open_slots = (uint32_t)plan->open_slots;
+  if (plan->open_slots != 0 && !plan->tile_state) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: open_slots without tile_state", who);
+  out->open_slots = (uint32_t)(plan->open_slots < 0 ? -(int64_t)plan->open_slots : (int64_t)plan->open_slots);
+  out->open_forced = plan->open_slots < 0;
   return SPLX_OK;
 }
 

@@ -72,7 +72,8 @@ struct PlanDev {
   PartView pv;
   CamDev cam[SPLX_MAX_VIEWS];
   float max_scale[SPLX_MAX_K];   // splx_plan.max_scale, or < 0: no reach test
-  uint32_t open_slots;           // splx_plan.open_slots
+  uint32_t open_slots;           // |splx_plan.open_slots|
+  bool open_forced;              // splx_plan.open_slots < 0: renumber even where no radix pass is saved
 };
 
 // Per-view buffers of the composition kernels (view b of the launch -> its own pointers), so that the views of a

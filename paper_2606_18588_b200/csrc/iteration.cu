@@ -71,7 +71,7 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (!ts || !buckets || !targets || !opts || n_buckets < 1 || n_views < 1)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: null argument or empty iteration");
-  if (opts->flags & ~SPLX_ITER_HOST) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: unknown flags %d", opts->flags);
+  if (opts->flags & ~(SPLX_ITER_HOST | SPLX_ITER_FUSED_PROJECTION)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: unknown flags %d", opts->flags);
   const bool host = (opts->flags & SPLX_ITER_HOST) != 0;
   if (!host && (images_out || loss_out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: images_out / loss_out need SPLX_ITER_HOST");
   const int64_t n = ts->params.n;
@@ -131,6 +131,11 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
     int r;
     // the colour only for the visible Gaussians, once the binning has compacted their list (the geometry alone decides
     // visibility, depth and footprint: the binning does not read the colour)
+    if (opts->flags & SPLX_ITER_FUSED_PROJECTION) {
+      if ((r = splx_project_plan(ctx, &g, K, ts->part_offsets, &bk.plan, ts->sh_degree, &fs.proj))) return r;
+      return splx_bin_sort_filtered_plan(ctx, &fs.proj, n, K, ts->part_offsets, &bk.plan, ts->cross_mask, bk.part_depth_range,
+                                         &fs.bins, fs.ws, fs.ws_bytes);
+    }
     if ((r = splx_project_geometry_plan(ctx, &g, K, ts->part_offsets, &bk.plan, &fs.proj))) return r;
     if ((r = splx_bin_sort_filtered_plan(ctx, &fs.proj, n, K, ts->part_offsets, &bk.plan, ts->cross_mask, bk.part_depth_range,
                                          &fs.bins, fs.ws, fs.ws_bytes))) return r;

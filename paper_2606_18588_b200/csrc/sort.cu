@@ -1049,7 +1049,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
     const uint32_t cap = plan.open_slots < cslots ? plan.open_slots : cslots;
     int obits = 1;
     while (((uint64_t)1 << obits) <= (uint64_t)cap + 1) ++obits;       // the values 0 .. cap + 1
-    if ((obits + SLOT_BITS - 1) / SLOT_BITS < (cbits + SLOT_BITS - 1) / SLOT_BITS) {
+    if (plan.open_forced || (obits + SLOT_BITS - 1) / SLOT_BITS < (cbits + SLOT_BITS - 1) / SLOT_BITS) {
       uint32_t* cmap = (uint32_t*)(base + L.cmap);
       uint32_t* inv = (uint32_t*)(base + L.inv);
       k_slot_map<<<1, 1024, 0, ctx->stream>>>(plan.tile_state, plan.pv, (uint32_t)ntiles, (uint32_t)K * (uint32_t)ntiles, cap, cmap, inv);

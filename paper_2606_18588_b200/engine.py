@@ -83,6 +83,10 @@ class Trainer:
         self.flagged_grads = True
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
         self.pipeline_buckets = True
+        #: a1 inside splx_iteration: None = fused (one kernel) when every partition takes part in every bucket -- then most
+        #: Gaussians are visible (aerial views) --, else geometry -> binning -> colour of the visible list (city views, where
+        #: most participating Gaussians are culled); True / False force one or the other.  Same results bit for bit
+        self.fused_projection = None
         self._touched = None
         self._cam = None
         self._aabb = None           # (lo, hi, max_scale or None): boxes of the geometric visibility prediction
@@ -396,6 +400,11 @@ class Trainer:
             if m > self.capacity:
                 raise CapacityError(f"{m} tile intersections exceed the capacity {self.capacity}: the farthest keys were dropped")
 
+    def use_fused_projection(self, plans) -> bool:
+        if self.fused_projection is not None:
+            return bool(self.fused_projection)
+        return all(v >= 0 for p in plans for v in p.view_of_part)
+
     def _run_iteration(self, plans, groups, n_views, targets, sat_eps, adam=True, host=False, images_out=None,
                        loss_out=None, flags=False):
         """plans: [(Plan, state_out)], groups: view positions per plan; targets: list of raw pointers per view."""
@@ -411,7 +420,8 @@ class Trainer:
             cfg = self._adam_cfg(self.step_count)
         self._plan = plans[-1][0]
         self.ctx.iteration(ts, bk, n_views, targets, images_out, loss_out, self._m_host.data_ptr(), host=host,
-                           sat_eps=0.0 if sat_eps is None else sat_eps, lambda_dssim=self.lambda_dssim, adam=cfg)
+                           sat_eps=0.0 if sat_eps is None else sat_eps, lambda_dssim=self.lambda_dssim, adam=cfg,
+                           fused_projection=self.use_fused_projection([p for p, _ in plans]))
         self._m_buckets = len(plans)
         return ts, bk
 
