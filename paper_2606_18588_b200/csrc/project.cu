@@ -335,25 +335,60 @@ k_project_geo(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
 
 // The colour of the visible Gaussians (the binning's list, index order): one thread per entry, persistent grid because
 // the count lives on the device.  Same arithmetic as the colour half of k_project_fwd (bit-equal rgb, clamp, blend[2]).
+// The 32 rows of a warp are scattered (192 contiguous bytes each): the warp copies them chunk by chunk -- lane c of
+// round r takes chunk (32 r + c) % NV of row (32 r + c) / NV, so that 12 consecutive lanes cover one row's 192 bytes --
+// into its swizzled shared-memory block with 16-byte cp.async, instead of every lane walking its own row with a
+// 192-byte stride (32 L1 wavefronts per load instruction).
 template <int DEG>
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_colour_list(splx_gaussians g, const __grid_constant__ PlanDev plan, const __grid_constant__ RunTable rt, splx_projected out,
               const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr) {
+  constexpr int NSH = (DEG + 1) * (DEG + 1);
+  constexpr int NV = (NSH * 3 + 3) / 4;
+  constexpr bool STAGE = DEG > 0;
+  __shared__ __align__(16) float4 s_sh[STAGE ? PROJ_THREADS * NV : 1];
   const uint64_t nvis = *nvis_ptr;
   const int lane = threadIdx.x & 31;
-  for (uint64_t j = (uint64_t)blockIdx.x * PROJ_THREADS + threadIdx.x; j < nvis; j += (uint64_t)gridDim.x * PROJ_THREADS) {
-    const int64_t i = (int64_t)vlist[j];
-    int lo = 0, hi = rt.n - 1;                          // the run (partition) of Gaussian i -> its view
-    while (lo < hi) {
-      const int mid = (lo + hi + 1) >> 1;
-      if (rt.begin[mid] <= i) lo = mid; else hi = mid - 1;
+  float4* ws = s_sh + (threadIdx.x & ~31) * NV;                 // this warp's 32 rows
+  // whole warps stay in the loop together (j0 is warp uniform): the staging below is warp cooperative
+  for (uint64_t j0 = (uint64_t)blockIdx.x * PROJ_THREADS + (threadIdx.x & ~31); j0 < nvis; j0 += (uint64_t)gridDim.x * PROJ_THREADS) {
+    const uint64_t j = j0 + lane;
+    const bool have = j < nvis;
+    const int64_t i = have ? (int64_t)vlist[j] : 0;
+    if (STAGE) {
+      const int rows = (int)(nvis - j0 < 32 ? nvis - j0 : 32);
+      __syncwarp();                                              // the previous round's reads of ws are done
+      for (int c = lane; c < 32 * NV; c += 32) {
+        const int row = c / NV, q = c - row * NV;
+        const int64_t ir = __shfl_sync(0xffffffffu, i, row);
+        if (row < rows) {
+          const unsigned dst = (unsigned)__cvta_generic_to_shared(ws + row * NV + sh_swz<NV>(q, row));
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(reinterpret_cast<const float4*>(g.sh + 48 * ir) + q));
+        }
+      }
+      asm volatile("cp.async.commit_group;");
     }
-    const CamDev& cam = plan.cam[rt.view[lo]];
-    float m[3];
+    const CamDev* cam = &plan.cam[0];
+    float m[3] = {0.f, 0.f, 0.f};
+    if (have) {
+      int lo = 0, hi = rt.n - 1;                          // the run (partition) of Gaussian i -> its view
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (rt.begin[mid] <= i) lo = mid; else hi = mid - 1;
+      }
+      cam = &plan.cam[rt.view[lo]];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) m[k] = g.mean[3 * i + k];
-    float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
-    colour<DEG, false>(reinterpret_cast<const float4*>(g.sh + 48 * i), lane, cam, m, i, out, bl);
+      for (int k = 0; k < 3; ++k) m[k] = g.mean[3 * i + k];
+    }
+    if (STAGE) {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      __syncwarp();
+    }
+    if (have) {
+      float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
+      if (STAGE) colour<DEG, true>(ws, lane, *cam, m, i, out, bl);
+      else colour<DEG, false>(reinterpret_cast<const float4*>(g.sh + 48 * i), lane, *cam, m, i, out, bl);
+    }
   }
 }
 
