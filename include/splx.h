@@ -310,8 +310,20 @@ typedef struct {
                                   key fall into an INVISIBLE slot all the same (or into an open slot beyond the bound), it is
                                   carried behind every list under slot number K*tiles + 1, gets no range, and is counted in
                                   num_intersections[1].  The renumbering is used where it saves a radix pass; a NEGATIVE value
-                                  (bound = -open_slots) forces it (tests). */
+                                  (bound = -open_slots) forces it (tests).  Needs slot_map. */
+  const uint32_t *slot_map;    /* DEVICE [splx_slot_map_words(K, cams)] or NULL (no renumbering): the numbering of the open slots
+                                  and its inverse, written ONCE by splx_slot_map for this (tile_state INVISIBLE bits,
+                                  view_of_part, open_slots) -- a caller who changes one of them rebuilds it; the saturated bits
+                                  that composition rewrites every iteration do not enter it */
 } splx_plan;
+
+/* The slot numbering behind splx_plan.open_slots: slot_map_out (DEVICE uint32[splx_slot_map_words]) receives, for the plan's
+ * tile_state, view_of_part and |open_slots| (plan->slot_map itself is ignored), cmap[K*tiles] = number of every open slot in
+ * slot order (others: |open_slots| + 1) followed by inv[|open_slots| + 2] = the way back.  One small launch on the context's
+ * stream; the plan that later carries slot_map must have the same three inputs. */
+size_t splx_slot_map_words(int K, const splx_camera *cam);
+int splx_slot_map(splx_ctx *ctx, int K, const splx_plan *plan, uint32_t *slot_map_out);
+
 
 /* Geometric visibility (L212, L227): HOST computation, no device work, ctx not needed.  n_boxes axis-aligned boxes
  * [aabb_lo[j], aabb_hi[j]] (HOST float[n_boxes][3], world space), box j belonging to partition box_part[j] (HOST

@@ -25,6 +25,7 @@ OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "splx_create", "splx_destroy", "splx_last_error", "splx_set_stream", "splx_launch_count",
+    "splx_slot_map_words", "splx_slot_map",
     "splx_project", "splx_bin_sort_ws_bytes", "splx_bin_sort", "splx_check_capacity",
     "splx_render_partial", "splx_compose", "splx_l1_loss_grad", "splx_compose_backward",
     "splx_raster_backward", "splx_project_backward", "splx_backward_ws_bytes", "splx_backward",
@@ -84,7 +85,8 @@ class PartialS(C.Structure):
 
 class PlanS(C.Structure):
     _fields_ = [("n_views", C.c_int32), ("cams", C.c_void_p), ("view_of_part", C.c_void_p),
-                ("tile_state", C.c_void_p), ("flags", C.c_int32), ("max_scale", C.c_void_p), ("open_slots", C.c_int32)]
+                ("tile_state", C.c_void_p), ("flags", C.c_int32), ("max_scale", C.c_void_p), ("open_slots", C.c_int32),
+                ("slot_map", C.c_void_p)]
 
 
 class FrontsetS(C.Structure):
@@ -131,6 +133,9 @@ def lib():
         L.splx_last_error.argtypes = [C.c_void_p]
         L.splx_launch_count.restype = C.c_int64
         L.splx_launch_count.argtypes = [C.c_void_p]
+        L.splx_slot_map_words.restype = C.c_size_t
+        L.splx_slot_map_words.argtypes = [C.c_int, C.c_void_p]
+        L.splx_slot_map.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.splx_bin_sort_ws_bytes.restype = C.c_size_t
         L.splx_bin_sort_ws_bytes.argtypes = [C.c_int64, C.c_uint64, C.c_int, C.c_void_p]
         L.splx_backward_ws_bytes.restype = C.c_size_t
@@ -219,7 +224,7 @@ class Plan:
     """splx_plan: B views of one size, the view each partition renders (-1 = not a participant), the
     optional device tile-state bytes [K*tiles] and the flags.  Keeps the ctypes storage alive."""
 
-    def __init__(self, cams, view_of_part, tile_state=None, sparse=False, max_scale=None, open_slots=0):
+    def __init__(self, cams, view_of_part, tile_state=None, sparse=False, max_scale=None, open_slots=0, slot_map=None):
         self.cams = list(cams)
         self.view_of_part = [int(v) for v in view_of_part]
         self.tile_state = tile_state
@@ -229,8 +234,9 @@ class Plan:
         self._ms = None if max_scale is None else (C.c_float * len(self.view_of_part))(*[float(x) for x in max_scale])
         self._s = PlanS(len(self.cams), C.cast(self._cams, C.c_void_p), C.cast(self._vop, C.c_void_p),
                         _ptr(tile_state), self.flags, C.cast(self._ms, C.c_void_p) if self._ms is not None else None,
-                        int(open_slots))
+                        int(open_slots), _ptr(slot_map))
         self.open_slots = int(open_slots)
+        self.slot_map = slot_map
 
     @property
     def K(self):
@@ -482,6 +488,18 @@ class Context:
         lr = (C.c_float * n)(*[float(x) for x in lrs])
         self._check(lib().splx_adam_groups_flagged(self._h, _ptr(param), _ptr(grad), _ptr(m), _ptr(v), n, offs, wd, int(rows),
                                                    _ptr(touched), lr, beta1, beta2, eps, step, grad_scale))
+
+    @staticmethod
+    def slot_map_words(K, cam) -> int:
+        cs = camera_struct(cam)
+        return int(lib().splx_slot_map_words(int(K), C.byref(cs)))
+
+    def slot_map(self, plan: "Plan", device=None):
+        """splx_slot_map: the numbering of the plan's open slots (a new device tensor), for Plan(..., slot_map=...)."""
+        words = self.slot_map_words(plan.K, plan.cams[0])
+        out = torch.empty(words, dtype=torch.int32, device=plan.tile_state.device if device is None else device)
+        self._check(lib().splx_slot_map(self._h, plan.K, plan.ref(), _ptr(out)))
+        return out
 
     # ---- the same stages under a launch plan (visibility prediction, consolidated views) ---------
     visible_regions = staticmethod(visible_regions)     # host computations: no context needed

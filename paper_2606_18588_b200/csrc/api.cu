@@ -59,6 +59,9 @@ int make_plan_dev(splx_ctx* ctx, const char* who, int K, const splx_plan* plan, 
   out->flags = plan->flags;
   out->tile_state = plan->tile_state;
   if (plan->open_slots != 0 && !plan->tile_state) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: open_slots without tile_state", who);
+  if (plan->slot_map && (plan->open_slots == 0 || !aligned16(plan->slot_map)))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "%s: slot_map without open_slots, or misaligned", who);
+  out->slot_map = plan->slot_map;
   out->open_slots = (uint32_t)(plan->open_slots < 0 ? -(int64_t)plan->open_slots : (int64_t)plan->open_slots);
   out->open_forced = plan->open_slots < 0;
   return SPLX_OK;
@@ -77,7 +80,7 @@ struct SinglePlan {
   explicit SinglePlan(const splx_camera* cam) {
     for (int k = 0; k < SPLX_MAX_K; ++k) views[k] = 0;
     plan.n_views = 1; plan.cams = cam; plan.view_of_part = views; plan.tile_state = nullptr; plan.flags = 0;
-    plan.max_scale = nullptr; plan.open_slots = 0;
+    plan.max_scale = nullptr; plan.open_slots = 0; plan.slot_map = nullptr;
   }
 };
 
@@ -134,6 +137,25 @@ int splx_set_stream(splx_ctx* ctx, void* cuda_stream) {
 }
 
 int64_t splx_launch_count(const splx_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+size_t splx_slot_map_words(int K, const splx_camera* cam) {
+  if (!cam || cam->width <= 0 || cam->height <= 0 || K < 1 || K > SPLX_MAX_K) return 0;
+  const size_t tiles = (size_t)((cam->width + SPLX_TILE - 1) / SPLX_TILE) * (size_t)((cam->height + SPLX_TILE - 1) / SPLX_TILE);
+  return 2 * (size_t)K * tiles + 2;
+}
+
+int splx_slot_map(splx_ctx* ctx, int K, const splx_plan* plan, uint32_t* slot_map_out) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!slot_map_out || !aligned16(slot_map_out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_slot_map: slot_map_out null or misaligned");
+  splx_plan p;
+  if (plan) { p = *plan; p.slot_map = nullptr; }
+  PlanDev pd;
+  int rc;
+  if ((rc = make_plan_dev(ctx, "splx_slot_map", K, plan ? &p : nullptr, &pd))) return rc;
+  if (!pd.tile_state || pd.open_slots == 0 || !aligned16(pd.tile_state))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_slot_map: the plan needs tile_state (16-byte aligned) and open_slots");
+  return launch_slot_map(ctx, pd, slot_map_out);
+}
 
 int splx_project_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets, const splx_plan* plan,
                       int sh_degree, const splx_projected* out) {

@@ -74,6 +74,7 @@ struct PlanDev {
   float max_scale[SPLX_MAX_K];   // splx_plan.max_scale, or < 0: no reach test
   uint32_t open_slots;           // |splx_plan.open_slots|
   bool open_forced;              // splx_plan.open_slots < 0: renumber even where no radix pass is saved
+  const uint32_t* slot_map;      // splx_plan.slot_map
 };
 
 // Per-view buffers of the composition kernels (view b of the launch -> its own pointers), so that the views of a
@@ -199,6 +200,7 @@ int launch_adam_sparse(splx_ctx*, const splx_gaussian_grads* params, const splx_
 int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX, int TY, const uint32_t** list,
                      const uint64_t** count);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
+int launch_slot_map(splx_ctx*, const PlanDev&, uint32_t* slot_map_out);
 int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, const PlanDev&, const int64_t* part_offsets,
                     const splx_binning*, void* ws, size_t ws_bytes, const CrossDev* cross = nullptr);
 int launch_cross_sets(splx_ctx*, const splx_gaussians*, int K, const int64_t* part_offsets, const float* cell_lo,

@@ -926,7 +926,7 @@ __global__ void k_publish_m(const Counters* cnt, uint64_t* out) { *out = cnt->m_
 // words: one memset per call), the radix passes' status words (cleared on the device, only as far as the
 // actual counts reach) and the sort buffers.
 struct Layout {
-  size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes, cmap, inv;
+  size_t counters, ghist_d, ghist_s, st_scan_v, st_scan_t, st_depth, st_slot, zero_bytes;
   size_t ckeys_a, cvals_a, ckeys_b, cvals_b, offs, vis_list, pairs_tmp, total;
 };
 
@@ -956,8 +956,6 @@ static Layout make_layout(int64_t n, uint64_t capacity, int sbits) {
   L.offs = take((size_t)n * 4);
   L.vis_list = take((size_t)n * 4);
   L.pairs_tmp = take((size_t)capacity * 8);      // (compact slot, depth-order position) pairs: two uint32[capacity]
-  L.cmap = take(((size_t)1 << sbits) * 4);       // renumbering of the open slots (k_slot_map) and its inverse
-  L.inv = take((((size_t)1 << sbits) + 2) * 4);
   L.total = off;
   return L;
 }
@@ -974,6 +972,14 @@ int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX
   const char* base = (const char*)ws;
   *list = (const uint32_t*)(base + L.vis_list);       // index order: consecutive rows of the list are close in memory
   *count = &((const Counters*)(base + L.counters))->n_visible;
+  return SPLX_OK;
+}
+
+int launch_slot_map(splx_ctx* ctx, const PlanDev& plan, uint32_t* slot_map_out) {
+  const uint32_t nslots = (uint32_t)plan.K * (uint32_t)plan.ntiles;
+  k_slot_map<<<1, 1024, 0, ctx->stream>>>(plan.tile_state, plan.pv, (uint32_t)plan.ntiles, nslots, plan.open_slots, slot_map_out,
+                                          slot_map_out + nslots);
+  SPLX_LAUNCH_CHECK(ctx, "k_slot_map");
   return SPLX_OK;
 }
 
@@ -1045,16 +1051,12 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
   CrossEmit cx;
   memset(&cx, 0, sizeof cx);
   cx.ntiles = (uint32_t)ntiles; cx.nslots = cslots;
-  if (plan.open_slots > 0 && plan.tile_state && aligned16(plan.tile_state)) {
-    const uint32_t cap = plan.open_slots < cslots ? plan.open_slots : cslots;
+  if (plan.open_slots > 0 && plan.slot_map) {
+    const uint32_t cap = plan.open_slots;       // the bound the caller built the map with (splx_slot_map)
     int obits = 1;
     while (((uint64_t)1 << obits) <= (uint64_t)cap + 1) ++obits;       // the values 0 .. cap + 1
     if (plan.open_forced || (obits + SLOT_BITS - 1) / SLOT_BITS < (cbits + SLOT_BITS - 1) / SLOT_BITS) {
-      uint32_t* cmap = (uint32_t*)(base + L.cmap);
-      uint32_t* inv = (uint32_t*)(base + L.inv);
-      k_slot_map<<<1, 1024, 0, ctx->stream>>>(plan.tile_state, plan.pv, (uint32_t)ntiles, (uint32_t)K * (uint32_t)ntiles, cap, cmap, inv);
-      SPLX_LAUNCH_CHECK(ctx, "k_slot_map");
-      cx.cmap = cmap; cx.nslots = cap; fin.inv = inv; cbits = obits;
+      cx.cmap = plan.slot_map; cx.nslots = cap; fin.inv = plan.slot_map + (size_t)K * ntiles; cbits = obits;
     }
   }
   const PassPlan spl = plan_passes(0, cbits, SLOT_BITS);

@@ -100,6 +100,7 @@ class Trainer:
         self._geom_state = {}       # view id -> host uint8 [K, tiles]
         self._bucket_state = {}     # tuple of view ids -> device uint8 [K * tiles] (geometric | saturated bits)
         self._bucket_open = {}      # tuple of view ids -> number of slots without the INVISIBLE bit (conservative regions), else 0
+        self._bucket_map = {}       # tuple of view ids -> device numbering of those slots (splx_slot_map)
         self._part_max_scale = None
         self._graphs = {}
         self._m_host = torch.zeros(max(self.max_views, 1), dtype=torch.int64).pin_memory()   # M of every bucket
@@ -179,10 +180,15 @@ class Trainer:
             self._graphs.clear()
         return self._images[:B], self._T_totals[:B], self._g_images[:B]
 
-    def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True, open_slots=0) -> binding.Plan:
+    def make_plan(self, cams, view_of_part=None, tile_state=None, sparse=True, open_slots=0, slot_map=None) -> binding.Plan:
+        """open_slots != 0 (splx_plan.open_slots): the numbering of the open slots is built here (splx_slot_map, one small
+        launch) unless the caller passes the one it keeps for these (tile_state, view_of_part, open_slots)."""
         if view_of_part is None:
             view_of_part = [0] * self.K
-        return binding.Plan(cams, view_of_part, tile_state, sparse, getattr(self, "_part_max_scale", None), open_slots)
+        ms = getattr(self, "_part_max_scale", None)
+        if open_slots and slot_map is None:
+            slot_map = self.ctx.slot_map(binding.Plan(cams, view_of_part, tile_state, sparse, ms, open_slots))
+        return binding.Plan(cams, view_of_part, tile_state, sparse, ms, open_slots, slot_map)
 
     def forward_plan(self, plan: binding.Plan, sat_eps=None, tile_state_out=None, count_pairs=False):
         """a1-a6 for all views of the plan in one launch per stage; returns images[B,H,W,3]."""
@@ -269,7 +275,7 @@ class Trainer:
                 k = j if bp is None else int(bp[j])
                 pms[k] = max(pms[k], float(self._aabb[2][j]))
             self._part_max_scale = pms
-        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear(); self._bucket_open.clear(); self._graphs.clear()
+        self._participants.clear(); self._geom_state.clear(); self._bucket_state.clear(); self._bucket_open.clear(); self._bucket_map.clear(); self._graphs.clear()
 
     def participants(self, view_id, cam) -> int:
         """GetParticipants(v) (L249): partitions whose boxes meet the view frustum; cached per view id."""
@@ -316,7 +322,10 @@ class Trainer:
             # the slot sort may renumber the open ones (splx_plan.open_slots); the geometric bits never change afterwards
             self._bucket_open[key] = int((st & binding.TILE_INVISIBLE == 0).sum()) if self._part_max_scale is not None else 0
         state = self._bucket_state[key]
-        return self.make_plan(cams, vop, state, sparse, self._bucket_open.get(key, 0)), (state if saturation else None)
+        n_open = self._bucket_open.get(key, 0)
+        if n_open and key not in self._bucket_map:         # built once per bucket: the INVISIBLE bits never change
+            self._bucket_map[key] = self.ctx.slot_map(binding.Plan(cams, vop, state, sparse, self._part_max_scale, n_open))
+        return self.make_plan(cams, vop, state, sparse, n_open, self._bucket_map.get(key)), (state if saturation else None)
 
     # ---- one library call per iteration (splx_iteration) -------------------------------------------------------
     def _frontset(self, which):
