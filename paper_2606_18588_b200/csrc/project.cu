@@ -515,10 +515,9 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     const int row = q / NV, c4 = q - row * NV;
     if (row < nrows && s_vis[row]) {
       cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * s_idx[row] + 4 * c4);
-      // (LIST == 2: most rows are fresh -- a Gaussian is seen by few views of an iteration -- so the previous gradient is
-      // not staged at all: the write-back reads it for the rare row that has one, and the block needs half the shared memory)
-      if (ACC && LIST != 2) {
-        cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
+      if (ACC) {
+        if (LIST == 2 && s_fresh[row]) *reinterpret_cast<float4*>(s_old + row * PB_STRIDE + 4 * c4) = make_float4(0.f, 0.f, 0.f, 0.f);
+        else cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
       }
     }
   }
@@ -673,8 +672,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       if (ACC) {
         if (live) {
           const float4 a = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
-          const float4 o = LIST == 2 ? (s_fresh[row] ? make_float4(0.f, 0.f, 0.f, 0.f) : *dst)
-                                     : *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
+          const float4 o = *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
           *dst = make_float4(o.x + a.x, o.y + a.y, o.z + a.z, o.w + a.w);
         } else if (LIST == 2 && s_fresh[row]) {
           *dst = make_float4(0.f, 0.f, 0.f, 0.f);       // coefficients above sh_degree of a freshly stored row
@@ -727,10 +725,9 @@ template <int DEG, int LIST>
 static void launch_pb_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
                            const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
                            const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
-  const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * (LIST == 2 ? 1 : 2);
-  const int per_sm = LIST == 2 ? 5 : 4;       // resident CTAs: 96 registers allow 5, the two staged tiles 4
+  const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * 2;
   const int64_t need = (rt.jprefix[rt.n] + PB_THREADS - 1) / PB_THREADS;
-  const int64_t grid = need < (int64_t)SPLX_SM_COUNT * per_sm ? need : (int64_t)SPLX_SM_COUNT * per_sm;
+  const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 4 ? need : (int64_t)SPLX_SM_COUNT * 4;
   cudaFuncSetAttribute(k_project_bwd<DEG, true, LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   cudaFuncSetAttribute(k_project_bwd<DEG, true, LIST>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   k_project_bwd<DEG, true, LIST><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
