@@ -836,6 +836,10 @@ k_slot_map(const uint8_t* __restrict__ state, const __grid_constant__ PartView p
   if (threadIdx.x == 0) { inv[cap] = nslots; inv[cap + 1] = nslots + 1; }
 }
 
+// Four consecutive keys per thread (two 16-byte loads; the neighbours of the group's ends come from the adjacent lanes,
+// from memory at the warp's ends); only a key that opens or closes a list looks at the tile state and writes -- the
+// one-key-per-thread version read three keys and a state byte for every intersection and sat on their latency
+// (ncu r02c, city_10M: 28 warps waiting on the long scoreboard per issued instruction).
 __global__ void __launch_bounds__(256)
 k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint8_t* __restrict__ tile_state,
               uint32_t* __restrict__ ranges, uint64_t* __restrict__ m_out, uint32_t nslots, bool filtered) {
@@ -845,22 +849,44 @@ k_tile_ranges(const uint64_t* __restrict__ keys, const Counters* cnt, const uint
   // key, when nothing was removed).
   const bool count_kept = filtered && cnt->m_total == m && m > 0;
   if (blockIdx.x == 0 && threadIdx.x == 0 && !count_kept) *m_out = cnt->m_total;
-  for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j < m; j += (uint64_t)gridDim.x * blockDim.x) {
-    const uint32_t s = (uint32_t)(keys[j] >> 32);
-    if (s >= nslots) {           // removed pairs: behind every list
-      if (count_kept && (j == 0 || (uint32_t)(keys[j - 1] >> 32) < nslots)) *m_out = j;
-      // renumbered open slots (splx_plan.open_slots): a key that landed in a slot the caller declared INVISIBLE
-      if (s == nslots + 1) atomicAdd((unsigned long long*)(m_out + 1), 1ull);
-      continue;
+  const int lane = threadIdx.x & 31;
+  const uint64_t groups = (m + 3) / 4;
+  // whole warps stay in the loop together (the shuffles below): the bound is rounded up to a multiple of 32 groups
+  for (uint64_t g0 = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); g0 < groups; g0 += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t j0 = 4 * (g0 + lane);
+    uint32_t s[4];
+    if (j0 + 4 <= m) {
+      const ulonglong2 a = *reinterpret_cast<const ulonglong2*>(keys + j0), c = *reinterpret_cast<const ulonglong2*>(keys + j0 + 2);
+      s[0] = (uint32_t)(a.x >> 32); s[1] = (uint32_t)(a.y >> 32); s[2] = (uint32_t)(c.x >> 32); s[3] = (uint32_t)(c.y >> 32);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) s[q] = j0 + q < m ? (uint32_t)(keys[j0 + q] >> 32) : 0xffffffffu;
     }
-    if (count_kept && j + 1 == m) *m_out = m;
-    if (tile_state && tile_state[s]) {           // a skipped (partition, tile) slot keeps the empty range (0,0)
-      // a NON-EMPTY list dropped on geometric grounds: the caller's regions were not conservative (splx_footprint_margin)
-      if ((tile_state[s] & SPLX_TILE_INVISIBLE) && (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s)) atomicAdd((unsigned long long*)(m_out + 1), 1ull);
-      continue;
+    uint32_t prev = __shfl_up_sync(0xffffffffu, s[3], 1), next = __shfl_down_sync(0xffffffffu, s[0], 1);
+    if (lane == 0) prev = (j0 > 0 && j0 <= m) ? (uint32_t)(keys[j0 - 1] >> 32) : 0xffffffffu;
+    if (lane == 31) next = j0 + 4 < m ? (uint32_t)(keys[j0 + 4] >> 32) : 0xffffffffu;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const uint64_t j = j0 + q;
+      if (j >= m) break;
+      const uint32_t sj = s[q], sp = q ? s[q - 1] : prev, sn = q < 3 ? s[q + 1] : next;
+      const bool first = j == 0 || sp != sj, last = j + 1 == m || sn != sj;
+      if (sj >= nslots) {           // removed pairs: behind every list
+        if (count_kept && (j == 0 || sp < nslots)) *m_out = j;
+        // renumbered open slots (splx_plan.open_slots): a key that landed in a slot the caller declared INVISIBLE
+        if (sj == nslots + 1) atomicAdd((unsigned long long*)(m_out + 1), 1ull);
+        continue;
+      }
+      if (count_kept && j + 1 == m) *m_out = m;
+      if (!first && !last) continue;
+      if (tile_state && tile_state[sj]) {           // a skipped (partition, tile) slot keeps the empty range (0,0)
+        // a NON-EMPTY list dropped on geometric grounds: the caller's regions were not conservative (splx_footprint_margin)
+        if ((tile_state[sj] & SPLX_TILE_INVISIBLE) && first) atomicAdd((unsigned long long*)(m_out + 1), 1ull);
+        continue;
+      }
+      if (first) ranges[2 * (uint64_t)sj] = (uint32_t)j;
+      if (last) ranges[2 * (uint64_t)sj + 1] = (uint32_t)(j + 1);
     }
-    if (j == 0 || (uint32_t)(keys[j - 1] >> 32) != s) ranges[2 * (uint64_t)s] = (uint32_t)j;
-    if (j + 1 == m || (uint32_t)(keys[j + 1] >> 32) != s) ranges[2 * (uint64_t)s + 1] = (uint32_t)(j + 1);
   }
 }
 
@@ -1069,7 +1095,7 @@ int launch_bin_sort(splx_ctx* ctx, const splx_projected* pr, int64_t n, const Pl
     cx.mask = cross->mask; cx.tile_state = plan.tile_state;
     for (int k = 0; k < K; ++k) { cx.zlo[k] = cross->zlo[k]; cx.zhi[k] = cross->zhi[k]; cx.view[k] = plan.pv.v[k]; }
   }
-  const uint64_t emit_blocks = ((uint64_t)n_act + 255) / 256, range_blocks = (out->capacity + 255) / 256;
+  const uint64_t emit_blocks = ((uint64_t)n_act + 255) / 256, range_blocks = (out->capacity / 4 + 255) / 256 + 1;
   const unsigned g_emit = (unsigned)(emit_blocks < 2 * PERSISTENT_CTAS ? emit_blocks : 2 * PERSISTENT_CTAS);
   const uint64_t emit_tiles = (out->capacity + 1023) / 1024;     // output tiles of 1024 keys
   const unsigned g_lb = (unsigned)(emit_tiles < PERSISTENT_CTAS ? emit_tiles : PERSISTENT_CTAS);
