@@ -332,7 +332,7 @@ static int compact_visible(splx_ctx* ctx, const VisibleOp& op, uint32_t* tile_co
 // ---------------------------------------------------------------------- LSD radix sort --
 // "Onesweep" organisation: the digit histograms of ALL passes are counted in one read of the
 // input (a histogram does not depend on the order), then each pass is ONE kernel: a tile ranks
-// its 2048 keys (stable; digit peers found with eight ballots, see digit_peers), chains its per-digit counts to
+// its 2048 keys (stable; digit peers found with MATCH.ANY), chains its per-digit counts to
 // its predecessors by look-back (256 independent chains, one per thread) and scatters.
 // Per item and pass: key+value read once and written once (24 B for 64-bit keys, 16 B for 32-bit).
 
@@ -349,20 +349,6 @@ static PassPlan plan_passes(int begin_bit, int end_bit, int max_bits = 8) {
     shift += p.bits[i];
   }
   return p;
-}
-
-// Lanes of the warp whose 8-bit digit equals this lane's, among the lanes of `vm`: eight ballots.
-// (Constant cost; the hardware MATCH.ANY serialises over the distinct values and the shared-memory
-// atomic unit over the lanes: measured mid-round.)
-__device__ __forceinline__ unsigned digit_peers(uint32_t d, unsigned vm) {
-  unsigned peers = vm;
-#pragma unroll
-  for (int b = 0; b < 8; ++b) {
-    const bool bit = (d >> b) & 1u;
-    const unsigned bal = __ballot_sync(0xffffffffu, bit);
-    peers &= bit ? bal : ~bal;
-  }
-  return peers;
 }
 
 // The LAST pass of the slot sort writes the binning itself: its 32-bit items are (compact slot, position j in the
@@ -388,7 +374,6 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
                                            uint32_t* dbase, const uint32_t* gbase, uint32_t* lbase, KeyT* skey, uint32_t* sval,
                                            uint32_t* sm) {
   constexpr int DPT = NB / RS_THREADS;      // digits per thread: thread x owns digits DPT x .. DPT x + DPT - 1
-  constexpr int MAXB = NB == 256 ? 8 : 9;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
   // warp w owns the contiguous segment [w*256, +256) of the tile; iteration `it` covers 32 consecutive
@@ -408,15 +393,10 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
     const bool valid = FULL || seg + (uint32_t)it * 32 < nv;
     const uint32_t d = (uint32_t)(key[it] >> shift) & mask;
     dg[it] = d;
-    // lanes of the warp with this lane's digit: one ballot per digit bit; (bit - 1) is all ones for a clear bit
-    unsigned peers = FULL ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
-#pragma unroll
-    for (int b = 0; b < MAXB; ++b) {
-      if (b < bits) {            // (uniform) a pass of fewer bits votes on those only
-        const uint32_t bit = (d >> b) & 1u;
-        peers &= __ballot_sync(0xffffffffu, bit) ^ (bit - 1u);
-      }
-    }
+    // lanes of the warp with this lane's digit (the invalid lanes of a ragged tile form a group of their own).  MATCH.ANY
+    // against one vote per digit bit (6 instructions each): neutral while the slot passes had 5-6 bit digits, -7 % of
+    // bin/sort at city scale once the renumbered slots made them 8-bit passes (sort, end of round 2)
+    const unsigned peers = __match_any_sync(0xffffffffu, (FULL || valid) ? d : 0xffffffffu);
     uint32_t old = 0;
     const int leader = __ffs(peers) - 1;               // (an invalid lane: its own digit-0 group among the invalid ones; unused)
     if (valid && lane == leader) { old = whist[warp][d]; whist[warp][d] = old + __popc(peers); }
