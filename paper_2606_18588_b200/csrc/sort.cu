@@ -5,11 +5,13 @@
 // of the (key, Gaussian index) pairs emitted in Gaussian-index order.
 //
 // B200 design: the full sort is split so that the wide keys are moved as little as possible.
-//   1. compact the visible Gaussians in index order            (4 B read, 8 B written / visible)
+//   1. compact the visible Gaussians in index order: count -> scan -> scatter (8 B read per participating Gaussian,
+//      12 B written per visible one)
 //   2. stable LSD radix sort of (depth bits, index), 4 x 8 bits (over N_visible, not over M)
-//   3. exclusive scan of tiles_touched in that depth order, emit the 64-bit keys in that order
-//   4. stable LSD radix sort on the SLOT bits only (ceil(log2(K*tiles)) bits, 2-3 passes)
-//   5. tile ranges from the sorted keys
+//   3. exclusive scan of tiles_touched in that depth order, emit (sort slot, depth-order position) pairs in that order
+//   4. stable LSD radix sort on the sort-slot bits only (the slots of the participating partitions, or -- splx_plan.open_slots --
+//      of their open slots: 2-3 passes); the last pass writes the 64-bit keys and the values
+//   5. tile ranges from the sorted keys, slot order by descending list length
 // Step 2 + step 4 give exactly the stable sort on the whole key: within a slot the entries
 // keep the order of step 2 = (depth bits, index).  No host synchronisation: the counts
 // (N_visible, M) stay on the device and every grid is sized from the caller's capacities.
