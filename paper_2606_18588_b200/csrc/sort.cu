@@ -64,45 +64,30 @@ __device__ __forceinline__ void st_status(uint64_t* p, uint64_t v) {
 // exclusive prefix of tile t (t > 0) given its own total: publish, look back, publish again.
 // The walk reads W predecessors per round trip (independent loads), consumes them nearest first
 // and stops at the first PREFIX; a predecessor that has published nothing yet ends the round.
-// The walk is 40 % of the instructions of a radix pass (source-level ncu, end of round 2: ~6 rounds per tile and
-// digit), in a kernel bound by instruction issue, so a round is written for few instructions: STRIDE is a compile-time
-// constant (the W loads take immediate offsets from one pointer), the bounds test is hoisted out of the common case
-// (at least W predecessors), and the W flags are folded into two bit masks -- how many of the nearest words are
-// published, where the first PREFIX stands -- instead of a chain of dependent tests per word.
-template <int W, int STRIDE>
-__device__ __forceinline__ uint64_t lookback(uint64_t* status, uint32_t t, uint64_t total) {
-  st_status(status + (uint64_t)t * STRIDE, ST_AGG | total);
+template <int W>
+__device__ __forceinline__ uint64_t lookback(uint64_t* status, uint32_t t, uint32_t stride, uint64_t total) {
+  st_status(status + (uint64_t)t * stride, ST_AGG | total);
   uint64_t excl = 0;
   int64_t p = (int64_t)t - 1;
   while (p >= 0) {
-    const uint64_t* q = status + (uint64_t)p * STRIDE;
     uint64_t v[W];
-    if (p >= W - 1) {
 #pragma unroll
-      for (int i = 0; i < W; ++i) v[i] = ld_status(q - (int64_t)i * STRIDE);
-    } else {
-#pragma unroll
-      for (int i = 0; i < W; ++i) v[i] = (p - i >= 0) ? ld_status(q - (int64_t)i * STRIDE) : ST_PREFIX;
-    }
-    unsigned pub = 0, pre = 0;            // bit i: word i is published / holds an inclusive prefix
+    for (int i = 0; i < W; ++i) v[i] = (p - i >= 0) ? ld_status(status + (uint64_t)(p - i) * stride) : ST_PREFIX;
+    bool done = false;
+    int used = 0;
 #pragma unroll
     for (int i = 0; i < W; ++i) {
-      const uint32_t f = (uint32_t)(v[i] >> 62);
-      pub |= (f != 0u ? 1u : 0u) << i;
-      pre |= (f == 2u ? 1u : 0u) << i;
+      if (!done && used == i && (v[i] & ST_MASK) != 0) {
+        excl += v[i] & ~ST_MASK;
+        ++used;
+        if ((v[i] & ST_MASK) == ST_PREFIX) done = true;
+      }
     }
-    const int n_pub = __ffs((int)~pub) - 1;                 // nearest words published without a gap (W if all are)
-    const int first_pre = pre ? __ffs((int)pre) - 1 : W;
-    const bool done = first_pre < n_pub;
-    const int take = done ? first_pre + 1 : n_pub;
-#pragma unroll
-    for (int i = 0; i < W; ++i)
-      if (i < take) excl += v[i] & ~ST_MASK;
     if (done) break;
-    p -= take;
-    if (take == 0) __nanosleep(20);
+    p -= used;
+    if (used == 0) __nanosleep(20);
   }
-  st_status(status + (uint64_t)t * STRIDE, ST_PREFIX | (excl + total));
+  st_status(status + (uint64_t)t * stride, ST_PREFIX | (excl + total));
   return excl;
 }
 
@@ -165,7 +150,7 @@ k_scan(const __grid_constant__ Op op, const uint64_t* n_ptr, uint64_t* status, u
     if (threadIdx.x == 0) {
       uint64_t excl = 0;
       if (t == 0) st_status(status, ST_PREFIX | (uint64_t)total);
-      else excl = lookback<16, 1>(status, t, total);
+      else excl = lookback<16>(status, t, 1, total);
       s_excl = excl;
       if (t + 1 == ntiles) {
         const uint64_t grand = excl + total;
@@ -456,7 +441,7 @@ __device__ __forceinline__ void radix_tile(const KeyT* __restrict__ kin, const u
     uint64_t excl = 0;
     uint64_t* st = status + d;
     if (t == 0) st_status(st, ST_PREFIX | (uint64_t)run[q]);
-    else excl = lookback<8, NB>(st, t, run[q]);
+    else excl = lookback<8>(st, t, NB, run[q]);
     dbase[d] = gbase[d] + (uint32_t)excl - lbase[d];      // global position = dbase[d] + position in the tile
   }
   __syncthreads();
