@@ -193,6 +193,7 @@ __device__ __forceinline__ bool project_one(const splx_gaussians& g, int64_t i, 
 #pragma unroll
   for (int k = 0; k < 3; ++k) gin.ls[k] = g.log_scale[3 * i + k];
   gin.q = *reinterpret_cast<const float4*>(g.quat + 4 * i);
+  const float logit = g.opacity_logit[i];       // requested with the others: one memory latency, not a second one behind the chain
   if (!geometry(gin, cam, cfg.dilation, G)) return false;
   const float mid = 0.5f * (G.a + G.c);
   const float hd = 0.5f * (G.a - G.c);
@@ -207,7 +208,7 @@ __device__ __forceinline__ bool project_one(const splx_gaussians& g, int64_t i, 
   if (tt <= 0) return false;
   float4* bl = reinterpret_cast<float4*>(out.blend + SPLX_BLEND_STRIDE * i);
   const float idet = 1.0f / G.det;
-  const float op = 1.0f / (1.0f + expf(-g.opacity_logit[i]));
+  const float op = 1.0f / (1.0f + expf(-logit));
   *reinterpret_cast<float2*>(out.means2d + 2 * i) = make_float2(u, v);
   out.depth[i] = G.p[2];
   const float cA = G.c * idet, cB = -G.b * idet, cC = G.a * idet;
