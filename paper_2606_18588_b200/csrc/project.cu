@@ -516,9 +516,9 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     const int row = q / NV, c4 = q - row * NV;
     if (row < nrows && s_vis[row]) {
       cp_async16(s_sh + row * PB_STRIDE + 4 * c4, g.sh + 48 * s_idx[row] + 4 * c4);
-      if (ACC) {
-        if (LIST == 2 && s_fresh[row]) *reinterpret_cast<float4*>(s_old + row * PB_STRIDE + 4 * c4) = make_float4(0.f, 0.f, 0.f, 0.f);
-        else cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
+      // (LIST: the previous gradient is never read: the write-back ADDS in memory with vector reductions, see below)
+      if (ACC && !LIST) {
+        cp_async16(s_old + row * PB_STRIDE + 4 * c4, out.sh + 48 * s_idx[row] + 4 * c4);
       }
     }
   }
@@ -651,10 +651,15 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     float4* oq = reinterpret_cast<float4*>(out.quat + 4 * i);
     if (ACC) {
       if (vis) {
-        float4 cur = fresh ? make_float4(0.f, 0.f, 0.f, 0.f) : *oq;
-        cur.x += dq.x; cur.y += dq.y; cur.z += dq.z; cur.w += dq.w;
-        *oq = cur;
-        out.opacity_logit[i] = (fresh ? 0.f : out.opacity_logit[i]) + dlogit;
+        if (LIST && !fresh) {       // a list holds a Gaussian once: the reduction is the plain sum old + new, without reading old here
+          atomicAdd(oq, dq);
+          atomicAdd(out.opacity_logit + i, dlogit);
+        } else {
+          float4 cur = fresh ? make_float4(0.f, 0.f, 0.f, 0.f) : *oq;
+          cur.x += dq.x; cur.y += dq.y; cur.z += dq.z; cur.w += dq.w;
+          *oq = cur;
+          out.opacity_logit[i] = (fresh ? 0.f : out.opacity_logit[i]) + dlogit;
+        }
       }
     } else {
       *oq = dq;
@@ -673,8 +678,15 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
       if (ACC) {
         if (live) {
           const float4 a = *reinterpret_cast<const float4*>(s_sh + row * PB_STRIDE + 4 * c4);
-          const float4 o = *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
-          *dst = make_float4(o.x + a.x, o.y + a.y, o.z + a.z, o.w + a.w);
+          if (LIST) {
+            // red.global.add.v4.f32 (sm_90+): the sum is formed in L2, nothing waits for the old value and no tile of
+            // old gradients is staged -- half the shared memory, 5 resident CTAs instead of 4
+            if (LIST == 2 && s_fresh[row]) *dst = make_float4(0.f + a.x, 0.f + a.y, 0.f + a.z, 0.f + a.w);
+            else atomicAdd(dst, a);
+          } else {
+            const float4 o = *reinterpret_cast<const float4*>(s_old + row * PB_STRIDE + 4 * c4);
+            *dst = make_float4(o.x + a.x, o.y + a.y, o.z + a.z, o.w + a.w);
+          }
         } else if (LIST == 2 && s_fresh[row]) {
           *dst = make_float4(0.f, 0.f, 0.f, 0.f);       // coefficients above sh_degree of a freshly stored row
         }
@@ -700,7 +712,9 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   } else if (i < run_end) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      if (ACC) {
+      if (ACC && LIST && !fresh) {
+        if (vis) { atomicAdd(out.mean + 3 * i + k, dmu[k]); atomicAdd(out.log_scale + 3 * i + k, dls[k]); }
+      } else if (ACC) {
         out.mean[3 * i + k] = (fresh ? 0.f : out.mean[3 * i + k]) + dmu[k];
         out.log_scale[3 * i + k] = (fresh ? 0.f : out.log_scale[3 * i + k]) + dls[k];
       }
@@ -726,9 +740,9 @@ template <int DEG, int LIST>
 static void launch_pb_list(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const RunTable& rt,
                            const splx_projected* pr, float* g2d, int clear_g2d, const splx_gaussian_grads* grads,
                            const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
-  const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float) * 2;
+  const size_t smem = (size_t)PB_THREADS * PB_STRIDE * sizeof(float);     // the SH tile only
   const int64_t need = (rt.jprefix[rt.n] + PB_THREADS - 1) / PB_THREADS;
-  const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 4 ? need : (int64_t)SPLX_SM_COUNT * 4;
+  const int64_t grid = need < (int64_t)SPLX_SM_COUNT * 5 ? need : (int64_t)SPLX_SM_COUNT * 5;     // 96 registers: 5 resident CTAs
   cudaFuncSetAttribute(k_project_bwd<DEG, true, LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   cudaFuncSetAttribute(k_project_bwd<DEG, true, LIST>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
   k_project_bwd<DEG, true, LIST><<<(unsigned)grid, PB_THREADS, smem, ctx->stream>>>(
