@@ -495,7 +495,8 @@ def run_ours(args):
             else:
                 lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
                 c.project_backward_list_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, lst, cnt,
-                                             clear_g2d=True, touched=tr._touched if flags else None)
+                                             clear_g2d=True, touched=tr._touched if flags else None,
+                                             skip_zero=flags and not tr.sparse_adam)
             e[6].record()
         tr.adam_step(B, flagged=flags)
         ev[-1][7].record()
@@ -512,6 +513,8 @@ def run_ours(args):
     for s in range(n_staged):
         staged_iteration(evs[s])
     torch.cuda.synchronize()
+    if flags and not tr.sparse_adam:
+        counts["rows_with_gradient"] = int(tr._touched.sum().item())
     stage_ms = {n: 0.0 for n in STAGES}
     for s in range(n_staged):
         for gi in range(len(plans)):
@@ -592,7 +595,11 @@ def run_ours(args):
         project=nv * 285 + (npart - nv) * 93,
         bin_sort=4 * npart + 12 * nv + 4 * 16 * nv + 4 * nv + (12 + 24 * n_slot_pass + 8) * M + 8 * K * ntiles * len(plans),
         compose=(20 + 16) * 256 * counts["live_slots"] + (12 + 12 + 4) * W * H * B,
-        project_backward=(236 * tr.n + 272 * vis0 + 740 * (nv - vis0)) if first_overwrite else 740 * nv,
+        # flag-tracked rows: every listed Gaussian costs its list entry, radius and 2-D gradient row (56 B); only a row with a
+        # non-zero 2-D gradient goes through the kernel (740 B).  rows_with_gradient = flagged Gaussians after the iteration: a
+        # LOWER bound of the rows processed (a Gaussian seen by two buckets counts once)
+        project_backward=(236 * tr.n + 272 * vis0 + 740 * (nv - vis0)) if first_overwrite else
+                         (56 * nv + 740 * counts["rows_with_gradient"] if counts.get("rows_with_gradient") else 740 * nv),
         # flagged gradient rows: 24 B per parameter (param, m, v read + written) + the gradient of the touched rows only
         adam=(24 * 59 * tr.n + tr.n + 4 * 59 * min(nv, tr.n)) if flags else 28 * 59 * tr.n)
     flops_fwd = counts["pairs_walked_fwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_FWD

@@ -231,6 +231,11 @@ int splx_raster_backward(splx_ctx *ctx, const splx_projected *proj, const splx_b
  * gradient buffer and reads none.  All five grads arrays must be 16-byte aligned. */
 #define SPLX_PB_CLEAR_G2D 1
 #define SPLX_PB_OVERWRITE 2
+#define SPLX_PB_SKIP_ZERO 4   /* splx_project_backward_list_plan with `touched` only: a listed Gaussian whose g2d row is all
+                                 zero (visible, but no pixel blended it) has a zero gradient -- the kernel is linear in that
+                                 row -- and is left out like a culled one: no flag set, nothing written.  Same gradients under
+                                 the flag semantics (an unflagged row counts as zero); on a city view about half of the visible
+                                 Gaussians are hidden behind opaque surfaces */
 int splx_project_backward(splx_ctx *ctx, const splx_gaussians *g, const splx_camera *cam,
                           int sh_degree, const splx_projected *proj, float *g2d, int flags,
                           const splx_gaussian_grads *grads);
@@ -440,7 +445,7 @@ int splx_bin_sort_filtered_plan(splx_ctx *ctx, const splx_projected *proj, int64
 /* splx_project_backward_plan in += mode over the visible Gaussians only: the rows processed are the entries of
  * `visible` (device uint32[*num_visible], *num_visible a device uint64) instead of every Gaussian of the
  * participating partitions -- same result (a culled Gaussian has no gradient), work proportional to the visible
- * count.  flags: SPLX_PB_CLEAR_G2D or 0. */
+ * count.  flags: SPLX_PB_CLEAR_G2D, SPLX_PB_SKIP_ZERO (needs `touched`) or 0. */
 int splx_project_backward_list_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                                     const splx_plan *plan, int sh_degree, const splx_projected *proj,
                                     float *g2d, int flags, const splx_gaussian_grads *grads,
@@ -529,6 +534,9 @@ typedef struct {
 } splx_adam_cfg;
 
 #define SPLX_ITER_HOST 1   /* targets[v] / images_out[v] / loss_out / m_out are pinned HOST pointers */
+#define SPLX_ITER_KEEP_ZERO_ROWS 8     /* with trainset.touched: do NOT pass SPLX_PB_SKIP_ZERO to the projection backward, i.e.
+                                          flag every visible Gaussian, also one whose gradient is exactly zero (the row set of
+                                          the visible-only optimiser option) */
 #define SPLX_ITER_FUSED_PROJECTION 4   /* a1 as ONE kernel (splx_project_plan: the colour of every visible Gaussian inside the
                                           projection).  Default: the geometry half (splx_project_geometry_plan), the binning, then
                                           the colour of the binning's list of visible Gaussians (splx_project_colour_list_plan) --

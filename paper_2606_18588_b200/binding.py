@@ -20,7 +20,7 @@ G2D_STRIDE = 12
 BLEND_STRIDE = 12
 TILE = 16
 MAX_K = 64
-PB_CLEAR_G2D, PB_OVERWRITE = 1, 2
+PB_CLEAR_G2D, PB_OVERWRITE, PB_SKIP_ZERO = 1, 2, 4
 OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA = 0, -1, -2, -3, -4
 
 EXPORTS = [
@@ -119,6 +119,7 @@ class IterOptsS(C.Structure):
 
 ITER_HOST = 1
 ITER_FUSED_PROJECTION = 4
+ITER_KEEP_ZERO_ROWS = 8
 
 
 def lib():
@@ -603,10 +604,10 @@ class Context:
         return lst.value, cnt.value
 
     def project_backward_list_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
-                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False, touched=None):
+                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False, touched=None, skip_zero=False):
         g, gg, ps = gaussians_struct(params), gaussians_struct(grads), proj.struct()
         self._check(lib().splx_project_backward_list_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
-                                                          sh_degree, C.byref(ps), _ptr(g2d), PB_CLEAR_G2D if clear_g2d else 0,
+                                                          sh_degree, C.byref(ps), _ptr(g2d), (PB_CLEAR_G2D if clear_g2d else 0) | (PB_SKIP_ZERO if skip_zero else 0),
                                                           C.byref(gg), C.c_void_p(visible_ptr), C.c_void_p(count_ptr),
                                                           _ptr(touched)))
 
@@ -639,14 +640,15 @@ class Context:
                                                       float(B if scale is None else scale), _ptr(g_image), _ptr(loss_sum)))
 
     def iteration(self, trainset: "TrainsetS", buckets, n_views, targets, images_out=None, loss_out=None, m_out=None,
-                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None, fused_projection=False):
+                  host=False, sat_eps=1e-4, lambda_dssim=0.0, adam: "AdamCfgS" = None, fused_projection=False, keep_zero_rows=False):
         """splx_iteration.  buckets: ctypes array of BucketS; targets / images_out: lists of raw pointers (ints; device
         pointers, or pinned host pointers with host=True); loss_out / m_out: raw pinned host pointers or None."""
         tg = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) for x in targets])
         io = None
         if images_out is not None:
             io = (C.c_void_p * n_views)(*[C.c_void_p(int(x)) if x else None for x in images_out])
-        opts = IterOptsS((ITER_HOST if host else 0) | (ITER_FUSED_PROJECTION if fused_projection else 0), float(sat_eps),
+        opts = IterOptsS((ITER_HOST if host else 0) | (ITER_FUSED_PROJECTION if fused_projection else 0) |
+                         (ITER_KEEP_ZERO_ROWS if keep_zero_rows else 0), float(sat_eps),
                          float(lambda_dssim))
         self._check(lib().splx_iteration(self._h, C.byref(trainset), len(buckets), buckets, int(n_views), tg, io,
                                          C.c_void_p(loss_out) if loss_out else None, C.c_void_p(m_out) if m_out else None,

@@ -433,7 +433,8 @@ int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int 
       grads->n != g->n)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: null/misaligned argument");
   if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: sh_degree %d not in [0,3]", sh_degree);
-  if (flags & ~SPLX_PB_CLEAR_G2D) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: unknown flags %d", flags);
+  if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_SKIP_ZERO) || ((flags & SPLX_PB_SKIP_ZERO) && !touched))
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: unknown flags %d, or SPLX_PB_SKIP_ZERO without touched", flags);
   PlanDev pd;
   int rc;
   if ((rc = make_plan_dev(ctx, "splx_project_backward_list", K, plan, &pd))) return rc;

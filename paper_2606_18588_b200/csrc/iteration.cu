@@ -71,7 +71,7 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
   if (!ctx) return SPLX_ERR_INVALID_ARG;
   if (!ts || !buckets || !targets || !opts || n_buckets < 1 || n_views < 1)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: null argument or empty iteration");
-  if (opts->flags & ~(SPLX_ITER_HOST | SPLX_ITER_FUSED_PROJECTION)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: unknown flags %d", opts->flags);
+  if (opts->flags & ~(SPLX_ITER_HOST | SPLX_ITER_FUSED_PROJECTION | SPLX_ITER_KEEP_ZERO_ROWS)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: unknown flags %d", opts->flags);
   const bool host = (opts->flags & SPLX_ITER_HOST) != 0;
   if (!host && (images_out || loss_out)) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_iteration: images_out / loss_out need SPLX_ITER_HOST");
   const int64_t n = ts->params.n;
@@ -198,8 +198,10 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
     const uint64_t* nvis = nullptr;
     if (ts->touched || gi > 0) {
       if ((r = splx_bin_sort_visible(fs.ws, n, fs.bins.capacity, K, &plan->cams[0], &vlist, &nvis))) SPLX_FAIL(ctx, r, "splx_iteration: visible list");
+      const bool skip_zero = ts->touched && !(opts->flags & SPLX_ITER_KEEP_ZERO_ROWS) && !(adam && adam->sparse);
       return splx_project_backward_list_plan(ctx, &g, K, ts->part_offsets, plan, ts->sh_degree, &fs.proj, ts->g2d,
-                                             SPLX_PB_CLEAR_G2D, &ts->grads, vlist, nvis, ts->touched);
+                                             SPLX_PB_CLEAR_G2D | (skip_zero ? SPLX_PB_SKIP_ZERO : 0), &ts->grads, vlist, nvis,
+                                             ts->touched);
     }
     return splx_project_backward_plan(ctx, &g, K, ts->part_offsets, plan, ts->sh_degree, &fs.proj, ts->g2d,
                                       SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE, &ts->grads);

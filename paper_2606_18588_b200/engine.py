@@ -83,6 +83,10 @@ class Trainer:
         self.flagged_grads = True
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
         self.pipeline_buckets = True
+        #: flag-tracked gradient rows: a visible Gaussian that no pixel blended has a zero gradient and is left out of the
+        #: projection backward like a culled one (SPLX_PB_SKIP_ZERO; same result, an unflagged row counts as zero).  True keeps
+        #: them (every visible Gaussian gets its flag); the visible-only optimiser option always keeps them
+        self.keep_zero_rows = False
         #: a1 inside splx_iteration: None = fused (one kernel) when every partition takes part in every bucket -- then most
         #: Gaussians are visible (aerial views) --, else geometry -> binning -> colour of the visible list (city views, where
         #: most participating Gaussians are culled); True / False force one or the other.  Same results bit for bit
@@ -430,7 +434,8 @@ class Trainer:
         self._plan = plans[-1][0]
         self.ctx.iteration(ts, bk, n_views, targets, images_out, loss_out, self._m_host.data_ptr(), host=host,
                            sat_eps=0.0 if sat_eps is None else sat_eps, lambda_dssim=self.lambda_dssim, adam=cfg,
-                           fused_projection=self.use_fused_projection([p for p, _ in plans]))
+                           fused_projection=self.use_fused_projection([p for p, _ in plans]),
+                           keep_zero_rows=self.sparse_adam or self.keep_zero_rows)   # (Adam may run outside the call)
         self._m_buckets = len(plans)
         return ts, bk
 

@@ -697,6 +697,38 @@ def test_flag_tracked_gradient_rows_equal_the_plain_buffer(blocks):
             assert close.float().mean().item() >= 0.999, key
 
 
+def test_rows_without_a_2d_gradient_are_skipped_exactly(city):
+    """SPLX_PB_SKIP_ZERO: a visible Gaussian that no pixel blended (hidden behind opaque surfaces) has an all-zero 2-D
+    gradient row, hence a zero gradient: the flag-tracked projection backward leaves it out like a culled one.  Against
+    the run that keeps such rows: the skipped rows are exactly the flagged rows whose gradient is zero there, every other
+    flagged row has the same gradient, and the dense Adam steps agree."""
+    sc = city
+    ids = list(range(len(sc.cameras)))
+    targets = torch.from_numpy(np.stack(sc.targets)).cuda()
+    a, b = _trainer_conservative(sc), _trainer_conservative(sc)
+    b.keep_zero_rows = True
+    for tr in (a, b):
+        tr._use_flags = lambda plan: True
+        tr.flat["grad"].fill_(float("nan"))
+    for it in range(2):
+        a.iteration_views(ids, sc.cameras, targets, saturation=False)
+        b.iteration_views(ids, sc.cameras, targets, saturation=False)
+        torch.cuda.synchronize()
+    ta, tb = a._touched.bool(), b._touched.bool()
+    assert not (ta & ~tb).any()                       # nothing flagged that the keeping run does not flag
+    skipped = tb & ~ta
+    assert int(skipped.sum()) > 0, "the opaque scene hides no visible Gaussian?"
+    for key in scenes.PARAM_KEYS:
+        w = scenes.PARAM_WIDTH[key]
+        ga, gb = a.grads[key].view(-1, w), b.grads[key].view(-1, w)
+        assert not gb[skipped].any(), key             # exactly zero where the row was skipped
+        assert torch.isfinite(ga[ta]).all()
+        assert float((ga[ta] - gb[ta]).abs().max()) <= 1e-4 * float(gb[tb].abs().max()) + 1e-12, key
+        for x, y in ((a.params[key], b.params[key]), (a.m[key], b.m[key]), (a.v[key], b.v[key])):
+            close = torch.isclose(x, y, rtol=1e-3, atol=2e-6)
+            assert close.float().mean().item() >= 0.999, key
+
+
 def test_reach_test_on_the_mean_culls_nothing_visible(city, blocks):
     """splx_plan.max_scale: the projection tests a Gaussian's mean against the half spaces outside which nothing of
     that scale reaches the image (reading s21) before it reads scale and rotation.  Same radius / tiles_touched for
