@@ -493,10 +493,12 @@ def run_ours(args):
             if gi == 0 and not flags:
                 c.project_backward_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True, overwrite=True)
             else:
-                lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
+                if flags and not tr.sparse_adam and not tr.keep_zero_rows:     # only the Gaussians that received a 2-D gradient
+                    lst, cnt = c.bin_sort_gradient_rows(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0], g2d)
+                else:
+                    lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])
                 c.project_backward_list_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, lst, cnt,
-                                             clear_g2d=True, touched=tr._touched if flags else None,
-                                             skip_zero=flags and not tr.sparse_adam)
+                                             clear_g2d=True, touched=tr._touched if flags else None)
             e[6].record()
         tr.adam_step(B, flagged=flags)
         ev[-1][7].record()
@@ -513,7 +515,7 @@ def run_ours(args):
     for s in range(n_staged):
         staged_iteration(evs[s])
     torch.cuda.synchronize()
-    if flags and not tr.sparse_adam:
+    if flags and not tr.sparse_adam and not tr.keep_zero_rows:
         counts["rows_with_gradient"] = int(tr._touched.sum().item())
     stage_ms = {n: 0.0 for n in STAGES}
     for s in range(n_staged):

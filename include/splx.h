@@ -231,11 +231,6 @@ int splx_raster_backward(splx_ctx *ctx, const splx_projected *proj, const splx_b
  * gradient buffer and reads none.  All five grads arrays must be 16-byte aligned. */
 #define SPLX_PB_CLEAR_G2D 1
 #define SPLX_PB_OVERWRITE 2
-#define SPLX_PB_SKIP_ZERO 4   /* splx_project_backward_list_plan with `touched` only: a listed Gaussian whose g2d row is all
-                                 zero (visible, but no pixel blended it) has a zero gradient -- the kernel is linear in that
-                                 row -- and is left out like a culled one: no flag set, nothing written.  Same gradients under
-                                 the flag semantics (an unflagged row counts as zero); on a city view about half of the visible
-                                 Gaussians are hidden behind opaque surfaces */
 int splx_project_backward(splx_ctx *ctx, const splx_gaussians *g, const splx_camera *cam,
                           int sh_degree, const splx_projected *proj, float *g2d, int flags,
                           const splx_gaussian_grads *grads);
@@ -442,10 +437,18 @@ int splx_cross_depth_ranges(int K, const float *aabb_lo, const float *aabb_hi, c
 int splx_bin_sort_filtered_plan(splx_ctx *ctx, const splx_projected *proj, int64_t n, int K,
                                 const int64_t *part_offsets, const splx_plan *plan, const uint64_t *cross_mask,
                                 const float *part_depth_range, const splx_binning *out, void *ws, size_t ws_bytes);
+/* The entries of that list whose g2d row ([n, SPLX_G2D_STRIDE], as splx_raster_backward* leaves it) is not all zero,
+ * compacted into scratch of the same workspace (valid until the next splx_bin_sort* on it): *rows = DEVICE uint32 list (in no
+ * particular order), *num_rows = its DEVICE uint64 count.  A visible Gaussian that no pixel blended -- hidden behind opaque
+ * surfaces: about half of the visible ones on a city view -- has an all-zero row and, the projection backward being linear
+ * in it, a zero gradient: splx_project_backward_list_plan over (*rows, *num_rows) WITH `touched` gives the same gradients
+ * under the flag semantics (an unflagged row counts as zero) for half the work.  One launch on the context's stream. */
+int splx_bin_sort_gradient_rows(splx_ctx *ctx, void *ws, int64_t n, uint64_t capacity, int K, const splx_camera *cam,
+                                const float *g2d, const uint32_t **rows, const uint64_t **num_rows);
 /* splx_project_backward_plan in += mode over the visible Gaussians only: the rows processed are the entries of
  * `visible` (device uint32[*num_visible], *num_visible a device uint64) instead of every Gaussian of the
  * participating partitions -- same result (a culled Gaussian has no gradient), work proportional to the visible
- * count.  flags: SPLX_PB_CLEAR_G2D, SPLX_PB_SKIP_ZERO (needs `touched`) or 0. */
+ * count.  flags: SPLX_PB_CLEAR_G2D or 0. */
 int splx_project_backward_list_plan(splx_ctx *ctx, const splx_gaussians *g, int K, const int64_t *part_offsets,
                                     const splx_plan *plan, int sh_degree, const splx_projected *proj,
                                     float *g2d, int flags, const splx_gaussian_grads *grads,
@@ -534,9 +537,9 @@ typedef struct {
 } splx_adam_cfg;
 
 #define SPLX_ITER_HOST 1   /* targets[v] / images_out[v] / loss_out / m_out are pinned HOST pointers */
-#define SPLX_ITER_KEEP_ZERO_ROWS 8     /* with trainset.touched: do NOT pass SPLX_PB_SKIP_ZERO to the projection backward, i.e.
-                                          flag every visible Gaussian, also one whose gradient is exactly zero (the row set of
-                                          the visible-only optimiser option) */
+#define SPLX_ITER_KEEP_ZERO_ROWS 8     /* with trainset.touched: the projection backward runs over EVERY visible Gaussian and flags
+                                          it, also one whose gradient is exactly zero (the row set of the visible-only optimiser
+                                          option).  Default: over splx_bin_sort_gradient_rows' list */
 #define SPLX_ITER_FUSED_PROJECTION 4   /* a1 as ONE kernel (splx_project_plan: the colour of every visible Gaussian inside the
                                           projection).  Default: the geometry half (splx_project_geometry_plan), the binning, then
                                           the colour of the binning's list of visible Gaussians (splx_project_colour_list_plan) --

@@ -20,7 +20,7 @@ G2D_STRIDE = 12
 BLEND_STRIDE = 12
 TILE = 16
 MAX_K = 64
-PB_CLEAR_G2D, PB_OVERWRITE, PB_SKIP_ZERO = 1, 2, 4
+PB_CLEAR_G2D, PB_OVERWRITE = 1, 2
 OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA = 0, -1, -2, -3, -4
 
 EXPORTS = [
@@ -35,7 +35,7 @@ EXPORTS = [
     "splx_render_partial_plan", "splx_compose_plan", "splx_compose_backward_plan",
     "splx_raster_backward_plan", "splx_project_backward_plan", "splx_backward_plan",
     "splx_compose_l1_backward_plan",
-    "splx_bin_sort_visible", "splx_project_backward_list_plan", "splx_adam_sparse",
+    "splx_bin_sort_visible", "splx_bin_sort_gradient_rows", "splx_project_backward_list_plan", "splx_adam_sparse",
     "splx_cross_sets", "splx_cross_depth_ranges", "splx_bin_sort_filtered_plan",
     "splx_adam_groups_flagged", "splx_dssim_ws_floats", "splx_dssim_loss_grad", "splx_dssim_loss_grad_static", "splx_iteration", "splx_microbench",
 ]
@@ -193,6 +193,7 @@ def lib():
         L.splx_backward_plan.argtypes = [vp, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp, vp,
                                          C.c_size_t, C.c_int]
         L.splx_bin_sort_visible.argtypes = [vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp]
+        L.splx_bin_sort_gradient_rows.argtypes = [vp, vp, C.c_int64, C.c_uint64, C.c_int, vp, vp, vp, vp]
         L.splx_project_backward_list_plan.argtypes = [vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, vp, vp, vp, vp]
         L.splx_adam_sparse.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.c_float, C.c_float, C.c_float, C.c_int, C.c_float]
         L.splx_cross_sets.argtypes = [vp, vp, C.c_int, vp, vp, vp, C.c_float, vp]
@@ -603,11 +604,18 @@ class Context:
             raise SplxError(rc, "splx_bin_sort_visible: invalid argument")
         return lst.value, cnt.value
 
+    def bin_sort_gradient_rows(self, ws: torch.Tensor, n, capacity, K, cam, g2d):
+        """splx_bin_sort_gradient_rows: device pointers (ints) of the list of Gaussians with a non-zero g2d row and of its count."""
+        cs = camera_struct(cam)
+        lst, cnt = C.c_void_p(), C.c_void_p()
+        self._check(lib().splx_bin_sort_gradient_rows(self._h, _ptr(ws), n, capacity, K, C.byref(cs), _ptr(g2d), C.byref(lst), C.byref(cnt)))
+        return lst.value, cnt.value
+
     def project_backward_list_plan(self, params: dict, part_offsets, plan: Plan, sh_degree, proj: Projected, g2d,
-                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False, touched=None, skip_zero=False):
+                                   grads: dict, visible_ptr: int, count_ptr: int, clear_g2d=False, touched=None):
         g, gg, ps = gaussians_struct(params), gaussians_struct(grads), proj.struct()
         self._check(lib().splx_project_backward_list_plan(self._h, C.byref(g), plan.K, self._offs(part_offsets), plan.ref(),
-                                                          sh_degree, C.byref(ps), _ptr(g2d), (PB_CLEAR_G2D if clear_g2d else 0) | (PB_SKIP_ZERO if skip_zero else 0),
+                                                          sh_degree, C.byref(ps), _ptr(g2d), PB_CLEAR_G2D if clear_g2d else 0,
                                                           C.byref(gg), C.c_void_p(visible_ptr), C.c_void_p(count_ptr),
                                                           _ptr(touched)))
 

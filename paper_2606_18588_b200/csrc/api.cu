@@ -419,6 +419,17 @@ int splx_bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, c
   return bin_sort_visible(ws, n, capacity, K, TX, TY, visible, num_visible);
 }
 
+int splx_bin_sort_gradient_rows(splx_ctx* ctx, void* ws, int64_t n, uint64_t capacity, int K, const splx_camera* cam,
+                                const float* g2d, const uint32_t** rows, const uint64_t** num_rows) {
+  if (!ctx) return SPLX_ERR_INVALID_ARG;
+  if (!ws || n < 0 || K < 1 || K > SPLX_MAX_K || !cam_ok(cam) || !g2d || !aligned16(g2d) || !rows || !num_rows)
+    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_bin_sort_gradient_rows: null/misaligned argument");
+  *rows = nullptr; *num_rows = nullptr;
+  if (n == 0) return SPLX_OK;
+  const int TX = (cam->width + SPLX_TILE - 1) / SPLX_TILE, TY = (cam->height + SPLX_TILE - 1) / SPLX_TILE;
+  return launch_gradient_rows(ctx, ws, n, capacity, K, TX, TY, g2d, rows, num_rows);
+}
+
 int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int K, const int64_t* part_offsets,
                                     const splx_plan* plan, int sh_degree, const splx_projected* proj, float* g2d, int flags,
                                     const splx_gaussian_grads* grads, const uint32_t* visible, const uint64_t* num_visible,
@@ -433,8 +444,7 @@ int splx_project_backward_list_plan(splx_ctx* ctx, const splx_gaussians* g, int 
       grads->n != g->n)
     SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: null/misaligned argument");
   if (sh_degree < 0 || sh_degree > 3) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: sh_degree %d not in [0,3]", sh_degree);
-  if (flags & ~(SPLX_PB_CLEAR_G2D | SPLX_PB_SKIP_ZERO) || ((flags & SPLX_PB_SKIP_ZERO) && !touched))
-    SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: unknown flags %d, or SPLX_PB_SKIP_ZERO without touched", flags);
+  if (flags & ~SPLX_PB_CLEAR_G2D) SPLX_FAIL(ctx, SPLX_ERR_INVALID_ARG, "splx_project_backward_list: unknown flags %d", flags);
   PlanDev pd;
   int rc;
   if ((rc = make_plan_dev(ctx, "splx_project_backward_list", K, plan, &pd))) return rc;

@@ -201,6 +201,8 @@ int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX
                      const uint64_t** count);
 size_t bin_sort_ws_bytes(int64_t n, uint64_t capacity, int K, int TX, int TY);
 int launch_slot_map(splx_ctx*, const PlanDev&, uint32_t* slot_map_out);
+int launch_gradient_rows(splx_ctx*, void* ws, int64_t n, uint64_t capacity, int K, int TX, int TY, const float* g2d,
+                         const uint32_t** rows, const uint64_t** num_rows);
 int launch_bin_sort(splx_ctx*, const splx_projected*, int64_t n, const PlanDev&, const int64_t* part_offsets,
                     const splx_binning*, void* ws, size_t ws_bytes, const CrossDev* cross = nullptr);
 int launch_cross_sets(splx_ctx*, const splx_gaussians*, int K, const int64_t* part_offsets, const float* cell_lo,

@@ -198,10 +198,11 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
     const uint64_t* nvis = nullptr;
     if (ts->touched || gi > 0) {
       if ((r = splx_bin_sort_visible(fs.ws, n, fs.bins.capacity, K, &plan->cams[0], &vlist, &nvis))) SPLX_FAIL(ctx, r, "splx_iteration: visible list");
-      const bool skip_zero = ts->touched && !(opts->flags & SPLX_ITER_KEEP_ZERO_ROWS) && !(adam && adam->sparse);
+      // flag-tracked rows: only the Gaussians that received a 2-D gradient (the others have a zero gradient and stay unflagged)
+      if (ts->touched && !(opts->flags & SPLX_ITER_KEEP_ZERO_ROWS) && !(adam && adam->sparse) &&
+          (r = splx_bin_sort_gradient_rows(ctx, fs.ws, n, fs.bins.capacity, K, &plan->cams[0], ts->g2d, &vlist, &nvis))) return r;
       return splx_project_backward_list_plan(ctx, &g, K, ts->part_offsets, plan, ts->sh_degree, &fs.proj, ts->g2d,
-                                             SPLX_PB_CLEAR_G2D | (skip_zero ? SPLX_PB_SKIP_ZERO : 0), &ts->grads, vlist, nvis,
-                                             ts->touched);
+                                             SPLX_PB_CLEAR_G2D, &ts->grads, vlist, nvis, ts->touched);
     }
     return splx_project_backward_plan(ctx, &g, K, ts->part_offsets, plan, ts->sh_degree, &fs.proj, ts->g2d,
                                       SPLX_PB_CLEAR_G2D | SPLX_PB_OVERWRITE, &ts->grads);

@@ -499,14 +499,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
     op = pr.conic_opacity[4 * i + 3];
     cl = pr.clamp[i];
   }
-  // SPLX_PB_SKIP_ZERO (flag-tracked rows only): a visible Gaussian that no pixel blended has an all-zero 2-D gradient
-  // row, hence -- every term of this kernel is linear in that row -- a zero gradient: it is left out like a culled
-  // one (no flag, nothing read beyond the 48 bytes tested here, nothing written); an unflagged row COUNTS as zero
-  bool nz = true;
-  if (LIST == 2 && (clear_g2d & 2))
-    nz = g0.x != 0.f || g0.y != 0.f || g0.z != 0.f || g0.w != 0.f || g1.x != 0.f || g1.y != 0.f || g1.z != 0.f || g1.w != 0.f ||
-         g2.x != 0.f;
-  const bool vis = inr && rad > 0 && nz;
+  const bool vis = inr && rad > 0;
   s_vis[threadIdx.x] = vis ? 1 : 0;
   // sparse-optimiser mode: a row whose flag is still clear has no gradient yet in this iteration: its old content is
   // garbage, this launch stores instead of accumulating and sets the flag (a list holds a Gaussian once: no race)
@@ -535,7 +528,7 @@ k_project_bwd(splx_gaussians g, const __grid_constant__ PlanDev plan, const __gr
   float grgb[3] = {0.f, 0.f, 0.f};
   Geo G;
   if (vis && geometry(gin, cam, cfg.dilation, G)) {
-    if (clear_g2d & 1) { const float4 zz = make_float4(0.f, 0.f, 0.f, 0.f); gp[0] = zz; gp[1] = zz; gp[2] = zz; }
+    if (clear_g2d) { const float4 zz = make_float4(0.f, 0.f, 0.f, 0.f); gp[0] = zz; gp[1] = zz; gp[2] = zz; }
     const float gu = g0.x, gv = g0.y, gA = g0.z, gB = g0.w, gC = g1.x, gop = g1.y;
     grgb[0] = g1.z; grgb[1] = g1.w; grgb[2] = g2.x;
 #pragma unroll
@@ -803,7 +796,7 @@ int launch_project_colour_list(splx_ctx* ctx, const splx_gaussians* g, const Pla
 int launch_project_bwd(splx_ctx* ctx, const splx_gaussians* g, const PlanDev& plan, const int64_t* part_offsets, int deg,
                        const splx_projected* pr, float* g2d, int flags, const splx_gaussian_grads* grads,
                        const uint32_t* vlist, const uint64_t* nvis, uint8_t* touched) {
-  const int clr = ((flags & SPLX_PB_CLEAR_G2D) ? 1 : 0) | ((flags & SPLX_PB_SKIP_ZERO) ? 2 : 0);
+  const int clr = (flags & SPLX_PB_CLEAR_G2D) ? 1 : 0;
   const bool overwrite = (flags & SPLX_PB_OVERWRITE) != 0;
   const bool list = vlist && nvis && !overwrite;      // += over the visible Gaussians only
   // "=" must also clear the rows of partitions that do not participate in this launch

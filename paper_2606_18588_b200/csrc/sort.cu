@@ -36,6 +36,7 @@ constexpr uint32_t PERSISTENT_CTAS = SPLX_SM_COUNT * 8;   // grid of the persist
 
 struct Counters {   // device-resident counts, written by kernels, read by later kernels
   uint64_t n_visible;
+  uint64_t n_rows;      // entries of the list of Gaussians with a non-zero 2-D gradient (k_gradient_rows)
   uint64_t m_total;     // true number of intersections
   uint64_t m_sorted;    // min(m_total, capacity)
   uint32_t ticket[16];  // dynamic tile counters, one per single-pass kernel of the pipeline
@@ -980,6 +981,51 @@ int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX
   const char* base = (const char*)ws;
   *list = (const uint32_t*)(base + L.vis_list);       // index order: consecutive rows of the list are close in memory
   *count = &((const Counters*)(base + L.counters))->n_visible;
+  return SPLX_OK;
+}
+
+// The Gaussians of the visible list that received a 2-D gradient: a visible Gaussian that no pixel blended (hidden
+// behind opaque surfaces: about half of the visible ones on a city view) has an all-zero g2d row and therefore -- the
+// projection backward is linear in that row -- a zero gradient.  Compacted here (a vote and one atomic per warp; the
+// order inside the list does not matter to its consumer) so that the projection backward runs on full blocks of rows
+// that have work: skipping them INSIDE that kernel left its blocks as slow as before (the block's time is the
+// latency of its phases, not the number of live rows: 4.53 -> 4.40 ms at city_100M).
+__global__ void __launch_bounds__(256)
+k_gradient_rows(const float* __restrict__ g2d, const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr,
+                uint32_t* __restrict__ rows, unsigned long long* __restrict__ n_rows) {
+  const uint64_t nvis = *nvis_ptr;
+  const int lane = threadIdx.x & 31;
+  for (uint64_t j0 = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); j0 < nvis; j0 += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t j = j0 + lane;
+    uint32_t i = 0;
+    bool nz = false;
+    if (j < nvis) {
+      i = vlist[j];
+      const float4* gp = reinterpret_cast<const float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
+      const float4 a = gp[0], b = gp[1], c = gp[2];
+      nz = a.x != 0.f || a.y != 0.f || a.z != 0.f || a.w != 0.f || b.x != 0.f || b.y != 0.f || b.z != 0.f || b.w != 0.f ||
+           c.x != 0.f;
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, nz);
+    unsigned long long base = 0;
+    if (lane == 0 && bal) base = atomicAdd(n_rows, (unsigned long long)__popc(bal));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (nz) rows[base + __popc(bal & ((1u << lane) - 1u))] = i;
+  }
+}
+
+int launch_gradient_rows(splx_ctx* ctx, void* ws, int64_t n, uint64_t capacity, int K, int TX, int TY, const float* g2d,
+                         const uint32_t** rows, const uint64_t** num_rows) {
+  const Layout L = make_layout(n, capacity, slot_bits(K, TX, TY));
+  char* base = (char*)ws;
+  Counters* cnt = (Counters*)(base + L.counters);
+  uint32_t* out = (uint32_t*)(base + L.cvals_b);      // scratch of the depth sort, free once the binning is built
+  SPLX_CUDA_OK(ctx, cudaMemsetAsync(&cnt->n_rows, 0, sizeof(uint64_t), ctx->stream));
+  k_gradient_rows<<<SPLX_SM_COUNT * 8, 256, 0, ctx->stream>>>(g2d, (const uint32_t*)(base + L.vis_list), &cnt->n_visible, out,
+                                                             (unsigned long long*)&cnt->n_rows);
+  SPLX_LAUNCH_CHECK(ctx, "k_gradient_rows");
+  *rows = out;
+  *num_rows = &cnt->n_rows;
   return SPLX_OK;
 }
 
