@@ -493,7 +493,7 @@ def run_ours(args):
             if gi == 0 and not flags:
                 c.project_backward_plan(tr.params, po, plan, tr.sh_degree, tr.proj, g2d, tr.grads, clear_g2d=True, overwrite=True)
             else:
-                if flags and not tr.sparse_adam and not tr.keep_zero_rows:     # only the Gaussians that received a 2-D gradient
+                if not (flags and (tr.sparse_adam or tr.keep_zero_rows)):     # only the Gaussians that received a 2-D gradient
                     lst, cnt = c.bin_sort_gradient_rows(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0], g2d)
                 else:
                     lst, cnt = c.bin_sort_visible(tr._ws_sort, tr.n, tr.capacity, K, plan.cams[0])

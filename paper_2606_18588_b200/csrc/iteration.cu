@@ -198,8 +198,10 @@ int splx_iteration(splx_ctx* ctx, const splx_trainset* ts, int n_buckets, const 
     const uint64_t* nvis = nullptr;
     if (ts->touched || gi > 0) {
       if ((r = splx_bin_sort_visible(fs.ws, n, fs.bins.capacity, K, &plan->cams[0], &vlist, &nvis))) SPLX_FAIL(ctx, r, "splx_iteration: visible list");
-      // flag-tracked rows: only the Gaussians that received a 2-D gradient (the others have a zero gradient and stay unflagged)
-      if (ts->touched && !(opts->flags & SPLX_ITER_KEEP_ZERO_ROWS) && !(adam && adam->sparse) &&
+      // only the Gaussians that received a 2-D gradient: the others have a zero gradient -- with flags they stay unflagged
+      // (an unflagged row counts as zero), without flags this is an accumulating launch and adding zero changes nothing
+      const bool keep_all = ts->touched && ((opts->flags & SPLX_ITER_KEEP_ZERO_ROWS) || (adam && adam->sparse));
+      if (!keep_all &&
           (r = splx_bin_sort_gradient_rows(ctx, fs.ws, n, fs.bins.capacity, K, &plan->cams[0], ts->g2d, &vlist, &nvis))) return r;
       return splx_project_backward_list_plan(ctx, &g, K, ts->part_offsets, plan, ts->sh_degree, &fs.proj, ts->g2d,
                                              SPLX_PB_CLEAR_G2D, &ts->grads, vlist, nvis, ts->touched);
