@@ -384,7 +384,7 @@ def run_ours(args):
     sc.params = None                                   # a device-generated scene: release the generator's copy
     torch.cuda.empty_cache()
     tr.sparse_adam = bool(args.sparse_adam)
-    tr.flagged_grads = not args.plain_grads
+    tr.flagged_grads = "always" if args.always_flags else (not args.plain_grads)
     tr.lambda_dssim = float(args.lambda_dssim)
     if args.no_visibility:   # boxes that contain everything: every partition participates in every view, no tile is invisible
         big = np.float32(1e6)
@@ -704,6 +704,7 @@ def main():
     ap.add_argument("--cross-filter", action="store_true", help="cross-boundary per-ray filtering (PAPER.md L474-L476, DESIGN.md s32)")
     ap.add_argument("--plain-grads", action="store_true",
                     help="do not track the gradient rows with flags: the first bucket writes every row, Adam reads every row")
+    ap.add_argument("--always-flags", action="store_true", help="flag-tracked gradient rows whatever the first bucket covers")
     ap.add_argument("--sparse-adam", action="store_true", help="visible-only Adam (an option outside the paper, DESIGN.md s31)")
     args = ap.parse_args()
     if args.impl == "reference":

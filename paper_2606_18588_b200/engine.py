@@ -83,9 +83,10 @@ class Trainer:
         self.flagged_grads = True
         #: multi-bucket iterations: project + sort of the next bucket on a second stream while this one is blended
         self.pipeline_buckets = True
-        #: flag-tracked gradient rows: a visible Gaussian that no pixel blended has a zero gradient and is left out of the
-        #: projection backward like a culled one (SPLX_PB_SKIP_ZERO; same result, an unflagged row counts as zero).  True keeps
-        #: them (every visible Gaussian gets its flag); the visible-only optimiser option always keeps them
+        #: a visible Gaussian that no pixel blended has a zero gradient: the projection backward of splx_iteration runs over the
+        #: Gaussians that received a 2-D gradient only (splx_bin_sort_gradient_rows; same result: an unflagged row counts as
+        #: zero, adding zero changes nothing).  True keeps every visible row (SPLX_ITER_KEEP_ZERO_ROWS); the visible-only
+        #: optimiser option always keeps them
         self.keep_zero_rows = False
         #: a1 inside splx_iteration: None = fused (one kernel) when every partition takes part in every bucket -- then most
         #: Gaussians are visible (aerial views) --, else geometry -> binning -> colour of the visible list (city views, where
@@ -480,6 +481,8 @@ class Trainer:
             return True
         if not self.flagged_grads:
             return False
+        if self.flagged_grads == "always":
+            return True
         held = sum(self.part_offsets[k + 1] - self.part_offsets[k] for k, v in enumerate(first_plan.view_of_part) if v >= 0)
         return held < 0.75 * self.n
 
