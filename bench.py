@@ -503,7 +503,11 @@ def run_ours(args):
         tr.adam_step(B, flagged=flags)
         ev[-1][7].record()
 
-    flags = tr._use_flags(plans[0][0])
+    if not single_graph:      # the first iteration over a set of views measures the fraction of Gaussians that receive a gradient
+        tr.iteration_views(ids, cams, targets, **kw)
+        torch.cuda.synchronize()
+        restore()
+    flags = tr.flags_decision(ids, plans[0][0]) if not single_graph else tr._use_flags(plans[0][0])
     fused_proj = tr.use_fused_projection([p for p, _ in plans])
     tr._trainset(B, False, flags)     # allocates the D-SSIM workspace / the touched flags
     n_staged = max(3, min(args.steps, 10))
@@ -603,7 +607,7 @@ def run_ours(args):
         project_backward=(236 * tr.n + 272 * vis0 + 740 * (nv - vis0)) if first_overwrite else
                          (56 * nv + 740 * counts["rows_with_gradient"] if counts.get("rows_with_gradient") else 740 * nv),
         # flagged gradient rows: 24 B per parameter (param, m, v read + written) + the gradient of the touched rows only
-        adam=(24 * 59 * tr.n + tr.n + 4 * 59 * min(nv, tr.n)) if flags else 28 * 59 * tr.n)
+        adam=(24 * 59 * tr.n + tr.n + 4 * 59 * min(counts.get("rows_with_gradient") or nv, tr.n)) if flags else 28 * 59 * tr.n)
     flops_fwd = counts["pairs_walked_fwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_FWD
     flops_bwd = counts["pairs_walked_bwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_BWD
     flops_fwd_exec = counts["pairs_evaluated_fwd"] * FLOPS_EVAL + counts["pairs_blended"] * FLOPS_BLEND_FWD
