@@ -993,24 +993,38 @@ int bin_sort_visible(const void* ws, int64_t n, uint64_t capacity, int K, int TX
 __global__ void __launch_bounds__(256)
 k_gradient_rows(const float* __restrict__ g2d, const uint32_t* __restrict__ vlist, const uint64_t* __restrict__ nvis_ptr,
                 uint32_t* __restrict__ rows, unsigned long long* __restrict__ n_rows) {
+  constexpr int U = 4;      // list entries per thread and trip: their dependent loads (entry -> row) overlap
   const uint64_t nvis = *nvis_ptr;
   const int lane = threadIdx.x & 31;
-  for (uint64_t j0 = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); j0 < nvis; j0 += (uint64_t)gridDim.x * blockDim.x) {
-    const uint64_t j = j0 + lane;
-    uint32_t i = 0;
-    bool nz = false;
-    if (j < nvis) {
-      i = vlist[j];
-      const float4* gp = reinterpret_cast<const float4*>(g2d + (int64_t)SPLX_G2D_STRIDE * i);
-      const float4 a = gp[0], b = gp[1], c = gp[2];
-      nz = a.x != 0.f || a.y != 0.f || a.z != 0.f || a.w != 0.f || b.x != 0.f || b.y != 0.f || b.z != 0.f || b.w != 0.f ||
-           c.x != 0.f;
+  const uint64_t warp0 = ((uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)) * U;
+  for (uint64_t j0 = warp0; j0 < nvis; j0 += (uint64_t)gridDim.x * blockDim.x * U) {
+    uint32_t i[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { const uint64_t j = j0 + 32 * u + lane; i[u] = j < nvis ? vlist[j] : 0xffffffffu; }
+    bool nz[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      nz[u] = false;
+      if (i[u] != 0xffffffffu) {
+        const float* gp = g2d + (int64_t)SPLX_G2D_STRIDE * i[u];
+        const float4 a = *reinterpret_cast<const float4*>(gp), b = *reinterpret_cast<const float4*>(gp + 4);
+        const float c = gp[8];
+        nz[u] = a.x != 0.f || a.y != 0.f || a.z != 0.f || a.w != 0.f || b.x != 0.f || b.y != 0.f || b.z != 0.f || b.w != 0.f ||
+                c != 0.f;
+      }
     }
-    const unsigned bal = __ballot_sync(0xffffffffu, nz);
+    unsigned bal[U];
+    int total = 0;
+#pragma unroll
+    for (int u = 0; u < U; ++u) { bal[u] = __ballot_sync(0xffffffffu, nz[u]); total += __popc(bal[u]); }
     unsigned long long base = 0;
-    if (lane == 0 && bal) base = atomicAdd(n_rows, (unsigned long long)__popc(bal));
+    if (lane == 0 && total) base = atomicAdd(n_rows, (unsigned long long)total);
     base = __shfl_sync(0xffffffffu, base, 0);
-    if (nz) rows[base + __popc(bal & ((1u << lane) - 1u))] = i;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (nz[u]) rows[base + __popc(bal[u] & ((1u << lane) - 1u))] = i[u];
+      base += __popc(bal[u]);
+    }
   }
 }
 
