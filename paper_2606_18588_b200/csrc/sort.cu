@@ -197,6 +197,12 @@ struct VisibleOp {  // step 1: compaction of the visible Gaussians, index order 
   __device__ void load_all(uint64_t base, uint64_t cnt, uint32_t (&v)[SCAN_IPT]) const {
     uint64_t gi0 = 0; uint32_t rem = 0;
     if (base < cnt) span(base, gi0, rem);
+    static_assert(SCAN_IPT == 8, "two 16-byte loads per thread");
+    if (rem == SCAN_IPT && base + SCAN_IPT <= cnt && (gi0 & 3) == 0) {     // the common case: eight consecutive, aligned counts
+      const uint4 a = *reinterpret_cast<const uint4*>(tiles_touched + gi0), b = *reinterpret_cast<const uint4*>(tiles_touched + gi0 + 4);
+      v[0] = a.x > 0; v[1] = a.y > 0; v[2] = a.z > 0; v[3] = a.w > 0; v[4] = b.x > 0; v[5] = b.y > 0; v[6] = b.z > 0; v[7] = b.w > 0;
+      return;
+    }
 #pragma unroll
     for (int k = 0; k < SCAN_IPT; ++k) {
       v[k] = 0;
